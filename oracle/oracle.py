@@ -1,0 +1,189 @@
+"""ctypes front end of the CPU fp64 oracle (submatrix_oracle.c).
+
+TEST INFRASTRUCTURE ONLY: only tests/, __graft_entry__.smoke() and bench.py's
+cpu_baseline / --impl reference legs may import this.  It imports nothing from
+the CUDA package; inputs come from workloads/generator.py.
+
+Every function takes the block-CSR arrays of a `Workload`-like object (fields
+n_blk, blk_size, row_ptr, col_idx, val_ptr, vals) and follows PAPER.md:110
+(Fig. 2, the three steps), :87 (Eq. 13) and :91 (Eq. 14 with S = I); see the
+header of submatrix_oracle.c for the passage behind each C function.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+from types import SimpleNamespace
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SO = os.path.join(_HERE, "liborc.so")
+_SRC = os.path.join(_HERE, "submatrix_oracle.c")
+
+
+def build(force: bool = False) -> str:
+    """Compile submatrix_oracle.c with gcc (building the checker is not using it)."""
+    if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < os.path.getmtime(_SRC):
+        subprocess.check_call(["gcc", "-O2", "-fPIC", "-shared", "-pthread", "-o", _SO, _SRC, "-lm"])
+    return _SO
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(build())
+        _lib.orc_gershgorin.restype = C.c_double
+        _lib.orc_trace.restype = C.c_double
+    return _lib
+
+
+def _p(a, t):
+    return a.ctypes.data_as(C.POINTER(t)) if a is not None else None
+
+
+def _i32(a):
+    return np.ascontiguousarray(a, dtype=np.int32)
+
+
+def _csr(w):
+    return (C.c_int32(w.n_blk), _p(_i32(w.blk_size), C.c_int32), _p(_i32(w.row_ptr), C.c_int32),
+            _p(_i32(w.col_idx), C.c_int32))
+
+
+def check_pattern(w) -> int:
+    return lib().orc_check_pattern(C.c_int32(w.n_blk), _p(_i32(w.row_ptr), C.c_int32),
+                                   _p(_i32(w.col_idx), C.c_int32))
+
+
+def pattern_sizes(w, pad_to: int):
+    out = np.zeros(5, dtype=np.int64)
+    rc = lib().orc_pattern_sizes(*_csr(w), C.c_int32(pad_to), _p(out, C.c_int64))
+    if rc:
+        raise ValueError(f"orc_pattern_sizes: {rc}")
+    return SimpleNamespace(nbr_len=int(out[0]), gmap_len=int(out[1]), packed_elems=int(out[2]),
+                           max_dim=int(out[3]), max_dim_pad=int(out[4]))
+
+
+def build_pattern(w, pad_to: int):
+    """Integer pattern arrays of PAPER.md:110 step 1 (see include/submatrix.h for names)."""
+    sz = pattern_sizes(w, pad_to)
+    n = w.n_blk
+    P = SimpleNamespace(
+        nbr_ptr=np.zeros(n + 1, np.int32), nbr_idx=np.zeros(sz.nbr_len, np.int32),
+        own_pos=np.zeros(n, np.int32), dim=np.zeros(n, np.int32), dim_pad=np.zeros(n, np.int32),
+        row_off=np.zeros(sz.nbr_len, np.int32), sub_off=np.zeros(n + 1, np.int64),
+        gmap_ptr=np.zeros(n + 1, np.int64), gmap=np.zeros(sz.gmap_len, np.int32),
+        tmap=np.zeros(w.nnzb, np.int32), order=np.zeros(n, np.int32), sizes=sz)
+    rc = lib().orc_build_pattern(
+        *_csr(w), C.c_int32(pad_to), _p(P.nbr_ptr, C.c_int32), _p(P.nbr_idx, C.c_int32),
+        _p(P.own_pos, C.c_int32), _p(P.dim, C.c_int32), _p(P.dim_pad, C.c_int32),
+        _p(P.row_off, C.c_int32), _p(P.sub_off, C.c_int64), _p(P.gmap_ptr, C.c_int64),
+        _p(P.gmap, C.c_int32), _p(P.tmap, C.c_int32), _p(P.order, C.c_int32))
+    if rc:
+        raise ValueError(f"orc_build_pattern: status {rc}")
+    return P
+
+
+def gather(w, i: int, mu: float = 0.0) -> np.ndarray:
+    """T_i(H) - mu*I as a dense m x m fp64 array."""
+    nb = w.col_idx[w.row_ptr[i]:w.row_ptr[i + 1]]
+    m = int(np.asarray(w.blk_size)[nb].sum())
+    T = np.zeros((m, m))
+    vp = np.ascontiguousarray(w.val_ptr, dtype=np.int64)
+    vals = np.ascontiguousarray(w.vals, dtype=np.float64)
+    lib().orc_gather(*_csr(w), _p(vp, C.c_int64), _p(vals, C.c_double), C.c_int32(i),
+                     C.c_double(mu), _p(T, C.c_double))
+    return T
+
+
+def gershgorin(T: np.ndarray) -> float:
+    T = np.ascontiguousarray(T, dtype=np.float64)
+    return float(lib().orc_gershgorin(C.c_int32(T.shape[0]), _p(T, C.c_double)))
+
+
+def jacobi_eigh(T: np.ndarray, max_sweeps: int = 30, rel_tol: float = 1e-15):
+    """(w, V, sweeps): T = V diag(w) V^T, columns of V are eigenvectors (own cyclic Jacobi)."""
+    A = np.array(T, dtype=np.float64, order="C", copy=True)
+    m = A.shape[0]
+    Vt = np.zeros((m, m))
+    w = np.zeros(m)
+    sw = lib().orc_jacobi(C.c_int32(m), _p(A, C.c_double), _p(Vt, C.c_double), _p(w, C.c_double),
+                          C.c_int32(max_sweeps), C.c_double(rel_tol))
+    return w, Vt.T.copy(), int(sw)
+
+
+def sign(T: np.ndarray) -> np.ndarray:
+    """sign(T) for symmetric T by Eq. 13's definition on the spectrum."""
+    w, V, _ = jacobi_eigh(T)
+    m = T.shape[0]
+    S = np.zeros((m, m))
+    Vt = np.ascontiguousarray(V.T)
+    lib().orc_sign_from_eig(C.c_int32(m), _p(Vt, C.c_double), _p(w, C.c_double), _p(S, C.c_double))
+    return S
+
+
+def ns_polynomial(T: np.ndarray, scale: float, k: int) -> np.ndarray:
+    """Exact-arithmetic result of k Newton-Schulz steps from T/scale (reading A13)."""
+    w, V, _ = jacobi_eigh(T)
+    m = T.shape[0]
+    S = np.zeros((m, m))
+    Vt = np.ascontiguousarray(V.T)
+    lib().orc_nsk_from_eig(C.c_int32(m), _p(Vt, C.c_double), _p(w, C.c_double), C.c_double(scale),
+                           C.c_int32(k), _p(S, C.c_double))
+    return S
+
+
+def density_columns(w, mu: float = 0.0, cols=None, mode: str = "exact", k_fixed: int = 0,
+                    scale=None, n_threads: int = 1):
+    """Raw D = 1/2 (I - sign(T_i - mu I)) blocks of the listed block columns (all if None).
+
+    Returns (d_vals in H's block-CSR layout with only the listed columns' blocks
+    written, stats).  mode "nsk": the NS-k polynomial at scale (Gershgorin if None).
+    """
+    vp = np.ascontiguousarray(w.val_ptr, dtype=np.int64)
+    vals = np.ascontiguousarray(w.vals, dtype=np.float64)
+    d = np.zeros_like(vals)
+    cols_a = None if cols is None else _i32(cols)
+    nc = w.n_blk if cols is None else int(cols_a.shape[0])
+    st = SimpleNamespace(min_abs_eig=np.zeros(nc), scale=np.zeros(nc), sweeps=np.zeros(nc, np.int32),
+                         n_neg=np.zeros(nc, np.int32))
+    sc = None if scale is None else np.ascontiguousarray(scale, dtype=np.float64)
+    rc = lib().orc_density_columns(
+        *_csr(w), _p(vp, C.c_int64), _p(vals, C.c_double), C.c_double(mu), C.c_int32(nc),
+        _p(cols_a, C.c_int32), C.c_int32(0 if mode == "exact" else 1), C.c_int32(k_fixed),
+        _p(sc, C.c_double), _p(d, C.c_double), _p(st.min_abs_eig, C.c_double),
+        _p(st.scale, C.c_double), _p(st.sweeps, C.c_int32), _p(st.n_neg, C.c_int32),
+        C.c_int32(n_threads))
+    if rc:
+        raise ValueError(f"orc_density_columns: status {rc}")
+    return d, st
+
+
+def symmetrise(w, d_raw: np.ndarray) -> np.ndarray:
+    vp = np.ascontiguousarray(w.val_ptr, dtype=np.int64)
+    d_raw = np.ascontiguousarray(d_raw, dtype=np.float64)
+    out = np.zeros_like(d_raw)
+    rc = lib().orc_symmetrise(*_csr(w), _p(vp, C.c_int64), _p(d_raw, C.c_double), _p(out, C.c_double))
+    if rc:
+        raise ValueError(f"orc_symmetrise: status {rc}")
+    return out
+
+
+def trace(w, d_vals: np.ndarray) -> float:
+    vp = np.ascontiguousarray(w.val_ptr, dtype=np.int64)
+    d_vals = np.ascontiguousarray(d_vals, dtype=np.float64)
+    return float(lib().orc_trace(*_csr(w), _p(vp, C.c_int64), _p(d_vals, C.c_double)))
+
+
+def column_mask(w, cols) -> np.ndarray:
+    """Boolean mask over d_vals elements that belong to blocks in the listed block columns."""
+    sel = np.zeros(w.n_blk, dtype=bool)
+    sel[np.asarray(cols)] = True
+    blk_sel = sel[np.asarray(w.col_idx)]
+    sizes = np.diff(np.asarray(w.val_ptr))
+    return np.repeat(blk_sel, sizes)

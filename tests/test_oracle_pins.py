@@ -1,0 +1,369 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix.
+
+PAPER.md prints no worked numerical example for this path, so the pins are closed
+forms, invariants of Eq. 13 / Eq. 14, limits in which the
+submatrix method is exact, library routines (LAPACK eigh, scipy
+signm, LDL^T inertia) and brute force on tiny inputs.
+"""
+import numpy as np
+import pytest
+import scipy.linalg
+
+from oracle import oracle as orc
+from workloads.generator import Workload, make_config, make_workload
+
+
+def _rand_sym(m, seed):
+    rng = np.random.default_rng(seed)
+    a = rng.standard_normal((m, m))
+    return 0.5 * (a + a.T)
+
+
+# ------------------------------------------------------------------ Jacobi
+
+def test_jacobi_diagonal_is_fixed_point():
+    d = np.array([3.0, -1.5, 0.25, -7.0])
+    w, V, sweeps = orc.jacobi_eigh(np.diag(d))
+    assert sweeps == 0
+    assert np.array_equal(w, d)
+    assert np.array_equal(V, np.eye(4))
+
+
+def test_jacobi_tridiagonal_toeplitz_closed_form():
+    # eigenvalues of tridiag(1, 0, 1) are 2 cos(k pi / (m+1)), k = 1..m
+    m = 37
+    T = np.diag(np.ones(m - 1), 1) + np.diag(np.ones(m - 1), -1)
+    w, V, _ = orc.jacobi_eigh(T)
+    expect = 2.0 * np.cos(np.arange(1, m + 1) * np.pi / (m + 1))
+    assert np.allclose(np.sort(w), np.sort(expect), atol=1e-13)
+
+
+@pytest.mark.parametrize("m,seed", [(1, 0), (2, 1), (17, 2), (64, 3), (131, 4)])
+def test_jacobi_reconstruction_orthogonality_and_lapack(m, seed):
+    T = _rand_sym(m, seed)
+    w, V, _ = orc.jacobi_eigh(T)
+    fro = np.linalg.norm(T)
+    assert np.linalg.norm((V * w) @ V.T - T) <= 1e-13 * max(fro, 1.0)
+    assert np.linalg.norm(V.T @ V - np.eye(m)) <= 1e-13 * np.sqrt(m)
+    assert np.allclose(np.sort(w), np.linalg.eigvalsh(T), atol=1e-12 * max(fro, 1.0))
+
+
+# -------------------------------------------------------------------- sign
+
+def test_sign_2x2_closed_form():
+    # T = [[a, b], [b, -a]]: T^2 = (a^2+b^2) I, so Eq. 13 gives sign(T) = T / sqrt(a^2+b^2)
+    a, b = 0.7, -1.9
+    T = np.array([[a, b], [b, -a]])
+    assert np.allclose(orc.sign(T), T / np.hypot(a, b), atol=1e-15)
+
+
+def test_sign_definite_matrices():
+    T = _rand_sym(9, 5)
+    P = T @ T + np.eye(9)
+    assert np.allclose(orc.sign(P), np.eye(9), atol=1e-13)
+    assert np.allclose(orc.sign(-P), -np.eye(9), atol=1e-13)
+
+
+@pytest.mark.parametrize("m,seed", [(6, 10), (40, 11), (97, 12)])
+def test_sign_invariants_eq13(m, seed):
+    T = _rand_sym(m, seed)
+    S = orc.sign(T)
+    eye = np.eye(m)
+    assert np.abs(S @ S - eye).max() < 1e-12            # sign^2 = A^2 (A^2)^-1 = I
+    assert np.abs(S - S.T).max() < 1e-13
+    assert np.abs(S @ T - T @ S).max() < 1e-12 * np.linalg.norm(T)
+    # S T = (T^2)^(1/2): symmetric positive definite with eigenvalues |lambda|
+    ST = S @ T
+    assert np.abs(ST - ST.T).max() < 1e-12 * np.linalg.norm(T)
+    assert np.allclose(np.linalg.eigvalsh(0.5 * (ST + ST.T)), np.sort(np.abs(np.linalg.eigvalsh(T))),
+                       atol=1e-11)
+    # Eq. 13 literally, with the inverse square root from scipy
+    ref = T @ np.linalg.inv(scipy.linalg.sqrtm(T @ T).real)
+    assert np.abs(S - ref).max() < 1e-9
+    assert np.abs(orc.sign(3.7 * T) - S).max() < 1e-12   # sign(cT) = sign(T), c > 0
+    assert np.abs(orc.sign(-T) + S).max() < 1e-12        # sign(-T) = -sign(T)
+    perm = np.random.default_rng(seed).permutation(m)
+    Q = eye[perm]
+    assert np.abs(orc.sign(Q @ T @ Q.T) - Q @ S @ Q.T).max() < 1e-12
+
+
+def test_sign_matches_scipy_signm_and_lapack():
+    T = _rand_sym(30, 21)
+    S = orc.sign(T)
+    lam, V = np.linalg.eigh(T)
+    assert np.abs(S - (V * np.sign(lam)) @ V.T).max() < 1e-12
+    assert np.abs(S - scipy.linalg.signm(T)).max() < 1e-8
+
+
+def test_sign_of_zero_eigenvalue_is_zero():
+    # reading A14: sgn(0) := 0, the Newton-Schulz fixed point
+    T = np.diag([2.0, 0.0, -3.0])
+    assert np.array_equal(orc.sign(T), np.diag([1.0, 0.0, -1.0]))
+
+
+# ------------------------------------------------------------ NS-k polynomial
+
+@pytest.mark.parametrize("k", [0, 1, 5, 12])
+def test_ns_polynomial_equals_matrix_iteration(k):
+    # the spectral form must equal k explicit steps X <- 1/2 X (3I - X^2) in fp64
+    T = _rand_sym(24, 33)
+    s = orc.gershgorin(T)
+    X = T / s
+    eye = np.eye(24)
+    for _ in range(k):
+        X = 0.5 * X @ (3.0 * eye - X @ X)
+    assert np.abs(orc.ns_polynomial(T, s, k) - X).max() < 1e-12
+
+
+def test_ns_polynomial_scalar_recursion_and_limit():
+    d = np.array([0.9, -0.4, 0.05, -1.0])
+    out = orc.ns_polynomial(np.diag(d), 1.0, 3)
+    x = d.copy()
+    for _ in range(3):
+        x = 0.5 * x * (3.0 - x * x)
+    assert np.allclose(np.diag(out), x, atol=1e-15)
+    T = _rand_sym(16, 34)
+    assert np.abs(orc.ns_polynomial(T, orc.gershgorin(T), 60) - orc.sign(T)).max() < 1e-10
+
+
+def test_gershgorin_bounds_spectral_radius():
+    T = _rand_sym(50, 40)
+    s = orc.gershgorin(T)
+    assert s == pytest.approx(np.abs(T).sum(axis=1).max(), rel=1e-15)
+    assert s >= np.abs(np.linalg.eigvalsh(T)).max()
+
+
+# -------------------------------------------------- submatrix method: worked example
+
+def _sign2(t):
+    lam = np.linalg.eigvalsh(t)
+    if lam[0] > 0:
+        return np.eye(2)
+    if lam[1] < 0:
+        return -np.eye(2)
+    # one eigenvalue of each sign: sign(T) = (2T - tr(T) I) / (lambda_+ - lambda_-)
+    gap = np.sqrt((t[0, 0] - t[1, 1]) ** 2 + 4 * t[0, 1] ** 2)
+    return (2 * t - np.trace(t) * np.eye(2)) / gap
+
+
+def test_submatrix_method_on_a_three_site_chain_by_hand():
+    # Fig. 2 by hand: a chain 0-1-2 with scalar blocks.  Column 0 sees {0,1},
+    # column 1 sees {0,1,2} (the whole matrix), column 2 sees {1,2}.
+    h = np.array([[-0.8, 0.5, 0.0], [0.5, 0.3, -0.7], [0.0, -0.7, 0.9]])
+    w = Workload(n_blk=3, blk_size=np.ones(3, np.int32), row_ptr=np.array([0, 2, 5, 7], np.int32),
+                 col_idx=np.array([0, 1, 0, 1, 2, 1, 2], np.int32), val_ptr=np.arange(8, dtype=np.int64),
+                 vals=np.array([h[0, 0], h[0, 1], h[1, 0], h[1, 1], h[1, 2], h[2, 1], h[2, 2]]),
+                 box=1.0, positions=np.zeros((3, 3)))
+    d, _ = orc.density_columns(w)
+    s0 = _sign2(h[:2, :2])
+    s2 = _sign2(h[1:, 1:])
+    lam, V = np.linalg.eigh(h)
+    s1 = (V * np.sign(lam)) @ V.T
+    expect = np.array([
+        0.5 * (1 - s0[0, 0]),      # D(0,0): column 0 of sign(T_0), row 0
+        -0.5 * s1[0, 1],           # D(0,1): column 1 of sign(T_1) = sign(H), row 0
+        -0.5 * s0[1, 0],           # D(1,0)
+        0.5 * (1 - s1[1, 1]),      # D(1,1)
+        -0.5 * s2[0, 1],           # D(1,2): column 2 -> local column 1 of sign(T_2), local row 0
+        -0.5 * s1[2, 1],           # D(2,1)
+        0.5 * (1 - s2[1, 1]),      # D(2,2)
+    ])
+    assert np.allclose(d, expect, atol=1e-14)
+
+
+# ------------------------------------------------------- limits where the method is exact
+
+def _neg_inertia(a):
+    """Number of negative eigenvalues via LDL^T (Sylvester's law), independent of Jacobi."""
+    _, d, _ = scipy.linalg.ldl(a)
+    n = d.shape[0]
+    neg, i = 0, 0
+    while i < n:
+        if i + 1 < n and d[i + 1, i] != 0.0:
+            blk = d[i:i + 2, i:i + 2]
+            det = blk[0, 0] * blk[1, 1] - blk[0, 1] * blk[1, 0]
+            neg += 1 if det < 0 else (2 if blk[0, 0] + blk[1, 1] < 0 else 0)
+            i += 2
+        else:
+            neg += int(d[i, i] < 0)
+            i += 1
+    return neg
+
+
+def test_full_coverage_equals_full_matrix_sign():
+    # every N(i) = all blocks  =>  every T_i = H  =>  D = 1/2 (I - sign(H))   [north_star pin]
+    w = make_config(0, cutoff=np.inf)
+    assert w.nnzb == w.n_blk ** 2
+    d, st = orc.density_columns(w, n_threads=4)
+    D = Workload(**{**w.__dict__, "vals": d}).dense()
+    H = w.dense()
+    lam, V = np.linalg.eigh(H)
+    D_full = 0.5 * (np.eye(w.n) - (V * np.sign(lam)) @ V.T)
+    assert np.abs(D - D_full).max() < 1e-13
+    assert np.abs(D @ D - D).max() < 1e-12              # idempotent
+    assert np.abs(D - D.T).max() < 1e-13
+    n_neg = _neg_inertia(H)
+    assert n_neg == int((lam < 0).sum())
+    assert abs(orc.trace(w, d) - n_neg) < 1e-10         # Tr D = number of negative eigenvalues
+    assert (st.n_neg == n_neg).all()
+
+
+def test_block_diagonal_limit_gives_block_projectors():
+    w = make_config(0, cutoff=0.0)
+    assert w.nnzb == w.n_blk
+    d, _ = orc.density_columns(w)
+    b = int(w.blk_size[0])
+    for i in range(w.n_blk):
+        h = w.vals[w.val_ptr[i]:w.val_ptr[i + 1]].reshape(b, b)
+        lam, V = np.linalg.eigh(h)
+        proj = V[:, lam < 0] @ V[:, lam < 0].T
+        assert np.abs(d[w.val_ptr[i]:w.val_ptr[i + 1]].reshape(b, b) - proj).max() < 1e-13
+
+
+def test_each_submatrix_density_is_idempotent_but_assembled_D_is_not():
+    w = make_config(0)
+    for i in (0, 7, 31):
+        T = orc.gather(w, i)
+        Dsub = 0.5 * (np.eye(T.shape[0]) - orc.sign(T))
+        assert np.abs(Dsub @ Dsub - Dsub).max() < 1e-12
+    d, _ = orc.density_columns(w)
+    D = Workload(**{**w.__dict__, "vals": d}).dense()
+    # the method is an approximation: away from the limits D^2 != D
+    assert 1e-4 < np.abs(D @ D - D).max() < 0.5
+
+
+def test_negated_hamiltonian_gives_complement():
+    w = make_config(0)
+    d, _ = orc.density_columns(w)
+    wn = Workload(**{**w.__dict__, "vals": -w.vals})
+    dn, _ = orc.density_columns(wn)
+    ident = np.zeros_like(d)
+    b = int(w.blk_size[0])
+    for i in range(w.n_blk):
+        p = w.row_ptr[i] + int(np.searchsorted(w.col_idx[w.row_ptr[i]:w.row_ptr[i + 1]], i))
+        ident[w.val_ptr[p]:w.val_ptr[p + 1]] = np.eye(b).ravel()
+    assert np.abs(dn - (ident - d)).max() < 1e-12
+
+
+def test_locality_subset_and_thread_count_do_not_change_columns():
+    w = make_config(0)
+    d_all, _ = orc.density_columns(w, n_threads=3)
+    cols = [2, 3, 17, 30]
+    d_sub, _ = orc.density_columns(w, cols=cols)
+    mask = orc.column_mask(w, cols)
+    assert np.array_equal(d_all[mask], d_sub[mask])
+    assert not d_sub[~mask].any()
+
+
+def test_relabelling_molecules_permutes_D():
+    w = make_workload(12, 3, 1, 5.0, seed=77)
+    perm = np.random.default_rng(5).permutation(w.n_blk)     # new label of old block i
+    H = w.dense()
+    b = 3
+    idx = np.concatenate([np.arange(b) + b * int(np.where(perm == k)[0][0]) for k in range(w.n_blk)])
+    Hp = H[np.ix_(idx, idx)]
+    # rebuild the block-CSR of the relabelled matrix from its dense form
+    nzb = [(i, j) for i in range(w.n_blk) for j in range(w.n_blk)
+           if np.any(Hp[i * b:(i + 1) * b, j * b:(j + 1) * b] != 0.0)]
+    row_ptr = np.zeros(w.n_blk + 1, np.int32)
+    for i, _ in nzb:
+        row_ptr[i + 1] += 1
+    row_ptr = np.cumsum(row_ptr).astype(np.int32)
+    col_idx = np.array([j for _, j in nzb], np.int32)
+    vals = np.concatenate([Hp[i * b:(i + 1) * b, j * b:(j + 1) * b].ravel() for i, j in nzb])
+    wp = Workload(n_blk=w.n_blk, blk_size=w.blk_size.copy(), row_ptr=row_ptr, col_idx=col_idx,
+                  val_ptr=np.arange(len(nzb) + 1, dtype=np.int64) * b * b, vals=vals, box=w.box,
+                  positions=w.positions)
+    d, _ = orc.density_columns(w)
+    dp, _ = orc.density_columns(wp)
+    D = Workload(**{**w.__dict__, "vals": d}).dense()
+    Dp = Workload(**{**wp.__dict__, "vals": dp}).dense()
+    assert np.abs(Dp - D[np.ix_(idx, idx)]).max() < 1e-12
+
+
+# ------------------------------------------------------------------ pattern
+
+@pytest.mark.parametrize("cfg,pad", [(0, 1), (0, 16), (1, 64)])
+def test_pattern_against_dense_boolean_adjacency(cfg, pad):
+    w = make_config(cfg)
+    P = orc.build_pattern(w, pad)
+    n = w.n_blk
+    adj = -np.ones((n, n), dtype=np.int64)               # stored-block index or -1
+    for i in range(n):
+        for p in range(w.row_ptr[i], w.row_ptr[i + 1]):
+            adj[i, w.col_idx[p]] = p
+    assert P.nbr_ptr[-1] == w.nnzb == P.sizes.nbr_len     # sum of counts = nnzb
+    for i in range(n):
+        nb = np.nonzero(adj[:, i] >= 0)[0]                # rows with a stored block in column i
+        lo, hi = P.nbr_ptr[i], P.nbr_ptr[i + 1]
+        assert np.array_equal(P.nbr_idx[lo:hi], nb)
+        assert nb[P.own_pos[i]] == i
+        sizes = w.blk_size[nb]
+        assert P.dim[i] == sizes.sum()
+        assert P.dim_pad[i] == -(-P.dim[i] // pad) * pad
+        assert np.array_equal(P.row_off[lo:hi], np.concatenate([[0], np.cumsum(sizes)[:-1]]))
+        g = P.gmap[P.gmap_ptr[i]:P.gmap_ptr[i + 1]].reshape(len(nb), len(nb))
+        assert np.array_equal(g, adj[np.ix_(nb, nb)])
+        assert (g[:, P.own_pos[i]] >= 0).all()            # column i is fully stored
+    assert np.array_equal(P.sub_off, np.concatenate([[0], np.cumsum(P.dim_pad.astype(np.int64) ** 2)]))
+    assert np.array_equal(P.tmap[P.tmap], np.arange(w.nnzb))
+    for i in range(n):
+        for p in range(w.row_ptr[i], w.row_ptr[i + 1]):
+            assert adj[w.col_idx[p], i] == P.tmap[p]
+    key = [(-int(P.dim_pad[i]), i) for i in range(n)]
+    assert [int(x) for x in P.order] == [i for _, i in sorted(key)]
+    assert P.sizes.max_dim == P.dim.max() and P.sizes.max_dim_pad == P.dim_pad.max()
+    assert P.sizes.packed_elems == P.sub_off[-1] and P.sizes.gmap_len == P.gmap_ptr[-1]
+
+
+def test_pattern_rejects_bad_structure():
+    w = make_config(0)
+    # drop one off-diagonal block: no longer structurally symmetric
+    i = int(np.argmax(np.diff(w.row_ptr) > 1))
+    p = w.row_ptr[i] + (1 if w.col_idx[w.row_ptr[i]] == i else 0)
+    keep = np.ones(w.nnzb, bool)
+    keep[p] = False
+    row_ptr = w.row_ptr.copy()
+    row_ptr[i + 1:] -= 1
+    bad = Workload(**{**w.__dict__, "row_ptr": row_ptr, "col_idx": w.col_idx[keep]})
+    assert orc.check_pattern(bad) == -3
+    # unsorted columns
+    ci = w.col_idx.copy()
+    lo = w.row_ptr[i]
+    ci[lo], ci[lo + 1] = ci[lo + 1], ci[lo]
+    assert orc.check_pattern(Workload(**{**w.__dict__, "col_idx": ci})) == -3
+    assert orc.check_pattern(w) == 0
+
+
+def test_gather_against_dense_indexing():
+    w = make_workload(20, np.array([2, 3, 5, 4] * 5), np.array([1, 1, 2, 2] * 5), 4.5, seed=9)
+    H = w.dense()
+    off = np.concatenate([[0], np.cumsum(w.blk_size)])
+    for i in (0, 5, 19):
+        nb = w.col_idx[w.row_ptr[i]:w.row_ptr[i + 1]]
+        idx = np.concatenate([np.arange(off[j], off[j + 1]) for j in nb])
+        # dense principal submatrix: entries between members of N(i) that are not stored are zero in H too
+        assert np.array_equal(orc.gather(w, i, mu=0.25), H[np.ix_(idx, idx)] - 0.25 * np.eye(len(idx)))
+
+
+# ------------------------------------------------------------- symmetrise / trace
+
+def test_symmetrise_is_exactly_symmetric_and_trace_preserving():
+    w = make_config(0)
+    d, _ = orc.density_columns(w)
+    ds = orc.symmetrise(w, d)
+    D = Workload(**{**w.__dict__, "vals": d}).dense()
+    Ds = Workload(**{**w.__dict__, "vals": ds}).dense()
+    assert np.array_equal(Ds, Ds.T)
+    assert np.array_equal(Ds, 0.5 * (D + D.T))
+    assert orc.trace(w, ds) == orc.trace(w, d)
+    assert orc.trace(w, d) == pytest.approx(np.trace(D), abs=1e-12)
+    assert np.abs(D - D.T).max() > 1e-4     # symmetrisation is not a no-op (reading A6)
+
+
+def test_trace_is_near_but_not_equal_to_electron_count():
+    w = make_config(0)
+    d, st = orc.density_columns(w)
+    tr = orc.trace(w, d)
+    n_neg_full = int((np.linalg.eigvalsh(w.dense()) < 0).sum())
+    assert abs(tr - n_neg_full) < 0.5 and abs(tr - round(tr)) > 1e-6
