@@ -1,0 +1,196 @@
+/*
+ * submatrix.h -- C ABI of libsubmatrix.so: the submatrix method for the matrix sign
+ * function of a block-sparse symmetric matrix on one NVIDIA B200 (sm_100a).
+ *
+ * What the calls compute (citations are /root/reference/PAPER.md lines):
+ *   "The first step is the construction of a submatrix T_i(A) for every column of the
+ *    matrix A.  Then the matrix function is applied to the dense submatrices, i.e.
+ *    f(T_i(A)), and finally the relevant result columns are inserted into the sparse
+ *    result matrix."                                   (Fig. 2 caption)
+ *   f = sign, sign(A) = A (A^2)^(-1/2)                  (Eq. 13)
+ *   P = 1/2 (I - sign(S^-1 H - mu I)) S^-1, here S = I  (Eq. 14)
+ *   dense work in "FP16 operations with FP32 accumulation" on tensor units
+ *
+ * Conventions
+ *   - Every call returns an int32 status: SM_OK, a negative SM_ERR_*, or a positive
+ *     SM_WARN_*.  No exceptions, no exit(), no output on stdout/stderr.
+ *   - Unless a parameter says "host", every pointer is a DEVICE pointer.  The library
+ *     never allocates or frees device memory: the caller owns every buffer (sizes come
+ *     from sm_pattern_sizes / sm_sign_ws_bytes / sm_density_ws_bytes) and must keep it
+ *     alive until `stream` has been synchronised.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = default stream).  All work is
+ *     enqueued on it; calls return without synchronising except sm_pattern_sizes
+ *     (which must read sizes back) -- status codes that depend on device data
+ *     (SM_ERR_PATTERN, SM_WARN_NOT_CONVERGED) are therefore reported by sm_pattern_sizes
+ *     and sm_sign_status, which synchronise.
+ *   - One submatrix per BLOCK column i (one molecule).  Its index set N(i) is the
+ *     ascending list of block rows with a stored block in column i; entries between two
+ *     members of N(i) that are not stored are zero.  "Stored" is structural, never a
+ *     value threshold, so all pattern arrays are integer functions of integers and are
+ *     bit-exact.  The pattern must be structurally symmetric with every diagonal block
+ *     present and column indices strictly ascending per row (else SM_ERR_PATTERN).
+ *
+ * Packed submatrix buffers
+ *   A call that works on the column list cols[0..n_cols) (NULL = all block columns, in
+ *   id order) addresses submatrix number c of the list at element offset col_off[c] of
+ *   the packed buffer; col_off comes from sm_plan_columns (for cols == NULL it equals
+ *   P->sub_off).  Submatrix i has true dimension dim[i] and padded dimension
+ *   Pd = dim_pad[i] and occupies Pd*Pd elements:
+ *     SM_F64 / SM_F32 : row-major, leading dimension Pd.
+ *     SM_BF16 / SM_F16: the "K-major 128-byte-swizzled UMMA image" that tcgen05.mma reads
+ *       from shared memory, stored as is so that a tile is one contiguous bulk copy.
+ *       Pd must be a multiple of 64.  Element (r, c) lives at element offset
+ *         (c / 64) * Pd * 64  +  r * 64  +  ((((c % 64) / 8) ^ (r % 8)) * 8)  +  c % 8.
+ *   Padding rows/columns hold zeros and stay zero through the iteration.
+ */
+#ifndef SUBMATRIX_H_
+#define SUBMATRIX_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* status codes */
+#define SM_OK 0
+#define SM_ERR_ARG (-1)         /* bad argument (NULL, negative size, pad_to not allowed for dtype) */
+#define SM_ERR_SPACE (-2)       /* a caller buffer / workspace is too small */
+#define SM_ERR_PATTERN (-3)     /* pattern not structurally symmetric / diagonal missing / unsorted */
+#define SM_ERR_CUDA (-4)        /* a CUDA call failed; code from sm_last_cuda_error() */
+#define SM_ERR_UNSUPPORTED (-5) /* dtype / mode combination not implemented */
+#define SM_WARN_NOT_CONVERGED 1 /* some submatrix hit max_iter with residual >= tol */
+
+/* element types */
+#define SM_F64 0
+#define SM_F32 1
+#define SM_BF16 2
+#define SM_F16 3
+
+/* spectral scaling of T_i - mu I before the iteration (reading A10) */
+#define SM_SCALE_NONE 0        /* s_i = 1 */
+#define SM_SCALE_GERSHGORIN 1  /* s_i = max_r sum_c |(T_i - mu I)_rc|  (>= spectral radius) */
+#define SM_SCALE_POWER 2       /* s_i = 1.05 * ||T v||_2 after 16 power steps on T_i - mu I from a
+                                  fixed start vector, never above the Gershgorin bound */
+
+/* Block-CSR description of the symmetric input A = H ("block-sparse"). */
+typedef struct {
+  int32_t n_blk;           /* host: N block rows = block columns                         */
+  int32_t nnzb;            /* host: number of stored blocks                              */
+  const int32_t *blk_size; /* [N]      b_i > 0                                           */
+  const int32_t *row_ptr;  /* [N+1]                                                      */
+  const int32_t *col_idx;  /* [nnzb]   strictly ascending within a row                   */
+  const int64_t *val_ptr;  /* [nnzb+1] element offset of block p; row-major b_i x b_j    */
+} sm_bcsr_t;
+
+/* Sizes the caller needs to allocate the pattern (host struct, filled by sm_pattern_sizes). */
+typedef struct {
+  int64_t nbr_len;         /* = nnzb                                        */
+  int64_t gmap_len;        /* sum_i |N(i)|^2                                */
+  int64_t packed_elems;    /* sum_i dim_pad[i]^2                            */
+  int64_t build_ws_bytes;  /* workspace for sm_build_pattern                */
+  int32_t max_dim;         /* max_i dim[i]                                  */
+  int32_t max_dim_pad;     /* max_i dim_pad[i]                              */
+  int32_t max_nbr;         /* max_i |N(i)|                                  */
+  int32_t reserved;
+} sm_sizes_t;
+
+/* Output of sm_build_pattern (PAPER.md:110 step 1, integer part).  Host scalars are copied
+ * from sm_sizes_t by the caller; arrays are device memory, caller-allocated. */
+typedef struct {
+  int32_t n_blk, nnzb, pad_to, max_dim, max_dim_pad, max_nbr;   /* host */
+  int64_t packed_elems, gmap_len;                                /* host */
+  int32_t *nbr_ptr;   /* [N+1]     start of N(i) in nbr_idx                               */
+  int32_t *nbr_idx;   /* [nnzb]    N(i), ascending block ids                              */
+  int32_t *own_pos;   /* [N]       position of i inside N(i)                              */
+  int32_t *dim;       /* [N]       m_i = sum of b_j over N(i)                             */
+  int32_t *dim_pad;   /* [N]       m_i rounded up to a multiple of pad_to                 */
+  int32_t *row_off;   /* [nnzb]    first row of neighbour a inside submatrix i            */
+  int64_t *sub_off;   /* [N+1]     exclusive scan of dim_pad^2                            */
+  int64_t *gmap_ptr;  /* [N+1]     exclusive scan of |N(i)|^2                             */
+  int32_t *gmap;      /* [gmap_len] stored-block index of (N(i)[a], N(i)[c]) at a*|N(i)|+c, or -1 */
+  int32_t *tmap;      /* [nnzb]    index of the transposed partner block (j,i) of p=(i,j) */
+  int32_t *order;     /* [N]       block columns by (dim_pad descending, id ascending)    */
+} sm_pattern_t;
+
+/* Last CUDA error code seen by the calling thread's library calls (0 = none). host. */
+int32_t sm_last_cuda_error(void);
+
+/* Validates the pattern and returns the sizes.  `scratch` >= 256 bytes of device memory.
+ * Synchronises `stream`.  Errors: SM_ERR_ARG, SM_ERR_PATTERN, SM_ERR_CUDA. */
+int32_t sm_pattern_sizes(const sm_bcsr_t *A, int32_t pad_to, sm_sizes_t *out /*host*/,
+                         void *scratch, void *stream);
+
+/* a1. Builds all pattern arrays of P (bit-exact integer work).  P's host scalars must be
+ * filled from sm_pattern_sizes; ws >= build_ws_bytes.  Asynchronous. */
+int32_t sm_build_pattern(const sm_bcsr_t *A, int32_t pad_to, sm_pattern_t *P, void *ws,
+                         int64_t ws_bytes, void *stream);
+
+/* Offsets of a column list inside a packed buffer: col_off[c] = sum_{c'<c} dim_pad[cols[c']]^2,
+ * col_off[n_cols] = total.  cols == NULL is not needed (use P->sub_off).  Asynchronous. */
+int32_t sm_plan_columns(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols,
+                        int64_t *col_off /*[n_cols+1]*/, void *stream);
+
+/* a2. X0 = (T_i(A) - mu I) / s_i for the listed columns, padded, in x_dtype (PAPER.md:110
+ * step 1, :91 for the shift).  A_vals are A's block values (a_dtype SM_F64 or SM_F32).
+ * scale[c] (fp64, [n_cols]) receives s_i.  ws >= sm_gather_ws_bytes.  Asynchronous.
+ * Errors: SM_ERR_ARG (x_dtype 16-bit with pad_to % 64 != 0), SM_ERR_UNSUPPORTED, SM_ERR_SPACE. */
+int64_t sm_gather_ws_bytes(const sm_bcsr_t *A, const sm_pattern_t *P, int32_t n_cols);
+int32_t sm_gather(const sm_bcsr_t *A, const void *A_vals, int32_t a_dtype, const sm_pattern_t *P,
+                  const int32_t *cols, int32_t n_cols, const int64_t *col_off, double mu,
+                  int32_t scale_mode, int32_t x_dtype, void *X_packed, double *scale,
+                  void *ws, int64_t ws_bytes, void *stream);
+
+/* a3. Newton-Schulz sign iteration on every listed submatrix, in place (Eq. 13,
+ * "various iterative methods" :85; iteration X <- 1/2 X (3I - X^2), reading A9):
+ *     k = 0,1,..:  Y = X_k^2;  r_k = ||Y - I||_F / sqrt(m_i)  (true m_i, padding excluded);
+ *                  X_{k+1} = 1.5 X_k - 0.5 X_k Y;  stop after this update if r_k < tol.
+ * tol <= 0 runs exactly max_iter updates.  iters[c] = updates applied, residual[c] = last
+ * r_k computed.  SM_BF16/SM_F16 run on tcgen05 tensor cores with fp32 accumulation
+ * (PAPER.md:104); SM_F32/SM_F64 on FFMA/DFMA.  packed_elems = col_off[n_cols] (host value).
+ * ws >= sm_sign_ws_bytes(...).  Asynchronous; sm_sign_status reports non-convergence. */
+int64_t sm_sign_ws_bytes(const sm_pattern_t *P, int32_t n_cols, int64_t packed_elems, int32_t x_dtype);
+int32_t sm_sign_ns(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols,
+                   const int64_t *col_off, int64_t packed_elems, int32_t x_dtype, void *X_packed,
+                   void *ws, int64_t ws_bytes, int32_t max_iter, double tol,
+                   int32_t *iters /*[n_cols]*/, double *residual /*[n_cols]*/, void *stream);
+/* Synchronises and returns SM_WARN_NOT_CONVERGED if tol > 0 and any residual[c] >= tol. */
+int32_t sm_sign_status(const double *residual, int32_t n_cols, double tol, void *scratch, void *stream);
+
+/* a4. R(N(i)[a], i) = S_i[rows of neighbour a, columns of block i] for the listed columns
+ * (PAPER.md:110 step 3) into block-CSR values with A's layout; r_dtype SM_F64 or SM_F32.
+ * S_i is symmetric, so the owned ROWS are read (contiguous) and transposed on the fly.
+ * symmetrise != 0 (only with all columns present, i.e. after the last chunk) additionally
+ * replaces R by 1/2 (R + R^T) blockwise through tmap (reading A6). Asynchronous. */
+int32_t sm_scatter(const sm_bcsr_t *A, const sm_pattern_t *P, const int32_t *cols, int32_t n_cols,
+                   const int64_t *col_off, int32_t x_dtype, const void *S_packed, int32_t r_dtype,
+                   void *R_vals, int32_t symmetrise, void *stream);
+/* In-place blockwise symmetrisation of block-CSR values (used after chunked scatters). */
+int32_t sm_symmetrise(const sm_bcsr_t *A, const sm_pattern_t *P, int32_t r_dtype, void *R_vals,
+                      void *stream);
+
+/* a5. The whole path, Eq. 14 with S = I: D = 1/2 (I - sign(H - mu I)) by the submatrix method:
+ * gather -> sign -> scatter (-> symmetrise) -> D = 1/2 (I - R), Tr D.  Columns are processed in
+ * chunks that fit ws_bytes; h_dim_pad is a HOST copy of P->dim_pad (needed to plan chunks).
+ * d_dtype SM_F64 or SM_F32; trace is a device fp64 scalar; iters/residual/scale are [N] device
+ * arrays.  ws >= sm_density_ws_bytes(P, x_dtype, max_chunk_elems) where max_chunk_elems bounds the
+ * packed elements per chunk (>= max_dim_pad^2; P->packed_elems for a single chunk).  Asynchronous. */
+int64_t sm_density_ws_bytes(const sm_bcsr_t *A, const sm_pattern_t *P, int32_t x_dtype,
+                            int64_t max_chunk_elems);
+int32_t sm_density(const sm_bcsr_t *A, const void *A_vals, int32_t a_dtype, double mu,
+                   int32_t x_dtype, int32_t scale_mode, int32_t max_iter, double tol,
+                   int32_t symmetrise, const sm_pattern_t *P, const int32_t *h_dim_pad /*host [N]*/,
+                   int64_t max_chunk_elems, void *ws, int64_t ws_bytes, int32_t d_dtype,
+                   void *D_vals, double *trace, int32_t *iters, double *residual, double *scale,
+                   void *stream);
+/* R -> D = 1/2 (I - R) in place on block-CSR values, and Tr D (device fp64 scalar, may be NULL). */
+int32_t sm_density_from_sign(const sm_bcsr_t *A, const sm_pattern_t *P, int32_t d_dtype,
+                             void *RD_vals, double *trace, void *stream);
+
+/* Number of kernels this thread's library calls have launched so far (bench bookkeeping). host. */
+int64_t sm_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SUBMATRIX_H_ */

@@ -1,0 +1,131 @@
+// C-ABI entry points that dispatch or compose: sm_sign_ns (a3) and sm_density (a5, the whole path
+// gather -> sign -> scatter -> D = 1/2 (I - R), PAPER.md:110 steps 1-3 + PAPER.md:91 Eq. 14, S = I).
+#include <algorithm>
+#include <numeric>
+#include <vector>
+
+#include "common.cuh"
+
+using namespace sm;
+
+namespace sm {
+static __global__ void k_count_unconverged(int32_t n, const double *__restrict__ residual, double tol,
+                                           int32_t *__restrict__ out) {
+  int32_t c = blockIdx.x * blockDim.x + threadIdx.x;
+  if (c < n && !(residual[c] < tol)) atomicAdd(out, 1);
+}
+}  // namespace sm
+
+extern "C" int64_t sm_sign_ws_bytes(const sm_pattern_t *P, int32_t n_cols, int64_t packed_elems,
+                                    int32_t x_dtype) {
+  if (!P || n_cols <= 0 || packed_elems <= 0) return SM_ERR_ARG;
+  if (is_16bit(x_dtype)) return sign_umma_ws_bytes(P, n_cols, packed_elems, x_dtype);
+  if (x_dtype == SM_F32 || x_dtype == SM_F64) return sign_simt_ws_bytes(P, n_cols, packed_elems, x_dtype);
+  return SM_ERR_UNSUPPORTED;
+}
+
+extern "C" int32_t sm_sign_ns(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols,
+                              const int64_t *col_off, int64_t packed_elems, int32_t x_dtype, void *X_packed,
+                              void *ws, int64_t ws_bytes, int32_t max_iter, double tol, int32_t *iters,
+                              double *residual, void *stream) {
+  if (!P || !col_off || !X_packed || !ws || !iters || !residual) return SM_ERR_ARG;
+  if (!cols) n_cols = P->n_blk;
+  if (n_cols <= 0 || max_iter < 0 || packed_elems <= 0) return SM_ERR_ARG;
+  cudaStream_t st = (cudaStream_t)stream;
+  if (is_16bit(x_dtype))
+    return sign_umma(P, cols, n_cols, col_off, packed_elems, x_dtype, X_packed, ws, ws_bytes, max_iter, tol,
+                     iters, residual, st);
+  if (x_dtype == SM_F32 || x_dtype == SM_F64)
+    return sign_simt(P, cols, n_cols, col_off, packed_elems, x_dtype, X_packed, ws, ws_bytes, max_iter, tol,
+                     iters, residual, st);
+  return SM_ERR_UNSUPPORTED;
+}
+
+extern "C" int32_t sm_sign_status(const double *residual, int32_t n_cols, double tol, void *scratch,
+                                  void *stream) {
+  if (!residual || !scratch || n_cols <= 0) return SM_ERR_ARG;
+  cudaStream_t st = (cudaStream_t)stream;
+  if (!(tol > 0.0)) { SM_CUDA(cudaStreamSynchronize(st)); return SM_OK; }
+  int32_t *d = (int32_t *)scratch;
+  SM_CUDA(cudaMemsetAsync(d, 0, sizeof(int32_t), st));
+  k_count_unconverged<<<(n_cols + 255) / 256, 256, 0, st>>>(n_cols, residual, tol, d);
+  SM_LAUNCHED();
+  int32_t h = 0;
+  SM_CUDA(cudaMemcpyAsync(&h, d, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+  SM_CUDA(cudaStreamSynchronize(st));
+  return h > 0 ? SM_WARN_NOT_CONVERGED : SM_OK;
+}
+
+namespace {
+struct DensityWs { int64_t *col_off; void *X; void *gws; int64_t gws_bytes; void *sws; int64_t sws_bytes; int64_t used; };
+
+DensityWs density_layout(void *ws, int64_t ws_bytes, const sm_bcsr_t *A, const sm_pattern_t *P, int32_t x_dtype,
+                         int64_t max_chunk_elems) {
+  WsCursor cur(ws, ws_bytes);
+  DensityWs w;
+  w.col_off = cur.take<int64_t>(P->n_blk + 1);
+  w.X = cur.take<char>(max_chunk_elems * dtype_bytes(x_dtype));
+  w.gws_bytes = sm_gather_ws_bytes(A, P, P->n_blk);
+  w.gws = cur.take<char>(w.gws_bytes);
+  w.sws_bytes = sm_sign_ws_bytes(P, P->n_blk, max_chunk_elems, x_dtype);
+  w.sws = cur.take<char>(w.sws_bytes > 0 ? w.sws_bytes : 1);
+  w.used = cur.used + 256;
+  return w;
+}
+}  // namespace
+
+extern "C" int64_t sm_density_ws_bytes(const sm_bcsr_t *A, const sm_pattern_t *P, int32_t x_dtype,
+                                       int64_t max_chunk_elems) {
+  if (!A || !P || dtype_bytes(x_dtype) == 0) return SM_ERR_ARG;
+  if (max_chunk_elems < (int64_t)P->max_dim_pad * P->max_dim_pad) return SM_ERR_ARG;
+  return density_layout(nullptr, 0, A, P, x_dtype, max_chunk_elems).used;
+}
+
+extern "C" int32_t sm_density(const sm_bcsr_t *A, const void *A_vals, int32_t a_dtype, double mu,
+                              int32_t x_dtype, int32_t scale_mode, int32_t max_iter, double tol,
+                              int32_t symmetrise, const sm_pattern_t *P, const int32_t *h_dim_pad,
+                              int64_t max_chunk_elems, void *ws, int64_t ws_bytes, int32_t d_dtype,
+                              void *D_vals, double *trace, int32_t *iters, double *residual, double *scale,
+                              void *stream) {
+  if (!A || !A_vals || !P || !h_dim_pad || !ws || !D_vals || !iters || !residual || !scale) return SM_ERR_ARG;
+  if (dtype_bytes(x_dtype) == 0) return SM_ERR_UNSUPPORTED;
+  if (d_dtype != SM_F64 && d_dtype != SM_F32) return SM_ERR_UNSUPPORTED;
+  if (max_chunk_elems < (int64_t)P->max_dim_pad * P->max_dim_pad) return SM_ERR_ARG;
+  DensityWs w = density_layout(ws, ws_bytes, A, P, x_dtype, max_chunk_elems);
+  if (w.sws_bytes < 0) return (int32_t)w.sws_bytes;
+  if (w.used > ws_bytes) return SM_ERR_SPACE;
+  const int32_t n = P->n_blk;
+  // Same key as P->order: (dim_pad descending, id ascending); chunks are ranges of that order, so
+  // the device list of a chunk is P->order + lo.  Output arrays are indexed by order position.
+  std::vector<int32_t> ord(n);
+  std::iota(ord.begin(), ord.end(), 0);
+  std::stable_sort(ord.begin(), ord.end(), [&](int32_t x, int32_t y) { return h_dim_pad[x] > h_dim_pad[y]; });
+  int32_t lo = 0;
+  while (lo < n) {
+    int64_t elems = 0;
+    int32_t hi = lo;
+    while (hi < n) {
+      int64_t e = (int64_t)h_dim_pad[ord[hi]] * h_dim_pad[ord[hi]];
+      if (hi > lo && elems + e > max_chunk_elems) break;
+      elems += e; ++hi;
+    }
+    const int32_t nc = hi - lo;
+    const int32_t *cols = P->order + lo;
+    int32_t rc = sm_plan_columns(P, cols, nc, w.col_off, stream);
+    if (rc != SM_OK) return rc;
+    rc = sm_gather(A, A_vals, a_dtype, P, cols, nc, w.col_off, mu, scale_mode, x_dtype, w.X, scale + lo, w.gws,
+                   w.gws_bytes, stream);
+    if (rc != SM_OK) return rc;
+    rc = sm_sign_ns(P, cols, nc, w.col_off, elems, x_dtype, w.X, w.sws, w.sws_bytes, max_iter, tol, iters + lo,
+                    residual + lo, stream);
+    if (rc != SM_OK) return rc;
+    rc = sm_scatter(A, P, cols, nc, w.col_off, x_dtype, w.X, d_dtype, D_vals, 0, stream);
+    if (rc != SM_OK) return rc;
+    lo = hi;
+  }
+  if (symmetrise) {
+    int32_t rc = sm_symmetrise(A, P, d_dtype, D_vals, stream);
+    if (rc != SM_OK) return rc;
+  }
+  return sm_density_from_sign(A, P, d_dtype, D_vals, trace, stream);
+}

@@ -1,0 +1,418 @@
+// a2 gather, a4 scatter (+ symmetrise), a5 density/trace: the HBM-bound ends of the path.
+// PAPER.md:110 (Fig. 2 steps 1 and 3), PAPER.md:91 (Eq. 14 with S = I).
+#include "common.cuh"
+
+namespace sm {
+
+// ---- spectral scale --------------------------------------------------------------------------
+// rowbase[i] = sum_{i'<i} |N(i')| * b_i'  (offset of block row i's abs-row-sums).
+__global__ void k_rowbase_in(int32_t n, const int32_t *__restrict__ blk, const int32_t *__restrict__ rp,
+                             int64_t *__restrict__ out) {
+  int32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) out[i] = (int64_t)(rp[i + 1] - rp[i]) * blk[i];
+}
+
+// babs[rowbase[i] + (p - rp[i]) * b_i + r] = sum_s |(A - mu I)_p[r, s]| for every stored block p.
+template <typename TA>
+__global__ void k_block_abs_rowsum(const int32_t *__restrict__ blk, const int32_t *__restrict__ rp,
+                                   const int32_t *__restrict__ ci, const int64_t *__restrict__ vp,
+                                   const TA *__restrict__ vals, double mu,
+                                   const int64_t *__restrict__ rowbase, double *__restrict__ babs) {
+  int32_t i = blockIdx.x;
+  int32_t bi = blk[i], lo = rp[i], cnt = rp[i + 1] - lo;
+  for (int32_t e = threadIdx.x; e < cnt * bi; e += blockDim.x) {
+    int32_t q = e / bi, r = e - q * bi;
+    int32_t p = lo + q, j = ci[p], bj = blk[j];
+    const TA *row = vals + vp[p] + (int64_t)r * bj;
+    double s = 0.0;
+    for (int32_t c = 0; c < bj; ++c) {
+      double v = to_double<TA>(row[c]);
+      if (j == i && c == r) v -= mu;
+      s += fabs(v);
+    }
+    babs[rowbase[i] + e] = s;
+  }
+}
+
+// Gershgorin: scale[c] = max over rows of T_i - mu I of the absolute row sum.  One CTA per column.
+__global__ void k_scale_gershgorin(const int32_t *__restrict__ cols, const int32_t *__restrict__ blk,
+                                   const int32_t *__restrict__ rp, const int32_t *__restrict__ ci,
+                                   const int64_t *__restrict__ gmap_ptr, const int32_t *__restrict__ gmap,
+                                   const int64_t *__restrict__ rowbase, const double *__restrict__ babs,
+                                   double *__restrict__ scale) {
+  int32_t c = blockIdx.x;
+  int32_t i = cols ? cols[c] : c;
+  int32_t lo = rp[i], cnt = rp[i + 1] - lo;
+  const int32_t *g = gmap + gmap_ptr[i];
+  double best = 0.0;
+  // rows are enumerated as (neighbour a, local row r); neighbour a is block row ja = ci[lo + a]
+  for (int32_t a = 0; a < cnt; ++a) {
+    int32_t ja = ci[lo + a], ba = blk[ja], rlo = rp[ja];
+    for (int32_t r = threadIdx.x; r < ba; r += blockDim.x) {
+      double s = 0.0;
+      for (int32_t cc = 0; cc < cnt; ++cc) {
+        int32_t p = g[a * cnt + cc];
+        if (p >= 0) s += babs[rowbase[ja] + (int64_t)(p - rlo) * ba + r];
+      }
+      best = fmax(best, s);
+    }
+  }
+  __shared__ double red[32];
+  for (int d = 16; d > 0; d >>= 1) best = fmax(best, __shfl_xor_sync(0xffffffffu, best, d));
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = best;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double m = 0.0;
+    for (int w = 0; w < (int)(blockDim.x >> 5); ++w) m = fmax(m, red[w]);
+    scale[c] = m > 0.0 ? m : 1.0;
+  }
+}
+
+__global__ void k_fill_double(int32_t n, double v, double *__restrict__ out) {
+  int32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) out[i] = v;
+}
+
+// ---- gather ------------------------------------------------------------------------------------
+// grid = (listed column, band of GATHER_ROWS rows).  Dynamic smem: int32 off[cnt+1], uint16 blkof[m].
+constexpr int GATHER_ROWS = 16;
+
+struct GatherArgs {
+  const int32_t *cols; const int64_t *col_off;
+  const int32_t *blk, *rp, *ci; const int64_t *vp;
+  const int64_t *gmap_ptr; const int32_t *gmap;
+  const int32_t *dim, *dim_pad;
+  const double *scale; double mu;
+};
+
+template <typename TA>
+__device__ inline double gather_elem(const GatherArgs &g, const TA *__restrict__ vals, const int32_t *off,
+                                     const uint16_t *blkof, const int32_t *gm, int32_t cnt, int32_t m,
+                                     int32_t r, int32_t c, double inv_s) {
+  if (r >= m || c >= m) return 0.0;
+  int32_t a = blkof[r], b = blkof[c];
+  int32_t p = gm[a * cnt + b];
+  double v = 0.0;
+  if (p >= 0) {
+    int32_t bc = off[b + 1] - off[b];
+    v = to_double<TA>(vals[g.vp[p] + (int64_t)(r - off[a]) * bc + (c - off[b])]);
+  }
+  if (r == c) v -= g.mu;
+  return v * inv_s;
+}
+
+template <typename TA, typename TX, bool IMG>
+__global__ void k_gather(GatherArgs g, const TA *__restrict__ vals, TX *__restrict__ X) {
+  extern __shared__ int32_t smem_i[];
+  int32_t c_list = blockIdx.x;
+  int32_t i = g.cols ? g.cols[c_list] : c_list;
+  int32_t Pd = g.dim_pad[i], m = g.dim[i];
+  int32_t r0 = blockIdx.y * GATHER_ROWS;
+  if (r0 >= Pd) return;
+  int32_t lo = g.rp[i], cnt = g.rp[i + 1] - lo;
+  int32_t *off = smem_i;
+  uint16_t *blkof = (uint16_t *)(smem_i + cnt + 1);
+  if (threadIdx.x == 0) {
+    int32_t o = 0;
+    for (int32_t a = 0; a < cnt; ++a) { off[a] = o; o += g.blk[g.ci[lo + a]]; }
+    off[cnt] = o;
+  }
+  __syncthreads();
+  for (int32_t a = 0; a < cnt; ++a)
+    for (int32_t r = off[a] + threadIdx.x; r < off[a + 1]; r += blockDim.x) blkof[r] = (uint16_t)a;
+  __syncthreads();
+  const int32_t *gm = g.gmap + g.gmap_ptr[i];
+  double inv_s = 1.0 / g.scale[c_list];
+  TX *Xs = X + g.col_off[c_list];
+  int32_t rows = min(GATHER_ROWS, Pd - r0);
+  if (IMG) {
+    int32_t chunks = Pd >> 3;
+    for (int32_t e = threadIdx.x; e < rows * chunks; e += blockDim.x) {
+      int32_t rr = e / chunks, ch = e - rr * chunks;
+      int32_t r = r0 + rr, c0 = ch << 3;
+      __align__(16) TX v[8];
+#pragma unroll
+      for (int k = 0; k < 8; ++k)
+        v[k] = from_double<TX>(gather_elem<TA>(g, vals, off, blkof, gm, cnt, m, r, c0 + k, inv_s));
+      *reinterpret_cast<uint4 *>(Xs + img_off(Pd, r, c0)) = *reinterpret_cast<const uint4 *>(v);
+    }
+  } else {
+    for (int32_t e = threadIdx.x; e < rows * Pd; e += blockDim.x) {
+      int32_t rr = e / Pd, c = e - rr * Pd;
+      int32_t r = r0 + rr;
+      Xs[(int64_t)r * Pd + c] = from_double<TX>(gather_elem<TA>(g, vals, off, blkof, gm, cnt, m, r, c, inv_s));
+    }
+  }
+}
+
+// ---- scatter -----------------------------------------------------------------------------------
+// One CTA per listed column i.  Reads the owned ROWS of S_i (S_i symmetric): element
+// S_i[own_off + s, r] goes to block (N(i)[a], i) at [r - off[a], s].
+template <typename TX, typename TR, bool IMG>
+__global__ void k_scatter(const int32_t *__restrict__ cols, const int64_t *__restrict__ col_off,
+                          const int32_t *__restrict__ blk, const int32_t *__restrict__ rp,
+                          const int32_t *__restrict__ ci, const int64_t *__restrict__ vp,
+                          const int32_t *__restrict__ own_pos, const int32_t *__restrict__ dim,
+                          const int32_t *__restrict__ dim_pad, const int32_t *__restrict__ tmap,
+                          const TX *__restrict__ S, TR *__restrict__ R) {
+  extern __shared__ int32_t smem_i[];
+  int32_t c_list = blockIdx.x;
+  int32_t i = cols ? cols[c_list] : c_list;
+  int32_t Pd = dim_pad[i], m = dim[i];
+  int32_t lo = rp[i], cnt = rp[i + 1] - lo;
+  int32_t *off = smem_i;
+  uint16_t *blkof = (uint16_t *)(smem_i + cnt + 1);
+  if (threadIdx.x == 0) {
+    int32_t o = 0;
+    for (int32_t a = 0; a < cnt; ++a) { off[a] = o; o += blk[ci[lo + a]]; }
+    off[cnt] = o;
+  }
+  __syncthreads();
+  for (int32_t a = 0; a < cnt; ++a)
+    for (int32_t r = off[a] + threadIdx.x; r < off[a + 1]; r += blockDim.x) blkof[r] = (uint16_t)a;
+  __syncthreads();
+  int32_t own = own_pos[i], own_off = off[own], bi = off[own + 1] - own_off;
+  const TX *Ss = S + col_off[c_list];
+  for (int32_t e = threadIdx.x; e < bi * m; e += blockDim.x) {
+    int32_t s = e / m, r = e - s * m;
+    int32_t row = own_off + s;
+    TX v = IMG ? Ss[img_off(Pd, row, r)] : Ss[(int64_t)row * Pd + r];
+    int32_t a = blkof[r];
+    int32_t p = tmap[lo + a];                 // block (N(i)[a], i)
+    R[vp[p] + (int64_t)(r - off[a]) * bi + s] = (TR)to_double<TX>(v);
+  }
+}
+
+// R <- 1/2 (R + R^T) blockwise, in place.  One CTA per block row; the lower-indexed partner of a
+// pair (p, tmap[p]) owns both blocks.
+template <typename TR>
+__global__ void k_symmetrise(const int32_t *__restrict__ blk, const int32_t *__restrict__ rp,
+                             const int32_t *__restrict__ ci, const int64_t *__restrict__ vp,
+                             const int32_t *__restrict__ tmap, TR *R) {
+  int32_t i = blockIdx.x, bi = blk[i];
+  for (int32_t p = rp[i]; p < rp[i + 1]; ++p) {
+    int32_t q = tmap[p];
+    if (q < p) continue;
+    int32_t bj = blk[ci[p]];
+    TR *Rp = R + vp[p], *Rq = R + vp[q];
+    for (int32_t e = threadIdx.x; e < bi * bj; e += blockDim.x) {
+      int32_t r = e / bj, s = e - r * bj;
+      if (p == q && s <= r) continue;
+      TR a = Rp[(int64_t)r * bj + s], b = Rq[(int64_t)s * bi + r];
+      TR v = (TR)0.5 * (a + b);
+      Rp[(int64_t)r * bj + s] = v;
+      Rq[(int64_t)s * bi + r] = v;
+    }
+  }
+}
+
+// D = 1/2 (I - R) in place (Eq. 14, S = I).  One CTA per block row.
+template <typename TR>
+__global__ void k_density(const int32_t *__restrict__ blk, const int32_t *__restrict__ rp,
+                          const int32_t *__restrict__ ci, const int64_t *__restrict__ vp, TR *RD) {
+  int32_t i = blockIdx.x, bi = blk[i];
+  for (int32_t p = rp[i]; p < rp[i + 1]; ++p) {
+    int32_t j = ci[p], bj = blk[j];
+    TR *B = RD + vp[p];
+    for (int32_t e = threadIdx.x; e < bi * bj; e += blockDim.x) {
+      int32_t r = e / bj, s = e - r * bj;
+      TR id = (j == i && r == s) ? (TR)1 : (TR)0;
+      B[e] = (TR)0.5 * (id - B[e]);
+    }
+  }
+}
+
+// Tr D: one CTA, fixed summation tree (deterministic).
+template <typename TR>
+__global__ void k_trace(int32_t n, const int32_t *__restrict__ blk, const int32_t *__restrict__ rp,
+                        const int64_t *__restrict__ vp, const int32_t *__restrict__ own_pos,
+                        const TR *__restrict__ D, double *__restrict__ trace) {
+  __shared__ double red[1024];
+  double acc = 0.0;
+  for (int32_t i = threadIdx.x; i < n; i += blockDim.x) {
+    int32_t b = blk[i];
+    const TR *B = D + vp[rp[i] + own_pos[i]];
+    double t = 0.0;
+    for (int32_t r = 0; r < b; ++r) t += (double)B[(int64_t)r * b + r];
+    acc += t;
+  }
+  red[threadIdx.x] = acc;
+  __syncthreads();
+  for (int d = blockDim.x >> 1; d > 0; d >>= 1) {
+    if ((int)threadIdx.x < d) red[threadIdx.x] += red[threadIdx.x + d];
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) *trace = red[0];
+}
+
+}  // namespace sm
+
+using namespace sm;
+
+
+extern "C" int64_t sm_gather_ws_bytes(const sm_bcsr_t *A, const sm_pattern_t *P, int32_t n_cols) {
+  if (!A || !P) return SM_ERR_ARG;
+  (void)n_cols;
+  WsCursor cur(nullptr, 0);
+  cur.take<int64_t>(A->n_blk + 1);
+  cur.take<double>((int64_t)A->n_blk * P->max_dim);
+  cur.take<double>(A->n_blk);
+  return cur.used + 256;
+}
+
+template <typename TA, typename TX, bool IMG>
+static int32_t launch_gather(const GatherArgs &g, const void *vals, void *X, int32_t n_cols, int32_t max_pd,
+                             int32_t max_nbr, int32_t max_dim, cudaStream_t st) {
+  dim3 grid(n_cols, (max_pd + GATHER_ROWS - 1) / GATHER_ROWS);
+  size_t smem = (size_t)(max_nbr + 1) * 4 + (size_t)(max_dim + 2) * 2;
+  k_gather<TA, TX, IMG><<<grid, 256, smem, st>>>(g, (const TA *)vals, (TX *)X);
+  SM_LAUNCHED();
+  return SM_OK;
+}
+
+extern "C" int32_t sm_gather(const sm_bcsr_t *A, const void *A_vals, int32_t a_dtype, const sm_pattern_t *P,
+                             const int32_t *cols, int32_t n_cols, const int64_t *col_off, double mu,
+                             int32_t scale_mode, int32_t x_dtype, void *X_packed, double *scale, void *ws,
+                             int64_t ws_bytes, void *stream) {
+  if (!A || !A_vals || !P || !X_packed || !scale || !ws || !col_off) return SM_ERR_ARG;
+  if (!cols) n_cols = P->n_blk;
+  if (n_cols <= 0) return SM_ERR_ARG;
+  if (a_dtype != SM_F64 && a_dtype != SM_F32) return SM_ERR_UNSUPPORTED;
+  if (dtype_bytes(x_dtype) == 0) return SM_ERR_UNSUPPORTED;
+  if (is_16bit(x_dtype) && (P->pad_to % 64) != 0) return SM_ERR_ARG;
+  if (scale_mode < SM_SCALE_NONE || scale_mode > SM_SCALE_POWER) return SM_ERR_UNSUPPORTED;
+  if (P->max_dim > 65535) return SM_ERR_UNSUPPORTED;
+  cudaStream_t st = (cudaStream_t)stream;
+  int32_t n = A->n_blk;
+  WsCursor cur(ws, ws_bytes);
+  int64_t *rowbase = cur.take<int64_t>(n + 1);
+  double *babs = cur.take<double>((int64_t)n * P->max_dim);
+  double *ratio = cur.take<double>(n);
+  if (!cur.ok()) return SM_ERR_SPACE;
+
+  if (scale_mode == SM_SCALE_NONE) {
+    k_fill_double<<<(n_cols + 255) / 256, 256, 0, st>>>(n_cols, 1.0, scale);
+    SM_LAUNCHED();
+  } else {
+    k_rowbase_in<<<(n + 127) / 128, 128, 0, st>>>(n, A->blk_size, A->row_ptr, rowbase);
+    SM_LAUNCHED();
+    { int32_t rc0 = exclusive_scan_i64(n, rowbase, rowbase, st); if (rc0 != SM_OK) return rc0; }
+    if (a_dtype == SM_F64)
+      k_block_abs_rowsum<double><<<n, 128, 0, st>>>(A->blk_size, A->row_ptr, A->col_idx, A->val_ptr,
+                                                    (const double *)A_vals, mu, rowbase, babs);
+    else
+      k_block_abs_rowsum<float><<<n, 128, 0, st>>>(A->blk_size, A->row_ptr, A->col_idx, A->val_ptr,
+                                                   (const float *)A_vals, mu, rowbase, babs);
+    SM_LAUNCHED();
+    k_scale_gershgorin<<<n_cols, 128, 0, st>>>(cols, A->blk_size, A->row_ptr, A->col_idx, P->gmap_ptr,
+                                               P->gmap, rowbase, babs, scale);
+    SM_LAUNCHED();
+  }
+
+  GatherArgs g{cols, col_off, A->blk_size, A->row_ptr, A->col_idx, A->val_ptr, P->gmap_ptr, P->gmap,
+               P->dim, P->dim_pad, scale, mu};
+  // SM_SCALE_POWER: gather at the Gershgorin scale, tighten the scale by power steps on that X0
+  // (power_scale.cu), then gather again so that X0 is rounded to the working type only once.
+  const int passes = (scale_mode == SM_SCALE_POWER) ? 2 : 1;
+  for (int pass = 0; pass < passes; ++pass) {
+    int32_t rc = SM_ERR_UNSUPPORTED;
+#define SM_GATHER_CASE(TA, TX, IMG) \
+  rc = launch_gather<TA, TX, IMG>(g, A_vals, X_packed, n_cols, P->max_dim_pad, P->max_nbr, P->max_dim, st)
+    if (a_dtype == SM_F64) {
+      if (x_dtype == SM_F64) SM_GATHER_CASE(double, double, false);
+      else if (x_dtype == SM_F32) SM_GATHER_CASE(double, float, false);
+      else if (x_dtype == SM_BF16) SM_GATHER_CASE(double, __nv_bfloat16, true);
+      else SM_GATHER_CASE(double, __half, true);
+    } else {
+      if (x_dtype == SM_F64) SM_GATHER_CASE(float, double, false);
+      else if (x_dtype == SM_F32) SM_GATHER_CASE(float, float, false);
+      else if (x_dtype == SM_BF16) SM_GATHER_CASE(float, __nv_bfloat16, true);
+      else SM_GATHER_CASE(float, __half, true);
+    }
+#undef SM_GATHER_CASE
+    if (rc != SM_OK) return rc;
+    if (pass == 0 && passes == 2) {
+      rc = power_scale(P, cols, n_cols, col_off, x_dtype, X_packed, scale, ratio, st);
+      if (rc != SM_OK) return rc;
+    }
+  }
+  return SM_OK;
+}
+
+template <typename TX, typename TR, bool IMG>
+static int32_t launch_scatter(const sm_bcsr_t *A, const sm_pattern_t *P, const int32_t *cols, int32_t n_cols,
+                              const int64_t *col_off, const void *S, void *R, cudaStream_t st) {
+  size_t smem = (size_t)(P->max_nbr + 1) * 4 + (size_t)(P->max_dim + 2) * 2;
+  k_scatter<TX, TR, IMG><<<n_cols, 256, smem, st>>>(cols, col_off, A->blk_size, A->row_ptr, A->col_idx,
+                                                    A->val_ptr, P->own_pos, P->dim, P->dim_pad, P->tmap,
+                                                    (const TX *)S, (TR *)R);
+  SM_LAUNCHED();
+  return SM_OK;
+}
+
+extern "C" int32_t sm_symmetrise(const sm_bcsr_t *A, const sm_pattern_t *P, int32_t r_dtype, void *R_vals,
+                                 void *stream) {
+  if (!A || !P || !R_vals) return SM_ERR_ARG;
+  cudaStream_t st = (cudaStream_t)stream;
+  if (r_dtype == SM_F64)
+    k_symmetrise<double><<<A->n_blk, 128, 0, st>>>(A->blk_size, A->row_ptr, A->col_idx, A->val_ptr, P->tmap,
+                                                   (double *)R_vals);
+  else if (r_dtype == SM_F32)
+    k_symmetrise<float><<<A->n_blk, 128, 0, st>>>(A->blk_size, A->row_ptr, A->col_idx, A->val_ptr, P->tmap,
+                                                  (float *)R_vals);
+  else
+    return SM_ERR_UNSUPPORTED;
+  SM_LAUNCHED();
+  return SM_OK;
+}
+
+extern "C" int32_t sm_scatter(const sm_bcsr_t *A, const sm_pattern_t *P, const int32_t *cols, int32_t n_cols,
+                              const int64_t *col_off, int32_t x_dtype, const void *S_packed, int32_t r_dtype,
+                              void *R_vals, int32_t symmetrise, void *stream) {
+  if (!A || !P || !S_packed || !R_vals || !col_off) return SM_ERR_ARG;
+  if (!cols) n_cols = P->n_blk;
+  if (n_cols <= 0) return SM_ERR_ARG;
+  if (r_dtype != SM_F64 && r_dtype != SM_F32) return SM_ERR_UNSUPPORTED;
+  if (symmetrise && cols && n_cols != P->n_blk) return SM_ERR_ARG;
+  if (P->max_dim > 65535) return SM_ERR_UNSUPPORTED;
+  cudaStream_t st = (cudaStream_t)stream;
+  int32_t rc = SM_ERR_UNSUPPORTED;
+#define SM_SCATTER_CASE(TX, IMG)                                                                   \
+  rc = (r_dtype == SM_F64)                                                                         \
+           ? launch_scatter<TX, double, IMG>(A, P, cols, n_cols, col_off, S_packed, R_vals, st)    \
+           : launch_scatter<TX, float, IMG>(A, P, cols, n_cols, col_off, S_packed, R_vals, st)
+  if (x_dtype == SM_F64) SM_SCATTER_CASE(double, false);
+  else if (x_dtype == SM_F32) SM_SCATTER_CASE(float, false);
+  else if (x_dtype == SM_BF16) SM_SCATTER_CASE(__nv_bfloat16, true);
+  else if (x_dtype == SM_F16) SM_SCATTER_CASE(__half, true);
+#undef SM_SCATTER_CASE
+  if (rc != SM_OK) return rc;
+  if (symmetrise) return sm_symmetrise(A, P, r_dtype, R_vals, stream);
+  return SM_OK;
+}
+
+extern "C" int32_t sm_density_from_sign(const sm_bcsr_t *A, const sm_pattern_t *P, int32_t d_dtype,
+                                        void *RD_vals, double *trace, void *stream) {
+  if (!A || !P || !RD_vals) return SM_ERR_ARG;
+  cudaStream_t st = (cudaStream_t)stream;
+  if (d_dtype == SM_F64) {
+    k_density<double><<<A->n_blk, 128, 0, st>>>(A->blk_size, A->row_ptr, A->col_idx, A->val_ptr, (double *)RD_vals);
+    SM_LAUNCHED();
+    if (trace) {
+      k_trace<double><<<1, 1024, 0, st>>>(A->n_blk, A->blk_size, A->row_ptr, A->val_ptr, P->own_pos,
+                                          (const double *)RD_vals, trace);
+      SM_LAUNCHED();
+    }
+  } else if (d_dtype == SM_F32) {
+    k_density<float><<<A->n_blk, 128, 0, st>>>(A->blk_size, A->row_ptr, A->col_idx, A->val_ptr, (float *)RD_vals);
+    SM_LAUNCHED();
+    if (trace) {
+      k_trace<float><<<1, 1024, 0, st>>>(A->n_blk, A->blk_size, A->row_ptr, A->val_ptr, P->own_pos,
+                                         (const float *)RD_vals, trace);
+      SM_LAUNCHED();
+    }
+  } else {
+    return SM_ERR_UNSUPPORTED;
+  }
+  return SM_OK;
+}

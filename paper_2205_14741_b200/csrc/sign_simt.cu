@@ -1,0 +1,192 @@
+// a3, fp32 / fp64 back end: Newton-Schulz X <- 1/2 X (3I - X^2) on row-major packed submatrices
+// with FFMA / DFMA register-tiled products (tcgen05 has no fp32/fp64 kind).  PAPER.md:87 (Eq. 13),
+// :110 (step 2); iteration and stopping rule: DESIGN.md readings A9, A11.
+#include "sign_state.cuh"
+
+namespace sm {
+
+constexpr int ST = 64;    // output tile edge
+constexpr int SK = 16;    // k step
+constexpr int SPAD = 4;
+
+// PHASE 1: Y = X X, partial ||Y - I||_F^2.   PHASE 2: X' = 1.5 X - 0.5 X Y.
+template <typename T, int PHASE>
+__global__ void __launch_bounds__(256)
+k_simt_gemm(const int32_t *__restrict__ cols, const int64_t *__restrict__ col_off,
+            const int32_t *__restrict__ dim, const int32_t *__restrict__ dim_pad, int32_t max_tiles_edge,
+            const T *__restrict__ Xsrc, const T *__restrict__ Ybuf, T *__restrict__ Out, SignState s) {
+  const int32_t tiles_per = max_tiles_edge * max_tiles_edge;
+  const int32_t c = blockIdx.x / tiles_per, t = blockIdx.x - c * tiles_per;
+  if (!s.active[c]) return;
+  if (PHASE == 1 && s.last[c]) return;
+  const int32_t i = cols ? cols[c] : c;
+  const int32_t m = dim[i], Pd = dim_pad[i];
+  const int32_t te = (m + ST - 1) / ST;
+  const int32_t tr = t / max_tiles_edge, tc = t - tr * max_tiles_edge;
+  if (tr >= te || tc >= te) return;
+  const T *A = Xsrc + col_off[c];
+  const T *B = (PHASE == 1 ? Xsrc : Ybuf) + col_off[c];
+  T *O = Out + col_off[c];
+
+  __shared__ T As[SK][ST + SPAD];
+  __shared__ T Bs[SK][ST + SPAD];
+  const int32_t tx = threadIdx.x & 15, ty = threadIdx.x >> 4;
+  const int32_t row0 = tr * ST, col0 = tc * ST;
+  T acc[4][4];
+#pragma unroll
+  for (int a = 0; a < 4; ++a)
+#pragma unroll
+    for (int b = 0; b < 4; ++b) acc[a][b] = (T)0;
+
+  for (int32_t k0 = 0; k0 < m; k0 += SK) {
+    // A tile: 64 rows x 16 k (row-major source: k contiguous)
+#pragma unroll
+    for (int l = 0; l < 4; ++l) {
+      int32_t e = threadIdx.x + l * 256;
+      int32_t r = e >> 4, k = e & 15;
+      int32_t gr = row0 + r, gk = k0 + k;
+      As[k][r] = (gr < m && gk < m) ? A[(int64_t)gr * Pd + gk] : (T)0;
+    }
+    // B tile: 16 k x 64 cols (column contiguous)
+#pragma unroll
+    for (int l = 0; l < 4; ++l) {
+      int32_t e = threadIdx.x + l * 256;
+      int32_t k = e >> 6, cc = e & 63;
+      int32_t gk = k0 + k, gc = col0 + cc;
+      Bs[k][cc] = (gk < m && gc < m) ? B[(int64_t)gk * Pd + gc] : (T)0;
+    }
+    __syncthreads();
+#pragma unroll
+    for (int k = 0; k < SK; ++k) {
+      T a[4], b[4];
+#pragma unroll
+      for (int q = 0; q < 4; ++q) { a[q] = As[k][ty * 4 + q]; b[q] = Bs[k][tx * 4 + q]; }
+#pragma unroll
+      for (int q = 0; q < 4; ++q)
+#pragma unroll
+        for (int p = 0; p < 4; ++p) acc[q][p] += a[q] * b[p];
+    }
+    __syncthreads();
+  }
+
+  double res = 0.0;
+#pragma unroll
+  for (int q = 0; q < 4; ++q) {
+    int32_t gr = row0 + ty * 4 + q;
+#pragma unroll
+    for (int p = 0; p < 4; ++p) {
+      int32_t gc = col0 + tx * 4 + p;
+      if (gr < m && gc < m) {
+        if (PHASE == 1) {
+          O[(int64_t)gr * Pd + gc] = acc[q][p];
+          double d = (double)acc[q][p] - (gr == gc ? 1.0 : 0.0);
+          res += d * d;
+        } else {
+          T x = A[(int64_t)gr * Pd + gc];
+          O[(int64_t)gr * Pd + gc] = (T)1.5 * x - (T)0.5 * acc[q][p];
+        }
+      }
+    }
+  }
+  if (PHASE == 1) {
+    // fixed-order CTA reduction: warp shuffles, then 8 warp sums in order
+    __shared__ double red[8];
+    for (int d = 16; d > 0; d >>= 1) res += __shfl_xor_sync(0xffffffffu, res, d);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = res;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      double sum = 0.0;
+      for (int w = 0; w < 8; ++w) sum += red[w];
+      s.partial[(int64_t)c * s.parts_per_col + tr * te + tc] = sum;
+    }
+  }
+}
+
+static __global__ void k_simt_nparts(int32_t n_cols, const int32_t *__restrict__ cols,
+                                     const int32_t *__restrict__ dim, int32_t *__restrict__ n_parts) {
+  int32_t c = blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= n_cols) return;
+  int32_t te = (dim[cols ? cols[c] : c] + ST - 1) / ST;
+  n_parts[c] = te * te;
+}
+
+struct SimtWs {
+  void *Y, *X2; int32_t *active, *last, *n_still, *n_parts; double *partial; int32_t parts_per_col;
+  int64_t used;
+};
+
+static SimtWs simt_layout(void *ws, int64_t ws_bytes, const sm_pattern_t *P, int32_t n_cols,
+                          int64_t packed_elems, int32_t eb) {
+  WsCursor cur(ws, ws_bytes);
+  SimtWs w;
+  int32_t edge = (P->max_dim + ST - 1) / ST;
+  w.parts_per_col = edge * edge;
+  w.Y = cur.take<char>(packed_elems * eb);
+  w.X2 = cur.take<char>(packed_elems * eb);
+  w.active = cur.take<int32_t>(n_cols);
+  w.last = cur.take<int32_t>(n_cols);
+  w.n_still = cur.take<int32_t>(1);
+  w.n_parts = cur.take<int32_t>(n_cols);
+  w.partial = cur.take<double>((int64_t)n_cols * w.parts_per_col);
+  w.used = cur.used + 256;
+  return w;
+}
+
+int64_t sign_simt_ws_bytes(const sm_pattern_t *P, int32_t n_cols, int64_t packed_elems, int32_t x_dtype) {
+  return simt_layout(nullptr, 0, P, n_cols, packed_elems, dtype_bytes(x_dtype)).used;
+}
+
+template <typename T>
+static int32_t sign_simt_t(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, const int64_t *col_off,
+                           int64_t packed_elems, T *X, void *ws, int64_t ws_bytes, int32_t max_iter,
+                           double tol, int32_t *iters, double *residual, cudaStream_t st) {
+  if ((P->pad_to & 3) != 0) return SM_ERR_ARG;   // 16-byte alignment of every submatrix
+  SimtWs w = simt_layout(ws, ws_bytes, P, n_cols, packed_elems, (int32_t)sizeof(T));
+  if (w.used > ws_bytes) return SM_ERR_SPACE;
+  SignState s{w.active, w.last, w.n_still, w.partial, w.parts_per_col};
+  const int32_t edge = (P->max_dim + ST - 1) / ST;
+  const int64_t grid64 = (int64_t)n_cols * edge * edge;
+  if (grid64 > 0x7fffffffLL) return SM_ERR_UNSUPPORTED;
+  const int32_t grid = (int32_t)grid64, nb = (n_cols + 255) / 256;
+  k_sign_init<<<nb, 256, 0, st>>>(n_cols, w.active, w.last, iters, residual);
+  SM_LAUNCHED();
+  k_simt_nparts<<<nb, 256, 0, st>>>(n_cols, cols, P->dim, w.n_parts);
+  SM_LAUNCHED();
+  T *buf[2] = {X, (T *)w.X2};
+  T *Y = (T *)w.Y;
+  for (int32_t k = 0; k < max_iter; ++k) {
+    T *src = buf[k & 1], *dst = buf[(k + 1) & 1];
+    k_simt_gemm<T, 1><<<grid, 256, 0, st>>>(cols, col_off, P->dim, P->dim_pad, edge, src, Y, Y, s);
+    SM_LAUNCHED();
+    SM_CUDA(cudaMemsetAsync(w.n_still, 0, sizeof(int32_t), st));
+    k_sign_post<<<nb, 256, 0, st>>>(n_cols, cols, P->dim, s, w.n_parts, tol, iters, residual);
+    SM_LAUNCHED();
+    k_simt_gemm<T, 2><<<grid, 256, 0, st>>>(cols, col_off, P->dim, P->dim_pad, edge, src, Y, dst, s);
+    SM_LAUNCHED();
+    if (tol > 0.0 && k >= 5 && (k & 1)) {
+      // convergence mode: read back how many submatrices continue (the only host sync of the path)
+      int32_t still = 1;
+      SM_CUDA(cudaMemcpyAsync(&still, w.n_still, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+      SM_CUDA(cudaStreamSynchronize(st));
+      if (still == 0) break;
+    }
+  }
+  dim3 cg(n_cols, 8);
+  k_copy_back<<<cg, 256, 0, st>>>(cols, col_off, iters, (int32_t)sizeof(T), (const char *)w.X2, (char *)X);
+  SM_LAUNCHED();
+  return SM_OK;
+}
+
+int32_t sign_simt(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, const int64_t *col_off,
+                  int64_t packed_elems, int32_t x_dtype, void *X, void *ws, int64_t ws_bytes,
+                  int32_t max_iter, double tol, int32_t *iters, double *residual, cudaStream_t st) {
+  if (x_dtype == SM_F64)
+    return sign_simt_t<double>(P, cols, n_cols, col_off, packed_elems, (double *)X, ws, ws_bytes, max_iter,
+                               tol, iters, residual, st);
+  if (x_dtype == SM_F32)
+    return sign_simt_t<float>(P, cols, n_cols, col_off, packed_elems, (float *)X, ws, ws_bytes, max_iter,
+                              tol, iters, residual, st);
+  return SM_ERR_UNSUPPORTED;
+}
+
+}  // namespace sm

@@ -1,0 +1,401 @@
+// a3, bf16 / fp16 back end: Newton-Schulz X <- 1/2 X (3I - X^2) as grouped tcgen05 GEMMs over ragged
+// submatrices ("FP16 operations with FP32 accumulation"; "evaluation of the matrix
+// function on many dense ... matrices", PAPER.md:106/:110 step 2; Eq. 13).
+//
+// Data layout: every submatrix is stored in HBM as the K-major 128B-swizzled UMMA shared-memory
+// image (include/submatrix.h), so an operand tile (rows x 64 k) is ONE contiguous bulk-TMA copy and
+// no tensor map is needed for ragged sizes.  X is symmetric, so the same image serves as the A
+// operand (rows of X) and as the B operand (B[n][k] = X[k][n] = X[n][k]): both products are
+// "A K-major, B K-major" and read row panels only.
+//
+// Symmetry is enforced exactly: only elements (r, c) with r >= c are taken from the accumulator and
+// each is stored twice, at (r, c) and mirrored at (c, r); tiles that lie entirely above the diagonal
+// are never computed.  This is required, not just cheaper: with rounded iterates the X X^T form
+// amplifies any antisymmetric perturbation by ~2x per step (measured: NaN after ~18 bf16 steps),
+// while exactly symmetric iterates make X X^T == X^2 and keep the iteration on Eq. 13's fixed point.
+//
+// Kernel: persistent, one CTA per SM, 192 threads = 1 TMA producer warp, 1 MMA issuer warp (also
+// owns TMEM), 4 epilogue warps.  Tile = 128 x (<=256) fp32 accumulator in TMEM, double buffered
+// (2 x 256 columns) so the epilogue of tile t overlaps the main loop of tile t+1; 4-stage smem ring.
+//   PHASE 1: Y = X X^T, epilogue writes Y and the fused ||Y - I||_F^2 partial sums (warp shuffles).
+//   PHASE 2: X' = 1.5 X - 0.5 X Y^T, epilogue reads the X tile and writes X'.
+#include "sign_state.cuh"
+#include "umma_ptx.cuh"
+
+namespace sm {
+
+constexpr int UM = 128;          // tile rows  (UMMA M)
+constexpr int UN = 256;          // max tile cols (UMMA N)
+constexpr int UK = 64;           // k chunk = one 128-byte swizzle row of 16-bit elements
+constexpr int USTAGES = 4;
+constexpr int A_BYTES = UM * UK * 2;           // 16 KB
+constexpr int B_BYTES = UN * UK * 2;           // 32 KB
+constexpr int STAGE_BYTES = A_BYTES + B_BYTES; // 48 KB
+constexpr int UMMA_SMEM = USTAGES * STAGE_BYTES + 1024 /*align slack*/ + 256 /*barriers*/;
+constexpr int UMMA_THREADS = 192;
+constexpr uint32_t TMEM_COLS = 512;
+
+struct UTile {
+  int32_t c, m, Pd, row0, n0, nt, kmax, tm, tn, Tn, lt, valid;
+  int64_t base;   // element offset of the submatrix in the packed buffer
+};
+
+struct UArgs {
+  const int32_t *cols; const int64_t *col_off; const int32_t *dim; const int32_t *dim_pad;
+  const int64_t *tile_ptr;   // [n_cols+1] exclusive scan of tiles per listed column
+  int32_t n_cols;
+  const void *Xsrc; const void *Ybuf; void *Out;
+  SignState s;
+  int32_t *err_flag;
+};
+
+__host__ __device__ inline int32_t u_n16(int32_t m) { return (m + 15) & ~15; }
+__host__ __device__ inline int32_t u_Tn(int32_t m) { return (u_n16(m) + UN - 1) / UN; }
+__host__ __device__ inline int32_t u_Tm(int32_t m) { return (m + UM - 1) / UM; }
+__host__ __device__ inline int32_t u_nbase(int32_t m) {
+  int32_t Tn = u_Tn(m);
+  return ((u_n16(m) / 16 + Tn - 1) / Tn) * 16;
+}
+
+// Tiles of one submatrix that touch the lower triangle: for tile row tm the tile columns tn with
+// n0 = tn * nbase <= row0 + UM - 1.
+__host__ __device__ inline int32_t u_row_tiles(int32_t m, int32_t tm) {
+  int32_t cnt = (tm * UM + UM - 1) / u_nbase(m) + 1;
+  int32_t Tn = u_Tn(m);
+  return cnt < Tn ? cnt : Tn;
+}
+__host__ __device__ inline int32_t u_tiles(int32_t m) {
+  int32_t t = 0;
+  for (int32_t tm = 0; tm < u_Tm(m); ++tm) t += u_row_tiles(m, tm);
+  return t;
+}
+
+template <int PHASE>
+__device__ __forceinline__ UTile decode_tile(const UArgs &a, int64_t t) {
+  UTile u;
+  u.c = upper_slot<int64_t>(a.tile_ptr, a.n_cols, t);
+  int32_t local = (int32_t)(t - a.tile_ptr[u.c]);
+  int32_t i = a.cols ? a.cols[u.c] : u.c;
+  u.m = a.dim[i]; u.Pd = a.dim_pad[i];
+  u.base = a.col_off[u.c];
+  u.Tn = u_Tn(u.m);
+  int32_t nb = u_nbase(u.m), n16 = u_n16(u.m);
+  u.tm = 0; u.lt = local;
+  for (;;) {
+    int32_t cnt = u_row_tiles(u.m, u.tm);
+    if (local < cnt) break;
+    local -= cnt; ++u.tm;
+  }
+  u.tn = local;
+  u.row0 = u.tm * UM;
+  u.n0 = u.tn * nb;
+  u.nt = min(nb, n16 - u.n0);
+  u.kmax = n16;
+  int32_t act = a.s.active[u.c];
+  if (PHASE == 1) act = act && !a.s.last[u.c];
+  u.valid = act;
+  return u;
+}
+
+template <bool BF16> __device__ __forceinline__ uint32_t pack2(float lo, float hi);
+template <> __device__ __forceinline__ uint32_t pack2<true>(float lo, float hi) {
+  __nv_bfloat162 v = __floats2bfloat162_rn(lo, hi);
+  return *reinterpret_cast<uint32_t *>(&v);
+}
+template <> __device__ __forceinline__ uint32_t pack2<false>(float lo, float hi) {
+  __half2 v = __floats2half2_rn(lo, hi);
+  return *reinterpret_cast<uint32_t *>(&v);
+}
+template <bool BF16> __device__ __forceinline__ float2 unpack2(uint32_t w);
+template <> __device__ __forceinline__ float2 unpack2<true>(uint32_t w) {
+  return __bfloat1622float2(*reinterpret_cast<__nv_bfloat162 *>(&w));
+}
+template <> __device__ __forceinline__ float2 unpack2<false>(uint32_t w) {
+  return __half22float2(*reinterpret_cast<__half2 *>(&w));
+}
+
+template <bool BF16, int PHASE>
+__global__ void __launch_bounds__(UMMA_THREADS, 1) k_umma_gemm(UArgs a) {
+  extern __shared__ uint8_t smem_raw[];
+  const uint32_t raw = ptx::smem_u32(smem_raw);
+  const uint32_t tiles = (raw + 1023u) & ~1023u;           // 1024-byte aligned operand ring
+  const uint32_t bars = tiles + USTAGES * STAGE_BYTES;     // barriers behind the ring
+  // barrier slots (8 bytes each): full[4], empty[4], tmem_full[2], tmem_empty[2]; then tmem base
+  auto full_bar = [&](int s) { return bars + 8u * s; };
+  auto empty_bar = [&](int s) { return bars + 8u * (USTAGES + s); };
+  auto tfull_bar = [&](int s) { return bars + 8u * (2 * USTAGES + s); };
+  auto tempty_bar = [&](int s) { return bars + 8u * (2 * USTAGES + 2 + s); };
+  const uint32_t tmem_slot = bars + 8u * (2 * USTAGES + 4);
+  volatile uint32_t *tmem_slot_ptr =
+      reinterpret_cast<volatile uint32_t *>(smem_raw + (tmem_slot - raw));
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < USTAGES; ++s) { ptx::mbar_init(full_bar(s), 1); ptx::mbar_init(empty_bar(s), 1); }
+    for (int s = 0; s < 2; ++s) { ptx::mbar_init(tfull_bar(s), 1); ptx::mbar_init(tempty_bar(s), 4); }
+    ptx::fence_barrier_init();
+    ptx::fence_proxy_async();
+  }
+  if (warp == 1) {
+    ptx::tmem_alloc(tmem_slot, TMEM_COLS);
+    ptx::tmem_relinquish();
+  }
+  ptx::tc_fence_before();
+  __syncthreads();
+  ptx::tc_fence_after();
+  const uint32_t tmem_base = *tmem_slot_ptr;
+
+  const int64_t total = a.tile_ptr[a.n_cols];
+  constexpr int ESZ = 2;
+
+  if (warp == 0) {
+    // ===================== TMA producer =====================
+    if (lane == 0) {
+      int stage = 0; uint32_t phase = 0;
+      for (int64_t t = blockIdx.x; t < total; t += gridDim.x) {
+        UTile u = decode_tile<PHASE>(a, t);
+        if (!u.valid) continue;
+        const char *Ag = (const char *)a.Xsrc + u.base * ESZ;
+        const char *Bg = (const char *)(PHASE == 1 ? a.Xsrc : a.Ybuf) + u.base * ESZ;
+        const uint32_t a_rows = (uint32_t)min(UM, u.Pd - u.row0);
+        const uint32_t a_bytes = a_rows * 128u, b_bytes = (uint32_t)u.nt * 128u;
+        const int nkc = (u.kmax + UK - 1) / UK;
+        for (int kc = 0; kc < nkc; ++kc) {
+          ptx::mbar_wait(empty_bar(stage), phase ^ 1u, a.err_flag, 1);
+          const uint32_t sa = tiles + stage * STAGE_BYTES, sb = sa + A_BYTES;
+          ptx::mbar_expect_tx(full_bar(stage), a_bytes + b_bytes);
+          const int64_t chunk = (int64_t)kc * u.Pd * 128;     // byte offset of k chunk kc
+          ptx::tma_bulk_g2s(sa, Ag + chunk + (int64_t)u.row0 * 128, a_bytes, full_bar(stage));
+          ptx::tma_bulk_g2s(sb, Bg + chunk + (int64_t)u.n0 * 128, b_bytes, full_bar(stage));
+          if (++stage == USTAGES) { stage = 0; phase ^= 1u; }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ===================== MMA issuer =====================
+    if (lane == 0) {
+      int stage = 0; uint32_t phase = 0;
+      uint32_t it = 0;
+      for (int64_t t = blockIdx.x; t < total; t += gridDim.x) {
+        UTile u = decode_tile<PHASE>(a, t);
+        if (!u.valid) continue;
+        const uint32_t as = it & 1u, aphase = (it >> 1) & 1u;
+        ptx::mbar_wait(tempty_bar(as), aphase ^ 1u, a.err_flag, 2);
+        ptx::tc_fence_after();
+        const uint32_t d_tmem = tmem_base + as * UN;
+        const uint32_t idesc = ptx::make_idesc_f16(BF16, UM, (uint32_t)u.nt);
+        const int nkc = (u.kmax + UK - 1) / UK;
+        for (int kc = 0; kc < nkc; ++kc) {
+          ptx::mbar_wait(full_bar(stage), phase, a.err_flag, 3);
+          ptx::tc_fence_after();
+          const uint32_t sa = tiles + stage * STAGE_BYTES, sb = sa + A_BYTES;
+          const uint64_t adesc = ptx::make_sw128_kmajor_desc(sa);
+          const uint64_t bdesc = ptx::make_sw128_kmajor_desc(sb);
+          const int ksteps = min(UK / 16, (u.kmax - kc * UK) / 16);
+          for (int ks = 0; ks < ksteps; ++ks) {
+            // advance 16 elements = 32 bytes inside the swizzle atom: +2 in the (addr >> 4) field
+            ptx::umma_f16(d_tmem, adesc + (uint64_t)(2 * ks), bdesc + (uint64_t)(2 * ks), idesc,
+                          (uint32_t)((kc | ks) != 0));
+          }
+          ptx::umma_commit(empty_bar(stage));      // frees the smem slot when these MMAs finish
+          if (++stage == USTAGES) { stage = 0; phase ^= 1u; }
+        }
+        ptx::umma_commit(tfull_bar(as));           // accumulator ready for the epilogue
+        ++it;
+      }
+    }
+  } else {
+    // ===================== epilogue (warps 2..5) =====================
+    const int q = warp & 3;                        // TMEM lane quadrant this warp may access
+    uint32_t it = 0;
+    for (int64_t t = blockIdx.x; t < total; t += gridDim.x) {
+      UTile u = decode_tile<PHASE>(a, t);
+      if (!u.valid) continue;
+      const uint32_t as = it & 1u, aphase = (it >> 1) & 1u;
+      ptx::mbar_wait(tfull_bar(as), aphase, a.err_flag, 4);
+      ptx::tc_fence_after();
+      const int32_t r = u.row0 + q * 32 + lane;
+      const bool row_ok = r < u.m;
+      const uint32_t taddr = tmem_base + as * UN + ((uint32_t)(q * 32) << 16);
+      uint16_t *Og = (uint16_t *)a.Out + u.base;
+      const uint16_t *Xg = (const uint16_t *)a.Xsrc + u.base;
+      float res = 0.f;
+      for (int g = 0; g < u.nt / 16; ++g) {
+        uint32_t v[16];
+        ptx::tmem_ld16(taddr + (uint32_t)(g * 16), v);
+        ptx::tmem_ld_wait();
+        if (row_ok) {
+          const int32_t c0 = u.n0 + g * 16;
+#pragma unroll
+          for (int h = 0; h < 2; ++h) {
+            const int32_t cc = c0 + h * 8;
+            if (cc > r) continue;                       // chunk entirely above the diagonal
+            const int64_t off = img_off(u.Pd, r, cc);
+            float f[8];
+#pragma unroll
+            for (int e = 0; e < 8; ++e) f[e] = __uint_as_float(v[h * 8 + e]);
+            if (PHASE == 1) {
+#pragma unroll
+              for (int e = 0; e < 8; ++e) {
+                const int32_t c = cc + e;
+                if (c <= r && c < u.m) {
+                  // off-diagonal elements stand for (r,c) and (c,r)
+                  float d = f[e] - (c == r ? 1.f : 0.f);
+                  res = fmaf(c == r ? d : 2.f * d, d, res);
+                }
+              }
+            } else {
+              uint4 xo = *reinterpret_cast<const uint4 *>(Xg + off);
+              float2 x0 = unpack2<BF16>(xo.x), x1 = unpack2<BF16>(xo.y), x2 = unpack2<BF16>(xo.z),
+                     x3 = unpack2<BF16>(xo.w);
+              f[0] = 1.5f * x0.x - 0.5f * f[0]; f[1] = 1.5f * x0.y - 0.5f * f[1];
+              f[2] = 1.5f * x1.x - 0.5f * f[2]; f[3] = 1.5f * x1.y - 0.5f * f[3];
+              f[4] = 1.5f * x2.x - 0.5f * f[4]; f[5] = 1.5f * x2.y - 0.5f * f[5];
+              f[6] = 1.5f * x3.x - 0.5f * f[6]; f[7] = 1.5f * x3.y - 0.5f * f[7];
+            }
+            uint4 o;
+            o.x = pack2<BF16>(f[0], f[1]); o.y = pack2<BF16>(f[2], f[3]);
+            o.z = pack2<BF16>(f[4], f[5]); o.w = pack2<BF16>(f[6], f[7]);
+            const uint16_t *ov = reinterpret_cast<const uint16_t *>(&o);
+            if (cc + 7 <= r) {
+              *reinterpret_cast<uint4 *>(Og + off) = o;  // whole chunk on or below the diagonal
+#pragma unroll
+              for (int e = 0; e < 8; ++e) Og[img_off(u.Pd, cc + e, r)] = ov[e];
+            } else {
+#pragma unroll
+              for (int e = 0; e < 8; ++e) {
+                const int32_t c = cc + e;
+                if (c <= r) {
+                  Og[off + e] = ov[e];
+                  if (c < r) Og[img_off(u.Pd, c, r)] = ov[e];
+                }
+              }
+            }
+          }
+        }
+      }
+      // accumulator drained: hand the TMEM stage back to the MMA warp
+      ptx::tc_fence_before();
+      __syncwarp();
+      if (lane == 0) ptx::mbar_arrive(tempty_bar(as));
+      if (PHASE == 1) {
+        for (int d = 16; d > 0; d >>= 1) res += __shfl_xor_sync(0xffffffffu, res, d);
+        if (lane == 0)
+          a.s.partial[(int64_t)u.c * a.s.parts_per_col + (int64_t)u.lt * 4 + q] = (double)res;
+      }
+      ++it;
+    }
+  }
+
+  ptx::tc_fence_before();
+  __syncthreads();
+  if (warp == 1) {
+    ptx::tc_fence_after();
+    ptx::tmem_dealloc(tmem_base, TMEM_COLS);
+  }
+}
+
+}  // namespace sm
+
+namespace sm {
+
+static __global__ void k_umma_tilecounts(int32_t n_cols, const int32_t *__restrict__ cols,
+                                         const int32_t *__restrict__ dim, int64_t *__restrict__ tiles,
+                                         int32_t *__restrict__ n_parts) {
+  int32_t c = blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= n_cols) return;
+  int32_t m = dim[cols ? cols[c] : c];
+  int32_t nt = u_tiles(m);
+  tiles[c] = nt;
+  n_parts[c] = nt * 4;
+}
+
+struct UmmaWs {
+  void *Y, *X2; int32_t *active, *last, *n_still, *n_parts, *err; int64_t *tile_ptr; double *partial;
+  int32_t parts_per_col; int64_t used;
+};
+
+static UmmaWs umma_layout(void *ws, int64_t ws_bytes, const sm_pattern_t *P, int32_t n_cols,
+                          int64_t packed_elems) {
+  WsCursor cur(ws, ws_bytes);
+  UmmaWs w;
+  w.parts_per_col = u_Tm(P->max_dim) * u_Tn(P->max_dim) * 4;
+  w.Y = cur.take<char>(packed_elems * 2);
+  w.X2 = cur.take<char>(packed_elems * 2);
+  w.active = cur.take<int32_t>(n_cols);
+  w.last = cur.take<int32_t>(n_cols);
+  w.n_still = cur.take<int32_t>(1);
+  w.err = cur.take<int32_t>(1);
+  w.n_parts = cur.take<int32_t>(n_cols);
+  w.tile_ptr = cur.take<int64_t>(n_cols + 1);
+  w.partial = cur.take<double>((int64_t)n_cols * w.parts_per_col);
+  w.used = cur.used + 256;
+  return w;
+}
+
+int64_t sign_umma_ws_bytes(const sm_pattern_t *P, int32_t n_cols, int64_t packed_elems, int32_t x_dtype) {
+  (void)x_dtype;
+  return umma_layout(nullptr, 0, P, n_cols, packed_elems).used;
+}
+
+template <bool BF16, int PHASE>
+static int32_t launch_umma(const UArgs &a, int32_t grid, cudaStream_t st) {
+  static bool configured = false;
+  if (!configured) {
+    SM_CUDA(cudaFuncSetAttribute(k_umma_gemm<BF16, PHASE>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 UMMA_SMEM));
+    configured = true;
+  }
+  k_umma_gemm<BF16, PHASE><<<grid, UMMA_THREADS, UMMA_SMEM, st>>>(a);
+  SM_LAUNCHED();
+  return SM_OK;
+}
+
+int32_t sign_umma(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, const int64_t *col_off,
+                  int64_t packed_elems, int32_t x_dtype, void *X, void *ws, int64_t ws_bytes,
+                  int32_t max_iter, double tol, int32_t *iters, double *residual, cudaStream_t st) {
+  if ((P->pad_to % 64) != 0) return SM_ERR_ARG;
+  const bool bf16 = x_dtype == SM_BF16;
+  UmmaWs w = umma_layout(ws, ws_bytes, P, n_cols, packed_elems);
+  if (w.used > ws_bytes) return SM_ERR_SPACE;
+  int dev = 0, n_sm = 0;
+  SM_CUDA(cudaGetDevice(&dev));
+  SM_CUDA(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
+  SignState s{w.active, w.last, w.n_still, w.partial, w.parts_per_col};
+  const int32_t nb = (n_cols + 255) / 256;
+  k_sign_init<<<nb, 256, 0, st>>>(n_cols, w.active, w.last, iters, residual);
+  SM_LAUNCHED();
+  k_umma_tilecounts<<<nb, 256, 0, st>>>(n_cols, cols, P->dim, w.tile_ptr, w.n_parts);
+  SM_LAUNCHED();
+  { int32_t rc = exclusive_scan_i64(n_cols, w.tile_ptr, w.tile_ptr, st); if (rc != SM_OK) return rc; }
+  // Y and the alternate X buffer start as zeros so that padding never holds NaN/Inf bit patterns.
+  SM_CUDA(cudaMemsetAsync(w.Y, 0, packed_elems * 2, st));
+  SM_CUDA(cudaMemsetAsync(w.X2, 0, packed_elems * 2, st));
+  SM_CUDA(cudaMemsetAsync(w.err, 0, sizeof(int32_t), st));
+  void *buf[2] = {X, w.X2};
+  for (int32_t k = 0; k < max_iter; ++k) {
+    void *src = buf[k & 1], *dst = buf[(k + 1) & 1];
+    UArgs a{cols, col_off, P->dim, P->dim_pad, w.tile_ptr, n_cols, src, w.Y, w.Y, s, w.err};
+    int32_t rc = bf16 ? launch_umma<true, 1>(a, n_sm, st) : launch_umma<false, 1>(a, n_sm, st);
+    if (rc != SM_OK) return rc;
+    SM_CUDA(cudaMemsetAsync(w.n_still, 0, sizeof(int32_t), st));
+    k_sign_post<<<nb, 256, 0, st>>>(n_cols, cols, P->dim, s, w.n_parts, tol, iters, residual);
+    SM_LAUNCHED();
+    a.Out = dst;
+    rc = bf16 ? launch_umma<true, 2>(a, n_sm, st) : launch_umma<false, 2>(a, n_sm, st);
+    if (rc != SM_OK) return rc;
+    if (tol > 0.0 && k >= 5 && (k & 1)) {
+      int32_t still = 1;
+      SM_CUDA(cudaMemcpyAsync(&still, w.n_still, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+      SM_CUDA(cudaStreamSynchronize(st));
+      if (still == 0) break;
+    }
+  }
+  dim3 cg(n_cols, 8);
+  k_copy_back<<<cg, 256, 0, st>>>(cols, col_off, iters, 2, (const char *)w.X2, (char *)X);
+  SM_LAUNCHED();
+  return SM_OK;
+}
+
+}  // namespace sm
