@@ -190,6 +190,13 @@ int32_t sm_density_from_sign(const sm_bcsr_t *A, const sm_pattern_t *P, int32_t 
 /* Number of kernels this thread's library calls have launched so far (bench bookkeeping). host. */
 int64_t sm_launch_count(void);
 
+/* Measurement hooks (host).  While enabled, every launch of the tensor-core Newton-Schulz kernel
+ * (the dominant kernel of a3 for SM_BF16/SM_F16) is bracketed by CUDA events on its stream.
+ * sm_profile_read synchronises on those events, returns their summed duration in ms and the number
+ * of launches covered, and resets the counters.  Not thread-safe; leave disabled in production. */
+int32_t sm_profile_enable(int32_t on);
+int32_t sm_profile_read(double *gemm_ms /*host*/, int64_t *gemm_launches /*host*/);
+
 #ifdef __cplusplus
 }
 #endif

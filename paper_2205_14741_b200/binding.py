@@ -32,7 +32,7 @@ SCALES = {"none": SM_SCALE_NONE, "gershgorin": SM_SCALE_GERSHGORIN, "power": SM_
 EXPORTS = ["sm_last_cuda_error", "sm_pattern_sizes", "sm_build_pattern", "sm_plan_columns",
            "sm_gather_ws_bytes", "sm_gather", "sm_sign_ws_bytes", "sm_sign_ns", "sm_sign_status",
            "sm_scatter", "sm_symmetrise", "sm_density_ws_bytes", "sm_density", "sm_density_from_sign",
-           "sm_launch_count"]
+           "sm_launch_count", "sm_profile_enable", "sm_profile_read"]
 
 
 class SmError(RuntimeError):
@@ -83,6 +83,17 @@ def _check(fn, status, allow_warn=False):
 
 def launch_count() -> int:
     return int(_lib.sm_launch_count())
+
+
+def profile_enable(on: bool) -> None:
+    _check("sm_profile_enable", _lib.sm_profile_enable(C.c_int32(1 if on else 0)))
+
+
+def profile_read():
+    """(summed duration in ms, number of launches) of the tensor-core NS kernel since enable/read."""
+    ms, n = C.c_double(0.0), C.c_int64(0)
+    _check("sm_profile_read", _lib.sm_profile_read(C.byref(ms), C.byref(n)))
+    return ms.value, int(n.value)
 
 
 class Bcsr:
