@@ -183,7 +183,8 @@ def run_ours(args, cfg, cfg_run):
 
     # Weak scaling: every rank owns an independent replica of the workload (independent problems,
     # PAPER.md:106 "large-scale parallel evaluation"); no data-path collective.
-    wl = make_config(args.config, seed=cfg["seed"] + 100 * rank)
+    from paper_2205_14741_b200 import dist_util
+    wl = make_config(args.config, seed=dist_util.rank_seed(cfg["seed"], rank))
     dims, sum_m3 = workload_stats(wl)
     A = sm.Bcsr(wl)
     P = sm.sm_build_pattern(A, pad)
@@ -224,12 +225,7 @@ def run_ours(args, cfg, cfg_run):
     k_eff = plan.iters.double().cpu().numpy()
     order = P.order.cpu().numpy()
     flops_step = 4.0 * float(((dims[order] ** 3) * k_eff).sum())    # per-column updates actually applied
-    t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
-    fl = torch.tensor([flops_step], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        dist.all_reduce(fl, op=dist.ReduceOp.SUM)
-    ms_total_max, flops_all = float(t.item()), float(fl.item())
+    ms_total_max, flops_all = dist_util.aggregate(ms_total, flops_step, torch.device("cuda", local))
     ms_per_step = ms_total_max / args.steps
     value = flops_all / (ms_per_step * 1e-3) / 1e12
 
@@ -283,10 +279,7 @@ def run_ours(args, cfg, cfg_run):
             e2e_step()
         b.record()
         torch.cuda.synchronize()
-        te = torch.tensor([a.elapsed_time(b)], dtype=torch.float64, device="cuda")
-        if world > 1:
-            dist.all_reduce(te, op=dist.ReduceOp.MAX)
-        e2e_ms = float(te.item()) / args.steps
+        e2e_ms = dist_util.aggregate(a.elapsed_time(b), 0.0, torch.device("cuda", local))[0] / args.steps
         h2d = int(h_vals.numel() * 8 + sum(x.numel() * x.element_size() for x in h_idx))
         d2h = int(h_D.numel() * 8 + 8)
         e2e = {"value": flops_all / (e2e_ms * 1e-3) / 1e12, "unit": UNIT, "ms_per_step": e2e_ms,

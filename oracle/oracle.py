@@ -187,3 +187,44 @@ def column_mask(w, cols) -> np.ndarray:
     blk_sel = sel[np.asarray(w.col_idx)]
     sizes = np.diff(np.asarray(w.val_ptr))
     return np.repeat(blk_sel, sizes)
+
+
+def density_columns_lapack(w, mu: float = 0.0, cols=None, mode: str = "exact", k_fixed: int = 0, scale=None):
+    """Same result as density_columns, with LAPACK's symmetric eigensolver (numpy.linalg.eigh, a
+    library primitive used as one step) in place of the Jacobi sweeps.  For the large submatrices
+    of configs[4] (m ~ 1650), where cyclic Jacobi needs ~10 min per submatrix.  Pinned to the Jacobi
+    path in tests/test_oracle_pins.py.  Steps: PAPER.md:110 (gather, f, insert columns), Eq. 13 on
+    the spectrum, Eq. 14 with S = I."""
+    blk = np.asarray(w.blk_size)
+    vp = np.asarray(w.val_ptr, dtype=np.int64)
+    d = np.zeros(int(vp[-1]))
+    col_list = list(range(w.n_blk)) if cols is None else [int(c) for c in cols]
+    st = SimpleNamespace(min_abs_eig=np.zeros(len(col_list)), scale=np.zeros(len(col_list)),
+                         n_neg=np.zeros(len(col_list), np.int32))
+    for ci, i in enumerate(col_list):
+        T = gather(w, i, mu)
+        m = T.shape[0]
+        gs = float(np.abs(T).sum(axis=1).max())
+        lam, V = np.linalg.eigh(T)
+        if mode == "exact":
+            f = np.sign(lam)
+        else:
+            x = lam / (gs if scale is None else float(scale[ci]))
+            for _ in range(k_fixed):
+                x = 0.5 * x * (3.0 - x * x)
+            f = x
+        S = (V * f) @ V.T
+        nb = np.asarray(w.col_idx[w.row_ptr[i]:w.row_ptr[i + 1]])
+        offs = np.concatenate([[0], np.cumsum(blk[nb])])
+        own = int(np.where(nb == i)[0][0])
+        bi = int(blk[i])
+        for a, j in enumerate(nb):
+            row = w.col_idx[w.row_ptr[j]:w.row_ptr[j + 1]]
+            p = int(w.row_ptr[j]) + int(np.searchsorted(row, i))
+            blk_s = S[offs[a]:offs[a + 1], offs[own]:offs[own + 1]]
+            ident = np.eye(bi) if a == own else 0.0
+            d[vp[p]:vp[p + 1]] = (0.5 * (ident - blk_s)).ravel()
+        st.min_abs_eig[ci] = np.abs(lam).min()
+        st.scale[ci] = gs
+        st.n_neg[ci] = int((lam < 0).sum())
+    return d, st

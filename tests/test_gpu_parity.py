@@ -1,0 +1,343 @@
+"""GPU parity: the CUDA path behind the C ABI against the CPU oracle, element by element, on the
+same seeded inputs.  Tolerances are BASELINE.json's: bit-exact integers; max-abs 1e-10 (fp64),
+1e-4 (fp32); relative Frobenius 2e-2 and |dTr D|/n 1e-3 (bf16/fp16).  DESIGN.md section 6."""
+import os
+
+import numpy as np
+import pytest
+
+from oracle import oracle as orc
+from workloads.generator import CONFIGS, Workload, make_config, make_workload, sample_columns
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+THREADS = os.cpu_count() or 4
+
+
+@pytest.fixture(scope="module")
+def sm():
+    import paper_2205_14741_b200.binding as b   # raises if libsubmatrix.so is missing: no fallback
+    return b
+
+
+def img_index(Pd):
+    """Element offsets of the K-major 128B-swizzled image (include/submatrix.h, packed buffers)."""
+    r = np.arange(Pd)[:, None]
+    c = np.arange(Pd)[None, :]
+    return (c >> 6) * Pd * 64 + r * 64 + ((((c & 63) >> 3) ^ (r & 7)) << 3) + (c & 7)
+
+
+def unpack(X, P_host, i, x_dtype, col_off=None, pos=None):
+    Pd = int(P_host.dim_pad[i])
+    lo = int(P_host.sub_off[i]) if col_off is None else int(col_off[pos])
+    buf = X[lo:lo + Pd * Pd].double().cpu().numpy()
+    return buf[img_index(Pd)] if x_dtype in ("bf16", "f16") else buf.reshape(Pd, Pd)
+
+
+def ragged_workload():
+    return make_workload(40, np.array([2, 3, 5, 4, 7] * 8), np.array([1, 1, 2, 2, 3] * 8), 5.5, seed=11)
+
+
+# ------------------------------------------------------------------ a1 pattern
+
+@pytest.mark.parametrize("maker,pad", [(lambda: make_config(0), 16), (lambda: make_config(1), 64),
+                                       (ragged_workload, 4), (lambda: make_config(0, cutoff=np.inf), 64)])
+def test_pattern_bit_exact(sm, maker, pad):
+    wl = maker()
+    A = sm.Bcsr(wl)
+    Ph = sm.pattern_to_host(sm.sm_build_pattern(A, pad))
+    Po = orc.build_pattern(wl, pad)
+    for k in sm.Pattern.INT32 + sm.Pattern.INT64:
+        ref = getattr(Po, k)
+        assert np.array_equal(getattr(Ph, k)[:len(ref)], ref), k
+
+
+def test_pattern_sizes_and_rejection(sm):
+    wl = make_config(0)
+    A = sm.Bcsr(wl)
+    sz = sm.sm_pattern_sizes(A, 16)
+    so = orc.pattern_sizes(wl, 16)
+    assert (sz.nbr_len, sz.gmap_len, sz.packed_elems, sz.max_dim, sz.max_dim_pad) == \
+        (so.nbr_len, so.gmap_len, so.packed_elems, so.max_dim, so.max_dim_pad)
+    # drop one off-diagonal block -> not structurally symmetric -> SM_ERR_PATTERN, as the oracle says
+    i = int(np.argmax(np.diff(wl.row_ptr) > 1))
+    p = wl.row_ptr[i] + (1 if wl.col_idx[wl.row_ptr[i]] == i else 0)
+    keep = np.ones(wl.nnzb, bool)
+    keep[p] = False
+    rp = wl.row_ptr.copy()
+    rp[i + 1:] -= 1
+    vp = np.concatenate([[0], np.cumsum(np.diff(wl.val_ptr)[keep])]).astype(np.int64)
+    bad = Workload(**{**wl.__dict__, "row_ptr": rp, "col_idx": wl.col_idx[keep], "val_ptr": vp,
+                      "vals": wl.vals[:vp[-1]]})
+    assert orc.check_pattern(bad) == -3
+    with pytest.raises(sm.SmError) as e:
+        sm.sm_pattern_sizes(sm.Bcsr(bad), 16)
+    assert e.value.status == sm.SM_ERR_PATTERN
+    with pytest.raises(sm.SmError) as e:
+        sm.sm_pattern_sizes(A, 0)
+    assert e.value.status == sm.SM_ERR_ARG
+
+
+# ------------------------------------------------------------------- a2 gather
+
+@pytest.mark.parametrize("maker", [lambda: make_config(0), ragged_workload])
+def test_gather_fp64_exact_and_padding_invisible(sm, maker):
+    wl = maker()
+    A = sm.Bcsr(wl)
+    for pad in (4, 16):
+        P = sm.sm_build_pattern(A, pad)
+        Ph = sm.pattern_to_host(P)
+        cols, col_off, n = sm.sm_plan_columns(P, None)
+        X, scale = sm.sm_gather(A, P, cols, col_off, n, 0.3, "none", "f64")
+        Xg, sg = sm.sm_gather(A, P, cols, col_off, n, 0.3, "gershgorin", "f64")
+        for i in range(wl.n_blk):
+            T = orc.gather(wl, i, 0.3)
+            m = T.shape[0]
+            x = unpack(X, Ph, i, "f64")
+            assert np.array_equal(x[:m, :m], T)                     # copy + shift: exact
+            assert not x[m:].any() and not x[:, m:].any()           # zero padding
+            s = orc.gershgorin(T)
+            assert abs(sg[i].item() - s) <= 4e-15 * s
+            assert np.abs(unpack(Xg, Ph, i, "f64")[:m, :m] * sg[i].item() - T).max() <= 1e-15 * s
+        assert (scale == 1.0).all()
+
+
+@pytest.mark.parametrize("x_dtype,eps", [("bf16", 2.0 ** -8), ("f16", 2.0 ** -11), ("f32", 2.0 ** -24)])
+def test_gather_low_precision_subset_in_listed_order(sm, x_dtype, eps):
+    wl = make_config(1)
+    A = sm.Bcsr(wl)
+    P = sm.sm_build_pattern(A, 64)
+    Ph = sm.pattern_to_host(P)
+    cols_h = np.array([977, 3, 500, 42], np.int32)
+    cols, col_off, n = sm.sm_plan_columns(P, cols_h)
+    X, scale = sm.sm_gather(A, P, cols, col_off, n, 0.0, "gershgorin", x_dtype)
+    off = col_off.cpu().numpy()
+    assert np.array_equal(off, np.concatenate([[0], np.cumsum(Ph.dim_pad[cols_h].astype(np.int64) ** 2)]))
+    for k, i in enumerate(cols_h):
+        T = orc.gather(wl, int(i))
+        m = T.shape[0]
+        x = unpack(X, Ph, int(i), x_dtype, off, k)
+        ref = T / orc.gershgorin(T)
+        assert np.abs(x[:m, :m] - ref).max() <= eps * 1.01     # one rounding of |x| <= 1
+        assert not x[m:].any() and not x[:, m:].any()
+
+
+# ---------------------------------------------------- a3 one Newton-Schulz step, all back ends
+
+@pytest.mark.parametrize("x_dtype,pad,tol_abs", [("f64", 16, 1e-14), ("f32", 16, 2e-6), ("bf16", 64, 8e-3),
+                                                  ("f16", 64, 1e-3)])
+def test_single_ns_step_matches_definition(sm, x_dtype, pad, tol_abs):
+    # X1 = 1/2 X0 (3I - X0^2) with X0 = T/s from the oracle; sizes span several tiles and ragged tails
+    wl = make_workload(60, 23, 4, 5.0, seed=21)
+    A = sm.Bcsr(wl)
+    P = sm.sm_build_pattern(A, pad)
+    Ph = sm.pattern_to_host(P)
+    cols, col_off, n = sm.sm_plan_columns(P, None)
+    X, scale = sm.sm_gather(A, P, cols, col_off, n, 0.0, "gershgorin", x_dtype)
+    iters, res = sm.sm_sign_ns(P, cols, col_off, n, P.packed_elems, x_dtype, X, 1, 0.0)
+    assert (iters == 1).all()
+    for i in (0, 17, 59):
+        T = orc.gather(wl, i)
+        m = T.shape[0]
+        x1 = unpack(X, Ph, i, x_dtype)[:m, :m]
+        assert np.abs(x1 - orc.ns_polynomial(T, orc.gershgorin(T), 1)).max() <= tol_abs
+        x0 = T / orc.gershgorin(T)
+        r0 = np.linalg.norm(x0 @ x0 - np.eye(m)) / np.sqrt(m)
+        assert abs(res[i].item() - r0) <= max(10 * tol_abs, 1e-12)       # fused residual of step 0
+        if x_dtype in ("bf16", "f16"):
+            assert np.array_equal(x1, x1.T)                               # mirrored stores: exact symmetry
+            xp = unpack(X, Ph, i, x_dtype)
+            assert not xp[m:].any() and not xp[:, m:].any()              # padding stays zero
+
+
+# ------------------------------------------------------------------- a4 scatter / symmetrise
+
+def test_scatter_places_owned_columns_bit_exact(sm):
+    # S_i := a symmetric matrix with integer-coded entries; the expected block values follow directly
+    # from PAPER.md:110 step 3: R(N(i)[a], i) = S_i[rows of neighbour a, columns of block i].
+    wl = ragged_workload()
+    A = sm.Bcsr(wl)
+    P = sm.sm_build_pattern(A, 4)
+    Ph = sm.pattern_to_host(P)
+    S = torch.zeros(P.packed_elems, dtype=torch.float64, device="cuda")
+    mats = []
+    for i in range(wl.n_blk):
+        m, Pd = int(Ph.dim[i]), int(Ph.dim_pad[i])
+        r = np.arange(m)
+        Si = 1000.0 * i + np.minimum.outer(r, r) * 64.0 + np.maximum.outer(r, r)   # symmetric, distinct
+        full = np.zeros((Pd, Pd))
+        full[:m, :m] = Si
+        S[int(Ph.sub_off[i]):int(Ph.sub_off[i + 1])] = torch.from_numpy(full.ravel()).cuda()
+        mats.append(Si)
+    R = sm.sm_scatter(A, P, None, P.sub_off, wl.n_blk, "f64", S).cpu().numpy()
+    off = {}
+    for i in range(wl.n_blk):
+        nb = wl.col_idx[wl.row_ptr[i]:wl.row_ptr[i + 1]]
+        o = np.concatenate([[0], np.cumsum(wl.blk_size[nb])])
+        off[i] = {int(j): (int(o[a]), int(o[a + 1])) for a, j in enumerate(nb)}
+    for j in range(wl.n_blk):                       # block (j, i) lives in row j
+        for p in range(wl.row_ptr[j], wl.row_ptr[j + 1]):
+            i = int(wl.col_idx[p])
+            (r0, r1), (c0, c1) = off[i][j], off[i][i]
+            assert np.array_equal(R[wl.val_ptr[p]:wl.val_ptr[p + 1]].reshape(r1 - r0, c1 - c0),
+                                  mats[i][r0:r1, c0:c1])
+    Rs = sm.sm_symmetrise(A, P, torch.from_numpy(R).cuda()).cpu().numpy()
+    assert np.array_equal(Rs, orc.symmetrise(wl, R))
+
+
+# ------------------------------------------------------------ a5 whole path, small configs
+
+def run_density(sm, wl, x_dtype, max_iter, tol, scale_mode, symmetrise=False, max_chunk_elems=None, pad=None):
+    A = sm.Bcsr(wl)
+    P = sm.sm_build_pattern(A, pad or (64 if x_dtype in ("bf16", "f16") else 16))
+    plan = sm.DensityPlan(A, P, x_dtype, max_chunk_elems=max_chunk_elems)
+    sm.sm_density(A, P, plan, mu=0.0, scale_mode=scale_mode, max_iter=max_iter, tol=tol, symmetrise=symmetrise)
+    torch.cuda.synchronize()
+    return A, P, plan
+
+
+def test_cfg0_fp64_all_columns(sm):
+    wl = make_config(0)
+    d_or, st = orc.density_columns(wl, n_threads=THREADS)
+    A, P, plan = run_density(sm, wl, "f64", 100, 1e-8, "gershgorin")
+    D = plan.D.cpu().numpy()
+    assert np.abs(D - d_or).max() <= 1e-10
+    assert abs(plan.trace.item() - orc.trace(wl, d_or)) <= 1e-10 * wl.n
+    assert sm.sm_sign_status(plan.residual, 1e-8) == sm.SM_OK
+    it = plan.iters.cpu().numpy()
+    assert it.min() >= 5 and it.max() <= 40
+    # scale parity (Gershgorin, fp64): per-column arrays are indexed by position in P.order
+    order = P.order.cpu().numpy()
+    assert np.allclose(plan.scale.cpu().numpy(), st.scale[order], rtol=1e-14)
+    # symmetrised result, chunked (two or more chunks) and with another padding: same numbers
+    _, _, plan2 = run_density(sm, wl, "f64", 100, 1e-8, "gershgorin", symmetrise=True,
+                              max_chunk_elems=int(P.packed_elems // 3), pad=4)
+    D2 = plan2.D.cpu().numpy()
+    assert np.abs(D2 - orc.symmetrise(wl, d_or)).max() <= 1e-10
+    assert plan2.trace.item() == pytest.approx(plan.trace.item(), abs=1e-11)
+
+
+def test_cfg0_limits_full_coverage_and_block_diagonal(sm):
+    wl = make_config(0, cutoff=np.inf)         # every T_i = H: D = full-matrix projector, Tr D integer
+    d_or, st = orc.density_columns(wl, n_threads=THREADS)
+    _, _, plan = run_density(sm, wl, "f64", 100, 1e-8, "gershgorin")
+    assert np.abs(plan.D.cpu().numpy() - d_or).max() <= 1e-10
+    assert abs(plan.trace.item() - st.n_neg[0]) <= 1e-9
+    wl = make_config(0, cutoff=0.0)            # block diagonal: m_i = b
+    d_or, _ = orc.density_columns(wl)
+    _, _, plan = run_density(sm, wl, "f64", 100, 1e-8, "gershgorin")
+    assert np.abs(plan.D.cpu().numpy() - d_or).max() <= 1e-10
+
+
+def test_cfg1_fp64_and_fp32_all_columns(sm):
+    wl = make_config(1)
+    d_or, _ = orc.density_columns(wl, n_threads=THREADS)
+    _, _, plan = run_density(sm, wl, "f64", 100, 1e-8, "gershgorin")
+    assert np.abs(plan.D.cpu().numpy() - d_or).max() <= 1e-10
+    assert sm.sm_sign_status(plan.residual, 1e-8) == sm.SM_OK
+    _, _, plan32 = run_density(sm, wl, "f32", 100, 1e-5, "gershgorin")
+    assert np.abs(plan32.D.cpu().numpy() - d_or).max() <= 1e-4
+    assert abs(plan32.trace.item() - orc.trace(wl, d_or)) / wl.n <= 1e-6
+    assert sm.sm_sign_status(plan32.residual, 1e-5) == sm.SM_OK
+
+
+def test_ragged_blocks_and_determinism(sm):
+    wl = ragged_workload()
+    d_or, _ = orc.density_columns(wl, n_threads=THREADS)
+    _, _, p1 = run_density(sm, wl, "f64", 100, 1e-8, "gershgorin")
+    assert np.abs(p1.D.cpu().numpy() - d_or).max() <= 1e-10
+    for x_dtype in ("f64", "bf16"):
+        a = run_density(sm, wl, x_dtype, 12, 0.0, "gershgorin", pad=64)[2].D.clone()
+        b = run_density(sm, wl, x_dtype, 12, 0.0, "gershgorin", pad=64)[2].D.clone()
+        assert torch.equal(a, b)                 # two runs bit-identical
+
+
+def test_not_converged_warning_and_odd_iteration_copy_back(sm):
+    wl = make_config(0)
+    _, _, plan = run_density(sm, wl, "f64", 3, 1e-8, "gershgorin")       # cap hit: warning status
+    assert sm.sm_sign_status(plan.residual, 1e-8) == sm.SM_WARN_NOT_CONVERGED
+    assert (plan.iters == 3).all()
+    d3, _ = orc.density_columns(wl, mode="nsk", k_fixed=3)
+    assert np.abs(plan.D.cpu().numpy() - d3).max() <= 1e-12
+    _, _, plan = run_density(sm, wl, "f16", 3, 0.0, "gershgorin")        # odd count: result copied back
+    assert np.abs(plan.D.cpu().numpy() - d3).max() <= 2e-3
+
+
+# ------------------------------------- full-size configs, bench.py's launch configuration, sampled columns
+
+def sampled_errors(wl, P, plan, cols, max_iter, lapack=True):
+    """(relF total vs exact sign, relF truncation, relF rounding vs NS-k, max-abs, |dTr|/rows) on the
+    owned columns of the sample (raw D).  Truncation / rounding split: DESIGN.md reading A13."""
+    dens = orc.density_columns_lapack if lapack else (lambda *a, **k: orc.density_columns(*a, n_threads=THREADS, **k))
+    d_or, st = dens(wl, cols=cols)
+    order = P.order.cpu().numpy()
+    pos = {int(c): k for k, c in enumerate(order)}
+    sc = plan.scale.cpu().numpy()[[pos[int(c)] for c in cols]]
+    d_k, _ = dens(wl, cols=cols, mode="nsk", k_fixed=max_iter, scale=sc)
+    mask = orc.column_mask(wl, cols)
+    D = plan.D.cpu().numpy()
+    nrm = np.linalg.norm(d_or[mask])
+    tr_g = tr_o = 0.0
+    rows = 0
+    for i in cols:
+        p = wl.row_ptr[i] + int(np.searchsorted(wl.col_idx[wl.row_ptr[i]:wl.row_ptr[i + 1]], i))
+        b = int(wl.blk_size[i])
+        tr_g += np.trace(D[wl.val_ptr[p]:wl.val_ptr[p + 1]].reshape(b, b))
+        tr_o += np.trace(d_or[wl.val_ptr[p]:wl.val_ptr[p + 1]].reshape(b, b))
+        rows += b
+    return dict(total=np.linalg.norm(D[mask] - d_or[mask]) / nrm, trunc=np.linalg.norm(d_k[mask] - d_or[mask]) / nrm,
+                rounding=np.linalg.norm(D[mask] - d_k[mask]) / nrm, maxabs=np.abs(D[mask] - d_or[mask]).max(),
+                maxabs_k=np.abs(D[mask] - d_k[mask]).max(), dtr=abs(tr_g - tr_o) / rows)
+
+
+def test_cfg2_bf16_full_size_sampled(sm):
+    wl = make_config(2)
+    run = CONFIGS[2]["runs"][0]
+    _, P, plan = run_density(sm, wl, "bf16", run["max_iter"], 0.0, "power", symmetrise=False)
+    assert (plan.iters == run["max_iter"]).all()
+    e = sampled_errors(wl, P, plan, sample_columns(wl, 24, 4242), run["max_iter"])
+    assert e["total"] <= 2e-2 and e["dtr"] <= 1e-3, e
+    assert e["rounding"] <= 1.2e-2, e            # bf16 rounding alone, against the NS-20 polynomial
+
+
+def test_cfg3_fp16_full_size_sampled(sm):
+    wl = make_config(3)
+    run = CONFIGS[3]["runs"][0]
+    _, P, plan = run_density(sm, wl, "f16", run["max_iter"], 0.0, "gershgorin")
+    e = sampled_errors(wl, P, plan, sample_columns(wl, 64, 4242), run["max_iter"], lapack=False)
+    assert e["total"] <= 2e-2 and e["dtr"] <= 1e-3, e
+    # "fp32 oracle comparison" (configs[3]): compare in fp32 after casting the fp64 oracle
+    assert np.float32(e["maxabs"]) <= np.float32(2e-3), e
+
+
+@pytest.mark.parametrize("x_dtype", ["bf16", "f16"])
+def test_cfg4_16bit_full_size_sampled(sm, x_dtype):
+    wl = make_config(4)
+    _, P, plan = run_density(sm, wl, x_dtype, 25, 0.0, "power")
+    e = sampled_errors(wl, P, plan, sample_columns(wl, 4, 4242), 25)
+    assert e["total"] <= 2e-2 and e["dtr"] <= 1e-3, e
+
+
+def test_cfg4_fp64_sampled_columns(sm):
+    # fp64 at 25 fixed iterations cannot meet 1e-10 against the exact sign (gapless spectrum, A13):
+    # (alpha) 25 fixed steps vs the oracle's NS-25 polynomial, (beta) convergence mode vs the exact sign.
+    wl = make_config(4)
+    cols_h = sample_columns(wl, 2, 4242)
+    A = sm.Bcsr(wl)
+    P = sm.sm_build_pattern(A, 16)
+    cols, col_off, n = sm.sm_plan_columns(P, cols_h)
+    ne = sm.packed_elems(P, cols_h)
+    mask = orc.column_mask(wl, cols_h)
+    d_or, st = orc.density_columns_lapack(wl, cols=cols_h)
+    for max_iter, tol, mode in ((25, 0.0, "nsk"), (100, 1e-8, "exact")):
+        X, scale = sm.sm_gather(A, P, cols, col_off, n, 0.0, "gershgorin", "f64")
+        iters, res = sm.sm_sign_ns(P, cols, col_off, n, ne, "f64", X, max_iter, tol)
+        R = sm.sm_scatter(A, P, cols, col_off, n, "f64", X)
+        D, _ = sm.sm_density_from_sign(A, P, R)
+        D = D.cpu().numpy()
+        ref = d_or if mode == "exact" else orc.density_columns_lapack(
+            wl, cols=cols_h, mode="nsk", k_fixed=25, scale=scale.cpu().numpy())[0]
+        assert np.abs(D[mask] - ref[mask]).max() <= 1e-10, (mode, iters.cpu().numpy())
+        if mode == "exact":
+            assert sm.sm_sign_status(res, tol) == sm.SM_OK

@@ -367,3 +367,21 @@ def test_trace_is_near_but_not_equal_to_electron_count():
     tr = orc.trace(w, d)
     n_neg_full = int((np.linalg.eigvalsh(w.dense()) < 0).sum())
     assert abs(tr - n_neg_full) < 0.5 and abs(tr - round(tr)) > 1e-6
+
+
+def test_lapack_variant_matches_jacobi_oracle():
+    # density_columns_lapack swaps the eigensolver only; it must reproduce the Jacobi path
+    w = make_config(0)
+    cols = [0, 5, 9, 31]
+    d_j, st_j = orc.density_columns(w, cols=cols)
+    d_l, st_l = orc.density_columns_lapack(w, cols=cols)
+    assert np.abs(d_j - d_l).max() < 1e-12
+    assert np.array_equal(st_j.n_neg, st_l.n_neg)
+    assert np.allclose(st_j.scale, st_l.scale, rtol=1e-14)
+    d_j, _ = orc.density_columns(w, cols=cols, mode="nsk", k_fixed=7)
+    d_l, _ = orc.density_columns_lapack(w, cols=cols, mode="nsk", k_fixed=7)
+    assert np.abs(d_j - d_l).max() < 1e-12
+    w2 = make_workload(40, 23, 4, 5.0, seed=3)
+    d_j, _ = orc.density_columns(w2, cols=[1, 2])
+    d_l, _ = orc.density_columns_lapack(w2, cols=[1, 2])
+    assert np.abs(d_j - d_l).max() < 1e-11
