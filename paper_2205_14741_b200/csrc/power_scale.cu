@@ -15,7 +15,7 @@ __device__ inline float px_load(const TX *Xs, int32_t Pd, int32_t r, int32_t c) 
   return (float)to_double<TX>(IMG ? Xs[img_off(Pd, r, c)] : Xs[(int64_t)r * Pd + c]);
 }
 
-// One CTA per listed column; dynamic smem: float v[m], w[m], red[32].
+// One CTA per listed column; dynamic smem: float v[Pd], w[Pd], red[64].
 template <typename TX, bool IMG>
 __global__ void k_power_scale(const int32_t *__restrict__ cols, const int64_t *__restrict__ col_off,
                               const int32_t *__restrict__ dim, const int32_t *__restrict__ dim_pad,
@@ -23,7 +23,8 @@ __global__ void k_power_scale(const int32_t *__restrict__ cols, const int64_t *_
   extern __shared__ float smem_f[];
   const int32_t c = blockIdx.x, i = cols ? cols[c] : c;
   const int32_t m = dim[i], Pd = dim_pad[i];
-  float *v = smem_f, *w = smem_f + m, *red = smem_f + 2 * m;
+  float *v = smem_f, *w = smem_f + Pd, *red = smem_f + 2 * Pd;
+  for (int32_t r = m + threadIdx.x; r < Pd; r += blockDim.x) { v[r] = 0.f; w[r] = 0.f; }
   TX *Xs = X + col_off[c];
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
   for (int32_t r = threadIdx.x; r < m; r += blockDim.x) {
@@ -36,7 +37,17 @@ __global__ void k_power_scale(const int32_t *__restrict__ cols, const int64_t *_
     // w = X v : one warp per row (X symmetric; rows are contiguous 128-byte runs in either layout)
     for (int32_t r = wid; r < m; r += nw) {
       float acc = 0.f;
-      for (int32_t cc = lane; cc < m; cc += 32) acc += px_load<TX, IMG>(Xs, Pd, r, cc) * v[cc];
+      if (IMG) {
+        // 16-byte chunks of 8 elements; padding columns of X are zero, v is zero-filled up to Pd
+        for (int32_t ch = lane; ch * 8 < m; ch += 32) {
+          const uint4 q4 = *reinterpret_cast<const uint4 *>(Xs + img_off(Pd, r, ch * 8));
+          const TX *e = reinterpret_cast<const TX *>(&q4);
+#pragma unroll
+          for (int k = 0; k < 8; ++k) acc += (float)to_double<TX>(e[k]) * v[ch * 8 + k];
+        }
+      } else {
+        for (int32_t cc = lane; cc < m; cc += 32) acc += px_load<TX, IMG>(Xs, Pd, r, cc) * v[cc];
+      }
       for (int d = 16; d > 0; d >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, d);
       if (lane == 0) w[r] = acc;
     }
@@ -65,7 +76,7 @@ __global__ void k_power_scale(const int32_t *__restrict__ cols, const int64_t *_
 template <typename TX, bool IMG>
 static int32_t launch_power(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, const int64_t *col_off,
                             void *X, double *scale, double *ratio, cudaStream_t st) {
-  size_t smem = (size_t)(2 * P->max_dim + 64) * sizeof(float);
+  size_t smem = (size_t)(2 * P->max_dim_pad + 64) * sizeof(float);
   k_power_scale<TX, IMG><<<n_cols, 512, smem, st>>>(cols, col_off, P->dim, P->dim_pad, (TX *)X, scale, ratio);
   SM_LAUNCHED();
   return SM_OK;

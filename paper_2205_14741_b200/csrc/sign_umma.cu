@@ -14,8 +14,8 @@
 // amplifies any antisymmetric perturbation by ~2x per step (measured: NaN after ~18 bf16 steps),
 // while exactly symmetric iterates make X X^T == X^2 and keep the iteration on Eq. 13's fixed point.
 //
-// Kernel: persistent, one CTA per SM, 192 threads = 1 TMA producer warp, 1 MMA issuer warp (also
-// owns TMEM), 4 epilogue warps.  Tile = 128 x (<=256) fp32 accumulator in TMEM, double buffered
+// Kernel: persistent, one CTA per SM, 320 threads = 1 TMA producer warp, 1 MMA issuer warp (also
+// owns TMEM), 8 epilogue warps.  Tile = 128 x (<=256) fp32 accumulator in TMEM, double buffered
 // (2 x 256 columns) so the epilogue of tile t overlaps the main loop of tile t+1; 4-stage smem ring.
 //   PHASE 1: Y = X X^T, epilogue writes Y and the fused ||Y - I||_F^2 partial sums (warp shuffles).
 //   PHASE 2: X' = 1.5 X - 0.5 X Y^T, epilogue reads the X tile and writes X'.
@@ -34,8 +34,10 @@ constexpr int USTAGES = 4;
 constexpr int A_BYTES = UM * UK * 2;           // 16 KB
 constexpr int B_BYTES = UN * UK * 2;           // 32 KB
 constexpr int STAGE_BYTES = A_BYTES + B_BYTES; // 48 KB
-constexpr int UMMA_SMEM = USTAGES * STAGE_BYTES + 1024 /*align slack*/ + 256 /*barriers*/;
-constexpr int UMMA_THREADS = 192;
+constexpr int EPI_WARPS = 8;
+constexpr int EPI_STAGE_BYTES = EPI_WARPS * 2048;   // 32 x 32 x 2 B transpose buffer per epilogue warp
+constexpr int UMMA_SMEM = USTAGES * STAGE_BYTES + EPI_STAGE_BYTES + 1024 /*align slack*/ + 256 /*barriers*/;
+constexpr int UMMA_THREADS = 64 + 32 * EPI_WARPS;
 constexpr uint32_t TMEM_COLS = 512;
 
 struct UTile {
@@ -122,7 +124,8 @@ __global__ void __launch_bounds__(UMMA_THREADS, 1) k_umma_gemm(UArgs a) {
   extern __shared__ uint8_t smem_raw[];
   const uint32_t raw = ptx::smem_u32(smem_raw);
   const uint32_t tiles = (raw + 1023u) & ~1023u;           // 1024-byte aligned operand ring
-  const uint32_t bars = tiles + USTAGES * STAGE_BYTES;     // barriers behind the ring
+  const uint32_t stage_base = tiles + USTAGES * STAGE_BYTES;   // epilogue transpose buffers
+  const uint32_t bars = stage_base + EPI_STAGE_BYTES;      // barriers behind them
   // barrier slots (8 bytes each): full[4], empty[4], tmem_full[2], tmem_empty[2]; then tmem base
   auto full_bar = [&](int s) { return bars + 8u * s; };
   auto empty_bar = [&](int s) { return bars + 8u * (USTAGES + s); };
@@ -136,7 +139,7 @@ __global__ void __launch_bounds__(UMMA_THREADS, 1) k_umma_gemm(UArgs a) {
 
   if (threadIdx.x == 0) {
     for (int s = 0; s < USTAGES; ++s) { ptx::mbar_init(full_bar(s), 1); ptx::mbar_init(empty_bar(s), 1); }
-    for (int s = 0; s < 2; ++s) { ptx::mbar_init(tfull_bar(s), 1); ptx::mbar_init(tempty_bar(s), 4); }
+    for (int s = 0; s < 2; ++s) { ptx::mbar_init(tfull_bar(s), 1); ptx::mbar_init(tempty_bar(s), EPI_WARPS); }
     ptx::fence_barrier_init();
     ptx::fence_proxy_async();
   }
@@ -209,8 +212,13 @@ __global__ void __launch_bounds__(UMMA_THREADS, 1) k_umma_gemm(UArgs a) {
       }
     }
   } else {
-    // ===================== epilogue (warps 2..5) =====================
+    // ===================== epilogue (warps 2..9) =====================
+    // Two warps per TMEM lane quadrant; a warp owns 32 rows and every other 32-column block.
+    // Per block: TMEM -> registers -> (a) 16-byte direct stores of row r, (b) a warp-private smem
+    // transpose so that the mirrored elements (c, r) also leave as 16-byte stores.
     const int q = warp & 3;                        // TMEM lane quadrant this warp may access
+    const int half = (warp - 2) >> 2;              // which column blocks (even / odd) this warp takes
+    uint16_t *stg = reinterpret_cast<uint16_t *>(smem_raw + (stage_base - raw)) + (warp - 2) * 1024;
     uint32_t it = 0;
     for (int64_t t = blockIdx.x; t < total; t += gridDim.x) {
       UTile u = decode_tile<PHASE>(a, t);
@@ -218,22 +226,64 @@ __global__ void __launch_bounds__(UMMA_THREADS, 1) k_umma_gemm(UArgs a) {
       const uint32_t as = it & 1u, aphase = (it >> 1) & 1u;
       ptx::mbar_wait(tfull_bar(as), aphase, a.err_flag, 4);
       ptx::tc_fence_after();
-      const int32_t r = u.row0 + q * 32 + lane;
-      const bool row_ok = r < u.m;
+      const int32_t R0 = u.row0 + q * 32;
+      const int32_t r = R0 + lane;
       const uint32_t taddr = tmem_base + as * UN + ((uint32_t)(q * 32) << 16);
       uint16_t *Og = (uint16_t *)a.Out + u.base;
       const uint16_t *Xg = (const uint16_t *)a.Xsrc + u.base;
       float res = 0.f;
-      for (int g = 0; g < u.nt / 16; ++g) {
-        uint32_t v[16];
-        ptx::tmem_ld16(taddr + (uint32_t)(g * 16), v);
+      const int nblk = (u.nt + 31) >> 5;
+      for (int bi = half; bi < nblk; bi += 2) {
+        const int32_t C0 = u.n0 + bi * 32;
+        const int w = min(32, u.nt - bi * 32);                 // 16 or 32 columns
+        if (C0 > R0 + 31 || R0 >= u.m) continue;               // block above the diagonal / padding rows
+        uint32_t v[32];
+        ptx::tmem_ld16(taddr + (uint32_t)(bi * 32), *reinterpret_cast<uint32_t(*)[16]>(&v[0]));
+        if (w == 32) ptx::tmem_ld16(taddr + (uint32_t)(bi * 32 + 16), *reinterpret_cast<uint32_t(*)[16]>(&v[16]));
         ptx::tmem_ld_wait();
-        if (row_ok) {
-          const int32_t c0 = u.n0 + g * 16;
+        const bool fast = (C0 + w - 1 < R0) && (R0 + 31 < u.m);   // strictly below the diagonal, rows valid
+        if (fast) {
 #pragma unroll
-          for (int h = 0; h < 2; ++h) {
-            const int32_t cc = c0 + h * 8;
-            if (cc > r) continue;                       // chunk entirely above the diagonal
+          for (int h = 0; h < 4; ++h) {
+            if (h * 8 < w) {
+              const int32_t cc = C0 + h * 8;
+              const int64_t off = img_off(u.Pd, r, cc);
+              float f[8];
+#pragma unroll
+              for (int e = 0; e < 8; ++e) f[e] = __uint_as_float(v[h * 8 + e]);
+              if (PHASE == 1) {
+#pragma unroll
+                for (int e = 0; e < 8; ++e) res = fmaf(2.f * f[e], f[e], res);   // stands for (r,c) and (c,r)
+              } else {
+                uint4 xo = *reinterpret_cast<const uint4 *>(Xg + off);
+                float2 x0 = unpack2<BF16>(xo.x), x1 = unpack2<BF16>(xo.y), x2 = unpack2<BF16>(xo.z),
+                       x3 = unpack2<BF16>(xo.w);
+                f[0] = 1.5f * x0.x - 0.5f * f[0]; f[1] = 1.5f * x0.y - 0.5f * f[1];
+                f[2] = 1.5f * x1.x - 0.5f * f[2]; f[3] = 1.5f * x1.y - 0.5f * f[3];
+                f[4] = 1.5f * x2.x - 0.5f * f[4]; f[5] = 1.5f * x2.y - 0.5f * f[5];
+                f[6] = 1.5f * x3.x - 0.5f * f[6]; f[7] = 1.5f * x3.y - 0.5f * f[7];
+              }
+              uint4 o;
+              o.x = pack2<BF16>(f[0], f[1]); o.y = pack2<BF16>(f[2], f[3]);
+              o.z = pack2<BF16>(f[4], f[5]); o.w = pack2<BF16>(f[6], f[7]);
+              *reinterpret_cast<uint4 *>(Og + off) = o;
+              const uint16_t *ov = reinterpret_cast<const uint16_t *>(&o);
+#pragma unroll
+              for (int e = 0; e < 8; ++e) stg[(h * 8 + e) * 32 + lane] = ov[e];   // transposed: [col][row]
+            }
+          }
+          __syncwarp();
+          for (int id = lane; id < w * 4; id += 32) {           // 16-byte chunks of the transposed block
+            const int c = id >> 2, j = id & 3;
+            const uint4 val = *reinterpret_cast<const uint4 *>(stg + id * 8);
+            *reinterpret_cast<uint4 *>(Og + img_off(u.Pd, C0 + c, R0 + 8 * j)) = val;
+          }
+          __syncwarp();
+        } else if (r < u.m) {
+          // block touching the diagonal or the ragged bottom edge: element-wise, c <= r only
+          for (int h = 0; h * 8 < w; ++h) {
+            const int32_t cc = C0 + h * 8;
+            if (cc > r) break;
             const int64_t off = img_off(u.Pd, r, cc);
             float f[8];
 #pragma unroll
@@ -242,8 +292,7 @@ __global__ void __launch_bounds__(UMMA_THREADS, 1) k_umma_gemm(UArgs a) {
 #pragma unroll
               for (int e = 0; e < 8; ++e) {
                 const int32_t c = cc + e;
-                if (c <= r && c < u.m) {
-                  // off-diagonal elements stand for (r,c) and (c,r)
+                if (c <= r) {
                   float d = f[e] - (c == r ? 1.f : 0.f);
                   res = fmaf(c == r ? d : 2.f * d, d, res);
                 }
@@ -261,18 +310,12 @@ __global__ void __launch_bounds__(UMMA_THREADS, 1) k_umma_gemm(UArgs a) {
             o.x = pack2<BF16>(f[0], f[1]); o.y = pack2<BF16>(f[2], f[3]);
             o.z = pack2<BF16>(f[4], f[5]); o.w = pack2<BF16>(f[6], f[7]);
             const uint16_t *ov = reinterpret_cast<const uint16_t *>(&o);
-            if (cc + 7 <= r) {
-              *reinterpret_cast<uint4 *>(Og + off) = o;  // whole chunk on or below the diagonal
 #pragma unroll
-              for (int e = 0; e < 8; ++e) Og[img_off(u.Pd, cc + e, r)] = ov[e];
-            } else {
-#pragma unroll
-              for (int e = 0; e < 8; ++e) {
-                const int32_t c = cc + e;
-                if (c <= r) {
-                  Og[off + e] = ov[e];
-                  if (c < r) Og[img_off(u.Pd, c, r)] = ov[e];
-                }
+            for (int e = 0; e < 8; ++e) {
+              const int32_t c = cc + e;
+              if (c <= r) {
+                Og[off + e] = ov[e];
+                if (c < r) Og[img_off(u.Pd, c, r)] = ov[e];
               }
             }
           }
@@ -285,7 +328,7 @@ __global__ void __launch_bounds__(UMMA_THREADS, 1) k_umma_gemm(UArgs a) {
       if (PHASE == 1) {
         for (int d = 16; d > 0; d >>= 1) res += __shfl_xor_sync(0xffffffffu, res, d);
         if (lane == 0)
-          a.s.partial[(int64_t)u.c * a.s.parts_per_col + (int64_t)u.lt * 4 + q] = (double)res;
+          a.s.partial[(int64_t)u.c * a.s.parts_per_col + (int64_t)u.lt * 8 + (warp - 2)] = (double)res;
       }
       ++it;
     }
@@ -311,7 +354,7 @@ static __global__ void k_umma_tilecounts(int32_t n_cols, const int32_t *__restri
   int32_t m = dim[cols ? cols[c] : c];
   int32_t nt = u_tiles(m);
   tiles[c] = nt;
-  n_parts[c] = nt * 4;
+  n_parts[c] = nt * EPI_WARPS;
 }
 
 struct UmmaWs {
@@ -323,7 +366,7 @@ static UmmaWs umma_layout(void *ws, int64_t ws_bytes, const sm_pattern_t *P, int
                           int64_t packed_elems) {
   WsCursor cur(ws, ws_bytes);
   UmmaWs w;
-  w.parts_per_col = u_Tm(P->max_dim) * u_Tn(P->max_dim) * 4;
+  w.parts_per_col = u_Tm(P->max_dim) * u_Tn(P->max_dim) * EPI_WARPS;
   w.Y = cur.take<char>(packed_elems * 2);
   w.X2 = cur.take<char>(packed_elems * 2);
   w.active = cur.take<int32_t>(n_cols);
