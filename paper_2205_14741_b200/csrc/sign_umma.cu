@@ -45,10 +45,22 @@ struct UTile {
   int64_t base;   // element offset of the submatrix in the packed buffer
 };
 
+// One entry per output tile, built once per sm_sign_ns call (k_umma_build_tiles) so that the
+// persistent roles fetch a tile with three 16-byte loads instead of a dependent binary search
+// (ncu, round 1: the search's long-scoreboard stalls were the top stall of every role).
+struct __align__(16) TileDesc {
+  int64_t base;                  // element offset of the submatrix in the packed buffer
+  int32_t c, m;                  // listed-column index, true dimension
+  int32_t Pd, row0, n0, nt;      // padded dimension, first row, first column, columns of the tile
+  int32_t lt, pad0, pad1, pad2;  // tile index inside its submatrix
+};
+
 struct UArgs {
   const int32_t *cols; const int64_t *col_off; const int32_t *dim; const int32_t *dim_pad;
   const int64_t *tile_ptr;   // [n_cols+1] exclusive scan of tiles per listed column
+  const TileDesc *tiles;     // [tile_ptr[n_cols]]
   int32_t n_cols;
+  int32_t check_flags;       // convergence mode: per-submatrix active/last flags are consulted
   const void *Xsrc; const void *Ybuf; void *Out;
   SignState s;
   int32_t *err_flag;
@@ -75,31 +87,52 @@ __host__ __device__ inline int32_t u_tiles(int32_t m) {
   return t;
 }
 
+__device__ __forceinline__ TileDesc load_desc(const UArgs &a, int64_t t) {
+  const uint4 *p = reinterpret_cast<const uint4 *>(a.tiles + t);
+  uint4 q0 = __ldg(p), q1 = __ldg(p + 1), q2 = __ldg(p + 2);
+  TileDesc d;
+  d.base = (int64_t)(((uint64_t)q0.y << 32) | q0.x);
+  d.c = (int32_t)q0.z; d.m = (int32_t)q0.w;
+  d.Pd = (int32_t)q1.x; d.row0 = (int32_t)q1.y; d.n0 = (int32_t)q1.z; d.nt = (int32_t)q1.w;
+  d.lt = (int32_t)q2.x; d.pad0 = d.pad1 = d.pad2 = 0;
+  return d;
+}
+
 template <int PHASE>
-__device__ __forceinline__ UTile decode_tile(const UArgs &a, int64_t t) {
+__device__ __forceinline__ UTile make_tile(const UArgs &a, const TileDesc &d) {
   UTile u;
-  u.c = upper_slot<int64_t>(a.tile_ptr, a.n_cols, t);
-  int32_t local = (int32_t)(t - a.tile_ptr[u.c]);
-  int32_t i = a.cols ? a.cols[u.c] : u.c;
-  u.m = a.dim[i]; u.Pd = a.dim_pad[i];
-  u.base = a.col_off[u.c];
-  u.Tn = u_Tn(u.m);
-  int32_t nb = u_nbase(u.m), n16 = u_n16(u.m);
-  u.tm = 0; u.lt = local;
-  for (;;) {
-    int32_t cnt = u_row_tiles(u.m, u.tm);
-    if (local < cnt) break;
-    local -= cnt; ++u.tm;
+  u.c = d.c; u.m = d.m; u.Pd = d.Pd; u.base = d.base;
+  u.row0 = d.row0; u.n0 = d.n0; u.nt = d.nt; u.lt = d.lt;
+  u.kmax = u_n16(d.m);
+  u.tm = 0; u.tn = 0; u.Tn = 0;
+  int32_t act = 1;
+  if (a.check_flags) {
+    act = a.s.active[d.c];
+    if (PHASE == 1) act = act && !a.s.last[d.c];
   }
-  u.tn = local;
-  u.row0 = u.tm * UM;
-  u.n0 = u.tn * nb;
-  u.nt = min(nb, n16 - u.n0);
-  u.kmax = n16;
-  int32_t act = a.s.active[u.c];
-  if (PHASE == 1) act = act && !a.s.last[u.c];
   u.valid = act;
   return u;
+}
+
+static __global__ void k_umma_build_tiles(int32_t n_cols, const int32_t *__restrict__ cols,
+                                          const int32_t *__restrict__ dim, const int32_t *__restrict__ dim_pad,
+                                          const int64_t *__restrict__ col_off,
+                                          const int64_t *__restrict__ tile_ptr, TileDesc *__restrict__ tiles) {
+  int32_t c = blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= n_cols) return;
+  int32_t i = cols ? cols[c] : c;
+  int32_t m = dim[i], nb = u_nbase(m), n16 = u_n16(m);
+  TileDesc d;
+  d.base = col_off[c]; d.c = c; d.m = m; d.Pd = dim_pad[i]; d.pad0 = d.pad1 = d.pad2 = 0;
+  int64_t t = tile_ptr[c];
+  int32_t lt = 0;
+  for (int32_t tm = 0; tm < u_Tm(m); ++tm) {
+    int32_t cnt = u_row_tiles(m, tm);
+    for (int32_t tn = 0; tn < cnt; ++tn, ++lt, ++t) {
+      d.row0 = tm * UM; d.n0 = tn * nb; d.nt = min(nb, n16 - d.n0); d.lt = lt;
+      tiles[t] = d;
+    }
+  }
 }
 
 template <bool BF16> __device__ __forceinline__ uint32_t pack2(float lo, float hi);
@@ -159,8 +192,11 @@ __global__ void __launch_bounds__(UMMA_THREADS, 1) k_umma_gemm(UArgs a) {
     // ===================== TMA producer =====================
     if (lane == 0) {
       int stage = 0; uint32_t phase = 0;
+      TileDesc nxt = load_desc(a, max((int64_t)0, min((int64_t)blockIdx.x, total - 1)));
       for (int64_t t = blockIdx.x; t < total; t += gridDim.x) {
-        UTile u = decode_tile<PHASE>(a, t);
+        const TileDesc cur = nxt;
+        nxt = load_desc(a, min(t + (int64_t)gridDim.x, total - 1));    // prefetch the next descriptor
+        UTile u = make_tile<PHASE>(a, cur);
         if (!u.valid) continue;
         const char *Ag = (const char *)a.Xsrc + u.base * ESZ;
         const char *Bg = (const char *)(PHASE == 1 ? a.Xsrc : a.Ybuf) + u.base * ESZ;
@@ -183,8 +219,11 @@ __global__ void __launch_bounds__(UMMA_THREADS, 1) k_umma_gemm(UArgs a) {
     if (lane == 0) {
       int stage = 0; uint32_t phase = 0;
       uint32_t it = 0;
+      TileDesc nxt = load_desc(a, max((int64_t)0, min((int64_t)blockIdx.x, total - 1)));
       for (int64_t t = blockIdx.x; t < total; t += gridDim.x) {
-        UTile u = decode_tile<PHASE>(a, t);
+        const TileDesc cur = nxt;
+        nxt = load_desc(a, min(t + (int64_t)gridDim.x, total - 1));
+        UTile u = make_tile<PHASE>(a, cur);
         if (!u.valid) continue;
         const uint32_t as = it & 1u, aphase = (it >> 1) & 1u;
         ptx::mbar_wait(tempty_bar(as), aphase ^ 1u, a.err_flag, 2);
@@ -220,8 +259,11 @@ __global__ void __launch_bounds__(UMMA_THREADS, 1) k_umma_gemm(UArgs a) {
     const int half = (warp - 2) >> 2;              // which column blocks (even / odd) this warp takes
     uint16_t *stg = reinterpret_cast<uint16_t *>(smem_raw + (stage_base - raw)) + (warp - 2) * 1024;
     uint32_t it = 0;
+    TileDesc nxt = load_desc(a, max((int64_t)0, min((int64_t)blockIdx.x, total - 1)));
     for (int64_t t = blockIdx.x; t < total; t += gridDim.x) {
-      UTile u = decode_tile<PHASE>(a, t);
+      const TileDesc cur = nxt;
+      nxt = load_desc(a, min(t + (int64_t)gridDim.x, total - 1));
+      UTile u = make_tile<PHASE>(a, cur);
       if (!u.valid) continue;
       const uint32_t as = it & 1u, aphase = (it >> 1) & 1u;
       ptx::mbar_wait(tfull_bar(as), aphase, a.err_flag, 4);
@@ -359,6 +401,7 @@ static __global__ void k_umma_tilecounts(int32_t n_cols, const int32_t *__restri
 
 struct UmmaWs {
   void *Y, *X2; int32_t *active, *last, *n_still, *n_parts, *err; int64_t *tile_ptr; double *partial;
+  TileDesc *tiles;
   int32_t parts_per_col; int64_t used;
 };
 
@@ -376,6 +419,7 @@ static UmmaWs umma_layout(void *ws, int64_t ws_bytes, const sm_pattern_t *P, int
   w.n_parts = cur.take<int32_t>(n_cols);
   w.tile_ptr = cur.take<int64_t>(n_cols + 1);
   w.partial = cur.take<double>((int64_t)n_cols * w.parts_per_col);
+  w.tiles = cur.take<TileDesc>((int64_t)n_cols * u_Tm(P->max_dim) * u_Tn(P->max_dim));
   w.used = cur.used + 256;
   return w;
 }
@@ -436,6 +480,8 @@ int32_t sign_umma(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, co
   k_umma_tilecounts<<<nb, 256, 0, st>>>(n_cols, cols, P->dim, w.tile_ptr, w.n_parts);
   SM_LAUNCHED();
   { int32_t rc = exclusive_scan_i64(n_cols, w.tile_ptr, w.tile_ptr, st); if (rc != SM_OK) return rc; }
+  k_umma_build_tiles<<<nb, 256, 0, st>>>(n_cols, cols, P->dim, P->dim_pad, col_off, w.tile_ptr, w.tiles);
+  SM_LAUNCHED();
   // Y and the alternate X buffer start as zeros so that padding never holds NaN/Inf bit patterns.
   SM_CUDA(cudaMemsetAsync(w.Y, 0, packed_elems * 2, st));
   SM_CUDA(cudaMemsetAsync(w.X2, 0, packed_elems * 2, st));
@@ -443,7 +489,7 @@ int32_t sign_umma(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, co
   void *buf[2] = {X, w.X2};
   for (int32_t k = 0; k < max_iter; ++k) {
     void *src = buf[k & 1], *dst = buf[(k + 1) & 1];
-    UArgs a{cols, col_off, P->dim, P->dim_pad, w.tile_ptr, n_cols, src, w.Y, w.Y, s, w.err};
+    UArgs a{cols, col_off, P->dim, P->dim_pad, w.tile_ptr, w.tiles, n_cols, tol > 0.0 ? 1 : 0, src, w.Y, w.Y, s, w.err};
     int32_t rc = bf16 ? launch_umma<true, 1>(a, n_sm, st) : launch_umma<false, 1>(a, n_sm, st);
     if (rc != SM_OK) return rc;
     SM_CUDA(cudaMemsetAsync(w.n_still, 0, sizeof(int32_t), st));
