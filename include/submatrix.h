@@ -70,7 +70,7 @@ extern "C" {
 /* spectral scaling of T_i - mu I before the iteration (reading A10) */
 #define SM_SCALE_NONE 0        /* s_i = 1 */
 #define SM_SCALE_GERSHGORIN 1  /* s_i = max_r sum_c |(T_i - mu I)_rc|  (>= spectral radius) */
-#define SM_SCALE_POWER 2       /* s_i = 1.05 * ||T v||_2 after 16 power steps on T_i - mu I from a
+#define SM_SCALE_POWER 2       /* s_i = 1.05 * ||T v||_2 after 10 power steps on T_i - mu I from a
                                   fixed start vector, never above the Gershgorin bound */
 
 /* Block-CSR description of the symmetric input A = H ("block-sparse"). */

@@ -74,73 +74,81 @@ __global__ void k_fill_double(int32_t n, double v, double *__restrict__ out) {
 }
 
 // ---- gather ------------------------------------------------------------------------------------
-// grid = (listed column, band of GATHER_ROWS rows).  Dynamic smem: int32 off[cnt+1], uint16 blkof[m].
-constexpr int GATHER_ROWS = 16;
+// grid = (listed column, band of GATHER_ROWS rows), 256 threads.  A work item is one 16-byte-aligned
+// run of 8 output elements (r, c0..c0+7); items are ordered so that the 8 lanes of a row cover one
+// 64-column chunk, i.e. a warp writes four full 128-byte lines of the image (or 4 contiguous row
+// segments of the row-major layout).  Dynamic smem: int32 off[cnt+1], uint16 blkof[Pd].
+constexpr int GATHER_ROWS = 64;
 
 struct GatherArgs {
   const int32_t *cols; const int64_t *col_off;
-  const int32_t *blk, *rp, *ci; const int64_t *vp;
+  const int32_t *rp; const int64_t *vp; const int32_t *row_off;
   const int64_t *gmap_ptr; const int32_t *gmap;
   const int32_t *dim, *dim_pad;
   const double *scale; double mu;
 };
 
-template <typename TA>
-__device__ inline double gather_elem(const GatherArgs &g, const TA *__restrict__ vals, const int32_t *off,
-                                     const uint16_t *blkof, const int32_t *gm, int32_t cnt, int32_t m,
-                                     int32_t r, int32_t c, double inv_s) {
-  if (r >= m || c >= m) return 0.0;
-  int32_t a = blkof[r], b = blkof[c];
-  int32_t p = gm[a * cnt + b];
-  double v = 0.0;
-  if (p >= 0) {
-    int32_t bc = off[b + 1] - off[b];
-    v = to_double<TA>(vals[g.vp[p] + (int64_t)(r - off[a]) * bc + (c - off[b])]);
-  }
-  if (r == c) v -= g.mu;
-  return v * inv_s;
-}
-
 template <typename TA, typename TX, bool IMG>
-__global__ void k_gather(GatherArgs g, const TA *__restrict__ vals, TX *__restrict__ X) {
+__global__ void __launch_bounds__(256) k_gather(GatherArgs g, const TA *__restrict__ vals, TX *__restrict__ X) {
   extern __shared__ int32_t smem_i[];
-  int32_t c_list = blockIdx.x;
-  int32_t i = g.cols ? g.cols[c_list] : c_list;
-  int32_t Pd = g.dim_pad[i], m = g.dim[i];
-  int32_t r0 = blockIdx.y * GATHER_ROWS;
+  const int32_t c_list = blockIdx.x;
+  const int32_t i = g.cols ? g.cols[c_list] : c_list;
+  const int32_t Pd = g.dim_pad[i], m = g.dim[i];
+  const int32_t r0 = blockIdx.y * GATHER_ROWS;
   if (r0 >= Pd) return;
-  int32_t lo = g.rp[i], cnt = g.rp[i + 1] - lo;
+  const int32_t lo = g.rp[i], cnt = g.rp[i + 1] - lo;
   int32_t *off = smem_i;
   uint16_t *blkof = (uint16_t *)(smem_i + cnt + 1);
-  if (threadIdx.x == 0) {
-    int32_t o = 0;
-    for (int32_t a = 0; a < cnt; ++a) { off[a] = o; o += g.blk[g.ci[lo + a]]; }
-    off[cnt] = o;
-  }
+  for (int32_t a = threadIdx.x; a < cnt; a += blockDim.x) off[a] = g.row_off[lo + a];
+  if (threadIdx.x == 0) off[cnt] = m;
   __syncthreads();
-  for (int32_t a = 0; a < cnt; ++a)
-    for (int32_t r = off[a] + threadIdx.x; r < off[a + 1]; r += blockDim.x) blkof[r] = (uint16_t)a;
+  for (int32_t a = threadIdx.x; a < cnt; a += blockDim.x)
+    for (int32_t r = off[a]; r < off[a + 1]; ++r) blkof[r] = (uint16_t)a;
   __syncthreads();
   const int32_t *gm = g.gmap + g.gmap_ptr[i];
-  double inv_s = 1.0 / g.scale[c_list];
+  const double inv_s = 1.0 / g.scale[c_list];
   TX *Xs = X + g.col_off[c_list];
-  int32_t rows = min(GATHER_ROWS, Pd - r0);
-  if (IMG) {
-    int32_t chunks = Pd >> 3;
-    for (int32_t e = threadIdx.x; e < rows * chunks; e += blockDim.x) {
-      int32_t rr = e / chunks, ch = e - rr * chunks;
-      int32_t r = r0 + rr, c0 = ch << 3;
-      __align__(16) TX v[8];
+  const int32_t rows = min(GATHER_ROWS, Pd - r0);
+  const int32_t n_cb = (Pd + 63) >> 6;                 // 64-column chunks (last may be partial: Pd % 16 == 0)
+  const int32_t items = n_cb * rows * 8;
+  for (int32_t e = threadIdx.x; e < items; e += blockDim.x) {
+    const int32_t j = e & 7, rr = (e >> 3) % rows, cb = (e >> 3) / rows;
+    const int32_t r = r0 + rr, c0 = (cb << 6) + (j << 3);
+    if (c0 >= Pd) continue;
+    __align__(16) TX v[8];
+    if (r >= m || c0 >= m) {
 #pragma unroll
-      for (int k = 0; k < 8; ++k)
-        v[k] = from_double<TX>(gather_elem<TA>(g, vals, off, blkof, gm, cnt, m, r, c0 + k, inv_s));
-      *reinterpret_cast<uint4 *>(Xs + img_off(Pd, r, c0)) = *reinterpret_cast<const uint4 *>(v);
+      for (int k = 0; k < 8; ++k) v[k] = from_double<TX>(0.0);
+    } else {
+      const int32_t a = blkof[r], ra = r - off[a];
+      const int32_t *gm_row = gm + (int64_t)a * cnt;
+      int32_t bprev = -1, cbase = 0;
+      const TA *src = nullptr;
+#pragma unroll
+      for (int k = 0; k < 8; ++k) {
+        const int32_t c = c0 + k;
+        double x = 0.0;
+        if (c < m) {
+          const int32_t b = blkof[c];
+          if (b != bprev) {
+            bprev = b; cbase = off[b];
+            const int32_t p = __ldg(gm_row + b);
+            src = p >= 0 ? vals + __ldg(g.vp + p) + (int64_t)ra * (off[b + 1] - cbase) : nullptr;
+          }
+          if (src) x = to_double<TA>(__ldg(src + (c - cbase)));
+          if (r == c) x -= g.mu;
+          x *= inv_s;
+        }
+        v[k] = from_double<TX>(x);
+      }
     }
-  } else {
-    for (int32_t e = threadIdx.x; e < rows * Pd; e += blockDim.x) {
-      int32_t rr = e / Pd, c = e - rr * Pd;
-      int32_t r = r0 + rr;
-      Xs[(int64_t)r * Pd + c] = from_double<TX>(gather_elem<TA>(g, vals, off, blkof, gm, cnt, m, r, c, inv_s));
+    TX *dst = IMG ? Xs + img_off(Pd, r, c0) : Xs + (int64_t)r * Pd + c0;
+    if (IMG || c0 + 8 <= Pd) {
+#pragma unroll
+      for (int q = 0; q < (int)(sizeof(TX) * 8 / 16); ++q)
+        reinterpret_cast<uint4 *>(dst)[q] = reinterpret_cast<const uint4 *>(v)[q];
+    } else {                                             // row tail when pad_to % 8 != 0 (row-major only)
+      for (int k = 0; c0 + k < Pd; ++k) dst[k] = v[k];
     }
   }
 }
@@ -154,7 +162,7 @@ __global__ void k_scatter(const int32_t *__restrict__ cols, const int64_t *__res
                           const int32_t *__restrict__ ci, const int64_t *__restrict__ vp,
                           const int32_t *__restrict__ own_pos, const int32_t *__restrict__ dim,
                           const int32_t *__restrict__ dim_pad, const int32_t *__restrict__ tmap,
-                          const TX *__restrict__ S, TR *__restrict__ R) {
+                          const int32_t *__restrict__ row_off, const TX *__restrict__ S, TR *__restrict__ R) {
   extern __shared__ int32_t smem_i[];
   int32_t c_list = blockIdx.x;
   int32_t i = cols ? cols[c_list] : c_list;
@@ -162,14 +170,11 @@ __global__ void k_scatter(const int32_t *__restrict__ cols, const int64_t *__res
   int32_t lo = rp[i], cnt = rp[i + 1] - lo;
   int32_t *off = smem_i;
   uint16_t *blkof = (uint16_t *)(smem_i + cnt + 1);
-  if (threadIdx.x == 0) {
-    int32_t o = 0;
-    for (int32_t a = 0; a < cnt; ++a) { off[a] = o; o += blk[ci[lo + a]]; }
-    off[cnt] = o;
-  }
+  for (int32_t a = threadIdx.x; a < cnt; a += blockDim.x) off[a] = row_off[lo + a];
+  if (threadIdx.x == 0) off[cnt] = m;
   __syncthreads();
-  for (int32_t a = 0; a < cnt; ++a)
-    for (int32_t r = off[a] + threadIdx.x; r < off[a + 1]; r += blockDim.x) blkof[r] = (uint16_t)a;
+  for (int32_t a = threadIdx.x; a < cnt; a += blockDim.x)
+    for (int32_t r = off[a]; r < off[a + 1]; ++r) blkof[r] = (uint16_t)a;
   __syncthreads();
   int32_t own = own_pos[i], own_off = off[own], bi = off[own + 1] - own_off;
   const TX *Ss = S + col_off[c_list];
@@ -264,7 +269,8 @@ template <typename TA, typename TX, bool IMG>
 static int32_t launch_gather(const GatherArgs &g, const void *vals, void *X, int32_t n_cols, int32_t max_pd,
                              int32_t max_nbr, int32_t max_dim, cudaStream_t st) {
   dim3 grid(n_cols, (max_pd + GATHER_ROWS - 1) / GATHER_ROWS);
-  size_t smem = (size_t)(max_nbr + 1) * 4 + (size_t)(max_dim + 2) * 2;
+  size_t smem = (size_t)(max_nbr + 1) * 4 + (size_t)(max_pd + 2) * 2;
+  (void)max_dim;
   k_gather<TA, TX, IMG><<<grid, 256, smem, st>>>(g, (const TA *)vals, (TX *)X);
   SM_LAUNCHED();
   return SM_OK;
@@ -309,7 +315,7 @@ extern "C" int32_t sm_gather(const sm_bcsr_t *A, const void *A_vals, int32_t a_d
     SM_LAUNCHED();
   }
 
-  GatherArgs g{cols, col_off, A->blk_size, A->row_ptr, A->col_idx, A->val_ptr, P->gmap_ptr, P->gmap,
+  GatherArgs g{cols, col_off, A->row_ptr, A->val_ptr, P->row_off, P->gmap_ptr, P->gmap,
                P->dim, P->dim_pad, scale, mu};
   // SM_SCALE_POWER: gather at the Gershgorin scale, tighten the scale by power steps on that X0
   // (power_scale.cu), then gather again so that X0 is rounded to the working type only once.
@@ -345,7 +351,7 @@ static int32_t launch_scatter(const sm_bcsr_t *A, const sm_pattern_t *P, const i
   size_t smem = (size_t)(P->max_nbr + 1) * 4 + (size_t)(P->max_dim + 2) * 2;
   k_scatter<TX, TR, IMG><<<n_cols, 256, smem, st>>>(cols, col_off, A->blk_size, A->row_ptr, A->col_idx,
                                                     A->val_ptr, P->own_pos, P->dim, P->dim_pad, P->tmap,
-                                                    (const TX *)S, (TR *)R);
+                                                    P->row_off, (const TX *)S, (TR *)R);
   SM_LAUNCHED();
   return SM_OK;
 }
