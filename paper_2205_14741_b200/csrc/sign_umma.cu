@@ -19,6 +19,7 @@
 // (2 x 256 columns) so the epilogue of tile t overlaps the main loop of tile t+1; 4-stage smem ring.
 //   PHASE 1: Y = X X^T, epilogue writes Y and the fused ||Y - I||_F^2 partial sums (warp shuffles).
 //   PHASE 2: X' = 1.5 X - 0.5 X Y^T, epilogue reads the X tile and writes X'.
+#include <cstdlib>
 #include <utility>
 #include <vector>
 
@@ -27,21 +28,29 @@
 
 namespace sm {
 
-constexpr int UM = 128;          // tile rows  (UMMA M)
+constexpr int UM = 128;          // tile rows per CTA (UMMA M per CTA)
 constexpr int UN = 256;          // max tile cols (UMMA N)
 constexpr int UK = 64;           // k chunk = one 128-byte swizzle row of 16-bit elements
-constexpr int USTAGES = 4;
 constexpr int A_BYTES = UM * UK * 2;           // 16 KB
-constexpr int B_BYTES = UN * UK * 2;           // 32 KB
-constexpr int STAGE_BYTES = A_BYTES + B_BYTES; // 48 KB
-constexpr int EPI_WARPS = 8;
+constexpr int EPI_WARPS = 16;
 constexpr int EPI_STAGE_BYTES = EPI_WARPS * 2048;   // 32 x 32 x 2 B transpose buffer per epilogue warp
-constexpr int UMMA_SMEM = USTAGES * STAGE_BYTES + EPI_STAGE_BYTES + 1024 /*align slack*/ + 256 /*barriers*/;
 constexpr int UMMA_THREADS = 64 + 32 * EPI_WARPS;
 constexpr uint32_t TMEM_COLS = 512;
 
+// NCTA = 1: one CTA per tile of 128 x (<=256).  NCTA = 2: a CTA pair (cta_group::2) per tile of
+// 256 x (<=256): each CTA stages its own 128 rows of A and HALF of the B rows, so a pair moves
+// (256 + nt) rows per k chunk for 256 x nt outputs instead of 2 x (128 + nt): the L2 -> SM bytes per
+// FLOP drop by 1.5x at nt = 256 (ncu, round 1: the single-CTA kernel sits on the L2 throughput cap).
+template <int NCTA> struct UCfg {
+  static constexpr int STAGES = NCTA == 2 ? 6 : 4;
+  static constexpr int B_BYTES = (UN / NCTA) * UK * 2;     // 32 KB / 16 KB
+  static constexpr int STAGE_BYTES = A_BYTES + B_BYTES;    // 48 KB / 32 KB
+  static constexpr int SMEM = STAGES * STAGE_BYTES + EPI_STAGE_BYTES + 1024 /*align slack*/ + 256 /*barriers*/;
+  static constexpr int ROWS = UM * NCTA;                   // tile rows
+};
+
 struct UTile {
-  int32_t c, m, Pd, row0, n0, nt, kmax, tm, tn, Tn, lt, valid;
+  int32_t c, m, Pd, row0, n0, nt, kmax, lt, valid;
   int64_t base;   // element offset of the submatrix in the packed buffer
 };
 
@@ -66,24 +75,25 @@ struct UArgs {
   int32_t *err_flag;
 };
 
+// Tile geometry.  Only elements (r, c) with c <= r are computed, so tile row tm (rows tm*R ..
+// tm*R + R - 1, R = 128 * NCTA) needs the columns [0, min(n16, tm*R + R)); they are split into the
+// fewest tiles of <= 256 columns, of equal width rounded up to 32 (the last one takes the rest).
 __host__ __device__ inline int32_t u_n16(int32_t m) { return (m + 15) & ~15; }
-__host__ __device__ inline int32_t u_Tn(int32_t m) { return (u_n16(m) + UN - 1) / UN; }
-__host__ __device__ inline int32_t u_Tm(int32_t m) { return (m + UM - 1) / UM; }
-__host__ __device__ inline int32_t u_nbase(int32_t m) {
-  int32_t Tn = u_Tn(m);
-  return ((u_n16(m) / 16 + Tn - 1) / Tn) * 16;
+__host__ __device__ inline int32_t u_Tm(int32_t m, int32_t R) { return (m + R - 1) / R; }
+__host__ __device__ inline int32_t u_ncols(int32_t m, int32_t R, int32_t tm) {
+  int32_t n16 = u_n16(m), e = tm * R + R;
+  return e < n16 ? e : n16;
 }
-
-// Tiles of one submatrix that touch the lower triangle: for tile row tm the tile columns tn with
-// n0 = tn * nbase <= row0 + UM - 1.
-__host__ __device__ inline int32_t u_row_tiles(int32_t m, int32_t tm) {
-  int32_t cnt = (tm * UM + UM - 1) / u_nbase(m) + 1;
-  int32_t Tn = u_Tn(m);
-  return cnt < Tn ? cnt : Tn;
+__host__ __device__ inline int32_t u_row_tiles(int32_t m, int32_t R, int32_t tm) {
+  return (u_ncols(m, R, tm) + UN - 1) / UN;
 }
-__host__ __device__ inline int32_t u_tiles(int32_t m) {
+__host__ __device__ inline int32_t u_row_nb(int32_t m, int32_t R, int32_t tm) {
+  int32_t nc = u_ncols(m, R, tm), Tn = (nc + UN - 1) / UN;
+  return (((nc + 31) / 32 + Tn - 1) / Tn) * 32;     // multiple of 32: epilogue blocks never straddle the diagonal
+}
+__host__ __device__ inline int32_t u_tiles(int32_t m, int32_t R) {
   int32_t t = 0;
-  for (int32_t tm = 0; tm < u_Tm(m); ++tm) t += u_row_tiles(m, tm);
+  for (int32_t tm = 0; tm < u_Tm(m, R); ++tm) t += u_row_tiles(m, R, tm);
   return t;
 }
 
@@ -104,7 +114,6 @@ __device__ __forceinline__ UTile make_tile(const UArgs &a, const TileDesc &d) {
   u.c = d.c; u.m = d.m; u.Pd = d.Pd; u.base = d.base;
   u.row0 = d.row0; u.n0 = d.n0; u.nt = d.nt; u.lt = d.lt;
   u.kmax = u_n16(d.m);
-  u.tm = 0; u.tn = 0; u.Tn = 0;
   int32_t act = 1;
   if (a.check_flags) {
     act = a.s.active[d.c];
@@ -114,22 +123,22 @@ __device__ __forceinline__ UTile make_tile(const UArgs &a, const TileDesc &d) {
   return u;
 }
 
-static __global__ void k_umma_build_tiles(int32_t n_cols, const int32_t *__restrict__ cols,
+static __global__ void k_umma_build_tiles(int32_t n_cols, int32_t R, const int32_t *__restrict__ cols,
                                           const int32_t *__restrict__ dim, const int32_t *__restrict__ dim_pad,
                                           const int64_t *__restrict__ col_off,
                                           const int64_t *__restrict__ tile_ptr, TileDesc *__restrict__ tiles) {
   int32_t c = blockIdx.x * blockDim.x + threadIdx.x;
   if (c >= n_cols) return;
   int32_t i = cols ? cols[c] : c;
-  int32_t m = dim[i], nb = u_nbase(m), n16 = u_n16(m);
+  int32_t m = dim[i];
   TileDesc d;
   d.base = col_off[c]; d.c = c; d.m = m; d.Pd = dim_pad[i]; d.pad0 = d.pad1 = d.pad2 = 0;
   int64_t t = tile_ptr[c];
   int32_t lt = 0;
-  for (int32_t tm = 0; tm < u_Tm(m); ++tm) {
-    int32_t cnt = u_row_tiles(m, tm);
+  for (int32_t tm = 0; tm < u_Tm(m, R); ++tm) {
+    int32_t cnt = u_row_tiles(m, R, tm), nb = u_row_nb(m, R, tm), nc = u_ncols(m, R, tm);
     for (int32_t tn = 0; tn < cnt; ++tn, ++lt, ++t) {
-      d.row0 = tm * UM; d.n0 = tn * nb; d.nt = min(nb, n16 - d.n0); d.lt = lt;
+      d.row0 = tm * R; d.n0 = tn * nb; d.nt = min(nb, nc - d.n0); d.lt = lt;
       tiles[t] = d;
     }
   }
@@ -152,36 +161,46 @@ template <> __device__ __forceinline__ float2 unpack2<false>(uint32_t w) {
   return __half22float2(*reinterpret_cast<__half2 *>(&w));
 }
 
-template <bool BF16, int PHASE>
+template <bool BF16, int PHASE, int NCTA>
 __global__ void __launch_bounds__(UMMA_THREADS, 1) k_umma_gemm(UArgs a) {
+  using Cfg = UCfg<NCTA>;
+  constexpr int USTAGES = Cfg::STAGES;
+  constexpr int STAGE_BYTES = Cfg::STAGE_BYTES;
+  constexpr bool PAIR = NCTA == 2;
   extern __shared__ uint8_t smem_raw[];
   const uint32_t raw = ptx::smem_u32(smem_raw);
   const uint32_t tiles = (raw + 1023u) & ~1023u;           // 1024-byte aligned operand ring
   const uint32_t stage_base = tiles + USTAGES * STAGE_BYTES;   // epilogue transpose buffers
   const uint32_t bars = stage_base + EPI_STAGE_BYTES;      // barriers behind them
-  // barrier slots (8 bytes each): full[4], empty[4], tmem_full[2], tmem_empty[2]; then tmem base
+  // barrier slots (8 bytes each): full[S], empty[S], pfull[S] (pair: peer's stage landed, leader only),
+  // tmem_full[2], tmem_empty[2]; then the TMEM base address
   auto full_bar = [&](int s) { return bars + 8u * s; };
   auto empty_bar = [&](int s) { return bars + 8u * (USTAGES + s); };
-  auto tfull_bar = [&](int s) { return bars + 8u * (2 * USTAGES + s); };
-  auto tempty_bar = [&](int s) { return bars + 8u * (2 * USTAGES + 2 + s); };
-  const uint32_t tmem_slot = bars + 8u * (2 * USTAGES + 4);
+  auto pfull_bar = [&](int s) { return bars + 8u * (2 * USTAGES + s); };
+  auto tfull_bar = [&](int s) { return bars + 8u * (3 * USTAGES + s); };
+  auto tempty_bar = [&](int s) { return bars + 8u * (3 * USTAGES + 2 + s); };
+  const uint32_t tmem_slot = bars + 8u * (3 * USTAGES + 4);
   volatile uint32_t *tmem_slot_ptr =
       reinterpret_cast<volatile uint32_t *>(smem_raw + (tmem_slot - raw));
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const uint32_t h = PAIR ? ptx::cluster_ctarank() : 0u;   // rank inside the CTA pair; 0 = leader
+  const int64_t unit = blockIdx.x / NCTA, n_units = gridDim.x / NCTA;
 
   if (threadIdx.x == 0) {
-    for (int s = 0; s < USTAGES; ++s) { ptx::mbar_init(full_bar(s), 1); ptx::mbar_init(empty_bar(s), 1); }
-    for (int s = 0; s < 2; ++s) { ptx::mbar_init(tfull_bar(s), 1); ptx::mbar_init(tempty_bar(s), EPI_WARPS); }
+    for (int s = 0; s < USTAGES; ++s) {
+      ptx::mbar_init(full_bar(s), 1); ptx::mbar_init(empty_bar(s), 1); ptx::mbar_init(pfull_bar(s), 1);
+    }
+    for (int s = 0; s < 2; ++s) { ptx::mbar_init(tfull_bar(s), 1); ptx::mbar_init(tempty_bar(s), EPI_WARPS * NCTA); }
     ptx::fence_barrier_init();
     ptx::fence_proxy_async();
   }
   if (warp == 1) {
-    ptx::tmem_alloc(tmem_slot, TMEM_COLS);
-    ptx::tmem_relinquish();
+    if (PAIR) { ptx::tmem_alloc2(tmem_slot, TMEM_COLS); ptx::tmem_relinquish2(); }
+    else { ptx::tmem_alloc(tmem_slot, TMEM_COLS); ptx::tmem_relinquish(); }
   }
   ptx::tc_fence_before();
-  __syncthreads();
+  if (PAIR) ptx::cluster_sync_all(); else __syncthreads();
   ptx::tc_fence_after();
   const uint32_t tmem_base = *tmem_slot_ptr;
 
@@ -189,50 +208,71 @@ __global__ void __launch_bounds__(UMMA_THREADS, 1) k_umma_gemm(UArgs a) {
   constexpr int ESZ = 2;
 
   if (warp == 0) {
-    // ===================== TMA producer =====================
+    // ===================== TMA producer (every CTA: its A rows and its share of the B rows) ==========
     if (lane == 0) {
       int stage = 0; uint32_t phase = 0;
-      TileDesc nxt = load_desc(a, max((int64_t)0, min((int64_t)blockIdx.x, total - 1)));
-      for (int64_t t = blockIdx.x; t < total; t += gridDim.x) {
+      TileDesc nxt = load_desc(a, max((int64_t)0, min(unit, total - 1)));
+      for (int64_t t = unit; t < total; t += n_units) {
         const TileDesc cur = nxt;
-        nxt = load_desc(a, min(t + (int64_t)gridDim.x, total - 1));    // prefetch the next descriptor
+        nxt = load_desc(a, min(t + n_units, total - 1));    // prefetch the next descriptor
         UTile u = make_tile<PHASE>(a, cur);
         if (!u.valid) continue;
         const char *Ag = (const char *)a.Xsrc + u.base * ESZ;
         const char *Bg = (const char *)(PHASE == 1 ? a.Xsrc : a.Ybuf) + u.base * ESZ;
-        const uint32_t a_rows = (uint32_t)min(UM, u.Pd - u.row0);
-        const uint32_t a_bytes = a_rows * 128u, b_bytes = (uint32_t)u.nt * 128u;
+        const int32_t arow0 = u.row0 + (int32_t)h * UM;
+        const uint32_t a_rows = (uint32_t)max(0, min(UM, u.Pd - arow0));
+        const int32_t b_cnt = u.nt / NCTA, brow0 = u.n0 + (int32_t)h * b_cnt;
+        const uint32_t a_bytes = a_rows * 128u, b_bytes = (uint32_t)b_cnt * 128u;
         const int nkc = (u.kmax + UK - 1) / UK;
         for (int kc = 0; kc < nkc; ++kc) {
           ptx::mbar_wait(empty_bar(stage), phase ^ 1u, a.err_flag, 1);
           const uint32_t sa = tiles + stage * STAGE_BYTES, sb = sa + A_BYTES;
           ptx::mbar_expect_tx(full_bar(stage), a_bytes + b_bytes);
           const int64_t chunk = (int64_t)kc * u.Pd * 128;     // byte offset of k chunk kc
-          ptx::tma_bulk_g2s(sa, Ag + chunk + (int64_t)u.row0 * 128, a_bytes, full_bar(stage));
-          ptx::tma_bulk_g2s(sb, Bg + chunk + (int64_t)u.n0 * 128, b_bytes, full_bar(stage));
+          if (a_bytes) ptx::tma_bulk_g2s(sa, Ag + chunk + (int64_t)arow0 * 128, a_bytes, full_bar(stage));
+          ptx::tma_bulk_g2s(sb, Bg + chunk + (int64_t)brow0 * 128, b_bytes, full_bar(stage));
+          if (++stage == USTAGES) { stage = 0; phase ^= 1u; }
+        }
+      }
+    }
+  } else if (warp == 1 && h != 0) {
+    // ===================== relay (peer CTA of a pair): tell the leader that this CTA's stage landed ======
+    if (lane == 0) {
+      int stage = 0; uint32_t phase = 0;
+      TileDesc nxt = load_desc(a, max((int64_t)0, min(unit, total - 1)));
+      for (int64_t t = unit; t < total; t += n_units) {
+        const TileDesc cur = nxt;
+        nxt = load_desc(a, min(t + n_units, total - 1));
+        UTile u = make_tile<PHASE>(a, cur);
+        if (!u.valid) continue;
+        const int nkc = (u.kmax + UK - 1) / UK;
+        for (int kc = 0; kc < nkc; ++kc) {
+          ptx::mbar_wait(full_bar(stage), phase, a.err_flag, 5);
+          ptx::mbar_arrive_remote(pfull_bar(stage), 0);
           if (++stage == USTAGES) { stage = 0; phase ^= 1u; }
         }
       }
     }
   } else if (warp == 1) {
-    // ===================== MMA issuer =====================
+    // ===================== MMA issuer (leader CTA) =====================
     if (lane == 0) {
       int stage = 0; uint32_t phase = 0;
       uint32_t it = 0;
-      TileDesc nxt = load_desc(a, max((int64_t)0, min((int64_t)blockIdx.x, total - 1)));
-      for (int64_t t = blockIdx.x; t < total; t += gridDim.x) {
+      TileDesc nxt = load_desc(a, max((int64_t)0, min(unit, total - 1)));
+      for (int64_t t = unit; t < total; t += n_units) {
         const TileDesc cur = nxt;
-        nxt = load_desc(a, min(t + (int64_t)gridDim.x, total - 1));
+        nxt = load_desc(a, min(t + n_units, total - 1));
         UTile u = make_tile<PHASE>(a, cur);
         if (!u.valid) continue;
         const uint32_t as = it & 1u, aphase = (it >> 1) & 1u;
         ptx::mbar_wait(tempty_bar(as), aphase ^ 1u, a.err_flag, 2);
         ptx::tc_fence_after();
         const uint32_t d_tmem = tmem_base + as * UN;
-        const uint32_t idesc = ptx::make_idesc_f16(BF16, UM, (uint32_t)u.nt);
+        const uint32_t idesc = ptx::make_idesc_f16(BF16, UM * NCTA, (uint32_t)u.nt);
         const int nkc = (u.kmax + UK - 1) / UK;
         for (int kc = 0; kc < nkc; ++kc) {
           ptx::mbar_wait(full_bar(stage), phase, a.err_flag, 3);
+          if (PAIR) ptx::mbar_wait(pfull_bar(stage), phase, a.err_flag, 6);
           ptx::tc_fence_after();
           const uint32_t sa = tiles + stage * STAGE_BYTES, sb = sa + A_BYTES;
           const uint64_t adesc = ptx::make_sw128_kmajor_desc(sa);
@@ -240,147 +280,169 @@ __global__ void __launch_bounds__(UMMA_THREADS, 1) k_umma_gemm(UArgs a) {
           const int ksteps = min(UK / 16, (u.kmax - kc * UK) / 16);
           for (int ks = 0; ks < ksteps; ++ks) {
             // advance 16 elements = 32 bytes inside the swizzle atom: +2 in the (addr >> 4) field
-            ptx::umma_f16(d_tmem, adesc + (uint64_t)(2 * ks), bdesc + (uint64_t)(2 * ks), idesc,
-                          (uint32_t)((kc | ks) != 0));
+            if (PAIR)
+              ptx::umma_f16_2cta(d_tmem, adesc + (uint64_t)(2 * ks), bdesc + (uint64_t)(2 * ks), idesc,
+                                 (uint32_t)((kc | ks) != 0));
+            else
+              ptx::umma_f16(d_tmem, adesc + (uint64_t)(2 * ks), bdesc + (uint64_t)(2 * ks), idesc,
+                            (uint32_t)((kc | ks) != 0));
           }
-          ptx::umma_commit(empty_bar(stage));      // frees the smem slot when these MMAs finish
+          // frees the smem slot (in both CTAs of a pair) when these MMAs finish
+          if (PAIR) ptx::umma_commit_2cta(empty_bar(stage)); else ptx::umma_commit(empty_bar(stage));
           if (++stage == USTAGES) { stage = 0; phase ^= 1u; }
         }
-        ptx::umma_commit(tfull_bar(as));           // accumulator ready for the epilogue
+        // accumulator ready for the epilogue warps (of both CTAs)
+        if (PAIR) ptx::umma_commit_2cta(tfull_bar(as)); else ptx::umma_commit(tfull_bar(as));
         ++it;
       }
     }
   } else {
-    // ===================== epilogue (warps 2..9) =====================
-    // Two warps per TMEM lane quadrant; a warp owns 32 rows and every other 32-column block.
-    // Per block: TMEM -> registers -> (a) 16-byte direct stores of row r, (b) a warp-private smem
-    // transpose so that the mirrored elements (c, r) also leave as 16-byte stores.
+    // ===================== epilogue (warps 2..17) =====================
+    // EPI_WARPS / 4 warps per TMEM lane quadrant; a warp owns 32 rows and every (EPI_WARPS/4)-th
+    // 32-column block at or below the diagonal.  Tiles start at multiples of 32 columns, so a block is
+    // either strictly below the diagonal (stored at (r, c) directly and at (c, r) through a warp-private
+    // smem transpose, both as 16-byte stores) or the diagonal block itself (symmetrised in smem: the
+    // lower triangle overwrites the upper one, then stored once).  Padding rows/columns of X are zero,
+    // so their accumulators are exactly zero and need no special path.
+    constexpr int NSUB = EPI_WARPS / 4;
     const int q = warp & 3;                        // TMEM lane quadrant this warp may access
-    const int half = (warp - 2) >> 2;              // which column blocks (even / odd) this warp takes
+    const int sub = (warp - 2) >> 2;               // which column blocks this warp takes
     uint16_t *stg = reinterpret_cast<uint16_t *>(smem_raw + (stage_base - raw)) + (warp - 2) * 1024;
     uint32_t it = 0;
-    TileDesc nxt = load_desc(a, max((int64_t)0, min((int64_t)blockIdx.x, total - 1)));
-    for (int64_t t = blockIdx.x; t < total; t += gridDim.x) {
+    TileDesc nxt = load_desc(a, max((int64_t)0, min(unit, total - 1)));
+    for (int64_t t = unit; t < total; t += n_units) {
       const TileDesc cur = nxt;
-      nxt = load_desc(a, min(t + (int64_t)gridDim.x, total - 1));
+      nxt = load_desc(a, min(t + n_units, total - 1));
       UTile u = make_tile<PHASE>(a, cur);
       if (!u.valid) continue;
       const uint32_t as = it & 1u, aphase = (it >> 1) & 1u;
-      ptx::mbar_wait(tfull_bar(as), aphase, a.err_flag, 4);
-      ptx::tc_fence_after();
-      const int32_t R0 = u.row0 + q * 32;
+      const int32_t R0 = u.row0 + (int32_t)h * UM + q * 32;   // this CTA's 128 rows of the tile
       const int32_t r = R0 + lane;
-      const uint32_t taddr = tmem_base + as * UN + ((uint32_t)(q * 32) << 16);
       uint16_t *Og = (uint16_t *)a.Out + u.base;
       const uint16_t *Xg = (const uint16_t *)a.Xsrc + u.base;
-      float res = 0.f;
       const int nblk = (u.nt + 31) >> 5;
-      for (int bi = half; bi < nblk; bi += 2) {
-        const int32_t C0 = u.n0 + bi * 32;
-        const int w = min(32, u.nt - bi * 32);                 // 16 or 32 columns
-        if (C0 > R0 + 31 || R0 >= u.m) continue;               // block above the diagonal / padding rows
-        uint32_t v[32];
-        ptx::tmem_ld16(taddr + (uint32_t)(bi * 32), *reinterpret_cast<uint32_t(*)[16]>(&v[0]));
-        if (w == 32) ptx::tmem_ld16(taddr + (uint32_t)(bi * 32 + 16), *reinterpret_cast<uint32_t(*)[16]>(&v[16]));
-        ptx::tmem_ld_wait();
-        const bool fast = (C0 + w - 1 < R0) && (R0 + 31 < u.m);   // strictly below the diagonal, rows valid
-        if (fast) {
+      ptx::mbar_wait(tfull_bar(as), aphase, a.err_flag, 4);
+      ptx::tc_fence_after();
+      const uint32_t taddr = tmem_base + as * UN + ((uint32_t)(q * 32) << 16);
+      float res = 0.f;
+      if (R0 < u.Pd) {
+        for (int bi = sub; bi < nblk; bi += NSUB) {
+          const int32_t C0 = u.n0 + bi * 32;
+          if (C0 > R0) break;                                    // block above the diagonal
+          const int w = min(32, u.nt - bi * 32);                 // 16 or 32 columns
+          uint32_t v[32];
+          ptx::tmem_ld16(taddr + (uint32_t)(bi * 32), *reinterpret_cast<uint32_t(*)[16]>(&v[0]));
+          if (w == 32) ptx::tmem_ld16(taddr + (uint32_t)(bi * 32 + 16), *reinterpret_cast<uint32_t(*)[16]>(&v[16]));
+          uint4 xo[4];
+          if (PHASE == 2) {
 #pragma unroll
-          for (int h = 0; h < 4; ++h) {
-            if (h * 8 < w) {
-              const int32_t cc = C0 + h * 8;
-              const int64_t off = img_off(u.Pd, r, cc);
+            for (int g = 0; g < 4; ++g)
+              if (g * 8 < w) xo[g] = *reinterpret_cast<const uint4 *>(Xg + img_off(u.Pd, r, C0 + g * 8));
+          }
+          ptx::tmem_ld_wait();
+          const bool diag = (C0 == R0);
+          uint32_t o[16];                                        // 32 output elements, packed pairs
+#pragma unroll
+          for (int g = 0; g < 4; ++g) {
+            if (g * 8 < w) {
               float f[8];
 #pragma unroll
-              for (int e = 0; e < 8; ++e) f[e] = __uint_as_float(v[h * 8 + e]);
+              for (int e = 0; e < 8; ++e) f[e] = __uint_as_float(v[g * 8 + e]);
               if (PHASE == 1) {
+                if (r < u.m) {
+                  if (!diag) {
 #pragma unroll
-                for (int e = 0; e < 8; ++e) res = fmaf(2.f * f[e], f[e], res);   // stands for (r,c) and (c,r)
+                    for (int e = 0; e < 8; ++e) res = fmaf(2.f * f[e], f[e], res);   // (r,c) and (c,r)
+                  } else {
+#pragma unroll
+                    for (int e = 0; e < 8; ++e) {
+                      const int j = g * 8 + e;
+                      const float d = f[e] - (j == lane ? 1.f : 0.f);
+                      if (j <= lane) res = fmaf(j == lane ? d : 2.f * d, d, res);
+                    }
+                  }
+                }
               } else {
-                uint4 xo = *reinterpret_cast<const uint4 *>(Xg + off);
-                float2 x0 = unpack2<BF16>(xo.x), x1 = unpack2<BF16>(xo.y), x2 = unpack2<BF16>(xo.z),
-                       x3 = unpack2<BF16>(xo.w);
-                f[0] = 1.5f * x0.x - 0.5f * f[0]; f[1] = 1.5f * x0.y - 0.5f * f[1];
-                f[2] = 1.5f * x1.x - 0.5f * f[2]; f[3] = 1.5f * x1.y - 0.5f * f[3];
-                f[4] = 1.5f * x2.x - 0.5f * f[4]; f[5] = 1.5f * x2.y - 0.5f * f[5];
-                f[6] = 1.5f * x3.x - 0.5f * f[6]; f[7] = 1.5f * x3.y - 0.5f * f[7];
-              }
-              uint4 o;
-              o.x = pack2<BF16>(f[0], f[1]); o.y = pack2<BF16>(f[2], f[3]);
-              o.z = pack2<BF16>(f[4], f[5]); o.w = pack2<BF16>(f[6], f[7]);
-              *reinterpret_cast<uint4 *>(Og + off) = o;
-              const uint16_t *ov = reinterpret_cast<const uint16_t *>(&o);
+                const uint32_t *xw = reinterpret_cast<const uint32_t *>(&xo[g]);
 #pragma unroll
-              for (int e = 0; e < 8; ++e) stg[(h * 8 + e) * 32 + lane] = ov[e];   // transposed: [col][row]
-            }
-          }
-          __syncwarp();
-          for (int id = lane; id < w * 4; id += 32) {           // 16-byte chunks of the transposed block
-            const int c = id >> 2, j = id & 3;
-            const uint4 val = *reinterpret_cast<const uint4 *>(stg + id * 8);
-            *reinterpret_cast<uint4 *>(Og + img_off(u.Pd, C0 + c, R0 + 8 * j)) = val;
-          }
-          __syncwarp();
-        } else if (r < u.m) {
-          // block touching the diagonal or the ragged bottom edge: element-wise, c <= r only
-          for (int h = 0; h * 8 < w; ++h) {
-            const int32_t cc = C0 + h * 8;
-            if (cc > r) break;
-            const int64_t off = img_off(u.Pd, r, cc);
-            float f[8];
-#pragma unroll
-            for (int e = 0; e < 8; ++e) f[e] = __uint_as_float(v[h * 8 + e]);
-            if (PHASE == 1) {
-#pragma unroll
-              for (int e = 0; e < 8; ++e) {
-                const int32_t c = cc + e;
-                if (c <= r) {
-                  float d = f[e] - (c == r ? 1.f : 0.f);
-                  res = fmaf(c == r ? d : 2.f * d, d, res);
+                for (int e2 = 0; e2 < 4; ++e2) {
+                  const float2 x = unpack2<BF16>(xw[e2]);
+                  f[2 * e2] = 1.5f * x.x - 0.5f * f[2 * e2];
+                  f[2 * e2 + 1] = 1.5f * x.y - 0.5f * f[2 * e2 + 1];
                 }
               }
-            } else {
-              uint4 xo = *reinterpret_cast<const uint4 *>(Xg + off);
-              float2 x0 = unpack2<BF16>(xo.x), x1 = unpack2<BF16>(xo.y), x2 = unpack2<BF16>(xo.z),
-                     x3 = unpack2<BF16>(xo.w);
-              f[0] = 1.5f * x0.x - 0.5f * f[0]; f[1] = 1.5f * x0.y - 0.5f * f[1];
-              f[2] = 1.5f * x1.x - 0.5f * f[2]; f[3] = 1.5f * x1.y - 0.5f * f[3];
-              f[4] = 1.5f * x2.x - 0.5f * f[4]; f[5] = 1.5f * x2.y - 0.5f * f[5];
-              f[6] = 1.5f * x3.x - 0.5f * f[6]; f[7] = 1.5f * x3.y - 0.5f * f[7];
-            }
-            uint4 o;
-            o.x = pack2<BF16>(f[0], f[1]); o.y = pack2<BF16>(f[2], f[3]);
-            o.z = pack2<BF16>(f[4], f[5]); o.w = pack2<BF16>(f[6], f[7]);
-            const uint16_t *ov = reinterpret_cast<const uint16_t *>(&o);
 #pragma unroll
-            for (int e = 0; e < 8; ++e) {
-              const int32_t c = cc + e;
-              if (c <= r) {
-                Og[off + e] = ov[e];
-                if (c < r) Og[img_off(u.Pd, c, r)] = ov[e];
+              for (int e2 = 0; e2 < 4; ++e2) o[g * 4 + e2] = pack2<BF16>(f[2 * e2], f[2 * e2 + 1]);
+            }
+          }
+          if (diag) {
+            // S[row][col] in smem; then element (row, j > row) is replaced by element (j, row)
+#pragma unroll
+            for (int g = 0; g < 4; ++g)
+              if (g * 8 < w)
+                *reinterpret_cast<uint4 *>(stg + lane * 32 + ((g ^ (lane & 3)) << 3)) =
+                    make_uint4(o[g * 4], o[g * 4 + 1], o[g * 4 + 2], o[g * 4 + 3]);
+            __syncwarp();
+            if (lane < w) {
+#pragma unroll
+              for (int j = 0; j < 32; ++j) {
+                if (j > lane && j < w) {
+                  // element (j, lane) sits in row j, chunk (lane >> 3) ^ (j & 3), position lane & 7
+                  const uint16_t m16 = stg[j * 32 + (((lane >> 3) ^ (j & 3)) << 3) + (lane & 7)];
+                  o[j >> 1] = (j & 1) ? ((o[j >> 1] & 0x0000FFFFu) | ((uint32_t)m16 << 16))
+                                      : ((o[j >> 1] & 0xFFFF0000u) | (uint32_t)m16);
+                }
               }
             }
+            __syncwarp();
+#pragma unroll
+            for (int g = 0; g < 4; ++g)
+              if (g * 8 < w)
+                *reinterpret_cast<uint4 *>(Og + img_off(u.Pd, r, C0 + g * 8)) =
+                    make_uint4(o[g * 4], o[g * 4 + 1], o[g * 4 + 2], o[g * 4 + 3]);
+          } else {
+#pragma unroll
+            for (int g = 0; g < 4; ++g) {
+              if (g * 8 < w) {
+                *reinterpret_cast<uint4 *>(Og + img_off(u.Pd, r, C0 + g * 8)) =
+                    make_uint4(o[g * 4], o[g * 4 + 1], o[g * 4 + 2], o[g * 4 + 3]);
+#pragma unroll
+                for (int e = 0; e < 8; ++e)                      // transposed: [col][row]
+                  stg[(g * 8 + e) * 32 + lane] = (uint16_t)(o[g * 4 + (e >> 1)] >> ((e & 1) * 16));
+              }
+            }
+            __syncwarp();
+            for (int id = lane; id < w * 4; id += 32) {          // 16-byte chunks of the transposed block
+              const int c = id >> 2, j = id & 3;
+              const uint4 val = *reinterpret_cast<const uint4 *>(stg + id * 8);
+              *reinterpret_cast<uint4 *>(Og + img_off(u.Pd, C0 + c, R0 + 8 * j)) = val;
+            }
+            __syncwarp();
           }
         }
       }
       // accumulator drained: hand the TMEM stage back to the MMA warp
       ptx::tc_fence_before();
       __syncwarp();
-      if (lane == 0) ptx::mbar_arrive(tempty_bar(as));
+      if (lane == 0) {
+        if (PAIR) ptx::mbar_arrive_remote(tempty_bar(as), 0); else ptx::mbar_arrive(tempty_bar(as));
+      }
       if (PHASE == 1) {
         for (int d = 16; d > 0; d >>= 1) res += __shfl_xor_sync(0xffffffffu, res, d);
         if (lane == 0)
-          a.s.partial[(int64_t)u.c * a.s.parts_per_col + (int64_t)u.lt * 8 + (warp - 2)] = (double)res;
+          a.s.partial[(int64_t)u.c * a.s.parts_per_col + (int64_t)u.lt * (EPI_WARPS * NCTA) + (int64_t)h * EPI_WARPS +
+                      (warp - 2)] = (double)res;
       }
       ++it;
     }
   }
 
   ptx::tc_fence_before();
-  __syncthreads();
+  __syncwarp();
+  if (PAIR) ptx::cluster_sync_all(); else __syncthreads();
   if (warp == 1) {
     ptx::tc_fence_after();
-    ptx::tmem_dealloc(tmem_base, TMEM_COLS);
+    if (PAIR) ptx::tmem_dealloc2(tmem_base, TMEM_COLS); else ptx::tmem_dealloc(tmem_base, TMEM_COLS);
   }
 }
 
@@ -388,15 +450,15 @@ __global__ void __launch_bounds__(UMMA_THREADS, 1) k_umma_gemm(UArgs a) {
 
 namespace sm {
 
-static __global__ void k_umma_tilecounts(int32_t n_cols, const int32_t *__restrict__ cols,
-                                         const int32_t *__restrict__ dim, int64_t *__restrict__ tiles,
-                                         int32_t *__restrict__ n_parts) {
+static __global__ void k_umma_tilecounts(int32_t n_cols, int32_t R, int32_t parts_per_tile,
+                                         const int32_t *__restrict__ cols, const int32_t *__restrict__ dim,
+                                         int64_t *__restrict__ tiles, int32_t *__restrict__ n_parts) {
   int32_t c = blockIdx.x * blockDim.x + threadIdx.x;
   if (c >= n_cols) return;
   int32_t m = dim[cols ? cols[c] : c];
-  int32_t nt = u_tiles(m);
+  int32_t nt = u_tiles(m, R);
   tiles[c] = nt;
-  n_parts[c] = nt * EPI_WARPS;
+  n_parts[c] = nt * parts_per_tile;
 }
 
 struct UmmaWs {
@@ -405,11 +467,23 @@ struct UmmaWs {
   int32_t parts_per_col; int64_t used;
 };
 
+// CTAs per tile: 2 (CTA pairs, cta_group::2) unless SM_UMMA_NCTA=1 is set in the environment
+// (kept for A/B measurements; both back ends produce the same tiles' worth of results).
+static int32_t umma_ncta() {
+  static int32_t v = 0;
+  if (v == 0) {
+    const char *e = getenv("SM_UMMA_NCTA");
+    v = (e && e[0] == '1') ? 1 : 2;
+  }
+  return v;
+}
+
 static UmmaWs umma_layout(void *ws, int64_t ws_bytes, const sm_pattern_t *P, int32_t n_cols,
                           int64_t packed_elems) {
   WsCursor cur(ws, ws_bytes);
   UmmaWs w;
-  w.parts_per_col = u_Tm(P->max_dim) * u_Tn(P->max_dim) * EPI_WARPS;
+  const int32_t ncta = umma_ncta(), max_tiles = u_tiles(P->max_dim, UM * ncta);
+  w.parts_per_col = max_tiles * EPI_WARPS * ncta;
   w.Y = cur.take<char>(packed_elems * 2);
   w.X2 = cur.take<char>(packed_elems * 2);
   w.active = cur.take<int32_t>(n_cols);
@@ -419,7 +493,7 @@ static UmmaWs umma_layout(void *ws, int64_t ws_bytes, const sm_pattern_t *P, int
   w.n_parts = cur.take<int32_t>(n_cols);
   w.tile_ptr = cur.take<int64_t>(n_cols + 1);
   w.partial = cur.take<double>((int64_t)n_cols * w.parts_per_col);
-  w.tiles = cur.take<TileDesc>((int64_t)n_cols * u_Tm(P->max_dim) * u_Tn(P->max_dim));
+  w.tiles = cur.take<TileDesc>((int64_t)n_cols * max_tiles);
   w.used = cur.used + 256;
   return w;
 }
@@ -438,12 +512,12 @@ struct GemmProfile {
 };
 static GemmProfile g_prof;
 
-template <bool BF16, int PHASE>
-static int32_t launch_umma(const UArgs &a, int32_t grid, cudaStream_t st) {
+template <bool BF16, int PHASE, int NCTA>
+static int32_t launch_umma(const UArgs &a, int32_t n_sm, cudaStream_t st) {
   static bool configured = false;
   if (!configured) {
-    SM_CUDA(cudaFuncSetAttribute(k_umma_gemm<BF16, PHASE>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 UMMA_SMEM));
+    SM_CUDA(cudaFuncSetAttribute(k_umma_gemm<BF16, PHASE, NCTA>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 UCfg<NCTA>::SMEM));
     configured = true;
   }
   std::pair<cudaEvent_t, cudaEvent_t> *pe = nullptr;
@@ -457,10 +531,25 @@ static int32_t launch_umma(const UArgs &a, int32_t grid, cudaStream_t st) {
     pe = &g_prof.ev[g_prof.used++];
     SM_CUDA(cudaEventRecord(pe->first, st));
   }
-  k_umma_gemm<BF16, PHASE><<<grid, UMMA_THREADS, UMMA_SMEM, st>>>(a);
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)(n_sm / NCTA * NCTA), 1, 1);     // one CTA per SM, whole pairs
+  cfg.blockDim = dim3(UMMA_THREADS, 1, 1);
+  cfg.dynamicSmemBytes = UCfg<NCTA>::SMEM;
+  cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeClusterDimension;
+  attr[0].val.clusterDim.x = NCTA; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+  cfg.attrs = attr; cfg.numAttrs = 1;
+  SM_CUDA(cudaLaunchKernelEx(&cfg, k_umma_gemm<BF16, PHASE, NCTA>, a));
   SM_LAUNCHED();
   if (pe) SM_CUDA(cudaEventRecord(pe->second, st));
   return SM_OK;
+}
+
+template <int PHASE>
+static int32_t launch_umma_any(bool bf16, int32_t ncta, const UArgs &a, int32_t n_sm, cudaStream_t st) {
+  if (ncta == 2) return bf16 ? launch_umma<true, PHASE, 2>(a, n_sm, st) : launch_umma<false, PHASE, 2>(a, n_sm, st);
+  return bf16 ? launch_umma<true, PHASE, 1>(a, n_sm, st) : launch_umma<false, PHASE, 1>(a, n_sm, st);
 }
 
 int32_t sign_umma(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, const int64_t *col_off,
@@ -468,6 +557,7 @@ int32_t sign_umma(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, co
                   int32_t max_iter, double tol, int32_t *iters, double *residual, cudaStream_t st) {
   if ((P->pad_to % 64) != 0) return SM_ERR_ARG;
   const bool bf16 = x_dtype == SM_BF16;
+  const int32_t ncta = umma_ncta(), R = UM * ncta;
   UmmaWs w = umma_layout(ws, ws_bytes, P, n_cols, packed_elems);
   if (w.used > ws_bytes) return SM_ERR_SPACE;
   int dev = 0, n_sm = 0;
@@ -477,10 +567,10 @@ int32_t sign_umma(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, co
   const int32_t nb = (n_cols + 255) / 256;
   k_sign_init<<<nb, 256, 0, st>>>(n_cols, w.active, w.last, iters, residual);
   SM_LAUNCHED();
-  k_umma_tilecounts<<<nb, 256, 0, st>>>(n_cols, cols, P->dim, w.tile_ptr, w.n_parts);
+  k_umma_tilecounts<<<nb, 256, 0, st>>>(n_cols, R, EPI_WARPS * ncta, cols, P->dim, w.tile_ptr, w.n_parts);
   SM_LAUNCHED();
   { int32_t rc = exclusive_scan_i64(n_cols, w.tile_ptr, w.tile_ptr, st); if (rc != SM_OK) return rc; }
-  k_umma_build_tiles<<<nb, 256, 0, st>>>(n_cols, cols, P->dim, P->dim_pad, col_off, w.tile_ptr, w.tiles);
+  k_umma_build_tiles<<<nb, 256, 0, st>>>(n_cols, R, cols, P->dim, P->dim_pad, col_off, w.tile_ptr, w.tiles);
   SM_LAUNCHED();
   // Y and the alternate X buffer start as zeros so that padding never holds NaN/Inf bit patterns.
   SM_CUDA(cudaMemsetAsync(w.Y, 0, packed_elems * 2, st));
@@ -490,13 +580,13 @@ int32_t sign_umma(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, co
   for (int32_t k = 0; k < max_iter; ++k) {
     void *src = buf[k & 1], *dst = buf[(k + 1) & 1];
     UArgs a{cols, col_off, P->dim, P->dim_pad, w.tile_ptr, w.tiles, n_cols, tol > 0.0 ? 1 : 0, src, w.Y, w.Y, s, w.err};
-    int32_t rc = bf16 ? launch_umma<true, 1>(a, n_sm, st) : launch_umma<false, 1>(a, n_sm, st);
+    int32_t rc = launch_umma_any<1>(bf16, ncta, a, n_sm, st);
     if (rc != SM_OK) return rc;
     SM_CUDA(cudaMemsetAsync(w.n_still, 0, sizeof(int32_t), st));
     k_sign_post<<<nb, 256, 0, st>>>(n_cols, cols, P->dim, s, w.n_parts, tol, iters, residual);
     SM_LAUNCHED();
     a.Out = dst;
-    rc = bf16 ? launch_umma<true, 2>(a, n_sm, st) : launch_umma<false, 2>(a, n_sm, st);
+    rc = launch_umma_any<2>(bf16, ncta, a, n_sm, st);
     if (rc != SM_OK) return rc;
     if (tol > 0.0 && k >= 5 && (k & 1)) {
       int32_t still = 1;
