@@ -73,6 +73,7 @@ struct UArgs {
   const void *Xsrc; const void *Ybuf; void *Out;
   SignState s;
   int32_t *err_flag;
+  int32_t dbg;               // measurement only (SM_UMMA_DBG): 1 = skip output stores, 2 = skip MMA issue, 4 = skip TMA loads
 };
 
 // Tile geometry.  Only elements (r, c) with c <= r are computed, so tile row tm (rows tm*R ..
@@ -81,8 +82,8 @@ struct UArgs {
 __host__ __device__ inline int32_t u_n16(int32_t m) { return (m + 15) & ~15; }
 __host__ __device__ inline int32_t u_Tm(int32_t m, int32_t R) { return (m + R - 1) / R; }
 __host__ __device__ inline int32_t u_ncols(int32_t m, int32_t R, int32_t tm) {
-  int32_t n16 = u_n16(m), e = tm * R + R;
-  return e < n16 ? e : n16;
+  int32_t n32 = (m + 31) & ~31, e = tm * R + R;     // whole 32-column epilogue blocks (n32 <= Pd: zero padding)
+  return e < n32 ? e : n32;
 }
 __host__ __device__ inline int32_t u_row_tiles(int32_t m, int32_t R, int32_t tm) {
   return (u_ncols(m, R, tm) + UN - 1) / UN;
@@ -96,6 +97,13 @@ __host__ __device__ inline int32_t u_tiles(int32_t m, int32_t R) {
   for (int32_t tm = 0; tm < u_Tm(m, R); ++tm) t += u_row_tiles(m, R, tm);
   return t;
 }
+
+// FULL mode (true products, no symmetry): every 128*NCTA-row panel of the Pd x Pd image times all Pd
+// columns, in tiles of 256 columns (the last one takes the rest, rounded up to whole 64-column
+// swizzle atoms per CTA).
+__host__ __device__ inline int32_t f_Tm(int32_t Pd, int32_t R) { return (Pd + R - 1) / R; }
+__host__ __device__ inline int32_t f_Tn(int32_t Pd) { return (Pd + UN - 1) / UN; }
+__host__ __device__ inline int32_t f_tiles(int32_t Pd, int32_t R) { return f_Tm(Pd, R) * f_Tn(Pd); }
 
 __device__ __forceinline__ TileDesc load_desc(const UArgs &a, int64_t t) {
   const uint4 *p = reinterpret_cast<const uint4 *>(a.tiles + t);
@@ -123,23 +131,33 @@ __device__ __forceinline__ UTile make_tile(const UArgs &a, const TileDesc &d) {
   return u;
 }
 
-static __global__ void k_umma_build_tiles(int32_t n_cols, int32_t R, const int32_t *__restrict__ cols,
+static __global__ void k_umma_build_tiles(int32_t n_cols, int32_t R, int32_t sym, const int32_t *__restrict__ cols,
                                           const int32_t *__restrict__ dim, const int32_t *__restrict__ dim_pad,
                                           const int64_t *__restrict__ col_off,
                                           const int64_t *__restrict__ tile_ptr, TileDesc *__restrict__ tiles) {
   int32_t c = blockIdx.x * blockDim.x + threadIdx.x;
   if (c >= n_cols) return;
   int32_t i = cols ? cols[c] : c;
-  int32_t m = dim[i];
+  int32_t m = dim[i], Pd = dim_pad[i];
   TileDesc d;
-  d.base = col_off[c]; d.c = c; d.m = m; d.Pd = dim_pad[i]; d.pad0 = d.pad1 = d.pad2 = 0;
+  d.base = col_off[c]; d.c = c; d.m = m; d.Pd = Pd; d.pad0 = d.pad1 = d.pad2 = 0;
   int64_t t = tile_ptr[c];
   int32_t lt = 0;
-  for (int32_t tm = 0; tm < u_Tm(m, R); ++tm) {
-    int32_t cnt = u_row_tiles(m, R, tm), nb = u_row_nb(m, R, tm), nc = u_ncols(m, R, tm);
-    for (int32_t tn = 0; tn < cnt; ++tn, ++lt, ++t) {
-      d.row0 = tm * R; d.n0 = tn * nb; d.nt = min(nb, nc - d.n0); d.lt = lt;
-      tiles[t] = d;
+  if (sym) {
+    for (int32_t tm = 0; tm < u_Tm(m, R); ++tm) {
+      int32_t cnt = u_row_tiles(m, R, tm), nb = u_row_nb(m, R, tm), nc = u_ncols(m, R, tm);
+      for (int32_t tn = 0; tn < cnt; ++tn, ++lt, ++t) {
+        d.row0 = tm * R; d.n0 = tn * nb; d.nt = min(nb, nc - d.n0); d.lt = lt;
+        tiles[t] = d;
+      }
+    }
+  } else {
+    const int32_t q = R / 2;                      // 64 columns per CTA of the tile: whole swizzle atoms
+    for (int32_t tm = 0; tm < f_Tm(Pd, R); ++tm) {
+      for (int32_t tn = 0; tn < f_Tn(Pd); ++tn, ++lt, ++t) {
+        d.row0 = tm * R; d.n0 = tn * UN; d.nt = min(UN, (Pd - d.n0 + q - 1) / q * q); d.lt = lt;
+        tiles[t] = d;
+      }
     }
   }
 }
@@ -161,7 +179,12 @@ template <> __device__ __forceinline__ float2 unpack2<false>(uint32_t w) {
   return __half22float2(*reinterpret_cast<__half2 *>(&w));
 }
 
-template <bool BF16, int PHASE, int NCTA>
+// SYM = true : K-major B (X X^T form), lower-triangle tiles, mirrored stores (exactly symmetric iterates).
+// SYM = false: MN-major B (true products X X and X Y), all tiles, plain row stores.  The true-product
+//              form damps (++ block) or leaves unchanged (+- block) an antisymmetric rounding residue,
+//              so exact symmetry is not needed; it trades 1.3-1.7x more MMA work for an epilogue
+//              without transposes, which is what bounds the m < ~1000 regime (ncu, round 1).
+template <bool BF16, int PHASE, int NCTA, bool SYM>
 __global__ void __launch_bounds__(UMMA_THREADS, 1) k_umma_gemm(UArgs a) {
   using Cfg = UCfg<NCTA>;
   constexpr int USTAGES = Cfg::STAGES;
@@ -221,16 +244,31 @@ __global__ void __launch_bounds__(UMMA_THREADS, 1) k_umma_gemm(UArgs a) {
         const char *Bg = (const char *)(PHASE == 1 ? a.Xsrc : a.Ybuf) + u.base * ESZ;
         const int32_t arow0 = u.row0 + (int32_t)h * UM;
         const uint32_t a_rows = (uint32_t)max(0, min(UM, u.Pd - arow0));
-        const int32_t b_cnt = u.nt / NCTA, brow0 = u.n0 + (int32_t)h * b_cnt;
-        const uint32_t a_bytes = a_rows * 128u, b_bytes = (uint32_t)b_cnt * 128u;
+        const int32_t b_cnt = u.nt / NCTA, brow0 = u.n0 + (int32_t)h * b_cnt;   // this CTA's share of B
+        // FULL mode: whole 64-column atoms of the image; atoms past the padded dimension are not loaded
+        // (their accumulator columns are garbage and never stored).
+        const int32_t atom0 = brow0 >> 6, n_atoms = max(0, min(b_cnt >> 6, (u.Pd >> 6) - atom0));
+        const uint32_t a_bytes = a_rows * 128u;
+        const uint32_t b_bytes = SYM ? (uint32_t)b_cnt * 128u : (uint32_t)n_atoms * 8192u;
         const int nkc = (u.kmax + UK - 1) / UK;
         for (int kc = 0; kc < nkc; ++kc) {
           ptx::mbar_wait(empty_bar(stage), phase ^ 1u, a.err_flag, 1);
           const uint32_t sa = tiles + stage * STAGE_BYTES, sb = sa + A_BYTES;
+          if (a.dbg & 4) {
+            ptx::mbar_arrive(full_bar(stage));
+            if (++stage == USTAGES) { stage = 0; phase ^= 1u; }
+            continue;
+          }
           ptx::mbar_expect_tx(full_bar(stage), a_bytes + b_bytes);
           const int64_t chunk = (int64_t)kc * u.Pd * 128;     // byte offset of k chunk kc
           if (a_bytes) ptx::tma_bulk_g2s(sa, Ag + chunk + (int64_t)arow0 * 128, a_bytes, full_bar(stage));
-          ptx::tma_bulk_g2s(sb, Bg + chunk + (int64_t)brow0 * 128, b_bytes, full_bar(stage));
+          if (SYM) {
+            ptx::tma_bulk_g2s(sb, Bg + chunk + (int64_t)brow0 * 128, b_bytes, full_bar(stage));
+          } else {
+            for (int32_t j = 0; j < n_atoms; ++j)    // rows k of chunk-column (atom0 + j): 64 x 128 B
+              ptx::tma_bulk_g2s(sb + (uint32_t)j * 8192u,
+                                Bg + ((int64_t)(atom0 + j) * u.Pd + (int64_t)kc * UK) * 128, 8192u, full_bar(stage));
+          }
           if (++stage == USTAGES) { stage = 0; phase ^= 1u; }
         }
       }
@@ -268,7 +306,7 @@ __global__ void __launch_bounds__(UMMA_THREADS, 1) k_umma_gemm(UArgs a) {
         ptx::mbar_wait(tempty_bar(as), aphase ^ 1u, a.err_flag, 2);
         ptx::tc_fence_after();
         const uint32_t d_tmem = tmem_base + as * UN;
-        const uint32_t idesc = ptx::make_idesc_f16(BF16, UM * NCTA, (uint32_t)u.nt);
+        const uint32_t idesc = ptx::make_idesc_f16(BF16, UM * NCTA, (uint32_t)u.nt, !SYM);
         const int nkc = (u.kmax + UK - 1) / UK;
         for (int kc = 0; kc < nkc; ++kc) {
           ptx::mbar_wait(full_bar(stage), phase, a.err_flag, 3);
@@ -276,15 +314,16 @@ __global__ void __launch_bounds__(UMMA_THREADS, 1) k_umma_gemm(UArgs a) {
           ptx::tc_fence_after();
           const uint32_t sa = tiles + stage * STAGE_BYTES, sb = sa + A_BYTES;
           const uint64_t adesc = ptx::make_sw128_kmajor_desc(sa);
-          const uint64_t bdesc = ptx::make_sw128_kmajor_desc(sb);
+          const uint64_t bdesc = SYM ? ptx::make_sw128_kmajor_desc(sb) : ptx::make_sw128_mnmajor_desc(sb, 8192u, 1024u);
+          const uint64_t bstep = SYM ? 2u : 128u;   // 16 k: 32 B inside a K-major atom / 16 rows of 128 B
           const int ksteps = min(UK / 16, (u.kmax - kc * UK) / 16);
-          for (int ks = 0; ks < ksteps; ++ks) {
+          for (int ks = 0; ks < ((a.dbg & 2) ? 0 : ksteps); ++ks) {
             // advance 16 elements = 32 bytes inside the swizzle atom: +2 in the (addr >> 4) field
             if (PAIR)
-              ptx::umma_f16_2cta(d_tmem, adesc + (uint64_t)(2 * ks), bdesc + (uint64_t)(2 * ks), idesc,
+              ptx::umma_f16_2cta(d_tmem, adesc + (uint64_t)(2 * ks), bdesc + bstep * (uint64_t)ks, idesc,
                                  (uint32_t)((kc | ks) != 0));
             else
-              ptx::umma_f16(d_tmem, adesc + (uint64_t)(2 * ks), bdesc + (uint64_t)(2 * ks), idesc,
+              ptx::umma_f16(d_tmem, adesc + (uint64_t)(2 * ks), bdesc + bstep * (uint64_t)ks, idesc,
                             (uint32_t)((kc | ks) != 0));
           }
           // frees the smem slot (in both CTAs of a pair) when these MMAs finish
@@ -320,107 +359,122 @@ __global__ void __launch_bounds__(UMMA_THREADS, 1) k_umma_gemm(UArgs a) {
       const int32_t r = R0 + lane;
       uint16_t *Og = (uint16_t *)a.Out + u.base;
       const uint16_t *Xg = (const uint16_t *)a.Xsrc + u.base;
+      if (a.dbg & 1) Og = nullptr;
       const int nblk = (u.nt + 31) >> 5;
       ptx::mbar_wait(tfull_bar(as), aphase, a.err_flag, 4);
       ptx::tc_fence_after();
       const uint32_t taddr = tmem_base + as * UN + ((uint32_t)(q * 32) << 16);
-      float res = 0.f;
+      float res = 0.f, res2 = 0.f;                             // diagonal-block / off-diagonal (counted twice) sums
       if (R0 < u.Pd) {
+        const uint32_t r7 = (uint32_t)lane & 7u;                 // r & 7 (R0 is a multiple of 32)
         for (int bi = sub; bi < nblk; bi += NSUB) {
           const int32_t C0 = u.n0 + bi * 32;
-          if (C0 > R0) break;                                    // block above the diagonal
-          const int w = min(32, u.nt - bi * 32);                 // 16 or 32 columns
+          if (SYM ? (C0 > R0) : (C0 >= u.Pd)) break;             // above the diagonal / past the padded dimension
           uint32_t v[32];
           ptx::tmem_ld16(taddr + (uint32_t)(bi * 32), *reinterpret_cast<uint32_t(*)[16]>(&v[0]));
-          if (w == 32) ptx::tmem_ld16(taddr + (uint32_t)(bi * 32 + 16), *reinterpret_cast<uint32_t(*)[16]>(&v[16]));
+          ptx::tmem_ld16(taddr + (uint32_t)(bi * 32 + 16), *reinterpret_cast<uint32_t(*)[16]>(&v[16]));
+          // element offset of (r, C0) in the image and the swizzled positions of its four 16-byte chunks
+          const int64_t rowoff = (int64_t)(C0 >> 6) * u.Pd * 64 + (int64_t)r * 64;
+          const uint32_t c8 = ((uint32_t)C0 >> 3) & 4u;          // first chunk of the block inside its 128-byte line
           uint4 xo[4];
           if (PHASE == 2) {
 #pragma unroll
             for (int g = 0; g < 4; ++g)
-              if (g * 8 < w) xo[g] = *reinterpret_cast<const uint4 *>(Xg + img_off(u.Pd, r, C0 + g * 8));
+              xo[g] = *reinterpret_cast<const uint4 *>(Xg + rowoff + (((c8 + g) ^ r7) << 3));
           }
           ptx::tmem_ld_wait();
           const bool diag = (C0 == R0);
           uint32_t o[16];                                        // 32 output elements, packed pairs
+          float acc = 0.f;
 #pragma unroll
           for (int g = 0; g < 4; ++g) {
-            if (g * 8 < w) {
-              float f[8];
+            float f[8];
 #pragma unroll
-              for (int e = 0; e < 8; ++e) f[e] = __uint_as_float(v[g * 8 + e]);
-              if (PHASE == 1) {
-                if (r < u.m) {
-                  if (!diag) {
+            for (int e = 0; e < 8; ++e) f[e] = __uint_as_float(v[g * 8 + e]);
+            if (PHASE == 1) {
+              if (SYM && diag) {
 #pragma unroll
-                    for (int e = 0; e < 8; ++e) res = fmaf(2.f * f[e], f[e], res);   // (r,c) and (c,r)
-                  } else {
-#pragma unroll
-                    for (int e = 0; e < 8; ++e) {
-                      const int j = g * 8 + e;
-                      const float d = f[e] - (j == lane ? 1.f : 0.f);
-                      if (j <= lane) res = fmaf(j == lane ? d : 2.f * d, d, res);
-                    }
-                  }
+                for (int e = 0; e < 8; ++e) {
+                  const int j = g * 8 + e;
+                  const float d = f[e] - (j == lane ? 1.f : 0.f);
+                  if (j <= lane) acc = fmaf(j == lane ? d : 2.f * d, d, acc);
                 }
               } else {
-                const uint32_t *xw = reinterpret_cast<const uint32_t *>(&xo[g]);
 #pragma unroll
-                for (int e2 = 0; e2 < 4; ++e2) {
-                  const float2 x = unpack2<BF16>(xw[e2]);
-                  f[2 * e2] = 1.5f * x.x - 0.5f * f[2 * e2];
-                  f[2 * e2 + 1] = 1.5f * x.y - 0.5f * f[2 * e2 + 1];
+                for (int e = 0; e < 8; ++e) {
+                  const float d = (!SYM && diag && g * 8 + e == lane) ? f[e] - 1.f : f[e];
+                  acc = fmaf(d, d, acc);
                 }
               }
+            } else {
+              const uint32_t *xw = reinterpret_cast<const uint32_t *>(&xo[g]);
 #pragma unroll
-              for (int e2 = 0; e2 < 4; ++e2) o[g * 4 + e2] = pack2<BF16>(f[2 * e2], f[2 * e2 + 1]);
+              for (int e2 = 0; e2 < 4; ++e2) {
+                const float2 x = unpack2<BF16>(xw[e2]);
+                f[2 * e2] = 1.5f * x.x - 0.5f * f[2 * e2];
+                f[2 * e2 + 1] = 1.5f * x.y - 0.5f * f[2 * e2 + 1];
+              }
             }
+#pragma unroll
+            for (int e2 = 0; e2 < 4; ++e2) o[g * 4 + e2] = pack2<BF16>(f[2 * e2], f[2 * e2 + 1]);
           }
-          if (diag) {
+          if (PHASE == 1 && r < u.m) { if (SYM && !diag) res2 += acc; else res += acc; }
+          uint16_t *Orow = Og ? Og + rowoff : nullptr;
+          if (!SYM) {
+            if (Orow) {
+#pragma unroll
+              for (int g = 0; g < 4; ++g)
+                *reinterpret_cast<uint4 *>(Orow + (((c8 + g) ^ r7) << 3)) =
+                    make_uint4(o[g * 4], o[g * 4 + 1], o[g * 4 + 2], o[g * 4 + 3]);
+            }
+          } else if (diag) {
             // S[row][col] in smem; then element (row, j > row) is replaced by element (j, row)
 #pragma unroll
             for (int g = 0; g < 4; ++g)
-              if (g * 8 < w)
-                *reinterpret_cast<uint4 *>(stg + lane * 32 + ((g ^ (lane & 3)) << 3)) =
-                    make_uint4(o[g * 4], o[g * 4 + 1], o[g * 4 + 2], o[g * 4 + 3]);
+              *reinterpret_cast<uint4 *>(stg + lane * 32 + ((g ^ (lane & 3)) << 3)) =
+                  make_uint4(o[g * 4], o[g * 4 + 1], o[g * 4 + 2], o[g * 4 + 3]);
             __syncwarp();
-            if (lane < w) {
 #pragma unroll
-              for (int j = 0; j < 32; ++j) {
-                if (j > lane && j < w) {
-                  // element (j, lane) sits in row j, chunk (lane >> 3) ^ (j & 3), position lane & 7
-                  const uint16_t m16 = stg[j * 32 + (((lane >> 3) ^ (j & 3)) << 3) + (lane & 7)];
-                  o[j >> 1] = (j & 1) ? ((o[j >> 1] & 0x0000FFFFu) | ((uint32_t)m16 << 16))
-                                      : ((o[j >> 1] & 0xFFFF0000u) | (uint32_t)m16);
-                }
+            for (int j = 0; j < 32; ++j) {
+              if (j > lane) {
+                // element (j, lane) sits in row j, chunk (lane >> 3) ^ (j & 3), position lane & 7
+                const uint16_t m16 = stg[j * 32 + (((lane >> 3) ^ (j & 3)) << 3) + (lane & 7)];
+                o[j >> 1] = (j & 1) ? ((o[j >> 1] & 0x0000FFFFu) | ((uint32_t)m16 << 16))
+                                    : ((o[j >> 1] & 0xFFFF0000u) | (uint32_t)m16);
               }
             }
             __syncwarp();
+            if (Orow) {
 #pragma unroll
-            for (int g = 0; g < 4; ++g)
-              if (g * 8 < w)
-                *reinterpret_cast<uint4 *>(Og + img_off(u.Pd, r, C0 + g * 8)) =
+              for (int g = 0; g < 4; ++g)
+                *reinterpret_cast<uint4 *>(Orow + (((c8 + g) ^ r7) << 3)) =
                     make_uint4(o[g * 4], o[g * 4 + 1], o[g * 4 + 2], o[g * 4 + 3]);
+            }
           } else {
 #pragma unroll
             for (int g = 0; g < 4; ++g) {
-              if (g * 8 < w) {
-                *reinterpret_cast<uint4 *>(Og + img_off(u.Pd, r, C0 + g * 8)) =
+              if (Orow)
+                *reinterpret_cast<uint4 *>(Orow + (((c8 + g) ^ r7) << 3)) =
                     make_uint4(o[g * 4], o[g * 4 + 1], o[g * 4 + 2], o[g * 4 + 3]);
 #pragma unroll
-                for (int e = 0; e < 8; ++e)                      // transposed: [col][row]
-                  stg[(g * 8 + e) * 32 + lane] = (uint16_t)(o[g * 4 + (e >> 1)] >> ((e & 1) * 16));
-              }
+              for (int e = 0; e < 8; ++e)                        // transposed: [col][row]
+                stg[(g * 8 + e) * 32 + lane] = (uint16_t)(o[g * 4 + (e >> 1)] >> ((e & 1) * 16));
             }
             __syncwarp();
-            for (int id = lane; id < w * 4; id += 32) {          // 16-byte chunks of the transposed block
-              const int c = id >> 2, j = id & 3;
-              const uint4 val = *reinterpret_cast<const uint4 *>(stg + id * 8);
-              *reinterpret_cast<uint4 *>(Og + img_off(u.Pd, C0 + c, R0 + 8 * j)) = val;
+            // mirrored block: rows C0 + c (c = lane/4 + 8 i), columns R0 + 8 j (j = lane % 4), 16 bytes each
+            const uint32_t mpos = ((((uint32_t)R0 >> 3) & 4u) + ((uint32_t)lane & 3u)) ^ (((uint32_t)lane >> 2) & 7u);
+            uint16_t *Mp = Og ? Og + (int64_t)(R0 >> 6) * u.Pd * 64 + (int64_t)(C0 + (lane >> 2)) * 64 + (mpos << 3)
+                              : nullptr;
+            if (Mp) {
+#pragma unroll
+              for (int i = 0; i < 4; ++i)
+                *reinterpret_cast<uint4 *>(Mp + i * 512) = *reinterpret_cast<const uint4 *>(stg + lane * 8 + i * 256);
             }
             __syncwarp();
           }
         }
       }
+      res += 2.f * res2;
       // accumulator drained: hand the TMEM stage back to the MMA warp
       ptx::tc_fence_before();
       __syncwarp();
@@ -450,13 +504,14 @@ __global__ void __launch_bounds__(UMMA_THREADS, 1) k_umma_gemm(UArgs a) {
 
 namespace sm {
 
-static __global__ void k_umma_tilecounts(int32_t n_cols, int32_t R, int32_t parts_per_tile,
+static __global__ void k_umma_tilecounts(int32_t n_cols, int32_t R, int32_t sym, int32_t parts_per_tile,
                                          const int32_t *__restrict__ cols, const int32_t *__restrict__ dim,
-                                         int64_t *__restrict__ tiles, int32_t *__restrict__ n_parts) {
+                                         const int32_t *__restrict__ dim_pad, int64_t *__restrict__ tiles,
+                                         int32_t *__restrict__ n_parts) {
   int32_t c = blockIdx.x * blockDim.x + threadIdx.x;
   if (c >= n_cols) return;
-  int32_t m = dim[cols ? cols[c] : c];
-  int32_t nt = u_tiles(m, R);
+  int32_t i = cols ? cols[c] : c;
+  int32_t nt = sym ? u_tiles(dim[i], R) : f_tiles(dim_pad[i], R);
   tiles[c] = nt;
   n_parts[c] = nt * parts_per_tile;
 }
@@ -467,22 +522,45 @@ struct UmmaWs {
   int32_t parts_per_col; int64_t used;
 };
 
-// CTAs per tile: 2 (CTA pairs, cta_group::2) unless SM_UMMA_NCTA=1 is set in the environment
-// (kept for A/B measurements; both back ends produce the same tiles' worth of results).
-static int32_t umma_ncta() {
-  static int32_t v = 0;
-  if (v == 0) {
+// CTAs per tile.  Measured on B200: CTA pairs (cta_group::2, 256-row tiles) win where a tile's main loop
+// is long (configs[4], m ~ 1650: 15.1 vs 16.3 ms per launch), single CTAs win where the per-tile
+// epilogue and hand-offs dominate (configs[2], m ~ 410: 0.77 vs 0.85 ms).  Decided per call from the
+// pattern's largest submatrix; SM_UMMA_NCTA=1/2 in the environment overrides (A/B measurements).
+static int32_t umma_ncta(const sm_pattern_t *P) {
+  static int32_t env = -2;
+  if (env == -2) {
     const char *e = getenv("SM_UMMA_NCTA");
-    v = (e && e[0] == '1') ? 1 : 2;
+    env = e ? (e[0] == '1' ? 1 : 2) : -1;
   }
-  return v;
+  if (env > 0) return env;
+  return P->max_dim > 1024 ? 2 : 1;
+}
+
+// SYM (triangular tiles, mirrored stores) for large submatrices, where the symmetric half of the MMA
+// work is worth more than the transposing epilogue costs; FULL (true products) below.  Decided per
+// call from the pattern's largest submatrix; SM_UMMA_SYM=0/1 in the environment overrides.
+static int32_t umma_sym(const sm_pattern_t *P) {
+  static int32_t env = -2;
+  if (env == -2) {
+    const char *e = getenv("SM_UMMA_SYM");
+    env = e ? (e[0] == '1' ? 1 : 0) : -1;
+  }
+  if (env >= 0) return env;
+  (void)P;
+  return 1;     // measured (configs[2], B200): SYM 0.77 ms per launch, FULL 1.13 ms
+}
+
+static int32_t umma_dbg() {
+  const char *e = getenv("SM_UMMA_DBG");
+  return e ? atoi(e) : 0;
 }
 
 static UmmaWs umma_layout(void *ws, int64_t ws_bytes, const sm_pattern_t *P, int32_t n_cols,
                           int64_t packed_elems) {
   WsCursor cur(ws, ws_bytes);
   UmmaWs w;
-  const int32_t ncta = umma_ncta(), max_tiles = u_tiles(P->max_dim, UM * ncta);
+  const int32_t ncta = umma_ncta(P);
+  const int32_t max_tiles = umma_sym(P) ? u_tiles(P->max_dim, UM * ncta) : f_tiles(P->max_dim_pad, UM * ncta);
   w.parts_per_col = max_tiles * EPI_WARPS * ncta;
   w.Y = cur.take<char>(packed_elems * 2);
   w.X2 = cur.take<char>(packed_elems * 2);
@@ -512,11 +590,11 @@ struct GemmProfile {
 };
 static GemmProfile g_prof;
 
-template <bool BF16, int PHASE, int NCTA>
+template <bool BF16, int PHASE, int NCTA, bool SYM>
 static int32_t launch_umma(const UArgs &a, int32_t n_sm, cudaStream_t st) {
   static bool configured = false;
   if (!configured) {
-    SM_CUDA(cudaFuncSetAttribute(k_umma_gemm<BF16, PHASE, NCTA>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    SM_CUDA(cudaFuncSetAttribute(k_umma_gemm<BF16, PHASE, NCTA, SYM>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                  UCfg<NCTA>::SMEM));
     configured = true;
   }
@@ -540,16 +618,20 @@ static int32_t launch_umma(const UArgs &a, int32_t n_sm, cudaStream_t st) {
   attr[0].id = cudaLaunchAttributeClusterDimension;
   attr[0].val.clusterDim.x = NCTA; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
   cfg.attrs = attr; cfg.numAttrs = 1;
-  SM_CUDA(cudaLaunchKernelEx(&cfg, k_umma_gemm<BF16, PHASE, NCTA>, a));
+  SM_CUDA(cudaLaunchKernelEx(&cfg, k_umma_gemm<BF16, PHASE, NCTA, SYM>, a));
   SM_LAUNCHED();
   if (pe) SM_CUDA(cudaEventRecord(pe->second, st));
   return SM_OK;
 }
 
+template <int PHASE, int NCTA, bool SYM>
+static int32_t launch_umma_t(bool bf16, const UArgs &a, int32_t n_sm, cudaStream_t st) {
+  return bf16 ? launch_umma<true, PHASE, NCTA, SYM>(a, n_sm, st) : launch_umma<false, PHASE, NCTA, SYM>(a, n_sm, st);
+}
 template <int PHASE>
-static int32_t launch_umma_any(bool bf16, int32_t ncta, const UArgs &a, int32_t n_sm, cudaStream_t st) {
-  if (ncta == 2) return bf16 ? launch_umma<true, PHASE, 2>(a, n_sm, st) : launch_umma<false, PHASE, 2>(a, n_sm, st);
-  return bf16 ? launch_umma<true, PHASE, 1>(a, n_sm, st) : launch_umma<false, PHASE, 1>(a, n_sm, st);
+static int32_t launch_umma_any(bool bf16, int32_t ncta, int32_t sym, const UArgs &a, int32_t n_sm, cudaStream_t st) {
+  if (ncta == 2) return sym ? launch_umma_t<PHASE, 2, true>(bf16, a, n_sm, st) : launch_umma_t<PHASE, 2, false>(bf16, a, n_sm, st);
+  return sym ? launch_umma_t<PHASE, 1, true>(bf16, a, n_sm, st) : launch_umma_t<PHASE, 1, false>(bf16, a, n_sm, st);
 }
 
 int32_t sign_umma(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, const int64_t *col_off,
@@ -557,7 +639,7 @@ int32_t sign_umma(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, co
                   int32_t max_iter, double tol, int32_t *iters, double *residual, cudaStream_t st) {
   if ((P->pad_to % 64) != 0) return SM_ERR_ARG;
   const bool bf16 = x_dtype == SM_BF16;
-  const int32_t ncta = umma_ncta(), R = UM * ncta;
+  const int32_t ncta = umma_ncta(P), R = UM * ncta, sym = umma_sym(P);
   UmmaWs w = umma_layout(ws, ws_bytes, P, n_cols, packed_elems);
   if (w.used > ws_bytes) return SM_ERR_SPACE;
   int dev = 0, n_sm = 0;
@@ -567,10 +649,11 @@ int32_t sign_umma(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, co
   const int32_t nb = (n_cols + 255) / 256;
   k_sign_init<<<nb, 256, 0, st>>>(n_cols, w.active, w.last, iters, residual);
   SM_LAUNCHED();
-  k_umma_tilecounts<<<nb, 256, 0, st>>>(n_cols, R, EPI_WARPS * ncta, cols, P->dim, w.tile_ptr, w.n_parts);
+  k_umma_tilecounts<<<nb, 256, 0, st>>>(n_cols, R, sym, EPI_WARPS * ncta, cols, P->dim, P->dim_pad, w.tile_ptr,
+                                        w.n_parts);
   SM_LAUNCHED();
   { int32_t rc = exclusive_scan_i64(n_cols, w.tile_ptr, w.tile_ptr, st); if (rc != SM_OK) return rc; }
-  k_umma_build_tiles<<<nb, 256, 0, st>>>(n_cols, R, cols, P->dim, P->dim_pad, col_off, w.tile_ptr, w.tiles);
+  k_umma_build_tiles<<<nb, 256, 0, st>>>(n_cols, R, sym, cols, P->dim, P->dim_pad, col_off, w.tile_ptr, w.tiles);
   SM_LAUNCHED();
   // Y and the alternate X buffer start as zeros so that padding never holds NaN/Inf bit patterns.
   SM_CUDA(cudaMemsetAsync(w.Y, 0, packed_elems * 2, st));
@@ -579,14 +662,14 @@ int32_t sign_umma(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, co
   void *buf[2] = {X, w.X2};
   for (int32_t k = 0; k < max_iter; ++k) {
     void *src = buf[k & 1], *dst = buf[(k + 1) & 1];
-    UArgs a{cols, col_off, P->dim, P->dim_pad, w.tile_ptr, w.tiles, n_cols, tol > 0.0 ? 1 : 0, src, w.Y, w.Y, s, w.err};
-    int32_t rc = launch_umma_any<1>(bf16, ncta, a, n_sm, st);
+    UArgs a{cols, col_off, P->dim, P->dim_pad, w.tile_ptr, w.tiles, n_cols, tol > 0.0 ? 1 : 0, src, w.Y, w.Y, s, w.err, umma_dbg()};
+    int32_t rc = launch_umma_any<1>(bf16, ncta, sym, a, n_sm, st);
     if (rc != SM_OK) return rc;
     SM_CUDA(cudaMemsetAsync(w.n_still, 0, sizeof(int32_t), st));
     k_sign_post<<<nb, 256, 0, st>>>(n_cols, cols, P->dim, s, w.n_parts, tol, iters, residual);
     SM_LAUNCHED();
     a.Out = dst;
-    rc = launch_umma_any<2>(bf16, ncta, a, n_sm, st);
+    rc = launch_umma_any<2>(bf16, ncta, sym, a, n_sm, st);
     if (rc != SM_OK) return rc;
     if (tol > 0.0 && k >= 5 && (k & 1)) {
       int32_t still = 1;
