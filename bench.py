@@ -237,7 +237,8 @@ def run_ours(args, cfg, cfg_run):
             torch.cuda.synchronize(); a.record(); out = fn(); b.record(); torch.cuda.synchronize()
             return out, a.elapsed_time(b)
         Pn, stages["pattern_ms"] = timed(lambda: sm.sm_build_pattern(A, pad))
-        if max_chunk >= P.packed_elems:
+        free_now, _ = torch.cuda.mem_get_info()
+        if max_chunk >= P.packed_elems and 3.3 * P.packed_elems * eb < free_now:   # X + Y + X' of a separate pass
             cols, col_off, n = sm.sm_plan_columns(Pn, Pn.order)
             (X, sc), stages["gather_ms"] = timed(lambda: sm.sm_gather(A, Pn, cols, col_off, n, 0.0, scale_mode, x_dtype))
             ws = torch.empty(sm.sm_sign_ws_bytes(Pn, n, Pn.packed_elems, x_dtype), dtype=torch.uint8, device="cuda")
@@ -307,7 +308,7 @@ def run_ours(args, cfg, cfg_run):
     else:
         peak = 37.2 if x_dtype == "f64" else 74.4   # 148 SMs x 64 (128) FMA lanes x 2 x 1.965 GHz, DESIGN.md
         achieved = stages.get("sign_tflops", value)
-        roofline = {"bound": "alu", "kernel": "k_simt_gemm", "achieved": achieved, "peak": peak,
+        roofline = {"bound": "alu", "kernel": "k_dmma_gemm" if x_dtype == "f64" else "k_simt_gemm", "achieved": achieved, "peak": peak,
                     "unit": "TFLOP/s", "frac": achieved / peak, "traffic": None,
                     "peak_source": "derived: 148 SMs x FMA lanes x 2 x 1.965 GHz"}
 

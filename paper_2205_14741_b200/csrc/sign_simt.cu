@@ -1,6 +1,8 @@
 // a3, fp32 / fp64 back end: Newton-Schulz X <- 1/2 X (3I - X^2) on row-major packed submatrices
 // with FFMA / DFMA register-tiled products (tcgen05 has no fp32/fp64 kind).  PAPER.md:87 (Eq. 13),
 // :110 (step 2); iteration and stopping rule: DESIGN.md readings A9, A11.
+#include <cstdlib>
+
 #include "sign_state.cuh"
 
 namespace sm {
@@ -102,11 +104,152 @@ k_simt_gemm(const int32_t *__restrict__ cols, const int64_t *__restrict__ col_of
   }
 }
 
-static __global__ void k_simt_nparts(int32_t n_cols, const int32_t *__restrict__ cols,
+// ---- fp64 on the tensor cores: warp-level DMMA (mma.sync.m8n8k4.f64), the only fp64 tensor path sm_100a
+// has (tcgen05 has no f64 kind).  128 x 128 output tile per CTA, 8 warps as 4 x 2, warp tile 32 x 64 =
+// 4 x 8 m8n8 accumulators; operands staged by 16-byte cp.async into a double-buffered ring:
+//   As[128][20]  rows of X, k contiguous (LD = 20: the fragment read row*20 + k is bank-conflict free)
+//   Bs[16][132]  rows k of X (PHASE 1) or Y (PHASE 2), n contiguous (true product, no transposition).
+// Padding rows/columns of X, Y and the alternate buffer hold zeros (gather / memset), so loads are only
+// bounded by the padded dimension.
+constexpr int DT = 128, DK = 16, DLA = 20, DLB = 132;
+constexpr int DMMA_STAGE_DOUBLES = DT * DLA + DK * DLB;
+constexpr int DMMA_SMEM = 2 * DMMA_STAGE_DOUBLES * 8;
+
+__device__ __forceinline__ void dmma_m8n8k4(double (&d)[2], double a, double b) {
+  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};"
+               : "+d"(d[0]), "+d"(d[1])
+               : "d"(a), "d"(b));
+}
+__device__ __forceinline__ void cp_async16(void *smem, const void *gmem, bool valid) {
+  uint32_t sa = (uint32_t)__cvta_generic_to_shared(smem);
+  int32_t n = valid ? 16 : 0;                       // src-size 0: the 16 bytes are zero-filled
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(sa), "l"(gmem), "r"(n) : "memory");
+}
+
+template <int PHASE>
+__global__ void __launch_bounds__(256)
+k_dmma_gemm(const int32_t *__restrict__ cols, const int64_t *__restrict__ col_off,
+            const int32_t *__restrict__ dim, const int32_t *__restrict__ dim_pad, int32_t max_tiles_edge,
+            const double *__restrict__ Xsrc, const double *__restrict__ Ybuf, double *__restrict__ Out,
+            SignState s) {
+  extern __shared__ double dsm[];
+  const int32_t tiles_per = max_tiles_edge * max_tiles_edge;
+  const int32_t c = blockIdx.x / tiles_per, t = blockIdx.x - c * tiles_per;
+  if (!s.active[c]) return;
+  if (PHASE == 1 && s.last[c]) return;
+  const int32_t i = cols ? cols[c] : c;
+  const int32_t m = dim[i], Pd = dim_pad[i];
+  const int32_t te = (m + DT - 1) / DT;
+  const int32_t tr = t / max_tiles_edge, tc = t - tr * max_tiles_edge;
+  if (tr >= te || tc > tr) return;                            // lower-triangle tiles only
+  const double *A = Xsrc + col_off[c];
+  const double *B = (PHASE == 1 ? Xsrc : Ybuf) + col_off[c];
+  double *O = Out + col_off[c];
+  const int32_t row0 = tr * DT, col0 = tc * DT;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int wr = (warp >> 1) * 32, wc = (warp & 1) * 64;      // warp tile origin inside the CTA tile
+  const int g = lane >> 2, q = lane & 3;
+
+  double acc[4][8][2];
+#pragma unroll
+  for (int a = 0; a < 4; ++a)
+#pragma unroll
+    for (int b = 0; b < 8; ++b) acc[a][b][0] = acc[a][b][1] = 0.0;
+
+  auto load_stage = [&](int st, int32_t k0) {
+    double *As = dsm + st * DMMA_STAGE_DOUBLES, *Bs = As + DT * DLA;
+    // A: 128 rows x 8 chunks of 2 doubles
+#pragma unroll
+    for (int l = 0; l < 4; ++l) {
+      int e = threadIdx.x + l * 256;
+      int r = e >> 3, ch = e & 7;
+      int32_t gr = row0 + r, gk = k0 + ch * 2;
+      bool ok = gr < Pd && gk < Pd;
+      cp_async16(As + r * DLA + ch * 2, ok ? A + (int64_t)gr * Pd + gk : A, ok);
+    }
+    // B: 16 k rows x 64 chunks of 2 doubles
+#pragma unroll
+    for (int l = 0; l < 4; ++l) {
+      int e = threadIdx.x + l * 256;
+      int k = e >> 6, ch = e & 63;
+      int32_t gk = k0 + k, gc = col0 + ch * 2;
+      bool ok = gk < Pd && gc < Pd;
+      cp_async16(Bs + k * DLB + ch * 2, ok ? B + (int64_t)gk * Pd + gc : B, ok);
+    }
+    asm volatile("cp.async.commit_group;" ::: "memory");
+  };
+
+  const int32_t nk = (m + DK - 1) / DK;
+  load_stage(0, 0);
+  for (int32_t kc = 0; kc < nk; ++kc) {
+    if (kc + 1 < nk) {
+      load_stage((kc + 1) & 1, (kc + 1) * DK);
+      asm volatile("cp.async.wait_group 1;" ::: "memory");
+    } else {
+      asm volatile("cp.async.wait_group 0;" ::: "memory");
+    }
+    __syncthreads();
+    const double *As = dsm + (kc & 1) * DMMA_STAGE_DOUBLES, *Bs = As + DT * DLA;
+#pragma unroll
+    for (int k4 = 0; k4 < DK; k4 += 4) {
+      double af[4], bf[8];
+#pragma unroll
+      for (int a = 0; a < 4; ++a) af[a] = As[(wr + a * 8 + g) * DLA + k4 + q];
+#pragma unroll
+      for (int b = 0; b < 8; ++b) bf[b] = Bs[(k4 + q) * DLB + wc + b * 8 + g];
+#pragma unroll
+      for (int a = 0; a < 4; ++a)
+#pragma unroll
+        for (int b = 0; b < 8; ++b) dmma_m8n8k4(acc[a][b], af[a], bf[b]);
+    }
+    __syncthreads();
+  }
+
+  // epilogue: lane holds C[row = g][cols 2q, 2q+1] of every 8 x 8 accumulator.  X is symmetric and so are
+  // Y = X X and X' = p(X): only tiles with tc <= tr are computed, an element (r, c <= r) is stored at
+  // (r, c) and mirrored to (c, r), which keeps the iterates exactly symmetric; off-diagonal elements
+  // count twice in the residual.
+  double res = 0.0;
+#pragma unroll
+  for (int a = 0; a < 4; ++a) {
+    const int32_t gr = row0 + wr + a * 8 + g;
+#pragma unroll
+    for (int b = 0; b < 8; ++b) {
+#pragma unroll
+      for (int e = 0; e < 2; ++e) {
+        const int32_t gc = col0 + wc + b * 8 + 2 * q + e;
+        if (gr < m && gc <= gr) {
+          double val = acc[a][b][e];
+          if (PHASE == 1) {
+            const double d = val - (gr == gc ? 1.0 : 0.0);
+            res += (gr == gc ? 1.0 : 2.0) * d * d;
+          } else {
+            val = 1.5 * A[(int64_t)gr * Pd + gc] - 0.5 * val;
+          }
+          O[(int64_t)gr * Pd + gc] = val;
+          if (gc < gr) O[(int64_t)gc * Pd + gr] = val;
+        }
+      }
+    }
+  }
+  if (PHASE == 1) {
+    __shared__ double red[8];
+    for (int d = 16; d > 0; d >>= 1) res += __shfl_xor_sync(0xffffffffu, res, d);
+    if (lane == 0) red[warp] = res;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      double sum = 0.0;
+      for (int w = 0; w < 8; ++w) sum += red[w];
+      s.partial[(int64_t)c * s.parts_per_col + tr * te + tc] = sum;
+    }
+  }
+}
+
+static __global__ void k_tile_nparts(int32_t n_cols, int32_t T, const int32_t *__restrict__ cols,
                                      const int32_t *__restrict__ dim, int32_t *__restrict__ n_parts) {
   int32_t c = blockIdx.x * blockDim.x + threadIdx.x;
   if (c >= n_cols) return;
-  int32_t te = (dim[cols ? cols[c] : c] + ST - 1) / ST;
+  int32_t te = (dim[cols ? cols[c] : c] + T - 1) / T;
   n_parts[c] = te * te;
 }
 
@@ -144,24 +287,53 @@ static int32_t sign_simt_t(const sm_pattern_t *P, const int32_t *cols, int32_t n
   SimtWs w = simt_layout(ws, ws_bytes, P, n_cols, packed_elems, (int32_t)sizeof(T));
   if (w.used > ws_bytes) return SM_ERR_SPACE;
   SignState s{w.active, w.last, w.n_still, w.partial, w.parts_per_col};
-  const int32_t edge = (P->max_dim + ST - 1) / ST;
+  // fp64: DMMA tensor-core tiles of 128 x 128 unless the submatrices are tiny (or SM_F64_BACKEND=simt)
+  static int32_t env_simt = -1;
+  if (env_simt < 0) {
+    const char *e = getenv("SM_F64_BACKEND");
+    env_simt = (e && e[0] == 's') ? 1 : 0;
+  }
+  const bool dmma = sizeof(T) == 8 && !env_simt && P->max_dim > 96;
+  const int32_t TS = dmma ? DT : ST;
+  const int32_t edge = (P->max_dim + TS - 1) / TS;
   const int64_t grid64 = (int64_t)n_cols * edge * edge;
   if (grid64 > 0x7fffffffLL) return SM_ERR_UNSUPPORTED;
   const int32_t grid = (int32_t)grid64, nb = (n_cols + 255) / 256;
   k_sign_init<<<nb, 256, 0, st>>>(n_cols, w.active, w.last, iters, residual);
   SM_LAUNCHED();
-  k_simt_nparts<<<nb, 256, 0, st>>>(n_cols, cols, P->dim, w.n_parts);
+  k_tile_nparts<<<nb, 256, 0, st>>>(n_cols, TS, cols, P->dim, w.n_parts);
   SM_LAUNCHED();
+  if (dmma) {
+    static bool configured = false;
+    if (!configured) {
+      SM_CUDA(cudaFuncSetAttribute(k_dmma_gemm<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, DMMA_SMEM));
+      SM_CUDA(cudaFuncSetAttribute(k_dmma_gemm<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, DMMA_SMEM));
+      configured = true;
+    }
+    // padding of Y and of the alternate X buffer must read as zeros (the kernel stores true elements only)
+    SM_CUDA(cudaMemsetAsync(w.Y, 0, packed_elems * sizeof(T), st));
+    SM_CUDA(cudaMemsetAsync(w.X2, 0, packed_elems * sizeof(T), st));
+    // partial-sum slots of the skipped upper-triangle tiles are never written: they must read as zero
+    SM_CUDA(cudaMemsetAsync(w.partial, 0, (size_t)n_cols * w.parts_per_col * sizeof(double), st));
+  }
   T *buf[2] = {X, (T *)w.X2};
   T *Y = (T *)w.Y;
   for (int32_t k = 0; k < max_iter; ++k) {
     T *src = buf[k & 1], *dst = buf[(k + 1) & 1];
-    k_simt_gemm<T, 1><<<grid, 256, 0, st>>>(cols, col_off, P->dim, P->dim_pad, edge, src, Y, Y, s);
+    if (dmma)
+      k_dmma_gemm<1><<<grid, 256, DMMA_SMEM, st>>>(cols, col_off, P->dim, P->dim_pad, edge, (const double *)src,
+                                                   (const double *)Y, (double *)Y, s);
+    else
+      k_simt_gemm<T, 1><<<grid, 256, 0, st>>>(cols, col_off, P->dim, P->dim_pad, edge, src, Y, Y, s);
     SM_LAUNCHED();
     SM_CUDA(cudaMemsetAsync(w.n_still, 0, sizeof(int32_t), st));
     k_sign_post<<<nb, 256, 0, st>>>(n_cols, cols, P->dim, s, w.n_parts, tol, iters, residual);
     SM_LAUNCHED();
-    k_simt_gemm<T, 2><<<grid, 256, 0, st>>>(cols, col_off, P->dim, P->dim_pad, edge, src, Y, dst, s);
+    if (dmma)
+      k_dmma_gemm<2><<<grid, 256, DMMA_SMEM, st>>>(cols, col_off, P->dim, P->dim_pad, edge, (const double *)src,
+                                                   (const double *)Y, (double *)dst, s);
+    else
+      k_simt_gemm<T, 2><<<grid, 256, 0, st>>>(cols, col_off, P->dim, P->dim_pad, edge, src, Y, dst, s);
     SM_LAUNCHED();
     if (tol > 0.0 && k >= 5 && (k & 1)) {
       // convergence mode: read back how many submatrices continue (the only host sync of the path)

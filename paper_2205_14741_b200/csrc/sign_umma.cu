@@ -29,7 +29,11 @@
 namespace sm {
 
 constexpr int UM = 128;          // tile rows per CTA (UMMA M per CTA)
-constexpr int UN = 256;          // max tile cols (UMMA N)
+#ifndef SM_UN
+#define SM_UN 256
+#endif
+constexpr int UN = SM_UN;        // max tile cols (UMMA N)
+constexpr int NACC = 512 / UN;   // accumulator stages in TMEM (512 columns)
 constexpr int UK = 64;           // k chunk = one 128-byte swizzle row of 16-bit elements
 constexpr int A_BYTES = UM * UK * 2;           // 16 KB
 constexpr int EPI_WARPS = 16;
@@ -201,8 +205,8 @@ __global__ void __launch_bounds__(UMMA_THREADS, 1) k_umma_gemm(UArgs a) {
   auto empty_bar = [&](int s) { return bars + 8u * (USTAGES + s); };
   auto pfull_bar = [&](int s) { return bars + 8u * (2 * USTAGES + s); };
   auto tfull_bar = [&](int s) { return bars + 8u * (3 * USTAGES + s); };
-  auto tempty_bar = [&](int s) { return bars + 8u * (3 * USTAGES + 2 + s); };
-  const uint32_t tmem_slot = bars + 8u * (3 * USTAGES + 4);
+  auto tempty_bar = [&](int s) { return bars + 8u * (3 * USTAGES + NACC + s); };
+  const uint32_t tmem_slot = bars + 8u * (3 * USTAGES + 2 * NACC);
   volatile uint32_t *tmem_slot_ptr =
       reinterpret_cast<volatile uint32_t *>(smem_raw + (tmem_slot - raw));
 
@@ -214,7 +218,7 @@ __global__ void __launch_bounds__(UMMA_THREADS, 1) k_umma_gemm(UArgs a) {
     for (int s = 0; s < USTAGES; ++s) {
       ptx::mbar_init(full_bar(s), 1); ptx::mbar_init(empty_bar(s), 1); ptx::mbar_init(pfull_bar(s), 1);
     }
-    for (int s = 0; s < 2; ++s) { ptx::mbar_init(tfull_bar(s), 1); ptx::mbar_init(tempty_bar(s), EPI_WARPS * NCTA); }
+    for (int s = 0; s < NACC; ++s) { ptx::mbar_init(tfull_bar(s), 1); ptx::mbar_init(tempty_bar(s), EPI_WARPS * NCTA); }
     ptx::fence_barrier_init();
     ptx::fence_proxy_async();
   }
@@ -302,7 +306,7 @@ __global__ void __launch_bounds__(UMMA_THREADS, 1) k_umma_gemm(UArgs a) {
         nxt = load_desc(a, min(t + n_units, total - 1));
         UTile u = make_tile<PHASE>(a, cur);
         if (!u.valid) continue;
-        const uint32_t as = it & 1u, aphase = (it >> 1) & 1u;
+        const uint32_t as = it % NACC, aphase = (it / NACC) & 1u;
         ptx::mbar_wait(tempty_bar(as), aphase ^ 1u, a.err_flag, 2);
         ptx::tc_fence_after();
         const uint32_t d_tmem = tmem_base + as * UN;
@@ -354,7 +358,7 @@ __global__ void __launch_bounds__(UMMA_THREADS, 1) k_umma_gemm(UArgs a) {
       nxt = load_desc(a, min(t + n_units, total - 1));
       UTile u = make_tile<PHASE>(a, cur);
       if (!u.valid) continue;
-      const uint32_t as = it & 1u, aphase = (it >> 1) & 1u;
+      const uint32_t as = it % NACC, aphase = (it / NACC) & 1u;
       const int32_t R0 = u.row0 + (int32_t)h * UM + q * 32;   // this CTA's 128 rows of the tile
       const int32_t r = R0 + lane;
       uint16_t *Og = (uint16_t *)a.Out + u.base;
