@@ -306,11 +306,20 @@ def run_ours(args, cfg, cfg_run):
                     "launches_timed": gemm_launches, "avg_launch_ms": avg_ms,
                     "algorithmic_flops_per_launch": flops_per_launch}
     else:
-        peak = 37.2 if x_dtype == "f64" else 74.4   # 148 SMs x 64 (128) FMA lanes x 2 x 1.965 GHz, DESIGN.md
-        achieved = stages.get("sign_tflops", value)
-        roofline = {"bound": "alu", "kernel": "k_dmma_gemm" if x_dtype == "f64" else "k_simt_gemm", "achieved": achieved, "peak": peak,
-                    "unit": "TFLOP/s", "frac": achieved / peak, "traffic": None,
-                    "peak_source": "derived: 148 SMs x FMA lanes x 2 x 1.965 GHz"}
+        # fp64: DMMA tensor path (k_dmma_gemm); fp32: FFMA (k_simt_gemm).  Peak derived:
+        # 148 SMs x 64 (fp64) / 128 (fp32) FMA per clock x 2 x 1.965 GHz.  Algorithmic FLOPs per launch = the
+        # products actually run: 2 sum_i m_i^3 k_i / (launches / 2 per step) -- convergence mode drops columns.
+        peak = 37.2 if x_dtype == "f64" else 74.4
+        avg_ms = gemm_ms / max(gemm_launches, 1)
+        flops_per_launch = flops_step * args.steps / max(gemm_launches, 1)
+        achieved = flops_per_launch / (avg_ms * 1e-3) / 1e12
+        roofline = {"bound": "alu", "kernel": "k_dmma_gemm" if x_dtype == "f64" else "k_simt_gemm",
+                    "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak, "traffic": None,
+                    "peak_source": "derived: 148 SMs x FMA lanes x 2 x 1.965 GHz",
+                    "launches_timed": gemm_launches, "avg_launch_ms": avg_ms,
+                    "algorithmic_flops_per_launch": flops_per_launch,
+                    "note": "fp64 kernel computes lower-triangle tiles only (symmetric iterates): achieved counts the "
+                            "full 2 m^3 per product and may exceed the derived peak" if x_dtype == "f64" else None}
 
     cpu = None
     if not args.no_cpu_baseline:

@@ -2,6 +2,7 @@
 // gather -> sign -> scatter -> D = 1/2 (I - R), PAPER.md:110 steps 1-3 + PAPER.md:91 Eq. 14, S = I).
 #include <algorithm>
 #include <numeric>
+#include <utility>
 #include <vector>
 
 #include "common.cuh"
@@ -9,6 +10,33 @@
 using namespace sm;
 
 namespace sm {
+// Optional per-launch timing of the dominant kernels (bench.py roofline): CUDA events recorded on the
+// launching stream around every Newton-Schulz product launch while profiling is enabled.
+struct GemmProfile {
+  bool on = false;
+  std::vector<std::pair<cudaEvent_t, cudaEvent_t>> ev;
+  size_t used = 0;
+};
+static GemmProfile g_prof;
+
+int32_t prof_begin(cudaStream_t st, int *slot) {
+  *slot = -1;
+  if (!g_prof.on) return SM_OK;
+  if (g_prof.used == g_prof.ev.size()) {
+    std::pair<cudaEvent_t, cudaEvent_t> e;
+    SM_CUDA(cudaEventCreate(&e.first));
+    SM_CUDA(cudaEventCreate(&e.second));
+    g_prof.ev.push_back(e);
+  }
+  *slot = (int)g_prof.used++;
+  SM_CUDA(cudaEventRecord(g_prof.ev[*slot].first, st));
+  return SM_OK;
+}
+int32_t prof_end(cudaStream_t st, int slot) {
+  if (slot >= 0) SM_CUDA(cudaEventRecord(g_prof.ev[slot].second, st));
+  return SM_OK;
+}
+
 static __global__ void k_count_unconverged(int32_t n, const double *__restrict__ residual, double tol,
                                            int32_t *__restrict__ out) {
   int32_t c = blockIdx.x * blockDim.x + threadIdx.x;
@@ -128,4 +156,25 @@ extern "C" int32_t sm_density(const sm_bcsr_t *A, const void *A_vals, int32_t a_
     if (rc != SM_OK) return rc;
   }
   return sm_density_from_sign(A, P, d_dtype, D_vals, trace, stream);
+}
+
+// ---- profiling hooks (host; see include/submatrix.h) ------------------------------------------
+extern "C" int32_t sm_profile_enable(int32_t on) {
+  sm::g_prof.on = on != 0;
+  sm::g_prof.used = 0;
+  return SM_OK;
+}
+extern "C" int32_t sm_profile_read(double *gemm_ms, int64_t *gemm_launches) {
+  if (!gemm_ms || !gemm_launches) return SM_ERR_ARG;
+  double total = 0.0;
+  for (size_t i = 0; i < sm::g_prof.used; ++i) {
+    SM_CUDA(cudaEventSynchronize(sm::g_prof.ev[i].second));
+    float ms = 0.f;
+    SM_CUDA(cudaEventElapsedTime(&ms, sm::g_prof.ev[i].first, sm::g_prof.ev[i].second));
+    total += ms;
+  }
+  *gemm_ms = total;
+  *gemm_launches = (int64_t)sm::g_prof.used;
+  sm::g_prof.used = 0;
+  return SM_OK;
 }

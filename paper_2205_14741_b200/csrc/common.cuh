@@ -96,6 +96,11 @@ template <> __device__ inline double to_double<float>(float v) { return (double)
 template <> __device__ inline double to_double<__nv_bfloat16>(__nv_bfloat16 v) { return (double)__bfloat162float(v); }
 template <> __device__ inline double to_double<__half>(__half v) { return (double)__half2float(v); }
 
+// ---- measurement hooks (api.cu): CUDA events around every launch of the Newton-Schulz product kernels
+// while sm_profile_enable(1) is in force; slot = -1 when disabled.
+int32_t prof_begin(cudaStream_t st, int *slot);
+int32_t prof_end(cudaStream_t st, int slot);
+
 // ---- internal entry points implemented across the .cu files
 int32_t exclusive_scan_i64(int32_t n, const int64_t *in, int64_t *out, cudaStream_t st);   // pattern.cu
 int32_t power_scale(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, const int64_t *col_off,

@@ -320,21 +320,26 @@ static int32_t sign_simt_t(const sm_pattern_t *P, const int32_t *cols, int32_t n
   T *Y = (T *)w.Y;
   for (int32_t k = 0; k < max_iter; ++k) {
     T *src = buf[k & 1], *dst = buf[(k + 1) & 1];
+    int slot = -1;
+    { int32_t rc = prof_begin(st, &slot); if (rc != SM_OK) return rc; }
     if (dmma)
       k_dmma_gemm<1><<<grid, 256, DMMA_SMEM, st>>>(cols, col_off, P->dim, P->dim_pad, edge, (const double *)src,
                                                    (const double *)Y, (double *)Y, s);
     else
       k_simt_gemm<T, 1><<<grid, 256, 0, st>>>(cols, col_off, P->dim, P->dim_pad, edge, src, Y, Y, s);
     SM_LAUNCHED();
+    { int32_t rc = prof_end(st, slot); if (rc != SM_OK) return rc; }
     SM_CUDA(cudaMemsetAsync(w.n_still, 0, sizeof(int32_t), st));
     k_sign_post<<<nb, 256, 0, st>>>(n_cols, cols, P->dim, s, w.n_parts, tol, iters, residual);
     SM_LAUNCHED();
+    { int32_t rc = prof_begin(st, &slot); if (rc != SM_OK) return rc; }
     if (dmma)
       k_dmma_gemm<2><<<grid, 256, DMMA_SMEM, st>>>(cols, col_off, P->dim, P->dim_pad, edge, (const double *)src,
                                                    (const double *)Y, (double *)dst, s);
     else
       k_simt_gemm<T, 2><<<grid, 256, 0, st>>>(cols, col_off, P->dim, P->dim_pad, edge, src, Y, dst, s);
     SM_LAUNCHED();
+    { int32_t rc = prof_end(st, slot); if (rc != SM_OK) return rc; }
     if (tol > 0.0 && k >= 5 && (k & 1)) {
       // convergence mode: read back how many submatrices continue (the only host sync of the path)
       int32_t still = 1;

@@ -585,15 +585,6 @@ int64_t sign_umma_ws_bytes(const sm_pattern_t *P, int32_t n_cols, int64_t packed
   return umma_layout(nullptr, 0, P, n_cols, packed_elems).used;
 }
 
-// Optional per-launch timing of the dominant kernel (bench.py roofline): CUDA events recorded on
-// the launching stream around every k_umma_gemm launch while profiling is enabled.
-struct GemmProfile {
-  bool on = false;
-  std::vector<std::pair<cudaEvent_t, cudaEvent_t>> ev;
-  size_t used = 0;
-};
-static GemmProfile g_prof;
-
 template <bool BF16, int PHASE, int NCTA, bool SYM>
 static int32_t launch_umma(const UArgs &a, int32_t n_sm, cudaStream_t st) {
   static bool configured = false;
@@ -602,17 +593,8 @@ static int32_t launch_umma(const UArgs &a, int32_t n_sm, cudaStream_t st) {
                                  UCfg<NCTA>::SMEM));
     configured = true;
   }
-  std::pair<cudaEvent_t, cudaEvent_t> *pe = nullptr;
-  if (g_prof.on) {
-    if (g_prof.used == g_prof.ev.size()) {
-      std::pair<cudaEvent_t, cudaEvent_t> e;
-      SM_CUDA(cudaEventCreate(&e.first));
-      SM_CUDA(cudaEventCreate(&e.second));
-      g_prof.ev.push_back(e);
-    }
-    pe = &g_prof.ev[g_prof.used++];
-    SM_CUDA(cudaEventRecord(pe->first, st));
-  }
+  int slot = -1;
+  { int32_t rc = prof_begin(st, &slot); if (rc != SM_OK) return rc; }
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3((unsigned)(n_sm / NCTA * NCTA), 1, 1);     // one CTA per SM, whole pairs
   cfg.blockDim = dim3(UMMA_THREADS, 1, 1);
@@ -624,8 +606,7 @@ static int32_t launch_umma(const UArgs &a, int32_t n_sm, cudaStream_t st) {
   cfg.attrs = attr; cfg.numAttrs = 1;
   SM_CUDA(cudaLaunchKernelEx(&cfg, k_umma_gemm<BF16, PHASE, NCTA, SYM>, a));
   SM_LAUNCHED();
-  if (pe) SM_CUDA(cudaEventRecord(pe->second, st));
-  return SM_OK;
+  return prof_end(st, slot);
 }
 
 template <int PHASE, int NCTA, bool SYM>
@@ -689,24 +670,3 @@ int32_t sign_umma(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, co
 }
 
 }  // namespace sm
-
-// ---- profiling hooks (host; see include/submatrix.h) ------------------------------------------
-extern "C" int32_t sm_profile_enable(int32_t on) {
-  sm::g_prof.on = on != 0;
-  sm::g_prof.used = 0;
-  return SM_OK;
-}
-extern "C" int32_t sm_profile_read(double *gemm_ms, int64_t *gemm_launches) {
-  if (!gemm_ms || !gemm_launches) return SM_ERR_ARG;
-  double total = 0.0;
-  for (size_t i = 0; i < sm::g_prof.used; ++i) {
-    SM_CUDA(cudaEventSynchronize(sm::g_prof.ev[i].second));
-    float ms = 0.f;
-    SM_CUDA(cudaEventElapsedTime(&ms, sm::g_prof.ev[i].first, sm::g_prof.ev[i].second));
-    total += ms;
-  }
-  *gemm_ms = total;
-  *gemm_launches = (int64_t)sm::g_prof.used;
-  sm::g_prof.used = 0;
-  return SM_OK;
-}
