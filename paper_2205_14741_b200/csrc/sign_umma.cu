@@ -77,7 +77,7 @@ struct UArgs {
   const void *Xsrc; const void *Ybuf; void *Out;
   SignState s;
   int32_t *err_flag;
-  int32_t dbg;               // measurement only (SM_UMMA_DBG): 1 = skip output stores, 2 = skip MMA issue, 4 = skip TMA loads
+  int32_t dbg;               // measurement only (SM_UMMA_DBG): 1 = skip output stores, 2 = skip MMA issue, 4 = skip TMA loads, 8 = skip the epilogue's work
 };
 
 // Tile geometry.  Only elements (r, c) with c <= r are computed, so tile row tm (rows tm*R ..
@@ -181,6 +181,15 @@ template <> __device__ __forceinline__ float2 unpack2<true>(uint32_t w) {
 }
 template <> __device__ __forceinline__ float2 unpack2<false>(uint32_t w) {
   return __half22float2(*reinterpret_cast<__half2 *>(&w));
+}
+
+// Row segment of 32 packed outputs (o[4g .. 4g+3] = chunk g) as two full 32-byte sectors.
+__device__ __forceinline__ void store_row_segment(uint16_t *Orow, uint32_t sec0, uint32_t sec1, bool swp,
+                                                  const uint32_t (&o)[16]) {
+  ptx::stg256(Orow + sec0, swp ? o[4] : o[0], swp ? o[5] : o[1], swp ? o[6] : o[2], swp ? o[7] : o[3],
+              swp ? o[0] : o[4], swp ? o[1] : o[5], swp ? o[2] : o[6], swp ? o[3] : o[7]);
+  ptx::stg256(Orow + sec1, swp ? o[12] : o[8], swp ? o[13] : o[9], swp ? o[14] : o[10], swp ? o[15] : o[11],
+              swp ? o[8] : o[12], swp ? o[9] : o[13], swp ? o[10] : o[14], swp ? o[11] : o[15]);
 }
 
 // SYM = true : K-major B (X X^T form), lower-triangle tiles, mirrored stores (exactly symmetric iterates).
@@ -369,7 +378,7 @@ __global__ void __launch_bounds__(UMMA_THREADS, 1) k_umma_gemm(UArgs a) {
       ptx::tc_fence_after();
       const uint32_t taddr = tmem_base + as * UN + ((uint32_t)(q * 32) << 16);
       float res = 0.f, res2 = 0.f;                             // diagonal-block / off-diagonal (counted twice) sums
-      if (R0 < u.Pd) {
+      if (R0 < u.Pd && !(a.dbg & 8)) {
         const uint32_t r7 = (uint32_t)lane & 7u;                 // r & 7 (R0 is a multiple of 32)
         for (int bi = sub; bi < nblk; bi += NSUB) {
           const int32_t C0 = u.n0 + bi * 32;
@@ -380,11 +389,15 @@ __global__ void __launch_bounds__(UMMA_THREADS, 1) k_umma_gemm(UArgs a) {
           // element offset of (r, C0) in the image and the swizzled positions of its four 16-byte chunks
           const int64_t rowoff = (int64_t)(C0 >> 6) * u.Pd * 64 + (int64_t)r * 64;
           const uint32_t c8 = ((uint32_t)C0 >> 3) & 4u;          // first chunk of the block inside its 128-byte line
-          uint4 xo[4];
+          // The four 16-byte chunks of a row segment sit in two 32-byte sectors; chunk 2s and 2s+1 swap places
+          // inside sector s when r is odd (128B swizzle).  One 256-bit access per sector keeps every L2
+          // request a full sector (ncu, round 1: 16-byte accesses doubled the sector count of these paths).
+          const bool swp = (lane & 1) != 0;
+          const uint32_t sec0 = ((c8 ^ r7) & ~1u) << 3, sec1 = (((c8 + 2u) ^ r7) & ~1u) << 3;   // element offsets
+          uint32_t xs[2][8];
           if (PHASE == 2) {
-#pragma unroll
-            for (int g = 0; g < 4; ++g)
-              xo[g] = *reinterpret_cast<const uint4 *>(Xg + rowoff + (((c8 + g) ^ r7) << 3));
+            ptx::ldg256(Xg + rowoff + sec0, xs[0]);
+            ptx::ldg256(Xg + rowoff + sec1, xs[1]);
           }
           ptx::tmem_ld_wait();
           const bool diag = (C0 == R0);
@@ -411,10 +424,11 @@ __global__ void __launch_bounds__(UMMA_THREADS, 1) k_umma_gemm(UArgs a) {
                 }
               }
             } else {
-              const uint32_t *xw = reinterpret_cast<const uint32_t *>(&xo[g]);
 #pragma unroll
               for (int e2 = 0; e2 < 4; ++e2) {
-                const float2 x = unpack2<BF16>(xw[e2]);
+                // chunk g lives in sector g/2, lower half iff (g odd) == swp
+                const uint32_t xw = (((g & 1) != 0) == swp) ? xs[g >> 1][e2] : xs[g >> 1][4 + e2];
+                const float2 x = unpack2<BF16>(xw);
                 f[2 * e2] = 1.5f * x.x - 0.5f * f[2 * e2];
                 f[2 * e2 + 1] = 1.5f * x.y - 0.5f * f[2 * e2 + 1];
               }
@@ -425,12 +439,7 @@ __global__ void __launch_bounds__(UMMA_THREADS, 1) k_umma_gemm(UArgs a) {
           if (PHASE == 1 && r < u.m) { if (SYM && !diag) res2 += acc; else res += acc; }
           uint16_t *Orow = Og ? Og + rowoff : nullptr;
           if (!SYM) {
-            if (Orow) {
-#pragma unroll
-              for (int g = 0; g < 4; ++g)
-                *reinterpret_cast<uint4 *>(Orow + (((c8 + g) ^ r7) << 3)) =
-                    make_uint4(o[g * 4], o[g * 4 + 1], o[g * 4 + 2], o[g * 4 + 3]);
-            }
+            if (Orow) store_row_segment(Orow, sec0, sec1, swp, o);
           } else if (diag) {
             // S[row][col] in smem; then element (row, j > row) is replaced by element (j, row)
 #pragma unroll
@@ -448,18 +457,11 @@ __global__ void __launch_bounds__(UMMA_THREADS, 1) k_umma_gemm(UArgs a) {
               }
             }
             __syncwarp();
-            if (Orow) {
-#pragma unroll
-              for (int g = 0; g < 4; ++g)
-                *reinterpret_cast<uint4 *>(Orow + (((c8 + g) ^ r7) << 3)) =
-                    make_uint4(o[g * 4], o[g * 4 + 1], o[g * 4 + 2], o[g * 4 + 3]);
-            }
+            if (Orow) store_row_segment(Orow, sec0, sec1, swp, o);
           } else {
+            if (Orow) store_row_segment(Orow, sec0, sec1, swp, o);
 #pragma unroll
             for (int g = 0; g < 4; ++g) {
-              if (Orow)
-                *reinterpret_cast<uint4 *>(Orow + (((c8 + g) ^ r7) << 3)) =
-                    make_uint4(o[g * 4], o[g * 4 + 1], o[g * 4 + 2], o[g * 4 + 3]);
 #pragma unroll
               for (int e = 0; e < 8; ++e)                        // transposed: [col][row]
                 stg[(g * 8 + e) * 32 + lane] = (uint16_t)(o[g * 4 + (e >> 1)] >> ((e & 1) * 16));

@@ -168,6 +168,19 @@ __device__ __forceinline__ void umma_commit_2cta(uint32_t bar) {
       : "memory");
 }
 
+// ---- 256-bit global accesses (sm_100+): one full 32-byte L2 sector per lane and instruction ------
+__device__ __forceinline__ void ldg256(const void *p, uint32_t (&r)[8]) {
+  asm volatile("ld.global.v8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
+               : "l"(p));
+}
+__device__ __forceinline__ void stg256(void *p, uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3, uint32_t a4,
+                                       uint32_t a5, uint32_t a6, uint32_t a7) {
+  asm volatile("st.global.v8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(p), "r"(a0), "r"(a1), "r"(a2), "r"(a3),
+               "r"(a4), "r"(a5), "r"(a6), "r"(a7)
+               : "memory");
+}
+
 // ---- descriptors ------------------------------------------------------------------------------
 // Shared-memory matrix descriptor, K-major, 128-byte swizzle: rows are 128 B apart, 8-row groups
 // (1024 B swizzle atoms) follow each other at SBO = 1024 B; LBO is unused for swizzled K-major (1).
