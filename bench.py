@@ -30,6 +30,10 @@ if ROOT not in sys.path:
 
 from workloads.generator import CONFIGS, make_config  # noqa: E402
 
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel (mean of its PHASE 1 / PHASE 2 launches),
+# from the committed `ncu --set full` captures under profiles/ (r1b_ncu_full_k_umma_gemm_cfg{2,4}.md, ..._k_dmma_gemm_cfg1.md).
+NCU_TRAFFIC_BYTES = {(2, "bf16"): 3.33e9, (4, "bf16"): 62.2e9, (1, "f64"): 0.72e9}
+
 METRIC = "submatrix_sign_effective_tflops"
 UNIT = "TFLOP/s"
 
@@ -301,7 +305,8 @@ def run_ours(args, cfg, cfg_run):
         avg_ms = gemm_ms / max(gemm_launches, 1)
         achieved = flops_per_launch / (avg_ms * 1e-3) / 1e12
         roofline = {"bound": "tensor", "kernel": "k_umma_gemm", "achieved": achieved, "peak": peak,
-                    "unit": "TFLOP/s", "frac": achieved / peak, "traffic": None,
+                    "unit": "TFLOP/s", "frac": achieved / peak,
+                    "traffic": NCU_TRAFFIC_BYTES.get((args.config, x_dtype)),
                     "peak_source": f"{peaks['src']} bf16 {'sustained' if long_region else 'burst'}",
                     "launches_timed": gemm_launches, "avg_launch_ms": avg_ms,
                     "algorithmic_flops_per_launch": flops_per_launch}
@@ -314,7 +319,8 @@ def run_ours(args, cfg, cfg_run):
         flops_per_launch = flops_step * args.steps / max(gemm_launches, 1)
         achieved = flops_per_launch / (avg_ms * 1e-3) / 1e12
         roofline = {"bound": "alu", "kernel": "k_dmma_gemm" if x_dtype == "f64" else "k_simt_gemm",
-                    "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak, "traffic": None,
+                    "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
+                    "traffic": NCU_TRAFFIC_BYTES.get((args.config, x_dtype)),
                     "peak_source": "derived: 148 SMs x FMA lanes x 2 x 1.965 GHz",
                     "launches_timed": gemm_launches, "avg_launch_ms": avg_ms,
                     "algorithmic_flops_per_launch": flops_per_launch,

@@ -1,0 +1,75 @@
+"""GPU parity of the alternative back ends of sm_sign_ns that the library selects by size or that the
+environment forces (each in its own process: the selection is read once per process):
+  SM_UMMA_NCTA=1|2   single CTAs / CTA pairs (cta_group::2) per tile of the tcgen05 kernel
+  SM_UMMA_SYM=1|0    symmetric half tiles with mirrored stores / true products with an MN-major B operand
+  SM_F64_BACKEND     DMMA tensor tiles (default) / DFMA register tiles
+Each case runs NS steps on a seeded workload whose submatrices span several tiles and ragged tails and
+compares with the oracle's NS-k polynomial (exact-arithmetic result of k steps, reading A13)."""
+import os
+import subprocess
+import sys
+import textwrap
+
+import pytest
+
+pytestmark = pytest.mark.gpu
+pytest.importorskip("torch")
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+SNIPPET = textwrap.dedent("""
+    import sys, numpy as np, torch
+    sys.path.insert(0, {root!r})
+    import paper_2205_14741_b200.binding as sm
+    from oracle import oracle as orc
+    from workloads.generator import make_workload
+    x_dtype, pad, k, tol_abs, sym_exact = {x_dtype!r}, {pad}, {k}, {tol_abs}, {sym_exact}
+    wl = make_workload({n_mol}, 23, 4, {cutoff}, seed=33)
+    A = sm.Bcsr(wl); P = sm.sm_build_pattern(A, pad); Ph = sm.pattern_to_host(P)
+    cols, col_off, n = sm.sm_plan_columns(P, None)
+    X, scale = sm.sm_gather(A, P, cols, col_off, n, 0.0, "gershgorin", x_dtype)
+    iters, res = sm.sm_sign_ns(P, cols, col_off, n, P.packed_elems, x_dtype, X, k, 0.0)
+    torch.cuda.synchronize()
+    assert (iters == k).all()
+    dims = Ph.dim
+    picks = sorted(set([int(np.argmin(dims)), int(np.argmax(dims)), 0, wl.n_blk // 2]))
+    def img_index(Pd):
+        r = np.arange(Pd)[:, None]; c = np.arange(Pd)[None, :]
+        return (c >> 6) * Pd * 64 + r * 64 + ((((c & 63) >> 3) ^ (r & 7)) << 3) + (c & 7)
+    worst = 0.0
+    for i in picks:
+        T = orc.gather(wl, i); m = T.shape[0]; Pd = int(Ph.dim_pad[i]); lo = int(Ph.sub_off[i])
+        buf = X[lo:lo + Pd * Pd].double().cpu().numpy()
+        x = buf[img_index(Pd)] if x_dtype in ("bf16", "f16") else buf.reshape(Pd, Pd)
+        ref = orc.ns_polynomial(T, orc.gershgorin(T), k)
+        err = np.abs(x[:m, :m] - ref).max(); worst = max(worst, err)
+        assert err <= tol_abs, (i, m, err)
+        assert not x[m:].any() and not x[:, m:].any(), "padding must stay zero"
+        if sym_exact:
+            assert np.array_equal(x, x.T), "iterate must be exactly symmetric"
+        else:
+            assert np.abs(x - x.T).max() <= tol_abs
+    print("OK dims", int(dims.min()), int(dims.max()), "worst", worst)
+""")
+
+CASES = [
+    # env, x_dtype, pad, n_mol, cutoff, steps, tolerance (max-abs vs the NS-k polynomial), exact symmetry
+    ({"SM_UMMA_NCTA": "1", "SM_UMMA_SYM": "1"}, "bf16", 64, 90, 5.0, 3, 2.5e-2, True),
+    ({"SM_UMMA_NCTA": "2", "SM_UMMA_SYM": "1"}, "bf16", 64, 90, 5.0, 3, 2.5e-2, True),
+    ({"SM_UMMA_NCTA": "2", "SM_UMMA_SYM": "1"}, "f16", 64, 90, 5.0, 3, 3e-3, True),
+    ({"SM_UMMA_NCTA": "1", "SM_UMMA_SYM": "0"}, "f16", 64, 90, 5.0, 3, 3e-3, False),
+    ({"SM_UMMA_NCTA": "2", "SM_UMMA_SYM": "0"}, "bf16", 64, 90, 5.0, 3, 2.5e-2, False),
+    ({"SM_F64_BACKEND": "dmma"}, "f64", 4, 90, 5.0, 4, 1e-13, True),
+    ({"SM_F64_BACKEND": "simt"}, "f64", 16, 90, 5.0, 4, 1e-13, False),
+]
+
+
+@pytest.mark.parametrize("env,x_dtype,pad,n_mol,cutoff,k,tol_abs,sym_exact", CASES)
+def test_backend_matches_ns_polynomial(env, x_dtype, pad, n_mol, cutoff, k, tol_abs, sym_exact):
+    code = SNIPPET.format(root=ROOT, x_dtype=x_dtype, pad=pad, k=k, tol_abs=tol_abs, sym_exact=sym_exact,
+                          n_mol=n_mol, cutoff=cutoff)
+    e = dict(os.environ)
+    e.update(env)
+    p = subprocess.run([sys.executable, "-c", code], env=e, capture_output=True, text=True, timeout=600, cwd=ROOT)
+    assert p.returncode == 0, p.stdout[-2000:] + p.stderr[-4000:]
+    assert "OK dims" in p.stdout
