@@ -17,8 +17,8 @@
 // Kernel: persistent, one CTA per SM, 320 threads = 1 TMA producer warp, 1 MMA issuer warp (also
 // owns TMEM), 8 epilogue warps.  Tile = 128 x (<=256) fp32 accumulator in TMEM, double buffered
 // (2 x 256 columns) so the epilogue of tile t overlaps the main loop of tile t+1; 4-stage smem ring.
-//   PHASE 1: Y = X X^T, epilogue writes Y and the fused ||Y - I||_F^2 partial sums (warp shuffles).
-//   PHASE 2: X' = 1.5 X - 0.5 X Y^T, epilogue reads the X tile and writes X'.
+//   PHASE 1: W = X X^T - I, epilogue writes W and the fused ||W||_F^2 partial sums (warp shuffles).
+//   PHASE 2: X' = X - 0.5 X W^T (= 1.5 X - 0.5 X Y), epilogue reads the X tile and writes X'.
 #include <cstdlib>
 #include <utility>
 #include <vector>
@@ -409,19 +409,22 @@ __global__ void __launch_bounds__(UMMA_THREADS, 1) k_umma_gemm(UArgs a) {
 #pragma unroll
             for (int e = 0; e < 8; ++e) f[e] = __uint_as_float(v[g * 8 + e]);
             if (PHASE == 1) {
+              // W = Y - I is what gets stored: near convergence Y_rr ~ 1 would lose 2^-9 absolute to the 16-bit
+              // rounding every step, W_rr ~ 0 loses nothing; PHASE 2 then forms X' = X - 1/2 X W.
+              if (diag && r < u.m) {                               // padding rows keep W = 0
+#pragma unroll
+                for (int e = 0; e < 8; ++e)
+                  if (g * 8 + e == lane) f[e] -= 1.f;
+              }
               if (SYM && diag) {
 #pragma unroll
                 for (int e = 0; e < 8; ++e) {
                   const int j = g * 8 + e;
-                  const float d = f[e] - (j == lane ? 1.f : 0.f);
-                  if (j <= lane) acc = fmaf(j == lane ? d : 2.f * d, d, acc);
+                  if (j <= lane) acc = fmaf(j == lane ? f[e] : 2.f * f[e], f[e], acc);
                 }
               } else {
 #pragma unroll
-                for (int e = 0; e < 8; ++e) {
-                  const float d = (!SYM && diag && g * 8 + e == lane) ? f[e] - 1.f : f[e];
-                  acc = fmaf(d, d, acc);
-                }
+                for (int e = 0; e < 8; ++e) acc = fmaf(f[e], f[e], acc);
               }
             } else {
 #pragma unroll
@@ -429,8 +432,8 @@ __global__ void __launch_bounds__(UMMA_THREADS, 1) k_umma_gemm(UArgs a) {
                 // chunk g lives in sector g/2, lower half iff (g odd) == swp
                 const uint32_t xw = (((g & 1) != 0) == swp) ? xs[g >> 1][e2] : xs[g >> 1][4 + e2];
                 const float2 x = unpack2<BF16>(xw);
-                f[2 * e2] = 1.5f * x.x - 0.5f * f[2 * e2];
-                f[2 * e2 + 1] = 1.5f * x.y - 0.5f * f[2 * e2 + 1];
+                f[2 * e2] = x.x - 0.5f * f[2 * e2];
+                f[2 * e2 + 1] = x.y - 0.5f * f[2 * e2 + 1];
               }
             }
 #pragma unroll
