@@ -341,3 +341,43 @@ def test_cfg4_fp64_sampled_columns(sm):
         assert np.abs(D[mask] - ref[mask]).max() <= 1e-10, (mode, iters.cpu().numpy())
         if mode == "exact":
             assert sm.sm_sign_status(res, tol) == sm.SM_OK
+
+
+# ------------------------------------------------------------------- degenerate inputs
+
+def tiny_workload(n_mol, b, cutoff, seed):
+    return make_workload(n_mol, b, max(1, b // 2) if np.isscalar(b) else np.maximum(1, np.asarray(b) // 2), cutoff, seed=seed)
+
+
+@pytest.mark.parametrize("x_dtype,pad,lim", [("f64", 16, 1e-10), ("f32", 16, 1e-4), ("bf16", 64, 2e-2), ("f16", 64, 2e-2)])
+def test_degenerate_sizes_all_dtypes(sm, x_dtype, pad, lim):
+    # a single molecule (N = 1, one 6 x 6 submatrix), 1 x 1 blocks (m_i = neighbour count), and a 3-molecule
+    # chain: submatrices far smaller than one tile / one 64-element swizzle row
+    for wl in (make_workload(1, 6, 3, 4.0, seed=5), tiny_workload(12, 1, 6.0, 6), make_workload(3, 6, 3, 20.0, seed=7)):
+        d_or, _ = orc.density_columns(wl)
+        conv = x_dtype in ("f64", "f32")
+        _, P, plan = run_density(sm, wl, x_dtype, 100 if conv else 30, (1e-8 if x_dtype == "f64" else 1e-5) if conv else 0.0,
+                                 "gershgorin", pad=pad)
+        D = plan.D.cpu().numpy()
+        assert np.isfinite(D).all()
+        if conv:
+            assert np.abs(D - d_or).max() <= lim
+        else:
+            assert np.linalg.norm(D - d_or) <= lim * max(np.linalg.norm(d_or), 1.0)
+        assert abs(plan.trace.item() - orc.trace(wl, d_or)) <= (1e-9 if x_dtype == "f64" else 1e-3) * wl.n
+
+
+def test_power_scale_is_a_valid_tight_deterministic_bound(sm):
+    wl = make_workload(60, 23, 4, 5.0, seed=21)
+    A = sm.Bcsr(wl)
+    P = sm.sm_build_pattern(A, 64)
+    cols, col_off, n = sm.sm_plan_columns(P, None)
+    _, sg = sm.sm_gather(A, P, cols, col_off, n, 0.0, "gershgorin", "bf16")
+    _, sp = sm.sm_gather(A, P, cols, col_off, n, 0.0, "power", "bf16")
+    _, sp2 = sm.sm_gather(A, P, cols, col_off, n, 0.0, "power", "bf16")
+    assert torch.equal(sp, sp2)                                   # fixed-order reductions: bit-identical
+    sg, sp = sg.cpu().numpy(), sp.cpu().numpy()
+    assert (sp <= sg * (1 + 1e-12)).all()                         # never above the Gershgorin bound
+    for i in (0, 13, 59):
+        rho = np.abs(np.linalg.eigvalsh(orc.gather(wl, i))).max()
+        assert 0.80 * rho <= sp[i] <= 1.06 * rho, (i, sp[i], rho)  # Newton-Schulz needs |x| < sqrt(3): s > rho / 1.73
