@@ -90,6 +90,10 @@ template <> __device__ inline float from_double<float>(double v) { return (float
 template <> __device__ inline __nv_bfloat16 from_double<__nv_bfloat16>(double v) { return __float2bfloat16_rn((float)v); }
 template <> __device__ inline __half from_double<__half>(double v) { return __float2half_rn((float)v); }
 
+template <typename T> __device__ inline T from_float(float v) { return from_double<T>((double)v); }
+template <> __device__ inline __nv_bfloat16 from_float<__nv_bfloat16>(float v) { return __float2bfloat16_rn(v); }
+template <> __device__ inline __half from_float<__half>(float v) { return __float2half_rn(v); }
+
 template <typename T> __device__ inline double to_double(T v);
 template <> __device__ inline double to_double<double>(double v) { return v; }
 template <> __device__ inline double to_double<float>(float v) { return (double)v; }

@@ -111,8 +111,12 @@ __global__ void __launch_bounds__(256) k_gather(GatherArgs g, const TA *__restri
   const int32_t rows = min(GATHER_ROWS, Pd - r0);
   const int32_t n_cb = (Pd + 63) >> 6;                 // 64-column chunks (last may be partial: Pd % 16 == 0)
   const int32_t items = n_cb * rows * 8;
+  constexpr bool LOWP = sizeof(TX) == 2;               // 16-bit outputs: fp32 arithmetic is 2^-15 below their rounding
+  const float inv_sf = (float)inv_s, muf = (float)g.mu;
   for (int32_t e = threadIdx.x; e < items; e += blockDim.x) {
-    const int32_t j = e & 7, rr = (e >> 3) % rows, cb = (e >> 3) / rows;
+    const int32_t j = e & 7;
+    const int32_t rr = rows == GATHER_ROWS ? ((e >> 3) & (GATHER_ROWS - 1)) : (e >> 3) % rows;
+    const int32_t cb = rows == GATHER_ROWS ? (e >> 3) / GATHER_ROWS : (e >> 3) / rows;
     const int32_t r = r0 + rr, c0 = (cb << 6) + (j << 3);
     if (c0 >= Pd) continue;
     __align__(16) TX v[8];
@@ -120,26 +124,33 @@ __global__ void __launch_bounds__(256) k_gather(GatherArgs g, const TA *__restri
 #pragma unroll
       for (int k = 0; k < 8; ++k) v[k] = from_double<TX>(0.0);
     } else {
+      // walk the (at most 8) columns block by block: the stored block under the previous column stays cached
       const int32_t a = blkof[r], ra = r - off[a];
       const int32_t *gm_row = gm + (int64_t)a * cnt;
-      int32_t bprev = -1, cbase = 0;
-      const TA *src = nullptr;
+      int32_t b = blkof[c0], bs = off[b], be = off[b + 1];
+      int32_t p = __ldg(gm_row + b);
+      const TA *src = p >= 0 ? vals + __ldg(g.vp + p) + (int64_t)ra * (be - bs) : nullptr;
 #pragma unroll
       for (int k = 0; k < 8; ++k) {
         const int32_t c = c0 + k;
-        double x = 0.0;
         if (c < m) {
-          const int32_t b = blkof[c];
-          if (b != bprev) {
-            bprev = b; cbase = off[b];
-            const int32_t p = __ldg(gm_row + b);
-            src = p >= 0 ? vals + __ldg(g.vp + p) + (int64_t)ra * (off[b + 1] - cbase) : nullptr;
+          if (c >= be) {                                  // next neighbour block (blocks are >= 1 wide)
+            ++b; bs = be; be = off[b + 1];
+            p = __ldg(gm_row + b);
+            src = p >= 0 ? vals + __ldg(g.vp + p) + (int64_t)ra * (be - bs) : nullptr;
           }
-          if (src) x = to_double<TA>(__ldg(src + (c - cbase)));
-          if (r == c) x -= g.mu;
-          x *= inv_s;
+          if (LOWP) {
+            float x = src ? (float)__ldg(src + (c - bs)) : 0.f;
+            if (r == c) x -= muf;
+            v[k] = from_float<TX>(x * inv_sf);
+          } else {
+            double x = src ? to_double<TA>(__ldg(src + (c - bs))) : 0.0;
+            if (r == c) x -= g.mu;
+            v[k] = from_double<TX>(x * inv_s);
+          }
+        } else {
+          v[k] = from_double<TX>(0.0);
         }
-        v[k] = from_double<TX>(x);
       }
     }
     TX *dst = IMG ? Xs + img_off(Pd, r, c0) : Xs + (int64_t)r * Pd + c0;
