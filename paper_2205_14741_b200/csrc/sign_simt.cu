@@ -330,7 +330,7 @@ static int32_t sign_simt_t(const sm_pattern_t *P, const int32_t *cols, int32_t n
     SM_LAUNCHED();
     { int32_t rc = prof_end(st, slot); if (rc != SM_OK) return rc; }
     SM_CUDA(cudaMemsetAsync(w.n_still, 0, sizeof(int32_t), st));
-    k_sign_post<<<nb, 256, 0, st>>>(n_cols, cols, P->dim, s, w.n_parts, tol, iters, residual);
+    k_sign_post<<<(n_cols + 7) / 8, 256, 0, st>>>(n_cols, cols, P->dim, s, w.n_parts, tol, iters, residual);
     SM_LAUNCHED();
     { int32_t rc = prof_begin(st, &slot); if (rc != SM_OK) return rc; }
     if (dmma)

@@ -21,27 +21,35 @@ static __global__ void k_sign_init(int32_t n_cols, int32_t *active, int32_t *las
   active[c] = 1; last[c] = 0; iters[c] = 0; residual[c] = 0.0;
 }
 
-// Runs between the Y = X^2 product and the update product of one iteration.
-// n_parts[c] partial sums are valid for column c.
+// Runs between the Y = X^2 product and the update product of one iteration.  One warp per listed
+// column: the n_parts[c] partial sums are added lane-strided and then by a fixed shuffle tree, so the
+// result does not depend on scheduling (deterministic), and a column costs ~n_parts/32 loads per lane.
 static __global__ void k_sign_post(int32_t n_cols, const int32_t *__restrict__ cols,
                                    const int32_t *__restrict__ dim, SignState s,
                                    const int32_t *__restrict__ n_parts, double tol, int32_t *iters,
                                    double *residual) {
-  int32_t c = blockIdx.x * blockDim.x + threadIdx.x;
+  const int32_t c = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
   if (c >= n_cols) return;
-  if (s.last[c]) { s.active[c] = 0; s.last[c] = 0; }
+  if (s.last[c]) {
+    __syncwarp();
+    if (lane == 0) { s.active[c] = 0; s.last[c] = 0; }
+    return;
+  }
   if (!s.active[c]) return;
-  int32_t i = cols ? cols[c] : c;
   const double *p = s.partial + (int64_t)c * s.parts_per_col;
   double sum = 0.0;
-  int32_t np = n_parts[c];
-  for (int32_t t = 0; t < np; ++t) sum += p[t];
-  double r = sqrt(sum / (double)dim[i]);
-  residual[c] = r;
-  iters[c] += 1;
-  bool fin = (tol > 0.0) && (r < tol);
-  s.last[c] = fin ? 1 : 0;
-  if (!fin) atomicAdd(s.n_still, 1);
+  const int32_t np = n_parts[c];
+  for (int32_t t = lane; t < np; t += 32) sum += p[t];
+  for (int d = 16; d > 0; d >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, d);
+  if (lane == 0) {
+    const int32_t i = cols ? cols[c] : c;
+    const double r = sqrt(sum / (double)dim[i]);
+    residual[c] = r;
+    iters[c] += 1;
+    const bool fin = (tol > 0.0) && (r < tol);
+    s.last[c] = fin ? 1 : 0;
+    if (!fin) atomicAdd(s.n_still, 1);
+  }
 }
 
 // After the loop: a submatrix that received an odd number of updates has its result in the
