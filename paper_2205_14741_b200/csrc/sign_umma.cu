@@ -19,6 +19,7 @@
 // (2 x 256 columns) so the epilogue of tile t overlaps the main loop of tile t+1; 4-stage smem ring.
 //   PHASE 1: W = X X^T - I, epilogue writes W and the fused ||W||_F^2 partial sums (warp shuffles).
 //   PHASE 2: X' = X - 0.5 X W^T (= 1.5 X - 0.5 X Y), epilogue reads the X tile and writes X'.
+#include <cstdio>
 #include <cstdlib>
 #include <utility>
 #include <vector>
@@ -190,6 +191,17 @@ __device__ __forceinline__ void store_row_segment(uint16_t *Orow, uint32_t sec0,
               swp ? o[0] : o[4], swp ? o[1] : o[5], swp ? o[2] : o[6], swp ? o[3] : o[7]);
   ptx::stg256(Orow + sec1, swp ? o[12] : o[8], swp ? o[13] : o[9], swp ? o[14] : o[10], swp ? o[15] : o[11],
               swp ? o[8] : o[12], swp ? o[9] : o[13], swp ? o[10] : o[14], swp ? o[11] : o[15]);
+}
+
+// Mirrored 32 x 32 block straight from the registers of a warp whose lane holds row R0 + lane, columns
+// C0 .. C0 + 31 as 16 packed pairs: element (r, C0 + j) goes to row C0 + j, column r of the swizzled image.
+__device__ __forceinline__ void mirror_store(uint16_t *Og, int32_t Pd, int32_t R0, int32_t C0, int lane,
+                                             const uint32_t (&o)[16]) {
+  uint16_t *Mb = Og + (int64_t)(R0 >> 6) * Pd * 64 + (int64_t)C0 * 64 + (lane & 7);
+  const uint32_t ch = (((uint32_t)R0 & 63u) >> 3) + ((uint32_t)lane >> 3);   // chunk of column r before the swizzle
+#pragma unroll
+  for (int j = 0; j < 32; ++j)
+    Mb[j * 64 + ((ch ^ (uint32_t)(j & 7)) << 3)] = (uint16_t)(o[j >> 1] >> ((j & 1) * 16));
 }
 
 // SYM = true : K-major B (X X^T form), lower-triangle tiles, mirrored stores (exactly symmetric iterates).
@@ -463,23 +475,12 @@ __global__ void __launch_bounds__(UMMA_THREADS, 1) k_umma_gemm(UArgs a) {
             if (Orow) store_row_segment(Orow, sec0, sec1, swp, o);
           } else {
             if (Orow) store_row_segment(Orow, sec0, sec1, swp, o);
-#pragma unroll
-            for (int g = 0; g < 4; ++g) {
-#pragma unroll
-              for (int e = 0; e < 8; ++e)                        // transposed: [col][row]
-                stg[(g * 8 + e) * 32 + lane] = (uint16_t)(o[g * 4 + (e >> 1)] >> ((e & 1) * 16));
-            }
-            __syncwarp();
-            // mirrored block: rows C0 + c (c = lane/4 + 8 i), columns R0 + 8 j (j = lane % 4), 16 bytes each
-            const uint32_t mpos = ((((uint32_t)R0 >> 3) & 4u) + ((uint32_t)lane & 3u)) ^ (((uint32_t)lane >> 2) & 7u);
-            uint16_t *Mp = Og ? Og + (int64_t)(R0 >> 6) * u.Pd * 64 + (int64_t)(C0 + (lane >> 2)) * 64 + (mpos << 3)
-                              : nullptr;
-            if (Mp) {
-#pragma unroll
-              for (int i = 0; i < 4; ++i)
-                *reinterpret_cast<uint4 *>(Mp + i * 512) = *reinterpret_cast<const uint4 *>(stg + lane * 8 + i * 256);
-            }
-            __syncwarp();
+            // Mirrored block straight from the registers: element (r, C0 + j) goes to row C0 + j, column r.  The
+            // 32 lanes are 32 consecutive columns of that row = 64 contiguous bytes (four swizzled 16-byte chunks
+            // of one 128-byte line), so every 2-byte store instruction fills two whole sectors.  No shared-memory
+            // transpose: its 2 KB of sub-word stores per block competed with the MMA and TMA for the shared-memory
+            // pipe (clock64 time line, round 1: 600-1000 cycles per block).
+            if (Og) mirror_store(Og, u.Pd, R0, C0, lane, o);
           }
         }
       }
@@ -506,6 +507,29 @@ __global__ void __launch_bounds__(UMMA_THREADS, 1) k_umma_gemm(UArgs a) {
   if (warp == 1) {
     ptx::tc_fence_after();
     if (PAIR) ptx::tmem_dealloc2(tmem_base, TMEM_COLS); else ptx::tmem_dealloc(tmem_base, TMEM_COLS);
+  }
+}
+
+
+#include "sign_umma_fused.cuh"
+
+// Fixed-iteration bookkeeping after k_umma_fused: residual of the last step from its partial sums (one
+// warp per listed column, fixed order), iters = max_iter.
+static __global__ void k_fused_post(int32_t n_cols, const int32_t *__restrict__ cols, const int32_t *__restrict__ dim,
+                                    const double *__restrict__ partial, int32_t parts_per_col,
+                                    const int32_t *__restrict__ n_parts, int32_t max_iter, int32_t *iters,
+                                    double *residual) {
+  const int32_t c = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+  if (c >= n_cols) return;
+  const double *p = partial + (int64_t)c * parts_per_col;
+  double sum = 0.0;
+  const int32_t np = n_parts[c];
+  for (int32_t t = lane; t < np; t += 32) sum += p[t];
+  for (int d = 16; d > 0; d >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, d);
+  if (lane == 0) {
+    const int32_t i = cols ? cols[c] : c;
+    residual[c] = max_iter > 0 ? sqrt(sum / (double)dim[i]) : 0.0;
+    iters[c] = max_iter;
   }
 }
 
@@ -559,6 +583,21 @@ static int32_t umma_sym(const sm_pattern_t *P) {
   return 1;     // measured (configs[2], B200): SYM 0.77 ms per launch, FULL 1.13 ms
 }
 
+// Fused kernel (whole iteration per submatrix inside one launch, iterates L2-resident): fixed iteration
+// counts only, and only where the per-phase design is HBM bound (largest submatrix <= 1024; above that
+// three iterates of one submatrix per CTA pair no longer fit L2 and the per-phase launches are compute
+// bound anyway).  SM_UMMA_FUSED=0/1 in the environment overrides (A/B measurements, tests).
+static int32_t umma_fused(const sm_pattern_t *P, double tol) {
+  static int32_t env = -2;
+  if (env == -2) {
+    const char *e = getenv("SM_UMMA_FUSED");
+    env = e ? (e[0] == '1' ? 1 : 0) : -1;
+  }
+  if (tol > 0.0) return 0;
+  if (env >= 0) return env;
+  return P->max_dim <= 1024 ? 1 : 0;
+}
+
 static int32_t umma_dbg() {
   const char *e = getenv("SM_UMMA_DBG");
   return e ? atoi(e) : 0;
@@ -568,9 +607,13 @@ static UmmaWs umma_layout(void *ws, int64_t ws_bytes, const sm_pattern_t *P, int
                           int64_t packed_elems) {
   WsCursor cur(ws, ws_bytes);
   UmmaWs w;
+  // sized for whichever variant sign_umma picks (the query does not know tol): per-phase launches with
+  // the selected NCTA / SYM, or the fused kernel (CTA pairs, SYM)
   const int32_t ncta = umma_ncta(P);
-  const int32_t max_tiles = umma_sym(P) ? u_tiles(P->max_dim, UM * ncta) : f_tiles(P->max_dim_pad, UM * ncta);
-  w.parts_per_col = max_tiles * EPI_WARPS * ncta;
+  const int32_t t_sel = umma_sym(P) ? u_tiles(P->max_dim, UM * ncta) : f_tiles(P->max_dim_pad, UM * ncta);
+  const int32_t t_fused = u_tiles(P->max_dim, UM * 2);
+  const int32_t max_tiles = t_sel > t_fused ? t_sel : t_fused;
+  w.parts_per_col = (t_sel * ncta > t_fused * 2 ? t_sel * ncta : t_fused * 2) * EPI_WARPS;
   w.Y = cur.take<char>(packed_elems * 2);
   w.X2 = cur.take<char>(packed_elems * 2);
   w.active = cur.take<int32_t>(n_cols);
@@ -614,6 +657,29 @@ static int32_t launch_umma(const UArgs &a, int32_t n_sm, cudaStream_t st) {
   return prof_end(st, slot);
 }
 
+template <bool BF16>
+static int32_t launch_fused(const FArgs &a, int32_t n_sm, cudaStream_t st) {
+  static bool configured = false;
+  if (!configured) {
+    SM_CUDA(cudaFuncSetAttribute(k_umma_fused<BF16>, cudaFuncAttributeMaxDynamicSharedMemorySize, UCfg<2>::SMEM));
+    configured = true;
+  }
+  int slot = -1;
+  { int32_t rc = prof_begin(st, &slot); if (rc != SM_OK) return rc; }
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)(n_sm / 2 * 2), 1, 1);
+  cfg.blockDim = dim3(UMMA_THREADS, 1, 1);
+  cfg.dynamicSmemBytes = UCfg<2>::SMEM;
+  cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeClusterDimension;
+  attr[0].val.clusterDim.x = 2; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+  cfg.attrs = attr; cfg.numAttrs = 1;
+  SM_CUDA(cudaLaunchKernelEx(&cfg, k_umma_fused<BF16>, a));
+  SM_LAUNCHED();
+  return prof_end(st, slot);
+}
+
 template <int PHASE, int NCTA, bool SYM>
 static int32_t launch_umma_t(bool bf16, const UArgs &a, int32_t n_sm, cudaStream_t st) {
   return bf16 ? launch_umma<true, PHASE, NCTA, SYM>(a, n_sm, st) : launch_umma<false, PHASE, NCTA, SYM>(a, n_sm, st);
@@ -629,7 +695,8 @@ int32_t sign_umma(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, co
                   int32_t max_iter, double tol, int32_t *iters, double *residual, cudaStream_t st) {
   if ((P->pad_to % 64) != 0) return SM_ERR_ARG;
   const bool bf16 = x_dtype == SM_BF16;
-  const int32_t ncta = umma_ncta(P), R = UM * ncta, sym = umma_sym(P);
+  const bool fused = umma_fused(P, tol) != 0;
+  const int32_t ncta = fused ? 2 : umma_ncta(P), R = UM * ncta, sym = fused ? 1 : umma_sym(P);
   UmmaWs w = umma_layout(ws, ws_bytes, P, n_cols, packed_elems);
   if (w.used > ws_bytes) return SM_ERR_SPACE;
   int dev = 0, n_sm = 0;
@@ -649,6 +716,33 @@ int32_t sign_umma(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, co
   SM_CUDA(cudaMemsetAsync(w.Y, 0, packed_elems * 2, st));
   SM_CUDA(cudaMemsetAsync(w.X2, 0, packed_elems * 2, st));
   SM_CUDA(cudaMemsetAsync(w.err, 0, sizeof(int32_t), st));
+  if (fused) {
+    // fixed iteration count: one launch runs every step of every submatrix (k_umma_fused)
+    FArgs f{cols, col_off, P->dim, P->dim_pad, n_cols, max_iter, X, w.X2, w.Y, w.partial, w.parts_per_col, w.err, nullptr, umma_dbg()};
+    // SM_UMMA_TRACE=<file>: measurement only -- clock64 time line of CTA pair 0 (debug allocation, synchronises)
+    const char *trace_path = getenv("SM_UMMA_TRACE");
+    const size_t trace_bytes = (size_t)2 * 4 * TRACE_N * 2 * sizeof(unsigned long long);
+    if (trace_path) {
+      SM_CUDA(cudaMalloc((void **)&f.trace, trace_bytes));
+      SM_CUDA(cudaMemsetAsync(f.trace, 0, trace_bytes, st));
+    }
+    int32_t rc = bf16 ? launch_fused<true>(f, n_sm, st) : launch_fused<false>(f, n_sm, st);
+    if (rc != SM_OK) return rc;
+    if (trace_path) {
+      std::vector<unsigned long long> hbuf(trace_bytes / sizeof(unsigned long long));
+      SM_CUDA(cudaMemcpyAsync(hbuf.data(), f.trace, trace_bytes, cudaMemcpyDeviceToHost, st));
+      SM_CUDA(cudaStreamSynchronize(st));
+      SM_CUDA(cudaFree(f.trace));
+      if (FILE *fp = fopen(trace_path, "wb")) { fwrite(hbuf.data(), 1, trace_bytes, fp); fclose(fp); }
+    }
+    k_fused_post<<<(n_cols + 7) / 8, 256, 0, st>>>(n_cols, cols, P->dim, w.partial, w.parts_per_col, w.n_parts,
+                                                   max_iter, iters, residual);
+    SM_LAUNCHED();
+    dim3 cgf(n_cols, 8);
+    k_copy_back<<<cgf, 256, 0, st>>>(cols, col_off, iters, 2, (const char *)w.X2, (char *)X);
+    SM_LAUNCHED();
+    return SM_OK;
+  }
   void *buf[2] = {X, w.X2};
   for (int32_t k = 0; k < max_iter; ++k) {
     void *src = buf[k & 1], *dst = buf[(k + 1) & 1];
