@@ -38,7 +38,8 @@ constexpr int NACC = 512 / UN;   // accumulator stages in TMEM (512 columns)
 constexpr int UK = 64;           // k chunk = one 128-byte swizzle row of 16-bit elements
 constexpr int A_BYTES = UM * UK * 2;           // 16 KB
 constexpr int EPI_WARPS = 16;
-constexpr int EPI_STAGE_BYTES = EPI_WARPS * 2048;   // 32 x 32 x 2 B transpose buffer per epilogue warp
+constexpr int EPI_STAGE_BYTES = 4 * NACC * 2048;    // 32 x 32 x 2 B buffer per (TMEM lane quadrant, accumulator stage): diagonal blocks only
+constexpr int IDENT_BYTES = 8192;                   // 64 x 64 identity image(s): B operand that folds "+ X" into the update product
 constexpr int UMMA_THREADS = 64 + 32 * EPI_WARPS;
 constexpr uint32_t TMEM_COLS = 512;
 
@@ -46,11 +47,17 @@ constexpr uint32_t TMEM_COLS = 512;
 // 256 x (<=256): each CTA stages its own 128 rows of A and HALF of the B rows, so a pair moves
 // (256 + nt) rows per k chunk for 256 x nt outputs instead of 2 x (128 + nt): the L2 -> SM bytes per
 // FLOP drop by 1.5x at nt = 256 (ncu, round 1: the single-CTA kernel sits on the L2 throughput cap).
-template <int NCTA> struct UCfg {
-  static constexpr int STAGES = NCTA == 2 ? 6 : 4;
-  static constexpr int B_BYTES = (UN / NCTA) * UK * 2;     // 32 KB / 16 KB
+//
+// MC (NCTA = 2 only): the same 256-row tile geometry, but each CTA issues its own cta_group::1 MMAs on its
+// 128 rows with the WHOLE B tile in its shared memory; each CTA fetches half of the B rows and multicasts
+// them to both (cp.async.bulk ... multicast::cluster), so the L2 -> SM bytes equal those of the cta_group::2
+// pair while no CTA waits on a relayed "peer's stage landed" signal.
+template <int NCTA, bool MC = false> struct UCfg {
+  static constexpr bool G2 = NCTA == 2 && !MC;             // cta_group::2 MMA
+  static constexpr int STAGES = G2 ? 6 : 4;
+  static constexpr int B_BYTES = (G2 ? UN / 2 : UN) * UK * 2;   // 16 KB / 32 KB
   static constexpr int STAGE_BYTES = A_BYTES + B_BYTES;    // 48 KB / 32 KB
-  static constexpr int SMEM = STAGES * STAGE_BYTES + EPI_STAGE_BYTES + 1024 /*align slack*/ + 256 /*barriers*/;
+  static constexpr int SMEM = STAGES * STAGE_BYTES + EPI_STAGE_BYTES + IDENT_BYTES + 1024 /*align slack*/ + 256 /*barriers*/;
   static constexpr int ROWS = UM * NCTA;                   // tile rows
 };
 
@@ -193,6 +200,30 @@ __device__ __forceinline__ void store_row_segment(uint16_t *Orow, uint32_t sec0,
               swp ? o[8] : o[12], swp ? o[9] : o[13], swp ? o[10] : o[14], swp ? o[11] : o[15]);
 }
 
+// Identity operand of the update product.  PHASE 2 computes X' = X - 1/2 X W as ONE accumulation:
+// PHASE 1 stores Wh = -1/2 (X X^T - I) (exact scaling), and while the A chunk X[rows, 64 kc ..] that covers
+// output columns of the tile sits in shared memory, one more MMA with B = a slice of the identity adds
+// X[rows, cols] * 1 to those accumulator columns.  The epilogue then only converts and stores: no global
+// read of the X tile (it cost 64 of the ~160 L1 wavefronts of a 32 x 32 block, and 1.3 GB of L2/HBM
+// reads per step at configs[2]).  The image is K-major SW128 like every operand: 64 rows x 128 B.
+// One CTA: row n has its 1 at k = n; a piece [lo, hi) of the chunk uses rows lo - 64 kc onwards.
+// CTA pair (each CTA supplies half of the N rows from the same offset): rows 0-31 serve N = 64 (1 at
+// k = 32 h + n), rows 32-47 N = 32 at k-offset 0 (k = 16 h + n'), rows 48-63 N = 32 at k-offset 32.
+template <bool BF16>
+__device__ __forceinline__ void ident_fill(uint8_t *img, bool pair, uint32_t h, int tid, int nthreads) {
+  for (int i = tid; i < IDENT_BYTES / 16; i += nthreads) reinterpret_cast<uint4 *>(img)[i] = make_uint4(0, 0, 0, 0);
+  __syncthreads();
+  if (tid < 64) {
+    const uint32_t n = (uint32_t)tid;
+    const uint32_t k = !pair ? n : (n < 32 ? 32 * h + n : (n < 48 ? 16 * h + (n - 32) : 32 + 16 * h + (n - 48)));
+    *reinterpret_cast<uint16_t *>(img + n * 128 + (((k >> 3) ^ (n & 7)) << 4) + (k & 7) * 2) = BF16 ? 0x3F80 : 0x3C00;
+  }
+}
+// Row of the identity image at which the B slice of a piece starts (s = lo - 64 kc in {0, 32}, N in {32, 64}).
+__device__ __forceinline__ uint32_t ident_row(bool pair, int32_t s, int32_t N) {
+  return !pair ? (uint32_t)s : (N == 64 ? 0u : (s ? 48u : 32u));
+}
+
 // Mirrored 32 x 32 block straight from the registers of a warp whose lane holds row R0 + lane, columns
 // C0 .. C0 + 31 as 16 packed pairs: element (r, C0 + j) goes to row C0 + j, column r of the swizzled image.
 __device__ __forceinline__ void mirror_store(uint16_t *Og, int32_t Pd, int32_t R0, int32_t C0, int lane,
@@ -209,17 +240,20 @@ __device__ __forceinline__ void mirror_store(uint16_t *Og, int32_t Pd, int32_t R
 //              form damps (++ block) or leaves unchanged (+- block) an antisymmetric rounding residue,
 //              so exact symmetry is not needed; it trades 1.3-1.7x more MMA work for an epilogue
 //              without transposes, which is what bounds the m < ~1000 regime (ncu, round 1).
-template <bool BF16, int PHASE, int NCTA, bool SYM>
+template <bool BF16, int PHASE, int NCTA, bool SYM, bool MC = false>
 __global__ void __launch_bounds__(UMMA_THREADS, 1) k_umma_gemm(UArgs a) {
-  using Cfg = UCfg<NCTA>;
+  static_assert(!MC || (NCTA == 2 && SYM), "multicast variant: two CTAs, SYM tiles");
+  using Cfg = UCfg<NCTA, MC>;
   constexpr int USTAGES = Cfg::STAGES;
   constexpr int STAGE_BYTES = Cfg::STAGE_BYTES;
-  constexpr bool PAIR = NCTA == 2;
+  constexpr bool PAIR = NCTA == 2 && !MC;                  // cta_group::2 MMAs issued by the leader
+  constexpr bool CL2 = NCTA == 2;                          // cluster of two CTAs on one 256-row tile
   extern __shared__ uint8_t smem_raw[];
   const uint32_t raw = ptx::smem_u32(smem_raw);
   const uint32_t tiles = (raw + 1023u) & ~1023u;           // 1024-byte aligned operand ring
   const uint32_t stage_base = tiles + USTAGES * STAGE_BYTES;   // epilogue transpose buffers
-  const uint32_t bars = stage_base + EPI_STAGE_BYTES;      // barriers behind them
+  const uint32_t ident = stage_base + EPI_STAGE_BYTES;     // identity image (1024-byte aligned)
+  const uint32_t bars = ident + IDENT_BYTES;               // barriers behind it
   // barrier slots (8 bytes each): full[S], empty[S], pfull[S] (pair: peer's stage landed, leader only),
   // tmem_full[2], tmem_empty[2]; then the TMEM base address
   auto full_bar = [&](int s) { return bars + 8u * s; };
@@ -232,14 +266,19 @@ __global__ void __launch_bounds__(UMMA_THREADS, 1) k_umma_gemm(UArgs a) {
       reinterpret_cast<volatile uint32_t *>(smem_raw + (tmem_slot - raw));
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const uint32_t h = PAIR ? ptx::cluster_ctarank() : 0u;   // rank inside the CTA pair; 0 = leader
+  const uint32_t h = CL2 ? ptx::cluster_ctarank() : 0u;    // rank inside the CTA pair; 0 = leader
   const int64_t unit = blockIdx.x / NCTA, n_units = gridDim.x / NCTA;
 
+  if (PHASE == 2) {
+    ident_fill<BF16>(smem_raw + (ident - raw), PAIR, h, (int)threadIdx.x, UMMA_THREADS);
+    ptx::fence_proxy_async();       // generic-proxy writes -> the MMA's async-proxy reads
+  }
   if (threadIdx.x == 0) {
     for (int s = 0; s < USTAGES; ++s) {
-      ptx::mbar_init(full_bar(s), 1); ptx::mbar_init(empty_bar(s), 1); ptx::mbar_init(pfull_bar(s), 1);
+      // MC: a stage is free once the MMAs of BOTH CTAs have read it (each producer writes into both)
+      ptx::mbar_init(full_bar(s), 1); ptx::mbar_init(empty_bar(s), MC ? 2 : 1); ptx::mbar_init(pfull_bar(s), 1);
     }
-    for (int s = 0; s < NACC; ++s) { ptx::mbar_init(tfull_bar(s), 1); ptx::mbar_init(tempty_bar(s), EPI_WARPS * NCTA); }
+    for (int s = 0; s < NACC; ++s) { ptx::mbar_init(tfull_bar(s), 1); ptx::mbar_init(tempty_bar(s), EPI_WARPS * (PAIR ? 2 : 1)); }
     ptx::fence_barrier_init();
     ptx::fence_proxy_async();
   }
@@ -248,7 +287,7 @@ __global__ void __launch_bounds__(UMMA_THREADS, 1) k_umma_gemm(UArgs a) {
     else { ptx::tmem_alloc(tmem_slot, TMEM_COLS); ptx::tmem_relinquish(); }
   }
   ptx::tc_fence_before();
-  if (PAIR) ptx::cluster_sync_all(); else __syncthreads();
+  if (CL2) ptx::cluster_sync_all(); else __syncthreads();
   ptx::tc_fence_after();
   const uint32_t tmem_base = *tmem_slot_ptr;
 
@@ -284,10 +323,13 @@ __global__ void __launch_bounds__(UMMA_THREADS, 1) k_umma_gemm(UArgs a) {
             if (++stage == USTAGES) { stage = 0; phase ^= 1u; }
             continue;
           }
-          ptx::mbar_expect_tx(full_bar(stage), a_bytes + b_bytes);
+          ptx::mbar_expect_tx(full_bar(stage), a_bytes + (MC ? 2u * b_bytes : b_bytes));
           const int64_t chunk = (int64_t)kc * u.Pd * 128;     // byte offset of k chunk kc
           if (a_bytes) ptx::tma_bulk_g2s(sa, Ag + chunk + (int64_t)arow0 * 128, a_bytes, full_bar(stage));
-          if (SYM) {
+          if (MC) {
+            // this CTA's half of the B rows, delivered into both CTAs at its place in the whole tile
+            ptx::tma_bulk_g2s_mc(sb + h * b_bytes, Bg + chunk + (int64_t)brow0 * 128, b_bytes, full_bar(stage), (uint16_t)3);
+          } else if (SYM) {
             ptx::tma_bulk_g2s(sb, Bg + chunk + (int64_t)brow0 * 128, b_bytes, full_bar(stage));
           } else {
             for (int32_t j = 0; j < n_atoms; ++j)    // rows k of chunk-column (atom0 + j): 64 x 128 B
@@ -298,7 +340,7 @@ __global__ void __launch_bounds__(UMMA_THREADS, 1) k_umma_gemm(UArgs a) {
         }
       }
     }
-  } else if (warp == 1 && h != 0) {
+  } else if (PAIR && warp == 1 && h != 0) {
     // ===================== relay (peer CTA of a pair): tell the leader that this CTA's stage landed ======
     if (lane == 0) {
       int stage = 0; uint32_t phase = 0;
@@ -331,7 +373,7 @@ __global__ void __launch_bounds__(UMMA_THREADS, 1) k_umma_gemm(UArgs a) {
         ptx::mbar_wait(tempty_bar(as), aphase ^ 1u, a.err_flag, 2);
         ptx::tc_fence_after();
         const uint32_t d_tmem = tmem_base + as * UN;
-        const uint32_t idesc = ptx::make_idesc_f16(BF16, UM * NCTA, (uint32_t)u.nt, !SYM);
+        const uint32_t idesc = ptx::make_idesc_f16(BF16, PAIR ? 2 * UM : UM, (uint32_t)u.nt, !SYM);
         const int nkc = (u.kmax + UK - 1) / UK;
         for (int kc = 0; kc < nkc; ++kc) {
           ptx::mbar_wait(full_bar(stage), phase, a.err_flag, 3);
@@ -351,8 +393,23 @@ __global__ void __launch_bounds__(UMMA_THREADS, 1) k_umma_gemm(UArgs a) {
               ptx::umma_f16(d_tmem, adesc + (uint64_t)(2 * ks), bdesc + bstep * (uint64_t)ks, idesc,
                             (uint32_t)((kc | ks) != 0));
           }
+          if (PHASE == 2 && !(a.dbg & 2)) {
+            // "+ X": the A chunk in this stage holds X[rows, 64 kc .. 64 kc + 63]; add it to the accumulator
+            // columns [lo, hi) of the tile that it covers (B = identity slice, K-major)
+            const int32_t lo = max(kc * UK, u.n0), hi = min(kc * UK + UK, u.n0 + u.nt);
+            if (lo < hi) {
+              const uint32_t idesc2 = ptx::make_idesc_f16(BF16, PAIR ? 2 * UM : UM, (uint32_t)(hi - lo), false);
+              const uint64_t idd = ptx::make_sw128_kmajor_desc(ident + ident_row(PAIR, lo - kc * UK, hi - lo) * 128u);
+              for (int ks = 0; ks < UK / 16; ++ks) {
+                if (PAIR) ptx::umma_f16_2cta(d_tmem + (uint32_t)(lo - u.n0), adesc + (uint64_t)(2 * ks), idd + (uint64_t)(2 * ks), idesc2, 1u);
+                else ptx::umma_f16(d_tmem + (uint32_t)(lo - u.n0), adesc + (uint64_t)(2 * ks), idd + (uint64_t)(2 * ks), idesc2, 1u);
+              }
+            }
+          }
           // frees the smem slot (in both CTAs of a pair) when these MMAs finish
-          if (PAIR) ptx::umma_commit_2cta(empty_bar(stage)); else ptx::umma_commit(empty_bar(stage));
+          if (PAIR) ptx::umma_commit_2cta(empty_bar(stage));
+          else if (MC) ptx::umma_commit_mc(empty_bar(stage), (uint16_t)3);
+          else ptx::umma_commit(empty_bar(stage));
           if (++stage == USTAGES) { stage = 0; phase ^= 1u; }
         }
         // accumulator ready for the epilogue warps (of both CTAs)
@@ -371,7 +428,7 @@ __global__ void __launch_bounds__(UMMA_THREADS, 1) k_umma_gemm(UArgs a) {
     constexpr int NSUB = EPI_WARPS / 4;
     const int q = warp & 3;                        // TMEM lane quadrant this warp may access
     const int sub = (warp - 2) >> 2;               // which column blocks this warp takes
-    uint16_t *stg = reinterpret_cast<uint16_t *>(smem_raw + (stage_base - raw)) + (warp - 2) * 1024;
+    uint16_t *const stg0 = reinterpret_cast<uint16_t *>(smem_raw + (stage_base - raw)) + q * NACC * 1024;
     uint32_t it = 0;
     TileDesc nxt = load_desc(a, max((int64_t)0, min(unit, total - 1)));
     for (int64_t t = unit; t < total; t += n_units) {
@@ -380,10 +437,12 @@ __global__ void __launch_bounds__(UMMA_THREADS, 1) k_umma_gemm(UArgs a) {
       UTile u = make_tile<PHASE>(a, cur);
       if (!u.valid) continue;
       const uint32_t as = it % NACC, aphase = (it / NACC) & 1u;
+      // diagonal-block buffer of (quadrant, accumulator stage): a tile has one diagonal block per quadrant, and
+      // two tiles on the same stage cannot be in flight at once
+      uint16_t *const stg = stg0 + as * 1024;
       const int32_t R0 = u.row0 + (int32_t)h * UM + q * 32;   // this CTA's 128 rows of the tile
       const int32_t r = R0 + lane;
       uint16_t *Og = (uint16_t *)a.Out + u.base;
-      const uint16_t *Xg = (const uint16_t *)a.Xsrc + u.base;
       if (a.dbg & 1) Og = nullptr;
       const int nblk = (u.nt + 31) >> 5;
       ptx::mbar_wait(tfull_bar(as), aphase, a.err_flag, 4);
@@ -406,11 +465,6 @@ __global__ void __launch_bounds__(UMMA_THREADS, 1) k_umma_gemm(UArgs a) {
           // request a full sector (ncu, round 1: 16-byte accesses doubled the sector count of these paths).
           const bool swp = (lane & 1) != 0;
           const uint32_t sec0 = ((c8 ^ r7) & ~1u) << 3, sec1 = (((c8 + 2u) ^ r7) & ~1u) << 3;   // element offsets
-          uint32_t xs[2][8];
-          if (PHASE == 2) {
-            ptx::ldg256(Xg + rowoff + sec0, xs[0]);
-            ptx::ldg256(Xg + rowoff + sec1, xs[1]);
-          }
           ptx::tmem_ld_wait();
           const bool diag = (C0 == R0);
           uint32_t o[16];                                        // 32 output elements, packed pairs
@@ -438,15 +492,8 @@ __global__ void __launch_bounds__(UMMA_THREADS, 1) k_umma_gemm(UArgs a) {
 #pragma unroll
                 for (int e = 0; e < 8; ++e) acc = fmaf(f[e], f[e], acc);
               }
-            } else {
 #pragma unroll
-              for (int e2 = 0; e2 < 4; ++e2) {
-                // chunk g lives in sector g/2, lower half iff (g odd) == swp
-                const uint32_t xw = (((g & 1) != 0) == swp) ? xs[g >> 1][e2] : xs[g >> 1][4 + e2];
-                const float2 x = unpack2<BF16>(xw);
-                f[2 * e2] = x.x - 0.5f * f[2 * e2];
-                f[2 * e2 + 1] = x.y - 0.5f * f[2 * e2 + 1];
-              }
+              for (int e = 0; e < 8; ++e) f[e] *= -0.5f;           // Wh = -1/2 W is what PHASE 2 multiplies by
             }
 #pragma unroll
             for (int e2 = 0; e2 < 4; ++e2) o[g * 4 + e2] = pack2<BF16>(f[2 * e2], f[2 * e2 + 1]);
@@ -503,7 +550,7 @@ __global__ void __launch_bounds__(UMMA_THREADS, 1) k_umma_gemm(UArgs a) {
 
   ptx::tc_fence_before();
   __syncwarp();
-  if (PAIR) ptx::cluster_sync_all(); else __syncthreads();
+  if (CL2) ptx::cluster_sync_all(); else __syncthreads();
   if (warp == 1) {
     ptx::tc_fence_after();
     if (PAIR) ptx::tmem_dealloc2(tmem_base, TMEM_COLS); else ptx::tmem_dealloc(tmem_base, TMEM_COLS);
@@ -569,6 +616,17 @@ static int32_t umma_ncta(const sm_pattern_t *P) {
   return P->max_dim > 1024 ? 2 : 1;
 }
 
+// Two-CTA tiles: cta_group::2 MMAs with a relayed "stage landed" (0) or two cta_group::1 MMAs with the B rows
+// multicast to both CTAs (1).  SM_UMMA_MC=0/1 in the environment overrides.
+static int32_t umma_mc() {
+  static int32_t env = -2;
+  if (env == -2) {
+    const char *e = getenv("SM_UMMA_MC");
+    env = e ? (e[0] == '1' ? 1 : 0) : -1;
+  }
+  return env >= 0 ? env : 1;     // measured (configs[4], B200): 654 ms (multicast) vs 690 ms (relay) for 25 steps
+}
+
 // SYM (triangular tiles, mirrored stores) for large submatrices, where the symmetric half of the MMA
 // work is worth more than the transposing epilogue costs; FULL (true products) below.  Decided per
 // call from the pattern's largest submatrix; SM_UMMA_SYM=0/1 in the environment overrides.
@@ -583,19 +641,19 @@ static int32_t umma_sym(const sm_pattern_t *P) {
   return 1;     // measured (configs[2], B200): SYM 0.77 ms per launch, FULL 1.13 ms
 }
 
-// Fused kernel (whole iteration per submatrix inside one launch, iterates L2-resident): fixed iteration
-// counts only, and only where the per-phase design is HBM bound (largest submatrix <= 1024; above that
-// three iterates of one submatrix per CTA pair no longer fit L2 and the per-phase launches are compute
-// bound anyway).  SM_UMMA_FUSED=0/1 in the environment overrides (A/B measurements, tests).
+// Fused kernel (whole iteration per submatrix inside one launch, iterates L2-resident; fixed iteration counts
+// only).  It halves the DRAM traffic of configs[2] (ncu: 62 GB vs 130 GB for 20 steps) but is bound by its
+// epilogue's store instructions and the per-phase hand-over, and measures slower than the per-phase launches
+// (33.4 vs 26.7 ms), so it is opt-in: SM_UMMA_FUSED=1 in the environment (A/B measurements, tests).
 static int32_t umma_fused(const sm_pattern_t *P, double tol) {
   static int32_t env = -2;
   if (env == -2) {
     const char *e = getenv("SM_UMMA_FUSED");
     env = e ? (e[0] == '1' ? 1 : 0) : -1;
   }
+  (void)P;
   if (tol > 0.0) return 0;
-  if (env >= 0) return env;
-  return P->max_dim <= 1024 ? 1 : 0;
+  return env > 0 ? 1 : 0;
 }
 
 static int32_t umma_dbg() {
@@ -633,12 +691,12 @@ int64_t sign_umma_ws_bytes(const sm_pattern_t *P, int32_t n_cols, int64_t packed
   return umma_layout(nullptr, 0, P, n_cols, packed_elems).used;
 }
 
-template <bool BF16, int PHASE, int NCTA, bool SYM>
+template <bool BF16, int PHASE, int NCTA, bool SYM, bool MC = false>
 static int32_t launch_umma(const UArgs &a, int32_t n_sm, cudaStream_t st) {
   static bool configured = false;
   if (!configured) {
-    SM_CUDA(cudaFuncSetAttribute(k_umma_gemm<BF16, PHASE, NCTA, SYM>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 UCfg<NCTA>::SMEM));
+    SM_CUDA(cudaFuncSetAttribute(k_umma_gemm<BF16, PHASE, NCTA, SYM, MC>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 UCfg<NCTA, MC>::SMEM));
     configured = true;
   }
   int slot = -1;
@@ -646,22 +704,22 @@ static int32_t launch_umma(const UArgs &a, int32_t n_sm, cudaStream_t st) {
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3((unsigned)(n_sm / NCTA * NCTA), 1, 1);     // one CTA per SM, whole pairs
   cfg.blockDim = dim3(UMMA_THREADS, 1, 1);
-  cfg.dynamicSmemBytes = UCfg<NCTA>::SMEM;
+  cfg.dynamicSmemBytes = UCfg<NCTA, MC>::SMEM;
   cfg.stream = st;
   cudaLaunchAttribute attr[1];
   attr[0].id = cudaLaunchAttributeClusterDimension;
   attr[0].val.clusterDim.x = NCTA; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
   cfg.attrs = attr; cfg.numAttrs = 1;
-  SM_CUDA(cudaLaunchKernelEx(&cfg, k_umma_gemm<BF16, PHASE, NCTA, SYM>, a));
+  SM_CUDA(cudaLaunchKernelEx(&cfg, k_umma_gemm<BF16, PHASE, NCTA, SYM, MC>, a));
   SM_LAUNCHED();
   return prof_end(st, slot);
 }
 
-template <bool BF16>
+template <bool BF16, int NSLOT>
 static int32_t launch_fused(const FArgs &a, int32_t n_sm, cudaStream_t st) {
   static bool configured = false;
   if (!configured) {
-    SM_CUDA(cudaFuncSetAttribute(k_umma_fused<BF16>, cudaFuncAttributeMaxDynamicSharedMemorySize, UCfg<2>::SMEM));
+    SM_CUDA(cudaFuncSetAttribute(k_umma_fused<BF16, NSLOT>, cudaFuncAttributeMaxDynamicSharedMemorySize, UCfg<2>::SMEM));
     configured = true;
   }
   int slot = -1;
@@ -675,17 +733,18 @@ static int32_t launch_fused(const FArgs &a, int32_t n_sm, cudaStream_t st) {
   attr[0].id = cudaLaunchAttributeClusterDimension;
   attr[0].val.clusterDim.x = 2; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
   cfg.attrs = attr; cfg.numAttrs = 1;
-  SM_CUDA(cudaLaunchKernelEx(&cfg, k_umma_fused<BF16>, a));
+  SM_CUDA(cudaLaunchKernelEx(&cfg, k_umma_fused<BF16, NSLOT>, a));
   SM_LAUNCHED();
   return prof_end(st, slot);
 }
 
-template <int PHASE, int NCTA, bool SYM>
+template <int PHASE, int NCTA, bool SYM, bool MC = false>
 static int32_t launch_umma_t(bool bf16, const UArgs &a, int32_t n_sm, cudaStream_t st) {
-  return bf16 ? launch_umma<true, PHASE, NCTA, SYM>(a, n_sm, st) : launch_umma<false, PHASE, NCTA, SYM>(a, n_sm, st);
+  return bf16 ? launch_umma<true, PHASE, NCTA, SYM, MC>(a, n_sm, st) : launch_umma<false, PHASE, NCTA, SYM, MC>(a, n_sm, st);
 }
 template <int PHASE>
 static int32_t launch_umma_any(bool bf16, int32_t ncta, int32_t sym, const UArgs &a, int32_t n_sm, cudaStream_t st) {
+  if (ncta == 3) return launch_umma_t<PHASE, 2, true, true>(bf16, a, n_sm, st);     // two CTAs, multicast B (SYM only)
   if (ncta == 2) return sym ? launch_umma_t<PHASE, 2, true>(bf16, a, n_sm, st) : launch_umma_t<PHASE, 2, false>(bf16, a, n_sm, st);
   return sym ? launch_umma_t<PHASE, 1, true>(bf16, a, n_sm, st) : launch_umma_t<PHASE, 1, false>(bf16, a, n_sm, st);
 }
@@ -726,7 +785,10 @@ int32_t sign_umma(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, co
       SM_CUDA(cudaMalloc((void **)&f.trace, trace_bytes));
       SM_CUDA(cudaMemsetAsync(f.trace, 0, trace_bytes, st));
     }
-    int32_t rc = bf16 ? launch_fused<true>(f, n_sm, st) : launch_fused<false>(f, n_sm, st);
+    static int32_t nslot = 0;      // SM_UMMA_SLOTS=1/2: submatrices a CTA pair interleaves (A/B measurements)
+    if (!nslot) { const char *e = getenv("SM_UMMA_SLOTS"); nslot = (e && e[0] == '1') ? 1 : 2; }
+    int32_t rc = nslot == 2 ? (bf16 ? launch_fused<true, 2>(f, n_sm, st) : launch_fused<false, 2>(f, n_sm, st))
+                            : (bf16 ? launch_fused<true, 1>(f, n_sm, st) : launch_fused<false, 1>(f, n_sm, st));
     if (rc != SM_OK) return rc;
     if (trace_path) {
       std::vector<unsigned long long> hbuf(trace_bytes / sizeof(unsigned long long));
@@ -743,17 +805,18 @@ int32_t sign_umma(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, co
     SM_LAUNCHED();
     return SM_OK;
   }
+  const int32_t mode = (ncta == 2 && sym && umma_mc()) ? 3 : ncta;    // 3: two CTAs per tile, multicast B
   void *buf[2] = {X, w.X2};
   for (int32_t k = 0; k < max_iter; ++k) {
     void *src = buf[k & 1], *dst = buf[(k + 1) & 1];
     UArgs a{cols, col_off, P->dim, P->dim_pad, w.tile_ptr, w.tiles, n_cols, tol > 0.0 ? 1 : 0, src, w.Y, w.Y, s, w.err, umma_dbg()};
-    int32_t rc = launch_umma_any<1>(bf16, ncta, sym, a, n_sm, st);
+    int32_t rc = launch_umma_any<1>(bf16, mode, sym, a, n_sm, st);
     if (rc != SM_OK) return rc;
     SM_CUDA(cudaMemsetAsync(w.n_still, 0, sizeof(int32_t), st));
     k_sign_post<<<(n_cols + 7) / 8, 256, 0, st>>>(n_cols, cols, P->dim, s, w.n_parts, tol, iters, residual);
     SM_LAUNCHED();
     a.Out = dst;
-    rc = launch_umma_any<2>(bf16, ncta, sym, a, n_sm, st);
+    rc = launch_umma_any<2>(bf16, mode, sym, a, n_sm, st);
     if (rc != SM_OK) return rc;
     if (tol > 0.0 && k >= 5 && (k & 1)) {
       int32_t still = 1;

@@ -202,6 +202,25 @@ __device__ __forceinline__ void umma_commit_2cta(uint32_t bar) {
       : "memory");
 }
 
+// ---- cluster multicast (two single-MMA CTAs sharing the B operand) -------------------------------
+// Bulk copy delivered to the same CTA-relative shared-memory offset (and complete_tx on the same
+// CTA-relative mbarrier) in every CTA of `mask`.
+__device__ __forceinline__ void tma_bulk_g2s_mc(uint32_t dst_smem, const void *src_gmem, uint32_t bytes,
+                                                uint32_t bar, uint16_t mask) {
+  asm volatile(
+      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.multicast::cluster [%0], [%1], %2, [%3], %4;" ::"r"(
+          dst_smem),
+      "l"(src_gmem), "r"(bytes), "r"(bar), "h"(mask)
+      : "memory");
+}
+// Completion of this thread's prior (cta_group::1) MMAs arrives on the mbarrier at this offset in every CTA of `mask`.
+__device__ __forceinline__ void umma_commit_mc(uint32_t bar, uint16_t mask) {
+  asm volatile(
+      "tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;" ::"r"(bar),
+      "h"(mask)
+      : "memory");
+}
+
 // ---- 256-bit global accesses (sm_100+): one full 32-byte L2 sector per lane and instruction ------
 __device__ __forceinline__ void ldg256(const void *p, uint32_t (&r)[8]) {
   asm volatile("ld.global.v8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"

@@ -2,6 +2,7 @@
 environment forces (each in its own process: the selection is read once per process):
   SM_UMMA_NCTA=1|2   single CTAs / CTA pairs (cta_group::2) per tile of the tcgen05 kernel
   SM_UMMA_SYM=1|0    symmetric half tiles with mirrored stores / true products with an MN-major B operand
+  SM_UMMA_FUSED=1|0  one launch runs every step of a submatrix (k_umma_fused) / one launch per product
   SM_F64_BACKEND     DMMA tensor tiles (default) / DFMA register tiles
 Each case runs NS steps on a seeded workload whose submatrices span several tiles and ragged tails and
 compares with the oracle's NS-k polynomial (exact-arithmetic result of k steps, reading A13)."""
@@ -54,11 +55,13 @@ SNIPPET = textwrap.dedent("""
 
 CASES = [
     # env, x_dtype, pad, n_mol, cutoff, steps, tolerance (max-abs vs the NS-k polynomial), exact symmetry
-    ({"SM_UMMA_NCTA": "1", "SM_UMMA_SYM": "1"}, "bf16", 64, 90, 5.0, 3, 2.5e-2, True),
-    ({"SM_UMMA_NCTA": "2", "SM_UMMA_SYM": "1"}, "bf16", 64, 90, 5.0, 3, 2.5e-2, True),
-    ({"SM_UMMA_NCTA": "2", "SM_UMMA_SYM": "1"}, "f16", 64, 90, 5.0, 3, 3e-3, True),
-    ({"SM_UMMA_NCTA": "1", "SM_UMMA_SYM": "0"}, "f16", 64, 90, 5.0, 3, 3e-3, False),
-    ({"SM_UMMA_NCTA": "2", "SM_UMMA_SYM": "0"}, "bf16", 64, 90, 5.0, 3, 2.5e-2, False),
+    ({"SM_UMMA_FUSED": "0", "SM_UMMA_NCTA": "1", "SM_UMMA_SYM": "1"}, "bf16", 64, 90, 5.0, 3, 2.5e-2, True),
+    ({"SM_UMMA_FUSED": "0", "SM_UMMA_NCTA": "2", "SM_UMMA_SYM": "1"}, "bf16", 64, 90, 5.0, 3, 2.5e-2, True),
+    ({"SM_UMMA_FUSED": "0", "SM_UMMA_NCTA": "2", "SM_UMMA_SYM": "1"}, "f16", 64, 90, 5.0, 3, 3e-3, True),
+    ({"SM_UMMA_FUSED": "0", "SM_UMMA_NCTA": "1", "SM_UMMA_SYM": "0"}, "f16", 64, 90, 5.0, 3, 3e-3, False),
+    ({"SM_UMMA_FUSED": "0", "SM_UMMA_NCTA": "2", "SM_UMMA_SYM": "0"}, "bf16", 64, 90, 5.0, 3, 2.5e-2, False),
+    ({"SM_UMMA_FUSED": "1"}, "bf16", 64, 90, 5.0, 3, 2.5e-2, True),
+    ({"SM_UMMA_FUSED": "1"}, "f16", 64, 90, 5.0, 4, 3e-3, True),
     ({"SM_F64_BACKEND": "dmma"}, "f64", 4, 90, 5.0, 4, 1e-13, True),
     ({"SM_F64_BACKEND": "simt"}, "f64", 16, 90, 5.0, 4, 1e-13, False),
 ]
