@@ -85,6 +85,7 @@ struct UArgs {
   const void *Xsrc; const void *Ybuf; void *Out;
   SignState s;
   int32_t *err_flag;
+  int32_t rev;               // walk the tile table backwards (alternates per launch)
   int32_t dbg;               // measurement only (SM_UMMA_DBG): 1 = skip output stores, 2 = skip MMA issue, 4 = skip TMA loads, 8 = skip the epilogue's work
 };
 
@@ -118,6 +119,9 @@ __host__ __device__ inline int32_t f_Tn(int32_t Pd) { return (Pd + UN - 1) / UN;
 __host__ __device__ inline int32_t f_tiles(int32_t Pd, int32_t R) { return f_Tm(Pd, R) * f_Tn(Pd); }
 
 __device__ __forceinline__ TileDesc load_desc(const UArgs &a, int64_t t) {
+  // a.rev: this launch walks the tile table backwards, so that it starts on the submatrices whose operands the
+  // previous launch touched last (still in L2) instead of on the ones evicted longest ago
+  if (a.rev) t = a.tile_ptr[a.n_cols] - 1 - t;
   const uint4 *p = reinterpret_cast<const uint4 *>(a.tiles + t);
   uint4 q0 = __ldg(p), q1 = __ldg(p + 1), q2 = __ldg(p + 2);
   TileDesc d;
@@ -806,16 +810,20 @@ int32_t sign_umma(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, co
     return SM_OK;
   }
   const int32_t mode = (ncta == 2 && sym && umma_mc()) ? 3 : ncta;    // 3: two CTAs per tile, multicast B
+  static int32_t rev_on = -1;     // SM_UMMA_REV=0 keeps every launch walking forwards (A/B measurements)
+  if (rev_on < 0) { const char *e = getenv("SM_UMMA_REV"); rev_on = (e && e[0] == '0') ? 0 : 1; }
   void *buf[2] = {X, w.X2};
   for (int32_t k = 0; k < max_iter; ++k) {
     void *src = buf[k & 1], *dst = buf[(k + 1) & 1];
-    UArgs a{cols, col_off, P->dim, P->dim_pad, w.tile_ptr, w.tiles, n_cols, tol > 0.0 ? 1 : 0, src, w.Y, w.Y, s, w.err, umma_dbg()};
+    UArgs a{cols, col_off, P->dim, P->dim_pad, w.tile_ptr, w.tiles, n_cols, tol > 0.0 ? 1 : 0, src, w.Y, w.Y, s, w.err, 0, umma_dbg()};
+    a.rev = 0;
     int32_t rc = launch_umma_any<1>(bf16, mode, sym, a, n_sm, st);
     if (rc != SM_OK) return rc;
     SM_CUDA(cudaMemsetAsync(w.n_still, 0, sizeof(int32_t), st));
     k_sign_post<<<(n_cols + 7) / 8, 256, 0, st>>>(n_cols, cols, P->dim, s, w.n_parts, tol, iters, residual);
     SM_LAUNCHED();
     a.Out = dst;
+    a.rev = rev_on;            // PHASE 2 starts where PHASE 1 ended, the next PHASE 1 where this launch ends
     rc = launch_umma_any<2>(bf16, mode, sym, a, n_sm, st);
     if (rc != SM_OK) return rc;
     if (tol > 0.0 && k >= 5 && (k & 1)) {

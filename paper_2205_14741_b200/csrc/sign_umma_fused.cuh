@@ -23,7 +23,7 @@ struct FArgs {
   double *partial; int32_t parts_per_col;
   int32_t *err_flag;
   unsigned long long *trace;   // measurement only (SM_UMMA_TRACE): clock64 time line of CTA pair 0, second submatrix
-  int32_t dbg;                 // measurement only (SM_UMMA_DBG): 1 = no phase hand-over (wrong results), 2 = no gpu-scope fence, 8 = skip the epilogue's work
+  int32_t dbg;                 // measurement only (SM_UMMA_DBG): 1 = no phase hand-over (wrong results), 2 = no gpu-scope fence, 8 = skip the epilogue's work, 16 / 32 = skip the direct / mirrored stores of off-diagonal blocks
 };
 
 // One submatrix of the caller's list as the fused kernel sees it.
@@ -325,8 +325,8 @@ __global__ void __launch_bounds__(UMMA_THREADS, 1) k_umma_fused(FArgs a) {
                   __syncwarp();
                   store_row_segment(Orow, sec0, sec1, swp, o);
                 } else {
-                  store_row_segment(Orow, sec0, sec1, swp, o);
-                  mirror_store(Og, Pd, R0, C0, lane, o);
+                  if (!(a.dbg & 16)) store_row_segment(Orow, sec0, sec1, swp, o);
+                  if (!(a.dbg & 32)) mirror_store(Og, Pd, R0, C0, lane, o);
                 }
               }
             }
