@@ -31,8 +31,8 @@ if ROOT not in sys.path:
 from workloads.generator import CONFIGS, make_config  # noqa: E402
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel (mean of its PHASE 1 / PHASE 2 launches),
-# from the committed `ncu --set full` captures under profiles/ (r1b_ncu_full_k_umma_gemm_cfg{2,4}.md, ..._k_dmma_gemm_cfg1.md).
-NCU_TRAFFIC_BYTES = {(2, "bf16"): 3.33e9, (4, "bf16"): 62.2e9, (1, "f64"): 0.72e9}
+# from the committed `ncu --set full` captures under profiles/ (r1c_ncu_full_k_umma_gemm_cfg{2,4}.md, r1b_ncu_full_k_dmma_gemm_cfg1.md).
+NCU_TRAFFIC_BYTES = {(2, "bf16"): 3.46e9, (4, "bf16"): 34.9e9, (1, "f64"): 0.72e9}
 
 METRIC = "submatrix_sign_effective_tflops"
 UNIT = "TFLOP/s"
@@ -298,15 +298,17 @@ def run_ours(args, cfg, cfg_run):
     peaks = load_peaks()
     if is16:
         # dominant kernel: k_umma_gemm.  Algorithmic FLOPs per launch = 2 sum m^3 (one m x m x m product per
-        # submatrix); launches inside the timed region = 2 * k * steps.
+        # submatrix); launches inside the timed region = 2 * k * steps.  With SM_UMMA_FUSED=1 one launch of
+        # k_umma_fused runs all 2 k products, so the per-launch figure is the total over the timed launches.
         long_region = ms_total_max > 4000.0
         peak = peaks["sustained"] if long_region else peaks["burst"]
-        flops_per_launch = 2.0 * sum_m3
+        flops_per_launch = flops_step * args.steps / max(gemm_launches, 1)
         avg_ms = gemm_ms / max(gemm_launches, 1)
         achieved = flops_per_launch / (avg_ms * 1e-3) / 1e12
-        roofline = {"bound": "tensor", "kernel": "k_umma_gemm", "achieved": achieved, "peak": peak,
+        fused = os.environ.get("SM_UMMA_FUSED", "0")[:1] == "1"
+        roofline = {"bound": "tensor", "kernel": "k_umma_fused" if fused else "k_umma_gemm", "achieved": achieved, "peak": peak,
                     "unit": "TFLOP/s", "frac": achieved / peak,
-                    "traffic": NCU_TRAFFIC_BYTES.get((args.config, x_dtype)),
+                    "traffic": None if fused else NCU_TRAFFIC_BYTES.get((args.config, x_dtype)),
                     "peak_source": f"{peaks['src']} bf16 {'sustained' if long_region else 'burst'}",
                     "launches_timed": gemm_launches, "avg_launch_ms": avg_ms,
                     "algorithmic_flops_per_launch": flops_per_launch}
