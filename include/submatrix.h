@@ -183,6 +183,23 @@ int32_t sm_density(const sm_bcsr_t *A, const void *A_vals, int32_t a_dtype, doub
                    int64_t max_chunk_elems, void *ws, int64_t ws_bytes, int32_t d_dtype,
                    void *D_vals, double *trace, int32_t *iters, double *residual, double *scale,
                    void *stream);
+/* Chemical potential for a fixed electron count (the first row past the hot path).
+ * Eq. 14 carries mu but the paper gives no rule for it; the usual closure is the electron count
+ * Tr D(mu) = n_target (with S = I, D = 1/2 (I - sign(H - mu I)) counts the eigenvalues below mu),
+ * and Tr D(mu) is non-decreasing in mu, so mu is found by bisection on [mu_lo, mu_hi].  Host driven: every trial is
+ * one sm_density call (same arguments, same buffers) followed by a synchronisation of `stream` to read the 8-byte
+ * trace.  Trials 1 and 2 evaluate the ends of the bracket (SM_ERR_ARG unless Tr D(mu_lo) <= n_target <= Tr D(mu_hi),
+ * both within tol_n); then mu = midpoint until |Tr D(mu) - n_target| <= tol_n, or the bracket is narrower than
+ * mu_tol, or max_trials (>= 3) trials were run.  On return *mu_out is the last midpoint evaluated (or the end of
+ * the bracket that already met tol_n), *trace_out its Tr D, *trials_out the number of sm_density calls, and
+ * D_vals / trace / iters / residual / scale hold that trial's results.  Synchronises. */
+int32_t sm_mu_search(const sm_bcsr_t *A, const void *A_vals, int32_t a_dtype, double n_target, double mu_lo,
+                     double mu_hi, double tol_n, double mu_tol, int32_t max_trials, int32_t x_dtype,
+                     int32_t scale_mode, int32_t max_iter, double tol, int32_t symmetrise, const sm_pattern_t *P,
+                     const int32_t *h_dim_pad /*host [N]*/, int64_t max_chunk_elems, void *ws, int64_t ws_bytes,
+                     int32_t d_dtype, void *D_vals, double *trace, int32_t *iters, double *residual,
+                     double *scale, double *mu_out /*host*/, double *trace_out /*host*/,
+                     int32_t *trials_out /*host*/, void *stream);
 /* R -> D = 1/2 (I - R) in place on block-CSR values, and Tr D (device fp64 scalar, may be NULL). */
 int32_t sm_density_from_sign(const sm_bcsr_t *A, const sm_pattern_t *P, int32_t d_dtype,
                              void *RD_vals, double *trace, void *stream);

@@ -164,6 +164,41 @@ def density_columns(w, mu: float = 0.0, cols=None, mode: str = "exact", k_fixed:
     return d, st
 
 
+def mu_search(w, n_target: float, mu_lo: float, mu_hi: float, tol_n: float = 1e-6, mu_tol: float = 1e-12,
+              max_trials: int = 60, n_threads: int = 1):
+    """Chemical potential for a fixed electron count: Eq. 14 carries mu,
+    PAPER.md:89-92 relate D to the occupied states; with S = I, Tr D(mu) counts the eigenvalues below mu and is
+    non-decreasing, so mu solves Tr D(mu) = n_target by bisection.  Step by step: the two ends of the bracket
+    (upper first), then midpoints until |Tr D - n_target| <= tol_n, the bracket is narrower than mu_tol, or
+    max_trials evaluations.  Each evaluation is the whole submatrix method with the exact sign (density_columns).
+    Returns (mu, Tr D(mu), trials, d_vals of the last trial)."""
+    def count(mu):
+        d, _ = density_columns(w, mu=mu, n_threads=n_threads)
+        return trace(w, d), d
+    trials = 0
+    n_hi, d = count(mu_hi); trials += 1
+    if n_hi < n_target - tol_n:
+        raise ValueError("bracket: Tr D(mu_hi) < n_target")
+    n_lo, d = count(mu_lo); trials += 1
+    if n_lo > n_target + tol_n:
+        raise ValueError("bracket: Tr D(mu_lo) > n_target")
+    if abs(n_lo - n_target) <= tol_n:
+        return mu_lo, n_lo, trials, d
+    lo, hi, mu, n_mid = mu_lo, mu_hi, mu_lo, n_lo
+    while trials < max_trials:
+        mu = 0.5 * (lo + hi)
+        n_mid, d = count(mu); trials += 1
+        if abs(n_mid - n_target) <= tol_n:
+            break
+        if n_mid < n_target:
+            lo = mu
+        else:
+            hi = mu
+        if hi - lo <= mu_tol:
+            break
+    return mu, n_mid, trials, d
+
+
 def symmetrise(w, d_raw: np.ndarray) -> np.ndarray:
     vp = np.ascontiguousarray(w.val_ptr, dtype=np.int64)
     d_raw = np.ascontiguousarray(d_raw, dtype=np.float64)

@@ -32,7 +32,7 @@ SCALES = {"none": SM_SCALE_NONE, "gershgorin": SM_SCALE_GERSHGORIN, "power": SM_
 EXPORTS = ["sm_last_cuda_error", "sm_pattern_sizes", "sm_build_pattern", "sm_plan_columns",
            "sm_gather_ws_bytes", "sm_gather", "sm_sign_ws_bytes", "sm_sign_ns", "sm_sign_status",
            "sm_scatter", "sm_symmetrise", "sm_density_ws_bytes", "sm_density", "sm_density_from_sign",
-           "sm_launch_count", "sm_profile_enable", "sm_profile_read"]
+           "sm_mu_search", "sm_launch_count", "sm_profile_enable", "sm_profile_read"]
 
 
 class SmError(RuntimeError):
@@ -295,6 +295,22 @@ def sm_density(A: Bcsr, P: Pattern, plan: DensityPlan, mu=0.0, scale_mode="gersh
         C.c_int64(plan.ws.numel()), C.c_int32(plan.d_dt), _ptr(plan.D), _ptr(plan.trace), _ptr(plan.iters),
         _ptr(plan.residual), _ptr(plan.scale), _stream()))
     return plan
+
+
+def sm_mu_search(A: Bcsr, P: Pattern, plan: DensityPlan, n_target, mu_lo, mu_hi, tol_n=1e-6, mu_tol=1e-12,
+                 max_trials=60, scale_mode="gershgorin", max_iter=100, tol=0.0, symmetrise=False, A_vals=None):
+    """Bisection on Tr D(mu) = n_target; returns (mu, trace, trials); D etc. of the last trial live in the plan."""
+    sc = SCALES[scale_mode] if isinstance(scale_mode, str) else scale_mode
+    vals = A.vals if A_vals is None else A_vals
+    mu, tr, nt = C.c_double(0.0), C.c_double(0.0), C.c_int32(0)
+    _check("sm_mu_search", _lib.sm_mu_search(
+        C.byref(A.c), _ptr(vals), C.c_int32(A.val_dtype), C.c_double(n_target), C.c_double(mu_lo),
+        C.c_double(mu_hi), C.c_double(tol_n), C.c_double(mu_tol), C.c_int32(max_trials), C.c_int32(plan.x_dt),
+        C.c_int32(sc), C.c_int32(max_iter), C.c_double(tol), C.c_int32(1 if symmetrise else 0), C.byref(P.c),
+        plan.h_dim_pad.ctypes.data_as(C.c_void_p), C.c_int64(plan.max_chunk_elems), _ptr(plan.ws),
+        C.c_int64(plan.ws.numel()), C.c_int32(plan.d_dt), _ptr(plan.D), _ptr(plan.trace), _ptr(plan.iters),
+        _ptr(plan.residual), _ptr(plan.scale), C.byref(mu), C.byref(tr), C.byref(nt), _stream()))
+    return mu.value, tr.value, nt.value
 
 
 def pattern_to_host(P: Pattern) -> SimpleNamespace:

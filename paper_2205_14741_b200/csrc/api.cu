@@ -1,6 +1,7 @@
 // C-ABI entry points that dispatch or compose: sm_sign_ns (a3) and sm_density (a5, the whole path
 // gather -> sign -> scatter -> D = 1/2 (I - R), PAPER.md:110 steps 1-3 + PAPER.md:91 Eq. 14, S = I).
 #include <algorithm>
+#include <cmath>
 #include <numeric>
 #include <utility>
 #include <vector>
@@ -156,6 +157,50 @@ extern "C" int32_t sm_density(const sm_bcsr_t *A, const void *A_vals, int32_t a_
     if (rc != SM_OK) return rc;
   }
   return sm_density_from_sign(A, P, d_dtype, D_vals, trace, stream);
+}
+
+// ---- chemical potential for a fixed electron count (Eq. 14) --------------
+extern "C" int32_t sm_mu_search(const sm_bcsr_t *A, const void *A_vals, int32_t a_dtype, double n_target,
+                                double mu_lo, double mu_hi, double tol_n, double mu_tol, int32_t max_trials,
+                                int32_t x_dtype, int32_t scale_mode, int32_t max_iter, double tol,
+                                int32_t symmetrise, const sm_pattern_t *P, const int32_t *h_dim_pad,
+                                int64_t max_chunk_elems, void *ws, int64_t ws_bytes, int32_t d_dtype, void *D_vals,
+                                double *trace, int32_t *iters, double *residual, double *scale, double *mu_out,
+                                double *trace_out, int32_t *trials_out, void *stream) {
+  if (!mu_out || !trace_out || !trials_out || !trace) return SM_ERR_ARG;
+  if (!(mu_lo < mu_hi) || !(tol_n >= 0.0) || !(mu_tol >= 0.0) || max_trials < 3) return SM_ERR_ARG;
+  cudaStream_t st = (cudaStream_t)stream;
+  int32_t trials = 0;
+  auto count = [&](double mu, double *n) -> int32_t {
+    int32_t rc = sm_density(A, A_vals, a_dtype, mu, x_dtype, scale_mode, max_iter, tol, symmetrise, P, h_dim_pad,
+                            max_chunk_elems, ws, ws_bytes, d_dtype, D_vals, trace, iters, residual, scale, stream);
+    if (rc != SM_OK) return rc;
+    SM_CUDA(cudaMemcpyAsync(n, trace, sizeof(double), cudaMemcpyDeviceToHost, st));
+    SM_CUDA(cudaStreamSynchronize(st));
+    ++trials;
+    return SM_OK;
+  };
+  double n_lo = 0.0, n_hi = 0.0, n_mid = 0.0, mu = mu_hi;
+  int32_t rc = count(mu_hi, &n_hi);
+  if (rc != SM_OK) return rc;
+  *mu_out = mu_hi; *trace_out = n_hi; *trials_out = trials;
+  if (n_hi < n_target - tol_n) return SM_ERR_ARG;
+  rc = count(mu_lo, &n_lo);
+  if (rc != SM_OK) return rc;
+  *mu_out = mu_lo; *trace_out = n_lo; *trials_out = trials;
+  if (n_lo > n_target + tol_n) return SM_ERR_ARG;
+  if (fabs(n_lo - n_target) <= tol_n) return SM_OK;          // the lower end already has the right count
+  double lo = mu_lo, hi = mu_hi;
+  while (trials < max_trials) {
+    mu = 0.5 * (lo + hi);
+    rc = count(mu, &n_mid);
+    if (rc != SM_OK) return rc;
+    *mu_out = mu; *trace_out = n_mid; *trials_out = trials;
+    if (fabs(n_mid - n_target) <= tol_n) break;
+    if (n_mid < n_target) lo = mu; else hi = mu;
+    if (hi - lo <= mu_tol) break;
+  }
+  return SM_OK;
 }
 
 // ---- profiling hooks (host; see include/submatrix.h) ------------------------------------------

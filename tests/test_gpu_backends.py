@@ -1,6 +1,9 @@
 """GPU parity of the alternative back ends of sm_sign_ns that the library selects by size or that the
 environment forces (each in its own process: the selection is read once per process):
-  SM_UMMA_NCTA=1|2   single CTAs / CTA pairs (cta_group::2) per tile of the tcgen05 kernel
+  SM_UMMA_NCTA=1|2   one CTA / two CTAs per tile of the tcgen05 kernel
+  SM_UMMA_MC=1|0     two CTAs: own cta_group::1 MMAs with the B rows multicast / cta_group::2 MMAs with a relayed stage signal
+  SM_UMMA_REV=1|0    PHASE 2 walks the tile table backwards / forwards
+  SM_UMMA_SLOTS=2|1  submatrices a CTA pair of the fused kernel interleaves
   SM_UMMA_SYM=1|0    symmetric half tiles with mirrored stores / true products with an MN-major B operand
   SM_UMMA_FUSED=1|0  one launch runs every step of a submatrix (k_umma_fused) / one launch per product
   SM_F64_BACKEND     DMMA tensor tiles (default) / DFMA register tiles
@@ -56,11 +59,14 @@ SNIPPET = textwrap.dedent("""
 CASES = [
     # env, x_dtype, pad, n_mol, cutoff, steps, tolerance (max-abs vs the NS-k polynomial), exact symmetry
     ({"SM_UMMA_FUSED": "0", "SM_UMMA_NCTA": "1", "SM_UMMA_SYM": "1"}, "bf16", 64, 90, 5.0, 3, 2.5e-2, True),
-    ({"SM_UMMA_FUSED": "0", "SM_UMMA_NCTA": "2", "SM_UMMA_SYM": "1"}, "bf16", 64, 90, 5.0, 3, 2.5e-2, True),
-    ({"SM_UMMA_FUSED": "0", "SM_UMMA_NCTA": "2", "SM_UMMA_SYM": "1"}, "f16", 64, 90, 5.0, 3, 3e-3, True),
+    ({"SM_UMMA_FUSED": "0", "SM_UMMA_NCTA": "2", "SM_UMMA_SYM": "1", "SM_UMMA_MC": "1"}, "bf16", 64, 90, 5.0, 3, 2.5e-2, True),
+    ({"SM_UMMA_FUSED": "0", "SM_UMMA_NCTA": "2", "SM_UMMA_SYM": "1", "SM_UMMA_MC": "0"}, "bf16", 64, 90, 5.0, 3, 2.5e-2, True),
+    ({"SM_UMMA_FUSED": "0", "SM_UMMA_NCTA": "2", "SM_UMMA_SYM": "1", "SM_UMMA_MC": "1", "SM_UMMA_REV": "0"}, "f16", 64, 90, 5.0, 3, 3e-3, True),
+    ({"SM_UMMA_FUSED": "0", "SM_UMMA_NCTA": "2", "SM_UMMA_SYM": "1", "SM_UMMA_MC": "0"}, "f16", 64, 90, 5.0, 4, 3e-3, True),
     ({"SM_UMMA_FUSED": "0", "SM_UMMA_NCTA": "1", "SM_UMMA_SYM": "0"}, "f16", 64, 90, 5.0, 3, 3e-3, False),
     ({"SM_UMMA_FUSED": "0", "SM_UMMA_NCTA": "2", "SM_UMMA_SYM": "0"}, "bf16", 64, 90, 5.0, 3, 2.5e-2, False),
     ({"SM_UMMA_FUSED": "1"}, "bf16", 64, 90, 5.0, 3, 2.5e-2, True),
+    ({"SM_UMMA_FUSED": "1", "SM_UMMA_SLOTS": "1"}, "bf16", 64, 90, 5.0, 4, 2.5e-2, True),
     ({"SM_UMMA_FUSED": "1"}, "f16", 64, 90, 5.0, 4, 3e-3, True),
     ({"SM_F64_BACKEND": "dmma"}, "f64", 4, 90, 5.0, 4, 1e-13, True),
     ({"SM_F64_BACKEND": "simt"}, "f64", 16, 90, 5.0, 4, 1e-13, False),

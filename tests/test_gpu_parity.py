@@ -230,6 +230,29 @@ def test_cfg0_limits_full_coverage_and_block_diagonal(sm):
     assert np.abs(plan.D.cpu().numpy() - d_or).max() <= 1e-10
 
 
+def test_mu_search_follows_the_oracle_bisection(sm):
+    # Tr D(mu) = n_target by bisection (Eq. 14).  fp64, convergence mode:
+    # the GPU's Tr D(mu) equals the oracle's to 1e-9, so both bisections take the same path.
+    wl = make_config(0)
+    A = sm.Bcsr(wl); P = sm.sm_build_pattern(A, 4)
+    plan = sm.DensityPlan(A, P, "f64")
+    for n_target in (96.0, 60.0):
+        mu_o, n_o, trials_o, d_o = orc.mu_search(wl, n_target, -2.5, 2.5, tol_n=1e-6, n_threads=THREADS)
+        mu_g, n_g, trials_g = sm.sm_mu_search(A, P, plan, n_target, -2.5, 2.5, tol_n=1e-6, max_iter=100, tol=1e-8)
+        assert trials_g == trials_o and mu_g == mu_o
+        assert abs(n_g - n_o) <= 1e-9
+        assert np.abs(plan.D.cpu().numpy() - d_o).max() <= 1e-10
+        assert abs(plan.trace.item() - n_g) == 0.0
+    # bf16, fixed 20 steps, power scale: the count is met to the bf16 trace tolerance (1e-3 n) around the oracle's mu
+    P16 = sm.sm_build_pattern(A, 64)
+    plan16 = sm.DensityPlan(A, P16, "bf16")
+    mu16, n16, _ = sm.sm_mu_search(A, P16, plan16, 96.0, -2.5, 2.5, tol_n=0.05, max_trials=30, scale_mode="power",
+                                   max_iter=20, tol=0.0)
+    assert abs(n16 - 96.0) <= 0.05 + 1e-3 * wl.n
+    with pytest.raises(sm.SmError):
+        sm.sm_mu_search(A, P, plan, 1000.0, -2.5, 2.5, max_iter=100, tol=1e-8)     # not bracketed
+
+
 def test_cfg1_fp64_and_fp32_all_columns(sm):
     wl = make_config(1)
     d_or, _ = orc.density_columns(wl, n_threads=THREADS)

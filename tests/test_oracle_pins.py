@@ -208,6 +208,33 @@ def test_full_coverage_equals_full_matrix_sign():
     assert (st.n_neg == n_neg).all()
 
 
+def test_mu_search_brackets_the_target_eigenvalue_in_the_full_coverage_limit():
+    # full coverage: Tr D(mu) = #{eigenvalues of H below mu} exactly, so the chemical potential that gives
+    # n_target electrons must lie strictly between eigenvalue n_target and eigenvalue n_target + 1 of H
+    # (numpy eigvalsh: independent of the oracle's Jacobi path)                     [PAPER.md:89-92, Eq. 14]
+    w = make_workload(10, 6, 3, np.inf, seed=5)
+    assert w.nnzb == w.n_blk ** 2
+    lam = np.linalg.eigvalsh(w.dense())
+    for n_target in (7, 30, 44):
+        mu, n, trials, d = orc.mu_search(w, n_target, -3.0, 3.0, tol_n=1e-8, n_threads=4)
+        assert lam[n_target - 1] < mu < lam[n_target], (mu, lam[n_target - 1], lam[n_target])
+        assert abs(n - n_target) < 1e-9 and abs(orc.trace(w, d) - n) < 1e-12
+        assert 3 <= trials <= 40
+    with pytest.raises(ValueError):
+        orc.mu_search(w, 200, -3.0, 3.0)              # more electrons than orbitals: not bracketed
+
+
+def test_trace_is_monotone_in_mu_away_from_the_limits():
+    w = make_config(0)
+    prev = -1.0
+    for mu in np.linspace(-2.5, 2.5, 11):
+        d, _ = orc.density_columns(w, mu=float(mu), n_threads=4)
+        t = orc.trace(w, d)
+        assert t >= prev - 1e-9
+        prev = t
+    assert prev == pytest.approx(w.n, abs=1e-9)        # everything occupied far above the spectrum
+
+
 def test_block_diagonal_limit_gives_block_projectors():
     w = make_config(0, cutoff=0.0)
     assert w.nnzb == w.n_blk
