@@ -46,7 +46,7 @@ def parse_args():
     ap.add_argument("--config", type=int, default=2)
     ap.add_argument("--run", type=int, default=0, help="index into the config's precision runs")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--scale", default=None, help="none|gershgorin|power (default: power for 16-bit)")
+    ap.add_argument("--scale", default=None, help="none|gershgorin|power|global (default: global for 16-bit, gershgorin otherwise)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -182,7 +182,9 @@ def run_ours(args, cfg, cfg_run):
     x_dtype = cfg_run["x_dtype"]
     is16 = x_dtype in ("bf16", "f16")
     pad = 64 if is16 else 16
-    scale_mode = args.scale or ("power" if is16 else "gershgorin")
+    # 16-bit, fixed iteration counts: SM_SCALE_GLOBAL (one interlacing bound from power steps on the block-sparse
+    # matrix; same error class as the per-submatrix power scale, no second gather -- DESIGN.md A10)
+    scale_mode = args.scale or ("global" if is16 else "gershgorin")
     max_iter, tol = cfg_run["max_iter"], cfg_run["tol"]
 
     # Weak scaling: every rank owns an independent replica of the workload (independent problems,

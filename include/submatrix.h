@@ -72,6 +72,9 @@ extern "C" {
 #define SM_SCALE_GERSHGORIN 1  /* s_i = max_r sum_c |(T_i - mu I)_rc|  (>= spectral radius) */
 #define SM_SCALE_POWER 2       /* s_i = 1.05 * ||T v||_2 after 10 power steps on T_i - mu I from a
                                   fixed start vector, never above the Gershgorin bound */
+#define SM_SCALE_GLOBAL 3      /* s_i = min(Gershgorin_i, 1.05 * ||(A - mu I) v||_2) after 10 power steps on the whole
+                                  block-sparse A - mu I: every T_i - mu I is a principal submatrix of it, so by Cauchy
+                                  interlacing rho(T_i - mu I) <= rho(A - mu I); one bound for all i, no second gather */
 
 /* Block-CSR description of the symmetric input A = H ("block-sparse"). */
 typedef struct {

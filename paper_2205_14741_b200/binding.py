@@ -24,11 +24,11 @@ _lib = C.CDLL(_SO)
 SM_OK, SM_ERR_ARG, SM_ERR_SPACE, SM_ERR_PATTERN, SM_ERR_CUDA, SM_ERR_UNSUPPORTED = 0, -1, -2, -3, -4, -5
 SM_WARN_NOT_CONVERGED = 1
 SM_F64, SM_F32, SM_BF16, SM_F16 = 0, 1, 2, 3
-SM_SCALE_NONE, SM_SCALE_GERSHGORIN, SM_SCALE_POWER = 0, 1, 2
+SM_SCALE_NONE, SM_SCALE_GERSHGORIN, SM_SCALE_POWER, SM_SCALE_GLOBAL = 0, 1, 2, 3
 
 DTYPES = {"f64": SM_F64, "f32": SM_F32, "bf16": SM_BF16, "f16": SM_F16}
 TORCH_DTYPE = {SM_F64: torch.float64, SM_F32: torch.float32, SM_BF16: torch.bfloat16, SM_F16: torch.float16}
-SCALES = {"none": SM_SCALE_NONE, "gershgorin": SM_SCALE_GERSHGORIN, "power": SM_SCALE_POWER}
+SCALES = {"none": SM_SCALE_NONE, "gershgorin": SM_SCALE_GERSHGORIN, "power": SM_SCALE_POWER, "global": SM_SCALE_GLOBAL}
 EXPORTS = ["sm_last_cuda_error", "sm_pattern_sizes", "sm_build_pattern", "sm_plan_columns",
            "sm_gather_ws_bytes", "sm_gather", "sm_sign_ws_bytes", "sm_sign_ns", "sm_sign_status",
            "sm_scatter", "sm_symmetrise", "sm_density_ws_bytes", "sm_density", "sm_density_from_sign",

@@ -107,6 +107,9 @@ int32_t prof_end(cudaStream_t st, int slot);
 
 // ---- internal entry points implemented across the .cu files
 int32_t exclusive_scan_i64(int32_t n, const int64_t *in, int64_t *out, cudaStream_t st);   // pattern.cu
+int64_t global_scale_ws_bytes(const sm_bcsr_t *A, const sm_pattern_t *P);                    // global_scale.cu
+int32_t global_scale(const sm_bcsr_t *A, const void *A_vals, int32_t a_dtype, const sm_pattern_t *P, double mu,
+                     int32_t n_cols, double *scale, void *ws, int64_t ws_bytes, cudaStream_t st);
 int32_t power_scale(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, const int64_t *col_off,
                     int32_t x_dtype, void *X, double *scale, double *ratio, cudaStream_t st);  // power_scale.cu
 int32_t sign_simt(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, const int64_t *col_off,

@@ -273,7 +273,7 @@ extern "C" int64_t sm_gather_ws_bytes(const sm_bcsr_t *A, const sm_pattern_t *P,
   cur.take<int64_t>(A->n_blk + 1);
   cur.take<double>((int64_t)A->n_blk * P->max_dim);
   cur.take<double>(A->n_blk);
-  return cur.used + 256;
+  return cur.used + 256 + global_scale_ws_bytes(A, P);
 }
 
 template <typename TA, typename TX, bool IMG>
@@ -297,7 +297,7 @@ extern "C" int32_t sm_gather(const sm_bcsr_t *A, const void *A_vals, int32_t a_d
   if (a_dtype != SM_F64 && a_dtype != SM_F32) return SM_ERR_UNSUPPORTED;
   if (dtype_bytes(x_dtype) == 0) return SM_ERR_UNSUPPORTED;
   if (is_16bit(x_dtype) && (P->pad_to % 64) != 0) return SM_ERR_ARG;
-  if (scale_mode < SM_SCALE_NONE || scale_mode > SM_SCALE_POWER) return SM_ERR_UNSUPPORTED;
+  if (scale_mode < SM_SCALE_NONE || scale_mode > SM_SCALE_GLOBAL) return SM_ERR_UNSUPPORTED;
   if (P->max_dim > 65535) return SM_ERR_UNSUPPORTED;
   cudaStream_t st = (cudaStream_t)stream;
   int32_t n = A->n_blk;
@@ -306,6 +306,7 @@ extern "C" int32_t sm_gather(const sm_bcsr_t *A, const void *A_vals, int32_t a_d
   double *babs = cur.take<double>((int64_t)n * P->max_dim);
   double *ratio = cur.take<double>(n);
   if (!cur.ok()) return SM_ERR_SPACE;
+  const int64_t g_off = align_up(cur.used, 256);        // SM_SCALE_GLOBAL: its own workspace behind these arrays
 
   if (scale_mode == SM_SCALE_NONE) {
     k_fill_double<<<(n_cols + 255) / 256, 256, 0, st>>>(n_cols, 1.0, scale);
@@ -324,6 +325,10 @@ extern "C" int32_t sm_gather(const sm_bcsr_t *A, const void *A_vals, int32_t a_d
     k_scale_gershgorin<<<n_cols, 128, 0, st>>>(cols, A->blk_size, A->row_ptr, A->col_idx, P->gmap_ptr,
                                                P->gmap, rowbase, babs, scale);
     SM_LAUNCHED();
+    if (scale_mode == SM_SCALE_GLOBAL) {
+      int32_t rcg = global_scale(A, A_vals, a_dtype, P, mu, n_cols, scale, (char *)ws + g_off, ws_bytes - g_off, st);
+      if (rcg != SM_OK) return rcg;
+    }
   }
 
   GatherArgs g{cols, col_off, A->row_ptr, A->val_ptr, P->row_off, P->gmap_ptr, P->gmap,

@@ -320,8 +320,20 @@ def test_cfg2_bf16_full_size_sampled(sm):
     _, P, plan = run_density(sm, wl, "bf16", run["max_iter"], 0.0, "power", symmetrise=False)
     assert (plan.iters == run["max_iter"]).all()
     e = sampled_errors(wl, P, plan, sample_columns(wl, 24, 4242), run["max_iter"])
+    print("cfg2 power-scale errors", e)
     assert e["total"] <= 2e-2 and e["dtr"] <= 1e-3, e
     assert e["rounding"] <= 1.2e-2, e            # bf16 rounding alone, against the NS-20 polynomial
+
+
+def test_cfg2_bf16_full_size_global_scale(sm):
+    # SM_SCALE_GLOBAL (one interlacing bound from power steps on the whole block-sparse matrix): bench.py's scale mode
+    wl = make_config(2)
+    run = CONFIGS[2]["runs"][0]
+    _, P, plan = run_density(sm, wl, "bf16", run["max_iter"], 0.0, "global", symmetrise=False)
+    e = sampled_errors(wl, P, plan, sample_columns(wl, 24, 4242), run["max_iter"])
+    print("cfg2 global-scale errors", e)
+    assert e["total"] <= 2e-2 and e["dtr"] <= 1e-3, e
+    assert e["rounding"] <= 1.2e-2, e
 
 
 def test_cfg3_fp16_full_size_sampled(sm):
@@ -334,11 +346,12 @@ def test_cfg3_fp16_full_size_sampled(sm):
     assert np.float32(e["maxabs"]) <= np.float32(2e-3), e
 
 
-@pytest.mark.parametrize("x_dtype", ["bf16", "f16"])
-def test_cfg4_16bit_full_size_sampled(sm, x_dtype):
+@pytest.mark.parametrize("x_dtype,scale_mode", [("bf16", "power"), ("f16", "power"), ("bf16", "global")])
+def test_cfg4_16bit_full_size_sampled(sm, x_dtype, scale_mode):
     wl = make_config(4)
-    _, P, plan = run_density(sm, wl, x_dtype, 25, 0.0, "power")
+    _, P, plan = run_density(sm, wl, x_dtype, 25, 0.0, scale_mode)
     e = sampled_errors(wl, P, plan, sample_columns(wl, 4, 4242), 25)
+    print("cfg4", x_dtype, scale_mode, e)
     assert e["total"] <= 2e-2 and e["dtr"] <= 1e-3, e
 
 
@@ -404,3 +417,32 @@ def test_power_scale_is_a_valid_tight_deterministic_bound(sm):
     for i in (0, 13, 59):
         rho = np.abs(np.linalg.eigvalsh(orc.gather(wl, i))).max()
         assert 0.80 * rho <= sp[i] <= 1.06 * rho, (i, sp[i], rho)  # Newton-Schulz needs |x| < sqrt(3): s > rho / 1.73
+
+
+def test_global_scale_is_a_valid_deterministic_bound(sm):
+    # Cauchy interlacing: rho(T_i - mu I) <= rho(A - mu I) for every principal submatrix; the power estimate is a
+    # lower bound of rho(A - mu I) times 1.05, and Newton-Schulz needs rho(T_i) / s_i < sqrt(3)
+    wl = make_workload(60, 23, 4, 5.0, seed=21)
+    A = sm.Bcsr(wl)
+    P = sm.sm_build_pattern(A, 64)
+    cols, col_off, n = sm.sm_plan_columns(P, None)
+    for mu in (0.0, 0.4):
+        _, sg = sm.sm_gather(A, P, cols, col_off, n, mu, "gershgorin", "bf16")
+        _, s1 = sm.sm_gather(A, P, cols, col_off, n, mu, "global", "bf16")
+        _, s2 = sm.sm_gather(A, P, cols, col_off, n, mu, "global", "bf16")
+        assert torch.equal(s1, s2)
+        sg, s1 = sg.cpu().numpy(), s1.cpu().numpy()
+        assert (s1 <= sg * (1 + 1e-12)).all()
+        rho_a = np.abs(np.linalg.eigvalsh(wl.dense() - mu * np.eye(wl.n))).max()
+        assert s1.max() <= 1.05 * rho_a * (1 + 1e-12)                 # est is a lower bound of rho(A - mu I)
+        assert s1.max() >= 0.75 * rho_a                               # and a useful one after 10 steps
+        for i in range(wl.n_blk):
+            T = orc.gather(wl, i, mu)
+            rho = np.abs(np.linalg.eigvalsh(T)).max()
+            assert rho <= rho_a * (1 + 1e-12)                         # interlacing itself
+            assert rho / s1[i] < 1.5, (i, rho, s1[i])                 # inside the convergence interval
+    # the fp64 path converges to the exact sign with this scale as well
+    wl0 = make_config(0)
+    d_or, _ = orc.density_columns(wl0, n_threads=THREADS)
+    _, _, plan = run_density(sm, wl0, "f64", 100, 1e-8, "global")
+    assert np.abs(plan.D.cpu().numpy() - d_or).max() <= 1e-10
