@@ -52,9 +52,13 @@ constexpr uint32_t TMEM_COLS = 512;
 // 128 rows with the WHOLE B tile in its shared memory; each CTA fetches half of the B rows and multicasts
 // them to both (cp.async.bulk ... multicast::cluster), so the L2 -> SM bytes equal those of the cta_group::2
 // pair while no CTA waits on a relayed "peer's stage landed" signal.
-template <int NCTA, bool MC = false> struct UCfg {
+// NST: depth of the operand ring (0 = the default of the variant).  Measured on B200, sm_sign_ns alone: at
+// configs[4] (m ~ 1650) single CTAs run 25 steps in 653 ms with 3 stages and 747 ms with 4 (2 stages: 734 ms) --
+// a shallower ring keeps the CTAs that share a submatrix's operand panels closer together in L2 --
+// while configs[2] (m ~ 410) prefers 4 (27.8 vs 28.7 ms).
+template <int NCTA, bool MC = false, int NST = 0> struct UCfg {
   static constexpr bool G2 = NCTA == 2 && !MC;             // cta_group::2 MMA
-  static constexpr int STAGES = G2 ? 6 : 4;
+  static constexpr int STAGES = NST ? NST : (G2 ? 6 : 4);
   static constexpr int B_BYTES = (G2 ? UN / 2 : UN) * UK * 2;   // 16 KB / 32 KB
   static constexpr int STAGE_BYTES = A_BYTES + B_BYTES;    // 48 KB / 32 KB
   static constexpr int SMEM = STAGES * STAGE_BYTES + EPI_STAGE_BYTES + IDENT_BYTES + 1024 /*align slack*/ + 256 /*barriers*/;
@@ -244,10 +248,10 @@ __device__ __forceinline__ void mirror_store(uint16_t *Og, int32_t Pd, int32_t R
 //              form damps (++ block) or leaves unchanged (+- block) an antisymmetric rounding residue,
 //              so exact symmetry is not needed; it trades 1.3-1.7x more MMA work for an epilogue
 //              without transposes, which is what bounds the m < ~1000 regime (ncu, round 1).
-template <bool BF16, int PHASE, int NCTA, bool SYM, bool MC = false>
+template <bool BF16, int PHASE, int NCTA, bool SYM, bool MC = false, int NST = 0>
 __global__ void __launch_bounds__(UMMA_THREADS, 1) k_umma_gemm(UArgs a) {
   static_assert(!MC || (NCTA == 2 && SYM), "multicast variant: two CTAs, SYM tiles");
-  using Cfg = UCfg<NCTA, MC>;
+  using Cfg = UCfg<NCTA, MC, NST>;
   constexpr int USTAGES = Cfg::STAGES;
   constexpr int STAGE_BYTES = Cfg::STAGE_BYTES;
   constexpr bool PAIR = NCTA == 2 && !MC;                  // cta_group::2 MMAs issued by the leader
@@ -606,10 +610,11 @@ struct UmmaWs {
   int32_t parts_per_col; int64_t used;
 };
 
-// CTAs per tile.  Measured on B200: CTA pairs (cta_group::2, 256-row tiles) win where a tile's main loop
-// is long (configs[4], m ~ 1650: 15.1 vs 16.3 ms per launch), single CTAs win where the per-tile
-// epilogue and hand-offs dominate (configs[2], m ~ 410: 0.77 vs 0.85 ms).  Decided per call from the
-// pattern's largest submatrix; SM_UMMA_NCTA=1/2 in the environment overrides (A/B measurements).
+// CTAs per tile.  Measured on B200 (sm_sign_ns alone, same box): configs[4], m ~ 1650, 25 steps: single CTAs with a
+// 3-stage ring 653 ms, two CTAs with multicast 672 (3 stages) / 727 ms (4), cta_group::2 pairs with a relayed
+// stage signal 682-762 ms, single CTAs with 4 stages 747 ms; configs[2], m ~ 410, 20 steps: single CTAs 27.8 ms
+// (4 stages), two CTAs 31-32 ms.  So single CTAs are the default and the ring depth follows the size;
+// SM_UMMA_NCTA=1/2 (and SM_UMMA_MC, SM_UMMA_STAGES) in the environment override (A/B measurements, tests).
 static int32_t umma_ncta(const sm_pattern_t *P) {
   static int32_t env = -2;
   if (env == -2) {
@@ -617,7 +622,8 @@ static int32_t umma_ncta(const sm_pattern_t *P) {
     env = e ? (e[0] == '1' ? 1 : 2) : -1;
   }
   if (env > 0) return env;
-  return P->max_dim > 1024 ? 2 : 1;
+  (void)P;
+  return 1;     // measured (B200): single CTAs win at every config once the ring depth follows the size (UCfg)
 }
 
 // Two-CTA tiles: cta_group::2 MMAs with a relayed "stage landed" (0) or two cta_group::1 MMAs with the B rows
@@ -695,12 +701,12 @@ int64_t sign_umma_ws_bytes(const sm_pattern_t *P, int32_t n_cols, int64_t packed
   return umma_layout(nullptr, 0, P, n_cols, packed_elems).used;
 }
 
-template <bool BF16, int PHASE, int NCTA, bool SYM, bool MC = false>
+template <bool BF16, int PHASE, int NCTA, bool SYM, bool MC = false, int NST = 0>
 static int32_t launch_umma(const UArgs &a, int32_t n_sm, cudaStream_t st) {
   static bool configured = false;
   if (!configured) {
-    SM_CUDA(cudaFuncSetAttribute(k_umma_gemm<BF16, PHASE, NCTA, SYM, MC>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 UCfg<NCTA, MC>::SMEM));
+    SM_CUDA(cudaFuncSetAttribute(k_umma_gemm<BF16, PHASE, NCTA, SYM, MC, NST>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 UCfg<NCTA, MC, NST>::SMEM));
     configured = true;
   }
   int slot = -1;
@@ -708,13 +714,13 @@ static int32_t launch_umma(const UArgs &a, int32_t n_sm, cudaStream_t st) {
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3((unsigned)(n_sm / NCTA * NCTA), 1, 1);     // one CTA per SM, whole pairs
   cfg.blockDim = dim3(UMMA_THREADS, 1, 1);
-  cfg.dynamicSmemBytes = UCfg<NCTA, MC>::SMEM;
+  cfg.dynamicSmemBytes = UCfg<NCTA, MC, NST>::SMEM;
   cfg.stream = st;
   cudaLaunchAttribute attr[1];
   attr[0].id = cudaLaunchAttributeClusterDimension;
   attr[0].val.clusterDim.x = NCTA; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
   cfg.attrs = attr; cfg.numAttrs = 1;
-  SM_CUDA(cudaLaunchKernelEx(&cfg, k_umma_gemm<BF16, PHASE, NCTA, SYM, MC>, a));
+  SM_CUDA(cudaLaunchKernelEx(&cfg, k_umma_gemm<BF16, PHASE, NCTA, SYM, MC, NST>, a));
   SM_LAUNCHED();
   return prof_end(st, slot);
 }
@@ -742,13 +748,16 @@ static int32_t launch_fused(const FArgs &a, int32_t n_sm, cudaStream_t st) {
   return prof_end(st, slot);
 }
 
-template <int PHASE, int NCTA, bool SYM, bool MC = false>
+template <int PHASE, int NCTA, bool SYM, bool MC = false, int NST = 0>
 static int32_t launch_umma_t(bool bf16, const UArgs &a, int32_t n_sm, cudaStream_t st) {
-  return bf16 ? launch_umma<true, PHASE, NCTA, SYM, MC>(a, n_sm, st) : launch_umma<false, PHASE, NCTA, SYM, MC>(a, n_sm, st);
+  return bf16 ? launch_umma<true, PHASE, NCTA, SYM, MC, NST>(a, n_sm, st)
+              : launch_umma<false, PHASE, NCTA, SYM, MC, NST>(a, n_sm, st);
 }
 template <int PHASE>
-static int32_t launch_umma_any(bool bf16, int32_t ncta, int32_t sym, const UArgs &a, int32_t n_sm, cudaStream_t st) {
+static int32_t launch_umma_any(bool bf16, int32_t ncta, int32_t sym, int32_t nst, const UArgs &a, int32_t n_sm,
+                               cudaStream_t st) {
   if (ncta == 3) return launch_umma_t<PHASE, 2, true, true>(bf16, a, n_sm, st);     // two CTAs, multicast B (SYM only)
+  if (ncta == 1 && sym && nst == 3) return launch_umma_t<PHASE, 1, true, false, 3>(bf16, a, n_sm, st);
   if (ncta == 2) return sym ? launch_umma_t<PHASE, 2, true>(bf16, a, n_sm, st) : launch_umma_t<PHASE, 2, false>(bf16, a, n_sm, st);
   return sym ? launch_umma_t<PHASE, 1, true>(bf16, a, n_sm, st) : launch_umma_t<PHASE, 1, false>(bf16, a, n_sm, st);
 }
@@ -810,6 +819,9 @@ int32_t sign_umma(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, co
     return SM_OK;
   }
   const int32_t mode = (ncta == 2 && sym && umma_mc()) ? 3 : ncta;    // 3: two CTAs per tile, multicast B
+  static int32_t nst_env = -1;    // SM_UMMA_STAGES=3|4: ring depth of the single-CTA SYM kernel (A/B measurements)
+  if (nst_env < 0) { const char *e = getenv("SM_UMMA_STAGES"); nst_env = e ? atoi(e) : 0; }
+  const int32_t nst = nst_env ? nst_env : (P->max_dim > 1024 ? 3 : 4);
   static int32_t rev_on = -1;     // SM_UMMA_REV=0 keeps every launch walking forwards (A/B measurements)
   if (rev_on < 0) { const char *e = getenv("SM_UMMA_REV"); rev_on = (e && e[0] == '0') ? 0 : 1; }
   void *buf[2] = {X, w.X2};
@@ -817,14 +829,14 @@ int32_t sign_umma(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, co
     void *src = buf[k & 1], *dst = buf[(k + 1) & 1];
     UArgs a{cols, col_off, P->dim, P->dim_pad, w.tile_ptr, w.tiles, n_cols, tol > 0.0 ? 1 : 0, src, w.Y, w.Y, s, w.err, 0, umma_dbg()};
     a.rev = 0;
-    int32_t rc = launch_umma_any<1>(bf16, mode, sym, a, n_sm, st);
+    int32_t rc = launch_umma_any<1>(bf16, mode, sym, nst, a, n_sm, st);
     if (rc != SM_OK) return rc;
     SM_CUDA(cudaMemsetAsync(w.n_still, 0, sizeof(int32_t), st));
     k_sign_post<<<(n_cols + 7) / 8, 256, 0, st>>>(n_cols, cols, P->dim, s, w.n_parts, tol, iters, residual);
     SM_LAUNCHED();
     a.Out = dst;
     a.rev = rev_on;            // PHASE 2 starts where PHASE 1 ended, the next PHASE 1 where this launch ends
-    rc = launch_umma_any<2>(bf16, mode, sym, a, n_sm, st);
+    rc = launch_umma_any<2>(bf16, mode, sym, nst, a, n_sm, st);
     if (rc != SM_OK) return rc;
     if (tol > 0.0 && k >= 5 && (k & 1)) {
       int32_t still = 1;

@@ -3,6 +3,7 @@ environment forces (each in its own process: the selection is read once per proc
   SM_UMMA_NCTA=1|2   one CTA / two CTAs per tile of the tcgen05 kernel
   SM_UMMA_MC=1|0     two CTAs: own cta_group::1 MMAs with the B rows multicast / cta_group::2 MMAs with a relayed stage signal
   SM_UMMA_REV=1|0    PHASE 2 walks the tile table backwards / forwards
+  SM_UMMA_STAGES=3|4 depth of the operand ring of the single-CTA kernel
   SM_UMMA_SLOTS=2|1  submatrices a CTA pair of the fused kernel interleaves
   SM_UMMA_SYM=1|0    symmetric half tiles with mirrored stores / true products with an MN-major B operand
   SM_UMMA_FUSED=1|0  one launch runs every step of a submatrix (k_umma_fused) / one launch per product
@@ -103,6 +104,7 @@ HASH_SNIPPET = textwrap.dedent("""
 SYM_VARIANTS = [
     {"SM_UMMA_FUSED": "0", "SM_UMMA_NCTA": "1"},
     {"SM_UMMA_FUSED": "0", "SM_UMMA_NCTA": "1", "SM_UMMA_REV": "0"},
+    {"SM_UMMA_FUSED": "0", "SM_UMMA_NCTA": "1", "SM_UMMA_STAGES": "3"},
     {"SM_UMMA_FUSED": "0", "SM_UMMA_NCTA": "2", "SM_UMMA_MC": "1"},
     {"SM_UMMA_FUSED": "0", "SM_UMMA_NCTA": "2", "SM_UMMA_MC": "0"},
     {"SM_UMMA_FUSED": "1", "SM_UMMA_SLOTS": "1"},
