@@ -211,6 +211,7 @@ int32_t sm_density_from_sign(const sm_bcsr_t *A, const sm_pattern_t *P, int32_t 
  * code leaves them unset and gets the measured-best variant for the pattern's largest submatrix):
  *   SM_UMMA_NCTA=1|2   16-bit: one CTA / two CTAs of a cluster per output tile
  *   SM_UMMA_MC=1|0     16-bit, two CTAs: cta_group::1 MMAs with the B rows multicast / cta_group::2 MMAs (relay)
+ *   SM_UMMA_TMAP=1     16-bit, cta_group::2 pairs: operands through tensor-map TMA that signals the leader's barrier (no relay)
  *   SM_UMMA_SYM=1|0    16-bit: lower-triangle tiles with mirrored stores / true products, all tiles
  *   SM_UMMA_REV=1|0    16-bit: the update product walks the tile table backwards / forwards
  *   SM_UMMA_STAGES=3|4 16-bit, one CTA per tile: depth of the operand ring

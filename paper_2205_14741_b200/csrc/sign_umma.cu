@@ -19,6 +19,7 @@
 // (2 x 256 columns) so the epilogue of tile t overlaps the main loop of tile t+1; 4-stage smem ring.
 //   PHASE 1: W = X X^T - I, epilogue writes W and the fused ||W||_F^2 partial sums (warp shuffles).
 //   PHASE 2: X' = X - 0.5 X W^T (= 1.5 X - 0.5 X Y), epilogue reads the X tile and writes X'.
+#include <cuda.h>   // CUtensorMap (type only; the encoder is fetched through cudaGetDriverEntryPoint)
 #include <cstdio>
 #include <cstdlib>
 #include <utility>
@@ -248,9 +249,14 @@ __device__ __forceinline__ void mirror_store(uint16_t *Og, int32_t Pd, int32_t R
 //              form damps (++ block) or leaves unchanged (+- block) an antisymmetric rounding residue,
 //              so exact symmetry is not needed; it trades 1.3-1.7x more MMA work for an epilogue
 //              without transposes, which is what bounds the m < ~1000 regime (ncu, round 1).
-template <bool BF16, int PHASE, int NCTA, bool SYM, bool MC = false, int NST = 0>
-__global__ void __launch_bounds__(UMMA_THREADS, 1) k_umma_gemm(UArgs a) {
+// TM (cta_group::2 pairs only): operands come through tensor-map TMA (2-D view of the packed buffer: rows of 64
+// elements, no swizzle -- the image is stored pre-swizzled) with `.cta_group::2`, which lets BOTH CTAs of a pair
+// credit their bytes to the LEADER's "stage full" barrier; no relay warp, no second barrier wait per stage.
+template <bool BF16, int PHASE, int NCTA, bool SYM, bool MC = false, int NST = 0, bool TM = false>
+__global__ void __launch_bounds__(UMMA_THREADS, 1)
+k_umma_gemm(UArgs a, const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapB) {
   static_assert(!MC || (NCTA == 2 && SYM), "multicast variant: two CTAs, SYM tiles");
+  static_assert(!TM || (NCTA == 2 && SYM && !MC), "tensor-map variant: cta_group::2 pairs, SYM tiles");
   using Cfg = UCfg<NCTA, MC, NST>;
   constexpr int USTAGES = Cfg::STAGES;
   constexpr int STAGE_BYTES = Cfg::STAGE_BYTES;
@@ -323,6 +329,27 @@ __global__ void __launch_bounds__(UMMA_THREADS, 1) k_umma_gemm(UArgs a) {
         const uint32_t a_bytes = a_rows * 128u;
         const uint32_t b_bytes = SYM ? (uint32_t)b_cnt * 128u : (uint32_t)n_atoms * 8192u;
         const int nkc = (u.kmax + UK - 1) / UK;
+        if (TM) {
+          // boxes: 128 rows (A: one copy; rows past the padded dimension are harmless) and 64 rows (B: b_cnt rounded
+          // up to whole boxes -- few, large copies: ten 2 KB boxes per stage kept the producer thread busy longer
+          // than the stage's MMAs take)
+          const uint32_t other_rows = (uint32_t)max(0, min(UM, u.Pd - (u.row0 + (int32_t)(1u - h) * UM)));
+          const int32_t nb64 = (b_cnt + 63) >> 6;
+          const uint32_t tx_all = ((a_rows ? 128u : 0u) + (other_rows ? 128u : 0u)) * 128u + 2u * (uint32_t)nb64 * 8192u;
+          const int32_t row_base = (int32_t)(u.base >> 6);            // first image row of the submatrix
+          for (int kc = 0; kc < nkc; ++kc) {
+            ptx::mbar_wait(empty_bar(stage), phase ^ 1u, a.err_flag, 1);
+            const uint32_t sa = tiles + stage * STAGE_BYTES, sb = sa + A_BYTES;
+            const uint32_t lead_full = ptx::mapa_u32(full_bar(stage), 0);
+            if (h == 0) ptx::mbar_expect_tx(full_bar(stage), tx_all);
+            const int32_t y0 = row_base + kc * u.Pd;
+            if (a_rows) ptx::tma_tensor2d_g2s_2cta(sa, &mapA, 0, y0 + arow0, lead_full);
+            for (int32_t j = 0; j < nb64; ++j)
+              ptx::tma_tensor2d_g2s_2cta(sb + (uint32_t)j * 8192u, &mapB, 0, y0 + brow0 + j * 64, lead_full);
+            if (++stage == USTAGES) { stage = 0; phase ^= 1u; }
+          }
+          continue;
+        }
         for (int kc = 0; kc < nkc; ++kc) {
           ptx::mbar_wait(empty_bar(stage), phase ^ 1u, a.err_flag, 1);
           const uint32_t sa = tiles + stage * STAGE_BYTES, sb = sa + A_BYTES;
@@ -348,7 +375,7 @@ __global__ void __launch_bounds__(UMMA_THREADS, 1) k_umma_gemm(UArgs a) {
         }
       }
     }
-  } else if (PAIR && warp == 1 && h != 0) {
+  } else if (PAIR && !TM && warp == 1 && h != 0) {
     // ===================== relay (peer CTA of a pair): tell the leader that this CTA's stage landed ======
     if (lane == 0) {
       int stage = 0; uint32_t phase = 0;
@@ -367,8 +394,8 @@ __global__ void __launch_bounds__(UMMA_THREADS, 1) k_umma_gemm(UArgs a) {
       }
     }
   } else if (warp == 1) {
-    // ===================== MMA issuer (leader CTA) =====================
-    if (lane == 0) {
+    // ===================== MMA issuer (leader CTA; every CTA when each issues its own MMAs) =====================
+    if (lane == 0 && !(PAIR && h != 0)) {
       int stage = 0; uint32_t phase = 0;
       uint32_t it = 0;
       TileDesc nxt = load_desc(a, max((int64_t)0, min(unit, total - 1)));
@@ -385,7 +412,7 @@ __global__ void __launch_bounds__(UMMA_THREADS, 1) k_umma_gemm(UArgs a) {
         const int nkc = (u.kmax + UK - 1) / UK;
         for (int kc = 0; kc < nkc; ++kc) {
           ptx::mbar_wait(full_bar(stage), phase, a.err_flag, 3);
-          if (PAIR) ptx::mbar_wait(pfull_bar(stage), phase, a.err_flag, 6);
+          if (PAIR && !TM) ptx::mbar_wait(pfull_bar(stage), phase, a.err_flag, 6);
           ptx::tc_fence_after();
           const uint32_t sa = tiles + stage * STAGE_BYTES, sb = sa + A_BYTES;
           const uint64_t adesc = ptx::make_sw128_kmajor_desc(sa);
@@ -701,11 +728,36 @@ int64_t sign_umma_ws_bytes(const sm_pattern_t *P, int32_t n_cols, int64_t packed
   return umma_layout(nullptr, 0, P, n_cols, packed_elems).used;
 }
 
-template <bool BF16, int PHASE, int NCTA, bool SYM, bool MC = false, int NST = 0>
-static int32_t launch_umma(const UArgs &a, int32_t n_sm, cudaStream_t st) {
+// 2-D tensor maps over a packed 16-bit buffer seen as rows of 64 elements (128 bytes): box = 64 x box_rows, no
+// swizzle (the image is stored pre-swizzled).  Used by the TM variant only; the others get zeroed maps.
+struct UMaps { CUtensorMap a, b; };
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+static int32_t make_map(CUtensorMap *m, void *buf, int64_t packed_elems, uint32_t box_rows) {
+  static EncodeTiledFn fn = nullptr;
+  if (!fn) {
+    void *p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    SM_CUDA(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q));
+    if (!p || q != cudaDriverEntryPointSuccess) return SM_ERR_UNSUPPORTED;
+    fn = (EncodeTiledFn)p;
+  }
+  cuuint64_t gdim[2] = {64, (cuuint64_t)(packed_elems / 64)};
+  cuuint64_t gstr[1] = {128};
+  cuuint32_t box[2] = {64, box_rows};
+  cuuint32_t estr[2] = {1, 1};
+  CUresult r = fn(m, CU_TENSOR_MAP_DATA_TYPE_UINT16, 2, buf, gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                  CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) { g_last_cuda_error = (int32_t)r; return SM_ERR_CUDA; }
+  return SM_OK;
+}
+
+template <bool BF16, int PHASE, int NCTA, bool SYM, bool MC = false, int NST = 0, bool TM = false>
+static int32_t launch_umma(const UArgs &a, const UMaps &maps, int32_t n_sm, cudaStream_t st) {
   static bool configured = false;
   if (!configured) {
-    SM_CUDA(cudaFuncSetAttribute(k_umma_gemm<BF16, PHASE, NCTA, SYM, MC, NST>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    SM_CUDA(cudaFuncSetAttribute(k_umma_gemm<BF16, PHASE, NCTA, SYM, MC, NST, TM>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                  UCfg<NCTA, MC, NST>::SMEM));
     configured = true;
   }
@@ -720,7 +772,7 @@ static int32_t launch_umma(const UArgs &a, int32_t n_sm, cudaStream_t st) {
   attr[0].id = cudaLaunchAttributeClusterDimension;
   attr[0].val.clusterDim.x = NCTA; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
   cfg.attrs = attr; cfg.numAttrs = 1;
-  SM_CUDA(cudaLaunchKernelEx(&cfg, k_umma_gemm<BF16, PHASE, NCTA, SYM, MC, NST>, a));
+  SM_CUDA(cudaLaunchKernelEx(&cfg, k_umma_gemm<BF16, PHASE, NCTA, SYM, MC, NST, TM>, a, maps.a, maps.b));
   SM_LAUNCHED();
   return prof_end(st, slot);
 }
@@ -748,18 +800,22 @@ static int32_t launch_fused(const FArgs &a, int32_t n_sm, cudaStream_t st) {
   return prof_end(st, slot);
 }
 
-template <int PHASE, int NCTA, bool SYM, bool MC = false, int NST = 0>
-static int32_t launch_umma_t(bool bf16, const UArgs &a, int32_t n_sm, cudaStream_t st) {
-  return bf16 ? launch_umma<true, PHASE, NCTA, SYM, MC, NST>(a, n_sm, st)
-              : launch_umma<false, PHASE, NCTA, SYM, MC, NST>(a, n_sm, st);
+template <int PHASE, int NCTA, bool SYM, bool MC = false, int NST = 0, bool TM = false>
+static int32_t launch_umma_t(bool bf16, const UArgs &a, const UMaps &m, int32_t n_sm, cudaStream_t st) {
+  return bf16 ? launch_umma<true, PHASE, NCTA, SYM, MC, NST, TM>(a, m, n_sm, st)
+              : launch_umma<false, PHASE, NCTA, SYM, MC, NST, TM>(a, m, n_sm, st);
 }
+// mode: 1 = one CTA per tile, 2 = cta_group::2 pair with relay, 3 = two CTAs with multicast B, 4 = pair with tensor maps
 template <int PHASE>
-static int32_t launch_umma_any(bool bf16, int32_t ncta, int32_t sym, int32_t nst, const UArgs &a, int32_t n_sm,
-                               cudaStream_t st) {
-  if (ncta == 3) return launch_umma_t<PHASE, 2, true, true>(bf16, a, n_sm, st);     // two CTAs, multicast B (SYM only)
-  if (ncta == 1 && sym && nst == 3) return launch_umma_t<PHASE, 1, true, false, 3>(bf16, a, n_sm, st);
-  if (ncta == 2) return sym ? launch_umma_t<PHASE, 2, true>(bf16, a, n_sm, st) : launch_umma_t<PHASE, 2, false>(bf16, a, n_sm, st);
-  return sym ? launch_umma_t<PHASE, 1, true>(bf16, a, n_sm, st) : launch_umma_t<PHASE, 1, false>(bf16, a, n_sm, st);
+static int32_t launch_umma_any(bool bf16, int32_t mode, int32_t sym, int32_t nst, const UArgs &a, const UMaps &m,
+                               int32_t n_sm, cudaStream_t st) {
+  if (mode == 4) return nst == 3 ? launch_umma_t<PHASE, 2, true, false, 3, true>(bf16, a, m, n_sm, st)
+                      : nst == 4 ? launch_umma_t<PHASE, 2, true, false, 4, true>(bf16, a, m, n_sm, st)
+                                 : launch_umma_t<PHASE, 2, true, false, 6, true>(bf16, a, m, n_sm, st);
+  if (mode == 3) return launch_umma_t<PHASE, 2, true, true>(bf16, a, m, n_sm, st);
+  if (mode == 1 && sym && nst == 3) return launch_umma_t<PHASE, 1, true, false, 3>(bf16, a, m, n_sm, st);
+  if (mode == 2) return sym ? launch_umma_t<PHASE, 2, true>(bf16, a, m, n_sm, st) : launch_umma_t<PHASE, 2, false>(bf16, a, m, n_sm, st);
+  return sym ? launch_umma_t<PHASE, 1, true>(bf16, a, m, n_sm, st) : launch_umma_t<PHASE, 1, false>(bf16, a, m, n_sm, st);
 }
 
 int32_t sign_umma(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, const int64_t *col_off,
@@ -818,10 +874,21 @@ int32_t sign_umma(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, co
     SM_LAUNCHED();
     return SM_OK;
   }
-  const int32_t mode = (ncta == 2 && sym && umma_mc()) ? 3 : ncta;    // 3: two CTAs per tile, multicast B
+  static int32_t tmap_env = -1;   // SM_UMMA_TMAP=1: cta_group::2 pairs load through tensor maps (with SM_UMMA_NCTA=2 SM_UMMA_MC=0)
+  if (tmap_env < 0) { const char *e = getenv("SM_UMMA_TMAP"); tmap_env = (e && e[0] == '1') ? 1 : 0; }
+  const int32_t mode = (ncta == 2 && sym && umma_mc()) ? 3 : (ncta == 2 && sym && tmap_env) ? 4 : ncta;
+  UMaps maps[3] = {};              // per buffer: X, alternate X, W (mode 4 only)
+  if (mode == 4) {
+    void *bufs[3] = {X, w.X2, w.Y};
+    for (int b = 0; b < 3; ++b) {
+      int32_t rc = make_map(&maps[b].a, bufs[b], packed_elems, 128);
+      if (rc == SM_OK) rc = make_map(&maps[b].b, bufs[b], packed_elems, 64);
+      if (rc != SM_OK) return rc;
+    }
+  }
   static int32_t nst_env = -1;    // SM_UMMA_STAGES=3|4: ring depth of the single-CTA SYM kernel (A/B measurements)
   if (nst_env < 0) { const char *e = getenv("SM_UMMA_STAGES"); nst_env = e ? atoi(e) : 0; }
-  const int32_t nst = nst_env ? nst_env : (P->max_dim > 1024 ? 3 : 4);
+  const int32_t nst = nst_env ? nst_env : (mode == 4 ? 6 : (P->max_dim > 1024 ? 3 : 4));
   static int32_t rev_on = -1;     // SM_UMMA_REV=0 keeps every launch walking forwards (A/B measurements)
   if (rev_on < 0) { const char *e = getenv("SM_UMMA_REV"); rev_on = (e && e[0] == '0') ? 0 : 1; }
   void *buf[2] = {X, w.X2};
@@ -829,14 +896,15 @@ int32_t sign_umma(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, co
     void *src = buf[k & 1], *dst = buf[(k + 1) & 1];
     UArgs a{cols, col_off, P->dim, P->dim_pad, w.tile_ptr, w.tiles, n_cols, tol > 0.0 ? 1 : 0, src, w.Y, w.Y, s, w.err, 0, umma_dbg()};
     a.rev = 0;
-    int32_t rc = launch_umma_any<1>(bf16, mode, sym, nst, a, n_sm, st);
+    const UMaps m1{maps[k & 1].a, maps[k & 1].b}, m2{maps[k & 1].a, maps[2].b};
+    int32_t rc = launch_umma_any<1>(bf16, mode, sym, nst, a, m1, n_sm, st);
     if (rc != SM_OK) return rc;
     SM_CUDA(cudaMemsetAsync(w.n_still, 0, sizeof(int32_t), st));
     k_sign_post<<<(n_cols + 7) / 8, 256, 0, st>>>(n_cols, cols, P->dim, s, w.n_parts, tol, iters, residual);
     SM_LAUNCHED();
     a.Out = dst;
     a.rev = rev_on;            // PHASE 2 starts where PHASE 1 ended, the next PHASE 1 where this launch ends
-    rc = launch_umma_any<2>(bf16, mode, sym, nst, a, n_sm, st);
+    rc = launch_umma_any<2>(bf16, mode, sym, nst, a, m2, n_sm, st);
     if (rc != SM_OK) return rc;
     if (tol > 0.0 && k >= 5 && (k & 1)) {
       int32_t still = 1;

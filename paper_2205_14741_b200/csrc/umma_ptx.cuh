@@ -202,6 +202,24 @@ __device__ __forceinline__ void umma_commit_2cta(uint32_t bar) {
       : "memory");
 }
 
+// ---- tensor-map TMA for CTA pairs ----------------------------------------------------------------
+// shared::cluster address of `addr` (a shared::cta address of this CTA) in CTA `rank` of the cluster.
+__device__ __forceinline__ uint32_t mapa_u32(uint32_t addr, uint32_t rank) {
+  uint32_t r;
+  asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(addr), "r"(rank));
+  return r;
+}
+// 2-D tiled copy global -> this CTA's shared memory whose bytes are credited to an mbarrier that may live in the
+// OTHER CTA of the pair (cta_group::2): both CTAs of a pair signal the leader's "stage full" barrier directly.
+__device__ __forceinline__ void tma_tensor2d_g2s_2cta(uint32_t dst_smem, const void *tmap, int32_t c0, int32_t c1,
+                                                      uint32_t bar_cluster) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];" ::"r"(
+          dst_smem),
+      "l"(tmap), "r"(c0), "r"(c1), "r"(bar_cluster)
+      : "memory");
+}
+
 // ---- cluster multicast (two single-MMA CTAs sharing the B operand) -------------------------------
 // Bulk copy delivered to the same CTA-relative shared-memory offset (and complete_tx on the same
 // CTA-relative mbarrier) in every CTA of `mask`.

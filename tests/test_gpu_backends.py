@@ -2,6 +2,7 @@
 environment forces (each in its own process: the selection is read once per process):
   SM_UMMA_NCTA=1|2   one CTA / two CTAs per tile of the tcgen05 kernel
   SM_UMMA_MC=1|0     two CTAs: own cta_group::1 MMAs with the B rows multicast / cta_group::2 MMAs with a relayed stage signal
+  SM_UMMA_TMAP=1     cta_group::2 MMAs whose operands come through tensor-map TMA signalling the leader's barrier directly
   SM_UMMA_REV=1|0    PHASE 2 walks the tile table backwards / forwards
   SM_UMMA_STAGES=3|4 depth of the operand ring of the single-CTA kernel
   SM_UMMA_SLOTS=2|1  submatrices a CTA pair of the fused kernel interleaves
@@ -107,6 +108,8 @@ SYM_VARIANTS = [
     {"SM_UMMA_FUSED": "0", "SM_UMMA_NCTA": "1", "SM_UMMA_STAGES": "3"},
     {"SM_UMMA_FUSED": "0", "SM_UMMA_NCTA": "2", "SM_UMMA_MC": "1"},
     {"SM_UMMA_FUSED": "0", "SM_UMMA_NCTA": "2", "SM_UMMA_MC": "0"},
+    {"SM_UMMA_FUSED": "0", "SM_UMMA_NCTA": "2", "SM_UMMA_MC": "0", "SM_UMMA_TMAP": "1"},
+    {"SM_UMMA_FUSED": "0", "SM_UMMA_NCTA": "2", "SM_UMMA_MC": "0", "SM_UMMA_TMAP": "1", "SM_UMMA_STAGES": "3"},
     {"SM_UMMA_FUSED": "1", "SM_UMMA_SLOTS": "1"},
     {"SM_UMMA_FUSED": "1", "SM_UMMA_SLOTS": "2"},
 ]
