@@ -62,7 +62,7 @@ template <int NCTA, bool MC = false, int NST = 0> struct UCfg {
   static constexpr int STAGES = NST ? NST : (G2 ? 6 : 4);
   static constexpr int B_BYTES = (G2 ? UN / 2 : UN) * UK * 2;   // 16 KB / 32 KB
   static constexpr int STAGE_BYTES = A_BYTES + B_BYTES;    // 48 KB / 32 KB
-  static constexpr int SMEM = STAGES * STAGE_BYTES + EPI_STAGE_BYTES + IDENT_BYTES + 1024 /*align slack*/ + 256 /*barriers*/;
+  static constexpr int SMEM = STAGES * STAGE_BYTES + EPI_STAGE_BYTES + IDENT_BYTES + 1024 /*align slack*/ + 512 /*barriers, tile queue*/;
   static constexpr int ROWS = UM * NCTA;                   // tile rows
 };
 
@@ -91,6 +91,7 @@ struct UArgs {
   SignState s;
   int32_t *err_flag;
   int32_t rev;               // walk the tile table backwards (alternates per launch)
+  unsigned long long *counter;   // DYN: this launch's tile counter (zeroed by the host)
   int32_t dbg;               // measurement only (SM_UMMA_DBG): 1 = skip output stores, 2 = skip MMA issue, 4 = skip TMA loads, 8 = skip the epilogue's work
 };
 
@@ -252,9 +253,18 @@ __device__ __forceinline__ void mirror_store(uint16_t *Og, int32_t Pd, int32_t R
 // TM (cta_group::2 pairs only): operands come through tensor-map TMA (2-D view of the packed buffer: rows of 64
 // elements, no swizzle -- the image is stored pre-swizzled) with `.cta_group::2`, which lets BOTH CTAs of a pair
 // credit their bytes to the LEADER's "stage full" barrier; no relay warp, no second barrier wait per stage.
-template <bool BF16, int PHASE, int NCTA, bool SYM, bool MC = false, int NST = 0, bool TM = false>
+// DYN (one CTA per tile only): tiles are handed out by a global counter instead of round robin.  The producer
+// thread pops the next index (the atomic's latency overlaps the current tile's loads), reads its descriptor and
+// publishes it through a 4-entry shared-memory queue (mbarrier full / empty pairs) to the MMA issuer and the 16
+// epilogue warps.  With a static deal the CTAs drift apart by tens of tiles over a launch (tile costs differ), so
+// the tiles of one submatrix -- which share their operand panels -- run further apart in time than a line lives
+// in L2 (126 MB at ~5 TB/s: ~25 us) and the panels are fetched from DRAM again; a dynamic deal keeps all CTAs
+// inside one window of the size-sorted tile table and also evens out the tail of the launch.
+constexpr int TQ = 4;
+template <bool BF16, int PHASE, int NCTA, bool SYM, bool MC = false, int NST = 0, bool TM = false, bool DYN = false>
 __global__ void __launch_bounds__(UMMA_THREADS, 1)
 k_umma_gemm(UArgs a, const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapB) {
+  static_assert(!DYN || NCTA == 1, "dynamic tile scheduling: one CTA per tile");
   static_assert(!MC || (NCTA == 2 && SYM), "multicast variant: two CTAs, SYM tiles");
   static_assert(!TM || (NCTA == 2 && SYM && !MC), "tensor-map variant: cta_group::2 pairs, SYM tiles");
   using Cfg = UCfg<NCTA, MC, NST>;
@@ -278,6 +288,10 @@ k_umma_gemm(UArgs a, const __grid_constant__ CUtensorMap mapA, const __grid_cons
   const uint32_t tmem_slot = bars + 8u * (3 * USTAGES + 2 * NACC);
   volatile uint32_t *tmem_slot_ptr =
       reinterpret_cast<volatile uint32_t *>(smem_raw + (tmem_slot - raw));
+  // DYN: tile queue behind the barriers: full[TQ], empty[TQ], then TQ descriptors (16-byte aligned)
+  auto tqf_bar = [&](int s) { return bars + 256u + 8u * s; };
+  auto tqe_bar = [&](int s) { return bars + 256u + 8u * (TQ + s); };
+  TileDesc *const tq = reinterpret_cast<TileDesc *>(smem_raw + (bars + 256u + 16u * TQ - raw));
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const uint32_t h = CL2 ? ptx::cluster_ctarank() : 0u;    // rank inside the CTA pair; 0 = leader
@@ -293,6 +307,7 @@ k_umma_gemm(UArgs a, const __grid_constant__ CUtensorMap mapA, const __grid_cons
       ptx::mbar_init(full_bar(s), 1); ptx::mbar_init(empty_bar(s), MC ? 2 : 1); ptx::mbar_init(pfull_bar(s), 1);
     }
     for (int s = 0; s < NACC; ++s) { ptx::mbar_init(tfull_bar(s), 1); ptx::mbar_init(tempty_bar(s), EPI_WARPS * (PAIR ? 2 : 1)); }
+    if (DYN) for (int s = 0; s < TQ; ++s) { ptx::mbar_init(tqf_bar(s), 1); ptx::mbar_init(tqe_bar(s), 1 + EPI_WARPS); }
     ptx::fence_barrier_init();
     ptx::fence_proxy_async();
   }
@@ -313,9 +328,29 @@ k_umma_gemm(UArgs a, const __grid_constant__ CUtensorMap mapA, const __grid_cons
     if (lane == 0) {
       int stage = 0; uint32_t phase = 0;
       TileDesc nxt = load_desc(a, max((int64_t)0, min(unit, total - 1)));
-      for (int64_t t = unit; t < total; t += n_units) {
-        const TileDesc cur = nxt;
+      int64_t t = DYN ? (int64_t)atomicAdd(a.counter, 1ULL) : unit;
+      uint32_t qs = 0, qp = 0;
+      // next tile of this CTA: static deal (descriptor prefetched one tile ahead) or DYN (pop, publish)
+      auto fetch = [&](TileDesc &cur) -> bool {
+        if (DYN) {
+          const int64_t mine = t;
+          ptx::mbar_wait(tqe_bar(qs), qp ^ 1u, a.err_flag, 8);
+          if (mine < total) cur = load_desc(a, mine); else cur.c = -1;
+          tq[qs] = cur;
+          ptx::mbar_arrive(tqf_bar(qs));            // release: the descriptor is visible to the consumers
+          if (++qs == TQ) { qs = 0; qp ^= 1u; }
+          if (mine >= total) return false;
+          t = (int64_t)atomicAdd(a.counter, 1ULL);  // its latency overlaps this tile's loads
+          return true;
+        }
+        if (t >= total) return false;
+        cur = nxt;
         nxt = load_desc(a, min(t + n_units, total - 1));    // prefetch the next descriptor
+        t += n_units;
+        return true;
+      };
+      TileDesc cur;
+      while (fetch(cur)) {
         UTile u = make_tile<PHASE>(a, cur);
         if (!u.valid) continue;
         const char *Ag = (const char *)a.Xsrc + u.base * ESZ;
@@ -399,9 +434,24 @@ k_umma_gemm(UArgs a, const __grid_constant__ CUtensorMap mapA, const __grid_cons
       int stage = 0; uint32_t phase = 0;
       uint32_t it = 0;
       TileDesc nxt = load_desc(a, max((int64_t)0, min(unit, total - 1)));
-      for (int64_t t = unit; t < total; t += n_units) {
-        const TileDesc cur = nxt;
+      int64_t t = unit;
+      uint32_t qs = 0, qp = 0;
+      auto fetch = [&](TileDesc &cur) -> bool {
+        if (DYN) {
+          ptx::mbar_wait(tqf_bar(qs), qp, a.err_flag, 9);
+          cur = tq[qs];
+          ptx::mbar_arrive(tqe_bar(qs));
+          if (++qs == TQ) { qs = 0; qp ^= 1u; }
+          return cur.c >= 0;
+        }
+        if (t >= total) return false;
+        cur = nxt;
         nxt = load_desc(a, min(t + n_units, total - 1));
+        t += n_units;
+        return true;
+      };
+      TileDesc cur;
+      while (fetch(cur)) {
         UTile u = make_tile<PHASE>(a, cur);
         if (!u.valid) continue;
         const uint32_t as = it % NACC, aphase = (it / NACC) & 1u;
@@ -466,9 +516,25 @@ k_umma_gemm(UArgs a, const __grid_constant__ CUtensorMap mapA, const __grid_cons
     uint16_t *const stg0 = reinterpret_cast<uint16_t *>(smem_raw + (stage_base - raw)) + q * NACC * 1024;
     uint32_t it = 0;
     TileDesc nxt = load_desc(a, max((int64_t)0, min(unit, total - 1)));
-    for (int64_t t = unit; t < total; t += n_units) {
-      const TileDesc cur = nxt;
+    int64_t t = unit;
+    uint32_t qs = 0, qp = 0;
+    auto fetch = [&](TileDesc &cur) -> bool {
+      if (DYN) {
+        ptx::mbar_wait(tqf_bar(qs), qp, a.err_flag, 10);
+        cur = tq[qs];
+        __syncwarp();                                   // every lane has its copy before the slot is handed back
+        if (lane == 0) ptx::mbar_arrive(tqe_bar(qs));
+        if (++qs == TQ) { qs = 0; qp ^= 1u; }
+        return cur.c >= 0;
+      }
+      if (t >= total) return false;
+      cur = nxt;
       nxt = load_desc(a, min(t + n_units, total - 1));
+      t += n_units;
+      return true;
+    };
+    TileDesc cur;
+    while (fetch(cur)) {
       UTile u = make_tile<PHASE>(a, cur);
       if (!u.valid) continue;
       const uint32_t as = it % NACC, aphase = (it / NACC) & 1u;
@@ -631,8 +697,10 @@ static __global__ void k_umma_tilecounts(int32_t n_cols, int32_t R, int32_t sym,
   n_parts[c] = nt * parts_per_tile;
 }
 
+constexpr int UMMA_MAX_COUNTERS = 256;      // 2 per step; more steps than that fall back to the static deal
 struct UmmaWs {
   void *Y, *X2; int32_t *active, *last, *n_still, *n_parts, *err; int64_t *tile_ptr; double *partial;
+  unsigned long long *counters;   // one tile counter per product launch (dynamic scheduling)
   TileDesc *tiles;
   int32_t parts_per_col; int64_t used;
 };
@@ -715,6 +783,7 @@ static UmmaWs umma_layout(void *ws, int64_t ws_bytes, const sm_pattern_t *P, int
   w.last = cur.take<int32_t>(n_cols);
   w.n_still = cur.take<int32_t>(1);
   w.err = cur.take<int32_t>(1);
+  w.counters = cur.take<unsigned long long>(UMMA_MAX_COUNTERS);
   w.n_parts = cur.take<int32_t>(n_cols);
   w.tile_ptr = cur.take<int64_t>(n_cols + 1);
   w.partial = cur.take<double>((int64_t)n_cols * w.parts_per_col);
@@ -753,11 +822,11 @@ static int32_t make_map(CUtensorMap *m, void *buf, int64_t packed_elems, uint32_
   return SM_OK;
 }
 
-template <bool BF16, int PHASE, int NCTA, bool SYM, bool MC = false, int NST = 0, bool TM = false>
+template <bool BF16, int PHASE, int NCTA, bool SYM, bool MC = false, int NST = 0, bool TM = false, bool DYN = false>
 static int32_t launch_umma(const UArgs &a, const UMaps &maps, int32_t n_sm, cudaStream_t st) {
   static bool configured = false;
   if (!configured) {
-    SM_CUDA(cudaFuncSetAttribute(k_umma_gemm<BF16, PHASE, NCTA, SYM, MC, NST, TM>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    SM_CUDA(cudaFuncSetAttribute(k_umma_gemm<BF16, PHASE, NCTA, SYM, MC, NST, TM, DYN>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                  UCfg<NCTA, MC, NST>::SMEM));
     configured = true;
   }
@@ -772,7 +841,7 @@ static int32_t launch_umma(const UArgs &a, const UMaps &maps, int32_t n_sm, cuda
   attr[0].id = cudaLaunchAttributeClusterDimension;
   attr[0].val.clusterDim.x = NCTA; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
   cfg.attrs = attr; cfg.numAttrs = 1;
-  SM_CUDA(cudaLaunchKernelEx(&cfg, k_umma_gemm<BF16, PHASE, NCTA, SYM, MC, NST, TM>, a, maps.a, maps.b));
+  SM_CUDA(cudaLaunchKernelEx(&cfg, k_umma_gemm<BF16, PHASE, NCTA, SYM, MC, NST, TM, DYN>, a, maps.a, maps.b));
   SM_LAUNCHED();
   return prof_end(st, slot);
 }
@@ -800,10 +869,10 @@ static int32_t launch_fused(const FArgs &a, int32_t n_sm, cudaStream_t st) {
   return prof_end(st, slot);
 }
 
-template <int PHASE, int NCTA, bool SYM, bool MC = false, int NST = 0, bool TM = false>
+template <int PHASE, int NCTA, bool SYM, bool MC = false, int NST = 0, bool TM = false, bool DYN = false>
 static int32_t launch_umma_t(bool bf16, const UArgs &a, const UMaps &m, int32_t n_sm, cudaStream_t st) {
-  return bf16 ? launch_umma<true, PHASE, NCTA, SYM, MC, NST, TM>(a, m, n_sm, st)
-              : launch_umma<false, PHASE, NCTA, SYM, MC, NST, TM>(a, m, n_sm, st);
+  return bf16 ? launch_umma<true, PHASE, NCTA, SYM, MC, NST, TM, DYN>(a, m, n_sm, st)
+              : launch_umma<false, PHASE, NCTA, SYM, MC, NST, TM, DYN>(a, m, n_sm, st);
 }
 // mode: 1 = one CTA per tile, 2 = cta_group::2 pair with relay, 3 = two CTAs with multicast B, 4 = pair with tensor maps
 template <int PHASE>
@@ -813,6 +882,9 @@ static int32_t launch_umma_any(bool bf16, int32_t mode, int32_t sym, int32_t nst
                       : nst == 4 ? launch_umma_t<PHASE, 2, true, false, 4, true>(bf16, a, m, n_sm, st)
                                  : launch_umma_t<PHASE, 2, true, false, 6, true>(bf16, a, m, n_sm, st);
   if (mode == 3) return launch_umma_t<PHASE, 2, true, true>(bf16, a, m, n_sm, st);
+  if (mode == 1 && sym && a.counter)      // dynamic tile scheduling
+    return nst == 3 ? launch_umma_t<PHASE, 1, true, false, 3, false, true>(bf16, a, m, n_sm, st)
+                    : launch_umma_t<PHASE, 1, true, false, 0, false, true>(bf16, a, m, n_sm, st);
   if (mode == 1 && sym && nst == 3) return launch_umma_t<PHASE, 1, true, false, 3>(bf16, a, m, n_sm, st);
   if (mode == 2) return sym ? launch_umma_t<PHASE, 2, true>(bf16, a, m, n_sm, st) : launch_umma_t<PHASE, 2, false>(bf16, a, m, n_sm, st);
   return sym ? launch_umma_t<PHASE, 1, true>(bf16, a, m, n_sm, st) : launch_umma_t<PHASE, 1, false>(bf16, a, m, n_sm, st);
@@ -888,14 +960,21 @@ int32_t sign_umma(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, co
   }
   static int32_t nst_env = -1;    // SM_UMMA_STAGES=3|4: ring depth of the single-CTA SYM kernel (A/B measurements)
   if (nst_env < 0) { const char *e = getenv("SM_UMMA_STAGES"); nst_env = e ? atoi(e) : 0; }
-  const int32_t nst = nst_env ? nst_env : (mode == 4 ? 6 : (P->max_dim > 1024 ? 3 : 4));
+  static int32_t dyn_on = -1;     // SM_UMMA_DYN=0: static round-robin deal of the tiles (A/B measurements)
+  if (dyn_on < 0) { const char *e = getenv("SM_UMMA_DYN"); dyn_on = (e && e[0] == '0') ? 0 : 1; }
+  const bool dyn = dyn_on && mode == 1 && sym && 2 * max_iter <= UMMA_MAX_COUNTERS;
+  // ring depth: with the static deal large submatrices want the shallow ring (see UCfg); the dynamic deal removes
+  // the drift that made the deep ring costly (configs[4], 25 steps: 603 ms with 4 stages, 615 ms with 3)
+  const int32_t nst = nst_env ? nst_env : (mode == 4 ? 6 : ((!dyn && P->max_dim > 1024) ? 3 : 4));
+  if (dyn) SM_CUDA(cudaMemsetAsync(w.counters, 0, sizeof(unsigned long long) * UMMA_MAX_COUNTERS, st));
   static int32_t rev_on = -1;     // SM_UMMA_REV=0 keeps every launch walking forwards (A/B measurements)
   if (rev_on < 0) { const char *e = getenv("SM_UMMA_REV"); rev_on = (e && e[0] == '0') ? 0 : 1; }
   void *buf[2] = {X, w.X2};
   for (int32_t k = 0; k < max_iter; ++k) {
     void *src = buf[k & 1], *dst = buf[(k + 1) & 1];
-    UArgs a{cols, col_off, P->dim, P->dim_pad, w.tile_ptr, w.tiles, n_cols, tol > 0.0 ? 1 : 0, src, w.Y, w.Y, s, w.err, 0, umma_dbg()};
+    UArgs a{cols, col_off, P->dim, P->dim_pad, w.tile_ptr, w.tiles, n_cols, tol > 0.0 ? 1 : 0, src, w.Y, w.Y, s, w.err, 0, nullptr, umma_dbg()};
     a.rev = 0;
+    a.counter = dyn ? w.counters + 2 * k : nullptr;
     const UMaps m1{maps[k & 1].a, maps[k & 1].b}, m2{maps[k & 1].a, maps[2].b};
     int32_t rc = launch_umma_any<1>(bf16, mode, sym, nst, a, m1, n_sm, st);
     if (rc != SM_OK) return rc;
@@ -904,6 +983,7 @@ int32_t sign_umma(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, co
     SM_LAUNCHED();
     a.Out = dst;
     a.rev = rev_on;            // PHASE 2 starts where PHASE 1 ended, the next PHASE 1 where this launch ends
+    a.counter = dyn ? w.counters + 2 * k + 1 : nullptr;
     rc = launch_umma_any<2>(bf16, mode, sym, nst, a, m2, n_sm, st);
     if (rc != SM_OK) return rc;
     if (tol > 0.0 && k >= 5 && (k & 1)) {
