@@ -155,9 +155,14 @@ class Pattern:
         return self._h_dim_pad
 
 
-def sm_build_pattern(A: Bcsr, pad_to: int) -> Pattern:
-    sizes = sm_pattern_sizes(A, pad_to)
+def sm_build_pattern(A: Bcsr, pad_to: int, sizes=None) -> Pattern:
+    """a1.  `sizes`: the result of an earlier sm_pattern_sizes call on the same geometry (e.g. `P.sizes` of a previous
+    build); sm_pattern_sizes validates the pattern and reads the sizes back, i.e. synchronises, so a caller that
+    evaluates the same geometry repeatedly passes them in and the build itself stays asynchronous."""
+    if sizes is None:
+        sizes = sm_pattern_sizes(A, pad_to)
     P = Pattern(A, pad_to, sizes)
+    P.sizes = sizes
     ws = torch.empty(int(sizes.build_ws_bytes), dtype=torch.uint8, device=A.device)
     _check("sm_build_pattern", _lib.sm_build_pattern(C.byref(A.c), C.c_int32(pad_to), C.byref(P.c), _ptr(ws),
                                                      C.c_int64(ws.numel()), _stream()))
