@@ -978,9 +978,16 @@ int32_t sign_umma(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, co
     const UMaps m1{maps[k & 1].a, maps[k & 1].b}, m2{maps[k & 1].a, maps[2].b};
     int32_t rc = launch_umma_any<1>(bf16, mode, sym, nst, a, m1, n_sm, st);
     if (rc != SM_OK) return rc;
-    SM_CUDA(cudaMemsetAsync(w.n_still, 0, sizeof(int32_t), st));
-    k_sign_post<<<(n_cols + 7) / 8, 256, 0, st>>>(n_cols, cols, P->dim, s, w.n_parts, tol, iters, residual);
-    SM_LAUNCHED();
+    if (tol > 0.0) {
+      SM_CUDA(cudaMemsetAsync(w.n_still, 0, sizeof(int32_t), st));
+      k_sign_post<<<(n_cols + 7) / 8, 256, 0, st>>>(n_cols, cols, P->dim, s, w.n_parts, tol, iters, residual);
+      SM_LAUNCHED();
+    } else if (k == max_iter - 1) {
+      // fixed iteration count: nothing depends on the residual, so only the last step's is reduced (and iters set)
+      k_fused_post<<<(n_cols + 7) / 8, 256, 0, st>>>(n_cols, cols, P->dim, w.partial, w.parts_per_col, w.n_parts,
+                                                     max_iter, iters, residual);
+      SM_LAUNCHED();
+    }
     a.Out = dst;
     a.rev = rev_on;            // PHASE 2 starts where PHASE 1 ended, the next PHASE 1 where this launch ends
     a.counter = dyn ? w.counters + 2 * k + 1 : nullptr;
