@@ -216,6 +216,8 @@ int32_t sm_density_from_sign(const sm_bcsr_t *A, const sm_pattern_t *P, int32_t 
  *   SM_UMMA_REV=1|0    16-bit: the update product walks the tile table backwards / forwards
  *   SM_UMMA_STAGES=3|4 16-bit, one CTA per tile: depth of the operand ring
  *   SM_UMMA_DYN=1|0    16-bit, one CTA per tile: tiles handed out by a global counter / dealt round robin
+ *   SM_UMMA_STREAM=1   16-bit, tol <= 0, one CTA per tile: one launch walks every product of every step, products of a
+ *                      submatrix ordered by per-group completion counters
  *   SM_UMMA_FUSED=1    16-bit, tol <= 0: one launch runs every step of a submatrix (SM_UMMA_SLOTS=1|2 in flight)
  *   SM_F64_BACKEND=dmma|simt   fp64: tensor-core m8n8k4 tiles / DFMA register tiles
  *   SM_UMMA_DBG, SM_UMMA_TRACE measurement only (skip-knobs that produce WRONG results; clock64 time line). */

@@ -92,6 +92,9 @@ struct UArgs {
   int32_t *err_flag;
   int32_t rev;               // walk the tile table backwards (alternates per launch)
   unsigned long long *counter;   // DYN: this launch's tile counter (zeroed by the host)
+  // PHASE = 0 ("stream": every product of every step in ONE launch; Xsrc / Out are the two X buffers, Ybuf is Wh):
+  int32_t n_ph;              // 2 * steps
+  int32_t *done;             // [groups][n_ph] epilogue-warp completions of (group, product), zeroed by the host
   int32_t dbg;               // measurement only (SM_UMMA_DBG): 1 = skip output stores, 2 = skip MMA issue, 4 = skip TMA loads, 8 = skip the epilogue's work
 };
 
@@ -261,10 +264,30 @@ __device__ __forceinline__ void mirror_store(uint16_t *Og, int32_t Pd, int32_t R
 // in L2 (126 MB at ~5 TB/s: ~25 us) and the panels are fetched from DRAM again; a dynamic deal keeps all CTAs
 // inside one window of the size-sorted tile table and also evens out the tail of the launch.
 constexpr int TQ = 4;
+// PHASE = 0, "stream" (fixed iteration counts): ONE launch runs every product of every step.  The dynamic deal walks
+// a virtual tile list: the listed columns are cut into super-groups of STREAM_SG submatrices (~77 MB of X, Wh, X' at
+// configs[2]: they stay in L2), and a super-group's tiles are walked once per product, all 2 * steps products before
+// the next super-group.  A product of a submatrix needs the previous product of the same submatrix complete: the
+// dependency is tracked per group of STREAM_G submatrices by a counter that every epilogue warp bumps (after a
+// gpu-scope fence and a generic->async proxy fence) when its part of a tile is stored; the producer thread of a
+// tile of (group, product ph) waits until the counter of (group, ph - 1) is complete, then fences and issues its bulk
+// copies.  The tiles in between (the other groups of the super-group, ~3/4 of it = ~2 tiles per CTA) are what hides
+// that wait.  Because tiles are popped in list order and every CTA is resident, a waiting CTA only ever waits for
+// tiles that are already running: no deadlock.
+#ifndef SM_STREAM_G
+#define SM_STREAM_G 16
+#endif
+#ifndef SM_STREAM_SG
+#define SM_STREAM_SG 96
+#endif
+constexpr int STREAM_G = SM_STREAM_G;
+constexpr int STREAM_SG = SM_STREAM_SG;
 template <bool BF16, int PHASE, int NCTA, bool SYM, bool MC = false, int NST = 0, bool TM = false, bool DYN = false>
 __global__ void __launch_bounds__(UMMA_THREADS, 1)
 k_umma_gemm(UArgs a, const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapB) {
   static_assert(!DYN || NCTA == 1, "dynamic tile scheduling: one CTA per tile");
+  static_assert(PHASE != 0 || (DYN && SYM), "stream mode needs the dynamic deal and symmetric tiles");
+  constexpr bool STREAM = PHASE == 0;
   static_assert(!MC || (NCTA == 2 && SYM), "multicast variant: two CTAs, SYM tiles");
   static_assert(!TM || (NCTA == 2 && SYM && !MC), "tensor-map variant: cta_group::2 pairs, SYM tiles");
   using Cfg = UCfg<NCTA, MC, NST>;
@@ -297,7 +320,7 @@ k_umma_gemm(UArgs a, const __grid_constant__ CUtensorMap mapA, const __grid_cons
   const uint32_t h = CL2 ? ptx::cluster_ctarank() : 0u;    // rank inside the CTA pair; 0 = leader
   const int64_t unit = blockIdx.x / NCTA, n_units = gridDim.x / NCTA;
 
-  if (PHASE == 2) {
+  if (PHASE != 1) {
     ident_fill<BF16>(smem_raw + (ident - raw), PAIR, h, (int)threadIdx.x, UMMA_THREADS);
     ptx::fence_proxy_async();       // generic-proxy writes -> the MMA's async-proxy reads
   }
@@ -330,17 +353,45 @@ k_umma_gemm(UArgs a, const __grid_constant__ CUtensorMap mapA, const __grid_cons
       TileDesc nxt = load_desc(a, max((int64_t)0, min(unit, total - 1)));
       int64_t t = DYN ? (int64_t)atomicAdd(a.counter, 1ULL) : unit;
       uint32_t qs = 0, qp = 0;
+      int32_t sg_c0 = 0;                                                     // STREAM: current super-group
+      int64_t sg_lo = 0, sg_hi = STREAM ? a.tile_ptr[min(STREAM_SG, a.n_cols)] : 0;
       // next tile of this CTA: static deal (descriptor prefetched one tile ahead) or DYN (pop, publish)
       auto fetch = [&](TileDesc &cur) -> bool {
         if (DYN) {
           const int64_t mine = t;
           ptx::mbar_wait(tqe_bar(qs), qp ^ 1u, a.err_flag, 8);
-          if (mine < total) cur = load_desc(a, mine); else cur.c = -1;
+          if (STREAM) {
+            // virtual index -> (super-group S, product ph, tile): super-group S = STREAM_SG consecutive listed
+            // columns; its tiles are walked once per product, all products of S before S + 1
+            if (mine < total * a.n_ph) {
+              while (mine >= (int64_t)a.n_ph * sg_hi) {
+                sg_c0 = min(sg_c0 + STREAM_SG, a.n_cols);
+                sg_lo = sg_hi; sg_hi = a.tile_ptr[min(sg_c0 + STREAM_SG, a.n_cols)];
+              }
+              const int64_t off = mine - (int64_t)a.n_ph * sg_lo, ts = sg_hi - sg_lo;
+              const int32_t ph = (int32_t)(off / ts);
+              cur = load_desc(a, sg_lo + (off - (int64_t)ph * ts));
+              const int32_t grp = cur.c / STREAM_G;
+              const int32_t g0 = grp * STREAM_G, g1 = min(g0 + STREAM_G, a.n_cols);
+              cur.pad0 = ph; cur.pad1 = grp;
+              cur.pad2 = (int32_t)(a.tile_ptr[g1] - a.tile_ptr[g0]) * EPI_WARPS;     // completions of one product of the group
+            } else cur.c = -1;
+          } else if (mine < total) cur = load_desc(a, mine); else cur.c = -1;
           tq[qs] = cur;
           ptx::mbar_arrive(tqf_bar(qs));            // release: the descriptor is visible to the consumers
           if (++qs == TQ) { qs = 0; qp ^= 1u; }
-          if (mine >= total) return false;
+          if (cur.c < 0) return false;
           t = (int64_t)atomicAdd(a.counter, 1ULL);  // its latency overlaps this tile's loads
+          if (STREAM && cur.pad0 > 0 && !(a.dbg & 64)) {
+            // the previous product of this group (written by other CTAs) must be complete and visible to the bulk copies
+            const volatile int32_t *flag = a.done + (int64_t)cur.pad1 * a.n_ph + (cur.pad0 - 1);
+            for (uint32_t spin = 0; *flag < cur.pad2; ++spin) {
+              __nanosleep(64);
+              if (spin > 40000000u) { atomicExch(a.err_flag, 11); __threadfence_system(); __trap(); }
+            }
+            __threadfence();
+            ptx::fence_proxy_async();
+          }
           return true;
         }
         if (t >= total) return false;
@@ -353,8 +404,10 @@ k_umma_gemm(UArgs a, const __grid_constant__ CUtensorMap mapA, const __grid_cons
       while (fetch(cur)) {
         UTile u = make_tile<PHASE>(a, cur);
         if (!u.valid) continue;
-        const char *Ag = (const char *)a.Xsrc + u.base * ESZ;
-        const char *Bg = (const char *)(PHASE == 1 ? a.Xsrc : a.Ybuf) + u.base * ESZ;
+        const bool p2 = STREAM ? (cur.pad0 & 1) != 0 : PHASE == 2;
+        const void *Xcur = (STREAM && ((cur.pad0 >> 1) & 1)) ? a.Out : a.Xsrc;     // stream: X ping-pongs per step
+        const char *Ag = (const char *)Xcur + u.base * ESZ;
+        const char *Bg = (const char *)(p2 ? a.Ybuf : Xcur) + u.base * ESZ;
         const int32_t arow0 = u.row0 + (int32_t)h * UM;
         const uint32_t a_rows = (uint32_t)max(0, min(UM, u.Pd - arow0));
         const int32_t b_cnt = u.nt / NCTA, brow0 = u.n0 + (int32_t)h * b_cnt;   // this CTA's share of B
@@ -478,7 +531,7 @@ k_umma_gemm(UArgs a, const __grid_constant__ CUtensorMap mapA, const __grid_cons
               ptx::umma_f16(d_tmem, adesc + (uint64_t)(2 * ks), bdesc + bstep * (uint64_t)ks, idesc,
                             (uint32_t)((kc | ks) != 0));
           }
-          if (PHASE == 2 && !(a.dbg & 2)) {
+          if ((STREAM ? (cur.pad0 & 1) != 0 : PHASE == 2) && !(a.dbg & 2)) {
             // "+ X": the A chunk in this stage holds X[rows, 64 kc .. 64 kc + 63]; add it to the accumulator
             // columns [lo, hi) of the tile that it covers (B = identity slice, K-major)
             const int32_t lo = max(kc * UK, u.n0), hi = min(kc * UK + UK, u.n0 + u.nt);
@@ -543,7 +596,9 @@ k_umma_gemm(UArgs a, const __grid_constant__ CUtensorMap mapA, const __grid_cons
       uint16_t *const stg = stg0 + as * 1024;
       const int32_t R0 = u.row0 + (int32_t)h * UM + q * 32;   // this CTA's 128 rows of the tile
       const int32_t r = R0 + lane;
-      uint16_t *Og = (uint16_t *)a.Out + u.base;
+      const bool p1 = STREAM ? (cur.pad0 & 1) == 0 : PHASE == 1;
+      // stream: product ph of step ph / 2 writes Wh (even ph) or the X buffer that step does not read (odd ph)
+      uint16_t *Og = (uint16_t *)(!STREAM ? a.Out : p1 ? a.Ybuf : (((cur.pad0 >> 1) & 1) ? (void *)a.Xsrc : a.Out)) + u.base;
       if (a.dbg & 1) Og = nullptr;
       const int nblk = (u.nt + 31) >> 5;
       ptx::mbar_wait(tfull_bar(as), aphase, a.err_flag, 4);
@@ -575,7 +630,7 @@ k_umma_gemm(UArgs a, const __grid_constant__ CUtensorMap mapA, const __grid_cons
             float f[8];
 #pragma unroll
             for (int e = 0; e < 8; ++e) f[e] = __uint_as_float(v[g * 8 + e]);
-            if (PHASE == 1) {
+            if (p1) {
               // W = Y - I is what gets stored: near convergence Y_rr ~ 1 would lose 2^-9 absolute to the 16-bit
               // rounding every step, W_rr ~ 0 loses nothing; PHASE 2 then forms X' = X - 1/2 X W.
               if (diag && r < u.m) {                               // padding rows keep W = 0
@@ -599,7 +654,7 @@ k_umma_gemm(UArgs a, const __grid_constant__ CUtensorMap mapA, const __grid_cons
 #pragma unroll
             for (int e2 = 0; e2 < 4; ++e2) o[g * 4 + e2] = pack2<BF16>(f[2 * e2], f[2 * e2 + 1]);
           }
-          if (PHASE == 1 && r < u.m) { if (SYM && !diag) res2 += acc; else res += acc; }
+          if (p1 && r < u.m) { if (SYM && !diag) res2 += acc; else res += acc; }
           uint16_t *Orow = Og ? Og + rowoff : nullptr;
           if (!SYM) {
             if (Orow) store_row_segment(Orow, sec0, sec1, swp, o);
@@ -639,11 +694,18 @@ k_umma_gemm(UArgs a, const __grid_constant__ CUtensorMap mapA, const __grid_cons
       if (lane == 0) {
         if (PAIR) ptx::mbar_arrive_remote(tempty_bar(as), 0); else ptx::mbar_arrive(tempty_bar(as));
       }
-      if (PHASE == 1) {
+      if (p1) {
         for (int d = 16; d > 0; d >>= 1) res += __shfl_xor_sync(0xffffffffu, res, d);
         if (lane == 0)
           a.s.partial[(int64_t)u.c * a.s.parts_per_col + (int64_t)u.lt * (EPI_WARPS * NCTA) + (int64_t)h * EPI_WARPS +
                       (warp - 2)] = (double)res;
+      }
+      if (STREAM && cur.pad0 + 1 < a.n_ph && !(a.dbg & 128)) {
+        // this warp's stores of the tile: visible gpu-wide and to the async proxy, then counted for the group's product
+        __threadfence();
+        ptx::fence_proxy_async();
+        __syncwarp();
+        if (lane == 0) atomicAdd(a.done + (int64_t)cur.pad1 * a.n_ph + cur.pad0, 1);
       }
       ++it;
     }
@@ -701,6 +763,7 @@ constexpr int UMMA_MAX_COUNTERS = 256;      // 2 per step; more steps than that 
 struct UmmaWs {
   void *Y, *X2; int32_t *active, *last, *n_still, *n_parts, *err; int64_t *tile_ptr; double *partial;
   unsigned long long *counters;   // one tile counter per product launch (dynamic scheduling)
+  int32_t *done;                  // stream mode: [groups][2 * steps] completion counters
   TileDesc *tiles;
   int32_t parts_per_col; int64_t used;
 };
@@ -784,6 +847,7 @@ static UmmaWs umma_layout(void *ws, int64_t ws_bytes, const sm_pattern_t *P, int
   w.n_still = cur.take<int32_t>(1);
   w.err = cur.take<int32_t>(1);
   w.counters = cur.take<unsigned long long>(UMMA_MAX_COUNTERS);
+  w.done = cur.take<int32_t>((int64_t)(n_cols / STREAM_G + 1) * UMMA_MAX_COUNTERS);
   w.n_parts = cur.take<int32_t>(n_cols);
   w.tile_ptr = cur.take<int64_t>(n_cols + 1);
   w.partial = cur.take<double>((int64_t)n_cols * w.parts_per_col);
@@ -967,12 +1031,29 @@ int32_t sign_umma(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, co
   // the drift that made the deep ring costly (configs[4], 25 steps: 603 ms with 4 stages, 615 ms with 3)
   const int32_t nst = nst_env ? nst_env : (mode == 4 ? 6 : ((!dyn && P->max_dim > 1024) ? 3 : 4));
   if (dyn) SM_CUDA(cudaMemsetAsync(w.counters, 0, sizeof(unsigned long long) * UMMA_MAX_COUNTERS, st));
+  static int32_t stream_on = -1;  // SM_UMMA_STREAM=1: one launch for all products (fixed iteration counts, dynamic deal)
+  if (stream_on < 0) { const char *e = getenv("SM_UMMA_STREAM"); stream_on = (e && e[0] == '1') ? 1 : 0; }
+  if (stream_on && dyn && !(tol > 0.0) && max_iter > 0) {
+    const int64_t n_done = (int64_t)(n_cols / STREAM_G + 1) * 2 * max_iter;
+    SM_CUDA(cudaMemsetAsync(w.done, 0, sizeof(int32_t) * n_done, st));
+    UArgs a{cols, col_off, P->dim, P->dim_pad, w.tile_ptr, w.tiles, n_cols, 0, X, w.Y, w.X2, s, w.err, 0, w.counters,
+            2 * max_iter, w.done, umma_dbg()};
+    int32_t rc = launch_umma_t<0, 1, true, false, 0, false, true>(bf16, a, maps[0], n_sm, st);
+    if (rc != SM_OK) return rc;
+    k_fused_post<<<(n_cols + 7) / 8, 256, 0, st>>>(n_cols, cols, P->dim, w.partial, w.parts_per_col, w.n_parts,
+                                                   max_iter, iters, residual);
+    SM_LAUNCHED();
+    dim3 cgs(n_cols, 8);
+    k_copy_back<<<cgs, 256, 0, st>>>(cols, col_off, iters, 2, (const char *)w.X2, (char *)X);
+    SM_LAUNCHED();
+    return SM_OK;
+  }
   static int32_t rev_on = -1;     // SM_UMMA_REV=0 keeps every launch walking forwards (A/B measurements)
   if (rev_on < 0) { const char *e = getenv("SM_UMMA_REV"); rev_on = (e && e[0] == '0') ? 0 : 1; }
   void *buf[2] = {X, w.X2};
   for (int32_t k = 0; k < max_iter; ++k) {
     void *src = buf[k & 1], *dst = buf[(k + 1) & 1];
-    UArgs a{cols, col_off, P->dim, P->dim_pad, w.tile_ptr, w.tiles, n_cols, tol > 0.0 ? 1 : 0, src, w.Y, w.Y, s, w.err, 0, nullptr, umma_dbg()};
+    UArgs a{cols, col_off, P->dim, P->dim_pad, w.tile_ptr, w.tiles, n_cols, tol > 0.0 ? 1 : 0, src, w.Y, w.Y, s, w.err, 0, nullptr, 0, nullptr, umma_dbg()};
     a.rev = 0;
     a.counter = dyn ? w.counters + 2 * k : nullptr;
     const UMaps m1{maps[k & 1].a, maps[k & 1].b}, m2{maps[k & 1].a, maps[2].b};

@@ -6,6 +6,7 @@ environment forces (each in its own process: the selection is read once per proc
   SM_UMMA_REV=1|0    PHASE 2 walks the tile table backwards / forwards
   SM_UMMA_STAGES=3|4 depth of the operand ring of the single-CTA kernel
   SM_UMMA_DYN=1|0    tiles handed out by a global counter / dealt round robin
+  SM_UMMA_STREAM=1   one launch walks every product of every step (dependency counters per group of submatrices)
   SM_UMMA_SLOTS=2|1  submatrices a CTA pair of the fused kernel interleaves
   SM_UMMA_SYM=1|0    symmetric half tiles with mirrored stores / true products with an MN-major B operand
   SM_UMMA_FUSED=1|0  one launch runs every step of a submatrix (k_umma_fused) / one launch per product
@@ -115,6 +116,7 @@ SYM_VARIANTS = [
     {"SM_UMMA_FUSED": "0", "SM_UMMA_NCTA": "2", "SM_UMMA_MC": "0", "SM_UMMA_TMAP": "1", "SM_UMMA_STAGES": "3"},
     {"SM_UMMA_FUSED": "1", "SM_UMMA_SLOTS": "1"},
     {"SM_UMMA_FUSED": "1", "SM_UMMA_SLOTS": "2"},
+    {"SM_UMMA_FUSED": "0", "SM_UMMA_NCTA": "1", "SM_UMMA_STREAM": "1"},
 ]
 
 
