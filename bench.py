@@ -129,7 +129,7 @@ def oracle_sample(wl, cfg_run, n_cols_sample, seed, n_threads):
 
 def oracle_sample_size(cfg_index, cores):
     # ~10-30 s of CPU work: per-submatrix cost of the Jacobi oracle ~ 2.2e-8 * m^3 s (measured here)
-    per = {0: 0.003, 1: 0.25, 2: 10.0, 3: 0.25, 4: 600.0}[cfg_index]
+    per = {0: 0.003, 1: 0.25, 2: 4.0, 3: 0.25, 4: 600.0}[cfg_index]      # cfg2: 32 columns took 7 s on 16 cores
     return max(1, min(int(20.0 * cores / per), {0: 32, 1: 1000, 2: 3000, 3: 10000, 4: 2000}[cfg_index])) \
         if per < 100 else max(1, min(cores, 8))
 
