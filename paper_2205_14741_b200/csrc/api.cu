@@ -152,10 +152,7 @@ extern "C" int32_t sm_density(const sm_bcsr_t *A, const void *A_vals, int32_t a_
     if (rc != SM_OK) return rc;
     lo = hi;
   }
-  if (symmetrise) {
-    int32_t rc = sm_symmetrise(A, P, d_dtype, D_vals, stream);
-    if (rc != SM_OK) return rc;
-  }
+  if (symmetrise) return sm::symmetrise_density(A, P, d_dtype, D_vals, trace, (cudaStream_t)stream);
   return sm_density_from_sign(A, P, d_dtype, D_vals, trace, stream);
 }
 

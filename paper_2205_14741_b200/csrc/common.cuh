@@ -106,6 +106,8 @@ int32_t prof_begin(cudaStream_t st, int *slot);
 int32_t prof_end(cudaStream_t st, int slot);
 
 // ---- internal entry points implemented across the .cu files
+int32_t symmetrise_density(const sm_bcsr_t *A, const sm_pattern_t *P, int32_t d_dtype, void *RD_vals,
+                           double *trace, cudaStream_t st);                                  // gather_scatter.cu
 int32_t exclusive_scan_i64(int32_t n, const int64_t *in, int64_t *out, cudaStream_t st);   // pattern.cu
 int64_t global_scale_ws_bytes(const sm_bcsr_t *A, const sm_pattern_t *P);                    // global_scale.cu
 int32_t global_scale(const sm_bcsr_t *A, const void *A_vals, int32_t a_dtype, const sm_pattern_t *P, double mu,

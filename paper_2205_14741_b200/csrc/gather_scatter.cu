@@ -88,9 +88,98 @@ struct GatherArgs {
   const double *scale; double mu;
 };
 
+// One 8-run through the branch-free walk: the run spans at most NB neighbour blocks (the CTA checked the
+// narrowest block of N(i)), so the NB candidate sources are set up once and every element picks its
+// source by compares against the block ends -- no divergent block switch, no per-element bounds test
+// (columns >= m fall into the pseudo block `cnt`, whose source is null).
+template <typename TA, typename TX, int NB>
+__device__ __forceinline__ void gather_run(const GatherArgs &g, const TA *__restrict__ vals, const int32_t *off,
+                                           const uint16_t *blkof, const int32_t *gm, int32_t cnt, int32_t r,
+                                           int32_t c0, float inv_sf, float muf, double inv_s, TX *v) {
+  constexpr bool LOWP = sizeof(TX) == 2;
+  const int32_t a = blkof[r], ra = r - off[a];
+  const int32_t *gm_row = gm + (int64_t)a * cnt;
+  const int32_t b = blkof[c0];
+  const TA *src[NB];
+  int32_t end[NB];
+#pragma unroll
+  for (int s = 0; s < NB; ++s) {
+    const int32_t bb = b + s;
+    const bool in = bb < cnt;
+    const int32_t bs = off[bb], be = off[bb + 1];        // off[] is padded behind cnt (k_gather)
+    const int32_t p = in ? __ldg(gm_row + bb) : -1;
+    // element c of the run lives at src[s][c]: row ra of the stored block, shifted by the block's first column
+    src[s] = p >= 0 ? vals + __ldg(g.vp + p) + (int64_t)ra * (be - bs) - bs : nullptr;
+    end[s] = be;
+  }
+  bool any = false;
+#pragma unroll
+  for (int s = 0; s < NB; ++s) any |= src[s] != nullptr;
+  if (!any) {                                             // no stored block under the run (about half of all runs)
+#pragma unroll
+    for (int k = 0; k < 8; ++k) v[k] = from_double<TX>(0.0);
+    return;
+  }
+  const int32_t kd = r - c0;                              // position of the diagonal inside the run, if 0..7
+#pragma unroll
+  for (int k = 0; k < 8; ++k) {
+    const int32_t c = c0 + k;
+    const TA *sp = src[0];
+#pragma unroll
+    for (int s = 1; s < NB; ++s) sp = c >= end[s - 1] ? src[s] : sp;
+    if (LOWP) {
+      float x = sp ? (float)__ldg(sp + c) : 0.f;
+      if (k == kd) x -= muf;
+      v[k] = from_float<TX>(x * inv_sf);
+    } else {
+      double x = sp ? to_double<TA>(__ldg(sp + c)) : 0.0;
+      if (k == kd) x -= g.mu;
+      v[k] = from_double<TX>(x * inv_s);
+    }
+  }
+}
+
+// The general walk (blocks narrower than 3 columns): one block switch per column at most.
+template <typename TA, typename TX>
+__device__ __forceinline__ void gather_run_any(const GatherArgs &g, const TA *__restrict__ vals, const int32_t *off,
+                                               const uint16_t *blkof, const int32_t *gm, int32_t cnt, int32_t m,
+                                               int32_t r, int32_t c0, float inv_sf, float muf, double inv_s, TX *v) {
+  constexpr bool LOWP = sizeof(TX) == 2;
+  const int32_t a = blkof[r], ra = r - off[a];
+  const int32_t *gm_row = gm + (int64_t)a * cnt;
+  int32_t b = blkof[c0], bs = off[b], be = off[b + 1];
+  int32_t p = __ldg(gm_row + b);
+  const TA *src = p >= 0 ? vals + __ldg(g.vp + p) + (int64_t)ra * (be - bs) : nullptr;
+#pragma unroll
+  for (int k = 0; k < 8; ++k) {
+    const int32_t c = c0 + k;
+    if (c < m) {
+      while (c >= be) {                                   // next neighbour block (blocks are >= 1 wide)
+        ++b; bs = be; be = off[b + 1];
+        p = __ldg(gm_row + b);
+        src = p >= 0 ? vals + __ldg(g.vp + p) + (int64_t)ra * (be - bs) : nullptr;
+      }
+      if (LOWP) {
+        float x = src ? (float)__ldg(src + (c - bs)) : 0.f;
+        if (r == c) x -= muf;
+        v[k] = from_float<TX>(x * inv_sf);
+      } else {
+        double x = src ? to_double<TA>(__ldg(src + (c - bs))) : 0.0;
+        if (r == c) x -= g.mu;
+        v[k] = from_double<TX>(x * inv_s);
+      }
+    } else {
+      v[k] = from_double<TX>(0.0);
+    }
+  }
+}
+
+constexpr int GATHER_OFF_PAD = 4;   // off[cnt+1 .. cnt+GATHER_OFF_PAD]: ends of the pseudo blocks behind the last one
+
 template <typename TA, typename TX, bool IMG>
 __global__ void __launch_bounds__(256) k_gather(GatherArgs g, const TA *__restrict__ vals, TX *__restrict__ X) {
   extern __shared__ int32_t smem_i[];
+  __shared__ int32_t s_minb;
   const int32_t c_list = blockIdx.x;
   const int32_t i = g.cols ? g.cols[c_list] : c_list;
   const int32_t Pd = g.dim_pad[i], m = g.dim[i];
@@ -98,21 +187,29 @@ __global__ void __launch_bounds__(256) k_gather(GatherArgs g, const TA *__restri
   if (r0 >= Pd) return;
   const int32_t lo = g.rp[i], cnt = g.rp[i + 1] - lo;
   int32_t *off = smem_i;
-  uint16_t *blkof = (uint16_t *)(smem_i + cnt + 1);
+  uint16_t *blkof = (uint16_t *)(smem_i + cnt + 1 + GATHER_OFF_PAD);
+  if (threadIdx.x == 0) s_minb = 0x7fffffff;
   for (int32_t a = threadIdx.x; a < cnt; a += blockDim.x) off[a] = g.row_off[lo + a];
-  if (threadIdx.x == 0) off[cnt] = m;
+  if (threadIdx.x <= GATHER_OFF_PAD) off[cnt + threadIdx.x] = threadIdx.x == 0 ? m : 0x3fffffff;
   __syncthreads();
-  for (int32_t a = threadIdx.x; a < cnt; a += blockDim.x)
+  int32_t minb = 0x7fffffff;
+  for (int32_t a = threadIdx.x; a < cnt; a += blockDim.x) {
+    minb = min(minb, off[a + 1] - off[a]);
     for (int32_t r = off[a]; r < off[a + 1]; ++r) blkof[r] = (uint16_t)a;
+  }
+  for (int32_t r = m + threadIdx.x; r < Pd; r += blockDim.x) blkof[r] = (uint16_t)cnt;   // padding: pseudo block
+  if (minb != 0x7fffffff) atomicMin(&s_minb, minb);
   __syncthreads();
+  // an 8-run that starts on the last column of a block covers 1 + 7 more columns: 2 blocks if every block is
+  // >= 7 wide, 3 if >= 4, 4 if >= 3 (CTA-uniform choice)
+  const int32_t nb = s_minb >= 7 ? 2 : s_minb >= 4 ? 3 : s_minb >= 3 ? 4 : 0;
   const int32_t *gm = g.gmap + g.gmap_ptr[i];
   const double inv_s = 1.0 / g.scale[c_list];
   TX *Xs = X + g.col_off[c_list];
   const int32_t rows = min(GATHER_ROWS, Pd - r0);
   const int32_t n_cb = (Pd + 63) >> 6;                 // 64-column chunks (last may be partial: Pd % 16 == 0)
   const int32_t items = n_cb * rows * 8;
-  constexpr bool LOWP = sizeof(TX) == 2;               // 16-bit outputs: fp32 arithmetic is 2^-15 below their rounding
-  const float inv_sf = (float)inv_s, muf = (float)g.mu;
+  const float inv_sf = (float)inv_s, muf = (float)g.mu; // 16-bit outputs: fp32 arithmetic is 2^-15 below their rounding
   for (int32_t e = threadIdx.x; e < items; e += blockDim.x) {
     const int32_t j = e & 7;
     const int32_t rr = rows == GATHER_ROWS ? ((e >> 3) & (GATHER_ROWS - 1)) : (e >> 3) % rows;
@@ -123,35 +220,14 @@ __global__ void __launch_bounds__(256) k_gather(GatherArgs g, const TA *__restri
     if (r >= m || c0 >= m) {
 #pragma unroll
       for (int k = 0; k < 8; ++k) v[k] = from_double<TX>(0.0);
+    } else if (nb == 2) {
+      gather_run<TA, TX, 2>(g, vals, off, blkof, gm, cnt, r, c0, inv_sf, muf, inv_s, v);
+    } else if (nb == 3) {
+      gather_run<TA, TX, 3>(g, vals, off, blkof, gm, cnt, r, c0, inv_sf, muf, inv_s, v);
+    } else if (nb == 4) {
+      gather_run<TA, TX, 4>(g, vals, off, blkof, gm, cnt, r, c0, inv_sf, muf, inv_s, v);
     } else {
-      // walk the (at most 8) columns block by block: the stored block under the previous column stays cached
-      const int32_t a = blkof[r], ra = r - off[a];
-      const int32_t *gm_row = gm + (int64_t)a * cnt;
-      int32_t b = blkof[c0], bs = off[b], be = off[b + 1];
-      int32_t p = __ldg(gm_row + b);
-      const TA *src = p >= 0 ? vals + __ldg(g.vp + p) + (int64_t)ra * (be - bs) : nullptr;
-#pragma unroll
-      for (int k = 0; k < 8; ++k) {
-        const int32_t c = c0 + k;
-        if (c < m) {
-          if (c >= be) {                                  // next neighbour block (blocks are >= 1 wide)
-            ++b; bs = be; be = off[b + 1];
-            p = __ldg(gm_row + b);
-            src = p >= 0 ? vals + __ldg(g.vp + p) + (int64_t)ra * (be - bs) : nullptr;
-          }
-          if (LOWP) {
-            float x = src ? (float)__ldg(src + (c - bs)) : 0.f;
-            if (r == c) x -= muf;
-            v[k] = from_float<TX>(x * inv_sf);
-          } else {
-            double x = src ? to_double<TA>(__ldg(src + (c - bs))) : 0.0;
-            if (r == c) x -= g.mu;
-            v[k] = from_double<TX>(x * inv_s);
-          }
-        } else {
-          v[k] = from_double<TX>(0.0);
-        }
-      }
+      gather_run_any<TA, TX>(g, vals, off, blkof, gm, cnt, m, r, c0, inv_sf, muf, inv_s, v);
     }
     TX *dst = IMG ? Xs + img_off(Pd, r, c0) : Xs + (int64_t)r * Pd + c0;
     if (IMG || c0 + 8 <= Pd) {
@@ -166,36 +242,84 @@ __global__ void __launch_bounds__(256) k_gather(GatherArgs g, const TA *__restri
 
 // ---- scatter -----------------------------------------------------------------------------------
 // One CTA per listed column i.  Reads the owned ROWS of S_i (S_i symmetric): element
-// S_i[own_off + s, r] goes to block (N(i)[a], i) at [r - off[a], s].
+// S_i[own_off + s, r] goes to block (N(i)[a], i) at [r - off[a], s].  The output dominates the bytes
+// (nnzb b^2 e_R against sum m b e_x), so the kernel is organised around its stores: a strip of rows r
+// is staged in shared memory as stage[(r - r_lo) * b_i + s] -- which IS the order of the output, the
+// blocks (N(i)[a], i) being row-major [r - off[a]][s] -- and streamed out with consecutive threads on
+// consecutive output elements (a warp writes 32 contiguous elements of one block, except where it
+// crosses into the next neighbour's block).  The loads are 16-byte runs along the owned rows.
+// Dynamic smem: int32 off[cnt+1], uint16 blkof[m] (4-byte aligned end), TX stage[SCATTER_STAGE_BYTES / sizeof(TX)].
+constexpr int SCATTER_STAGE_BYTES = 48 * 1024;
+
 template <typename TX, typename TR, bool IMG>
-__global__ void k_scatter(const int32_t *__restrict__ cols, const int64_t *__restrict__ col_off,
+__global__ void __launch_bounds__(256) k_scatter(const int32_t *__restrict__ cols, const int64_t *__restrict__ col_off,
                           const int32_t *__restrict__ blk, const int32_t *__restrict__ rp,
                           const int32_t *__restrict__ ci, const int64_t *__restrict__ vp,
                           const int32_t *__restrict__ own_pos, const int32_t *__restrict__ dim,
                           const int32_t *__restrict__ dim_pad, const int32_t *__restrict__ tmap,
-                          const int32_t *__restrict__ row_off, const TX *__restrict__ S, TR *__restrict__ R) {
+                          const int32_t *__restrict__ row_off, int32_t stage_off_bytes,
+                          const TX *__restrict__ S, TR *__restrict__ R) {
   extern __shared__ int32_t smem_i[];
-  int32_t c_list = blockIdx.x;
-  int32_t i = cols ? cols[c_list] : c_list;
-  int32_t Pd = dim_pad[i], m = dim[i];
-  int32_t lo = rp[i], cnt = rp[i + 1] - lo;
+  constexpr int VEC = 16 / (int)sizeof(TX);
+  constexpr int STAGE = SCATTER_STAGE_BYTES / (int)sizeof(TX);
+  const int32_t c_list = blockIdx.x;
+  const int32_t i = cols ? cols[c_list] : c_list;
+  const int32_t Pd = dim_pad[i], m = dim[i];
+  const int32_t lo = rp[i], cnt = rp[i + 1] - lo;
   int32_t *off = smem_i;
   uint16_t *blkof = (uint16_t *)(smem_i + cnt + 1);
+  TX *stage = (TX *)((char *)smem_i + stage_off_bytes);
   for (int32_t a = threadIdx.x; a < cnt; a += blockDim.x) off[a] = row_off[lo + a];
   if (threadIdx.x == 0) off[cnt] = m;
   __syncthreads();
   for (int32_t a = threadIdx.x; a < cnt; a += blockDim.x)
     for (int32_t r = off[a]; r < off[a + 1]; ++r) blkof[r] = (uint16_t)a;
-  __syncthreads();
-  int32_t own = own_pos[i], own_off = off[own], bi = off[own + 1] - own_off;
+  const int32_t own = own_pos[i], own_off = off[own], bi = off[own + 1] - own_off;
   const TX *Ss = S + col_off[c_list];
-  for (int32_t e = threadIdx.x; e < bi * m; e += blockDim.x) {
-    int32_t s = e / m, r = e - s * m;
-    int32_t row = own_off + s;
-    TX v = IMG ? Ss[img_off(Pd, row, r)] : Ss[(int64_t)row * Pd + r];
-    int32_t a = blkof[r];
-    int32_t p = tmap[lo + a];                 // block (N(i)[a], i)
-    R[vp[p] + (int64_t)(r - off[a]) * bi + s] = (TR)to_double<TX>(v);
+  // rows per strip: a multiple of VEC so that every 16-byte run of the source lies inside one strip
+  const int32_t W = (STAGE / bi) / VEC * VEC;
+  if (W <= 0) {                                          // a block wider than the stage: element-wise fallback
+    __syncthreads();
+    for (int32_t e = threadIdx.x; e < bi * m; e += blockDim.x) {
+      int32_t s = e / m, r = e - s * m;
+      int32_t row = own_off + s;
+      TX v = IMG ? Ss[img_off(Pd, row, r)] : Ss[(int64_t)row * Pd + r];
+      int32_t a = blkof[r];
+      R[vp[tmap[lo + a]] + (int64_t)(r - off[a]) * bi + s] = (TR)to_double<TX>(v);
+    }
+    return;
+  }
+  // 16-byte loads need the rows of this submatrix 16-byte aligned (always true for the image)
+  const bool vec_ok = IMG || ((Pd % VEC) == 0 && (col_off[c_list] % VEC) == 0);
+  const uint32_t magic = 0xffffffffu / (uint32_t)bi + 1u;  // idx / bi == umulhi(idx, magic) for idx * bi < 2^32
+  for (int32_t r_lo = 0; r_lo < m; r_lo += W) {
+    const int32_t w = min(W, m - r_lo);
+    __syncthreads();                                      // blkof ready / previous strip drained
+    if (vec_ok) {
+      const int32_t groups = (w + VEC - 1) / VEC;         // a tail group may reach into the zero padding (r < Pd)
+      for (int32_t e = threadIdx.x; e < groups * bi; e += blockDim.x) {
+        const int32_t s = e / groups, gq = e - s * groups;
+        const int32_t r = r_lo + gq * VEC, row = own_off + s;
+        const TX *src = IMG ? Ss + img_off(Pd, row, r) : Ss + (int64_t)row * Pd + r;
+        __align__(16) TX v[VEC];
+        *reinterpret_cast<uint4 *>(v) = __ldg(reinterpret_cast<const uint4 *>(src));
+#pragma unroll
+        for (int k = 0; k < VEC; ++k)
+          if (gq * VEC + k < w) stage[(gq * VEC + k) * bi + s] = v[k];
+      }
+    } else {
+      for (int32_t e = threadIdx.x; e < w * bi; e += blockDim.x) {
+        const int32_t s = e / w, q = e - s * w;
+        stage[q * bi + s] = Ss[(int64_t)(own_off + s) * Pd + r_lo + q];
+      }
+    }
+    __syncthreads();
+    for (int32_t e = threadIdx.x; e < w * bi; e += blockDim.x) {
+      const int32_t q = bi == 1 ? e : (int32_t)__umulhi((uint32_t)e, magic);   // (2^32 / 1 does not fit the magic)
+      const int32_t r = r_lo + q, a = blkof[r];
+      // e - q*bi = s, so the target is block start + (r - off[a]) * bi + s = block start + e + (r_lo - off[a]) * bi
+      R[__ldg(vp + __ldg(tmap + lo + a)) + (int64_t)(r_lo - off[a]) * bi + e] = (TR)to_double<TX>(stage[e]);
+    }
   }
 }
 
@@ -218,6 +342,70 @@ __global__ void k_symmetrise(const int32_t *__restrict__ blk, const int32_t *__r
       TR v = (TR)0.5 * (a + b);
       Rp[(int64_t)r * bj + s] = v;
       Rq[(int64_t)s * bi + r] = v;
+    }
+  }
+}
+
+// D = 1/2 (I - 1/2 (R + R^T)) in place: k_symmetrise followed by k_density in one pass over the values
+// (same operations in the same order, so the bits equal the two-kernel sequence).  One CTA per block row,
+// one WARP per pair (p, q = tmap[p] >= p): both blocks are read into shared memory with consecutive lanes on
+// consecutive elements, and both are written back the same way, the transposition happening in shared memory
+// (every value is computed twice, once per target layout, from the same operands in the same order).  Pairs
+// whose blocks exceed SYMD_CAP elements take the element-wise path.
+constexpr int SYMD_WARPS = 4;
+constexpr int SYMD_CAP = 576;   // 24 x 24: 4 warps x 2 blocks x 576 fp64 = 36 KB of static shared memory
+
+template <typename TR>
+__global__ void __launch_bounds__(32 * SYMD_WARPS)
+k_symmetrise_density(const int32_t *__restrict__ blk, const int32_t *__restrict__ rp,
+                     const int32_t *__restrict__ ci, const int64_t *__restrict__ vp,
+                     const int32_t *__restrict__ tmap, TR *R) {
+  __shared__ TR sbuf[SYMD_WARPS][2][SYMD_CAP];
+  const int32_t i = blockIdx.x, bi = blk[i];
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  TR *sa = sbuf[wid][0], *sb = sbuf[wid][1];
+  for (int32_t p = rp[i] + wid; p < rp[i + 1]; p += SYMD_WARPS) {
+    const int32_t q = tmap[p];
+    if (q < p) continue;
+    const int32_t bj = blk[ci[p]], ne = bi * bj;
+    TR *Rp = R + vp[p], *Rq = R + vp[q];
+    if (ne > SYMD_CAP) {
+      for (int32_t e = lane; e < ne; e += 32) {
+        int32_t r = e / bj, s = e - r * bj;
+        if (p == q) {
+          if (s < r) continue;
+          if (s == r) { Rp[e] = (TR)0.5 * ((TR)1 - Rp[e]); continue; }
+        }
+        TR a = Rp[(int64_t)r * bj + s], b = Rq[(int64_t)s * bi + r];
+        TR v = (TR)0.5 * ((TR)0 - (TR)0.5 * (a + b));
+        Rp[(int64_t)r * bj + s] = v;
+        Rq[(int64_t)s * bi + r] = v;
+      }
+      continue;
+    }
+    __syncwarp();                                         // the previous pair's reads of sa / sb are done
+    for (int32_t e = lane; e < ne; e += 32) { sa[e] = Rp[e]; sb[e] = Rq[e]; }
+    __syncwarp();
+    if (p == q) {                                         // diagonal block: a pair (r, s), (s, r) inside one block
+      for (int32_t e = lane; e < ne; e += 32) {
+        const int32_t r = e / bj, s = e - r * bj;
+        TR v;
+        if (s == r) v = (TR)0.5 * ((TR)1 - sa[e]);
+        else {
+          const TR a = s > r ? sa[e] : sa[s * bj + r], b = s > r ? sa[s * bj + r] : sa[e];   // a = upper, b = lower
+          v = (TR)0.5 * ((TR)0 - (TR)0.5 * (a + b));
+        }
+        Rp[e] = v;
+      }
+    } else {
+      for (int32_t e = lane; e < ne; e += 32) {           // block p = (i, j): element (r, s) pairs with q's (s, r)
+        const int32_t r = e / bj, s = e - r * bj;
+        Rp[e] = (TR)0.5 * ((TR)0 - (TR)0.5 * (sa[e] + sb[s * bi + r]));
+      }
+      for (int32_t e = lane; e < ne; e += 32) {           // block q = (j, i): element (s, r), same operand order
+        const int32_t s = e / bi, r = e - s * bi;
+        Rq[e] = (TR)0.5 * ((TR)0 - (TR)0.5 * (sa[r * bj + s] + sb[e]));
+      }
     }
   }
 }
@@ -280,7 +468,7 @@ template <typename TA, typename TX, bool IMG>
 static int32_t launch_gather(const GatherArgs &g, const void *vals, void *X, int32_t n_cols, int32_t max_pd,
                              int32_t max_nbr, int32_t max_dim, cudaStream_t st) {
   dim3 grid(n_cols, (max_pd + GATHER_ROWS - 1) / GATHER_ROWS);
-  size_t smem = (size_t)(max_nbr + 1) * 4 + (size_t)(max_pd + 2) * 2;
+  size_t smem = (size_t)(max_nbr + 1 + GATHER_OFF_PAD) * 4 + (size_t)(max_pd + 2) * 2;
   (void)max_dim;
   k_gather<TA, TX, IMG><<<grid, 256, smem, st>>>(g, (const TA *)vals, (TX *)X);
   SM_LAUNCHED();
@@ -364,10 +552,17 @@ extern "C" int32_t sm_gather(const sm_bcsr_t *A, const void *A_vals, int32_t a_d
 template <typename TX, typename TR, bool IMG>
 static int32_t launch_scatter(const sm_bcsr_t *A, const sm_pattern_t *P, const int32_t *cols, int32_t n_cols,
                               const int64_t *col_off, const void *S, void *R, cudaStream_t st) {
-  size_t smem = (size_t)(P->max_nbr + 1) * 4 + (size_t)(P->max_dim + 2) * 2;
+  const int32_t stage_off = (int32_t)align_up((int64_t)(P->max_nbr + 1) * 4 + (int64_t)(P->max_dim + 2) * 2, 16);
+  const size_t smem = (size_t)stage_off + SCATTER_STAGE_BYTES;
+  static bool attr_set = false;                          // per instantiation: opt in to > 48 KB of dynamic smem
+  if (!attr_set) {
+    SM_CUDA(cudaFuncSetAttribute(k_scatter<TX, TR, IMG>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024));
+    attr_set = true;
+  }
+  if (smem > 160 * 1024) return SM_ERR_UNSUPPORTED;
   k_scatter<TX, TR, IMG><<<n_cols, 256, smem, st>>>(cols, col_off, A->blk_size, A->row_ptr, A->col_idx,
                                                     A->val_ptr, P->own_pos, P->dim, P->dim_pad, P->tmap,
-                                                    P->row_off, (const TX *)S, (TR *)R);
+                                                    P->row_off, stage_off, (const TX *)S, (TR *)R);
   SM_LAUNCHED();
   return SM_OK;
 }
@@ -410,6 +605,33 @@ extern "C" int32_t sm_scatter(const sm_bcsr_t *A, const sm_pattern_t *P, const i
 #undef SM_SCATTER_CASE
   if (rc != SM_OK) return rc;
   if (symmetrise) return sm_symmetrise(A, P, r_dtype, R_vals, stream);
+  return SM_OK;
+}
+
+// sm_symmetrise followed by sm_density_from_sign in one pass over the values (used by sm_density).
+int32_t sm::symmetrise_density(const sm_bcsr_t *A, const sm_pattern_t *P, int32_t d_dtype, void *RD_vals,
+                               double *trace, cudaStream_t st) {
+  if (d_dtype == SM_F64) {
+    k_symmetrise_density<double><<<A->n_blk, 32 * SYMD_WARPS, 0, st>>>(A->blk_size, A->row_ptr, A->col_idx, A->val_ptr, P->tmap,
+                                                           (double *)RD_vals);
+    SM_LAUNCHED();
+    if (trace) {
+      k_trace<double><<<1, 1024, 0, st>>>(A->n_blk, A->blk_size, A->row_ptr, A->val_ptr, P->own_pos,
+                                          (const double *)RD_vals, trace);
+      SM_LAUNCHED();
+    }
+  } else if (d_dtype == SM_F32) {
+    k_symmetrise_density<float><<<A->n_blk, 32 * SYMD_WARPS, 0, st>>>(A->blk_size, A->row_ptr, A->col_idx, A->val_ptr, P->tmap,
+                                                          (float *)RD_vals);
+    SM_LAUNCHED();
+    if (trace) {
+      k_trace<float><<<1, 1024, 0, st>>>(A->n_blk, A->blk_size, A->row_ptr, A->val_ptr, P->own_pos,
+                                         (const float *)RD_vals, trace);
+      SM_LAUNCHED();
+    }
+  } else {
+    return SM_ERR_UNSUPPORTED;
+  }
   return SM_OK;
 }
 
