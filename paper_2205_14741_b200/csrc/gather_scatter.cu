@@ -45,10 +45,12 @@ __global__ void k_scale_gershgorin(const int32_t *__restrict__ cols, const int32
   int32_t lo = rp[i], cnt = rp[i + 1] - lo;
   const int32_t *g = gmap + gmap_ptr[i];
   double best = 0.0;
-  // rows are enumerated as (neighbour a, local row r); neighbour a is block row ja = ci[lo + a]
-  for (int32_t a = 0; a < cnt; ++a) {
+  // rows are enumerated as (neighbour a, local row r); neighbour a is block row ja = ci[lo + a].  A warp takes
+  // every (blockDim / 32)-th neighbour and a lane one of its rows (the maximum does not depend on the order).
+  const int32_t lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
+  for (int32_t a = wid; a < cnt; a += nw) {
     int32_t ja = ci[lo + a], ba = blk[ja], rlo = rp[ja];
-    for (int32_t r = threadIdx.x; r < ba; r += blockDim.x) {
+    for (int32_t r = lane; r < ba; r += 32) {
       double s = 0.0;
       for (int32_t cc = 0; cc < cnt; ++cc) {
         int32_t p = g[a * cnt + cc];
@@ -510,7 +512,7 @@ extern "C" int32_t sm_gather(const sm_bcsr_t *A, const void *A_vals, int32_t a_d
       k_block_abs_rowsum<float><<<n, 128, 0, st>>>(A->blk_size, A->row_ptr, A->col_idx, A->val_ptr,
                                                    (const float *)A_vals, mu, rowbase, babs);
     SM_LAUNCHED();
-    k_scale_gershgorin<<<n_cols, 128, 0, st>>>(cols, A->blk_size, A->row_ptr, A->col_idx, P->gmap_ptr,
+    k_scale_gershgorin<<<n_cols, 256, 0, st>>>(cols, A->blk_size, A->row_ptr, A->col_idx, P->gmap_ptr,
                                                P->gmap, rowbase, babs, scale);
     SM_LAUNCHED();
     if (scale_mode == SM_SCALE_GLOBAL) {

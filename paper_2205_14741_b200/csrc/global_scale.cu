@@ -17,7 +17,10 @@
 namespace sm {
 
 constexpr int GLOBAL_STEPS = 10;
-constexpr int SPMV_WARPS = 4;
+#ifndef SM_SPMV_WARPS
+#define SM_SPMV_WARPS 4
+#endif
+constexpr int SPMV_WARPS = SM_SPMV_WARPS;
 constexpr int GLOBAL_MAX_BLK = 128;
 
 __global__ void k_widen_blk(int32_t n, const int32_t *__restrict__ blk, int64_t *__restrict__ out) {
