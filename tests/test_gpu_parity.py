@@ -81,7 +81,11 @@ def test_pattern_sizes_and_rejection(sm):
 
 # ------------------------------------------------------------------- a2 gather
 
-@pytest.mark.parametrize("maker", [lambda: make_config(0), ragged_workload])
+# block widths 23 / 6, 4 / 3 / (2..7 mixed) take the 2- / 3- / 4-block branch-free walk / the general walk of k_gather
+@pytest.mark.parametrize("maker", [lambda: make_config(0), ragged_workload,
+                                   lambda: make_workload(24, 23, 4, 5.0, seed=31),
+                                   lambda: make_workload(30, 4, 2, 5.0, seed=32),
+                                   lambda: make_workload(30, 3, 1, 5.0, seed=33)])
 def test_gather_fp64_exact_and_padding_invisible(sm, maker):
     wl = maker()
     A = sm.Bcsr(wl)
@@ -184,6 +188,76 @@ def test_scatter_places_owned_columns_bit_exact(sm):
                                   mats[i][r0:r1, c0:c1])
     Rs = sm.sm_symmetrise(A, P, torch.from_numpy(R).cuda()).cpu().numpy()
     assert np.array_equal(Rs, orc.symmetrise(wl, R))
+
+
+def _block_offsets(wl):
+    off = {}
+    for i in range(wl.n_blk):
+        nb = wl.col_idx[wl.row_ptr[i]:wl.row_ptr[i + 1]]
+        o = np.concatenate([[0], np.cumsum(wl.blk_size[nb])])
+        off[i] = {int(j): (int(o[a]), int(o[a + 1])) for a, j in enumerate(nb)}
+    return off
+
+
+@pytest.mark.parametrize("x_dtype,pad", [("f64", 16), ("bf16", 64), ("f16", 64)])
+def test_scatter_strips_and_images_bit_exact(sm, x_dtype, pad):
+    # 23-wide blocks with m ~ 700: several shared-memory strips per column in fp64 (266 rows each), one in the 16-bit
+    # image layout.  Entries are small integers (< 251: exact in bf16 and fp16), symmetric, so the expected block
+    # values follow directly from PAPER.md:110 step 3.
+    wl = make_workload(48, 23, 4, 6.0, seed=41)
+    A = sm.Bcsr(wl)
+    P = sm.sm_build_pattern(A, pad)
+    Ph = sm.pattern_to_host(P)
+    assert int(Ph.dim.max()) > 2 * 266
+    tdt = {"f64": torch.float64, "bf16": torch.bfloat16, "f16": torch.float16}[x_dtype]
+    S = torch.zeros(P.packed_elems, dtype=tdt, device="cuda")
+    mats = []
+    for i in range(wl.n_blk):
+        m, Pd = int(Ph.dim[i]), int(Ph.dim_pad[i])
+        r = np.arange(m)
+        Si = ((np.minimum.outer(r, r) * 7 + np.maximum.outer(r, r) * 3 + i) % 251).astype(np.float64)
+        full = np.zeros((Pd, Pd))
+        full[:m, :m] = Si
+        flat = np.zeros(Pd * Pd)
+        if x_dtype == "f64":
+            flat[:] = full.ravel()
+        else:
+            flat[img_index(Pd).ravel()] = full.ravel()
+        S[int(Ph.sub_off[i]):int(Ph.sub_off[i + 1])] = torch.from_numpy(flat).to(tdt).cuda()
+        mats.append(Si)
+    for r_dtype in ("f64", "f32"):
+        R = sm.sm_scatter(A, P, None, P.sub_off, wl.n_blk, x_dtype, S, r_dtype=r_dtype).double().cpu().numpy()
+        off = _block_offsets(wl)
+        for j in range(wl.n_blk):
+            for p in range(wl.row_ptr[j], wl.row_ptr[j + 1]):
+                i = int(wl.col_idx[p])
+                (r0, r1), (c0, c1) = off[i][j], off[i][i]
+                assert np.array_equal(R[wl.val_ptr[p]:wl.val_ptr[p + 1]].reshape(r1 - r0, c1 - c0),
+                                      mats[i][r0:r1, c0:c1]), (j, i)
+
+
+@pytest.mark.parametrize("maker", [ragged_workload, lambda: make_workload(24, 23, 4, 5.0, seed=31),
+                                   lambda: make_workload(12, 30, 5, 5.0, seed=34)])
+def test_fused_symmetrise_density_equals_the_two_calls(sm, maker):
+    # sm_density ends with ONE pass (k_symmetrise_density); sm_symmetrise + sm_density_from_sign are its definition.
+    # 30-wide blocks exceed the kernel's shared-memory pair buffer and take its element-wise path.
+    wl = maker()
+    A = sm.Bcsr(wl)
+    P = sm.sm_build_pattern(A, 16)
+    for sym in (False, True):
+        plan = sm.DensityPlan(A, P, "f64")
+        sm.sm_density(A, P, plan, mu=0.0, scale_mode="gershgorin", max_iter=7, tol=0.0, symmetrise=sym)
+        cols, col_off, n = sm.sm_plan_columns(P, None)
+        X, _ = sm.sm_gather(A, P, cols, col_off, n, 0.0, "gershgorin", "f64")
+        sm.sm_sign_ns(P, cols, col_off, n, P.packed_elems, "f64", X, 7, 0.0)
+        R = sm.sm_scatter(A, P, cols, col_off, n, "f64", X)
+        if sym:
+            R = sm.sm_symmetrise(A, P, R)
+            assert np.array_equal(R.cpu().numpy(), orc.symmetrise(wl, R.cpu().numpy()))   # already symmetric: a fixed point
+        D, tr = sm.sm_density_from_sign(A, P, R)
+        torch.cuda.synchronize()
+        assert torch.equal(plan.D, D)
+        assert plan.trace.item() == tr.item()
 
 
 # ------------------------------------------------------------ a5 whole path, small configs
