@@ -47,6 +47,7 @@ def parse_args():
     ap.add_argument("--run", type=int, default=0, help="index into the config's precision runs")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--scale", default=None, help="none|gershgorin|power|global (default: global for 16-bit, gershgorin otherwise)")
+    ap.add_argument("--h-dtype", default=None, choices=["f64", "f32"], help="storage type of the H values (default: f32 for 16-bit runs, f64 otherwise)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -192,7 +193,11 @@ def run_ours(args, cfg, cfg_run):
     from paper_2205_14741_b200 import dist_util
     wl = make_config(args.config, seed=dist_util.rank_seed(cfg["seed"], rank))
     dims, sum_m3 = workload_stats(wl)
-    A = sm.Bcsr(wl)
+    # H storage (SURVEY 8(d) G5 / reading A16): the fp64 master copy for the fp64 / fp32 runs, an fp32 copy for the
+    # 16-bit runs (cast once on the host when the workload is made; X0 is rounded from fp32 arithmetic either way)
+    h_dtype = args.h_dtype or ("f32" if is16 else "f64")
+    hb = {"f64": 8, "f32": 4}[h_dtype]
+    A = sm.Bcsr(wl, val_dtype=h_dtype)
     P = sm.sm_build_pattern(A, pad)
     eb = {"f64": 8, "f32": 4, "bf16": 2, "f16": 2}[x_dtype]
     free_b, _ = torch.cuda.mem_get_info()
@@ -258,13 +263,13 @@ def run_ours(args, cfg, cfg_run):
             _, stages["density_ms"] = timed(lambda: sm.sm_density_from_sign(A, Pn, R))
             stages["sign_tflops"] = flops_step / (stages["sign_ms"] * 1e-3) / 1e12
             e_x = eb
-            stages["gather_gbs"] = (Pn.packed_elems * e_x + A.n_vals * 8 + Pn.gmap_len * 4) / (stages["gather_ms"] * 1e-3) / 1e9
+            stages["gather_gbs"] = (Pn.packed_elems * e_x + A.n_vals * hb + Pn.gmap_len * 4) / (stages["gather_ms"] * 1e-3) / 1e9
             del X, ws
 
     # ---- end to end through the public call with HOST buffers (pinned), copies inside the timed region
     e2e = None
     if not args.no_e2e:
-        h_vals = torch.from_numpy(np.ascontiguousarray(wl.vals)).pin_memory()
+        h_vals = torch.from_numpy(np.ascontiguousarray(wl.vals, dtype=np.float32 if h_dtype == "f32" else np.float64)).pin_memory()
         h_D = torch.empty(A.n_vals, dtype=torch.float64).pin_memory()
         h_tr = torch.empty(1, dtype=torch.float64).pin_memory()
         h_idx = [torch.from_numpy(np.ascontiguousarray(x)).pin_memory() for x in
@@ -277,7 +282,7 @@ def run_ours(args, cfg, cfg_run):
         # memory and its own D and Tr D back, all inside the timed region.  Two sets of device inputs and outputs
         # (the large workspace is shared: compute is serial on the main stream).
         import copy
-        A_b = [A, sm.Bcsr(wl)]
+        A_b = [A, sm.Bcsr(wl, val_dtype=h_dtype)]
         plan_b = [plan, copy.copy(plan)]
         plan_b[1].D = torch.zeros_like(plan.D); plan_b[1].trace = torch.zeros_like(plan.trace)
         plan_b[1].iters = torch.zeros_like(plan.iters); plan_b[1].residual = torch.zeros_like(plan.residual)
@@ -321,7 +326,7 @@ def run_ours(args, cfg, cfg_run):
         b.record()
         torch.cuda.synchronize()
         e2e_ms = dist_util.aggregate(a.elapsed_time(b), 0.0, torch.device("cuda", local))[0] / args.steps
-        h2d = int(h_vals.numel() * 8 + sum(x.numel() * x.element_size() for x in h_idx))
+        h2d = int(h_vals.numel() * hb + sum(x.numel() * x.element_size() for x in h_idx))
         d2h = int(h_D.numel() * 8 + 8)
         e2e = {"value": flops_all / (e2e_ms * 1e-3) / 1e12, "unit": UNIT, "ms_per_step": e2e_ms,
                "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
@@ -380,7 +385,7 @@ def run_ours(args, cfg, cfg_run):
         "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": x_dtype, "data": "synthetic",
         "config": {"workload": cfg["name"], "n_mol": cfg["n_mol"], "orbitals": cfg["b"], "cutoff_A": cfg["cutoff"],
-                   "x_dtype": x_dtype, "max_iter": max_iter, "tol": tol, "scale_mode": scale_mode, "pad_to": pad,
+                   "x_dtype": x_dtype, "max_iter": max_iter, "tol": tol, "scale_mode": scale_mode, "h_dtype": h_dtype, "pad_to": pad,
                    "l2": "inputs_exceed_l2" if P.packed_elems * eb > 200e6 else "inputs_fit_l2",
                    "chunks": int(-(-P.packed_elems // max_chunk))},
         "block_columns_per_s": world * wl.n_blk / (ms_per_step * 1e-3),

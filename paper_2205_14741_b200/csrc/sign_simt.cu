@@ -40,14 +40,18 @@ k_simt_gemm(const int32_t *__restrict__ cols, const int64_t *__restrict__ col_of
 #pragma unroll
     for (int b = 0; b < 4; ++b) acc[a][b] = (T)0;
 
-  for (int32_t k0 = 0; k0 < m; k0 += SK) {
+  // Register-staged software pipeline: the global loads of k tile t + 1 are issued before the FMAs of tile t and
+  // written to shared memory after them, so their latency overlaps the arithmetic (same summation order as a
+  // plain loop: results are bit-identical).
+  T ra[4], rb[4];
+  auto gload = [&](int32_t k0) {
     // A tile: 64 rows x 16 k (row-major source: k contiguous)
 #pragma unroll
     for (int l = 0; l < 4; ++l) {
       int32_t e = threadIdx.x + l * 256;
       int32_t r = e >> 4, k = e & 15;
       int32_t gr = row0 + r, gk = k0 + k;
-      As[k][r] = (gr < m && gk < m) ? A[(int64_t)gr * Pd + gk] : (T)0;
+      ra[l] = (gr < m && gk < m) ? A[(int64_t)gr * Pd + gk] : (T)0;
     }
     // B tile: 16 k x 64 cols (column contiguous)
 #pragma unroll
@@ -55,9 +59,23 @@ k_simt_gemm(const int32_t *__restrict__ cols, const int64_t *__restrict__ col_of
       int32_t e = threadIdx.x + l * 256;
       int32_t k = e >> 6, cc = e & 63;
       int32_t gk = k0 + k, gc = col0 + cc;
-      Bs[k][cc] = (gk < m && gc < m) ? B[(int64_t)gk * Pd + gc] : (T)0;
+      rb[l] = (gk < m && gc < m) ? B[(int64_t)gk * Pd + gc] : (T)0;
     }
-    __syncthreads();
+  };
+  auto sstore = [&]() {
+#pragma unroll
+    for (int l = 0; l < 4; ++l) {
+      int32_t e = threadIdx.x + l * 256;
+      As[e & 15][e >> 4] = ra[l];
+      Bs[e >> 6][e & 63] = rb[l];
+    }
+  };
+  gload(0);
+  sstore();
+  __syncthreads();
+  for (int32_t k0 = 0; k0 < m; k0 += SK) {
+    const bool more = k0 + SK < m;
+    if (more) gload(k0 + SK);
 #pragma unroll
     for (int k = 0; k < SK; ++k) {
       T a[4], b[4];
@@ -68,6 +86,8 @@ k_simt_gemm(const int32_t *__restrict__ cols, const int64_t *__restrict__ col_of
 #pragma unroll
         for (int p = 0; p < 4; ++p) acc[q][p] += a[q] * b[p];
     }
+    __syncthreads();
+    if (more) sstore();
     __syncthreads();
   }
 

@@ -108,9 +108,10 @@ def test_gather_fp64_exact_and_padding_invisible(sm, maker):
 
 
 @pytest.mark.parametrize("x_dtype,eps", [("bf16", 2.0 ** -8), ("f16", 2.0 ** -11), ("f32", 2.0 ** -24)])
-def test_gather_low_precision_subset_in_listed_order(sm, x_dtype, eps):
+@pytest.mark.parametrize("val_dtype", ["f64", "f32"])
+def test_gather_low_precision_subset_in_listed_order(sm, x_dtype, eps, val_dtype):
     wl = make_config(1)
-    A = sm.Bcsr(wl)
+    A = sm.Bcsr(wl, val_dtype=val_dtype)
     P = sm.sm_build_pattern(A, 64)
     Ph = sm.pattern_to_host(P)
     cols_h = np.array([977, 3, 500, 42], np.int32)
@@ -123,7 +124,8 @@ def test_gather_low_precision_subset_in_listed_order(sm, x_dtype, eps):
         m = T.shape[0]
         x = unpack(X, Ph, int(i), x_dtype, off, k)
         ref = T / orc.gershgorin(T)
-        assert np.abs(x[:m, :m] - ref).max() <= eps * 1.01     # one rounding of |x| <= 1
+        # one rounding of |x| <= 1 (H read from its fp32 copy: plus the 2^-24 of that cast and of the fp32 scale)
+        assert np.abs(x[:m, :m] - ref).max() <= eps * 1.01 + (2.0 ** -22 if val_dtype == "f32" else 0.0)
         assert not x[m:].any() and not x[:, m:].any()
 
 
@@ -262,8 +264,9 @@ def test_fused_symmetrise_density_equals_the_two_calls(sm, maker):
 
 # ------------------------------------------------------------ a5 whole path, small configs
 
-def run_density(sm, wl, x_dtype, max_iter, tol, scale_mode, symmetrise=False, max_chunk_elems=None, pad=None):
-    A = sm.Bcsr(wl)
+def run_density(sm, wl, x_dtype, max_iter, tol, scale_mode, symmetrise=False, max_chunk_elems=None, pad=None,
+                val_dtype="f64"):
+    A = sm.Bcsr(wl, val_dtype=val_dtype)
     P = sm.sm_build_pattern(A, pad or (64 if x_dtype in ("bf16", "f16") else 16))
     plan = sm.DensityPlan(A, P, x_dtype, max_chunk_elems=max_chunk_elems)
     sm.sm_density(A, P, plan, mu=0.0, scale_mode=scale_mode, max_iter=max_iter, tol=tol, symmetrise=symmetrise)
@@ -399,31 +402,35 @@ def test_cfg2_bf16_full_size_sampled(sm):
     assert e["rounding"] <= 1.2e-2, e            # bf16 rounding alone, against the NS-20 polynomial
 
 
-def test_cfg2_bf16_full_size_global_scale(sm):
-    # SM_SCALE_GLOBAL (one interlacing bound from power steps on the whole block-sparse matrix): bench.py's scale mode
+@pytest.mark.parametrize("val_dtype", ["f32", "f64"])
+def test_cfg2_bf16_full_size_global_scale(sm, val_dtype):
+    # SM_SCALE_GLOBAL (one interlacing bound from power steps on the whole block-sparse matrix) on the fp32 copy of H
+    # (reading A16): bench.py's configuration for the 16-bit runs.  The oracle reads the fp64 H.
     wl = make_config(2)
     run = CONFIGS[2]["runs"][0]
-    _, P, plan = run_density(sm, wl, "bf16", run["max_iter"], 0.0, "global", symmetrise=False)
+    _, P, plan = run_density(sm, wl, "bf16", run["max_iter"], 0.0, "global", symmetrise=False, val_dtype=val_dtype)
     e = sampled_errors(wl, P, plan, sample_columns(wl, 24, 4242), run["max_iter"])
     print("cfg2 global-scale errors", e)
     assert e["total"] <= 2e-2 and e["dtr"] <= 1e-3, e
     assert e["rounding"] <= 1.2e-2, e
 
 
-def test_cfg3_fp16_full_size_sampled(sm):
+@pytest.mark.parametrize("scale_mode,val_dtype", [("gershgorin", "f64"), ("global", "f32")])   # the second is bench.py's
+def test_cfg3_fp16_full_size_sampled(sm, scale_mode, val_dtype):
     wl = make_config(3)
     run = CONFIGS[3]["runs"][0]
-    _, P, plan = run_density(sm, wl, "f16", run["max_iter"], 0.0, "gershgorin")
+    _, P, plan = run_density(sm, wl, "f16", run["max_iter"], 0.0, scale_mode, val_dtype=val_dtype)
     e = sampled_errors(wl, P, plan, sample_columns(wl, 64, 4242), run["max_iter"], lapack=False)
     assert e["total"] <= 2e-2 and e["dtr"] <= 1e-3, e
     # "fp32 oracle comparison" (configs[3]): compare in fp32 after casting the fp64 oracle
     assert np.float32(e["maxabs"]) <= np.float32(2e-3), e
 
 
-@pytest.mark.parametrize("x_dtype,scale_mode", [("bf16", "power"), ("f16", "power"), ("bf16", "global")])
-def test_cfg4_16bit_full_size_sampled(sm, x_dtype, scale_mode):
+@pytest.mark.parametrize("x_dtype,scale_mode,val_dtype", [("bf16", "power", "f64"), ("f16", "power", "f64"),
+                                                          ("bf16", "global", "f32"), ("f16", "global", "f32")])
+def test_cfg4_16bit_full_size_sampled(sm, x_dtype, scale_mode, val_dtype):
     wl = make_config(4)
-    _, P, plan = run_density(sm, wl, x_dtype, 25, 0.0, scale_mode)
+    _, P, plan = run_density(sm, wl, x_dtype, 25, 0.0, scale_mode, val_dtype=val_dtype)
     e = sampled_errors(wl, P, plan, sample_columns(wl, 4, 4242), 25)
     print("cfg4", x_dtype, scale_mode, e)
     assert e["total"] <= 2e-2 and e["dtr"] <= 1e-3, e
