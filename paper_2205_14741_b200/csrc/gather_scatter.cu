@@ -79,7 +79,8 @@ __global__ void k_fill_double(int32_t n, double v, double *__restrict__ out) {
 // grid = (listed column, band of GATHER_ROWS rows), 256 threads.  A work item is one 16-byte-aligned
 // run of 8 output elements (r, c0..c0+7); items are ordered so that the 8 lanes of a row cover one
 // 64-column chunk, i.e. a warp writes four full 128-byte lines of the image (or 4 contiguous row
-// segments of the row-major layout).  Dynamic smem: int32 off[cnt+1], uint16 blkof[Pd].
+// segments of the row-major layout).  Dynamic smem: int32 off[cnt+1+GATHER_OFF_PAD]
+// (block starts, then m, then the ends of the pseudo blocks behind the last neighbour), uint16 blkof[Pd].
 constexpr int GATHER_ROWS = 64;
 
 struct GatherArgs {
