@@ -48,6 +48,7 @@ def parse_args():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--scale", default=None, help="none|gershgorin|power|global (default: global for 16-bit, gershgorin otherwise)")
     ap.add_argument("--h-dtype", default=None, choices=["f64", "f32"], help="storage type of the H values (default: f32 for 16-bit runs, f64 otherwise)")
+    ap.add_argument("--chunk-elems", type=int, default=0, help="cap on the packed elements per chunk of sm_density (0: one chunk if it fits)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -203,6 +204,8 @@ def run_ours(args, cfg, cfg_run):
     free_b, _ = torch.cuda.mem_get_info()
     budget = int(0.25 * free_b / eb)
     max_chunk = P.packed_elems if P.packed_elems <= budget else max(budget, P.max_dim_pad ** 2)
+    if args.chunk_elems > 0:
+        max_chunk = max(min(max_chunk, args.chunk_elems), P.max_dim_pad ** 2)
     plan = sm.DensityPlan(A, P, x_dtype, max_chunk_elems=max_chunk)
 
     def step():
