@@ -412,3 +412,28 @@ def test_lapack_variant_matches_jacobi_oracle():
     d_j, _ = orc.density_columns(w2, cols=[1, 2])
     d_l, _ = orc.density_columns_lapack(w2, cols=[1, 2])
     assert np.abs(d_j - d_l).max() < 1e-11
+
+
+def test_oracle_matches_stored_golden():
+    # Regression fixture (tests/golden/README.md): what the pinned oracle returns for configs[0], written by
+    # tests/golden/make_golden.py from oracle/ alone.  Tr D in the full-coverage limit is also a pin of its own:
+    # 3 occupied orbitals x 32 molecules = 96 negative eigenvalues (BASELINE.json configs[0], north_star).
+    import importlib.util
+    import os
+    here = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+    spec = importlib.util.spec_from_file_location("make_golden", os.path.join(here, "make_golden.py"))
+    mod = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mod)
+    now = mod.golden_values()
+    stored = {}
+    with open(os.path.join(here, "cfg0_oracle.txt")) as f:
+        for line in f:
+            if line.startswith("#") or not line.strip():
+                continue
+            k, v = line.split()
+            stored[k] = float(v)
+    assert set(stored) == set(now)
+    for k, v in stored.items():
+        assert abs(now[k] - v) <= 1e-11 * max(1.0, abs(v)), (k, now[k], v)
+    assert abs(stored["trace_full_coverage"] - 96.0) <= 1e-9
+    assert stored["trace_sym"] == stored["trace"]
