@@ -326,31 +326,9 @@ __global__ void __launch_bounds__(256) k_scatter(const int32_t *__restrict__ col
   }
 }
 
-// R <- 1/2 (R + R^T) blockwise, in place.  One CTA per block row; the lower-indexed partner of a
-// pair (p, tmap[p]) owns both blocks.
-template <typename TR>
-__global__ void k_symmetrise(const int32_t *__restrict__ blk, const int32_t *__restrict__ rp,
-                             const int32_t *__restrict__ ci, const int64_t *__restrict__ vp,
-                             const int32_t *__restrict__ tmap, TR *R) {
-  int32_t i = blockIdx.x, bi = blk[i];
-  for (int32_t p = rp[i]; p < rp[i + 1]; ++p) {
-    int32_t q = tmap[p];
-    if (q < p) continue;
-    int32_t bj = blk[ci[p]];
-    TR *Rp = R + vp[p], *Rq = R + vp[q];
-    for (int32_t e = threadIdx.x; e < bi * bj; e += blockDim.x) {
-      int32_t r = e / bj, s = e - r * bj;
-      if (p == q && s <= r) continue;
-      TR a = Rp[(int64_t)r * bj + s], b = Rq[(int64_t)s * bi + r];
-      TR v = (TR)0.5 * (a + b);
-      Rp[(int64_t)r * bj + s] = v;
-      Rq[(int64_t)s * bi + r] = v;
-    }
-  }
-}
-
-// D = 1/2 (I - 1/2 (R + R^T)) in place: k_symmetrise followed by k_density in one pass over the values
-// (same operations in the same order, so the bits equal the two-kernel sequence).  One CTA per block row,
+// D = 1/2 (I - 1/2 (R + R^T)) in place: the blockwise symmetrisation R <- 1/2 (R + R^T) (the lower-indexed partner of a
+// pair (p, tmap[p]) owns both blocks) followed by k_density, in one pass over the values (same operations in the same
+// order, so the bits equal sm_symmetrise followed by sm_density_from_sign).  One CTA per block row,
 // one WARP per pair (p, q = tmap[p] >= p): both blocks are read into shared memory with consecutive lanes on
 // consecutive elements, and both are written back the same way, the transposition happening in shared memory
 // (every value is computed twice, once per target layout, from the same operands in the same order).  Pairs
@@ -358,7 +336,8 @@ __global__ void k_symmetrise(const int32_t *__restrict__ blk, const int32_t *__r
 constexpr int SYMD_WARPS = 4;
 constexpr int SYMD_CAP = 576;   // 24 x 24: 4 warps x 2 blocks x 576 fp64 = 36 KB of static shared memory
 
-template <typename TR>
+// DENS = false: the symmetrisation alone (sm_symmetrise), R <- 1/2 (R + R^T), diagonal elements untouched.
+template <typename TR, bool DENS>
 __global__ void __launch_bounds__(32 * SYMD_WARPS)
 k_symmetrise_density(const int32_t *__restrict__ blk, const int32_t *__restrict__ rp,
                      const int32_t *__restrict__ ci, const int64_t *__restrict__ vp,
@@ -377,10 +356,10 @@ k_symmetrise_density(const int32_t *__restrict__ blk, const int32_t *__restrict_
         int32_t r = e / bj, s = e - r * bj;
         if (p == q) {
           if (s < r) continue;
-          if (s == r) { Rp[e] = (TR)0.5 * ((TR)1 - Rp[e]); continue; }
+          if (s == r) { if (DENS) Rp[e] = (TR)0.5 * ((TR)1 - Rp[e]); continue; }
         }
         TR a = Rp[(int64_t)r * bj + s], b = Rq[(int64_t)s * bi + r];
-        TR v = (TR)0.5 * ((TR)0 - (TR)0.5 * (a + b));
+        TR v = DENS ? (TR)0.5 * ((TR)0 - (TR)0.5 * (a + b)) : (TR)0.5 * (a + b);
         Rp[(int64_t)r * bj + s] = v;
         Rq[(int64_t)s * bi + r] = v;
       }
@@ -393,21 +372,23 @@ k_symmetrise_density(const int32_t *__restrict__ blk, const int32_t *__restrict_
       for (int32_t e = lane; e < ne; e += 32) {
         const int32_t r = e / bj, s = e - r * bj;
         TR v;
-        if (s == r) v = (TR)0.5 * ((TR)1 - sa[e]);
+        if (s == r) v = DENS ? (TR)0.5 * ((TR)1 - sa[e]) : sa[e];
         else {
           const TR a = s > r ? sa[e] : sa[s * bj + r], b = s > r ? sa[s * bj + r] : sa[e];   // a = upper, b = lower
-          v = (TR)0.5 * ((TR)0 - (TR)0.5 * (a + b));
+          v = DENS ? (TR)0.5 * ((TR)0 - (TR)0.5 * (a + b)) : (TR)0.5 * (a + b);
         }
         Rp[e] = v;
       }
     } else {
       for (int32_t e = lane; e < ne; e += 32) {           // block p = (i, j): element (r, s) pairs with q's (s, r)
         const int32_t r = e / bj, s = e - r * bj;
-        Rp[e] = (TR)0.5 * ((TR)0 - (TR)0.5 * (sa[e] + sb[s * bi + r]));
+        const TR h = (TR)0.5 * (sa[e] + sb[s * bi + r]);
+        Rp[e] = DENS ? (TR)0.5 * ((TR)0 - h) : h;
       }
       for (int32_t e = lane; e < ne; e += 32) {           // block q = (j, i): element (s, r), same operand order
         const int32_t s = e / bi, r = e - s * bi;
-        Rq[e] = (TR)0.5 * ((TR)0 - (TR)0.5 * (sa[r * bj + s] + sb[e]));
+        const TR h = (TR)0.5 * (sa[r * bj + s] + sb[e]);
+        Rq[e] = DENS ? (TR)0.5 * ((TR)0 - h) : h;
       }
     }
   }
@@ -575,11 +556,11 @@ extern "C" int32_t sm_symmetrise(const sm_bcsr_t *A, const sm_pattern_t *P, int3
   if (!A || !P || !R_vals) return SM_ERR_ARG;
   cudaStream_t st = (cudaStream_t)stream;
   if (r_dtype == SM_F64)
-    k_symmetrise<double><<<A->n_blk, 128, 0, st>>>(A->blk_size, A->row_ptr, A->col_idx, A->val_ptr, P->tmap,
-                                                   (double *)R_vals);
+    k_symmetrise_density<double, false><<<A->n_blk, 32 * SYMD_WARPS, 0, st>>>(A->blk_size, A->row_ptr, A->col_idx,
+                                                                             A->val_ptr, P->tmap, (double *)R_vals);
   else if (r_dtype == SM_F32)
-    k_symmetrise<float><<<A->n_blk, 128, 0, st>>>(A->blk_size, A->row_ptr, A->col_idx, A->val_ptr, P->tmap,
-                                                  (float *)R_vals);
+    k_symmetrise_density<float, false><<<A->n_blk, 32 * SYMD_WARPS, 0, st>>>(A->blk_size, A->row_ptr, A->col_idx,
+                                                                            A->val_ptr, P->tmap, (float *)R_vals);
   else
     return SM_ERR_UNSUPPORTED;
   SM_LAUNCHED();
@@ -615,7 +596,7 @@ extern "C" int32_t sm_scatter(const sm_bcsr_t *A, const sm_pattern_t *P, const i
 int32_t sm::symmetrise_density(const sm_bcsr_t *A, const sm_pattern_t *P, int32_t d_dtype, void *RD_vals,
                                double *trace, cudaStream_t st) {
   if (d_dtype == SM_F64) {
-    k_symmetrise_density<double><<<A->n_blk, 32 * SYMD_WARPS, 0, st>>>(A->blk_size, A->row_ptr, A->col_idx, A->val_ptr, P->tmap,
+    k_symmetrise_density<double, true><<<A->n_blk, 32 * SYMD_WARPS, 0, st>>>(A->blk_size, A->row_ptr, A->col_idx, A->val_ptr, P->tmap,
                                                            (double *)RD_vals);
     SM_LAUNCHED();
     if (trace) {
@@ -624,7 +605,7 @@ int32_t sm::symmetrise_density(const sm_bcsr_t *A, const sm_pattern_t *P, int32_
       SM_LAUNCHED();
     }
   } else if (d_dtype == SM_F32) {
-    k_symmetrise_density<float><<<A->n_blk, 32 * SYMD_WARPS, 0, st>>>(A->blk_size, A->row_ptr, A->col_idx, A->val_ptr, P->tmap,
+    k_symmetrise_density<float, true><<<A->n_blk, 32 * SYMD_WARPS, 0, st>>>(A->blk_size, A->row_ptr, A->col_idx, A->val_ptr, P->tmap,
                                                           (float *)RD_vals);
     SM_LAUNCHED();
     if (trace) {
