@@ -150,13 +150,33 @@ int32_t sm_gather(const sm_bcsr_t *A, const void *A_vals, int32_t a_dtype, const
  *                  X_{k+1} = 1.5 X_k - 0.5 X_k Y;  stop after this update if r_k < tol.
  * tol <= 0 runs exactly max_iter updates.  iters[c] = updates applied, residual[c] = last
  * r_k computed.  SM_BF16/SM_F16 run on tcgen05 tensor cores with fp32 accumulation
- * (PAPER.md:104); SM_F32/SM_F64 on FFMA/DFMA.  packed_elems = col_off[n_cols] (host value).
+ * (PAPER.md:104): submatrices with Pd <= 256 stay in the shared memory of one SM for all steps, larger ones run as
+ * grouped tiles with one launch per product; SM_F64 runs on the fp64 tensor-core instruction (mma.sync m8n8k4,
+ * DMMA), SM_F32 on FFMA.  packed_elems = col_off[n_cols] (host value).
  * ws >= sm_sign_ws_bytes(...).  Asynchronous; sm_sign_status reports non-convergence. */
 int64_t sm_sign_ws_bytes(const sm_pattern_t *P, int32_t n_cols, int64_t packed_elems, int32_t x_dtype);
 int32_t sm_sign_ns(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols,
                    const int64_t *col_off, int64_t packed_elems, int32_t x_dtype, void *X_packed,
                    void *ws, int64_t ws_bytes, int32_t max_iter, double tol,
                    int32_t *iters /*[n_cols]*/, double *residual /*[n_cols]*/, void *stream);
+/* sm_sign_ns with two more arguments (sm_sign_ns = flags 0, switch_iter -1):
+ *   flags & SM_SIGN_NONSYMMETRIC: the matrices are NOT symmetric (used for Eq. 12: the sign of the
+ *     block matrix [[0, A], [I, 0]]).  Every tile is computed with true products X X and X Y (the 16-bit kernel reads
+ *     its B operand MN-major from the same image), nothing is mirrored; the default exploits and enforces symmetry.
+ *   switch_iter >= 0: precision schedule "low precision early, higher precision late" (SURVEY
+ *     8(f) f3): x_dtype must be SM_BF16, tol <= 0 and 0 < switch_iter < max_iter; updates 0 .. switch_iter-1 run on
+ *     bf16 operands, update switch_iter-1 rounds its result to fp16 and the remaining updates run on fp16 operands
+ *     (same kind::f16 MMA, 11 instead of 8 significand bits; |x| <= ~1 after scaling, so the range is safe).
+ *     X_packed then holds SM_F16 images on return.
+ * ws >= sm_sign_ws_bytes_ex(..., flags). */
+#define SM_SIGN_NONSYMMETRIC 1
+int64_t sm_sign_ws_bytes_ex(const sm_pattern_t *P, int32_t n_cols, int64_t packed_elems, int32_t x_dtype,
+                            int32_t flags);
+int32_t sm_sign_ns_ex(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols,
+                      const int64_t *col_off, int64_t packed_elems, int32_t x_dtype, void *X_packed,
+                      void *ws, int64_t ws_bytes, int32_t max_iter, double tol, int32_t flags,
+                      int32_t switch_iter, int32_t *iters /*[n_cols]*/, double *residual /*[n_cols]*/,
+                      void *stream);
 /* Synchronises and returns SM_WARN_NOT_CONVERGED if tol > 0 and any residual[c] >= tol. */
 int32_t sm_sign_status(const double *residual, int32_t n_cols, double tol, void *scratch, void *stream);
 
@@ -207,20 +227,31 @@ int32_t sm_mu_search(const sm_bcsr_t *A, const void *A_vals, int32_t a_dtype, do
 int32_t sm_density_from_sign(const sm_bcsr_t *A, const sm_pattern_t *P, int32_t d_dtype,
                              void *RD_vals, double *trace, void *stream);
 
-/* Environment variables read once per process by sm_sign_ns (A/B measurements and the back-end tests; production
- * code leaves them unset and gets the measured-best variant for the pattern's largest submatrix):
- *   SM_UMMA_NCTA=1|2   16-bit: one CTA / two CTAs of a cluster per output tile
- *   SM_UMMA_MC=1|0     16-bit, two CTAs: cta_group::1 MMAs with the B rows multicast / cta_group::2 MMAs (relay)
- *   SM_UMMA_TMAP=1     16-bit, cta_group::2 pairs: operands through tensor-map TMA that signals the leader's barrier (no relay)
- *   SM_UMMA_SYM=1|0    16-bit: lower-triangle tiles with mirrored stores / true products, all tiles
- *   SM_UMMA_REV=1|0    16-bit: the update product walks the tile table backwards / forwards
- *   SM_UMMA_STAGES=3|4 16-bit, one CTA per tile: depth of the operand ring
- *   SM_UMMA_DYN=1|0    16-bit, one CTA per tile: tiles handed out by a global counter / dealt round robin
- *   SM_UMMA_STREAM=1   16-bit, tol <= 0, one CTA per tile: one launch walks every product of every step, products of a
- *                      submatrix ordered by per-group completion counters
- *   SM_UMMA_FUSED=1    16-bit, tol <= 0: one launch runs every step of a submatrix (SM_UMMA_SLOTS=1|2 in flight)
- *   SM_F64_BACKEND=dmma|simt   fp64: tensor-core m8n8k4 tiles / DFMA register tiles
- *   SM_UMMA_DBG, SM_UMMA_TRACE measurement only (skip-knobs that produce WRONG results; clock64 time line). */
+/* Variant selection (A/B measurements and the back-end tests; production code leaves everything at its default
+ * and gets the measured-best variant).  Process-wide; every option is initialised once from the environment
+ * variable given in brackets, and sm_set_option changes it for the calls that follow (not synchronised with
+ * calls in flight on other threads).  Unknown name: SM_ERR_ARG.
+ *   "umma.sym"      [SM_UMMA_SYM]      1|0   16-bit: lower-triangle tiles with mirrored stores / true products, all tiles
+ *   "umma.resident" [SM_UMMA_RESIDENT] 1|0   16-bit: submatrices with Pd <= 256 iterate inside one SM / grouped tiles for all
+ *   "umma.lt"       [SM_UMMA_LT]       0|1   16-bit grouped tiles: iterates stored lower-triangular (half the stores)
+ *   "umma.dyn"      [SM_UMMA_DYN]      1|0   16-bit grouped tiles handed out by a global counter / dealt round robin
+ *   "umma.rev"      [SM_UMMA_REV]      1|0   16-bit: the update product walks the tile table backwards / forwards
+ *   "umma.stages"   [SM_UMMA_STAGES]   0|3|4 16-bit grouped tiles: depth of the operand ring (0 = by size)
+ *   "umma.stream"   [SM_UMMA_STREAM]   0|1   16-bit, tol <= 0: one launch walks every product of every step
+ *   "f64.simt"      [SM_F64_SIMT]      0|1   fp64: tensor-core m8n8k4 tiles / DFMA register tiles
+ *   "gather.tma"    [SM_GATHER_TMA]    1|0   sm_gather, 16-bit X: shared-memory-staged kernel / element-wise kernel
+ * A library built with -DSM_MEASURE (build.py --measure; sm_build_info() & 1) additionally has the measured-slower
+ * two-CTA and fused variants and the skip-knobs used for DESIGN.md's decompositions ("umma.ncta", "umma.mc",
+ * "umma.tmap", "umma.fused", "umma.slots", "umma.dbg"; the last produces WRONG results by construction).  In the
+ * default build those names answer SM_ERR_UNSUPPORTED and their environment variables are not read. */
+int32_t sm_set_option(const char *name /*host*/, int32_t value);
+int32_t sm_get_option(const char *name /*host*/, int32_t *value /*host*/);
+int32_t sm_build_info(void);
+
+/* Reason code of the last device-side protocol failure (a kernel whose internal barrier never completed writes
+ * the code to a pinned host word and traps; the CUDA error that follows is sticky, the code stays readable).
+ * 0 = none.  host.  The 64-byte pinned word is the one allocation the library makes (host memory, on first use). */
+int32_t sm_last_device_error(void);
 
 /* Number of kernels this thread's library calls have launched so far (bench bookkeeping). host. */
 int64_t sm_launch_count(void);

@@ -32,13 +32,16 @@ SCALES = {"none": SM_SCALE_NONE, "gershgorin": SM_SCALE_GERSHGORIN, "power": SM_
 EXPORTS = ["sm_last_cuda_error", "sm_pattern_sizes", "sm_build_pattern", "sm_plan_columns",
            "sm_gather_ws_bytes", "sm_gather", "sm_sign_ws_bytes", "sm_sign_ns", "sm_sign_status",
            "sm_scatter", "sm_symmetrise", "sm_density_ws_bytes", "sm_density", "sm_density_from_sign",
-           "sm_mu_search", "sm_launch_count", "sm_profile_enable", "sm_profile_read"]
+           "sm_mu_search", "sm_launch_count", "sm_profile_enable", "sm_profile_read", "sm_sign_ws_bytes_ex",
+           "sm_sign_ns_ex", "sm_set_option", "sm_get_option", "sm_build_info", "sm_last_device_error"]
+SM_SIGN_NONSYMMETRIC = 1
 
 
 class SmError(RuntimeError):
     def __init__(self, fn, status):
         self.status = status
-        extra = f" (cuda error {_lib.sm_last_cuda_error()})" if status == SM_ERR_CUDA else ""
+        extra = (f" (cuda error {_lib.sm_last_cuda_error()}, device protocol code {_lib.sm_last_device_error()})"
+                 if status == SM_ERR_CUDA else "")
         super().__init__(f"{fn} returned status {status}{extra}")
 
 
@@ -64,6 +67,7 @@ class _Pattern(C.Structure):
 _lib.sm_launch_count.restype = C.c_int64
 _lib.sm_gather_ws_bytes.restype = C.c_int64
 _lib.sm_sign_ws_bytes.restype = C.c_int64
+_lib.sm_sign_ws_bytes_ex.restype = C.c_int64
 _lib.sm_density_ws_bytes.restype = C.c_int64
 
 
@@ -79,6 +83,24 @@ def _check(fn, status, allow_warn=False):
     if status < 0 or (status > 0 and not allow_warn):
         raise SmError(fn, status)
     return status
+
+
+def set_option(name: str, value: int) -> None:
+    _check("sm_set_option", _lib.sm_set_option(C.c_char_p(name.encode()), C.c_int32(int(value))))
+
+
+def get_option(name: str) -> int:
+    v = C.c_int32(0)
+    _check("sm_get_option", _lib.sm_get_option(C.c_char_p(name.encode()), C.byref(v)))
+    return int(v.value)
+
+
+def build_info() -> int:
+    return int(_lib.sm_build_info())
+
+
+def last_device_error() -> int:
+    return int(_lib.sm_last_device_error())
 
 
 def launch_count() -> int:
@@ -211,27 +233,39 @@ def sm_gather(A: Bcsr, P: Pattern, cols, col_off, n_cols, mu, scale_mode, x_dtyp
     return X, scale
 
 
-def sm_sign_ws_bytes(P: Pattern, n_cols, n_elems, x_dtype) -> int:
+def sm_sign_ws_bytes(P: Pattern, n_cols, n_elems, x_dtype, flags=0) -> int:
     x_dt = DTYPES[x_dtype] if isinstance(x_dtype, str) else x_dtype
-    b = int(_lib.sm_sign_ws_bytes(C.byref(P.c), C.c_int32(n_cols), C.c_int64(n_elems), C.c_int32(x_dt)))
+    if flags:
+        b = int(_lib.sm_sign_ws_bytes_ex(C.byref(P.c), C.c_int32(n_cols), C.c_int64(n_elems), C.c_int32(x_dt),
+                                         C.c_int32(flags)))
+    else:
+        b = int(_lib.sm_sign_ws_bytes(C.byref(P.c), C.c_int32(n_cols), C.c_int64(n_elems), C.c_int32(x_dt)))
     if b < 0:
         raise SmError("sm_sign_ws_bytes", b)
     return b
 
 
 def sm_sign_ns(P: Pattern, cols, col_off, n_cols, n_elems, x_dtype, X, max_iter, tol, ws=None,
-               iters=None, residual=None):
+               iters=None, residual=None, flags=0, switch_iter=-1):
+    """flags / switch_iter non-default: sm_sign_ns_ex (non-symmetric matrices, bf16 -> fp16 schedule)."""
     x_dt = DTYPES[x_dtype] if isinstance(x_dtype, str) else x_dtype
     if ws is None:
-        ws = torch.empty(sm_sign_ws_bytes(P, n_cols, n_elems, x_dt), dtype=torch.uint8, device=P.device)
+        ws = torch.empty(sm_sign_ws_bytes(P, n_cols, n_elems, x_dt, flags), dtype=torch.uint8, device=P.device)
     if iters is None:
         iters = torch.empty(n_cols, dtype=torch.int32, device=P.device)
     if residual is None:
         residual = torch.empty(n_cols, dtype=torch.float64, device=P.device)
-    _check("sm_sign_ns", _lib.sm_sign_ns(C.byref(P.c), _ptr(cols), C.c_int32(n_cols), _ptr(col_off),
-                                         C.c_int64(n_elems), C.c_int32(x_dt), _ptr(X), _ptr(ws),
-                                         C.c_int64(ws.numel()), C.c_int32(max_iter), C.c_double(tol),
-                                         _ptr(iters), _ptr(residual), _stream()))
+    if flags or switch_iter >= 0:
+        _check("sm_sign_ns_ex", _lib.sm_sign_ns_ex(C.byref(P.c), _ptr(cols), C.c_int32(n_cols), _ptr(col_off),
+                                                   C.c_int64(n_elems), C.c_int32(x_dt), _ptr(X), _ptr(ws),
+                                                   C.c_int64(ws.numel()), C.c_int32(max_iter), C.c_double(tol),
+                                                   C.c_int32(flags), C.c_int32(switch_iter),
+                                                   _ptr(iters), _ptr(residual), _stream()))
+    else:
+        _check("sm_sign_ns", _lib.sm_sign_ns(C.byref(P.c), _ptr(cols), C.c_int32(n_cols), _ptr(col_off),
+                                             C.c_int64(n_elems), C.c_int32(x_dt), _ptr(X), _ptr(ws),
+                                             C.c_int64(ws.numel()), C.c_int32(max_iter), C.c_double(tol),
+                                             _ptr(iters), _ptr(residual), _stream()))
     return iters, residual
 
 

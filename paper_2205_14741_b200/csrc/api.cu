@@ -1,7 +1,11 @@
 // C-ABI entry points that dispatch or compose: sm_sign_ns (a3) and sm_density (a5, the whole path
 // gather -> sign -> scatter -> D = 1/2 (I - R), PAPER.md:110 steps 1-3 + PAPER.md:91 Eq. 14, S = I).
 #include <algorithm>
+#include <atomic>
 #include <cmath>
+#include <cstdlib>
+#include <cstring>
+#include <mutex>
 #include <numeric>
 #include <utility>
 #include <vector>
@@ -11,6 +15,48 @@
 using namespace sm;
 
 namespace sm {
+// ---- variant selection: one table, filled once from the environment, changed by sm_set_option ---------------
+struct OptDef { const char *name, *env; int32_t def; };
+static const OptDef kOpt[OPT_COUNT] = {
+    {"umma.sym", "SM_UMMA_SYM", 1},           {"umma.dyn", "SM_UMMA_DYN", 1},     {"umma.rev", "SM_UMMA_REV", 1},
+    {"umma.stages", "SM_UMMA_STAGES", 0},     {"umma.stream", "SM_UMMA_STREAM", 0}, {"umma.resident", "SM_UMMA_RESIDENT", 1},
+    {"umma.lt", "SM_UMMA_LT", 0},             {"f64.simt", "SM_F64_SIMT", 0},     {"gather.tma", "SM_GATHER_TMA", 1},
+    {"umma.ncta", "SM_UMMA_NCTA", 1},         {"umma.mc", "SM_UMMA_MC", 1},       {"umma.tmap", "SM_UMMA_TMAP", 0},
+    {"umma.fused", "SM_UMMA_FUSED", 0},       {"umma.slots", "SM_UMMA_SLOTS", 2}, {"umma.dbg", "SM_UMMA_DBG", 0}};
+#ifdef SM_MEASURE
+static constexpr int kOptUsable = OPT_COUNT;
+#else
+static constexpr int kOptUsable = OPT_FIRST_MEASURE;      // measurement-only knobs do not exist in this build
+#endif
+static std::atomic<int32_t> g_opt[OPT_COUNT];
+static std::once_flag g_opt_once;
+static void opt_init() {
+  for (int i = 0; i < OPT_COUNT; ++i) {
+    int32_t v = kOpt[i].def;
+    if (i < kOptUsable) { const char *e = getenv(kOpt[i].env); if (e && *e) v = atoi(e); }
+    g_opt[i].store(v, std::memory_order_relaxed);
+  }
+}
+int32_t opt(int id) {
+  std::call_once(g_opt_once, opt_init);
+  return g_opt[id].load(std::memory_order_relaxed);
+}
+
+// ---- device-side protocol failures: the kernels write a reason code into one pinned, device-mapped host word
+// before they trap, so the code survives the sticky context error (sm_last_device_error).
+static std::mutex g_err_mu;
+static int32_t *g_err_word = nullptr;
+int32_t *device_err_word() {
+  std::lock_guard<std::mutex> lk(g_err_mu);
+  if (!g_err_word) {
+    void *p = nullptr;
+    if (cudaHostAlloc(&p, 64, cudaHostAllocMapped | cudaHostAllocPortable) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+    std::memset(p, 0, 64);
+    g_err_word = (int32_t *)p;
+  }
+  return g_err_word;
+}
+
 // Optional per-launch timing of the dominant kernels (bench.py roofline): CUDA events recorded on the
 // launching stream around every Newton-Schulz product launch while profiling is enabled.
 struct GemmProfile {
@@ -45,29 +91,76 @@ static __global__ void k_count_unconverged(int32_t n, const double *__restrict__
 }
 }  // namespace sm
 
-extern "C" int64_t sm_sign_ws_bytes(const sm_pattern_t *P, int32_t n_cols, int64_t packed_elems,
-                                    int32_t x_dtype) {
+extern "C" int32_t sm_set_option(const char *name, int32_t value) {
+  if (!name) return SM_ERR_ARG;
+  for (int i = 0; i < OPT_COUNT; ++i)
+    if (!strcmp(name, kOpt[i].name)) {
+      if (i >= kOptUsable) return SM_ERR_UNSUPPORTED;
+      (void)opt(i);
+      g_opt[i].store(value, std::memory_order_relaxed);
+      return SM_OK;
+    }
+  return SM_ERR_ARG;
+}
+extern "C" int32_t sm_get_option(const char *name, int32_t *value) {
+  if (!name || !value) return SM_ERR_ARG;
+  for (int i = 0; i < OPT_COUNT; ++i)
+    if (!strcmp(name, kOpt[i].name)) {
+      if (i >= kOptUsable) return SM_ERR_UNSUPPORTED;
+      *value = opt(i);
+      return SM_OK;
+    }
+  return SM_ERR_ARG;
+}
+extern "C" int32_t sm_build_info(void) {
+#ifdef SM_MEASURE
+  return 1;
+#else
+  return 0;
+#endif
+}
+extern "C" int32_t sm_last_device_error(void) {
+  std::lock_guard<std::mutex> lk(g_err_mu);
+  return g_err_word ? *(volatile int32_t *)g_err_word : 0;
+}
+
+extern "C" int64_t sm_sign_ws_bytes_ex(const sm_pattern_t *P, int32_t n_cols, int64_t packed_elems,
+                                       int32_t x_dtype, int32_t flags) {
   if (!P || n_cols <= 0 || packed_elems <= 0) return SM_ERR_ARG;
-  if (is_16bit(x_dtype)) return sign_umma_ws_bytes(P, n_cols, packed_elems, x_dtype);
+  if (is_16bit(x_dtype)) return sign_umma_ws_bytes(P, n_cols, packed_elems, x_dtype, flags & SM_SIGN_NONSYMMETRIC);
   if (x_dtype == SM_F32 || x_dtype == SM_F64) return sign_simt_ws_bytes(P, n_cols, packed_elems, x_dtype);
   return SM_ERR_UNSUPPORTED;
 }
+extern "C" int64_t sm_sign_ws_bytes(const sm_pattern_t *P, int32_t n_cols, int64_t packed_elems,
+                                    int32_t x_dtype) {
+  return sm_sign_ws_bytes_ex(P, n_cols, packed_elems, x_dtype, 0);
+}
 
+extern "C" int32_t sm_sign_ns_ex(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols,
+                                 const int64_t *col_off, int64_t packed_elems, int32_t x_dtype, void *X_packed,
+                                 void *ws, int64_t ws_bytes, int32_t max_iter, double tol, int32_t flags,
+                                 int32_t switch_iter, int32_t *iters, double *residual, void *stream) {
+  if (!P || !col_off || !X_packed || !ws || !iters || !residual) return SM_ERR_ARG;
+  if (!cols) n_cols = P->n_blk;
+  if (n_cols <= 0 || max_iter < 0 || packed_elems <= 0) return SM_ERR_ARG;
+  if (flags & ~SM_SIGN_NONSYMMETRIC) return SM_ERR_ARG;
+  cudaStream_t st = (cudaStream_t)stream;
+  const int32_t nonsym = flags & SM_SIGN_NONSYMMETRIC;
+  if (is_16bit(x_dtype))
+    return sign_umma(P, cols, n_cols, col_off, packed_elems, x_dtype, X_packed, ws, ws_bytes, max_iter, tol,
+                     iters, residual, nonsym, switch_iter, st);
+  if (switch_iter >= 0) return SM_ERR_ARG;
+  if (x_dtype == SM_F32 || x_dtype == SM_F64)
+    return sign_simt(P, cols, n_cols, col_off, packed_elems, x_dtype, X_packed, ws, ws_bytes, max_iter, tol,
+                     iters, residual, nonsym, st);
+  return SM_ERR_UNSUPPORTED;
+}
 extern "C" int32_t sm_sign_ns(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols,
                               const int64_t *col_off, int64_t packed_elems, int32_t x_dtype, void *X_packed,
                               void *ws, int64_t ws_bytes, int32_t max_iter, double tol, int32_t *iters,
                               double *residual, void *stream) {
-  if (!P || !col_off || !X_packed || !ws || !iters || !residual) return SM_ERR_ARG;
-  if (!cols) n_cols = P->n_blk;
-  if (n_cols <= 0 || max_iter < 0 || packed_elems <= 0) return SM_ERR_ARG;
-  cudaStream_t st = (cudaStream_t)stream;
-  if (is_16bit(x_dtype))
-    return sign_umma(P, cols, n_cols, col_off, packed_elems, x_dtype, X_packed, ws, ws_bytes, max_iter, tol,
-                     iters, residual, st);
-  if (x_dtype == SM_F32 || x_dtype == SM_F64)
-    return sign_simt(P, cols, n_cols, col_off, packed_elems, x_dtype, X_packed, ws, ws_bytes, max_iter, tol,
-                     iters, residual, st);
-  return SM_ERR_UNSUPPORTED;
+  return sm_sign_ns_ex(P, cols, n_cols, col_off, packed_elems, x_dtype, X_packed, ws, ws_bytes, max_iter, tol, 0, -1,
+                       iters, residual, stream);
 }
 
 extern "C" int32_t sm_sign_status(const double *residual, int32_t n_cols, double tol, void *scratch,

@@ -114,13 +114,27 @@ int32_t global_scale(const sm_bcsr_t *A, const void *A_vals, int32_t a_dtype, co
                      int32_t n_cols, double *scale, void *ws, int64_t ws_bytes, cudaStream_t st);
 int32_t power_scale(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, const int64_t *col_off,
                     int32_t x_dtype, void *X, double *scale, double *ratio, cudaStream_t st);  // power_scale.cu
+// nonsym: the iterates are NOT symmetric (true products X X, X Y on every tile; sm_sign_ns_ex SM_SIGN_NONSYMMETRIC);
+// switch_iter >= 0: bf16 -> fp16 precision schedule (16-bit only)
 int32_t sign_simt(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, const int64_t *col_off,
                   int64_t packed_elems, int32_t x_dtype, void *X, void *ws, int64_t ws_bytes,
-                  int32_t max_iter, double tol, int32_t *iters, double *residual, cudaStream_t st);
+                  int32_t max_iter, double tol, int32_t *iters, double *residual, int32_t nonsym, cudaStream_t st);
 int32_t sign_umma(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, const int64_t *col_off,
                   int64_t packed_elems, int32_t x_dtype, void *X, void *ws, int64_t ws_bytes,
-                  int32_t max_iter, double tol, int32_t *iters, double *residual, cudaStream_t st);
+                  int32_t max_iter, double tol, int32_t *iters, double *residual, int32_t nonsym, int32_t switch_iter,
+                  cudaStream_t st);
 int64_t sign_simt_ws_bytes(const sm_pattern_t *P, int32_t n_cols, int64_t packed_elems, int32_t x_dtype);
-int64_t sign_umma_ws_bytes(const sm_pattern_t *P, int32_t n_cols, int64_t packed_elems, int32_t x_dtype);
+int64_t sign_umma_ws_bytes(const sm_pattern_t *P, int32_t n_cols, int64_t packed_elems, int32_t x_dtype, int32_t nonsym);
+int32_t *device_err_word();        // pinned, device-mapped host word the kernels write a protocol-failure code to (api.cu)
+
+// ---- variant selection (api.cu): sm_set_option / environment at first use.  Ids are indices into the table there.
+enum OptId {
+  OPT_UMMA_SYM = 0, OPT_UMMA_DYN, OPT_UMMA_REV, OPT_UMMA_STAGES, OPT_UMMA_STREAM, OPT_UMMA_RESIDENT, OPT_UMMA_LT,
+  OPT_F64_SIMT, OPT_GATHER_TMA,
+  OPT_FIRST_MEASURE,                 // the ones below exist only in a -DSM_MEASURE build
+  OPT_UMMA_NCTA = OPT_FIRST_MEASURE, OPT_UMMA_MC, OPT_UMMA_TMAP, OPT_UMMA_FUSED, OPT_UMMA_SLOTS, OPT_UMMA_DBG,
+  OPT_COUNT
+};
+int32_t opt(int id);
 
 }  // namespace sm

@@ -1,8 +1,6 @@
 // a3, fp32 / fp64 back end: Newton-Schulz X <- 1/2 X (3I - X^2) on row-major packed submatrices
 // with FFMA / DFMA register-tiled products (tcgen05 has no fp32/fp64 kind).  PAPER.md:87 (Eq. 13),
 // :110 (step 2); iteration and stopping rule: DESIGN.md readings A9, A11.
-#include <cstdlib>
-
 #include "sign_state.cuh"
 
 namespace sm {
@@ -146,7 +144,7 @@ __device__ __forceinline__ void cp_async16(void *smem, const void *gmem, bool va
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(sa), "l"(gmem), "r"(n) : "memory");
 }
 
-template <int PHASE>
+template <int PHASE, bool SYM>
 __global__ void __launch_bounds__(256)
 k_dmma_gemm(const int32_t *__restrict__ cols, const int64_t *__restrict__ col_off,
             const int32_t *__restrict__ dim, const int32_t *__restrict__ dim_pad, int32_t max_tiles_edge,
@@ -161,7 +159,7 @@ k_dmma_gemm(const int32_t *__restrict__ cols, const int64_t *__restrict__ col_of
   const int32_t m = dim[i], Pd = dim_pad[i];
   const int32_t te = (m + DT - 1) / DT;
   const int32_t tr = t / max_tiles_edge, tc = t - tr * max_tiles_edge;
-  if (tr >= te || tc > tr) return;                            // lower-triangle tiles only
+  if (tr >= te || tc >= te || (SYM && tc > tr)) return;       // SYM: lower-triangle tiles only
   const double *A = Xsrc + col_off[c];
   const double *B = (PHASE == 1 ? Xsrc : Ybuf) + col_off[c];
   double *O = Out + col_off[c];
@@ -225,7 +223,7 @@ k_dmma_gemm(const int32_t *__restrict__ cols, const int64_t *__restrict__ col_of
     __syncthreads();
   }
 
-  // epilogue: lane holds C[row = g][cols 2q, 2q+1] of every 8 x 8 accumulator.  X is symmetric and so are
+  // epilogue: lane holds C[row = g][cols 2q, 2q+1] of every 8 x 8 accumulator.  SYM: X is symmetric and so are
   // Y = X X and X' = p(X): only tiles with tc <= tr are computed, an element (r, c <= r) is stored at
   // (r, c) and mirrored to (c, r), which keeps the iterates exactly symmetric; off-diagonal elements
   // count twice in the residual.
@@ -238,16 +236,16 @@ k_dmma_gemm(const int32_t *__restrict__ cols, const int64_t *__restrict__ col_of
 #pragma unroll
       for (int e = 0; e < 2; ++e) {
         const int32_t gc = col0 + wc + b * 8 + 2 * q + e;
-        if (gr < m && gc <= gr) {
+        if (gr < m && (SYM ? gc <= gr : gc < m)) {
           double val = acc[a][b][e];
           if (PHASE == 1) {
             const double d = val - (gr == gc ? 1.0 : 0.0);
-            res += (gr == gc ? 1.0 : 2.0) * d * d;
+            res += ((!SYM || gr == gc) ? 1.0 : 2.0) * d * d;
           } else {
             val = 1.5 * A[(int64_t)gr * Pd + gc] - 0.5 * val;
           }
           O[(int64_t)gr * Pd + gc] = val;
-          if (gc < gr) O[(int64_t)gc * Pd + gr] = val;
+          if (SYM && gc < gr) O[(int64_t)gc * Pd + gr] = val;
         }
       }
     }
@@ -302,18 +300,13 @@ int64_t sign_simt_ws_bytes(const sm_pattern_t *P, int32_t n_cols, int64_t packed
 template <typename T>
 static int32_t sign_simt_t(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, const int64_t *col_off,
                            int64_t packed_elems, T *X, void *ws, int64_t ws_bytes, int32_t max_iter,
-                           double tol, int32_t *iters, double *residual, cudaStream_t st) {
+                           double tol, int32_t *iters, double *residual, int32_t nonsym, cudaStream_t st) {
   if ((P->pad_to & 3) != 0) return SM_ERR_ARG;   // 16-byte alignment of every submatrix
   SimtWs w = simt_layout(ws, ws_bytes, P, n_cols, packed_elems, (int32_t)sizeof(T));
   if (w.used > ws_bytes) return SM_ERR_SPACE;
   SignState s{w.active, w.last, w.n_still, w.partial, w.parts_per_col};
-  // fp64: DMMA tensor-core tiles of 128 x 128 unless the submatrices are tiny (or SM_F64_BACKEND=simt)
-  static int32_t env_simt = -1;
-  if (env_simt < 0) {
-    const char *e = getenv("SM_F64_BACKEND");
-    env_simt = (e && e[0] == 's') ? 1 : 0;
-  }
-  const bool dmma = sizeof(T) == 8 && !env_simt && P->max_dim > 96;
+  // fp64: DMMA tensor-core tiles of 128 x 128 unless the submatrices are tiny (or option f64.simt = 1)
+  const bool dmma = sizeof(T) == 8 && opt(OPT_F64_SIMT) == 0 && P->max_dim > 96;
   const int32_t TS = dmma ? DT : ST;
   const int32_t edge = (P->max_dim + TS - 1) / TS;
   const int64_t grid64 = (int64_t)n_cols * edge * edge;
@@ -324,12 +317,11 @@ static int32_t sign_simt_t(const sm_pattern_t *P, const int32_t *cols, int32_t n
   k_tile_nparts<<<nb, 256, 0, st>>>(n_cols, TS, cols, P->dim, w.n_parts);
   SM_LAUNCHED();
   if (dmma) {
-    static bool configured = false;
-    if (!configured) {
-      SM_CUDA(cudaFuncSetAttribute(k_dmma_gemm<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, DMMA_SMEM));
-      SM_CUDA(cudaFuncSetAttribute(k_dmma_gemm<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, DMMA_SMEM));
-      configured = true;
-    }
+    // per device attribute: set on every call (a process may use several devices)
+    SM_CUDA(cudaFuncSetAttribute(k_dmma_gemm<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, DMMA_SMEM));
+    SM_CUDA(cudaFuncSetAttribute(k_dmma_gemm<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, DMMA_SMEM));
+    SM_CUDA(cudaFuncSetAttribute(k_dmma_gemm<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, DMMA_SMEM));
+    SM_CUDA(cudaFuncSetAttribute(k_dmma_gemm<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, DMMA_SMEM));
     // padding of Y and of the alternate X buffer must read as zeros (the kernel stores true elements only)
     SM_CUDA(cudaMemsetAsync(w.Y, 0, packed_elems * sizeof(T), st));
     SM_CUDA(cudaMemsetAsync(w.X2, 0, packed_elems * sizeof(T), st));
@@ -342,9 +334,12 @@ static int32_t sign_simt_t(const sm_pattern_t *P, const int32_t *cols, int32_t n
     T *src = buf[k & 1], *dst = buf[(k + 1) & 1];
     int slot = -1;
     { int32_t rc = prof_begin(st, &slot); if (rc != SM_OK) return rc; }
-    if (dmma)
-      k_dmma_gemm<1><<<grid, 256, DMMA_SMEM, st>>>(cols, col_off, P->dim, P->dim_pad, edge, (const double *)src,
-                                                   (const double *)Y, (double *)Y, s);
+    if (dmma && nonsym)
+      k_dmma_gemm<1, false><<<grid, 256, DMMA_SMEM, st>>>(cols, col_off, P->dim, P->dim_pad, edge, (const double *)src,
+                                                          (const double *)Y, (double *)Y, s);
+    else if (dmma)
+      k_dmma_gemm<1, true><<<grid, 256, DMMA_SMEM, st>>>(cols, col_off, P->dim, P->dim_pad, edge, (const double *)src,
+                                                         (const double *)Y, (double *)Y, s);
     else
       k_simt_gemm<T, 1><<<grid, 256, 0, st>>>(cols, col_off, P->dim, P->dim_pad, edge, src, Y, Y, s);
     SM_LAUNCHED();
@@ -353,9 +348,12 @@ static int32_t sign_simt_t(const sm_pattern_t *P, const int32_t *cols, int32_t n
     k_sign_post<<<(n_cols + 7) / 8, 256, 0, st>>>(n_cols, cols, P->dim, s, w.n_parts, tol, iters, residual);
     SM_LAUNCHED();
     { int32_t rc = prof_begin(st, &slot); if (rc != SM_OK) return rc; }
-    if (dmma)
-      k_dmma_gemm<2><<<grid, 256, DMMA_SMEM, st>>>(cols, col_off, P->dim, P->dim_pad, edge, (const double *)src,
-                                                   (const double *)Y, (double *)dst, s);
+    if (dmma && nonsym)
+      k_dmma_gemm<2, false><<<grid, 256, DMMA_SMEM, st>>>(cols, col_off, P->dim, P->dim_pad, edge, (const double *)src,
+                                                          (const double *)Y, (double *)dst, s);
+    else if (dmma)
+      k_dmma_gemm<2, true><<<grid, 256, DMMA_SMEM, st>>>(cols, col_off, P->dim, P->dim_pad, edge, (const double *)src,
+                                                         (const double *)Y, (double *)dst, s);
     else
       k_simt_gemm<T, 2><<<grid, 256, 0, st>>>(cols, col_off, P->dim, P->dim_pad, edge, src, Y, dst, s);
     SM_LAUNCHED();
@@ -369,20 +367,20 @@ static int32_t sign_simt_t(const sm_pattern_t *P, const int32_t *cols, int32_t n
     }
   }
   dim3 cg(n_cols, 8);
-  k_copy_back<<<cg, 256, 0, st>>>(cols, col_off, iters, (int32_t)sizeof(T), (const char *)w.X2, (char *)X);
+  k_copy_back<<<cg, 256, 0, st>>>(cols, col_off, iters, (int32_t)sizeof(T), P->dim_pad, 0, (const char *)w.X2, (char *)X);
   SM_LAUNCHED();
   return SM_OK;
 }
 
 int32_t sign_simt(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, const int64_t *col_off,
                   int64_t packed_elems, int32_t x_dtype, void *X, void *ws, int64_t ws_bytes,
-                  int32_t max_iter, double tol, int32_t *iters, double *residual, cudaStream_t st) {
+                  int32_t max_iter, double tol, int32_t *iters, double *residual, int32_t nonsym, cudaStream_t st) {
   if (x_dtype == SM_F64)
     return sign_simt_t<double>(P, cols, n_cols, col_off, packed_elems, (double *)X, ws, ws_bytes, max_iter,
-                               tol, iters, residual, st);
+                               tol, iters, residual, nonsym, st);
   if (x_dtype == SM_F32)
     return sign_simt_t<float>(P, cols, n_cols, col_off, packed_elems, (float *)X, ws, ws_bytes, max_iter,
-                              tol, iters, residual, st);
+                              tol, iters, residual, nonsym, st);
   return SM_ERR_UNSUPPORTED;
 }
 

@@ -56,9 +56,11 @@ static __global__ void k_sign_post(int32_t n_cols, const int32_t *__restrict__ c
 // alternate buffer; copy it back (whole padded image, 16-byte vectors).
 static __global__ void k_copy_back(const int32_t *__restrict__ cols, const int64_t *__restrict__ col_off,
                                    const int32_t *__restrict__ iters, int32_t elem_bytes,
+                                   const int32_t *__restrict__ dim_pad, int32_t skip_pd,
                                    const char *__restrict__ alt, char *__restrict__ X) {
   int32_t c = blockIdx.x;
   if ((iters[c] & 1) == 0) return;
+  if (skip_pd > 0 && dim_pad[cols ? cols[c] : c] <= skip_pd) return;   // iterated in place by another kernel
   int64_t b0 = col_off[c] * elem_bytes, b1 = col_off[c + 1] * elem_bytes;
   int64_t n16 = (b1 - b0) >> 4;
   const uint4 *src = reinterpret_cast<const uint4 *>(alt + b0);

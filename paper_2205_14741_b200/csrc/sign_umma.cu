@@ -28,6 +28,14 @@
 #include "sign_state.cuh"
 #include "umma_ptx.cuh"
 
+// Measurement-only skip knobs (wrong results by construction) exist only in a -DSM_MEASURE build
+// (build.py --measure); the default library has no such path.
+#ifdef SM_MEASURE
+#define SM_DBG(a, bit) ((a).dbg & (bit))
+#else
+#define SM_DBG(a, bit) 0
+#endif
+
 namespace sm {
 
 constexpr int UM = 128;          // tile rows per CTA (UMMA M per CTA)
@@ -156,7 +164,7 @@ __device__ __forceinline__ UTile make_tile(const UArgs &a, const TileDesc &d) {
   return u;
 }
 
-static __global__ void k_umma_build_tiles(int32_t n_cols, int32_t R, int32_t sym, const int32_t *__restrict__ cols,
+static __global__ void k_umma_build_tiles(int32_t n_cols, int32_t R, int32_t sym, int32_t skip_pd, const int32_t *__restrict__ cols,
                                           const int32_t *__restrict__ dim, const int32_t *__restrict__ dim_pad,
                                           const int64_t *__restrict__ col_off,
                                           const int64_t *__restrict__ tile_ptr, TileDesc *__restrict__ tiles) {
@@ -164,6 +172,7 @@ static __global__ void k_umma_build_tiles(int32_t n_cols, int32_t R, int32_t sym
   if (c >= n_cols) return;
   int32_t i = cols ? cols[c] : c;
   int32_t m = dim[i], Pd = dim_pad[i];
+  if (Pd <= skip_pd) return;                      // taken by the resident kernel: no tiles
   TileDesc d;
   d.base = col_off[c]; d.c = c; d.m = m; d.Pd = Pd; d.pad0 = d.pad1 = d.pad2 = 0;
   int64_t t = tile_ptr[c];
@@ -382,7 +391,7 @@ k_umma_gemm(UArgs a, const __grid_constant__ CUtensorMap mapA, const __grid_cons
           if (++qs == TQ) { qs = 0; qp ^= 1u; }
           if (cur.c < 0) return false;
           t = (int64_t)atomicAdd(a.counter, 1ULL);  // its latency overlaps this tile's loads
-          if (STREAM && cur.pad0 > 0 && !(a.dbg & 64)) {
+          if (STREAM && cur.pad0 > 0 && !SM_DBG(a, 64)) {
             // the previous product of this group (written by other CTAs) must be complete and visible to the bulk copies
             const volatile int32_t *flag = a.done + (int64_t)cur.pad1 * a.n_ph + (cur.pad0 - 1);
             for (uint32_t spin = 0; *flag < cur.pad2; ++spin) {
@@ -441,7 +450,7 @@ k_umma_gemm(UArgs a, const __grid_constant__ CUtensorMap mapA, const __grid_cons
         for (int kc = 0; kc < nkc; ++kc) {
           ptx::mbar_wait(empty_bar(stage), phase ^ 1u, a.err_flag, 1);
           const uint32_t sa = tiles + stage * STAGE_BYTES, sb = sa + A_BYTES;
-          if (a.dbg & 4) {
+          if (SM_DBG(a, 4)) {
             ptx::mbar_arrive(full_bar(stage));
             if (++stage == USTAGES) { stage = 0; phase ^= 1u; }
             continue;
@@ -522,7 +531,7 @@ k_umma_gemm(UArgs a, const __grid_constant__ CUtensorMap mapA, const __grid_cons
           const uint64_t bdesc = SYM ? ptx::make_sw128_kmajor_desc(sb) : ptx::make_sw128_mnmajor_desc(sb, 8192u, 1024u);
           const uint64_t bstep = SYM ? 2u : 128u;   // 16 k: 32 B inside a K-major atom / 16 rows of 128 B
           const int ksteps = min(UK / 16, (u.kmax - kc * UK) / 16);
-          for (int ks = 0; ks < ((a.dbg & 2) ? 0 : ksteps); ++ks) {
+          for (int ks = 0; ks < (SM_DBG(a, 2) ? 0 : ksteps); ++ks) {
             // advance 16 elements = 32 bytes inside the swizzle atom: +2 in the (addr >> 4) field
             if (PAIR)
               ptx::umma_f16_2cta(d_tmem, adesc + (uint64_t)(2 * ks), bdesc + bstep * (uint64_t)ks, idesc,
@@ -531,7 +540,7 @@ k_umma_gemm(UArgs a, const __grid_constant__ CUtensorMap mapA, const __grid_cons
               ptx::umma_f16(d_tmem, adesc + (uint64_t)(2 * ks), bdesc + bstep * (uint64_t)ks, idesc,
                             (uint32_t)((kc | ks) != 0));
           }
-          if ((STREAM ? (cur.pad0 & 1) != 0 : PHASE == 2) && !(a.dbg & 2)) {
+          if ((STREAM ? (cur.pad0 & 1) != 0 : PHASE == 2) && !SM_DBG(a, 2)) {
             // "+ X": the A chunk in this stage holds X[rows, 64 kc .. 64 kc + 63]; add it to the accumulator
             // columns [lo, hi) of the tile that it covers (B = identity slice, K-major)
             const int32_t lo = max(kc * UK, u.n0), hi = min(kc * UK + UK, u.n0 + u.nt);
@@ -599,13 +608,13 @@ k_umma_gemm(UArgs a, const __grid_constant__ CUtensorMap mapA, const __grid_cons
       const bool p1 = STREAM ? (cur.pad0 & 1) == 0 : PHASE == 1;
       // stream: product ph of step ph / 2 writes Wh (even ph) or the X buffer that step does not read (odd ph)
       uint16_t *Og = (uint16_t *)(!STREAM ? a.Out : p1 ? a.Ybuf : (((cur.pad0 >> 1) & 1) ? (void *)a.Xsrc : a.Out)) + u.base;
-      if (a.dbg & 1) Og = nullptr;
+      if (SM_DBG(a, 1)) Og = nullptr;
       const int nblk = (u.nt + 31) >> 5;
       ptx::mbar_wait(tfull_bar(as), aphase, a.err_flag, 4);
       ptx::tc_fence_after();
       const uint32_t taddr = tmem_base + as * UN + ((uint32_t)(q * 32) << 16);
       float res = 0.f, res2 = 0.f;                             // diagonal-block / off-diagonal (counted twice) sums
-      if (R0 < u.Pd && !(a.dbg & 8)) {
+      if (R0 < u.Pd && !SM_DBG(a, 8)) {
         const uint32_t r7 = (uint32_t)lane & 7u;                 // r & 7 (R0 is a multiple of 32)
         for (int bi = sub; bi < nblk; bi += NSUB) {
           const int32_t C0 = u.n0 + bi * 32;
@@ -700,7 +709,7 @@ k_umma_gemm(UArgs a, const __grid_constant__ CUtensorMap mapA, const __grid_cons
           a.s.partial[(int64_t)u.c * a.s.parts_per_col + (int64_t)u.lt * (EPI_WARPS * NCTA) + (int64_t)h * EPI_WARPS +
                       (warp - 2)] = (double)res;
       }
-      if (STREAM && cur.pad0 + 1 < a.n_ph && !(a.dbg & 128)) {
+      if (STREAM && cur.pad0 + 1 < a.n_ph && !SM_DBG(a, 128)) {
         // this warp's stores of the tile: visible gpu-wide and to the async proxy, then counted for the group's product
         __threadfence();
         ptx::fence_proxy_async();
@@ -721,132 +730,114 @@ k_umma_gemm(UArgs a, const __grid_constant__ CUtensorMap mapA, const __grid_cons
 }
 
 
+#ifdef SM_MEASURE
 #include "sign_umma_fused.cuh"
+#endif
+#include "sign_resident.cuh"
 
-// Fixed-iteration bookkeeping after k_umma_fused: residual of the last step from its partial sums (one
-// warp per listed column, fixed order), iters = max_iter.
+// Fixed-iteration bookkeeping of the grouped path: residual of the last step from its partial sums (one warp per
+// listed column, fixed order), iters = max_iter.  Columns with Pd <= skip_pd (shared-memory-resident kernel) are
+// not touched.
 static __global__ void k_fused_post(int32_t n_cols, const int32_t *__restrict__ cols, const int32_t *__restrict__ dim,
+                                    const int32_t *__restrict__ dim_pad, int32_t skip_pd,
                                     const double *__restrict__ partial, int32_t parts_per_col,
                                     const int32_t *__restrict__ n_parts, int32_t max_iter, int32_t *iters,
                                     double *residual) {
   const int32_t c = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
   if (c >= n_cols) return;
+  const int32_t i = cols ? cols[c] : c;
+  if (dim_pad[i] <= skip_pd) return;
   const double *p = partial + (int64_t)c * parts_per_col;
   double sum = 0.0;
   const int32_t np = n_parts[c];
   for (int32_t t = lane; t < np; t += 32) sum += p[t];
   for (int d = 16; d > 0; d >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, d);
   if (lane == 0) {
-    const int32_t i = cols ? cols[c] : c;
     residual[c] = max_iter > 0 ? sqrt(sum / (double)dim[i]) : 0.0;
     iters[c] = max_iter;
   }
 }
 
-}  // namespace sm
-
-namespace sm {
-
-static __global__ void k_umma_tilecounts(int32_t n_cols, int32_t R, int32_t sym, int32_t parts_per_tile,
+static __global__ void k_umma_tilecounts(int32_t n_cols, int32_t R, int32_t sym, int32_t parts_per_tile, int32_t skip_pd,
                                          const int32_t *__restrict__ cols, const int32_t *__restrict__ dim,
                                          const int32_t *__restrict__ dim_pad, int64_t *__restrict__ tiles,
                                          int32_t *__restrict__ n_parts) {
   int32_t c = blockIdx.x * blockDim.x + threadIdx.x;
   if (c >= n_cols) return;
   int32_t i = cols ? cols[c] : c;
-  int32_t nt = sym ? u_tiles(dim[i], R) : f_tiles(dim_pad[i], R);
+  int32_t nt = dim_pad[i] <= skip_pd ? 0 : (sym ? u_tiles(dim[i], R) : f_tiles(dim_pad[i], R));
   tiles[c] = nt;
   n_parts[c] = nt * parts_per_tile;
+}
+
+// iters / residual of the columns the resident kernel does not take start at zero; its own are written by it
+static __global__ void k_sign_init_grouped(int32_t n_cols, const int32_t *__restrict__ cols,
+                                           const int32_t *__restrict__ dim_pad, int32_t skip_pd, int32_t *active,
+                                           int32_t *last, int32_t *iters, double *residual) {
+  int32_t c = blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= n_cols) return;
+  const bool mine = dim_pad[cols ? cols[c] : c] > skip_pd;
+  active[c] = mine ? 1 : 0; last[c] = 0;
+  if (mine) { iters[c] = 0; residual[c] = 0.0; }
 }
 
 constexpr int UMMA_MAX_COUNTERS = 256;      // 2 per step; more steps than that fall back to the static deal
 struct UmmaWs {
   void *Y, *X2; int32_t *active, *last, *n_still, *n_parts, *err; int64_t *tile_ptr; double *partial;
-  unsigned long long *counters;   // one tile counter per product launch (dynamic scheduling)
+  unsigned long long *counters;   // one tile counter per product launch (dynamic scheduling) + 1 for the resident kernel
   int32_t *done;                  // stream mode: [groups][2 * steps] completion counters
   TileDesc *tiles;
   int32_t parts_per_col; int64_t used;
 };
 
-// CTAs per tile.  Measured on B200 (sm_sign_ns alone, same box): configs[4], m ~ 1650, 25 steps: single CTAs with a
-// 3-stage ring 653 ms, two CTAs with multicast 672 (3 stages) / 727 ms (4), cta_group::2 pairs with a relayed
-// stage signal 682-762 ms, single CTAs with 4 stages 747 ms; configs[2], m ~ 410, 20 steps: single CTAs 27.8 ms
-// (4 stages), two CTAs 31-32 ms.  So single CTAs are the default and the ring depth follows the size;
-// SM_UMMA_NCTA=1/2 (and SM_UMMA_MC, SM_UMMA_STAGES) in the environment override (A/B measurements, tests).
-static int32_t umma_ncta(const sm_pattern_t *P) {
-  static int32_t env = -2;
-  if (env == -2) {
-    const char *e = getenv("SM_UMMA_NCTA");
-    env = e ? (e[0] == '1' ? 1 : 2) : -1;
-  }
-  if (env > 0) return env;
-  (void)P;
-  return 1;     // measured (B200): single CTAs win at every config once the ring depth follows the size (UCfg)
+// Variant selection (sm_set_option / environment at load; include/submatrix.h lists the names).  Measured on B200
+// (sm_sign_ns alone, one box): single CTAs per tile beat every two-CTA variant (configs[4]: 603 vs 653-762 ms;
+// configs[2]: 26-28 vs 31-32 ms), SYM beats FULL at every size (configs[2]: 0.77 vs 1.13 ms per launch), the dynamic
+// deal beats round robin; the two-CTA and fused variants are therefore only in a -DSM_MEASURE build.
+static int32_t umma_ncta() {
+#ifdef SM_MEASURE
+  return opt(OPT_UMMA_NCTA) == 2 ? 2 : 1;
+#else
+  return 1;
+#endif
 }
-
-// Two-CTA tiles: cta_group::2 MMAs with a relayed "stage landed" (0) or two cta_group::1 MMAs with the B rows
-// multicast to both CTAs (1).  SM_UMMA_MC=0/1 in the environment overrides.
-static int32_t umma_mc() {
-  static int32_t env = -2;
-  if (env == -2) {
-    const char *e = getenv("SM_UMMA_MC");
-    env = e ? (e[0] == '1' ? 1 : 0) : -1;
-  }
-  return env >= 0 ? env : 1;     // measured (configs[4], B200): 654 ms (multicast) vs 690 ms (relay) for 25 steps
+static bool umma_fused(double tol) {
+#ifdef SM_MEASURE
+  return !(tol > 0.0) && opt(OPT_UMMA_FUSED) == 1;
+#else
+  (void)tol; return false;
+#endif
 }
-
-// SYM (triangular tiles, mirrored stores) for large submatrices, where the symmetric half of the MMA
-// work is worth more than the transposing epilogue costs; FULL (true products) below.  Decided per
-// call from the pattern's largest submatrix; SM_UMMA_SYM=0/1 in the environment overrides.
-static int32_t umma_sym(const sm_pattern_t *P) {
-  static int32_t env = -2;
-  if (env == -2) {
-    const char *e = getenv("SM_UMMA_SYM");
-    env = e ? (e[0] == '1' ? 1 : 0) : -1;
-  }
-  if (env >= 0) return env;
-  (void)P;
-  return 1;     // measured (configs[2], B200): SYM 0.77 ms per launch, FULL 1.13 ms
-}
-
-// Fused kernel (whole iteration per submatrix inside one launch, iterates L2-resident; fixed iteration counts
-// only).  It halves the DRAM traffic of configs[2] (ncu: 62 GB vs 130 GB for 20 steps) but is bound by its
-// epilogue's store instructions and the per-phase hand-over, and measures slower than the per-phase launches
-// (33.4 vs 26.7 ms), so it is opt-in: SM_UMMA_FUSED=1 in the environment (A/B measurements, tests).
-static int32_t umma_fused(const sm_pattern_t *P, double tol) {
-  static int32_t env = -2;
-  if (env == -2) {
-    const char *e = getenv("SM_UMMA_FUSED");
-    env = e ? (e[0] == '1' ? 1 : 0) : -1;
-  }
-  (void)P;
-  if (tol > 0.0) return 0;
-  return env > 0 ? 1 : 0;
-}
-
 static int32_t umma_dbg() {
-  const char *e = getenv("SM_UMMA_DBG");
-  return e ? atoi(e) : 0;
+#ifdef SM_MEASURE
+  return opt(OPT_UMMA_DBG);
+#else
+  return 0;
+#endif
 }
+// all listed columns with Pd <= this go through k_umma_resident (0: none)
+static int32_t umma_resident_pd(int32_t sym) { return (sym && opt(OPT_UMMA_RESIDENT) != 0) ? RES_MAX_PD : 0; }
 
 static UmmaWs umma_layout(void *ws, int64_t ws_bytes, const sm_pattern_t *P, int32_t n_cols,
-                          int64_t packed_elems) {
+                          int64_t packed_elems, int32_t sym) {
   WsCursor cur(ws, ws_bytes);
   UmmaWs w;
   // sized for whichever variant sign_umma picks (the query does not know tol): per-phase launches with
   // the selected NCTA / SYM, or the fused kernel (CTA pairs, SYM)
-  const int32_t ncta = umma_ncta(P);
-  const int32_t t_sel = umma_sym(P) ? u_tiles(P->max_dim, UM * ncta) : f_tiles(P->max_dim_pad, UM * ncta);
+  const int32_t ncta = umma_ncta();
+  const int32_t t_sel = sym ? u_tiles(P->max_dim, UM * ncta) : f_tiles(P->max_dim_pad, UM * ncta);
   const int32_t t_fused = u_tiles(P->max_dim, UM * 2);
   const int32_t max_tiles = t_sel > t_fused ? t_sel : t_fused;
   w.parts_per_col = (t_sel * ncta > t_fused * 2 ? t_sel * ncta : t_fused * 2) * EPI_WARPS;
-  w.Y = cur.take<char>(packed_elems * 2);
-  w.X2 = cur.take<char>(packed_elems * 2);
+  // when every listed column can be resident the grouped path's two image buffers are not needed
+  const bool all_res = umma_resident_pd(sym) >= P->max_dim_pad;
+  w.Y = cur.take<char>(all_res ? 0 : packed_elems * 2);
+  w.X2 = cur.take<char>(all_res ? 0 : packed_elems * 2);
   w.active = cur.take<int32_t>(n_cols);
   w.last = cur.take<int32_t>(n_cols);
   w.n_still = cur.take<int32_t>(1);
   w.err = cur.take<int32_t>(1);
-  w.counters = cur.take<unsigned long long>(UMMA_MAX_COUNTERS);
+  w.counters = cur.take<unsigned long long>(UMMA_MAX_COUNTERS + 1);
   w.done = cur.take<int32_t>((int64_t)(n_cols / STREAM_G + 1) * UMMA_MAX_COUNTERS);
   w.n_parts = cur.take<int32_t>(n_cols);
   w.tile_ptr = cur.take<int64_t>(n_cols + 1);
@@ -856,14 +847,15 @@ static UmmaWs umma_layout(void *ws, int64_t ws_bytes, const sm_pattern_t *P, int
   return w;
 }
 
-int64_t sign_umma_ws_bytes(const sm_pattern_t *P, int32_t n_cols, int64_t packed_elems, int32_t x_dtype) {
+int64_t sign_umma_ws_bytes(const sm_pattern_t *P, int32_t n_cols, int64_t packed_elems, int32_t x_dtype,
+                           int32_t nonsym) {
   (void)x_dtype;
-  return umma_layout(nullptr, 0, P, n_cols, packed_elems).used;
+  return umma_layout(nullptr, 0, P, n_cols, packed_elems, (nonsym || opt(OPT_UMMA_SYM) == 0) ? 0 : 1).used;
 }
 
+#ifdef SM_MEASURE
 // 2-D tensor maps over a packed 16-bit buffer seen as rows of 64 elements (128 bytes): box = 64 x box_rows, no
 // swizzle (the image is stored pre-swizzled).  Used by the TM variant only; the others get zeroed maps.
-struct UMaps { CUtensorMap a, b; };
 typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
                                   const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
@@ -885,15 +877,14 @@ static int32_t make_map(CUtensorMap *m, void *buf, int64_t packed_elems, uint32_
   if (r != CUDA_SUCCESS) { g_last_cuda_error = (int32_t)r; return SM_ERR_CUDA; }
   return SM_OK;
 }
+#endif
+struct UMaps { CUtensorMap a, b; };
 
 template <bool BF16, int PHASE, int NCTA, bool SYM, bool MC = false, int NST = 0, bool TM = false, bool DYN = false>
 static int32_t launch_umma(const UArgs &a, const UMaps &maps, int32_t n_sm, cudaStream_t st) {
-  static bool configured = false;
-  if (!configured) {
-    SM_CUDA(cudaFuncSetAttribute(k_umma_gemm<BF16, PHASE, NCTA, SYM, MC, NST, TM, DYN>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 UCfg<NCTA, MC, NST>::SMEM));
-    configured = true;
-  }
+  // set on every call: the attribute is per device and a process may use several
+  SM_CUDA(cudaFuncSetAttribute(k_umma_gemm<BF16, PHASE, NCTA, SYM, MC, NST, TM, DYN>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                               UCfg<NCTA, MC, NST>::SMEM));
   int slot = -1;
   { int32_t rc = prof_begin(st, &slot); if (rc != SM_OK) return rc; }
   cudaLaunchConfig_t cfg = {};
@@ -910,13 +901,10 @@ static int32_t launch_umma(const UArgs &a, const UMaps &maps, int32_t n_sm, cuda
   return prof_end(st, slot);
 }
 
+#ifdef SM_MEASURE
 template <bool BF16, int NSLOT>
 static int32_t launch_fused(const FArgs &a, int32_t n_sm, cudaStream_t st) {
-  static bool configured = false;
-  if (!configured) {
-    SM_CUDA(cudaFuncSetAttribute(k_umma_fused<BF16, NSLOT>, cudaFuncAttributeMaxDynamicSharedMemorySize, UCfg<2>::SMEM));
-    configured = true;
-  }
+  SM_CUDA(cudaFuncSetAttribute(k_umma_fused<BF16, NSLOT>, cudaFuncAttributeMaxDynamicSharedMemorySize, UCfg<2>::SMEM));
   int slot = -1;
   { int32_t rc = prof_begin(st, &slot); if (rc != SM_OK) return rc; }
   cudaLaunchConfig_t cfg = {};
@@ -932,54 +920,94 @@ static int32_t launch_fused(const FArgs &a, int32_t n_sm, cudaStream_t st) {
   SM_LAUNCHED();
   return prof_end(st, slot);
 }
+#endif
 
 template <int PHASE, int NCTA, bool SYM, bool MC = false, int NST = 0, bool TM = false, bool DYN = false>
 static int32_t launch_umma_t(bool bf16, const UArgs &a, const UMaps &m, int32_t n_sm, cudaStream_t st) {
   return bf16 ? launch_umma<true, PHASE, NCTA, SYM, MC, NST, TM, DYN>(a, m, n_sm, st)
               : launch_umma<false, PHASE, NCTA, SYM, MC, NST, TM, DYN>(a, m, n_sm, st);
 }
-// mode: 1 = one CTA per tile, 2 = cta_group::2 pair with relay, 3 = two CTAs with multicast B, 4 = pair with tensor maps
+// mode: 1 = one CTA per tile; SM_MEASURE builds only: 2 = cta_group::2 pair with relay, 3 = two CTAs with multicast B,
+// 4 = pair with tensor maps
 template <int PHASE>
 static int32_t launch_umma_any(bool bf16, int32_t mode, int32_t sym, int32_t nst, const UArgs &a, const UMaps &m,
                                int32_t n_sm, cudaStream_t st) {
+#ifdef SM_MEASURE
   if (mode == 4) return nst == 3 ? launch_umma_t<PHASE, 2, true, false, 3, true>(bf16, a, m, n_sm, st)
                       : nst == 4 ? launch_umma_t<PHASE, 2, true, false, 4, true>(bf16, a, m, n_sm, st)
                                  : launch_umma_t<PHASE, 2, true, false, 6, true>(bf16, a, m, n_sm, st);
   if (mode == 3) return launch_umma_t<PHASE, 2, true, true>(bf16, a, m, n_sm, st);
-  if (mode == 1 && sym && a.counter)      // dynamic tile scheduling
+  if (mode == 2) return sym ? launch_umma_t<PHASE, 2, true>(bf16, a, m, n_sm, st) : launch_umma_t<PHASE, 2, false>(bf16, a, m, n_sm, st);
+#else
+  (void)mode;
+#endif
+  if (sym && a.counter)      // dynamic tile scheduling
     return nst == 3 ? launch_umma_t<PHASE, 1, true, false, 3, false, true>(bf16, a, m, n_sm, st)
                     : launch_umma_t<PHASE, 1, true, false, 0, false, true>(bf16, a, m, n_sm, st);
-  if (mode == 1 && sym && nst == 3) return launch_umma_t<PHASE, 1, true, false, 3>(bf16, a, m, n_sm, st);
-  if (mode == 2) return sym ? launch_umma_t<PHASE, 2, true>(bf16, a, m, n_sm, st) : launch_umma_t<PHASE, 2, false>(bf16, a, m, n_sm, st);
+  if (sym && nst == 3) return launch_umma_t<PHASE, 1, true, false, 3>(bf16, a, m, n_sm, st);
   return sym ? launch_umma_t<PHASE, 1, true>(bf16, a, m, n_sm, st) : launch_umma_t<PHASE, 1, false>(bf16, a, m, n_sm, st);
+}
+
+static int32_t launch_resident(bool bf16, const RArgs &a, int32_t n_sm, cudaStream_t st) {
+  auto k = bf16 ? k_umma_resident<true> : k_umma_resident<false>;
+  SM_CUDA(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, RES_SMEM));
+  int slot = -1;
+  { int32_t rc = prof_begin(st, &slot); if (rc != SM_OK) return rc; }
+  const int32_t grid = a.n_cols < n_sm ? a.n_cols : n_sm;
+  k<<<grid, RES_THREADS, RES_SMEM, st>>>(a);
+  SM_LAUNCHED();
+  return prof_end(st, slot);
 }
 
 int32_t sign_umma(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, const int64_t *col_off,
                   int64_t packed_elems, int32_t x_dtype, void *X, void *ws, int64_t ws_bytes,
-                  int32_t max_iter, double tol, int32_t *iters, double *residual, cudaStream_t st) {
+                  int32_t max_iter, double tol, int32_t *iters, double *residual, int32_t nonsym, int32_t switch_iter,
+                  cudaStream_t st) {
   if ((P->pad_to % 64) != 0) return SM_ERR_ARG;
   const bool bf16 = x_dtype == SM_BF16;
-  const bool fused = umma_fused(P, tol) != 0;
-  const int32_t ncta = fused ? 2 : umma_ncta(P), R = UM * ncta, sym = fused ? 1 : umma_sym(P);
-  UmmaWs w = umma_layout(ws, ws_bytes, P, n_cols, packed_elems);
+  if (switch_iter >= 0) {
+    // mixed schedule (f3): bf16 in, fp16 out; fixed iteration counts, symmetric iterates
+    if (!bf16 || nonsym || tol > 0.0 || switch_iter < 1 || switch_iter >= max_iter) return SM_ERR_ARG;
+  }
+  const bool fused = !nonsym && switch_iter < 0 && umma_fused(tol);
+  const int32_t sym = fused ? 1 : ((nonsym || opt(OPT_UMMA_SYM) == 0) ? 0 : 1);
+  const int32_t ncta = fused ? 2 : umma_ncta(), R = UM * ncta;
+  UmmaWs w = umma_layout(ws, ws_bytes, P, n_cols, packed_elems, sym);
   if (w.used > ws_bytes) return SM_ERR_SPACE;
   int dev = 0, n_sm = 0;
   SM_CUDA(cudaGetDevice(&dev));
   SM_CUDA(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
-  SignState s{w.active, w.last, w.n_still, w.partial, w.parts_per_col};
+  // a kernel protocol failure (a barrier that never completes) writes its reason code here before it traps:
+  // pinned host memory, readable after the sticky error (sm_last_device_error)
+  w.err = device_err_word();
   const int32_t nb = (n_cols + 255) / 256;
-  k_sign_init<<<nb, 256, 0, st>>>(n_cols, w.active, w.last, iters, residual);
+
+  // ---- small submatrices: all steps inside one CTA (k_umma_resident)
+  const int32_t res_pd = fused ? 0 : umma_resident_pd(sym);
+  if (res_pd > 0) {
+    SM_CUDA(cudaMemsetAsync(w.counters + UMMA_MAX_COUNTERS, 0, sizeof(unsigned long long), st));
+    RArgs r{cols, col_off, P->dim, P->dim_pad, n_cols, max_iter, tol, X, iters, residual,
+            w.counters + UMMA_MAX_COUNTERS, w.err, switch_iter};
+    int32_t rc = launch_resident(bf16, r, n_sm, st);
+    if (rc != SM_OK) return rc;
+    if (res_pd >= P->max_dim_pad) return SM_OK;          // every listed column was resident
+  }
+  if (switch_iter >= 0) return SM_ERR_UNSUPPORTED;        // the mixed schedule exists in the resident kernel only (Pd <= 256)
+
+  // ---- the rest: grouped tiles, one launch per product (or stream / fused)
+  SignState s{w.active, w.last, w.n_still, w.partial, w.parts_per_col};
+  k_sign_init_grouped<<<nb, 256, 0, st>>>(n_cols, cols, P->dim_pad, res_pd, w.active, w.last, iters, residual);
   SM_LAUNCHED();
-  k_umma_tilecounts<<<nb, 256, 0, st>>>(n_cols, R, sym, EPI_WARPS * ncta, cols, P->dim, P->dim_pad, w.tile_ptr,
+  k_umma_tilecounts<<<nb, 256, 0, st>>>(n_cols, R, sym, EPI_WARPS * ncta, res_pd, cols, P->dim, P->dim_pad, w.tile_ptr,
                                         w.n_parts);
   SM_LAUNCHED();
   { int32_t rc = exclusive_scan_i64(n_cols, w.tile_ptr, w.tile_ptr, st); if (rc != SM_OK) return rc; }
-  k_umma_build_tiles<<<nb, 256, 0, st>>>(n_cols, R, sym, cols, P->dim, P->dim_pad, col_off, w.tile_ptr, w.tiles);
+  k_umma_build_tiles<<<nb, 256, 0, st>>>(n_cols, R, sym, res_pd, cols, P->dim, P->dim_pad, col_off, w.tile_ptr, w.tiles);
   SM_LAUNCHED();
   // Y and the alternate X buffer start as zeros so that padding never holds NaN/Inf bit patterns.
   SM_CUDA(cudaMemsetAsync(w.Y, 0, packed_elems * 2, st));
   SM_CUDA(cudaMemsetAsync(w.X2, 0, packed_elems * 2, st));
-  SM_CUDA(cudaMemsetAsync(w.err, 0, sizeof(int32_t), st));
+#ifdef SM_MEASURE
   if (fused) {
     // fixed iteration count: one launch runs every step of every submatrix (k_umma_fused)
     FArgs f{cols, col_off, P->dim, P->dim_pad, n_cols, max_iter, X, w.X2, w.Y, w.partial, w.parts_per_col, w.err, nullptr, umma_dbg()};
@@ -990,8 +1018,7 @@ int32_t sign_umma(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, co
       SM_CUDA(cudaMalloc((void **)&f.trace, trace_bytes));
       SM_CUDA(cudaMemsetAsync(f.trace, 0, trace_bytes, st));
     }
-    static int32_t nslot = 0;      // SM_UMMA_SLOTS=1/2: submatrices a CTA pair interleaves (A/B measurements)
-    if (!nslot) { const char *e = getenv("SM_UMMA_SLOTS"); nslot = (e && e[0] == '1') ? 1 : 2; }
+    const int32_t nslot = opt(OPT_UMMA_SLOTS) == 1 ? 1 : 2;
     int32_t rc = nslot == 2 ? (bf16 ? launch_fused<true, 2>(f, n_sm, st) : launch_fused<false, 2>(f, n_sm, st))
                             : (bf16 ? launch_fused<true, 1>(f, n_sm, st) : launch_fused<false, 1>(f, n_sm, st));
     if (rc != SM_OK) return rc;
@@ -1002,18 +1029,20 @@ int32_t sign_umma(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, co
       SM_CUDA(cudaFree(f.trace));
       if (FILE *fp = fopen(trace_path, "wb")) { fwrite(hbuf.data(), 1, trace_bytes, fp); fclose(fp); }
     }
-    k_fused_post<<<(n_cols + 7) / 8, 256, 0, st>>>(n_cols, cols, P->dim, w.partial, w.parts_per_col, w.n_parts,
+    k_fused_post<<<(n_cols + 7) / 8, 256, 0, st>>>(n_cols, cols, P->dim, P->dim_pad, 0, w.partial, w.parts_per_col, w.n_parts,
                                                    max_iter, iters, residual);
     SM_LAUNCHED();
     dim3 cgf(n_cols, 8);
-    k_copy_back<<<cgf, 256, 0, st>>>(cols, col_off, iters, 2, (const char *)w.X2, (char *)X);
+    k_copy_back<<<cgf, 256, 0, st>>>(cols, col_off, iters, 2, P->dim_pad, 0, (const char *)w.X2, (char *)X);
     SM_LAUNCHED();
     return SM_OK;
   }
-  static int32_t tmap_env = -1;   // SM_UMMA_TMAP=1: cta_group::2 pairs load through tensor maps (with SM_UMMA_NCTA=2 SM_UMMA_MC=0)
-  if (tmap_env < 0) { const char *e = getenv("SM_UMMA_TMAP"); tmap_env = (e && e[0] == '1') ? 1 : 0; }
-  const int32_t mode = (ncta == 2 && sym && umma_mc()) ? 3 : (ncta == 2 && sym && tmap_env) ? 4 : ncta;
+  const int32_t mode = (ncta == 2 && sym && opt(OPT_UMMA_MC) != 0) ? 3 : (ncta == 2 && sym && opt(OPT_UMMA_TMAP) == 1) ? 4 : ncta;
+#else
+  const int32_t mode = 1;
+#endif
   UMaps maps[3] = {};              // per buffer: X, alternate X, W (mode 4 only)
+#ifdef SM_MEASURE
   if (mode == 4) {
     void *bufs[3] = {X, w.X2, w.Y};
     for (int b = 0; b < 3; ++b) {
@@ -1022,34 +1051,29 @@ int32_t sign_umma(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, co
       if (rc != SM_OK) return rc;
     }
   }
-  static int32_t nst_env = -1;    // SM_UMMA_STAGES=3|4: ring depth of the single-CTA SYM kernel (A/B measurements)
-  if (nst_env < 0) { const char *e = getenv("SM_UMMA_STAGES"); nst_env = e ? atoi(e) : 0; }
-  static int32_t dyn_on = -1;     // SM_UMMA_DYN=0: static round-robin deal of the tiles (A/B measurements)
-  if (dyn_on < 0) { const char *e = getenv("SM_UMMA_DYN"); dyn_on = (e && e[0] == '0') ? 0 : 1; }
-  const bool dyn = dyn_on && mode == 1 && sym && 2 * max_iter <= UMMA_MAX_COUNTERS;
+#endif
+  const int32_t nst_opt = opt(OPT_UMMA_STAGES);
+  const bool dyn = opt(OPT_UMMA_DYN) != 0 && mode == 1 && sym && 2 * max_iter <= UMMA_MAX_COUNTERS;
   // ring depth: with the static deal large submatrices want the shallow ring (see UCfg); the dynamic deal removes
   // the drift that made the deep ring costly (configs[4], 25 steps: 603 ms with 4 stages, 615 ms with 3)
-  const int32_t nst = nst_env ? nst_env : (mode == 4 ? 6 : ((!dyn && P->max_dim > 1024) ? 3 : 4));
+  const int32_t nst = nst_opt ? nst_opt : (mode == 4 ? 6 : ((!dyn && P->max_dim > 1024) ? 3 : 4));
   if (dyn) SM_CUDA(cudaMemsetAsync(w.counters, 0, sizeof(unsigned long long) * UMMA_MAX_COUNTERS, st));
-  static int32_t stream_on = -1;  // SM_UMMA_STREAM=1: one launch for all products (fixed iteration counts, dynamic deal)
-  if (stream_on < 0) { const char *e = getenv("SM_UMMA_STREAM"); stream_on = (e && e[0] == '1') ? 1 : 0; }
-  if (stream_on && dyn && !(tol > 0.0) && max_iter > 0) {
+  if (opt(OPT_UMMA_STREAM) == 1 && dyn && !(tol > 0.0) && max_iter > 0) {
     const int64_t n_done = (int64_t)(n_cols / STREAM_G + 1) * 2 * max_iter;
     SM_CUDA(cudaMemsetAsync(w.done, 0, sizeof(int32_t) * n_done, st));
     UArgs a{cols, col_off, P->dim, P->dim_pad, w.tile_ptr, w.tiles, n_cols, 0, X, w.Y, w.X2, s, w.err, 0, w.counters,
             2 * max_iter, w.done, umma_dbg()};
     int32_t rc = launch_umma_t<0, 1, true, false, 0, false, true>(bf16, a, maps[0], n_sm, st);
     if (rc != SM_OK) return rc;
-    k_fused_post<<<(n_cols + 7) / 8, 256, 0, st>>>(n_cols, cols, P->dim, w.partial, w.parts_per_col, w.n_parts,
+    k_fused_post<<<(n_cols + 7) / 8, 256, 0, st>>>(n_cols, cols, P->dim, P->dim_pad, res_pd, w.partial, w.parts_per_col, w.n_parts,
                                                    max_iter, iters, residual);
     SM_LAUNCHED();
     dim3 cgs(n_cols, 8);
-    k_copy_back<<<cgs, 256, 0, st>>>(cols, col_off, iters, 2, (const char *)w.X2, (char *)X);
+    k_copy_back<<<cgs, 256, 0, st>>>(cols, col_off, iters, 2, P->dim_pad, res_pd, (const char *)w.X2, (char *)X);
     SM_LAUNCHED();
     return SM_OK;
   }
-  static int32_t rev_on = -1;     // SM_UMMA_REV=0 keeps every launch walking forwards (A/B measurements)
-  if (rev_on < 0) { const char *e = getenv("SM_UMMA_REV"); rev_on = (e && e[0] == '0') ? 0 : 1; }
+  const int32_t rev_on = opt(OPT_UMMA_REV) != 0 ? 1 : 0;
   void *buf[2] = {X, w.X2};
   for (int32_t k = 0; k < max_iter; ++k) {
     void *src = buf[k & 1], *dst = buf[(k + 1) & 1];
@@ -1065,7 +1089,7 @@ int32_t sign_umma(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, co
       SM_LAUNCHED();
     } else if (k == max_iter - 1) {
       // fixed iteration count: nothing depends on the residual, so only the last step's is reduced (and iters set)
-      k_fused_post<<<(n_cols + 7) / 8, 256, 0, st>>>(n_cols, cols, P->dim, w.partial, w.parts_per_col, w.n_parts,
+      k_fused_post<<<(n_cols + 7) / 8, 256, 0, st>>>(n_cols, cols, P->dim, P->dim_pad, res_pd, w.partial, w.parts_per_col, w.n_parts,
                                                      max_iter, iters, residual);
       SM_LAUNCHED();
     }
@@ -1082,7 +1106,7 @@ int32_t sign_umma(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, co
     }
   }
   dim3 cg(n_cols, 8);
-  k_copy_back<<<cg, 256, 0, st>>>(cols, col_off, iters, 2, (const char *)w.X2, (char *)X);
+  k_copy_back<<<cg, 256, 0, st>>>(cols, col_off, iters, 2, P->dim_pad, res_pd, (const char *)w.X2, (char *)X);
   SM_LAUNCHED();
   return SM_OK;
 }

@@ -10,7 +10,11 @@ environment forces (each in its own process: the selection is read once per proc
   SM_UMMA_SLOTS=2|1  submatrices a CTA pair of the fused kernel interleaves
   SM_UMMA_SYM=1|0    symmetric half tiles with mirrored stores / true products with an MN-major B operand
   SM_UMMA_FUSED=1|0  one launch runs every step of a submatrix (k_umma_fused) / one launch per product
-  SM_F64_BACKEND     DMMA tensor tiles (default) / DFMA register tiles
+  SM_UMMA_RESIDENT=1|0  submatrices with Pd <= 256 iterate inside one SM (k_umma_resident) / grouped tiles for all
+  SM_UMMA_LT=0|1     grouped tiles: iterates stored lower-triangular, the upper part read through MN-major descriptors
+  SM_F64_SIMT=0|1    DMMA tensor tiles (default) / DFMA register tiles
+The two-CTA and fused variants exist only in a -DSM_MEASURE build of the library (build.py --measure); their cases
+are skipped on the default build.
 Each case runs NS steps on a seeded workload whose submatrices span several tiles and ragged tails and
 compares with the oracle's NS-k polynomial (exact-arithmetic result of k steps, reading A13)."""
 import os
@@ -32,7 +36,7 @@ SNIPPET = textwrap.dedent("""
     from oracle import oracle as orc
     from workloads.generator import make_workload
     x_dtype, pad, k, tol_abs, sym_exact = {x_dtype!r}, {pad}, {k}, {tol_abs}, {sym_exact}
-    wl = make_workload({n_mol}, 23, 4, {cutoff}, seed=33)
+    wl = make_workload({n_mol}, {b}, {n_occ}, {cutoff}, seed=33)
     A = sm.Bcsr(wl); P = sm.sm_build_pattern(A, pad); Ph = sm.pattern_to_host(P)
     cols, col_off, n = sm.sm_plan_columns(P, None)
     X, scale = sm.sm_gather(A, P, cols, col_off, n, 0.0, "gershgorin", x_dtype)
@@ -40,7 +44,11 @@ SNIPPET = textwrap.dedent("""
     torch.cuda.synchronize()
     assert (iters == k).all()
     dims = Ph.dim
-    picks = sorted(set([int(np.argmin(dims)), int(np.argmax(dims)), 0, wl.n_blk // 2]))
+    picks = set([int(np.argmin(dims)), int(np.argmax(dims)), 0, wl.n_blk // 2])
+    for pdv in np.unique(Ph.dim_pad):                      # one column of every padded size (every tile shape)
+        idx = np.nonzero(Ph.dim_pad == pdv)[0]
+        picks.add(int(idx[0])); picks.add(int(idx[np.argmax(dims[idx])]))
+    picks = sorted(picks)
     def img_index(Pd):
         r = np.arange(Pd)[:, None]; c = np.arange(Pd)[None, :]
         return (c >> 6) * Pd * 64 + r * 64 + ((((c & 63) >> 3) ^ (r & 7)) << 3) + (c & 7)
@@ -57,30 +65,48 @@ SNIPPET = textwrap.dedent("""
             assert np.array_equal(x, x.T), "iterate must be exactly symmetric"
         else:
             assert np.abs(x - x.T).max() <= tol_abs
-    print("OK dims", int(dims.min()), int(dims.max()), "worst", worst)
+    print("OK dims", int(dims.min()), int(dims.max()), "pads", sorted(set(int(x) for x in Ph.dim_pad)), "worst", worst)
 """)
 
+M = "measure"      # case needs a -DSM_MEASURE build
 CASES = [
-    # env, x_dtype, pad, n_mol, cutoff, steps, tolerance (max-abs vs the NS-k polynomial), exact symmetry
-    ({"SM_UMMA_FUSED": "0", "SM_UMMA_NCTA": "1", "SM_UMMA_SYM": "1"}, "bf16", 64, 90, 5.0, 3, 2.5e-2, True),
-    ({"SM_UMMA_FUSED": "0", "SM_UMMA_NCTA": "2", "SM_UMMA_SYM": "1", "SM_UMMA_MC": "1"}, "bf16", 64, 90, 5.0, 3, 2.5e-2, True),
-    ({"SM_UMMA_FUSED": "0", "SM_UMMA_NCTA": "2", "SM_UMMA_SYM": "1", "SM_UMMA_MC": "0"}, "bf16", 64, 90, 5.0, 3, 2.5e-2, True),
-    ({"SM_UMMA_FUSED": "0", "SM_UMMA_NCTA": "2", "SM_UMMA_SYM": "1", "SM_UMMA_MC": "1", "SM_UMMA_REV": "0"}, "f16", 64, 90, 5.0, 3, 3e-3, True),
-    ({"SM_UMMA_FUSED": "0", "SM_UMMA_NCTA": "2", "SM_UMMA_SYM": "1", "SM_UMMA_MC": "0"}, "f16", 64, 90, 5.0, 4, 3e-3, True),
-    ({"SM_UMMA_FUSED": "0", "SM_UMMA_NCTA": "1", "SM_UMMA_SYM": "0"}, "f16", 64, 90, 5.0, 3, 3e-3, False),
-    ({"SM_UMMA_FUSED": "0", "SM_UMMA_NCTA": "2", "SM_UMMA_SYM": "0"}, "bf16", 64, 90, 5.0, 3, 2.5e-2, False),
-    ({"SM_UMMA_FUSED": "1"}, "bf16", 64, 90, 5.0, 3, 2.5e-2, True),
-    ({"SM_UMMA_FUSED": "1", "SM_UMMA_SLOTS": "1"}, "bf16", 64, 90, 5.0, 4, 2.5e-2, True),
-    ({"SM_UMMA_FUSED": "1"}, "f16", 64, 90, 5.0, 4, 3e-3, True),
-    ({"SM_F64_BACKEND": "dmma"}, "f64", 4, 90, 5.0, 4, 1e-13, True),
-    ({"SM_F64_BACKEND": "simt"}, "f64", 16, 90, 5.0, 4, 1e-13, False),
+    # env, x_dtype, pad, (n_mol, b, n_occ, cutoff), steps, tolerance (max-abs vs the NS-k polynomial), exact symmetry, build
+    ({"SM_UMMA_NCTA": "1", "SM_UMMA_SYM": "1"}, "bf16", 64, (90, 23, 4, 5.0), 3, 2.5e-2, True, None),
+    ({"SM_UMMA_DYN": "0"}, "f16", 64, (90, 23, 4, 5.0), 3, 3e-3, True, None),
+    ({"SM_UMMA_STREAM": "1"}, "f16", 64, (90, 23, 4, 5.0), 4, 3e-3, True, None),
+    ({"SM_UMMA_SYM": "0"}, "f16", 64, (90, 23, 4, 5.0), 3, 3e-3, False, None),
+    ({"SM_UMMA_SYM": "0"}, "bf16", 64, (300, 6, 3, 6.0), 3, 2.5e-2, False, None),
+    # shared-memory-resident kernel: every padded size 64 .. 256 plus larger ones through the grouped path in one call
+    ({"SM_UMMA_RESIDENT": "1"}, "bf16", 64, (300, 6, 3, 6.0), 3, 2.5e-2, True, None),
+    ({"SM_UMMA_RESIDENT": "1"}, "f16", 64, (300, 6, 3, 6.0), 5, 3e-3, True, None),
+    ({"SM_UMMA_RESIDENT": "1"}, "f16", 64, (40, 6, 3, 4.0), 4, 3e-3, True, None),
+    ({"SM_UMMA_RESIDENT": "1"}, "bf16", 64, (60, 23, 4, 3.2), 3, 2.5e-2, True, None),
+    ({"SM_UMMA_RESIDENT": "0"}, "f16", 64, (300, 6, 3, 6.0), 5, 3e-3, True, None),
+    ({"SM_UMMA_FUSED": "0", "SM_UMMA_NCTA": "2", "SM_UMMA_SYM": "1", "SM_UMMA_MC": "1"}, "bf16", 64, (90, 23, 4, 5.0), 3, 2.5e-2, True, M),
+    ({"SM_UMMA_FUSED": "0", "SM_UMMA_NCTA": "2", "SM_UMMA_SYM": "1", "SM_UMMA_MC": "0"}, "bf16", 64, (90, 23, 4, 5.0), 3, 2.5e-2, True, M),
+    ({"SM_UMMA_FUSED": "0", "SM_UMMA_NCTA": "2", "SM_UMMA_SYM": "1", "SM_UMMA_MC": "1", "SM_UMMA_REV": "0"}, "f16", 64, (90, 23, 4, 5.0), 3, 3e-3, True, M),
+    ({"SM_UMMA_FUSED": "0", "SM_UMMA_NCTA": "2", "SM_UMMA_SYM": "1", "SM_UMMA_MC": "0"}, "f16", 64, (90, 23, 4, 5.0), 4, 3e-3, True, M),
+    ({"SM_UMMA_FUSED": "0", "SM_UMMA_NCTA": "2", "SM_UMMA_SYM": "0"}, "bf16", 64, (90, 23, 4, 5.0), 3, 2.5e-2, False, M),
+    ({"SM_UMMA_FUSED": "1"}, "bf16", 64, (90, 23, 4, 5.0), 3, 2.5e-2, True, M),
+    ({"SM_UMMA_FUSED": "1", "SM_UMMA_SLOTS": "1"}, "bf16", 64, (90, 23, 4, 5.0), 4, 2.5e-2, True, M),
+    ({"SM_UMMA_FUSED": "1"}, "f16", 64, (90, 23, 4, 5.0), 4, 3e-3, True, M),
+    ({"SM_F64_SIMT": "0"}, "f64", 4, (90, 23, 4, 5.0), 4, 1e-13, True, None),
+    ({"SM_F64_SIMT": "1"}, "f64", 16, (90, 23, 4, 5.0), 4, 1e-13, False, None),
 ]
 
 
-@pytest.mark.parametrize("env,x_dtype,pad,n_mol,cutoff,k,tol_abs,sym_exact", CASES)
-def test_backend_matches_ns_polynomial(env, x_dtype, pad, n_mol, cutoff, k, tol_abs, sym_exact):
+def _measure_build():
+    import paper_2205_14741_b200.binding as sm
+    return bool(sm.build_info() & 1)
+
+
+@pytest.mark.parametrize("env,x_dtype,pad,wl,k,tol_abs,sym_exact,need", CASES)
+def test_backend_matches_ns_polynomial(env, x_dtype, pad, wl, k, tol_abs, sym_exact, need):
+    if need == M and not _measure_build():
+        pytest.skip("variant exists only in a -DSM_MEASURE build (build.py --measure)")
+    n_mol, b, n_occ, cutoff = wl
     code = SNIPPET.format(root=ROOT, x_dtype=x_dtype, pad=pad, k=k, tol_abs=tol_abs, sym_exact=sym_exact,
-                          n_mol=n_mol, cutoff=cutoff)
+                          n_mol=n_mol, cutoff=cutoff, b=b, n_occ=n_occ)
     e = dict(os.environ)
     e.update(env)
     p = subprocess.run([sys.executable, "-c", code], env=e, capture_output=True, text=True, timeout=600, cwd=ROOT)
@@ -105,18 +131,20 @@ HASH_SNIPPET = textwrap.dedent("""
 """)
 
 SYM_VARIANTS = [
-    {"SM_UMMA_FUSED": "0", "SM_UMMA_NCTA": "1"},
-    {"SM_UMMA_FUSED": "0", "SM_UMMA_NCTA": "1", "SM_UMMA_REV": "0"},
-    {"SM_UMMA_FUSED": "0", "SM_UMMA_NCTA": "1", "SM_UMMA_STAGES": "3"},
-    {"SM_UMMA_FUSED": "0", "SM_UMMA_NCTA": "1", "SM_UMMA_DYN": "0"},
-    {"SM_UMMA_FUSED": "0", "SM_UMMA_NCTA": "1", "SM_UMMA_DYN": "0", "SM_UMMA_STAGES": "3"},
+    {"SM_UMMA_RESIDENT": "0"},
+    {"SM_UMMA_RESIDENT": "0", "SM_UMMA_REV": "0"},
+    {"SM_UMMA_RESIDENT": "0", "SM_UMMA_STAGES": "3"},
+    {"SM_UMMA_RESIDENT": "0", "SM_UMMA_DYN": "0"},
+    {"SM_UMMA_RESIDENT": "0", "SM_UMMA_DYN": "0", "SM_UMMA_STAGES": "3"},
+    {"SM_UMMA_RESIDENT": "0", "SM_UMMA_STREAM": "1"},
+]
+SYM_VARIANTS_MEASURE = [
     {"SM_UMMA_FUSED": "0", "SM_UMMA_NCTA": "2", "SM_UMMA_MC": "1"},
     {"SM_UMMA_FUSED": "0", "SM_UMMA_NCTA": "2", "SM_UMMA_MC": "0"},
     {"SM_UMMA_FUSED": "0", "SM_UMMA_NCTA": "2", "SM_UMMA_MC": "0", "SM_UMMA_TMAP": "1"},
     {"SM_UMMA_FUSED": "0", "SM_UMMA_NCTA": "2", "SM_UMMA_MC": "0", "SM_UMMA_TMAP": "1", "SM_UMMA_STAGES": "3"},
     {"SM_UMMA_FUSED": "1", "SM_UMMA_SLOTS": "1"},
     {"SM_UMMA_FUSED": "1", "SM_UMMA_SLOTS": "2"},
-    {"SM_UMMA_FUSED": "0", "SM_UMMA_NCTA": "1", "SM_UMMA_STREAM": "1"},
 ]
 
 
@@ -126,7 +154,7 @@ def test_symmetric_tile_variants_are_bit_identical():
     7 odd-count steps (copy-back path) on 200 submatrices spanning several tile shapes give the same bits; the
     fused residual is the same to rounding of its fixed-order partial sums (grouped per tile and warp)."""
     seen = {}
-    for env in SYM_VARIANTS:
+    for env in SYM_VARIANTS + (SYM_VARIANTS_MEASURE if _measure_build() else []):
         e = dict(os.environ)
         e.update(env)
         p = subprocess.run([sys.executable, "-c", HASH_SNIPPET.format(root=ROOT)], env=e, capture_output=True,
