@@ -124,19 +124,32 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_umma_resident(RArgs a) {
     }
   } else if (warp == 1) {
     // ===================== MMA issuer =====================
-    if (lane == 0) {
+    // The whole warp runs this loop converged, on warp-uniform values (shuffle broadcasts tell ptxas so); one
+    // elected lane issues each MMA / commit (umma_f16_elect).
+    {
       uint32_t p_xload = 0, p_w = 0, p_x = 0;
       for (;;) {
         ptx::mbar_wait(b_xload, p_xload, a.err_flag, 22); p_xload ^= 1u;
-        const int64_t c = *cur_c;
+        const int32_t c = __shfl_sync(0xffffffffu, (int32_t)*cur_c, 0);
         if (c < 0) break;
-        const Sub s = sub_of(c);
+        Sub s = sub_of(c);
+        s.m = __shfl_sync(0xffffffffu, s.m, 0); s.Pd = __shfl_sync(0xffffffffu, s.Pd, 0);
+        s.kmax = (s.m + 15) & ~15; s.nkc = (s.kmax + 63) >> 6; s.n0 = s.Pd < 128 ? s.Pd : 128; s.two = s.Pd > 128;
         const uint32_t Pd = (uint32_t)s.Pd;
         bool bf = BF16_IN;
+#ifdef SM_RES_TRACE
+        long long tr_a = 0, tr_b = 0, tr_c = 0, tr_d = 0, tr_t;
+#endif
         for (int32_t k = 0; k < a.max_iter; ++k) {
           if (k == a.switch_iter) bf = false;     // 0 < switch_iter < max_iter (host-checked), tol <= 0
-          // ---- product 1: Y = X X^T (both operands K-major rows of XS)
-          for (int t = 0; t < (s.two ? 2 : 1); ++t) {
+#ifdef SM_RES_TRACE
+          tr_t = clock64();
+#endif
+          // ---- product 1: Y = X X^T (both operands K-major rows of XS).  T1 first: its epilogue (more blocks, and
+          // only the quadrants that hold its rows) then overlaps T0's MMAs and the shorter T0 epilogue is the exposed
+          // one.  (Product 2 must keep T0 first: T1's mirrored stores land in rows 0..127 of XS, which T0 reads.)
+          for (int tt = 0; tt < (s.two ? 2 : 1); ++tt) {
+            const int t = s.two ? 1 - tt : 0;
             const uint32_t N = t ? Pd : (uint32_t)s.n0;
             const uint32_t idesc = ptx::make_idesc_f16(bf, 128, N, false);
             const uint32_t d = tmem_base + (t ? 128u : 0u);
@@ -144,13 +157,23 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_umma_resident(RArgs a) {
               const uint64_t ad = ptx::make_sw128_kmajor_desc(xs + (uint32_t)kc * Pd * 128u + (t ? 128u * 128u : 0u));
               const uint64_t bd = ptx::make_sw128_kmajor_desc(xs + (uint32_t)kc * Pd * 128u);
               const int ksteps = min(4, (s.kmax - kc * 64) / 16);
-              for (int ks = 0; ks < ksteps; ++ks)
-                ptx::umma_f16(d, ad + (uint64_t)(2 * ks), bd + (uint64_t)(2 * ks), idesc, (uint32_t)((kc | ks) != 0));
+              if (ksteps == 4) {
+#pragma unroll
+                for (int ks = 0; ks < 4; ++ks) ptx::umma_f16_elect(d, ad + (uint64_t)(2 * ks), bd + (uint64_t)(2 * ks), idesc, (uint32_t)((kc | ks) != 0));
+              } else {
+                for (int ks = 0; ks < ksteps; ++ks) ptx::umma_f16_elect(d, ad + (uint64_t)(2 * ks), bd + (uint64_t)(2 * ks), idesc, (uint32_t)((kc | ks) != 0));
+              }
             }
-            ptx::umma_commit(t ? b_tfull1 : b_tfull0);
+            ptx::umma_commit_elect(t ? b_tfull1 : b_tfull0);
           }
+#ifdef SM_RES_TRACE
+          { long long n = clock64(); tr_a += n - tr_t; tr_t = n; }
+#endif
           ptx::mbar_wait(b_wready, p_w, a.err_flag, 23); p_w ^= 1u;
           ptx::tc_fence_after();
+#ifdef SM_RES_TRACE
+          { long long n = clock64(); tr_b += n - tr_t; tr_t = n; }
+#endif
           bool last = k + 1 == a.max_iter;
           if (a.tol > 0.0 && residual_now(s.m) < a.tol) last = true;
           // ---- product 2: X Wh^T (A = rows of XS, B = Wh from WS: stored rows K-major, the rest through the transpose)
@@ -164,27 +187,46 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_umma_resident(RArgs a) {
                 const uint32_t N = t ? Pd : (uint32_t)s.n0;
                 const uint32_t idesc = ptx::make_idesc_f16(bf, 128, N, false);
                 const uint64_t bd = ptx::make_sw128_kmajor_desc(ws + res_woff((uint32_t)kc, Pd));
-                for (int ks = 0; ks < ksteps; ++ks)
-                  ptx::umma_f16(d, ad + (uint64_t)(2 * ks), bd + (uint64_t)(2 * ks), idesc, acc0 | (uint32_t)(ks != 0));
+                if (ksteps == 4) {
+#pragma unroll
+                for (int ks = 0; ks < 4; ++ks) ptx::umma_f16_elect(d, ad + (uint64_t)(2 * ks), bd + (uint64_t)(2 * ks), idesc, acc0 | (uint32_t)(ks != 0));
+              } else {
+                for (int ks = 0; ks < ksteps; ++ks) ptx::umma_f16_elect(d, ad + (uint64_t)(2 * ks), bd + (uint64_t)(2 * ks), idesc, acc0 | (uint32_t)(ks != 0));
+              }
               } else {
                 // output columns 0..127: Wh[n][k] = Wh[k][n], rows 64 kc.. of chunks 0 and 1, MN-major
                 const uint32_t idesc_t = ptx::make_idesc_f16(bf, 128, 128, true);
                 const uint64_t bt = ptx::make_sw128_mnmajor_desc(ws + (uint32_t)kc * 64u * 128u, Pd * 128u, 1024u);
-                for (int ks = 0; ks < ksteps; ++ks)
-                  ptx::umma_f16(d, ad + (uint64_t)(2 * ks), bt + (uint64_t)(128 * ks), idesc_t, 1u);
+                if (ksteps == 4) {
+#pragma unroll
+                for (int ks = 0; ks < 4; ++ks) ptx::umma_f16_elect(d, ad + (uint64_t)(2 * ks), bt + (uint64_t)(128 * ks), idesc_t, 1u);
+              } else {
+                for (int ks = 0; ks < ksteps; ++ks) ptx::umma_f16_elect(d, ad + (uint64_t)(2 * ks), bt + (uint64_t)(128 * ks), idesc_t, 1u);
+              }
                 if (t) {
                   // output columns 128..Pd-1: rows 128.. of chunk kc are stored, K-major
                   const uint32_t idesc_d = ptx::make_idesc_f16(bf, 128, Pd - 128u, false);
                   const uint64_t bd = ptx::make_sw128_kmajor_desc(ws + res_woff((uint32_t)kc, Pd));
-                  for (int ks = 0; ks < ksteps; ++ks)
-                    ptx::umma_f16(d + 128u, ad + (uint64_t)(2 * ks), bd + (uint64_t)(2 * ks), idesc_d, 1u);
+                  if (ksteps == 4) {
+#pragma unroll
+                for (int ks = 0; ks < 4; ++ks) ptx::umma_f16_elect(d + 128u, ad + (uint64_t)(2 * ks), bd + (uint64_t)(2 * ks), idesc_d, 1u);
+              } else {
+                for (int ks = 0; ks < ksteps; ++ks) ptx::umma_f16_elect(d + 128u, ad + (uint64_t)(2 * ks), bd + (uint64_t)(2 * ks), idesc_d, 1u);
+              }
                 }
               }
             }
-            ptx::umma_commit(t ? b_tfull1 : b_tfull0);
+            ptx::umma_commit_elect(t ? b_tfull1 : b_tfull0);
           }
+#ifdef SM_RES_TRACE
+          { long long n = clock64(); tr_c += n - tr_t; tr_t = n; }
+#endif
           ptx::mbar_wait(b_xready, p_x, a.err_flag, 24); p_x ^= 1u;
           ptx::tc_fence_after();
+#ifdef SM_RES_TRACE
+          { long long n = clock64(); tr_d += n - tr_t; tr_t = n; }
+          if (last && blockIdx.x == 0 && lane == 0) printf("res trace c=%lld m=%d Pd=%d steps=%d issue1=%lld wait1=%lld issue2=%lld wait2=%lld (cycles per step)\n", (long long)c, s.m, s.Pd, k + 1, tr_a / (k + 1), tr_b / (k + 1), tr_c / (k + 1), tr_d / (k + 1));
+#endif
           if (last) break;
         }
       }
@@ -214,7 +256,8 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_umma_resident(RArgs a) {
         auto pass = [&](const bool P2, const bool bf_out, float &res) {
           float res2 = 0.f;
           const int g = lane >> 2, q2 = lane & 3, rl = lane & 7, ml = lane >> 3;
-          for (int t = 0; t < (s.two ? 2 : 1); ++t) {
+          for (int tt = 0; tt < (s.two ? 2 : 1); ++tt) {
+            const int t = (s.two && !P2) ? 1 - tt : tt;             // the order the MMAs of this product were issued in
             ptx::mbar_wait(t ? b_tfull1 : b_tfull0, p_t[t], a.err_flag, 26); p_t[t] ^= 1u;
             ptx::tc_fence_after();
             const int32_t R0 = 128 * t + 32 * q;

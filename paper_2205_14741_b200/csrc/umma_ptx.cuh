@@ -113,6 +113,33 @@ __device__ __forceinline__ void umma_f16(uint32_t tmem_d, uint64_t adesc, uint64
       "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
       : "memory");
 }
+// Warp-convergent issue: EVERY lane of the (converged) warp executes this with the same operands and one elected lane
+// issues the MMA.  With the issuing code under `if (lane == 0)` ptxas cannot keep descriptors in uniform registers
+// and wraps every tcgen05.mma in an ELECT / 7 x R2UR.BROADCAST / BRA.U.ANY loop: ~150 cycles per MMA measured
+// (ncu + clock64, round 2) against 64-128 cycles of tensor-pipe time -- the issue path, not the operands, was the
+// bottleneck.  Operands must be warp-uniform (derive them from kernel parameters, loop counters and __shfl_sync
+// broadcasts).
+__device__ __forceinline__ void umma_f16_elect(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t idesc,
+                                               uint32_t accumulate) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p, q;\n"
+      "setp.ne.b32 p, %4, 0;\n"
+      "elect.sync _|q, 0xffffffff;\n"
+      "@q tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n"
+      "}\n" ::"r"(tmem_d),
+      "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
+      : "memory");
+}
+__device__ __forceinline__ void umma_commit_elect(uint32_t bar) {
+  asm volatile(
+      "{\n"
+      ".reg .pred q;\n"
+      "elect.sync _|q, 0xffffffff;\n"
+      "@q tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];\n"
+      "}\n" ::"r"(bar)
+      : "memory");
+}
 // All previously issued MMAs of this thread arrive (once) on the mbarrier when they complete.
 __device__ __forceinline__ void umma_commit(uint32_t bar) {
   asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar)
