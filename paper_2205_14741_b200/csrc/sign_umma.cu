@@ -65,12 +65,15 @@ constexpr uint32_t TMEM_COLS = 512;
 // configs[4] (m ~ 1650) single CTAs run 25 steps in 653 ms with 3 stages and 747 ms with 4 (2 stages: 734 ms) --
 // a shallower ring keeps the CTAs that share a submatrix's operand panels closer together in L2 --
 // while configs[2] (m ~ 410) prefers 4 (27.8 vs 28.7 ms).
-template <int NCTA, bool MC = false, int NST = 0> struct UCfg {
+// EPI = 1: staged epilogue (two 32 KB output staging buffers, bulk stores; the ring then has 3 stages).
+constexpr int EPI_STG_UNIT = 32768;
+template <int NCTA, bool MC = false, int NST = 0, int EPI = 0> struct UCfg {
   static constexpr bool G2 = NCTA == 2 && !MC;             // cta_group::2 MMA
-  static constexpr int STAGES = NST ? NST : (G2 ? 6 : 4);
+  static constexpr int STAGES = NST ? NST : (EPI ? 3 : (G2 ? 6 : 4));
   static constexpr int B_BYTES = (G2 ? UN / 2 : UN) * UK * 2;   // 16 KB / 32 KB
   static constexpr int STAGE_BYTES = A_BYTES + B_BYTES;    // 48 KB / 32 KB
-  static constexpr int SMEM = STAGES * STAGE_BYTES + EPI_STAGE_BYTES + IDENT_BYTES + 1024 /*align slack*/ + 512 /*barriers, tile queue*/;
+  static constexpr int EPI_BYTES = EPI ? 2 * EPI_STG_UNIT : EPI_STAGE_BYTES;
+  static constexpr int SMEM = STAGES * STAGE_BYTES + EPI_BYTES + IDENT_BYTES + 1024 /*align slack*/ + 512 /*barriers, tile queue*/;
   static constexpr int ROWS = UM * NCTA;                   // tile rows
 };
 
@@ -128,6 +131,20 @@ __host__ __device__ inline int32_t u_tiles(int32_t m, int32_t R) {
   return t;
 }
 
+// Geometry of the staged epilogue (EPI = 1, 128-row tiles): tile columns are whole 64-column chunks of the image (a
+// chunk of a row range is contiguous in memory: one bulk store) and the tiles of a row panel are cut from the RIGHT
+// in steps of 256, so that the 128 x 128 diagonal square of the panel always lies inside its last tile.
+__host__ __device__ inline int32_t v_ncols(int32_t m, int32_t tm) {
+  int32_t n64 = (m + 63) & ~63, e = tm * UM + UM;
+  return e < n64 ? e : n64;
+}
+__host__ __device__ inline int32_t v_row_tiles(int32_t m, int32_t tm) { return (v_ncols(m, tm) + UN - 1) / UN; }
+__host__ __device__ inline int32_t v_tiles(int32_t m) {
+  int32_t t = 0;
+  for (int32_t tm = 0; tm < u_Tm(m, UM); ++tm) t += v_row_tiles(m, tm);
+  return t;
+}
+
 // FULL mode (true products, no symmetry): every 128*NCTA-row panel of the Pd x Pd image times all Pd
 // columns, in tiles of 256 columns (the last one takes the rest, rounded up to whole 64-column
 // swizzle atoms per CTA).
@@ -177,7 +194,15 @@ static __global__ void k_umma_build_tiles(int32_t n_cols, int32_t R, int32_t sym
   d.base = col_off[c]; d.c = c; d.m = m; d.Pd = Pd; d.pad0 = d.pad1 = d.pad2 = 0;
   int64_t t = tile_ptr[c];
   int32_t lt = 0;
-  if (sym) {
+  if (sym == 2) {
+    for (int32_t tm = 0; tm < u_Tm(m, UM); ++tm) {
+      const int32_t cnt = v_row_tiles(m, tm), nc = v_ncols(m, tm), w0 = nc - UN * (cnt - 1);
+      for (int32_t tn = 0; tn < cnt; ++tn, ++lt, ++t) {
+        d.row0 = tm * UM; d.n0 = tn ? w0 + UN * (tn - 1) : 0; d.nt = tn ? UN : w0; d.lt = lt;
+        tiles[t] = d;
+      }
+    }
+  } else if (sym) {
     for (int32_t tm = 0; tm < u_Tm(m, R); ++tm) {
       int32_t cnt = u_row_tiles(m, R, tm), nb = u_row_nb(m, R, tm), nc = u_ncols(m, R, tm);
       for (int32_t tn = 0; tn < cnt; ++tn, ++lt, ++t) {
@@ -291,15 +316,17 @@ constexpr int TQ = 4;
 #endif
 constexpr int STREAM_G = SM_STREAM_G;
 constexpr int STREAM_SG = SM_STREAM_SG;
-template <bool BF16, int PHASE, int NCTA, bool SYM, bool MC = false, int NST = 0, bool TM = false, bool DYN = false>
+template <bool BF16, int PHASE, int NCTA, bool SYM, bool MC = false, int NST = 0, bool TM = false, bool DYN = false, int EPI = 0>
 __global__ void __launch_bounds__(UMMA_THREADS, 1)
 k_umma_gemm(UArgs a, const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapB) {
   static_assert(!DYN || NCTA == 1, "dynamic tile scheduling: one CTA per tile");
+  static_assert(EPI == 0 || (SYM && NCTA == 1 && PHASE != 0), "staged epilogue: single CTAs, SYM tiles, one launch per product");
+  constexpr bool STG = EPI == 1;
   static_assert(PHASE != 0 || (DYN && SYM), "stream mode needs the dynamic deal and symmetric tiles");
   constexpr bool STREAM = PHASE == 0;
   static_assert(!MC || (NCTA == 2 && SYM), "multicast variant: two CTAs, SYM tiles");
   static_assert(!TM || (NCTA == 2 && SYM && !MC), "tensor-map variant: cta_group::2 pairs, SYM tiles");
-  using Cfg = UCfg<NCTA, MC, NST>;
+  using Cfg = UCfg<NCTA, MC, NST, EPI>;
   constexpr int USTAGES = Cfg::STAGES;
   constexpr int STAGE_BYTES = Cfg::STAGE_BYTES;
   constexpr bool PAIR = NCTA == 2 && !MC;                  // cta_group::2 MMAs issued by the leader
@@ -307,8 +334,8 @@ k_umma_gemm(UArgs a, const __grid_constant__ CUtensorMap mapA, const __grid_cons
   extern __shared__ uint8_t smem_raw[];
   const uint32_t raw = ptx::smem_u32(smem_raw);
   const uint32_t tiles = (raw + 1023u) & ~1023u;           // 1024-byte aligned operand ring
-  const uint32_t stage_base = tiles + USTAGES * STAGE_BYTES;   // epilogue transpose buffers
-  const uint32_t ident = stage_base + EPI_STAGE_BYTES;     // identity image (1024-byte aligned)
+  const uint32_t stage_base = tiles + USTAGES * STAGE_BYTES;   // epilogue transpose / staging buffers (1024-byte aligned)
+  const uint32_t ident = stage_base + Cfg::EPI_BYTES;      // identity image (1024-byte aligned)
   const uint32_t bars = ident + IDENT_BYTES;               // barriers behind it
   // barrier slots (8 bytes each): full[S], empty[S], pfull[S] (pair: peer's stage landed, leader only),
   // tmem_full[2], tmem_empty[2]; then the TMEM base address
@@ -492,7 +519,11 @@ k_umma_gemm(UArgs a, const __grid_constant__ CUtensorMap mapA, const __grid_cons
     }
   } else if (warp == 1) {
     // ===================== MMA issuer (leader CTA; every CTA when each issues its own MMAs) =====================
-    if (lane == 0 && !(PAIR && h != 0)) {
+    // The whole warp walks the tiles converged, on warp-uniform values (the tile descriptor is broadcast by shuffles,
+    // which tells ptxas so), and one elected lane issues each MMA / commit (umma_f16_elect).  Under `if (lane == 0)`
+    // every tcgen05.mma was wrapped in an ELECT / R2UR.BROADCAST / BRA.U.ANY loop of ~150 cycles (clock64, round 2),
+    // more than the 128 cycles a 128 x 256 x 16 MMA occupies the tensor pipe.
+    if (!(PAIR && h != 0)) {
       int stage = 0; uint32_t phase = 0;
       uint32_t it = 0;
       TileDesc nxt = load_desc(a, max((int64_t)0, min(unit, total - 1)));
@@ -502,7 +533,8 @@ k_umma_gemm(UArgs a, const __grid_constant__ CUtensorMap mapA, const __grid_cons
         if (DYN) {
           ptx::mbar_wait(tqf_bar(qs), qp, a.err_flag, 9);
           cur = tq[qs];
-          ptx::mbar_arrive(tqe_bar(qs));
+          __syncwarp();
+          if (lane == 0) ptx::mbar_arrive(tqe_bar(qs));
           if (++qs == TQ) { qs = 0; qp ^= 1u; }
           return cur.c >= 0;
         }
@@ -512,9 +544,22 @@ k_umma_gemm(UArgs a, const __grid_constant__ CUtensorMap mapA, const __grid_cons
         t += n_units;
         return true;
       };
+      auto mma = [&](uint32_t d, uint64_t ad, uint64_t bd, uint32_t id, uint32_t acc) {
+        if (PAIR) ptx::umma_f16_2cta_elect(d, ad, bd, id, acc);
+        else ptx::umma_f16_elect(d, ad, bd, id, acc);
+      };
+      auto commit = [&](uint32_t bar) {
+        if (PAIR) ptx::umma_commit_2cta_elect(bar);
+        else if (MC) ptx::umma_commit_mc_elect(bar, (uint16_t)3);
+        else ptx::umma_commit_elect(bar);
+      };
       TileDesc cur;
       while (fetch(cur)) {
+        cur.c = __shfl_sync(0xffffffffu, cur.c, 0); cur.m = __shfl_sync(0xffffffffu, cur.m, 0);
+        cur.n0 = __shfl_sync(0xffffffffu, cur.n0, 0); cur.nt = __shfl_sync(0xffffffffu, cur.nt, 0);
+        cur.pad0 = __shfl_sync(0xffffffffu, cur.pad0, 0);
         UTile u = make_tile<PHASE>(a, cur);
+        u.valid = __shfl_sync(0xffffffffu, u.valid, 0);
         if (!u.valid) continue;
         const uint32_t as = it % NACC, aphase = (it / NACC) & 1u;
         ptx::mbar_wait(tempty_bar(as), aphase ^ 1u, a.err_flag, 2);
@@ -522,6 +567,7 @@ k_umma_gemm(UArgs a, const __grid_constant__ CUtensorMap mapA, const __grid_cons
         const uint32_t d_tmem = tmem_base + as * UN;
         const uint32_t idesc = ptx::make_idesc_f16(BF16, PAIR ? 2 * UM : UM, (uint32_t)u.nt, !SYM);
         const int nkc = (u.kmax + UK - 1) / UK;
+        const bool p2 = STREAM ? (cur.pad0 & 1) != 0 : PHASE == 2;
         for (int kc = 0; kc < nkc; ++kc) {
           ptx::mbar_wait(full_bar(stage), phase, a.err_flag, 3);
           if (PAIR && !TM) ptx::mbar_wait(pfull_bar(stage), phase, a.err_flag, 6);
@@ -530,40 +576,189 @@ k_umma_gemm(UArgs a, const __grid_constant__ CUtensorMap mapA, const __grid_cons
           const uint64_t adesc = ptx::make_sw128_kmajor_desc(sa);
           const uint64_t bdesc = SYM ? ptx::make_sw128_kmajor_desc(sb) : ptx::make_sw128_mnmajor_desc(sb, 8192u, 1024u);
           const uint64_t bstep = SYM ? 2u : 128u;   // 16 k: 32 B inside a K-major atom / 16 rows of 128 B
-          const int ksteps = min(UK / 16, (u.kmax - kc * UK) / 16);
-          for (int ks = 0; ks < (SM_DBG(a, 2) ? 0 : ksteps); ++ks) {
-            // advance 16 elements = 32 bytes inside the swizzle atom: +2 in the (addr >> 4) field
-            if (PAIR)
-              ptx::umma_f16_2cta(d_tmem, adesc + (uint64_t)(2 * ks), bdesc + bstep * (uint64_t)ks, idesc,
-                                 (uint32_t)((kc | ks) != 0));
-            else
-              ptx::umma_f16(d_tmem, adesc + (uint64_t)(2 * ks), bdesc + bstep * (uint64_t)ks, idesc,
-                            (uint32_t)((kc | ks) != 0));
+          const int ksteps = SM_DBG(a, 2) ? 0 : min(UK / 16, (u.kmax - kc * UK) / 16);
+          if (ksteps == UK / 16) {
+#pragma unroll
+            for (int ks = 0; ks < UK / 16; ++ks)
+              mma(d_tmem, adesc + (uint64_t)(2 * ks), bdesc + bstep * (uint64_t)ks, idesc, (uint32_t)((kc | ks) != 0));
+          } else {
+            for (int ks = 0; ks < ksteps; ++ks)
+              mma(d_tmem, adesc + (uint64_t)(2 * ks), bdesc + bstep * (uint64_t)ks, idesc, (uint32_t)((kc | ks) != 0));
           }
-          if ((STREAM ? (cur.pad0 & 1) != 0 : PHASE == 2) && !SM_DBG(a, 2)) {
+          if (p2 && !SM_DBG(a, 2)) {
             // "+ X": the A chunk in this stage holds X[rows, 64 kc .. 64 kc + 63]; add it to the accumulator
             // columns [lo, hi) of the tile that it covers (B = identity slice, K-major)
             const int32_t lo = max(kc * UK, u.n0), hi = min(kc * UK + UK, u.n0 + u.nt);
             if (lo < hi) {
               const uint32_t idesc2 = ptx::make_idesc_f16(BF16, PAIR ? 2 * UM : UM, (uint32_t)(hi - lo), false);
               const uint64_t idd = ptx::make_sw128_kmajor_desc(ident + ident_row(PAIR, lo - kc * UK, hi - lo) * 128u);
-              for (int ks = 0; ks < UK / 16; ++ks) {
-                if (PAIR) ptx::umma_f16_2cta(d_tmem + (uint32_t)(lo - u.n0), adesc + (uint64_t)(2 * ks), idd + (uint64_t)(2 * ks), idesc2, 1u);
-                else ptx::umma_f16(d_tmem + (uint32_t)(lo - u.n0), adesc + (uint64_t)(2 * ks), idd + (uint64_t)(2 * ks), idesc2, 1u);
-              }
+#pragma unroll
+              for (int ks = 0; ks < UK / 16; ++ks)
+                mma(d_tmem + (uint32_t)(lo - u.n0), adesc + (uint64_t)(2 * ks), idd + (uint64_t)(2 * ks), idesc2, 1u);
             }
           }
           // frees the smem slot (in both CTAs of a pair) when these MMAs finish
-          if (PAIR) ptx::umma_commit_2cta(empty_bar(stage));
-          else if (MC) ptx::umma_commit_mc(empty_bar(stage), (uint16_t)3);
-          else ptx::umma_commit(empty_bar(stage));
+          commit(empty_bar(stage));
           if (++stage == USTAGES) { stage = 0; phase ^= 1u; }
         }
         // accumulator ready for the epilogue warps (of both CTAs)
-        if (PAIR) ptx::umma_commit_2cta(tfull_bar(as)); else ptx::umma_commit(tfull_bar(as));
+        if (PAIR) ptx::umma_commit_2cta_elect(tfull_bar(as)); else ptx::umma_commit_elect(tfull_bar(as));
         ++it;
       }
     }
+  } else if (STG) {
+    // ===================== staged epilogue (warps 2..17; EPI = 1) =====================
+    // The output of a tile leaves the SM as bulk stores of whole image pieces instead of per-lane global stores
+    // (round 1: the epilogue's 2 x 256-bit + 32 x 2-byte global stores per 32 x 32 block and lane made it the
+    // bound of configs[2]: 9000 cycles per tile against 3600 of MMA time).  A tile is cut into UNITS that each fill
+    // one 32 KB staging buffer: a 64-column chunk left of the panel's diagonal square (direct piece 128 rows x 128 B
+    // = rows of the tile in that chunk, plus the mirrored pieces 2 x (64 rows x 128 B) = rows of that chunk in the
+    // two chunks of the square's columns), or the diagonal square itself (2 chunks x 128 rows x 128 B, the upper
+    // blocks filled by mirroring the lower ones).  Blocks are read from TMEM in the mma fragment layout
+    // (tcgen05.ld 16x256b), packed, and written with stmatrix (direct) / stmatrix.trans (mirror) into the staging
+    // buffer, which has the swizzled layout of the image; one thread then issues the unit's 1-3 bulk stores.
+    // Two teams of 8 warps (2 per TMEM lane quadrant) alternate over the units, each with its own buffer.
+    const int q = warp & 3;                        // TMEM lane quadrant this warp may access
+    const int sub = (warp - 2) >> 2, team = sub >> 1, tsub = sub & 1;
+    const uint32_t stg = stage_base + (uint32_t)team * EPI_STG_UNIT;
+    const bool leader = warp == 2 + 8 * team && lane == 0;
+    auto team_bar = [&]() { asm volatile("bar.sync %0, %1;" ::"r"(1 + team), "r"(256) : "memory"); };
+    const int g = lane >> 2, q2 = lane & 3, rl = lane & 7, ml = lane >> 3;
+    uint32_t it = 0;
+    TileDesc nxt = load_desc(a, max((int64_t)0, min(unit, total - 1)));
+    int64_t t = unit;
+    uint32_t qs = 0, qp = 0;
+    auto fetch = [&](TileDesc &cur) -> bool {
+      if (DYN) {
+        ptx::mbar_wait(tqf_bar(qs), qp, a.err_flag, 10);
+        cur = tq[qs];
+        __syncwarp();                                   // every lane has its copy before the slot is handed back
+        if (lane == 0) ptx::mbar_arrive(tqe_bar(qs));
+        if (++qs == TQ) { qs = 0; qp ^= 1u; }
+        return cur.c >= 0;
+      }
+      if (t >= total) return false;
+      cur = nxt;
+      nxt = load_desc(a, min(t + n_units, total - 1));
+      t += n_units;
+      return true;
+    };
+    TileDesc cur;
+    while (fetch(cur)) {
+      UTile u = make_tile<PHASE>(a, cur);
+      if (!u.valid) continue;
+      const uint32_t as = it % NACC, aphase = (it / NACC) & 1u;
+      constexpr bool p1 = PHASE == 1;
+      uint16_t *Og = (uint16_t *)a.Out + u.base;
+      if (SM_DBG(a, 1)) Og = nullptr;
+      const int32_t R0 = u.row0 + q * 32;                     // this warp's 32 rows of the tile
+      const int32_t a_rows = min(UM, u.Pd - u.row0);
+      const int32_t n_below = max(0, min(u.nt, u.row0 - u.n0)) >> 6;   // whole chunks left of the diagonal square
+      const int32_t n_un = n_below + (u.n0 + u.nt > u.row0 ? 1 : 0);
+      const uint32_t rb = ((uint32_t)R0 & 63u) >> 3;
+      ptx::mbar_wait(tfull_bar(as), aphase, a.err_flag, 4);
+      ptx::tc_fence_after();
+      const uint32_t taddr = tmem_base + as * UN + ((uint32_t)(q * 32) << 16);
+      float res = 0.f, res2 = 0.f;                             // diagonal-block / off-diagonal (counted twice) sums
+      for (int ui = team; ui < n_un; ui += 2) {
+        if (leader) ptx::bulk_wait_read0();                    // the buffer's previous bulk stores have read it
+        team_bar();
+        const bool sq = ui == n_below;
+        const int32_t cu0 = sq ? u.row0 : u.n0 + 64 * ui;     // first column of the unit
+        if (R0 < u.Pd && !SM_DBG(a, 8)) {
+          for (int bj = tsub; sq ? (cu0 + 32 * bj <= R0) : (bj < 2); bj += 2) {
+            const int32_t C0 = cu0 + 32 * bj;
+            uint32_t v[2][16];
+            ptx::tmem_ld_16x256b_x4(taddr + (uint32_t)(C0 - u.n0), v[0]);                  // rows R0 + {g, g + 8}
+            ptx::tmem_ld_16x256b_x4(taddr + (16u << 16) + (uint32_t)(C0 - u.n0), v[1]);    // rows R0 + 16 + {g, g + 8}
+            const uint32_t cb = ((uint32_t)C0 & 63u) >> 3;
+            ptx::tmem_ld_wait();
+            const bool diag = (C0 == R0);
+            uint32_t o[4][4];
+            float acc = 0.f;
+#pragma unroll
+            for (int ti = 0; ti < 4; ++ti) {
+#pragma unroll
+              for (int tj = 0; tj < 4; ++tj) {
+                float f0 = __uint_as_float(v[ti >> 1][4 * tj + 2 * (ti & 1)]);
+                float f1 = __uint_as_float(v[ti >> 1][4 * tj + 2 * (ti & 1) + 1]);
+                if (p1) {
+                  if (diag) {
+                    const int rr = 8 * ti + g, c0 = 8 * tj + 2 * q2;
+                    if (R0 + rr < u.m) { if (c0 == rr) f0 -= 1.f; if (c0 + 1 == rr) f1 -= 1.f; }   // W = Y - I
+                    if (tj <= ti) {
+                      if (c0 <= rr) acc = fmaf(c0 == rr ? f0 : 2.f * f0, f0, acc);
+                      if (c0 + 1 <= rr) acc = fmaf(c0 + 1 == rr ? f1 : 2.f * f1, f1, acc);
+                    }
+                  } else {
+                    acc = fmaf(f0, f0, acc); acc = fmaf(f1, f1, acc);
+                  }
+                  f0 *= -0.5f; f1 *= -0.5f;                 // Wh = -1/2 W is what PHASE 2 multiplies by
+                }
+                o[ti][tj] = pack2<BF16>(f0, f1);
+              }
+            }
+            if (p1) { if (diag) res += acc; else res2 += acc; }
+            if (diag) {
+              // diagonal tiles: element (r, c > r) := element (c, r), through the transposed fragment
+#pragma unroll
+              for (int ti = 0; ti < 4; ++ti) {
+                const uint32_t tr = ptx::movmatrix_t(o[ti][ti]);
+                const uint32_t sel = (2 * q2 <= g ? 0x10u : 0x54u) | ((2 * q2 + 1 <= g ? 0x32u : 0x76u) << 8);
+                o[ti][ti] = __byte_perm(o[ti][ti], tr, sel);
+              }
+            }
+            // direct: rows R0 .., columns C0 .. of the unit's direct piece
+            const uint32_t dbase = stg + (sq ? (uint32_t)((C0 - u.row0) >> 6) * 16384u : 0u) +
+                                   (uint32_t)(R0 - u.row0 + rl) * 128u + (((cb + (uint32_t)ml) ^ (uint32_t)rl) << 4);
+#pragma unroll
+            for (int ti = 0; ti < 4; ++ti) ptx::stsm_x4(dbase + ti * 1024u, o[ti][0], o[ti][1], o[ti][2], o[ti][3]);
+            // mirror: tile (ti, tj) transposed -> rows C0 + 8 tj .., columns R0 + 8 ti ..
+            const uint32_t mbase = sq ? stg + (uint32_t)((R0 - u.row0) >> 6) * 16384u + (uint32_t)(C0 - u.row0 + rl) * 128u
+                                      : stg + 16384u + (uint32_t)((R0 - u.row0) >> 6) * 8192u + (uint32_t)((C0 & 63) + rl) * 128u;
+            if (!diag) {
+              const uint32_t ma = mbase + (((rb + (uint32_t)ml) ^ (uint32_t)rl) << 4);
+#pragma unroll
+              for (int tj = 0; tj < 4; ++tj) ptx::stsm_x4_t(ma + tj * 1024u, o[0][tj], o[1][tj], o[2][tj], o[3][tj]);
+            } else {
+              __syncwarp();       // the direct stores of the upper tiles come first
+              ptx::stsm_x4_t(mbase + (((rb + (uint32_t)ml) ^ (uint32_t)rl) << 4), o[0][0], o[1][0], o[2][0], o[3][0]);
+              ptx::stsm_x2_t(mbase + 1024u + (((rb + 2u + (uint32_t)(ml & 1)) ^ (uint32_t)rl) << 4), o[2][1], o[3][1]);
+              ptx::stsm_x1_t(mbase + 2048u + (((rb + 3u) ^ (uint32_t)rl) << 4), o[3][2]);
+            }
+          }
+        }
+        ptx::fence_proxy_async_smem();             // generic-proxy stores -> the bulk copies' async-proxy reads
+        team_bar();
+        if (leader && Og) {
+          const int64_t Pd64 = (int64_t)u.Pd * 64;
+          if (sq) {
+            for (int pz = 0; pz < 2; ++pz)
+              if (u.row0 + 64 * pz < u.Pd)
+                ptx::tma_bulk_s2g(Og + ((int64_t)((u.row0 >> 6) + pz) * Pd64 + (int64_t)u.row0 * 64), stg + pz * 16384u,
+                                  (uint32_t)a_rows * 128u);
+          } else {
+            ptx::tma_bulk_s2g(Og + ((int64_t)(cu0 >> 6) * Pd64 + (int64_t)u.row0 * 64), stg, (uint32_t)a_rows * 128u);
+            for (int pz = 0; pz < 2; ++pz)
+              if (u.row0 + 64 * pz < u.Pd)
+                ptx::tma_bulk_s2g(Og + ((int64_t)((u.row0 >> 6) + pz) * Pd64 + (int64_t)cu0 * 64), stg + 16384u + pz * 8192u, 8192u);
+          }
+          ptx::bulk_commit();
+        }
+      }
+      res += 2.f * res2;
+      // accumulator drained: hand the TMEM stage back to the MMA warp
+      ptx::tc_fence_before();
+      __syncwarp();
+      if (lane == 0) ptx::mbar_arrive(tempty_bar(as));
+      if (p1) {
+        for (int d = 16; d > 0; d >>= 1) res += __shfl_xor_sync(0xffffffffu, res, d);
+        if (lane == 0)
+          a.s.partial[(int64_t)u.c * a.s.parts_per_col + (int64_t)u.lt * EPI_WARPS + (warp - 2)] = (double)res;
+      }
+      ++it;
+    }
+    if (leader) ptx::bulk_wait0();
   } else {
     // ===================== epilogue (warps 2..17) =====================
     // EPI_WARPS / 4 warps per TMEM lane quadrant; a warp owns 32 rows and every (EPI_WARPS/4)-th
@@ -765,7 +960,7 @@ static __global__ void k_umma_tilecounts(int32_t n_cols, int32_t R, int32_t sym,
   int32_t c = blockIdx.x * blockDim.x + threadIdx.x;
   if (c >= n_cols) return;
   int32_t i = cols ? cols[c] : c;
-  int32_t nt = dim_pad[i] <= skip_pd ? 0 : (sym ? u_tiles(dim[i], R) : f_tiles(dim_pad[i], R));
+  int32_t nt = dim_pad[i] <= skip_pd ? 0 : (sym == 2 ? v_tiles(dim[i]) : sym ? u_tiles(dim[i], R) : f_tiles(dim_pad[i], R));
   tiles[c] = nt;
   n_parts[c] = nt * parts_per_tile;
 }
@@ -815,6 +1010,14 @@ static int32_t umma_dbg() {
   return 0;
 #endif
 }
+// 0 = true products on all tiles, 1 = symmetric half tiles with per-lane global stores, 2 = symmetric half tiles with
+// the staged epilogue (single CTAs, one launch per product)
+static int32_t umma_sym_mode(int32_t nonsym, bool fused, int32_t ncta, double tol, int32_t max_iter) {
+  if (fused) return 1;
+  if (nonsym || opt(OPT_UMMA_SYM) == 0) return 0;
+  const bool stream = opt(OPT_UMMA_STREAM) == 1 && !(tol > 0.0) && max_iter > 0;
+  return (opt(OPT_UMMA_EPI) != 0 && ncta == 1 && !stream) ? 2 : 1;
+}
 // all listed columns with Pd <= this go through k_umma_resident (0: none)
 static int32_t umma_resident_pd(int32_t sym) { return (sym && opt(OPT_UMMA_RESIDENT) != 0) ? RES_MAX_PD : 0; }
 
@@ -825,7 +1028,7 @@ static UmmaWs umma_layout(void *ws, int64_t ws_bytes, const sm_pattern_t *P, int
   // sized for whichever variant sign_umma picks (the query does not know tol): per-phase launches with
   // the selected NCTA / SYM, or the fused kernel (CTA pairs, SYM)
   const int32_t ncta = umma_ncta();
-  const int32_t t_sel = sym ? u_tiles(P->max_dim, UM * ncta) : f_tiles(P->max_dim_pad, UM * ncta);
+  const int32_t t_sel = sym == 2 ? v_tiles(P->max_dim) : sym ? u_tiles(P->max_dim, UM * ncta) : f_tiles(P->max_dim_pad, UM * ncta);
   const int32_t t_fused = u_tiles(P->max_dim, UM * 2);
   const int32_t max_tiles = t_sel > t_fused ? t_sel : t_fused;
   w.parts_per_col = (t_sel * ncta > t_fused * 2 ? t_sel * ncta : t_fused * 2) * EPI_WARPS;
@@ -850,7 +1053,10 @@ static UmmaWs umma_layout(void *ws, int64_t ws_bytes, const sm_pattern_t *P, int
 int64_t sign_umma_ws_bytes(const sm_pattern_t *P, int32_t n_cols, int64_t packed_elems, int32_t x_dtype,
                            int32_t nonsym) {
   (void)x_dtype;
-  return umma_layout(nullptr, 0, P, n_cols, packed_elems, (nonsym || opt(OPT_UMMA_SYM) == 0) ? 0 : 1).used;
+  // sized for the larger of the tile tables the call may pick (the query does not know tol / max_iter)
+  const int64_t a = umma_layout(nullptr, 0, P, n_cols, packed_elems, umma_sym_mode(nonsym, false, umma_ncta(), 0.0, 1)).used;
+  const int64_t b = umma_layout(nullptr, 0, P, n_cols, packed_elems, umma_sym_mode(nonsym, false, umma_ncta(), 1.0, 1)).used;
+  return a > b ? a : b;
 }
 
 #ifdef SM_MEASURE
@@ -880,23 +1086,23 @@ static int32_t make_map(CUtensorMap *m, void *buf, int64_t packed_elems, uint32_
 #endif
 struct UMaps { CUtensorMap a, b; };
 
-template <bool BF16, int PHASE, int NCTA, bool SYM, bool MC = false, int NST = 0, bool TM = false, bool DYN = false>
+template <bool BF16, int PHASE, int NCTA, bool SYM, bool MC = false, int NST = 0, bool TM = false, bool DYN = false, int EPI = 0>
 static int32_t launch_umma(const UArgs &a, const UMaps &maps, int32_t n_sm, cudaStream_t st) {
   // set on every call: the attribute is per device and a process may use several
-  SM_CUDA(cudaFuncSetAttribute(k_umma_gemm<BF16, PHASE, NCTA, SYM, MC, NST, TM, DYN>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                               UCfg<NCTA, MC, NST>::SMEM));
+  SM_CUDA(cudaFuncSetAttribute(k_umma_gemm<BF16, PHASE, NCTA, SYM, MC, NST, TM, DYN, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                               UCfg<NCTA, MC, NST, EPI>::SMEM));
   int slot = -1;
   { int32_t rc = prof_begin(st, &slot); if (rc != SM_OK) return rc; }
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3((unsigned)(n_sm / NCTA * NCTA), 1, 1);     // one CTA per SM, whole pairs
   cfg.blockDim = dim3(UMMA_THREADS, 1, 1);
-  cfg.dynamicSmemBytes = UCfg<NCTA, MC, NST>::SMEM;
+  cfg.dynamicSmemBytes = UCfg<NCTA, MC, NST, EPI>::SMEM;
   cfg.stream = st;
   cudaLaunchAttribute attr[1];
   attr[0].id = cudaLaunchAttributeClusterDimension;
   attr[0].val.clusterDim.x = NCTA; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
   cfg.attrs = attr; cfg.numAttrs = 1;
-  SM_CUDA(cudaLaunchKernelEx(&cfg, k_umma_gemm<BF16, PHASE, NCTA, SYM, MC, NST, TM, DYN>, a, maps.a, maps.b));
+  SM_CUDA(cudaLaunchKernelEx(&cfg, k_umma_gemm<BF16, PHASE, NCTA, SYM, MC, NST, TM, DYN, EPI>, a, maps.a, maps.b));
   SM_LAUNCHED();
   return prof_end(st, slot);
 }
@@ -922,10 +1128,10 @@ static int32_t launch_fused(const FArgs &a, int32_t n_sm, cudaStream_t st) {
 }
 #endif
 
-template <int PHASE, int NCTA, bool SYM, bool MC = false, int NST = 0, bool TM = false, bool DYN = false>
+template <int PHASE, int NCTA, bool SYM, bool MC = false, int NST = 0, bool TM = false, bool DYN = false, int EPI = 0>
 static int32_t launch_umma_t(bool bf16, const UArgs &a, const UMaps &m, int32_t n_sm, cudaStream_t st) {
-  return bf16 ? launch_umma<true, PHASE, NCTA, SYM, MC, NST, TM, DYN>(a, m, n_sm, st)
-              : launch_umma<false, PHASE, NCTA, SYM, MC, NST, TM, DYN>(a, m, n_sm, st);
+  return bf16 ? launch_umma<true, PHASE, NCTA, SYM, MC, NST, TM, DYN, EPI>(a, m, n_sm, st)
+              : launch_umma<false, PHASE, NCTA, SYM, MC, NST, TM, DYN, EPI>(a, m, n_sm, st);
 }
 // mode: 1 = one CTA per tile; SM_MEASURE builds only: 2 = cta_group::2 pair with relay, 3 = two CTAs with multicast B,
 // 4 = pair with tensor maps
@@ -941,6 +1147,9 @@ static int32_t launch_umma_any(bool bf16, int32_t mode, int32_t sym, int32_t nst
 #else
   (void)mode;
 #endif
+  if (sym == 2)              // staged epilogue (bulk stores), 3-stage ring
+    return a.counter ? launch_umma_t<PHASE, 1, true, false, 0, false, true, 1>(bf16, a, m, n_sm, st)
+                     : launch_umma_t<PHASE, 1, true, false, 0, false, false, 1>(bf16, a, m, n_sm, st);
   if (sym && a.counter)      // dynamic tile scheduling
     return nst == 3 ? launch_umma_t<PHASE, 1, true, false, 3, false, true>(bf16, a, m, n_sm, st)
                     : launch_umma_t<PHASE, 1, true, false, 0, false, true>(bf16, a, m, n_sm, st);
@@ -970,8 +1179,8 @@ int32_t sign_umma(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, co
     if (!bf16 || nonsym || tol > 0.0 || switch_iter < 1 || switch_iter >= max_iter) return SM_ERR_ARG;
   }
   const bool fused = !nonsym && switch_iter < 0 && umma_fused(tol);
-  const int32_t sym = fused ? 1 : ((nonsym || opt(OPT_UMMA_SYM) == 0) ? 0 : 1);
   const int32_t ncta = fused ? 2 : umma_ncta(), R = UM * ncta;
+  const int32_t sym = umma_sym_mode(nonsym, fused, ncta, tol, max_iter);
   UmmaWs w = umma_layout(ws, ws_bytes, P, n_cols, packed_elems, sym);
   if (w.used > ws_bytes) return SM_ERR_SPACE;
   int dev = 0, n_sm = 0;
