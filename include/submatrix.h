@@ -233,7 +233,10 @@ int32_t sm_density_from_sign(const sm_bcsr_t *A, const sm_pattern_t *P, int32_t 
  * calls in flight on other threads).  Unknown name: SM_ERR_ARG.
  *   "umma.sym"      [SM_UMMA_SYM]      1|0   16-bit: lower-triangle tiles with mirrored stores / true products, all tiles
  *   "umma.resident" [SM_UMMA_RESIDENT] 1|0   16-bit: submatrices with Pd <= 256 iterate inside one SM / grouped tiles for all
- *   "umma.lt"       [SM_UMMA_LT]       0|1   16-bit grouped tiles: iterates stored lower-triangular (half the stores)
+ *   "umma.epi"      [SM_UMMA_EPI]      0|1   16-bit grouped tiles: per-lane global stores / staged epilogue (stmatrix into
+ *                                            shared-memory staging, bulk stores; 3-stage operand ring)
+ *   "umma.lt"       [SM_UMMA_LT]       0|1   with umma.epi = 1: iterates stored "128-lower" (nothing above the 128 x 128
+ *                                            diagonal squares), the rest read through MN-major descriptors
  *   "umma.dyn"      [SM_UMMA_DYN]      1|0   16-bit grouped tiles handed out by a global counter / dealt round robin
  *   "umma.rev"      [SM_UMMA_REV]      1|0   16-bit: the update product walks the tile table backwards / forwards
  *   "umma.stages"   [SM_UMMA_STAGES]   0|3|4 16-bit grouped tiles: depth of the operand ring (0 = by size)

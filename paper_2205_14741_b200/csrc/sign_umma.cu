@@ -107,6 +107,12 @@ struct UArgs {
   int32_t n_ph;              // 2 * steps
   int32_t *done;             // [groups][n_ph] epilogue-warp completions of (group, product), zeroed by the host
   int32_t dbg;               // measurement only (SM_UMMA_DBG): 1 = skip output stores, 2 = skip MMA issue, 4 = skip TMA loads, 8 = skip the epilogue's work
+  // staged epilogue only (EPI = 1): "128-lower" storage of the iterates.  lt_in: the operands hold valid data only at
+  // (r, c) with r >= (c & ~127) -- everything on or below the 128 x 128 diagonal squares -- and the rest is read
+  // through the transpose (MN-major descriptors over the rows 64 kc .. of the chunk that holds the wanted columns);
+  // lt_out: the output is written that way (no mirrored pieces below the diagonal squares).  The last update of a
+  // submatrix writes the full image (lt_out = 0, or s.last in convergence mode): sm_scatter reads whole rows.
+  int32_t lt_in, lt_out;
 };
 
 // Tile geometry.  Only elements (r, c) with c <= r are computed, so tile row tm (rows tm*R ..
@@ -132,8 +138,8 @@ __host__ __device__ inline int32_t u_tiles(int32_t m, int32_t R) {
 }
 
 // Geometry of the staged epilogue (EPI = 1, 128-row tiles): tile columns are whole 64-column chunks of the image (a
-// chunk of a row range is contiguous in memory: one bulk store) and the tiles of a row panel are cut from the RIGHT
-// in steps of 256, so that the 128 x 128 diagonal square of the panel always lies inside its last tile.
+// chunk of a row range is contiguous in memory: one bulk store); the tiles of a row panel start at multiples of 256
+// columns, so that every 128-column block -- in particular the panel's 128 x 128 diagonal square -- lies inside one tile.
 __host__ __device__ inline int32_t v_ncols(int32_t m, int32_t tm) {
   int32_t n64 = (m + 63) & ~63, e = tm * UM + UM;
   return e < n64 ? e : n64;
@@ -196,9 +202,9 @@ static __global__ void k_umma_build_tiles(int32_t n_cols, int32_t R, int32_t sym
   int32_t lt = 0;
   if (sym == 2) {
     for (int32_t tm = 0; tm < u_Tm(m, UM); ++tm) {
-      const int32_t cnt = v_row_tiles(m, tm), nc = v_ncols(m, tm), w0 = nc - UN * (cnt - 1);
+      const int32_t cnt = v_row_tiles(m, tm), nc = v_ncols(m, tm);
       for (int32_t tn = 0; tn < cnt; ++tn, ++lt, ++t) {
-        d.row0 = tm * UM; d.n0 = tn ? w0 + UN * (tn - 1) : 0; d.nt = tn ? UN : w0; d.lt = lt;
+        d.row0 = tm * UM; d.n0 = tn * UN; d.nt = min(UN, nc - d.n0); d.lt = lt;
         tiles[t] = d;
       }
     }
@@ -474,6 +480,41 @@ k_umma_gemm(UArgs a, const __grid_constant__ CUtensorMap mapA, const __grid_cons
           }
           continue;
         }
+        if (STG && a.lt_in) {
+          // "128-lower" operands: a 128-row block of a chunk that lies above the diagonal squares is fetched as the
+          // transposed pieces (64 k rows x 128 B each, contiguous) of the chunk(s) holding its rows as columns
+          const int32_t rb128 = u.row0 >> 7, jb0 = u.n0 >> 7;
+          const int32_t np = (u.nt + 127) >> 7;                      // 128-column sub-panels of the B rows
+          for (int kc = 0; kc < nkc; ++kc) {
+            ptx::mbar_wait(empty_bar(stage), phase ^ 1u, a.err_flag, 1);
+            const uint32_t sa = tiles + stage * STAGE_BYTES, sb = sa + A_BYTES;
+            const int32_t kb = kc >> 1;
+            const int64_t chunk = (int64_t)kc * u.Pd * 128;          // byte offset of k chunk kc
+            // bytes first (one expect_tx), then the copies
+            uint32_t tx = 0;
+            const bool a_dir = rb128 >= kb;
+            const int32_t a_pieces = min(2, (u.Pd - u.row0 + 63) >> 6);
+            tx += a_dir ? a_bytes : (uint32_t)a_pieces * 8192u;
+            for (int pz = 0; pz < np; ++pz) {
+              const int32_t rows = min(128, u.nt - 128 * pz);
+              tx += (jb0 + pz >= kb) ? (uint32_t)rows * 128u : (uint32_t)((rows + 63) >> 6) * 8192u;
+            }
+            ptx::mbar_expect_tx(full_bar(stage), tx);
+            if (a_dir) ptx::tma_bulk_g2s(sa, Ag + chunk + (int64_t)u.row0 * 128, a_bytes, full_bar(stage));
+            else
+              for (int32_t j = 0; j < a_pieces; ++j)      // rows 64 kc .. of chunk-column (row0 / 64 + j)
+                ptx::tma_bulk_g2s(sa + (uint32_t)j * 8192u, Ag + ((int64_t)((u.row0 >> 6) + j) * u.Pd + (int64_t)kc * UK) * 128, 8192u, full_bar(stage));
+            for (int pz = 0; pz < np; ++pz) {
+              const int32_t rows = min(128, u.nt - 128 * pz), j0 = u.n0 + 128 * pz;
+              if (jb0 + pz >= kb) ptx::tma_bulk_g2s(sb + (uint32_t)pz * 16384u, Bg + chunk + (int64_t)j0 * 128, (uint32_t)rows * 128u, full_bar(stage));
+              else
+                for (int32_t j = 0; j < ((rows + 63) >> 6); ++j)
+                  ptx::tma_bulk_g2s(sb + (uint32_t)pz * 16384u + (uint32_t)j * 8192u, Bg + ((int64_t)((j0 >> 6) + j) * u.Pd + (int64_t)kc * UK) * 128, 8192u, full_bar(stage));
+            }
+            if (++stage == USTAGES) { stage = 0; phase ^= 1u; }
+          }
+          continue;
+        }
         for (int kc = 0; kc < nkc; ++kc) {
           ptx::mbar_wait(empty_bar(stage), phase ^ 1u, a.err_flag, 1);
           const uint32_t sa = tiles + stage * STAGE_BYTES, sb = sa + A_BYTES;
@@ -558,6 +599,7 @@ k_umma_gemm(UArgs a, const __grid_constant__ CUtensorMap mapA, const __grid_cons
         cur.c = __shfl_sync(0xffffffffu, cur.c, 0); cur.m = __shfl_sync(0xffffffffu, cur.m, 0);
         cur.n0 = __shfl_sync(0xffffffffu, cur.n0, 0); cur.nt = __shfl_sync(0xffffffffu, cur.nt, 0);
         cur.pad0 = __shfl_sync(0xffffffffu, cur.pad0, 0);
+        const int32_t cur_row0 = __shfl_sync(0xffffffffu, cur.row0, 0);
         UTile u = make_tile<PHASE>(a, cur);
         u.valid = __shfl_sync(0xffffffffu, u.valid, 0);
         if (!u.valid) continue;
@@ -577,7 +619,33 @@ k_umma_gemm(UArgs a, const __grid_constant__ CUtensorMap mapA, const __grid_cons
           const uint64_t bdesc = SYM ? ptx::make_sw128_kmajor_desc(sb) : ptx::make_sw128_mnmajor_desc(sb, 8192u, 1024u);
           const uint64_t bstep = SYM ? 2u : 128u;   // 16 k: 32 B inside a K-major atom / 16 rows of 128 B
           const int ksteps = SM_DBG(a, 2) ? 0 : min(UK / 16, (u.kmax - kc * UK) / 16);
-          if (ksteps == UK / 16) {
+          if (STG && a.lt_in) {
+            // "128-lower" operands (see the producer): per 128-row block of A and of the B rows, K-major as stored or
+            // MN-major through the transposed pieces; the two 128-column halves of the tile may differ
+            const int32_t kb = kc >> 1, rb128 = cur_row0 >> 7, jb0 = u.n0 >> 7;
+            const bool a_t = rb128 < kb;
+            const uint64_t ad = a_t ? ptx::make_sw128_mnmajor_desc(sa, 8192u, 1024u) : adesc;
+            const uint64_t astep = a_t ? 128u : 2u;
+            const bool b0_t = jb0 < kb, b1_t = jb0 + 1 < kb;
+            const int32_t n1 = u.nt - 128;                           // columns of the second half (<= 0: none)
+            const bool one = n1 <= 0 || b0_t == b1_t;
+            const uint32_t id0 = one ? ptx::make_idesc_f16(BF16, UM, (uint32_t)u.nt, b0_t, a_t) : ptx::make_idesc_f16(BF16, UM, 128u, true, a_t);
+            const uint32_t id1 = ptx::make_idesc_f16(BF16, UM, (uint32_t)max(n1, 16), false, a_t);
+            const uint64_t bd0 = b0_t ? ptx::make_sw128_mnmajor_desc(sb, 8192u, 1024u) : ptx::make_sw128_kmajor_desc(sb);
+            const uint64_t bd1 = ptx::make_sw128_kmajor_desc(sb + 16384u);
+            const uint64_t b0step = b0_t ? 128u : 2u;
+            auto issue = [&](int ks) {
+              const uint32_t acc = (uint32_t)((kc | ks) != 0);
+              mma(d_tmem, ad + astep * (uint64_t)ks, bd0 + b0step * (uint64_t)ks, id0, acc);
+              if (!one) mma(d_tmem + 128u, ad + astep * (uint64_t)ks, bd1 + 2u * (uint64_t)ks, id1, acc);
+            };
+            if (ksteps == UK / 16) {
+#pragma unroll
+              for (int ks = 0; ks < UK / 16; ++ks) issue(ks);
+            } else {
+              for (int ks = 0; ks < ksteps; ++ks) issue(ks);
+            }
+          } else if (ksteps == UK / 16) {
 #pragma unroll
             for (int ks = 0; ks < UK / 16; ++ks)
               mma(d_tmem, adesc + (uint64_t)(2 * ks), bdesc + bstep * (uint64_t)ks, idesc, (uint32_t)((kc | ks) != 0));
@@ -656,6 +724,8 @@ k_umma_gemm(UArgs a, const __grid_constant__ CUtensorMap mapA, const __grid_cons
       const int32_t n_below = max(0, min(u.nt, u.row0 - u.n0)) >> 6;   // whole chunks left of the diagonal square
       const int32_t n_un = n_below + (u.n0 + u.nt > u.row0 ? 1 : 0);
       const uint32_t rb = ((uint32_t)R0 & 63u) >> 3;
+      // mirrored pieces of the units below the diagonal square: always, unless the output is stored "128-lower"
+      const bool mirror_out = !a.lt_out || (a.check_flags && a.s.last[u.c]);
       ptx::mbar_wait(tfull_bar(as), aphase, a.err_flag, 4);
       ptx::tc_fence_after();
       const uint32_t taddr = tmem_base + as * UN + ((uint32_t)(q * 32) << 16);
@@ -717,9 +787,11 @@ k_umma_gemm(UArgs a, const __grid_constant__ CUtensorMap mapA, const __grid_cons
             const uint32_t mbase = sq ? stg + (uint32_t)((R0 - u.row0) >> 6) * 16384u + (uint32_t)(C0 - u.row0 + rl) * 128u
                                       : stg + 16384u + (uint32_t)((R0 - u.row0) >> 6) * 8192u + (uint32_t)((C0 & 63) + rl) * 128u;
             if (!diag) {
-              const uint32_t ma = mbase + (((rb + (uint32_t)ml) ^ (uint32_t)rl) << 4);
+              if (sq || mirror_out) {
+                const uint32_t ma = mbase + (((rb + (uint32_t)ml) ^ (uint32_t)rl) << 4);
 #pragma unroll
-              for (int tj = 0; tj < 4; ++tj) ptx::stsm_x4_t(ma + tj * 1024u, o[0][tj], o[1][tj], o[2][tj], o[3][tj]);
+                for (int tj = 0; tj < 4; ++tj) ptx::stsm_x4_t(ma + tj * 1024u, o[0][tj], o[1][tj], o[2][tj], o[3][tj]);
+              }
             } else {
               __syncwarp();       // the direct stores of the upper tiles come first
               ptx::stsm_x4_t(mbase + (((rb + (uint32_t)ml) ^ (uint32_t)rl) << 4), o[0][0], o[1][0], o[2][0], o[3][0]);
@@ -740,7 +812,7 @@ k_umma_gemm(UArgs a, const __grid_constant__ CUtensorMap mapA, const __grid_cons
           } else {
             ptx::tma_bulk_s2g(Og + ((int64_t)(cu0 >> 6) * Pd64 + (int64_t)u.row0 * 64), stg, (uint32_t)a_rows * 128u);
             for (int pz = 0; pz < 2; ++pz)
-              if (u.row0 + 64 * pz < u.Pd)
+              if (mirror_out && u.row0 + 64 * pz < u.Pd)
                 ptx::tma_bulk_s2g(Og + ((int64_t)((u.row0 >> 6) + pz) * Pd64 + (int64_t)cu0 * 64), stg + 16384u + pz * 8192u, 8192u);
           }
           ptx::bulk_commit();
@@ -1271,7 +1343,7 @@ int32_t sign_umma(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, co
     const int64_t n_done = (int64_t)(n_cols / STREAM_G + 1) * 2 * max_iter;
     SM_CUDA(cudaMemsetAsync(w.done, 0, sizeof(int32_t) * n_done, st));
     UArgs a{cols, col_off, P->dim, P->dim_pad, w.tile_ptr, w.tiles, n_cols, 0, X, w.Y, w.X2, s, w.err, 0, w.counters,
-            2 * max_iter, w.done, umma_dbg()};
+            2 * max_iter, w.done, umma_dbg(), 0, 0};
     int32_t rc = launch_umma_t<0, 1, true, false, 0, false, true>(bf16, a, maps[0], n_sm, st);
     if (rc != SM_OK) return rc;
     k_fused_post<<<(n_cols + 7) / 8, 256, 0, st>>>(n_cols, cols, P->dim, P->dim_pad, res_pd, w.partial, w.parts_per_col, w.n_parts,
@@ -1286,7 +1358,12 @@ int32_t sign_umma(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, co
   void *buf[2] = {X, w.X2};
   for (int32_t k = 0; k < max_iter; ++k) {
     void *src = buf[k & 1], *dst = buf[(k + 1) & 1];
-    UArgs a{cols, col_off, P->dim, P->dim_pad, w.tile_ptr, w.tiles, n_cols, tol > 0.0 ? 1 : 0, src, w.Y, w.Y, s, w.err, 0, nullptr, 0, nullptr, umma_dbg()};
+    UArgs a{cols, col_off, P->dim, P->dim_pad, w.tile_ptr, w.tiles, n_cols, tol > 0.0 ? 1 : 0, src, w.Y, w.Y, s, w.err, 0, nullptr, 0, nullptr, umma_dbg(), 0, 0};
+    // "128-lower" storage (staged epilogue only): Wh is always written and read that way; X is read that way from the
+    // second step on (X0 from sm_gather is a full image, a superset) and written that way except by the last update
+    // of a submatrix (fixed counts: the last step; convergence mode: per submatrix, s.last)
+    const int32_t lt = (sym == 2 && opt(OPT_UMMA_LT) != 0) ? 1 : 0;
+    a.lt_in = lt && k > 0; a.lt_out = lt;
     a.rev = 0;
     a.counter = dyn ? w.counters + 2 * k : nullptr;
     const UMaps m1{maps[k & 1].a, maps[k & 1].b}, m2{maps[k & 1].a, maps[2].b};
@@ -1303,6 +1380,8 @@ int32_t sign_umma(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, co
       SM_LAUNCHED();
     }
     a.Out = dst;
+    a.lt_in = lt;              // PHASE 2 reads X (lower from step 1 on; X0 is full, which is a superset) and Wh (lower)
+    a.lt_out = lt && k + 1 < max_iter;     // (convergence mode: an earlier last update is mirrored per submatrix, s.last)
     a.rev = rev_on;            // PHASE 2 starts where PHASE 1 ended, the next PHASE 1 where this launch ends
     a.counter = dyn ? w.counters + 2 * k + 1 : nullptr;
     rc = launch_umma_any<2>(bf16, mode, sym, nst, a, m2, n_sm, st);

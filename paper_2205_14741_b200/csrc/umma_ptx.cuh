@@ -392,9 +392,11 @@ __device__ __forceinline__ uint64_t make_sw128_mnmajor_desc(uint32_t smem_addr, 
 }
 // Instruction descriptor for kind::f16: D fp32 (bits [4,6) = 1), A/B format at [7,10)/[10,13)
 // (0 = fp16, 1 = bf16), both K-major (bits 15, 16 = 0), N>>3 at [17,23), M>>4 at [24,29).
-__host__ __device__ inline uint32_t make_idesc_f16(bool bf16, uint32_t M, uint32_t N, bool b_mn_major = false) {
+__host__ __device__ inline uint32_t make_idesc_f16(bool bf16, uint32_t M, uint32_t N, bool b_mn_major = false,
+                                                   bool a_mn_major = false) {
   uint32_t f = bf16 ? 1u : 0u;
-  return (1u << 4) | (f << 7) | (f << 10) | ((b_mn_major ? 1u : 0u) << 16) | ((N >> 3) << 17) | ((M >> 4) << 24);
+  return (1u << 4) | (f << 7) | (f << 10) | ((a_mn_major ? 1u : 0u) << 15) | ((b_mn_major ? 1u : 0u) << 16) |
+         ((N >> 3) << 17) | ((M >> 4) << 24);
 }
 
 }  // namespace ptx

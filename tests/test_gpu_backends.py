@@ -82,6 +82,12 @@ CASES = [
     ({"SM_UMMA_RESIDENT": "1"}, "f16", 64, (40, 6, 3, 4.0), 4, 3e-3, True, None),
     ({"SM_UMMA_RESIDENT": "1"}, "bf16", 64, (60, 23, 4, 3.2), 3, 2.5e-2, True, None),
     ({"SM_UMMA_RESIDENT": "0"}, "f16", 64, (300, 6, 3, 6.0), 5, 3e-3, True, None),
+    # staged epilogue (bulk stores) and "128-lower" storage with transposed (MN-major) operand reads
+    ({"SM_UMMA_EPI": "1"}, "bf16", 64, (90, 23, 4, 5.0), 3, 2.5e-2, True, None),
+    ({"SM_UMMA_EPI": "1", "SM_UMMA_RESIDENT": "0"}, "f16", 64, (300, 6, 3, 6.0), 5, 3e-3, True, None),
+    ({"SM_UMMA_EPI": "1", "SM_UMMA_LT": "1"}, "bf16", 64, (90, 23, 4, 5.0), 3, 2.5e-2, True, None),
+    ({"SM_UMMA_EPI": "1", "SM_UMMA_LT": "1", "SM_UMMA_RESIDENT": "0"}, "f16", 64, (300, 6, 3, 6.0), 5, 3e-3, True, None),
+    ({"SM_UMMA_EPI": "1", "SM_UMMA_LT": "1"}, "f16", 64, (40, 23, 4, 8.0), 4, 3e-3, True, None),
     ({"SM_UMMA_FUSED": "0", "SM_UMMA_NCTA": "2", "SM_UMMA_SYM": "1", "SM_UMMA_MC": "1"}, "bf16", 64, (90, 23, 4, 5.0), 3, 2.5e-2, True, M),
     ({"SM_UMMA_FUSED": "0", "SM_UMMA_NCTA": "2", "SM_UMMA_SYM": "1", "SM_UMMA_MC": "0"}, "bf16", 64, (90, 23, 4, 5.0), 3, 2.5e-2, True, M),
     ({"SM_UMMA_FUSED": "0", "SM_UMMA_NCTA": "2", "SM_UMMA_SYM": "1", "SM_UMMA_MC": "1", "SM_UMMA_REV": "0"}, "f16", 64, (90, 23, 4, 5.0), 3, 3e-3, True, M),
@@ -137,6 +143,9 @@ SYM_VARIANTS = [
     {"SM_UMMA_RESIDENT": "0", "SM_UMMA_DYN": "0"},
     {"SM_UMMA_RESIDENT": "0", "SM_UMMA_DYN": "0", "SM_UMMA_STAGES": "3"},
     {"SM_UMMA_RESIDENT": "0", "SM_UMMA_STREAM": "1"},
+    {"SM_UMMA_RESIDENT": "0", "SM_UMMA_EPI": "1"},
+    {"SM_UMMA_RESIDENT": "0", "SM_UMMA_EPI": "1", "SM_UMMA_DYN": "0"},
+    {"SM_UMMA_RESIDENT": "0", "SM_UMMA_EPI": "1", "SM_UMMA_LT": "1"},
 ]
 SYM_VARIANTS_MEASURE = [
     {"SM_UMMA_FUSED": "0", "SM_UMMA_NCTA": "2", "SM_UMMA_MC": "1"},
