@@ -30,9 +30,28 @@ if ROOT not in sys.path:
 
 from workloads.generator import CONFIGS, make_config  # noqa: E402
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel (mean of its PHASE 1 / PHASE 2 launches),
-# from the committed `ncu --set full` captures under profiles/ (r1c_ncu_full_k_umma_gemm_cfg{2,4}.md, r1b_ncu_full_k_dmma_gemm_cfg1.md).
-NCU_TRAFFIC_BYTES = {(2, "bf16"): 3.47e9, (4, "bf16"): 28.8e9, (1, "f64"): 0.72e9}
+# `roofline.traffic` (dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel) is NOT measured
+# by this program: it is read from profiles/r2_traffic.json, written by hand from the committed `ncu --set full`
+# captures, each entry naming the capture file and the commit of the kernel it profiled.  No entry -> null.
+def ncu_traffic(cfg_index, x_dtype, kernel):
+    p = os.path.join(ROOT, "profiles", "r2_traffic.json")
+    if not os.path.exists(p):
+        return None, None
+    with open(p) as f:
+        d = json.load(f)
+    e = d.get(f"cfg{cfg_index}_{x_dtype}_{kernel}")
+    return (e["dram_bytes_per_launch"], f"ncu capture {e['capture']} at commit {e['commit']}, not measured in this run") if e else (None, None)
+
+
+# Peaks of the dtypes MEASURED_PEAKS.json does not carry (fp16 tensor, fp32 FFMA, fp64 DMMA), measured on the box the
+# same way (torch.matmul 8192^3, burst = best of 10, sustained = back to back for 4 s) by `bench.py --measure-peaks`
+# and committed as profiles/r2_peaks.json; missing file -> the derived figures, labelled as such.
+def extra_peaks():
+    p = os.path.join(ROOT, "profiles", "r2_peaks.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            return json.load(f)
+    return None
 
 METRIC = "submatrix_sign_effective_tflops"
 UNIT = "TFLOP/s"
@@ -50,6 +69,9 @@ def parse_args():
     ap.add_argument("--h-dtype", default=None, choices=["f64", "f32"], help="storage type of the H values (default: f32 for 16-bit runs, f64 otherwise)")
     ap.add_argument("--chunk-elems", type=int, default=0, help="cap on the packed elements per chunk of sm_density (0: one chunk if it fits)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-also", action="store_true", help="skip the short configs[4] sub-record of the default run")
+    ap.add_argument("--measure-peaks", action="store_true", help="measure fp16 / fp32 / fp64 matmul peaks and print them as JSON")
+    ap.add_argument("--switch-iter", type=int, default=-1, help="bf16 -> fp16 precision schedule (f3): first fp16 update")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
 
@@ -58,6 +80,64 @@ def workload_stats(wl):
     cnt_dim = np.array([wl.blk_size[wl.col_idx[wl.row_ptr[i]:wl.row_ptr[i + 1]]].sum()
                         for i in range(wl.n_blk)], dtype=np.float64)
     return cnt_dim, float((cnt_dim ** 3).sum())
+
+
+def issued_flops_per_step(dims, pad, k_eff, resident_pd=256):
+    """Tensor-core FLOPs the 16-bit kernels ISSUE for one Newton-Schulz step of every submatrix (both products), with
+    padding, the lower-triangle tile selection and the identity MMAs of the update product -- what goes against the
+    hardware peak ("state both, never mix").  Mirrors the tile geometry of sign_umma.cu (128-row tiles,
+    columns up to the next multiple of 32 cut into equal tiles of <= 256) and of k_umma_resident (Pd <= 256)."""
+    total = 0.0
+    for m, k in zip(dims.astype(np.int64), k_eff):
+        m = int(m)
+        Pd = -(-m // pad) * pad
+        kmax = -(-m // 16) * 16
+        f = 0.0
+        if Pd <= resident_pd:
+            n0 = min(128, Pd)
+            f = 2.0 * 128 * n0 * kmax + (2.0 * 128 * Pd * kmax if Pd > 128 else 0.0)
+            f *= 2                                      # both products issue the same shapes
+        else:
+            n32 = -(-m // 32) * 32
+            for tm in range(-(-m // 128)):
+                nc = min(n32, 128 * (tm + 1))
+                tn_cnt = -(-nc // 256)
+                nb = -(-(-(-nc // 32)) // tn_cnt) * 32
+                for tn in range(tn_cnt):
+                    n_0 = tn * nb
+                    nt = min(nb, nc - n_0)
+                    f += 2 * (2.0 * 128 * nt * kmax)    # Y = X X^T and X Wh^T
+                    f += 2.0 * 128 * nt * 64            # "+ X": identity MMAs over the chunks that cover the tile's columns
+        total += f * float(k)
+    return total
+
+
+def measure_peaks():
+    """torch.matmul 8192^3 per dtype: burst (best of 10) and sustained (4 s back to back), as MEASURED_PEAKS.json does."""
+    import torch
+    out = {"how": "torch.matmul 8192^3 (2*N^3 FLOP): best of 10 (burst) and back to back for 4 s (sustained), CUDA events",
+           "gpu": torch.cuda.get_device_name(0), "torch": torch.__version__}
+    torch.backends.cuda.matmul.allow_tf32 = False
+    for name, dt in (("f16", torch.float16), ("bf16", torch.bfloat16), ("f32", torch.float32), ("f64", torch.float64)):
+        n = 8192 if name != "f64" else 4096
+        a = torch.randn(n, n, device="cuda", dtype=dt); b = torch.randn(n, n, device="cuda", dtype=dt)
+        for _ in range(3):
+            torch.matmul(a, b)
+        torch.cuda.synchronize()
+        best = 1e30
+        for _ in range(10):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(); torch.matmul(a, b); e1.record(); torch.cuda.synchronize()
+            best = min(best, e0.elapsed_time(e1))
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        reps = max(1, int(4000.0 / best))
+        e0.record()
+        for _ in range(reps):
+            torch.matmul(a, b)
+        e1.record(); torch.cuda.synchronize()
+        out[name] = {"n": n, "burst_tflops": 2.0 * n ** 3 / (best * 1e-3) / 1e12,
+                     "sustained_tflops": 2.0 * n ** 3 * reps / (e0.elapsed_time(e1) * 1e-3) / 1e12}
+    print(json.dumps(out), flush=True)
 
 
 def load_peaks():
@@ -341,38 +421,74 @@ def run_ours(args, cfg, cfg_run):
         return
 
     peaks = load_peaks()
+    xp = extra_peaks()
+    long_region = ms_total_max > 4000.0
     if is16:
-        # dominant kernel: k_umma_gemm.  Algorithmic FLOPs per launch = 2 sum m^3 (one m x m x m product per
-        # submatrix); launches inside the timed region = 2 * k * steps.  With SM_UMMA_FUSED=1 one launch of
-        # k_umma_fused runs all 2 k products, so the per-launch figure is the total over the timed launches.
-        long_region = ms_total_max > 4000.0
+        # dominant kernels: k_umma_resident (submatrices with Pd <= 256: all steps in one launch) and k_umma_gemm (one
+        # launch per product for the rest).  Algorithmic FLOPs of the timed launches = 4 sum m^3 k per step (true m, no
+        # padding, no symmetry discount); ISSUED FLOPs = what the MMAs of those launches compute (padding, lower
+        # triangle tiles only, identity MMAs).  frac = algorithmic / peak (may exceed the MMA rate: half the tiles are
+        # never issued), frac_issued = issued / peak (tensor-pipe view).  Peak: MEASURED_PEAKS.json bf16 (fp16 from
+        # profiles/r2_peaks.json when present, else the bf16 figure).
         peak = peaks["sustained"] if long_region else peaks["burst"]
+        peak_src = f"{peaks['src']} bf16 {'sustained' if long_region else 'burst'}"
+        if x_dtype == "f16" and xp and "f16" in xp:
+            peak = xp["f16"]["sustained_tflops" if long_region else "burst_tflops"]
+            peak_src = f"profiles/r2_peaks.json f16 {'sustained' if long_region else 'burst'}"
         flops_per_launch = flops_step * args.steps / max(gemm_launches, 1)
         avg_ms = gemm_ms / max(gemm_launches, 1)
         achieved = flops_per_launch / (avg_ms * 1e-3) / 1e12
-        fused = os.environ.get("SM_UMMA_FUSED", "0")[:1] == "1"
-        roofline = {"bound": "tensor", "kernel": "k_umma_fused" if fused else "k_umma_gemm", "achieved": achieved, "peak": peak,
+        issued_step = issued_flops_per_step(dims[order], pad, k_eff)
+        issued_per_launch = issued_step * args.steps / max(gemm_launches, 1)
+        n_res = int((np.ceil(dims / pad) * pad <= 256).sum())
+        kernel = "k_umma_resident" if n_res == wl.n_blk else ("k_umma_gemm" if n_res == 0 else "k_umma_gemm+k_umma_resident")
+        traffic, traffic_src = ncu_traffic(args.config, x_dtype, kernel)
+        roofline = {"bound": "tensor", "kernel": kernel, "achieved": achieved, "peak": peak,
                     "unit": "TFLOP/s", "frac": achieved / peak,
-                    "traffic": None if fused else NCU_TRAFFIC_BYTES.get((args.config, x_dtype)),
-                    "peak_source": f"{peaks['src']} bf16 {'sustained' if long_region else 'burst'}",
+                    "issued": issued_per_launch / (avg_ms * 1e-3) / 1e12, "frac_issued": issued_per_launch / (avg_ms * 1e-3) / 1e12 / peak,
+                    "traffic": traffic, "traffic_source": traffic_src,
+                    "peak_source": peak_src,
                     "launches_timed": gemm_launches, "avg_launch_ms": avg_ms,
-                    "algorithmic_flops_per_launch": flops_per_launch}
+                    "algorithmic_flops_per_launch": flops_per_launch, "issued_flops_per_launch": issued_per_launch,
+                    "note": "frac counts 2 m^3 per product although only the lower-triangle tiles are issued; frac_issued "
+                            "counts the MMAs actually issued (with padding) and is the tensor-pipe figure"}
     else:
-        # fp64: DMMA tensor path (k_dmma_gemm); fp32: FFMA (k_simt_gemm).  Peak derived:
-        # 148 SMs x 64 (fp64) / 128 (fp32) FMA per clock x 2 x 1.965 GHz.  Algorithmic FLOPs per launch = the
-        # products actually run: 2 sum_i m_i^3 k_i / (launches / 2 per step) -- convergence mode drops columns.
-        peak = 37.2 if x_dtype == "f64" else 74.4
+        # fp64: DMMA tensor path (k_dmma_gemm); fp32: FFMA (k_simt_gemm).  Peak measured (profiles/r2_peaks.json:
+        # cuBLAS 4096^3 fp64 / 8192^3 fp32 through torch.matmul) when present, else derived:
+        # 148 SMs x 64 (fp64) / 128 (fp32) FMA per clock x 2 x 1.965 GHz.  Algorithmic FLOPs per launch = the products
+        # actually run: 2 sum_i m_i^3 k_i / (launches / 2 per step) -- convergence mode drops columns.  The fp64 kernel
+        # computes lower-triangle tiles only: issued = algorithmic x (tiles computed / all tiles).
+        key = "f64" if x_dtype == "f64" else "f32"
+        if xp and key in xp:
+            peak = xp[key]["sustained_tflops" if long_region else "burst_tflops"]
+            peak_src = f"profiles/r2_peaks.json {key} {'sustained' if long_region else 'burst'} (torch.matmul)"
+        else:
+            peak = 37.2 if x_dtype == "f64" else 74.4
+            peak_src = "derived: 148 SMs x FMA lanes x 2 x 1.965 GHz"
         avg_ms = gemm_ms / max(gemm_launches, 1)
         flops_per_launch = flops_step * args.steps / max(gemm_launches, 1)
         achieved = flops_per_launch / (avg_ms * 1e-3) / 1e12
-        roofline = {"bound": "alu", "kernel": "k_dmma_gemm" if x_dtype == "f64" else "k_simt_gemm",
+        if x_dtype == "f64":
+            te = np.ceil(dims[order] / 128.0)
+            pd = np.ceil(dims[order] / pad) * pad
+            issued_step = float((2 * 2.0 * 128 * 128 * (te * (te + 1) / 2) * np.ceil(dims[order] / 16.0) * 16 * k_eff).sum()) \
+                if dims.max() > 96 else flops_step
+        else:
+            te = np.ceil(dims[order] / 64.0)
+            issued_step = float((2 * 2.0 * 64 * 64 * te * te * np.ceil(dims[order] / 16.0) * 16 * k_eff).sum())
+        issued_per_launch = issued_step * args.steps / max(gemm_launches, 1)
+        kernel = "k_dmma_gemm" if x_dtype == "f64" else "k_simt_gemm"
+        traffic, traffic_src = ncu_traffic(args.config, x_dtype, kernel)
+        roofline = {"bound": "tensor" if x_dtype == "f64" else "alu", "kernel": kernel,
                     "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-                    "traffic": NCU_TRAFFIC_BYTES.get((args.config, x_dtype)),
-                    "peak_source": "derived: 148 SMs x FMA lanes x 2 x 1.965 GHz",
+                    "issued": issued_per_launch / (avg_ms * 1e-3) / 1e12, "frac_issued": issued_per_launch / (avg_ms * 1e-3) / 1e12 / peak,
+                    "traffic": traffic, "traffic_source": traffic_src,
+                    "peak_source": peak_src,
                     "launches_timed": gemm_launches, "avg_launch_ms": avg_ms,
-                    "algorithmic_flops_per_launch": flops_per_launch,
-                    "note": "fp64 kernel computes lower-triangle tiles only (symmetric iterates): achieved counts the "
-                            "full 2 m^3 per product and may exceed the derived peak" if x_dtype == "f64" else None}
+                    "algorithmic_flops_per_launch": flops_per_launch, "issued_flops_per_launch": issued_per_launch,
+                    "note": ("fp64 kernel computes lower-triangle tiles only (symmetric iterates): frac counts the full 2 m^3 per "
+                             "product and may exceed the peak; frac_issued counts the tiles actually computed, with padding")
+                    if x_dtype == "f64" else "frac_issued counts the 64 x 64 tiles computed, with padding"}
 
     cpu = None
     if not args.no_cpu_baseline:
@@ -397,6 +513,20 @@ def run_ours(args, cfg, cfg_run):
         "stages": stages, "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e,
         "gpu_launches": int(launches), "clocks": clocks,
     }
+    # The metric is quoted on configs[2] AND configs[4]: the default run (configs[2]) carries a short configs[4] bf16
+    # measurement as a sub-record (own process after this one's GPU work is done; same contract: 3 warm-up steps,
+    # CUDA-event timing, clocks sampled during its timed region).
+    if world == 1 and args.config == 2 and not args.no_also:
+        del plan
+        torch.cuda.empty_cache()
+        try:
+            out = subprocess.run([sys.executable, os.path.abspath(__file__), "--config", "4", "--steps", "3", "--warmup", "3",
+                                  "--no-e2e", "--no-cpu-baseline", "--no-also"], capture_output=True, text=True, timeout=900)
+            sub = json.loads([ln for ln in out.stdout.splitlines() if ln.startswith("{")][-1])
+            line["also"] = {k: sub[k] for k in ("metric", "value", "unit", "steps", "warmup", "ms_per_step", "dtype", "config",
+                                                "block_columns_per_s", "stages", "roofline", "clocks", "gpu_launches")}
+        except Exception as e:      # the headline line must not depend on the sub-record
+            line["also"] = {"error": repr(e)[:300]}
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.barrier(); dist.destroy_process_group()
@@ -406,7 +536,9 @@ def main():
     args = parse_args()
     cfg = CONFIGS[args.config]
     cfg_run = cfg["runs"][args.run]
-    if args.impl == "reference":
+    if args.measure_peaks:
+        measure_peaks()
+    elif args.impl == "reference":
         run_reference(args, cfg, cfg_run)
     else:
         run_ours(args, cfg, cfg_run)
