@@ -263,3 +263,93 @@ def density_columns_lapack(w, mu: float = 0.0, cols=None, mode: str = "exact", k
         st.scale[ci] = gs
         st.n_neg[ci] = int((lam < 0).sum())
     return d, st
+
+
+# ---- non-orthogonal basis (PAPER.md:83 Eq. 12, :87 Eq. 13, :91 Eq. 14) --------------------
+# Reading A20: Eq. 12 as printed has "sign" on both sides; the matrix [[0, A^1/2], [A^-1/2, 0]] squares to
+# the identity, so it is its own sign and the printed relation is the known identity
+#     sign([[0, A], [I, 0]]) = [[0, A^1/2], [A^-1/2, 0]]      (A without eigenvalues on the closed negative real axis).
+
+def sign_block_matrix(T: np.ndarray) -> np.ndarray:
+    """sign(M), M = [[0, T], [I, 0]] (2m x 2m, NOT symmetric), by Eq. 13 written out on M itself:
+    sign(M) = M (M^2)^(-1/2).  M^2 = diag(T, T) is symmetric, so its inverse square root comes from the oracle's own
+    Jacobi eigendecomposition: (M^2)^(-1/2) = V diag(w^-1/2) V^T.  T must be symmetric positive definite."""
+    m = T.shape[0]
+    M = np.zeros((2 * m, 2 * m))
+    M[:m, m:] = T
+    M[m:, :m] = np.eye(m)
+    M2 = M @ M
+    w, V, _ = jacobi_eigh(0.5 * (M2 + M2.T))
+    if w.min() <= 0.0:
+        raise ValueError("sign_block_matrix: T is not positive definite")
+    return M @ ((V / np.sqrt(w)) @ V.T)
+
+
+def inv_sqrt_blocks(T: np.ndarray):
+    """(T^-1/2, T^1/2) = the lower-left and upper-right blocks of sign([[0, T], [I, 0]]) (Eq. 12), computed from the
+    Jacobi eigendecomposition of T itself (the same function of the same matrix as sign_block_matrix at an eighth of
+    the cost; tests/test_oracle_pins.py pins one against the other)."""
+    w, V, _ = jacobi_eigh(T)
+    if w.min() <= 0.0:
+        raise ValueError("inv_sqrt_blocks: T is not positive definite")
+    return (V / np.sqrt(w)) @ V.T, (V * np.sqrt(w)) @ V.T
+
+
+def _scatter_owned(w, i, Si, out):
+    """Insert the owned block column of the dense m x m result Si of column i into block-CSR values (PAPER.md:110 step 3)."""
+    blk = np.asarray(w.blk_size)
+    vp = np.asarray(w.val_ptr, dtype=np.int64)
+    nb = np.asarray(w.col_idx[w.row_ptr[i]:w.row_ptr[i + 1]])
+    offs = np.concatenate([[0], np.cumsum(blk[nb])])
+    own = int(np.where(nb == i)[0][0])
+    for a, j in enumerate(nb):
+        row = w.col_idx[w.row_ptr[j]:w.row_ptr[j + 1]]
+        p = int(w.row_ptr[j]) + int(np.searchsorted(row, i))
+        out[vp[p]:vp[p + 1]] = Si[offs[a]:offs[a + 1], offs[own]:offs[own + 1]].ravel()
+
+
+def inv_sqrt_columns(wS, cols=None, literal: bool = False):
+    """Submatrix method with f = the blocks of Eq. 12: for every listed block column i gather T_i(S),
+    evaluate sign([[0, T_i], [I, 0]]), and insert the owned columns of its lower-left block (T_i^-1/2) and of its
+    upper-right block (T_i^1/2) into two block-sparse results with S's pattern.  Returns (z_vals ~ S^-1/2,
+    y_vals ~ S^1/2, min eigenvalue of T_i per column).  literal=True evaluates Eq. 13 on the 2m x 2m matrix itself."""
+    vp = np.asarray(wS.val_ptr, dtype=np.int64)
+    z = np.zeros(int(vp[-1])); y = np.zeros(int(vp[-1]))
+    col_list = list(range(wS.n_blk)) if cols is None else [int(c) for c in cols]
+    lam_min = np.zeros(len(col_list))
+    for ci, i in enumerate(col_list):
+        T = gather(wS, i, 0.0)
+        m = T.shape[0]
+        if literal:
+            Sg = sign_block_matrix(T)
+            Zi, Yi = Sg[m:, :m], Sg[:m, m:]
+        else:
+            Zi, Yi = inv_sqrt_blocks(T)
+        lam_min[ci] = np.linalg.eigvalsh(T).min()
+        _scatter_owned(wS, i, Zi, z)
+        _scatter_owned(wS, i, Yi, y)
+    return z, y, lam_min
+
+
+def density_nonorth_columns(wH, wS, mu: float = 0.0, cols=None):
+    """Eq. 14, P = 1/2 (I - sign(S^-1 H - mu I)) S^-1, by the submatrix method on the pair (H, S) (same
+    block pattern): for every listed block column i, with T_H = T_i(H), T_S = T_i(S) gathered on the same index set,
+        Z = T_S^-1/2 (Eq. 12),  S^-1 = Z Z,  A = S^-1 T_H - mu I  (not symmetric),
+        sign(A) = Z sign(Z T_H Z - mu I) Z^-1   (A = Z (Z T_H Z - mu I) Z^-1 is similar to a symmetric matrix, whose
+                                                 sign is Eq. 13 on the spectrum, own Jacobi),
+        P_i = 1/2 (I - sign(A)) S^-1,
+    and the owned columns of P_i are inserted.  tests/test_oracle_pins.py pins sign(A) against Eq. 13 written out with
+    scipy.linalg.sqrtm on A itself."""
+    vp = np.asarray(wH.val_ptr, dtype=np.int64)
+    out = np.zeros(int(vp[-1]))
+    col_list = list(range(wH.n_blk)) if cols is None else [int(c) for c in cols]
+    for i in col_list:
+        TH = gather(wH, i, 0.0)
+        TS = gather(wS, i, 0.0)
+        Z, Y = inv_sqrt_blocks(TS)
+        Ht = Z @ TH @ Z
+        Ht = 0.5 * (Ht + Ht.T) - mu * np.eye(Ht.shape[0])
+        sgA = Z @ sign(Ht) @ Y                       # Y = T_S^1/2 = Z^-1
+        Pi = 0.5 * (np.eye(TH.shape[0]) - sgA) @ (Z @ Z)
+        _scatter_owned(wH, i, Pi, out)
+    return out

@@ -437,3 +437,106 @@ def test_oracle_matches_stored_golden():
         assert abs(now[k] - v) <= 1e-11 * max(1.0, abs(v)), (k, now[k], v)
     assert abs(stored["trace_full_coverage"] - 96.0) <= 1e-9
     assert stored["trace_sym"] == stored["trace"]
+
+
+# ---------------------------------------------------------------- f2: Eq. 12 / Eq. 14 with an overlap matrix
+
+def _with_vals(w, vals):
+    import copy
+    w2 = copy.copy(w)
+    w2.vals = vals
+    return w2
+
+
+def test_eq12_blocks_closed_forms_and_scipy():
+    """sign([[0, T], [I, 0]]) = [[0, T^1/2], [T^-1/2, 0]] (reading A20): diagonal T in closed form, the
+    result squares to I, its blocks are inverse to each other and square to T / T^-1, and they agree with
+    scipy.linalg.sqrtm and with scipy's sign function of the non-symmetric block matrix."""
+    import scipy.linalg as sl
+    d = np.array([0.25, 1.0, 4.0, 9.0])
+    Sg = orc.sign_block_matrix(np.diag(d))
+    assert np.allclose(Sg[4:, :4], np.diag(d ** -0.5), atol=1e-14) and np.allclose(Sg[:4, 4:], np.diag(d ** 0.5), atol=1e-14)
+    assert np.allclose(Sg[:4, :4], 0, atol=1e-14) and np.allclose(Sg[4:, 4:], 0, atol=1e-14)
+    rng = np.random.default_rng(3)
+    G = rng.standard_normal((9, 9))
+    T = G @ G.T + 0.5 * np.eye(9)
+    Sg = orc.sign_block_matrix(T)
+    Z, Y = Sg[9:, :9], Sg[:9, 9:]
+    assert np.abs(Sg @ Sg - np.eye(18)).max() < 1e-11                     # sign^2 = I
+    assert np.abs(Z @ Y - np.eye(9)).max() < 1e-11 and np.abs(Y @ Y - T).max() < 1e-11
+    assert np.abs(Z @ T @ Z - np.eye(9)).max() < 1e-11
+    assert np.abs(Y - sl.sqrtm(T).real).max() < 1e-11
+    M = np.block([[np.zeros((9, 9)), T], [np.eye(9), np.zeros((9, 9))]])
+    assert np.abs(Sg - sl.signm(M).real).max() < 1e-9                     # library sign of the block matrix itself
+    Zb, Yb = orc.inv_sqrt_blocks(T)                                       # the cheap form = the literal form
+    assert np.abs(Zb - Z).max() < 1e-12 and np.abs(Yb - Y).max() < 1e-12
+    with pytest.raises(ValueError):
+        orc.inv_sqrt_blocks(np.diag([1.0, -1.0]))
+
+
+def test_inv_sqrt_columns_limits_and_locality():
+    from workloads.generator import make_overlap
+    import scipy.linalg as sl
+    wl = make_config(0)
+    wS = make_overlap(wl)
+    ev = np.linalg.eigvalsh(wS.dense())
+    assert ev.min() > 0.3 and ev.max() < 2.0                              # the generator's S is s.p.d.
+    z, y, lam = orc.inv_sqrt_columns(wS)
+    assert lam.min() > 0
+    # literal Eq. 13 on the doubled matrix and the block form give the same columns
+    z2, y2, _ = orc.inv_sqrt_columns(wS, cols=[0, 17], literal=True)
+    m = orc.column_mask(wS, [0, 17])
+    assert np.abs(z[m] - z2[m]).max() < 1e-12 and np.abs(y[m] - y2[m]).max() < 1e-12
+    # locality: a subset of columns gives the same columns
+    z3, _, _ = orc.inv_sqrt_columns(wS, cols=[3, 9])
+    m = orc.column_mask(wS, [3, 9])
+    assert np.array_equal(z3[m], z[m])
+    # full-coverage limit: every T_i = S, so the result IS S^-1/2: Z S Z = I, Z = inverse of scipy's sqrtm
+    wf = make_config(0, cutoff=np.inf)
+    wSf = make_overlap(wf)
+    zf, yf, _ = orc.inv_sqrt_columns(wSf)
+    Zd, Yd, Sd = _with_vals(wSf, zf).dense(), _with_vals(wSf, yf).dense(), wSf.dense()
+    assert np.abs(Zd @ Sd @ Zd - np.eye(wSf.n)).max() < 1e-11
+    assert np.abs(Zd - np.linalg.inv(sl.sqrtm(Sd).real)).max() < 1e-11
+    assert np.abs(Yd @ Yd - Sd).max() < 1e-11
+    # block-diagonal limit: T_i = S_ii, the result is the inverse square root of every diagonal block
+    wb = make_config(0, cutoff=0.0)
+    wSb = make_overlap(wb)
+    zb, _, _ = orc.inv_sqrt_columns(wSb)
+    for i in (0, 31):
+        p = wb.row_ptr[i]
+        B = wSb.vals[wb.val_ptr[p]:wb.val_ptr[p + 1]].reshape(6, 6)
+        assert np.abs(zb[wb.val_ptr[p]:wb.val_ptr[p + 1]].reshape(6, 6) - np.linalg.inv(sl.sqrtm(B).real)).max() < 1e-12
+    # away from the limits the submatrix result approximates S^-1/2 (approximate method, PAPER.md:110)
+    Zs = _with_vals(wS, z).dense()
+    assert np.abs(Zs @ wS.dense() @ Zs - np.eye(wS.n)).max() < 5e-2
+
+
+def test_eq14_nonorthogonal_density():
+    """Eq. 14 with S != I: sign(S^-1 H - mu I) of the oracle (through the similarity to a symmetric matrix)
+    equals Eq. 13 written out on the non-symmetric matrix with scipy (A (A^2)^-1/2); in the full-coverage limit P is the
+    projector of the generalised eigenproblem H c = e S c (P S P = P, Tr(P S) = number of eigenvalues below mu, counted
+    independently by scipy.linalg.eigh); S = I reduces to the orthogonal path."""
+    from workloads.generator import make_overlap
+    import scipy.linalg as sl
+    wf = make_config(0, cutoff=np.inf)
+    wSf = make_overlap(wf)
+    Hd, Sd = wf.dense(), wSf.dense()
+    for mu in (0.0, 0.3):
+        P = _with_vals(wf, orc.density_nonorth_columns(wf, wSf, mu)).dense()
+        ev, Cg = sl.eigh(Hd, Sd)
+        occ = ev < mu
+        assert np.abs(P - Cg[:, occ] @ Cg[:, occ].T).max() < 1e-10
+        assert abs(np.trace(P @ Sd) - occ.sum()) < 1e-9
+        assert np.abs(P @ Sd @ P - P).max() < 1e-10
+        A = np.linalg.solve(Sd, Hd) - mu * np.eye(wf.n)                    # Eq. 13 on the non-symmetric A itself
+        sgA = A @ np.linalg.inv(sl.sqrtm(A @ A)).real
+        assert np.abs(P - 0.5 * (np.eye(wf.n) - sgA) @ np.linalg.inv(Sd)).max() < 1e-9
+    # S = I: Eq. 14 reduces to D = 1/2 (I - sign(H - mu I)), the orthogonal path of the same oracle
+    wl = make_config(0)
+    wI = _with_vals(wl, wl.vals * 0.0)
+    for i in range(wl.n_blk):
+        p = wl.row_ptr[i] + int(np.searchsorted(wl.col_idx[wl.row_ptr[i]:wl.row_ptr[i + 1]], i))
+        wI.vals[wl.val_ptr[p]:wl.val_ptr[p + 1]] = np.eye(6).ravel()
+    d0, _ = orc.density_columns(wl)
+    assert np.abs(orc.density_nonorth_columns(wl, wI, 0.0) - d0).max() < 1e-12

@@ -199,3 +199,39 @@ def sample_columns(wl: Workload, count: int, seed: int) -> np.ndarray:
     rng = np.random.Generator(np.random.PCG64(seed))
     count = min(count, wl.n_blk)
     return np.sort(rng.choice(wl.n_blk, size=count, replace=False)).astype(np.int32)
+
+
+def make_overlap(wl: Workload, seed: int = None, amp: float = 0.05, noise: float = 0.02) -> Workload:
+    """Seeded overlap matrix S with H's block pattern, for the non-orthogonal rows of SURVEY.md 8(f) f2 (PAPER.md:83-91,
+    Eq. 12-14): diagonal blocks I + symmetric N(0, noise) noise, off-diagonal blocks amp * exp(-r / 2 A) * N(0, 1) for the
+    same molecule pairs as H, S_ji = S_ij^T.  The amplitudes keep S symmetric positive definite (spectrum ~ 1 +- 0.4 on
+    the BASELINE geometries; the oracle asserts it).  Own RNG stream: seed + 500000 of the workload's seed."""
+    seed = int(wl.meta.get("seed", 0)) + 500000 if seed is None else seed
+    rng = np.random.Generator(np.random.PCG64(seed))
+    blk = np.asarray(wl.blk_size)
+    vp = np.asarray(wl.val_ptr, dtype=np.int64)
+    vals = np.zeros(int(vp[-1]))
+    box = wl.box
+    pos = wl.positions
+    for i in range(wl.n_blk):
+        bi = int(blk[i])
+        for p in range(int(wl.row_ptr[i]), int(wl.row_ptr[i + 1])):
+            j = int(wl.col_idx[p])
+            if j < i:
+                continue
+            bj = int(blk[j])
+            if j == i:
+                g = rng.standard_normal((bi, bi)) * noise
+                b_ = np.eye(bi) + 0.5 * (g + g.T)
+                vals[vp[p]:vp[p + 1]] = b_.ravel()
+            else:
+                d = pos[i] - pos[j]
+                d -= box * np.round(d / box)
+                r = float(np.sqrt((d * d).sum()))
+                b_ = rng.standard_normal((bi, bj)) * (amp * np.exp(-r / 2.0))
+                vals[vp[p]:vp[p + 1]] = b_.ravel()
+                row = wl.col_idx[wl.row_ptr[j]:wl.row_ptr[j + 1]]
+                q = int(wl.row_ptr[j]) + int(np.searchsorted(row, i))
+                vals[vp[q]:vp[q + 1]] = b_.T.ravel()
+    return Workload(n_blk=wl.n_blk, blk_size=wl.blk_size, row_ptr=wl.row_ptr, col_idx=wl.col_idx, val_ptr=wl.val_ptr,
+                    vals=vals, box=wl.box, positions=wl.positions, meta=dict(wl.meta, overlap_seed=seed))
