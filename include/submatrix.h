@@ -223,6 +223,36 @@ int32_t sm_mu_search(const sm_bcsr_t *A, const void *A_vals, int32_t a_dtype, do
                      int32_t d_dtype, void *D_vals, double *trace, int32_t *iters, double *residual,
                      double *scale, double *mu_out /*host*/, double *trace_out /*host*/,
                      int32_t *trials_out /*host*/, void *stream);
+/* ---- non-orthogonal basis (PAPER.md:83 Eq. 12, :87 Eq. 13, :91 Eq. 14) ----------------------------
+ * sm_inv_sqrt: Z ~ S^-1/2 (and optionally Y ~ S^1/2) of a symmetric positive definite block-sparse S by the submatrix
+ * method with f = the blocks of Eq. 12: for every block column i, T_i(S) is gathered (a2), the 2m x 2m matrix
+ * [[0, T_i], [I, 0]] / sqrt(Gershgorin bound of T_i) is iterated by the same Newton-Schulz kernels at doubled dimension
+ * with SM_SIGN_NONSYMMETRIC (a3), and the owned columns of its lower-left block T_i^-1/2 (upper-right: T_i^1/2) are
+ * inserted (a4).  All four x_dtype; tol > 0 = convergence mode, tol <= 0 = exactly max_iter steps.  Columns are processed
+ * in chunks of P->order whose DOUBLED images (dimension 2 m_i rounded up to pad_to) hold at most max_chunk_elems2
+ * elements (>= the largest one); h_dim is a HOST copy of P->dim.  Z_vals / Y_vals: block-CSR values with S's layout
+ * (z_dtype SM_F64 or SM_F32; Y_vals may be NULL); iters / residual / scale are [N] device arrays indexed by position in
+ * P->order (scale = the Gershgorin bound of T_i).  Not positive definite input is not detected: the iteration then
+ * does not converge (residual stays large).  Asynchronous. */
+int64_t sm_inv_sqrt_ws_bytes(const sm_bcsr_t *S, const sm_pattern_t *P, int32_t x_dtype, int64_t max_chunk_elems2);
+int32_t sm_inv_sqrt(const sm_bcsr_t *S, const void *S_vals, int32_t s_dtype, int32_t x_dtype, int32_t max_iter,
+                    double tol, const sm_pattern_t *P, const int32_t *h_dim /*host [N]*/, int64_t max_chunk_elems2,
+                    void *ws, int64_t ws_bytes, int32_t z_dtype, void *Z_vals, void *Y_vals, int32_t *iters,
+                    double *residual, double *scale, void *stream);
+/* sm_density_nonorth: Eq. 14 with S != I by the submatrix method on the pair (H, S) (one block pattern, two value
+ * arrays of type a_dtype): per block column, Z = T_S^-1/2 as in sm_inv_sqrt, S^-1 = Z Z, A = S^-1 T_H - mu I (not
+ * symmetric) scaled by its infinity norm, sign(A) by the non-symmetric Newton-Schulz kernels, P_i = 1/2 (I - sign(A)) S^-1,
+ * owned columns inserted (optionally symmetrised).  x_dtype = d_dtype = SM_F64 or SM_F32 (the dense products run on
+ * the DMMA / FFMA kernels; 16-bit: SM_ERR_UNSUPPORTED).  trace_ps (device fp64 scalar, may be NULL; synchronises once)
+ * receives Tr(P S), the electron count.  iters / residual / scale report the sign(A) iteration.  Asynchronous
+ * otherwise. */
+int64_t sm_density_nonorth_ws_bytes(const sm_bcsr_t *A, const sm_pattern_t *P, int32_t x_dtype, int64_t max_chunk_elems2);
+int32_t sm_density_nonorth(const sm_bcsr_t *A, const void *H_vals, const void *S_vals, int32_t a_dtype, double mu,
+                           int32_t x_dtype, int32_t max_iter, double tol, int32_t symmetrise, const sm_pattern_t *P,
+                           const int32_t *h_dim /*host [N]*/, int64_t max_chunk_elems2, void *ws, int64_t ws_bytes,
+                           int32_t d_dtype, void *P_vals, double *trace_ps, int32_t *iters, double *residual,
+                           double *scale, void *stream);
+
 /* R -> D = 1/2 (I - R) in place on block-CSR values, and Tr D (device fp64 scalar, may be NULL). */
 int32_t sm_density_from_sign(const sm_bcsr_t *A, const sm_pattern_t *P, int32_t d_dtype,
                              void *RD_vals, double *trace, void *stream);

@@ -33,7 +33,8 @@ EXPORTS = ["sm_last_cuda_error", "sm_pattern_sizes", "sm_build_pattern", "sm_pla
            "sm_gather_ws_bytes", "sm_gather", "sm_sign_ws_bytes", "sm_sign_ns", "sm_sign_status",
            "sm_scatter", "sm_symmetrise", "sm_density_ws_bytes", "sm_density", "sm_density_from_sign",
            "sm_mu_search", "sm_launch_count", "sm_profile_enable", "sm_profile_read", "sm_sign_ws_bytes_ex",
-           "sm_sign_ns_ex", "sm_set_option", "sm_get_option", "sm_build_info", "sm_last_device_error"]
+           "sm_sign_ns_ex", "sm_set_option", "sm_get_option", "sm_build_info", "sm_last_device_error",
+           "sm_inv_sqrt_ws_bytes", "sm_inv_sqrt", "sm_density_nonorth_ws_bytes", "sm_density_nonorth"]
 SM_SIGN_NONSYMMETRIC = 1
 
 
@@ -68,6 +69,8 @@ _lib.sm_launch_count.restype = C.c_int64
 _lib.sm_gather_ws_bytes.restype = C.c_int64
 _lib.sm_sign_ws_bytes.restype = C.c_int64
 _lib.sm_sign_ws_bytes_ex.restype = C.c_int64
+_lib.sm_inv_sqrt_ws_bytes.restype = C.c_int64
+_lib.sm_density_nonorth_ws_bytes.restype = C.c_int64
 _lib.sm_density_ws_bytes.restype = C.c_int64
 
 
@@ -334,6 +337,62 @@ def sm_density(A: Bcsr, P: Pattern, plan: DensityPlan, mu=0.0, scale_mode="gersh
         C.c_int64(plan.ws.numel()), C.c_int32(plan.d_dt), _ptr(plan.D), _ptr(plan.trace), _ptr(plan.iters),
         _ptr(plan.residual), _ptr(plan.scale), _stream()))
     return plan
+
+
+def _doubled_elems(P: Pattern):
+    """Elements of the doubled images (dimension 2 m_i rounded up to pad_to): buffer sizing only."""
+    m2 = 2 * P.dim.cpu().numpy().astype(np.int64)
+    p2 = (m2 + P.pad_to - 1) // P.pad_to * P.pad_to
+    return int((p2 * p2).sum()), int((p2 * p2).max())
+
+
+def sm_inv_sqrt(S: Bcsr, P: Pattern, x_dtype, max_iter=100, tol=0.0, max_chunk_elems2=None, z_dtype="f64", want_sqrt=False):
+    """f2 (Eq. 12): returns (Z ~ S^-1/2, Y ~ S^1/2 or None, iters, residual, scale), per-column arrays by position in P.order."""
+    x_dt, z_dt = DTYPES[x_dtype], DTYPES[z_dtype]
+    total2, largest2 = _doubled_elems(P)
+    mce = int(max_chunk_elems2 or total2)
+    mce = max(mce, largest2)
+    wsb = int(_lib.sm_inv_sqrt_ws_bytes(C.byref(S.c), C.byref(P.c), C.c_int32(x_dt), C.c_int64(mce)))
+    if wsb < 0:
+        raise SmError("sm_inv_sqrt_ws_bytes", wsb)
+    dev = S.device
+    ws = torch.empty(wsb, dtype=torch.uint8, device=dev)
+    Z = torch.zeros(S.n_vals, dtype=TORCH_DTYPE[z_dt], device=dev)
+    Y = torch.zeros(S.n_vals, dtype=TORCH_DTYPE[z_dt], device=dev) if want_sqrt else None
+    iters = torch.zeros(S.n_blk, dtype=torch.int32, device=dev)
+    residual = torch.zeros(S.n_blk, dtype=torch.float64, device=dev)
+    scale = torch.zeros(S.n_blk, dtype=torch.float64, device=dev)
+    h_dim = np.ascontiguousarray(P.dim.cpu().numpy(), dtype=np.int32)
+    _check("sm_inv_sqrt", _lib.sm_inv_sqrt(
+        C.byref(S.c), _ptr(S.vals), C.c_int32(S.val_dtype), C.c_int32(x_dt), C.c_int32(max_iter), C.c_double(tol),
+        C.byref(P.c), h_dim.ctypes.data_as(C.c_void_p), C.c_int64(mce), _ptr(ws), C.c_int64(ws.numel()), C.c_int32(z_dt),
+        _ptr(Z), _ptr(Y), _ptr(iters), _ptr(residual), _ptr(scale), _stream()))
+    return Z, Y, iters, residual, scale
+
+
+def sm_density_nonorth(A: Bcsr, S_vals, P: Pattern, x_dtype, mu=0.0, max_iter=100, tol=0.0, symmetrise=False,
+                       max_chunk_elems2=None):
+    """f2 (Eq. 14 with S != I): returns (P_vals, Tr(P S), iters, residual, scale)."""
+    x_dt = DTYPES[x_dtype]
+    total2, largest2 = _doubled_elems(P)
+    mce = max(int(max_chunk_elems2 or total2), largest2)
+    wsb = int(_lib.sm_density_nonorth_ws_bytes(C.byref(A.c), C.byref(P.c), C.c_int32(x_dt), C.c_int64(mce)))
+    if wsb < 0:
+        raise SmError("sm_density_nonorth_ws_bytes", wsb)
+    dev = A.device
+    ws = torch.empty(wsb, dtype=torch.uint8, device=dev)
+    Pv = torch.zeros(A.n_vals, dtype=TORCH_DTYPE[x_dt], device=dev)
+    tr = torch.zeros(1, dtype=torch.float64, device=dev)
+    iters = torch.zeros(A.n_blk, dtype=torch.int32, device=dev)
+    residual = torch.zeros(A.n_blk, dtype=torch.float64, device=dev)
+    scale = torch.zeros(A.n_blk, dtype=torch.float64, device=dev)
+    h_dim = np.ascontiguousarray(P.dim.cpu().numpy(), dtype=np.int32)
+    _check("sm_density_nonorth", _lib.sm_density_nonorth(
+        C.byref(A.c), _ptr(A.vals), _ptr(S_vals), C.c_int32(A.val_dtype), C.c_double(mu), C.c_int32(x_dt),
+        C.c_int32(max_iter), C.c_double(tol), C.c_int32(1 if symmetrise else 0), C.byref(P.c),
+        h_dim.ctypes.data_as(C.c_void_p), C.c_int64(mce), _ptr(ws), C.c_int64(ws.numel()), C.c_int32(x_dt), _ptr(Pv),
+        _ptr(tr), _ptr(iters), _ptr(residual), _ptr(scale), _stream()))
+    return Pv, tr, iters, residual, scale
 
 
 def sm_mu_search(A: Bcsr, P: Pattern, plan: DensityPlan, n_target, mu_lo, mu_hi, tol_n=1e-6, mu_tol=1e-12,

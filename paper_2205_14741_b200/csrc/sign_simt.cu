@@ -9,7 +9,7 @@ constexpr int ST = 64;    // output tile edge
 constexpr int SK = 16;    // k step
 constexpr int SPAD = 4;
 
-// PHASE 1: Y = X X, partial ||Y - I||_F^2.   PHASE 2: X' = 1.5 X - 0.5 X Y.
+// PHASE 1: Y = X X, partial ||Y - I||_F^2.   PHASE 2: X' = 1.5 X - 0.5 X Y.   PHASE 3: O = X Y (plain product, f2).
 template <typename T, int PHASE>
 __global__ void __launch_bounds__(256)
 k_simt_gemm(const int32_t *__restrict__ cols, const int64_t *__restrict__ col_off,
@@ -97,7 +97,9 @@ k_simt_gemm(const int32_t *__restrict__ cols, const int64_t *__restrict__ col_of
     for (int p = 0; p < 4; ++p) {
       int32_t gc = col0 + tx * 4 + p;
       if (gr < m && gc < m) {
-        if (PHASE == 1) {
+        if (PHASE == 3) {
+          O[(int64_t)gr * Pd + gc] = acc[q][p];
+        } else if (PHASE == 1) {
           O[(int64_t)gr * Pd + gc] = acc[q][p];
           double d = (double)acc[q][p] - (gr == gc ? 1.0 : 0.0);
           res += d * d;
@@ -241,7 +243,7 @@ k_dmma_gemm(const int32_t *__restrict__ cols, const int64_t *__restrict__ col_of
           if (PHASE == 1) {
             const double d = val - (gr == gc ? 1.0 : 0.0);
             res += ((!SYM || gr == gc) ? 1.0 : 2.0) * d * d;
-          } else {
+          } else if (PHASE == 2) {
             val = 1.5 * A[(int64_t)gr * Pd + gc] - 0.5 * val;
           }
           O[(int64_t)gr * Pd + gc] = val;
@@ -368,6 +370,32 @@ static int32_t sign_simt_t(const sm_pattern_t *P, const int32_t *cols, int32_t n
   }
   dim3 cg(n_cols, 8);
   k_copy_back<<<cg, 256, 0, st>>>(cols, col_off, iters, (int32_t)sizeof(T), P->dim_pad, 0, (const char *)w.X2, (char *)X);
+  SM_LAUNCHED();
+  return SM_OK;
+}
+
+// O_c = A_c B_c for every listed submatrix (row-major packed buffers, zero padding; true products on all tiles).
+// `active` is a device array of n_cols ones (the kernels' per-submatrix switch).  Used by sm_density_nonorth (f2).
+int32_t dense_product(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, const int64_t *col_off, int32_t x_dtype,
+                      const void *A, const void *B, void *O, int32_t *active, int32_t *last_zero, cudaStream_t st) {
+  SignState s{active, last_zero, nullptr, nullptr, 0};
+  const bool dmma = x_dtype == SM_F64 && opt(OPT_F64_SIMT) == 0 && P->max_dim > 96;
+  const int32_t TS = dmma ? DT : ST;
+  const int32_t edge = (P->max_dim + TS - 1) / TS;
+  const int64_t grid64 = (int64_t)n_cols * edge * edge;
+  if (grid64 > 0x7fffffffLL) return SM_ERR_UNSUPPORTED;
+  const int32_t grid = (int32_t)grid64;
+  if (dmma) {
+    SM_CUDA(cudaFuncSetAttribute(k_dmma_gemm<3, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, DMMA_SMEM));
+    k_dmma_gemm<3, false><<<grid, 256, DMMA_SMEM, st>>>(cols, col_off, P->dim, P->dim_pad, edge, (const double *)A,
+                                                        (const double *)B, (double *)O, s);
+  } else if (x_dtype == SM_F64) {
+    k_simt_gemm<double, 3><<<grid, 256, 0, st>>>(cols, col_off, P->dim, P->dim_pad, edge, (const double *)A, (const double *)B, (double *)O, s);
+  } else if (x_dtype == SM_F32) {
+    k_simt_gemm<float, 3><<<grid, 256, 0, st>>>(cols, col_off, P->dim, P->dim_pad, edge, (const float *)A, (const float *)B, (float *)O, s);
+  } else {
+    return SM_ERR_UNSUPPORTED;
+  }
   SM_LAUNCHED();
   return SM_OK;
 }

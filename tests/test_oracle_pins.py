@@ -5,6 +5,8 @@ forms, invariants of Eq. 13 / Eq. 14, limits in which the
 submatrix method is exact, library routines (LAPACK eigh, scipy
 signm, LDL^T inertia) and brute force on tiny inputs.
 """
+import os
+
 import numpy as np
 import pytest
 import scipy.linalg
@@ -540,3 +542,26 @@ def test_eq14_nonorthogonal_density():
         wI.vals[wl.val_ptr[p]:wl.val_ptr[p + 1]] = np.eye(6).ravel()
     d0, _ = orc.density_columns(wl)
     assert np.abs(orc.density_nonorth_columns(wl, wI, 0.0) - d0).max() < 1e-12
+
+
+def test_lapack_variant_is_pinned_to_jacobi_at_configs4_size():
+    """The full-size configs[2] / configs[4] parity tests use oracle.density_columns_lapack; BASELINE.json names the
+    Jacobi oracle.  tests/golden/cfg4_jacobi_vs_lapack.txt records one configs[4] column (m ~ 1600) through BOTH (written
+    by tests/golden/make_cfg4_jacobi_pin.py from oracle/ alone, ~5 min of Jacobi sweeps): they agree to 1e-10.
+    RUN_SLOW=1 repeats the comparison instead of reading the record."""
+    import importlib.util
+    here = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+    if os.environ.get("RUN_SLOW") == "1":
+        spec = importlib.util.spec_from_file_location("make_cfg4_jacobi_pin", os.path.join(here, "make_cfg4_jacobi_pin.py"))
+        mod = importlib.util.module_from_spec(spec)
+        spec.loader.exec_module(mod)
+        rec = mod.compare()
+    else:
+        rec = {}
+        for ln in open(os.path.join(here, "cfg4_jacobi_vs_lapack.txt")):
+            if not ln.startswith("#"):
+                k, v = ln.split(None, 1)
+                rec[k] = float(v)
+    assert rec["m"] >= 1200                                   # a large-submatrix-regime column, not a small one
+    assert rec["max_abs_diff"] <= 1e-10
+    assert rec["frobenius_jacobi"] > 1.0                      # a real block column of D, not zeros
