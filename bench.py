@@ -292,7 +292,7 @@ def run_ours(args, cfg, cfg_run):
         # a1 runs every step; its size query (a validation pass plus a read-back that synchronises the stream) is
         # per geometry and was done once above
         Pn = sm.sm_build_pattern(A, pad, sizes=P.sizes)
-        sm.sm_density(A, Pn, plan, mu=0.0, scale_mode=scale_mode, max_iter=max_iter, tol=tol, symmetrise=True)
+        sm.sm_density(A, Pn, plan, mu=0.0, scale_mode=scale_mode, max_iter=max_iter, tol=tol, symmetrise=True, switch_iter=args.switch_iter)
         return Pn
 
     for _ in range(args.warmup):
@@ -340,8 +340,9 @@ def run_ours(args, cfg, cfg_run):
             (X, sc), stages["gather_ms"] = timed(lambda: sm.sm_gather(A, Pn, cols, col_off, n, 0.0, scale_mode, x_dtype, X=X))
             ws = torch.empty(sm.sm_sign_ws_bytes(Pn, n, Pn.packed_elems, x_dtype), dtype=torch.uint8, device="cuda")
             _, stages["sign_ms"] = timed(lambda: sm.sm_sign_ns(Pn, cols, col_off, n, Pn.packed_elems, x_dtype, X,
-                                                               max_iter, tol, ws=ws))
-            R, stages["scatter_ms"] = timed(lambda: sm.sm_scatter(A, Pn, cols, col_off, n, x_dtype, X, "f64",
+                                                               max_iter, tol, ws=ws, switch_iter=args.switch_iter))
+            s_dtype = "f16" if args.switch_iter >= 0 else x_dtype
+            R, stages["scatter_ms"] = timed(lambda: sm.sm_scatter(A, Pn, cols, col_off, n, s_dtype, X, "f64",
                                                                  R=plan.D, symmetrise=True))
             _, stages["density_ms"] = timed(lambda: sm.sm_density_from_sign(A, Pn, R))
             stages["sign_tflops"] = flops_step / (stages["sign_ms"] * 1e-3) / 1e12
@@ -390,7 +391,7 @@ def run_ours(args, cfg, cfg_run):
             s_main.wait_event(ev_in[b_])
             s_main.wait_event(ev_out[b_])               # this buffer's previous result has left the device
             Pn = sm.sm_build_pattern(Ab, pad, sizes=P.sizes)
-            sm.sm_density(Ab, Pn, pb, mu=0.0, scale_mode=scale_mode, max_iter=max_iter, tol=tol, symmetrise=True)
+            sm.sm_density(Ab, Pn, pb, mu=0.0, scale_mode=scale_mode, max_iter=max_iter, tol=tol, symmetrise=True, switch_iter=args.switch_iter)
             ev_done[b_].record(s_main)
             with torch.cuda.stream(s_out):
                 s_out.wait_event(ev_done[b_])
@@ -505,6 +506,7 @@ def run_ours(args, cfg, cfg_run):
         "vs_baseline": None, "dtype": x_dtype, "data": "synthetic",
         "config": {"workload": cfg["name"], "n_mol": cfg["n_mol"], "orbitals": cfg["b"], "cutoff_A": cfg["cutoff"],
                    "x_dtype": x_dtype, "max_iter": max_iter, "tol": tol, "scale_mode": scale_mode, "h_dtype": h_dtype, "pad_to": pad,
+                   "switch_iter": args.switch_iter,
                    "l2": "inputs_exceed_l2" if P.packed_elems * eb > 200e6 else "inputs_fit_l2",
                    "chunks": int(-(-P.packed_elems // max_chunk))},
         "block_columns_per_s": world * wl.n_blk / (ms_per_step * 1e-3),

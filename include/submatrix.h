@@ -206,6 +206,15 @@ int32_t sm_density(const sm_bcsr_t *A, const void *A_vals, int32_t a_dtype, doub
                    int64_t max_chunk_elems, void *ws, int64_t ws_bytes, int32_t d_dtype,
                    void *D_vals, double *trace, int32_t *iters, double *residual, double *scale,
                    void *stream);
+/* sm_density with a precision schedule (SURVEY 8(f) f3; PAPER.md:104 "FP16 operations with FP32 accumulation", :15):
+ * switch_iter >= 0 (x_dtype SM_BF16, tol <= 0, 0 < switch_iter < max_iter) runs the first switch_iter updates on bf16
+ * operands and the rest on fp16 operands (see sm_sign_ns_ex); switch_iter < 0 is sm_density. */
+int32_t sm_density_ex(const sm_bcsr_t *A, const void *A_vals, int32_t a_dtype, double mu,
+                      int32_t x_dtype, int32_t scale_mode, int32_t max_iter, double tol, int32_t switch_iter,
+                      int32_t symmetrise, const sm_pattern_t *P, const int32_t *h_dim_pad /*host [N]*/,
+                      int64_t max_chunk_elems, void *ws, int64_t ws_bytes, int32_t d_dtype,
+                      void *D_vals, double *trace, int32_t *iters, double *residual, double *scale,
+                      void *stream);
 /* Chemical potential for a fixed electron count (the first row past the hot path).
  * Eq. 14 carries mu but the paper gives no rule for it; the usual closure is the electron count
  * Tr D(mu) = n_target (with S = I, D = 1/2 (I - sign(H - mu I)) counts the eigenvalues below mu),

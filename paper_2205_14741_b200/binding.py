@@ -34,7 +34,7 @@ EXPORTS = ["sm_last_cuda_error", "sm_pattern_sizes", "sm_build_pattern", "sm_pla
            "sm_scatter", "sm_symmetrise", "sm_density_ws_bytes", "sm_density", "sm_density_from_sign",
            "sm_mu_search", "sm_launch_count", "sm_profile_enable", "sm_profile_read", "sm_sign_ws_bytes_ex",
            "sm_sign_ns_ex", "sm_set_option", "sm_get_option", "sm_build_info", "sm_last_device_error",
-           "sm_inv_sqrt_ws_bytes", "sm_inv_sqrt", "sm_density_nonorth_ws_bytes", "sm_density_nonorth"]
+           "sm_inv_sqrt_ws_bytes", "sm_inv_sqrt", "sm_density_nonorth_ws_bytes", "sm_density_nonorth", "sm_density_ex"]
 SM_SIGN_NONSYMMETRIC = 1
 
 
@@ -325,11 +325,19 @@ class DensityPlan:
 
 
 def sm_density(A: Bcsr, P: Pattern, plan: DensityPlan, mu=0.0, scale_mode="gershgorin", max_iter=100,
-               tol=0.0, symmetrise=False, A_vals=None):
+               tol=0.0, symmetrise=False, A_vals=None, switch_iter=-1):
     """Whole path; returns the plan (D, trace, iters, residual, scale live in it; the per-column
-    arrays are indexed by position in P.order)."""
+    arrays are indexed by position in P.order).  switch_iter >= 0: bf16 -> fp16 schedule (sm_density_ex)."""
     sc = SCALES[scale_mode] if isinstance(scale_mode, str) else scale_mode
     vals = A.vals if A_vals is None else A_vals
+    if switch_iter >= 0:
+        _check("sm_density_ex", _lib.sm_density_ex(
+            C.byref(A.c), _ptr(vals), C.c_int32(A.val_dtype), C.c_double(mu), C.c_int32(plan.x_dt), C.c_int32(sc),
+            C.c_int32(max_iter), C.c_double(tol), C.c_int32(switch_iter), C.c_int32(1 if symmetrise else 0), C.byref(P.c),
+            plan.h_dim_pad.ctypes.data_as(C.c_void_p), C.c_int64(plan.max_chunk_elems), _ptr(plan.ws),
+            C.c_int64(plan.ws.numel()), C.c_int32(plan.d_dt), _ptr(plan.D), _ptr(plan.trace), _ptr(plan.iters),
+            _ptr(plan.residual), _ptr(plan.scale), _stream()))
+        return plan
     _check("sm_density", _lib.sm_density(
         C.byref(A.c), _ptr(vals), C.c_int32(A.val_dtype), C.c_double(mu), C.c_int32(plan.x_dt), C.c_int32(sc),
         C.c_int32(max_iter), C.c_double(tol), C.c_int32(1 if symmetrise else 0), C.byref(P.c),

@@ -210,6 +210,16 @@ extern "C" int32_t sm_density(const sm_bcsr_t *A, const void *A_vals, int32_t a_
                               int64_t max_chunk_elems, void *ws, int64_t ws_bytes, int32_t d_dtype,
                               void *D_vals, double *trace, int32_t *iters, double *residual, double *scale,
                               void *stream) {
+  return sm_density_ex(A, A_vals, a_dtype, mu, x_dtype, scale_mode, max_iter, tol, -1, symmetrise, P, h_dim_pad,
+                       max_chunk_elems, ws, ws_bytes, d_dtype, D_vals, trace, iters, residual, scale, stream);
+}
+
+extern "C" int32_t sm_density_ex(const sm_bcsr_t *A, const void *A_vals, int32_t a_dtype, double mu,
+                                 int32_t x_dtype, int32_t scale_mode, int32_t max_iter, double tol, int32_t switch_iter,
+                                 int32_t symmetrise, const sm_pattern_t *P, const int32_t *h_dim_pad,
+                                 int64_t max_chunk_elems, void *ws, int64_t ws_bytes, int32_t d_dtype,
+                                 void *D_vals, double *trace, int32_t *iters, double *residual, double *scale,
+                                 void *stream) {
   if (!A || !A_vals || !P || !h_dim_pad || !ws || !D_vals || !iters || !residual || !scale) return SM_ERR_ARG;
   if (dtype_bytes(x_dtype) == 0) return SM_ERR_UNSUPPORTED;
   if (d_dtype != SM_F64 && d_dtype != SM_F32) return SM_ERR_UNSUPPORTED;
@@ -239,10 +249,11 @@ extern "C" int32_t sm_density(const sm_bcsr_t *A, const void *A_vals, int32_t a_
     rc = sm_gather(A, A_vals, a_dtype, P, cols, nc, w.col_off, mu, scale_mode, x_dtype, w.X, scale + lo, w.gws,
                    w.gws_bytes, stream);
     if (rc != SM_OK) return rc;
-    rc = sm_sign_ns(P, cols, nc, w.col_off, elems, x_dtype, w.X, w.sws, w.sws_bytes, max_iter, tol, iters + lo,
-                    residual + lo, stream);
+    rc = sm_sign_ns_ex(P, cols, nc, w.col_off, elems, x_dtype, w.X, w.sws, w.sws_bytes, max_iter, tol, 0, switch_iter,
+                       iters + lo, residual + lo, stream);
     if (rc != SM_OK) return rc;
-    rc = sm_scatter(A, P, cols, nc, w.col_off, x_dtype, w.X, d_dtype, D_vals, 0, stream);
+    // after a bf16 -> fp16 schedule the images hold fp16
+    rc = sm_scatter(A, P, cols, nc, w.col_off, switch_iter >= 0 ? SM_F16 : x_dtype, w.X, d_dtype, D_vals, 0, stream);
     if (rc != SM_OK) return rc;
     lo = hi;
   }

@@ -113,6 +113,7 @@ struct UArgs {
   // lt_out: the output is written that way (no mirrored pieces below the diagonal squares).  The last update of a
   // submatrix writes the full image (lt_out = 0, or s.last in convergence mode): sm_scatter reads whole rows.
   int32_t lt_in, lt_out;
+  int32_t out_f16;           // precision schedule (f3): this launch reads bf16 operands and rounds its output to fp16
 };
 
 // Tile geometry.  Only elements (r, c) with c <= r are computed, so tile row tm (rows tm*R ..
@@ -765,7 +766,7 @@ k_umma_gemm(UArgs a, const __grid_constant__ CUtensorMap mapA, const __grid_cons
                   }
                   f0 *= -0.5f; f1 *= -0.5f;                 // Wh = -1/2 W is what PHASE 2 multiplies by
                 }
-                o[ti][tj] = pack2<BF16>(f0, f1);
+                o[ti][tj] = (BF16 && !a.out_f16) ? pack2<true>(f0, f1) : pack2<false>(f0, f1);
               }
             }
             if (p1) { if (diag) res += acc; else res2 += acc; }
@@ -928,7 +929,8 @@ k_umma_gemm(UArgs a, const __grid_constant__ CUtensorMap mapA, const __grid_cons
               for (int e = 0; e < 8; ++e) f[e] *= -0.5f;           // Wh = -1/2 W is what PHASE 2 multiplies by
             }
 #pragma unroll
-            for (int e2 = 0; e2 < 4; ++e2) o[g * 4 + e2] = pack2<BF16>(f[2 * e2], f[2 * e2 + 1]);
+            for (int e2 = 0; e2 < 4; ++e2)
+              o[g * 4 + e2] = (BF16 && !a.out_f16) ? pack2<true>(f[2 * e2], f[2 * e2 + 1]) : pack2<false>(f[2 * e2], f[2 * e2 + 1]);
           }
           if (p1 && r < u.m) { if (SYM && !diag) res2 += acc; else res += acc; }
           uint16_t *Orow = Og ? Og + rowoff : nullptr;
@@ -1273,7 +1275,6 @@ int32_t sign_umma(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, co
     if (rc != SM_OK) return rc;
     if (res_pd >= P->max_dim_pad) return SM_OK;          // every listed column was resident
   }
-  if (switch_iter >= 0) return SM_ERR_UNSUPPORTED;        // the mixed schedule exists in the resident kernel only (Pd <= 256)
 
   // ---- the rest: grouped tiles, one launch per product (or stream / fused)
   SignState s{w.active, w.last, w.n_still, w.partial, w.parts_per_col};
@@ -1339,11 +1340,11 @@ int32_t sign_umma(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, co
   // the drift that made the deep ring costly (configs[4], 25 steps: 603 ms with 4 stages, 615 ms with 3)
   const int32_t nst = nst_opt ? nst_opt : (mode == 4 ? 6 : ((!dyn && P->max_dim > 1024) ? 3 : 4));
   if (dyn) SM_CUDA(cudaMemsetAsync(w.counters, 0, sizeof(unsigned long long) * UMMA_MAX_COUNTERS, st));
-  if (opt(OPT_UMMA_STREAM) == 1 && dyn && !(tol > 0.0) && max_iter > 0) {
+  if (opt(OPT_UMMA_STREAM) == 1 && dyn && !(tol > 0.0) && max_iter > 0 && switch_iter < 0) {
     const int64_t n_done = (int64_t)(n_cols / STREAM_G + 1) * 2 * max_iter;
     SM_CUDA(cudaMemsetAsync(w.done, 0, sizeof(int32_t) * n_done, st));
     UArgs a{cols, col_off, P->dim, P->dim_pad, w.tile_ptr, w.tiles, n_cols, 0, X, w.Y, w.X2, s, w.err, 0, w.counters,
-            2 * max_iter, w.done, umma_dbg(), 0, 0};
+            2 * max_iter, w.done, umma_dbg(), 0, 0, 0};
     int32_t rc = launch_umma_t<0, 1, true, false, 0, false, true>(bf16, a, maps[0], n_sm, st);
     if (rc != SM_OK) return rc;
     k_fused_post<<<(n_cols + 7) / 8, 256, 0, st>>>(n_cols, cols, P->dim, P->dim_pad, res_pd, w.partial, w.parts_per_col, w.n_parts,
@@ -1358,7 +1359,7 @@ int32_t sign_umma(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, co
   void *buf[2] = {X, w.X2};
   for (int32_t k = 0; k < max_iter; ++k) {
     void *src = buf[k & 1], *dst = buf[(k + 1) & 1];
-    UArgs a{cols, col_off, P->dim, P->dim_pad, w.tile_ptr, w.tiles, n_cols, tol > 0.0 ? 1 : 0, src, w.Y, w.Y, s, w.err, 0, nullptr, 0, nullptr, umma_dbg(), 0, 0};
+    UArgs a{cols, col_off, P->dim, P->dim_pad, w.tile_ptr, w.tiles, n_cols, tol > 0.0 ? 1 : 0, src, w.Y, w.Y, s, w.err, 0, nullptr, 0, nullptr, umma_dbg(), 0, 0, 0};
     // "128-lower" storage (staged epilogue only): Wh is always written and read that way; X is read that way from the
     // second step on (X0 from sm_gather is a full image, a superset) and written that way except by the last update
     // of a submatrix (fixed counts: the last step; convergence mode: per submatrix, s.last)
@@ -1367,7 +1368,9 @@ int32_t sign_umma(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, co
     a.rev = 0;
     a.counter = dyn ? w.counters + 2 * k : nullptr;
     const UMaps m1{maps[k & 1].a, maps[k & 1].b}, m2{maps[k & 1].a, maps[2].b};
-    int32_t rc = launch_umma_any<1>(bf16, mode, sym, nst, a, m1, n_sm, st);
+    // precision schedule (f3): updates 0 .. switch_iter-1 run on bf16 operands, update switch_iter-1 rounds X' to fp16
+    const bool bf16_k = bf16 && (switch_iter < 0 || k < switch_iter);
+    int32_t rc = launch_umma_any<1>(bf16_k, mode, sym, nst, a, m1, n_sm, st);
     if (rc != SM_OK) return rc;
     if (tol > 0.0) {
       SM_CUDA(cudaMemsetAsync(w.n_still, 0, sizeof(int32_t), st));
@@ -1384,7 +1387,8 @@ int32_t sign_umma(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, co
     a.lt_out = lt && k + 1 < max_iter;     // (convergence mode: an earlier last update is mirrored per submatrix, s.last)
     a.rev = rev_on;            // PHASE 2 starts where PHASE 1 ended, the next PHASE 1 where this launch ends
     a.counter = dyn ? w.counters + 2 * k + 1 : nullptr;
-    rc = launch_umma_any<2>(bf16, mode, sym, nst, a, m2, n_sm, st);
+    a.out_f16 = (bf16_k && k + 1 == switch_iter) ? 1 : 0;
+    rc = launch_umma_any<2>(bf16_k, mode, sym, nst, a, m2, n_sm, st);
     if (rc != SM_OK) return rc;
     if (tol > 0.0 && k >= 5 && (k & 1)) {
       int32_t still = 1;

@@ -479,6 +479,44 @@ def test_cfg4_16bit_full_size_sampled(sm, x_dtype, scale_mode, val_dtype):
     assert e["total"] <= 2e-2 and e["dtr"] <= 1e-3, e
 
 
+def test_precision_schedule_bf16_to_fp16(sm):
+    # bf16 operands for the first updates, fp16 operands for the rest.  Rounding
+    # errors that anticommute with sign(T) are neither damped nor amplified by the iteration, so what the
+    # late fp16 steps buy is that THEY add 8x less of it; what remains is the one rounding of X0 to bf16 (measured on
+    # configs[2], 48 columns: rounding 7.6e-3 all bf16, 4.9e-3 with fp16 from the second update on, 9.7e-4 all fp16), so
+    # the useful schedule switches right after the first update.  Checked on a workload that mixes resident
+    # (Pd <= 256) and grouped submatrices, and on configs[2] in bench.py's configuration.
+    wl = make_workload(120, np.array([23, 6, 23, 6] * 30), np.array([4, 3, 4, 3] * 30), 5.0, seed=51)
+    A = sm.Bcsr(wl)
+    P = sm.sm_build_pattern(A, 64)
+    assert P.max_dim_pad > 256 and int((P.dim_pad <= 256).sum().item()) > 0
+    cols = np.arange(wl.n_blk, dtype=np.int32)
+    out = {}
+    for sw in (-1, 1):
+        plan = sm.DensityPlan(A, P, "bf16")
+        sm.sm_density(A, P, plan, mu=0.0, scale_mode="global", max_iter=20, tol=0.0, symmetrise=False, switch_iter=sw)
+        torch.cuda.synchronize()
+        assert (plan.iters == 20).all()
+        out[sw] = sampled_errors(wl, P, plan, cols, 20, label=f"mixed-size workload, switch_iter {sw}")
+    assert out[1]["total"] <= 2e-2 and out[1]["dtr"] <= 1e-3
+    assert out[1]["rounding"] <= 0.85 * out[-1]["rounding"], out
+    with pytest.raises(sm.SmError):                       # the schedule needs bf16 input and a fixed iteration count
+        sm.sm_density(A, P, sm.DensityPlan(A, P, "f16"), max_iter=20, tol=0.0, switch_iter=12)
+
+
+def test_cfg2_precision_schedule_full_size(sm):
+    wl = make_config(2)
+    run = CONFIGS[2]["runs"][0]
+    A = sm.Bcsr(wl, val_dtype="f32")
+    P = sm.sm_build_pattern(A, 64)
+    plan = sm.DensityPlan(A, P, "bf16")
+    sm.sm_density(A, P, plan, mu=0.0, scale_mode="global", max_iter=run["max_iter"], tol=0.0, symmetrise=False, switch_iter=1)
+    torch.cuda.synchronize()
+    e = sampled_errors(wl, P, plan, sample_columns(wl, 128, 4242), run["max_iter"], label="cfg2 bf16 -> fp16 after the first update")
+    assert e["total"] <= 2e-2 and e["dtr"] <= 1e-3, e
+    assert e["rounding"] <= 6.5e-3, e         # all bf16: 8.7e-3 on the same sample
+
+
 def test_cfg4_fp64_full_size_sm_density(sm):
     # the full-size fp64 run that bench.py --config 4 --run 2 times (25 fixed steps, chunked: one fp64 buffer is 48 GB),
     # checked on 4 columns by protocol (alpha): against the oracle's NS-25 polynomial at the GPU's own scales (A13)
