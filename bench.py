@@ -68,6 +68,8 @@ def parse_args():
     ap.add_argument("--scale", default=None, help="none|gershgorin|power|global (default: global for 16-bit, gershgorin otherwise)")
     ap.add_argument("--h-dtype", default=None, choices=["f64", "f32"], help="storage type of the H values (default: f32 for 16-bit runs, f64 otherwise)")
     ap.add_argument("--chunk-elems", type=int, default=0, help="cap on the packed elements per chunk of sm_density (0: one chunk if it fits)")
+    ap.add_argument("--gapped", action="store_true", help="the gapped 23-orbital workload (non-overlapping molecules, f4) with the config's sizes")
+    ap.add_argument("--shard", action="store_true", help="N > 1: ONE workload with its block columns sharded over the ranks and an all-gather of the column-owned D blocks (strong scaling, f4) instead of independent replicas")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-also", action="store_true", help="skip the short configs[4] sub-record of the default run")
     ap.add_argument("--measure-peaks", action="store_true", help="measure fp16 / fp32 / fp64 matmul peaks and print them as JSON")
@@ -272,7 +274,13 @@ def run_ours(args, cfg, cfg_run):
     # Weak scaling: every rank owns an independent replica of the workload (independent problems,
     # PAPER.md:106 "large-scale parallel evaluation"); no data-path collective.
     from paper_2205_14741_b200 import dist_util
-    wl = make_config(args.config, seed=dist_util.rank_seed(cfg["seed"], rank))
+    shard = args.shard and world > 1
+    seed = cfg["seed"] if shard else dist_util.rank_seed(cfg["seed"], rank)      # sharded: every rank holds the same H
+    if args.gapped:
+        from workloads.generator import make_workload_gapped
+        wl = make_workload_gapped(cfg["n_mol"], cfg["b"], cfg["n_occ"], cfg["cutoff"], seed, name=cfg["name"] + "-gapped")
+    else:
+        wl = make_config(args.config, seed=seed)
     dims, sum_m3 = workload_stats(wl)
     # H storage (SURVEY 8(d) G5 / reading A16): the fp64 master copy for the fp64 / fp32 runs, an fp32 copy for the
     # 16-bit runs (cast once on the host when the workload is made; X0 is rounded from fp32 arithmetic either way)
@@ -288,10 +296,19 @@ def run_ours(args, cfg, cfg_run):
         max_chunk = max(min(max_chunk, args.chunk_elems), P.max_dim_pad ** 2)
     plan = sm.DensityPlan(A, P, x_dtype, max_chunk_elems=max_chunk)
 
+    shard_state = {"st": None}
+
     def step():
         # a1 runs every step; its size query (a validation pass plus a read-back that synchronises the stream) is
         # per geometry and was done once above
         Pn = sm.sm_build_pattern(A, pad, sizes=P.sizes)
+        if shard:
+            # block columns partitioned over the ranks, one NCCL all-gather of the column-owned blocks per step
+            D, tr, shard_state["st"] = dist_util.sharded_density(sm, wl, A, Pn, x_dtype, rank, world, mu=0.0, scale_mode=scale_mode,
+                                                                 max_iter=max_iter, tol=tol, symmetrise=True,
+                                                                 switch_iter=args.switch_iter, state=shard_state["st"])
+            plan.D, plan.trace = D, tr
+            return Pn
         sm.sm_density(A, Pn, plan, mu=0.0, scale_mode=scale_mode, max_iter=max_iter, tol=tol, symmetrise=True, switch_iter=args.switch_iter)
         return Pn
 
@@ -317,6 +334,12 @@ def run_ours(args, cfg, cfg_run):
     sm.profile_enable(False)
     launches = sm.launch_count() - l0
     clocks = sampler.stop() if rank == 0 else None
+    if shard:
+        # this rank's share: iters of its own columns (the other entries stay 0 and drop out of the FLOP count)
+        stt = shard_state["st"]
+        it_full = np.zeros(wl.n_blk)
+        it_full[stt["cols"].cpu().numpy()] = stt["iters"].double().cpu().numpy()
+        plan.iters = torch.as_tensor(it_full[P.order.cpu().numpy()], device=plan.iters.device).to(plan.iters.dtype)
     iters_mean = float(plan.iters.double().mean().item())
     k_eff = plan.iters.double().cpu().numpy()
     order = P.order.cpu().numpy()
@@ -352,7 +375,7 @@ def run_ours(args, cfg, cfg_run):
 
     # ---- end to end through the public call with HOST buffers (pinned), copies inside the timed region
     e2e = None
-    if not args.no_e2e:
+    if not args.no_e2e and not shard:
         h_vals = torch.from_numpy(np.ascontiguousarray(wl.vals, dtype=np.float32 if h_dtype == "f32" else np.float64)).pin_memory()
         h_D = torch.empty(A.n_vals, dtype=torch.float64).pin_memory()
         h_tr = torch.empty(1, dtype=torch.float64).pin_memory()
@@ -502,14 +525,15 @@ def run_ours(args, cfg, cfg_run):
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+        "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "strong" if shard else "weak",
         "vs_baseline": None, "dtype": x_dtype, "data": "synthetic",
         "config": {"workload": cfg["name"], "n_mol": cfg["n_mol"], "orbitals": cfg["b"], "cutoff_A": cfg["cutoff"],
                    "x_dtype": x_dtype, "max_iter": max_iter, "tol": tol, "scale_mode": scale_mode, "h_dtype": h_dtype, "pad_to": pad,
-                   "switch_iter": args.switch_iter,
+                   "switch_iter": args.switch_iter, "gapped": bool(args.gapped),
+                   "parallelism": (f"columns sharded over {world} ranks, all-gather of D blocks" if shard else f"{world} independent replica(s)"),
                    "l2": "inputs_exceed_l2" if P.packed_elems * eb > 200e6 else "inputs_fit_l2",
                    "chunks": int(-(-P.packed_elems // max_chunk))},
-        "block_columns_per_s": world * wl.n_blk / (ms_per_step * 1e-3),
+        "block_columns_per_s": (1 if shard else world) * wl.n_blk / (ms_per_step * 1e-3),
         "iters_mean": iters_mean, "trace": float(plan.trace.item()),
         "residual_max": float(plan.residual.max().item()),
         "stages": stages, "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e,

@@ -42,5 +42,55 @@ def test_two_rank_aggregation_and_partition():
     assert out[0][3] == 1002 and out[1][3] == 1102
 
 
+def _shard_worker(rank, world, port, out):
+    """f4 host logic on CPU: every rank computes ITS block columns (with the oracle standing in for the GPU stages),
+    the column-owned blocks are exchanged by dist_util.exchange_columns (gloo all-gather), and the assembled matrix
+    must equal the one a single process computes."""
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    from oracle import oracle as orc
+    from workloads.generator import make_config
+    wl = make_config(0)
+    dim = np.array([wl.blk_size[wl.col_idx[wl.row_ptr[i]:wl.row_ptr[i + 1]]].sum() for i in range(wl.n_blk)])
+    idx = [torch.as_tensor(dist_util.column_value_index(wl.n_blk, wl.row_ptr, wl.col_idx, wl.val_ptr,
+                                                        dist_util.shard_columns(dim, world, r))) for r in range(world)]
+    mine = dist_util.shard_columns(dim, world, rank)
+    d_mine, _ = orc.density_columns(wl, cols=mine)
+    R = torch.from_numpy(d_mine.copy())
+    dist_util.exchange_columns(R, idx, rank, world)
+    out[rank] = (R.numpy().copy(), [int(ix.numel()) for ix in idx], mine.tolist())
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_two_rank_sharded_columns_assemble_the_single_process_result():
+    from oracle import oracle as orc
+    from workloads.generator import make_config
+    world = 2
+    mgr = mp.Manager()
+    out = mgr.dict()
+    mp.spawn(_shard_worker, args=(world, _free_port(), out), nprocs=world, join=True)
+    wl = make_config(0)
+    d_all, _ = orc.density_columns(wl)
+    for r in range(world):
+        assert np.array_equal(out[r][0], d_all)               # bit-identical: every element comes from exactly one rank
+    sizes = out[0][1]
+    assert sum(sizes) == d_all.size                           # the ranks' index sets partition the value array
+    assert sorted(out[0][2] + out[1][2]) == list(range(wl.n_blk))
+
+
+def test_column_value_index_is_a_partition_and_matches_the_mask():
+    from oracle import oracle as orc
+    from workloads.generator import make_workload
+    wl = make_workload(40, np.array([2, 3, 5, 4, 7] * 8), np.array([1, 1, 2, 2, 3] * 8), 5.5, seed=11)
+    cols = np.array([0, 7, 13, 39])
+    ix = dist_util.column_value_index(wl.n_blk, wl.row_ptr, wl.col_idx, wl.val_ptr, cols)
+    mask = np.zeros(int(wl.val_ptr[-1]), bool)
+    mask[ix] = True
+    assert np.array_equal(mask, orc.column_mask(wl, cols)) and len(set(ix.tolist())) == ix.size
+    allc = dist_util.column_value_index(wl.n_blk, wl.row_ptr, wl.col_idx, wl.val_ptr, np.arange(wl.n_blk))
+    assert np.array_equal(np.sort(allc), np.arange(int(wl.val_ptr[-1])))
+
+
 def test_single_process_aggregate_is_identity():
     assert dist_util.aggregate(3.5, 7.0, torch.device("cpu")) == (3.5, 7.0)

@@ -109,11 +109,13 @@ def _min_image_pairs(pos: np.ndarray, box: float, cutoff: float):
 
 
 def make_workload(n_mol: int, b, n_occ, cutoff: float, seed: int,
-                  name: str = "custom") -> Workload:
-    """Build one seeded workload.  `b`/`n_occ` may be ints or per-molecule arrays."""
+                  name: str = "custom", pos=None, coupling: float = 0.3) -> Workload:
+    """Build one seeded workload.  `b`/`n_occ` may be ints or per-molecule arrays.  `pos` (N x 3, inside the box) and
+    `coupling` (amplitude of the off-diagonal blocks, BASELINE: 0.3) are overridden only by make_workload_gapped."""
     rng = np.random.Generator(np.random.PCG64(seed))
     box = (n_mol / RHO) ** (1.0 / 3.0)
-    pos = rng.random((n_mol, 3)) * box
+    if pos is None:
+        pos = rng.random((n_mol, 3)) * box
 
     blk = np.broadcast_to(np.asarray(b, dtype=np.int32), (n_mol,)).copy()
     occ = np.broadcast_to(np.asarray(n_occ, dtype=np.int32), (n_mol,)).copy()
@@ -149,7 +151,7 @@ def make_workload(n_mol: int, b, n_occ, cutoff: float, seed: int,
         onsite = np.where(np.arange(bb)[None, :] < occ[:, None], -1.0, 1.0)
         diag[:, np.arange(bb), np.arange(bb)] += onsite
         offd = rng.standard_normal((npairs, bb, bb))
-        offd *= (0.3 * np.exp(-r / 2.0))[:, None, None]
+        offd *= (coupling * np.exp(-r / 2.0))[:, None, None]
         v3 = vals.reshape(nnzb, bb, bb)
         k0, k1, k2 = kind == 0, kind == 1, kind == 2
         v3[k0] = diag[src[k0]]
@@ -169,7 +171,7 @@ def make_workload(n_mol: int, b, n_occ, cutoff: float, seed: int,
         off_blocks = []
         for p in range(npairs):
             bi, bj = int(blk[ii[p]]), int(blk[jj[p]])
-            off_blocks.append(rng.standard_normal((bi, bj)) * (0.3 * np.exp(-r[p] / 2.0)))
+            off_blocks.append(rng.standard_normal((bi, bj)) * (coupling * np.exp(-r[p] / 2.0)))
         for q in range(nnzb):
             s = int(src[q])
             if kind[q] == 0:
@@ -235,3 +237,20 @@ def make_overlap(wl: Workload, seed: int = None, amp: float = 0.05, noise: float
                 vals[vp[q]:vp[q + 1]] = b_.T.ravel()
     return Workload(n_blk=wl.n_blk, blk_size=wl.blk_size, row_ptr=wl.row_ptr, col_idx=wl.col_idx, val_ptr=wl.val_ptr,
                     vals=vals, box=wl.box, positions=wl.positions, meta=dict(wl.meta, overlap_seed=seed))
+
+
+def make_workload_gapped(n_mol: int, b, n_occ, cutoff: float, seed: int, coupling: float = 0.04, jitter: float = 0.15,
+                         name: str = "gapped") -> Workload:
+    """Second workload of SURVEY.md 8(f) f4: the same block structure and value recipe as make_workload, but with
+    NON-OVERLAPPING molecules (a jittered simple-cubic lattice at the same number density: nearest distances ~ 2.2-3.9 A
+    instead of down to 0.06 A) and weaker couplings, so that the spectrum of H keeps the gap between the onsite levels
+    -1 and +1 around mu = 0 and a fixed Newton-Schulz count converges (reading A13: the BASELINE generator is gapless).
+    Seeded: lattice sites drawn without replacement, then the jitter, then the blocks as in make_workload."""
+    rng = np.random.Generator(np.random.PCG64(seed + 700000))
+    box = (n_mol / RHO) ** (1.0 / 3.0)
+    side = int(np.ceil(n_mol ** (1.0 / 3.0) - 1e-9))
+    a = box / side
+    sites = rng.choice(side ** 3, size=n_mol, replace=False)
+    ijk = np.stack([sites // (side * side), (sites // side) % side, sites % side], axis=1).astype(np.float64)
+    pos = (ijk + 0.5 + (rng.random((n_mol, 3)) - 0.5) * 2.0 * jitter) * a
+    return make_workload(n_mol, b, n_occ, cutoff, seed, name=name, pos=pos, coupling=coupling)
