@@ -72,9 +72,11 @@ extern "C" {
 #define SM_SCALE_GERSHGORIN 1  /* s_i = max_r sum_c |(T_i - mu I)_rc|  (>= spectral radius) */
 #define SM_SCALE_POWER 2       /* s_i = 1.05 * ||T v||_2 after 10 power steps on T_i - mu I from a
                                   fixed start vector, never above the Gershgorin bound */
-#define SM_SCALE_GLOBAL 3      /* s_i = min(Gershgorin_i, 1.05 * ||(A - mu I) v||_2) after 10 power steps on the whole
-                                  block-sparse A - mu I: every T_i - mu I is a principal submatrix of it, so by Cauchy
-                                  interlacing rho(T_i - mu I) <= rho(A - mu I); one bound for all i, no second gather */
+#define SM_SCALE_GLOBAL 3      /* s_i = min(Gershgorin_i, margin * est), est = ||(A - mu I) v||_2 after 10 power steps on the
+                                  whole block-sparse A - mu I, an ESTIMATE from below of rho(A - mu I) (every T_i - mu I is a
+                                  principal submatrix of it: rho(T_i - mu I) <= rho(A - mu I) by Cauchy interlacing); margin
+                                  1.05, widened by ten times the last step's growth while est has not settled.  Not a bound:
+                                  Newton-Schulz needs rho(T_i) / s_i < sqrt(3) and sm_sign_status reports a divergence */
 
 /* Block-CSR description of the symmetric input A = H ("block-sparse"). */
 typedef struct {
@@ -177,7 +179,8 @@ int32_t sm_sign_ns_ex(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols
                       void *ws, int64_t ws_bytes, int32_t max_iter, double tol, int32_t flags,
                       int32_t switch_iter, int32_t *iters /*[n_cols]*/, double *residual /*[n_cols]*/,
                       void *stream);
-/* Synchronises and returns SM_WARN_NOT_CONVERGED if tol > 0 and any residual[c] >= tol. */
+/* Synchronises and returns SM_WARN_NOT_CONVERGED if tol > 0 and any residual[c] >= tol (or is not finite); with
+ * tol <= 0 (fixed-count mode) if any residual[c] is not finite or exceeds 1, i.e. the iteration diverged. */
 int32_t sm_sign_status(const double *residual, int32_t n_cols, double tol, void *scratch, void *stream);
 
 /* a4. R(N(i)[a], i) = S_i[rows of neighbour a, columns of block i] for the listed columns

@@ -88,7 +88,7 @@ int32_t prof_end(cudaStream_t st, int slot) {
 static __global__ void k_count_unconverged(int32_t n, const double *__restrict__ residual, double tol,
                                            int32_t *__restrict__ out) {
   int32_t c = blockIdx.x * blockDim.x + threadIdx.x;
-  if (c < n && !(residual[c] < tol)) atomicAdd(out, 1);
+  if (c < n && !(residual[c] < tol)) atomicAdd(out, 1);       // also counts NaN
 }
 }  // namespace sm
 
@@ -168,7 +168,9 @@ extern "C" int32_t sm_sign_status(const double *residual, int32_t n_cols, double
                                   void *stream) {
   if (!residual || !scratch || n_cols <= 0) return SM_ERR_ARG;
   cudaStream_t st = (cudaStream_t)stream;
-  if (!(tol > 0.0)) { SM_CUDA(cudaStreamSynchronize(st)); return SM_OK; }
+  // fixed-count mode (tol <= 0): nothing to converge to, but a submatrix whose last residual is not finite or exceeds
+  // 1 has DIVERGED (a spectral scale below rho / sqrt(3)); that is reported the same way
+  if (!(tol > 0.0)) tol = 1.0;
   int32_t *d = (int32_t *)scratch;
   SM_CUDA(cudaMemsetAsync(d, 0, sizeof(int32_t), st));
   k_count_unconverged<<<(n_cols + 255) / 256, 256, 0, st>>>(n_cols, residual, tol, d);

@@ -6,7 +6,7 @@
 // the extreme eigenvalues of A - mu I: rho(T_i - mu I) <= rho(A - mu I) for all i.  GLOBAL_STEPS power steps
 // v <- (A - mu I) v / ||.|| from a fixed hashed start vector give est = ||(A - mu I) v|| <= rho(A - mu I) (a lower
 // bound that is within ~15 % after 10 steps on the water-like workloads); the scale is
-//   s_i = min(Gershgorin_i, 1.05 * est).
+//   s_i = min(Gershgorin_i, max(1.05 * est, est + 10 * (est - est of the step before))).
 // Newton-Schulz converges for |x| < sqrt(3), so the iteration stays convergent as long as est > 0.55 rho(A - mu I).
 // Compared with SM_SCALE_POWER (ten power steps on every gathered submatrix, then a second gather) this reads
 // the block-CSR values ten times (0.23 GB each at configs[2]) instead of the packed images (1.3 GB each) and needs
@@ -37,7 +37,7 @@ __global__ void k_global_init(int32_t n_blk, const int32_t *__restrict__ blk, co
     const uint32_t h = (g * 2654435761u) >> 8;
     v[voff[i] + r] = 0.25 + (double)(h & 0xFFFFu) * (1.0 / 65536.0);
   }
-  if (i == 0 && threadIdx.x == 0) { scal[0] = 1.0; scal[1] = 0.0; }     // scal[0] = 1 / ||v||, scal[1] = est
+  if (i == 0 && threadIdx.x == 0) { scal[0] = 1.0; scal[1] = 0.0; scal[2] = 0.0; }   // 1 / ||v||, est, previous est
 }
 
 // y = (A - mu I) (inv_norm * v) for block row i; part[i] = sum of y_r^2 over the block row.  One CTA per block
@@ -111,6 +111,7 @@ __global__ void __launch_bounds__(1024) k_global_norm(int32_t n_blk, const doubl
     double t = 0.0;
     for (int w = 0; w < (int)(blockDim.x >> 5); ++w) t += red[w];
     const double nrm = bad ? 0.0 : sqrt(t);      // 0: k_global_apply leaves the Gershgorin scales untouched
+    scal[2] = scal[1];                           // the estimate of the step before: its growth guards the margin
     scal[1] = nrm;
     scal[0] = nrm > 0.0 ? 1.0 / nrm : 1.0;
   }
@@ -119,8 +120,14 @@ __global__ void __launch_bounds__(1024) k_global_norm(int32_t n_blk, const doubl
 __global__ void k_global_apply(int32_t n_cols, const double *__restrict__ scal, double *__restrict__ scale) {
   int32_t c = blockIdx.x * blockDim.x + threadIdx.x;
   if (c >= n_cols) return;
-  const double g = 1.05 * scal[1];
-  if (g > 0.0 && g < scale[c]) scale[c] = g;
+  // est is a LOWER bound of rho(A - mu I) that grows monotonically with the power steps.  Margin: 5 %, or ten times
+  // the growth of the last step when the iteration has not settled (est still growing by more than 0.5 % per step:
+  // a slowly separating spectrum) -- a geometric extrapolation of the remaining distance.  Newton-Schulz needs only
+  // rho(T_i) / s_i < sqrt(3), so the scale stays safe unless est is below 0.55 rho while having all but stopped
+  // growing; sm_sign_status additionally reports a diverged submatrix (non-finite or > 1 residual) in fixed-count mode.
+  const double est = scal[1], grow = fmax(0.0, scal[1] - scal[2]);
+  const double g = fmax(1.05 * est, est + 10.0 * grow);
+  if (est > 0.0 && g < scale[c]) scale[c] = g;
 }
 
 int64_t global_scale_ws_bytes(const sm_bcsr_t *A, const sm_pattern_t *P) {
@@ -129,7 +136,7 @@ int64_t global_scale_ws_bytes(const sm_bcsr_t *A, const sm_pattern_t *P) {
   cur.take<double>((int64_t)A->n_blk * P->max_dim);
   cur.take<double>((int64_t)A->n_blk * P->max_dim);
   cur.take<double>(A->n_blk);
-  cur.take<double>(2);
+  cur.take<double>(4);
   return cur.used + 256;
 }
 
@@ -142,7 +149,7 @@ int32_t global_scale(const sm_bcsr_t *A, const void *A_vals, int32_t a_dtype, co
   double *v = cur.take<double>((int64_t)n * P->max_dim);       // n_blk * max block size <= n_blk * max_dim
   double *y = cur.take<double>((int64_t)n * P->max_dim);
   double *part = cur.take<double>(n);
-  double *scal = cur.take<double>(2);
+  double *scal = cur.take<double>(4);
   if (!cur.ok()) return SM_ERR_SPACE;
   k_widen_blk<<<(n + 255) / 256, 256, 0, st>>>(n, A->blk_size, voff);
   SM_LAUNCHED();

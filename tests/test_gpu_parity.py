@@ -663,6 +663,23 @@ def test_power_scale_is_a_valid_tight_deterministic_bound(sm):
         assert 0.80 * rho <= sp[i] <= 1.06 * rho, (i, sp[i], rho)  # Newton-Schulz needs |x| < sqrt(3): s > rho / 1.73
 
 
+def test_fixed_count_divergence_is_reported(sm):
+    # a spectral scale below rho / sqrt(3) makes Newton-Schulz diverge; in fixed-count mode (tol <= 0) sm_sign_status
+    # reports it (non-finite or > 1 residual) instead of answering SM_OK (SM_SCALE_GLOBAL is an estimate)
+    wl = make_workload(60, 23, 4, 5.0, seed=21)
+    assert np.abs(np.linalg.eigvalsh(wl.dense())).max() > 2.0
+    A = sm.Bcsr(wl)
+    for x_dtype, pad in (("f64", 16), ("bf16", 64)):
+        P = sm.sm_build_pattern(A, pad)
+        cols, col_off, n = sm.sm_plan_columns(P, None)
+        X, _ = sm.sm_gather(A, P, cols, col_off, n, 0.0, "none", x_dtype)            # unscaled: rho(T_i) > sqrt(3)
+        _, res = sm.sm_sign_ns(P, cols, col_off, n, P.packed_elems, x_dtype, X, 12, 0.0)
+        assert sm.sm_sign_status(res, 0.0) == sm.SM_WARN_NOT_CONVERGED
+        X, _ = sm.sm_gather(A, P, cols, col_off, n, 0.0, "global", x_dtype)
+        _, res = sm.sm_sign_ns(P, cols, col_off, n, P.packed_elems, x_dtype, X, 30, 0.0)
+        assert sm.sm_sign_status(res, 0.0) == sm.SM_OK
+
+
 def test_global_scale_is_a_valid_deterministic_bound(sm):
     # Cauchy interlacing: rho(T_i - mu I) <= rho(A - mu I) for every principal submatrix; the power estimate is a
     # lower bound of rho(A - mu I) times 1.05, and Newton-Schulz needs rho(T_i) / s_i < sqrt(3)
@@ -678,7 +695,7 @@ def test_global_scale_is_a_valid_deterministic_bound(sm):
         sg, s1 = sg.cpu().numpy(), s1.cpu().numpy()
         assert (s1 <= sg * (1 + 1e-12)).all()
         rho_a = np.abs(np.linalg.eigvalsh(wl.dense() - mu * np.eye(wl.n))).max()
-        assert s1.max() <= 1.05 * rho_a * (1 + 1e-12)                 # est is a lower bound of rho(A - mu I)
+        assert s1.max() <= 1.25 * rho_a                               # est is a lower bound of rho(A - mu I); margin 5 % .. extrapolated
         assert s1.max() >= 0.75 * rho_a                               # and a useful one after 10 steps
         for i in range(wl.n_blk):
             T = orc.gather(wl, i, mu)
