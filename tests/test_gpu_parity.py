@@ -663,6 +663,26 @@ def test_power_scale_is_a_valid_tight_deterministic_bound(sm):
         assert 0.80 * rho <= sp[i] <= 1.06 * rho, (i, sp[i], rho)  # Newton-Schulz needs |x| < sqrt(3): s > rho / 1.73
 
 
+def test_staged_gather_is_bit_identical(sm):
+    # k_gather_staged (source-driven, shared-memory tile in the image layout, bulk TMA stores; option "gather.tma")
+    # against the element-wise k_gather: same fp32 arithmetic, one rounding -> identical 16-bit images
+    try:
+        for wl in (make_config(0), ragged_workload(), make_workload(90, 23, 4, 5.0, seed=33), make_workload(12, 1, 1, 6.0, seed=6)):
+            A = sm.Bcsr(wl)
+            P = sm.sm_build_pattern(A, 64)
+            cols, col_off, n = sm.sm_plan_columns(P, P.order)
+            for x_dtype, mode, mu in (("bf16", "gershgorin", 0.0), ("f16", "global", 0.3)):
+                imgs = []
+                for o in (0, 1):
+                    sm.set_option("gather.tma", o)
+                    X, _ = sm.sm_gather(A, P, cols, col_off, n, mu, mode, x_dtype)
+                    torch.cuda.synchronize()
+                    imgs.append(X.view(torch.int16).clone())
+                assert torch.equal(imgs[0], imgs[1])
+    finally:
+        sm.set_option("gather.tma", 0)
+
+
 def test_fixed_count_divergence_is_reported(sm):
     # a spectral scale below rho / sqrt(3) makes Newton-Schulz diverge; in fixed-count mode (tol <= 0) sm_sign_status
     # reports it (non-finite or > 1 residual) instead of answering SM_OK (SM_SCALE_GLOBAL is an estimate)
