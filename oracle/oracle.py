@@ -36,7 +36,8 @@ _lib = None
 def lib():
     global _lib
     if _lib is None:
-        _lib = C.CDLL(build())
+        # ORC_SO: an alternative build of the same source (the address/UB-sanitizer build of tests/test_oracle_pins.py)
+        _lib = C.CDLL(os.environ.get("ORC_SO") or build())
         _lib.orc_gershgorin.restype = C.c_double
         _lib.orc_trace.restype = C.c_double
     return _lib

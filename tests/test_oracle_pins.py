@@ -565,3 +565,30 @@ def test_lapack_variant_is_pinned_to_jacobi_at_configs4_size():
     assert rec["m"] >= 1200                                   # a large-submatrix-regime column, not a small one
     assert rec["max_abs_diff"] <= 1e-10
     assert rec["frobenius_jacobi"] > 1.0                      # a real block column of D, not zeros
+
+
+def test_oracle_under_address_and_undefined_behaviour_sanitizers(tmp_path):
+    """the host oracle built with -fsanitize=address,undefined runs configs[0] (pattern, gather,
+    Jacobi, sign, NS-k polynomial, scatter, symmetrise, trace; two threads) without a report."""
+    import subprocess
+    import sys
+    so = str(tmp_path / "liborc_asan.so")
+    src = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "oracle", "submatrix_oracle.c")
+    subprocess.check_call(["gcc", "-O1", "-g", "-fsanitize=address,undefined", "-fno-omit-frame-pointer", "-fPIC", "-shared",
+                           "-pthread", "-o", so, src, "-lm"])
+    asan = subprocess.check_output(["gcc", "-print-file-name=libasan.so"], text=True).strip()
+    code = ("import numpy as np\n"
+            "from oracle import oracle as orc\n"
+            "from workloads.generator import make_config\n"
+            "wl = make_config(0)\n"
+            "P = orc.build_pattern(wl, 16)\n"
+            "d, st = orc.density_columns(wl, n_threads=2)\n"
+            "dk, _ = orc.density_columns(wl, cols=np.arange(4, dtype=np.int32), mode='nsk', k_fixed=5)\n"
+            "ds = orc.symmetrise(wl, d)\n"
+            "print('TRACE', orc.trace(wl, ds))\n")
+    env = dict(os.environ, ORC_SO=so, LD_PRELOAD=asan, ASAN_OPTIONS="detect_leaks=0", UBSAN_OPTIONS="halt_on_error=1",
+               PYTHONPATH=os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
+    p = subprocess.run([sys.executable, "-c", code], env=env, capture_output=True, text=True, timeout=600)
+    assert p.returncode == 0, p.stderr[-3000:]
+    assert "TRACE" in p.stdout
+    assert "AddressSanitizer" not in p.stderr and "runtime error" not in p.stderr, p.stderr[-3000:]
