@@ -498,10 +498,10 @@ def run_ours(args, cfg, cfg_run):
             issued_step = float((2 * 2.0 * 128 * 128 * (te * (te + 1) / 2) * np.ceil(dims[order] / 16.0) * 16 * k_eff).sum()) \
                 if dims.max() > 96 else flops_step
         else:
-            te = np.ceil(dims[order] / 64.0)
-            issued_step = float((2 * 2.0 * 64 * 64 * te * te * np.ceil(dims[order] / 16.0) * 16 * k_eff).sum())
+            te = np.ceil(dims[order] / 64.0)           # k_ffma_sym: lower-triangle 64 x 64 tiles
+            issued_step = float((2 * 2.0 * 64 * 64 * (te * (te + 1) / 2) * np.ceil(dims[order] / 16.0) * 16 * k_eff).sum())
         issued_per_launch = issued_step * args.steps / max(gemm_launches, 1)
-        kernel = "k_dmma_gemm" if x_dtype == "f64" else "k_simt_gemm"
+        kernel = "k_dmma_gemm" if x_dtype == "f64" else "k_ffma_sym"
         traffic, traffic_src = ncu_traffic(args.config, x_dtype, kernel)
         roofline = {"bound": "tensor" if x_dtype == "f64" else "alu", "kernel": kernel,
                     "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
@@ -512,7 +512,8 @@ def run_ours(args, cfg, cfg_run):
                     "algorithmic_flops_per_launch": flops_per_launch, "issued_flops_per_launch": issued_per_launch,
                     "note": ("fp64 kernel computes lower-triangle tiles only (symmetric iterates): frac counts the full 2 m^3 per "
                              "product and may exceed the peak; frac_issued counts the tiles actually computed, with padding")
-                    if x_dtype == "f64" else "frac_issued counts the 64 x 64 tiles computed, with padding"}
+                    if x_dtype == "f64" else "fp32 kernel computes lower-triangle 64 x 64 tiles only: frac counts the full 2 m^3 per product, "
+                            "frac_issued the tiles actually computed, with padding"}
 
     cpu = None
     if not args.no_cpu_baseline:

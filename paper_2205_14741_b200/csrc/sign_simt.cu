@@ -265,6 +265,114 @@ k_dmma_gemm(const int32_t *__restrict__ cols, const int64_t *__restrict__ col_of
   }
 }
 
+// ---- fp32, symmetric iterates: 64 x 64 tiles, 8 x 8 register blocks, cp.async double buffering -------------------
+// X and Y are symmetric (exactly: only tiles with tc <= tr are computed and every element (r, c <= r) is stored at (r, c)
+// and mirrored to (c, r)), so BOTH operands of a tile can be read as rows k with the tile's rows / columns contiguous:
+// A[m][k] = X[k][row0 + m], B[k][n] = B[k][col0 + n] -- 16-byte cp.async without a transposition.  64 threads per
+// CTA, thread (ty, tx) of an 8 x 8 grid owns rows ty * 8 .. and columns tx * 8 .. (64 independent FFMA chains per k for
+// four 128-bit shared loads), many CTAs per SM.  Against k_simt_gemm (all tiles, 4 x 4 blocks, scalar bounds-checked
+// loads, two __syncthreads per 16 k: 0.27 of the FFMA peak at configs[1]) this halves the tiles
+// and raises the FFMA share of the issue slots.  Padding rows / columns of X, Y and the alternate buffer are zero
+// (gather / memset), so loads are bounded by the padded dimension only.
+constexpr int FT = 64, FK = 16;
+
+template <int PHASE>
+__global__ void __launch_bounds__(64)
+k_ffma_sym(const int32_t *__restrict__ cols, const int64_t *__restrict__ col_off,
+           const int32_t *__restrict__ dim, const int32_t *__restrict__ dim_pad, int32_t max_tiles_edge,
+           const float *__restrict__ Xsrc, const float *__restrict__ Ybuf, float *__restrict__ Out, SignState s) {
+  const int32_t tiles_per = max_tiles_edge * max_tiles_edge;
+  const int32_t c = blockIdx.x / tiles_per, t = blockIdx.x - c * tiles_per;
+  if (!s.active[c]) return;
+  if (PHASE == 1 && s.last[c]) return;
+  const int32_t i = cols ? cols[c] : c;
+  const int32_t m = dim[i], Pd = dim_pad[i];
+  const int32_t te = (m + FT - 1) / FT;
+  const int32_t tr = t / max_tiles_edge, tc = t - tr * max_tiles_edge;
+  if (tr >= te || tc > tr) return;                              // lower-triangle tiles only
+  const float *A = Xsrc + col_off[c];
+  const float *B = (PHASE == 1 ? Xsrc : Ybuf) + col_off[c];
+  float *O = Out + col_off[c];
+  const int32_t row0 = tr * FT, col0 = tc * FT;
+  __shared__ __align__(16) float As[2][FK][FT];
+  __shared__ __align__(16) float Bs[2][FK][FT];
+  const int tx = threadIdx.x & 7, ty = threadIdx.x >> 3;
+
+  auto load_stage = [&](int st, int32_t k0) {
+    // 16 k rows x 16 chunks of 4 floats, for A (columns row0 ..) and B (columns col0 ..): 4 + 4 copies per thread
+#pragma unroll
+    for (int l = 0; l < 4; ++l) {
+      const int e = threadIdx.x + l * 64, k = e >> 4, ch = e & 15;
+      const int32_t gk = k0 + k, ga = row0 + ch * 4, gb = col0 + ch * 4;
+      const bool oka = gk < Pd && ga < Pd, okb = gk < Pd && gb < Pd;
+      cp_async16(&As[st][k][ch * 4], oka ? A + (int64_t)gk * Pd + ga : A, oka);
+      cp_async16(&Bs[st][k][ch * 4], okb ? B + (int64_t)gk * Pd + gb : B, okb);
+    }
+    asm volatile("cp.async.commit_group;" ::: "memory");
+  };
+
+  float acc[8][8];
+#pragma unroll
+  for (int a = 0; a < 8; ++a)
+#pragma unroll
+    for (int b = 0; b < 8; ++b) acc[a][b] = 0.f;
+
+  const int32_t nk = (m + FK - 1) / FK;
+  load_stage(0, 0);
+  for (int32_t kc = 0; kc < nk; ++kc) {
+    if (kc + 1 < nk) {
+      load_stage((kc + 1) & 1, (kc + 1) * FK);
+      asm volatile("cp.async.wait_group 1;" ::: "memory");
+    } else {
+      asm volatile("cp.async.wait_group 0;" ::: "memory");
+    }
+    __syncthreads();
+    const int st = kc & 1;
+#pragma unroll
+    for (int k = 0; k < FK; ++k) {
+      const float4 a0 = *reinterpret_cast<const float4 *>(&As[st][k][ty * 8]);
+      const float4 a1 = *reinterpret_cast<const float4 *>(&As[st][k][ty * 8 + 4]);
+      const float4 b0 = *reinterpret_cast<const float4 *>(&Bs[st][k][tx * 8]);
+      const float4 b1 = *reinterpret_cast<const float4 *>(&Bs[st][k][tx * 8 + 4]);
+      const float av[8] = {a0.x, a0.y, a0.z, a0.w, a1.x, a1.y, a1.z, a1.w};
+      const float bv[8] = {b0.x, b0.y, b0.z, b0.w, b1.x, b1.y, b1.z, b1.w};
+#pragma unroll
+      for (int a = 0; a < 8; ++a)
+#pragma unroll
+        for (int b = 0; b < 8; ++b) acc[a][b] = fmaf(av[a], bv[b], acc[a][b]);
+    }
+    __syncthreads();
+  }
+
+  double res = 0.0;
+#pragma unroll
+  for (int a = 0; a < 8; ++a) {
+    const int32_t gr = row0 + ty * 8 + a;
+#pragma unroll
+    for (int b = 0; b < 8; ++b) {
+      const int32_t gc = col0 + tx * 8 + b;
+      if (gr < m && gc <= gr) {
+        float val = acc[a][b];
+        if (PHASE == 1) {
+          const double d = (double)val - (gr == gc ? 1.0 : 0.0);
+          res += (gr == gc ? 1.0 : 2.0) * d * d;
+        } else {
+          val = 1.5f * A[(int64_t)gr * Pd + gc] - 0.5f * val;
+        }
+        O[(int64_t)gr * Pd + gc] = val;
+        if (gc < gr) O[(int64_t)gc * Pd + gr] = val;
+      }
+    }
+  }
+  if (PHASE == 1) {
+    __shared__ double red[2];
+    for (int d = 16; d > 0; d >>= 1) res += __shfl_xor_sync(0xffffffffu, res, d);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = res;
+    __syncthreads();
+    if (threadIdx.x == 0) s.partial[(int64_t)c * s.parts_per_col + tr * te + tc] = red[0] + red[1];
+  }
+}
+
 static __global__ void k_tile_nparts(int32_t n_cols, int32_t T, const int32_t *__restrict__ cols,
                                      const int32_t *__restrict__ dim, int32_t *__restrict__ n_parts) {
   int32_t c = blockIdx.x * blockDim.x + threadIdx.x;
@@ -309,6 +417,8 @@ static int32_t sign_simt_t(const sm_pattern_t *P, const int32_t *cols, int32_t n
   SignState s{w.active, w.last, w.n_still, w.partial, w.parts_per_col};
   // fp64: DMMA tensor-core tiles of 128 x 128 unless the submatrices are tiny (or option f64.simt = 1)
   const bool dmma = sizeof(T) == 8 && opt(OPT_F64_SIMT) == 0 && P->max_dim > 96;
+  // fp32, symmetric iterates: lower-triangle 64 x 64 tiles with 8 x 8 register blocks (option "f32.sym", default on)
+  const bool fsym = sizeof(T) == 4 && !nonsym && opt(OPT_F32_SYM) != 0 && (P->pad_to & 3) == 0;
   const int32_t TS = dmma ? DT : ST;
   const int32_t edge = (P->max_dim + TS - 1) / TS;
   const int64_t grid64 = (int64_t)n_cols * edge * edge;
@@ -318,6 +428,12 @@ static int32_t sign_simt_t(const sm_pattern_t *P, const int32_t *cols, int32_t n
   SM_LAUNCHED();
   k_tile_nparts<<<nb, 256, 0, st>>>(n_cols, TS, cols, P->dim, w.n_parts);
   SM_LAUNCHED();
+  if (fsym) {
+    // padding of Y / the alternate X buffer must read as zeros; slots of the skipped upper tiles too
+    SM_CUDA(cudaMemsetAsync(w.Y, 0, packed_elems * sizeof(T), st));
+    SM_CUDA(cudaMemsetAsync(w.X2, 0, packed_elems * sizeof(T), st));
+    SM_CUDA(cudaMemsetAsync(w.partial, 0, (size_t)n_cols * w.parts_per_col * sizeof(double), st));
+  }
   if (dmma) {
     // per device attribute: set on every call (a process may use several devices)
     SM_CUDA(cudaFuncSetAttribute(k_dmma_gemm<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, DMMA_SMEM));
@@ -342,6 +458,8 @@ static int32_t sign_simt_t(const sm_pattern_t *P, const int32_t *cols, int32_t n
     else if (dmma)
       k_dmma_gemm<1, true><<<grid, 256, DMMA_SMEM, st>>>(cols, col_off, P->dim, P->dim_pad, edge, (const double *)src,
                                                          (const double *)Y, (double *)Y, s);
+    else if (fsym)
+      k_ffma_sym<1><<<grid, 64, 0, st>>>(cols, col_off, P->dim, P->dim_pad, edge, (const float *)src, (const float *)Y, (float *)Y, s);
     else
       k_simt_gemm<T, 1><<<grid, 256, 0, st>>>(cols, col_off, P->dim, P->dim_pad, edge, src, Y, Y, s);
     SM_LAUNCHED();
@@ -356,6 +474,8 @@ static int32_t sign_simt_t(const sm_pattern_t *P, const int32_t *cols, int32_t n
     else if (dmma)
       k_dmma_gemm<2, true><<<grid, 256, DMMA_SMEM, st>>>(cols, col_off, P->dim, P->dim_pad, edge, (const double *)src,
                                                          (const double *)Y, (double *)dst, s);
+    else if (fsym)
+      k_ffma_sym<2><<<grid, 64, 0, st>>>(cols, col_off, P->dim, P->dim_pad, edge, (const float *)src, (const float *)Y, (float *)dst, s);
     else
       k_simt_gemm<T, 2><<<grid, 256, 0, st>>>(cols, col_off, P->dim, P->dim_pad, edge, src, Y, dst, s);
     SM_LAUNCHED();
