@@ -18,9 +18,10 @@
 // LBO = one chunk, the next 8 k at SBO = 1024 B).
 //
 // Tiles per product (128-row UMMA M, lower triangle at 128 granularity): T0 = rows 0..127 x cols 0..min(128, Pd),
-// T1 = rows 128..255 x cols 0..Pd (only if Pd > 128), accumulators at TMEM columns 0 and 128.  T0's epilogue
-// overlaps T1's MMAs.  Symmetry is enforced exactly as in k_umma_gemm: only elements (r, c), r >= c, are taken
-// from the accumulators, stored at (r, c) and mirrored to (c, r).
+// T1 = rows 128..255 x cols 0..Pd (only if Pd > 128); accumulators: T1 at TMEM columns 128.., T0 at columns 0.. for
+// product 1 and at columns 384.. for product 2, so that the early part of a product can be issued while the other
+// tile's epilogue of the previous product still converts (schedule: see the MMA issuer).  Symmetry is enforced exactly
+// as in k_umma_gemm: only elements (r, c), r >= c, are taken from the accumulators, stored at (r, c) and mirrored to (c, r).
 //   product 1: Y = X X^T; epilogue: W = Y - I, fused ||W||_F^2 (warp shuffles + fixed-order sum of the 16 warp
 //              partials), Wh = -1/2 W -> WS.
 //   product 2: X' = X + X Wh^T; the accumulator holds X Wh^T, the epilogue adds the X tile it reads back from XS
@@ -61,8 +62,10 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_umma_resident(RArgs a) {
   const uint32_t xs = (raw + 1023u) & ~1023u;
   const uint32_t ws = xs + RES_XS_BYTES;
   const uint32_t bars = ws + RES_WS_BYTES;
-  const uint32_t b_xload = bars, b_tfull0 = bars + 8, b_tfull1 = bars + 16, b_wready = bars + 24,
-                 b_xready = bars + 32, b_free = bars + 40, tmem_slot = bars + 48;
+  // b_w1 / b_w0: the epilogue of product 1 has written T1's / T0's part of Wh (and drained that accumulator);
+  // b_x0 / b_x1: the epilogue of product 2 has written T0's / T1's part of X'.  16 warp arrivals each, once per step.
+  const uint32_t b_xload = bars, b_tfull0 = bars + 8, b_tfull1 = bars + 16, b_w1 = bars + 24, b_w0 = bars + 32,
+                 b_x0 = bars + 40, b_x1 = bars + 48, b_free = bars + 56, tmem_slot = bars + 80;
   volatile uint32_t *tmem_slot_ptr = reinterpret_cast<volatile uint32_t *>(smem_raw + (tmem_slot - raw));
   volatile int64_t *cur_c = reinterpret_cast<volatile int64_t *>(smem_raw + (bars + 64 - raw));
   volatile float *res_s = reinterpret_cast<volatile float *>(smem_raw + (bars + 128 - raw));   // [16]
@@ -70,7 +73,8 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_umma_resident(RArgs a) {
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   if (threadIdx.x == 0) {
     ptx::mbar_init(b_xload, 1); ptx::mbar_init(b_tfull0, 1); ptx::mbar_init(b_tfull1, 1);
-    ptx::mbar_init(b_wready, RES_EPI_WARPS); ptx::mbar_init(b_xready, RES_EPI_WARPS); ptx::mbar_init(b_free, 1);
+    ptx::mbar_init(b_w1, RES_EPI_WARPS); ptx::mbar_init(b_w0, RES_EPI_WARPS); ptx::mbar_init(b_x0, RES_EPI_WARPS);
+    ptx::mbar_init(b_x1, RES_EPI_WARPS); ptx::mbar_init(b_free, 1);
     ptx::fence_barrier_init();
     ptx::fence_proxy_async();
   }
@@ -126,8 +130,20 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_umma_resident(RArgs a) {
     // ===================== MMA issuer =====================
     // The whole warp runs this loop converged, on warp-uniform values (shuffle broadcasts tell ptxas so); one
     // elected lane issues each MMA / commit (umma_f16_elect).
+    //
+    // Schedule of one step (two tiles; T0 alternates between the accumulators T0a = TMEM columns 0.. for product 1 and
+    // T0b = columns 384.. for product 2, T1 stays at columns 128..).  Chunks kc < 2 are the columns 0..127, chunks
+    // kc >= 2 the columns 128.. :
+    //   product 1 (Y = X X^T):   T0a[kc < 2]            needs X'[0:128, 0:128]                = T0's epilogue 2   (b_x0)
+    //                            T1[all], T0a[kc >= 2]  need all of X'                        + T1's epilogue 2   (b_x1)
+    //   product 2 (X Wh^T):      T0b[kc >= 2], T1[kc >= 2] need Wh[128.., :] only             = T1's epilogue 1   (b_w1)
+    //                            T0b[kc < 2], T1[kc < 2]   need Wh[0:128, 0:128] as well      + T0's epilogue 1   (b_w0)
+    // so the MMAs of the early parts run while the other tile's epilogue is still converting, instead of the whole chain
+    // MMA -> epilogue -> MMA being serial (clock64, first version: two hand-overs of ~2 000 cycles per step exposed).
+    // Product 1 finishes T1 before T0a and product 2 finishes T0b before T1: T1's mirrored X' stores land in rows
+    // 0..127 of XS, which T0b's MMAs read, so T1's epilogue 2 may only start when they are done.
     {
-      uint32_t p_xload = 0, p_w = 0, p_x = 0;
+      uint32_t p_xload = 0, p_w1 = 0, p_w0 = 0, p_x0 = 0, p_x1 = 0;
       for (;;) {
         ptx::mbar_wait(b_xload, p_xload, a.err_flag, 22); p_xload ^= 1u;
         const int32_t c = __shfl_sync(0xffffffffu, (int32_t)*cur_c, 0);
@@ -136,98 +152,96 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_umma_resident(RArgs a) {
         s.m = __shfl_sync(0xffffffffu, s.m, 0); s.Pd = __shfl_sync(0xffffffffu, s.Pd, 0);
         s.kmax = (s.m + 15) & ~15; s.nkc = (s.kmax + 63) >> 6; s.n0 = s.Pd < 128 ? s.Pd : 128; s.two = s.Pd > 128;
         const uint32_t Pd = (uint32_t)s.Pd;
+        const uint32_t dT0a = tmem_base, dT1 = tmem_base + 128u, dT0b = tmem_base + 384u;
         bool bf = BF16_IN;
-#ifdef SM_RES_TRACE
-        long long tr_a = 0, tr_b = 0, tr_c = 0, tr_d = 0, tr_t;
-#endif
-        for (int32_t k = 0; k < a.max_iter; ++k) {
-          if (k == a.switch_iter) bf = false;     // 0 < switch_iter < max_iter (host-checked), tol <= 0
-#ifdef SM_RES_TRACE
-          tr_t = clock64();
-#endif
-          // ---- product 1: Y = X X^T (both operands K-major rows of XS).  T1 first: its epilogue (more blocks, and
-          // only the quadrants that hold its rows) then overlaps T0's MMAs and the shorter T0 epilogue is the exposed
-          // one.  (Product 2 must keep T0 first: T1's mirrored stores land in rows 0..127 of XS, which T0 reads.)
-          for (int tt = 0; tt < (s.two ? 2 : 1); ++tt) {
-            const int t = s.two ? 1 - tt : 0;
-            const uint32_t N = t ? Pd : (uint32_t)s.n0;
-            const uint32_t idesc = ptx::make_idesc_f16(bf, 128, N, false);
-            const uint32_t d = tmem_base + (t ? 128u : 0u);
-            for (int kc = 0; kc < s.nkc; ++kc) {
-              const uint64_t ad = ptx::make_sw128_kmajor_desc(xs + (uint32_t)kc * Pd * 128u + (t ? 128u * 128u : 0u));
-              const uint64_t bd = ptx::make_sw128_kmajor_desc(xs + (uint32_t)kc * Pd * 128u);
-              const int ksteps = min(4, (s.kmax - kc * 64) / 16);
-              if (ksteps == 4) {
+        // product 1, tile t, chunks [k_lo, k_hi): first = no MMA has written this accumulator yet
+        auto p1 = [&](int t, int k_lo, int k_hi, bool first) {
+          const uint32_t N = t ? Pd : (uint32_t)s.n0;
+          const uint32_t idesc = ptx::make_idesc_f16(bf, 128, N, false);
+          const uint32_t d = t ? dT1 : dT0a;
+          for (int kc = k_lo; kc < k_hi; ++kc) {
+            const uint64_t ad = ptx::make_sw128_kmajor_desc(xs + (uint32_t)kc * Pd * 128u + (t ? 128u * 128u : 0u));
+            const uint64_t bd = ptx::make_sw128_kmajor_desc(xs + (uint32_t)kc * Pd * 128u);
+            const int ksteps = min(4, (s.kmax - kc * 64) / 16);
+            const uint32_t acc0 = (uint32_t)(!first || kc != k_lo);
+            if (ksteps == 4) {
 #pragma unroll
-                for (int ks = 0; ks < 4; ++ks) ptx::umma_f16_elect(d, ad + (uint64_t)(2 * ks), bd + (uint64_t)(2 * ks), idesc, (uint32_t)((kc | ks) != 0));
-              } else {
-                for (int ks = 0; ks < ksteps; ++ks) ptx::umma_f16_elect(d, ad + (uint64_t)(2 * ks), bd + (uint64_t)(2 * ks), idesc, (uint32_t)((kc | ks) != 0));
-              }
+              for (int ks = 0; ks < 4; ++ks) ptx::umma_f16_elect(d, ad + (uint64_t)(2 * ks), bd + (uint64_t)(2 * ks), idesc, acc0 | (uint32_t)(ks != 0));
+            } else {
+              for (int ks = 0; ks < ksteps; ++ks) ptx::umma_f16_elect(d, ad + (uint64_t)(2 * ks), bd + (uint64_t)(2 * ks), idesc, acc0 | (uint32_t)(ks != 0));
             }
-            ptx::umma_commit_elect(t ? b_tfull1 : b_tfull0);
           }
-#ifdef SM_RES_TRACE
-          { long long n = clock64(); tr_a += n - tr_t; tr_t = n; }
-#endif
-          ptx::mbar_wait(b_wready, p_w, a.err_flag, 23); p_w ^= 1u;
-          ptx::tc_fence_after();
-#ifdef SM_RES_TRACE
-          { long long n = clock64(); tr_b += n - tr_t; tr_t = n; }
-#endif
-          bool last = k + 1 == a.max_iter;
-          if (a.tol > 0.0 && residual_now(s.m) < a.tol) last = true;
-          // ---- product 2: X Wh^T (A = rows of XS, B = Wh from WS: stored rows K-major, the rest through the transpose)
-          for (int t = 0; t < (s.two ? 2 : 1); ++t) {
-            const uint32_t d = tmem_base + (t ? 128u : 0u);
-            for (int kc = 0; kc < s.nkc; ++kc) {
-              const uint64_t ad = ptx::make_sw128_kmajor_desc(xs + (uint32_t)kc * Pd * 128u + (t ? 128u * 128u : 0u));
-              const int ksteps = min(4, (s.kmax - kc * 64) / 16);
-              const uint32_t acc0 = (uint32_t)(kc != 0);
-              if (kc < 2) {
-                const uint32_t N = t ? Pd : (uint32_t)s.n0;
-                const uint32_t idesc = ptx::make_idesc_f16(bf, 128, N, false);
-                const uint64_t bd = ptx::make_sw128_kmajor_desc(ws + res_woff((uint32_t)kc, Pd));
-                if (ksteps == 4) {
+        };
+        // product 2 (A = rows of XS, B = Wh from WS: stored rows K-major, the rest through the transpose)
+        auto p2 = [&](int t, int k_lo, int k_hi, bool first) {
+          const uint32_t d = t ? dT1 : dT0b;
+          for (int kc = k_lo; kc < k_hi; ++kc) {
+            const uint64_t ad = ptx::make_sw128_kmajor_desc(xs + (uint32_t)kc * Pd * 128u + (t ? 128u * 128u : 0u));
+            const int ksteps = min(4, (s.kmax - kc * 64) / 16);
+            const uint32_t acc0 = (uint32_t)(!first || kc != k_lo);
+            if (kc < 2) {
+              const uint32_t N = t ? Pd : (uint32_t)s.n0;
+              const uint32_t idesc = ptx::make_idesc_f16(bf, 128, N, false);
+              const uint64_t bd = ptx::make_sw128_kmajor_desc(ws + res_woff((uint32_t)kc, Pd));
+              if (ksteps == 4) {
 #pragma unroll
                 for (int ks = 0; ks < 4; ++ks) ptx::umma_f16_elect(d, ad + (uint64_t)(2 * ks), bd + (uint64_t)(2 * ks), idesc, acc0 | (uint32_t)(ks != 0));
               } else {
                 for (int ks = 0; ks < ksteps; ++ks) ptx::umma_f16_elect(d, ad + (uint64_t)(2 * ks), bd + (uint64_t)(2 * ks), idesc, acc0 | (uint32_t)(ks != 0));
               }
-              } else {
-                // output columns 0..127: Wh[n][k] = Wh[k][n], rows 64 kc.. of chunks 0 and 1, MN-major
-                const uint32_t idesc_t = ptx::make_idesc_f16(bf, 128, 128, true);
-                const uint64_t bt = ptx::make_sw128_mnmajor_desc(ws + (uint32_t)kc * 64u * 128u, Pd * 128u, 1024u);
-                if (ksteps == 4) {
+            } else {
+              // output columns 0..127: Wh[n][k] = Wh[k][n], rows 64 kc.. of chunks 0 and 1, MN-major;
+              // output columns 128..Pd-1 (T1 only): rows 128.. of chunk kc are stored, K-major
+              const uint32_t idesc_t = ptx::make_idesc_f16(bf, 128, 128, true);
+              const uint64_t bt = ptx::make_sw128_mnmajor_desc(ws + (uint32_t)kc * 64u * 128u, Pd * 128u, 1024u);
+              const uint32_t idesc_d = ptx::make_idesc_f16(bf, 128, t ? Pd - 128u : 16u, false);
+              const uint64_t bd = ptx::make_sw128_kmajor_desc(ws + res_woff((uint32_t)kc, Pd));
+              if (ksteps == 4) {
 #pragma unroll
-                for (int ks = 0; ks < 4; ++ks) ptx::umma_f16_elect(d, ad + (uint64_t)(2 * ks), bt + (uint64_t)(128 * ks), idesc_t, 1u);
+                for (int ks = 0; ks < 4; ++ks) {
+                  ptx::umma_f16_elect(d, ad + (uint64_t)(2 * ks), bt + (uint64_t)(128 * ks), idesc_t, acc0 | (uint32_t)(ks != 0));
+                  if (t) ptx::umma_f16_elect(d + 128u, ad + (uint64_t)(2 * ks), bd + (uint64_t)(2 * ks), idesc_d, acc0 | (uint32_t)(ks != 0));
+                }
               } else {
-                for (int ks = 0; ks < ksteps; ++ks) ptx::umma_f16_elect(d, ad + (uint64_t)(2 * ks), bt + (uint64_t)(128 * ks), idesc_t, 1u);
-              }
-                if (t) {
-                  // output columns 128..Pd-1: rows 128.. of chunk kc are stored, K-major
-                  const uint32_t idesc_d = ptx::make_idesc_f16(bf, 128, Pd - 128u, false);
-                  const uint64_t bd = ptx::make_sw128_kmajor_desc(ws + res_woff((uint32_t)kc, Pd));
-                  if (ksteps == 4) {
-#pragma unroll
-                for (int ks = 0; ks < 4; ++ks) ptx::umma_f16_elect(d + 128u, ad + (uint64_t)(2 * ks), bd + (uint64_t)(2 * ks), idesc_d, 1u);
-              } else {
-                for (int ks = 0; ks < ksteps; ++ks) ptx::umma_f16_elect(d + 128u, ad + (uint64_t)(2 * ks), bd + (uint64_t)(2 * ks), idesc_d, 1u);
-              }
+                for (int ks = 0; ks < ksteps; ++ks) {
+                  ptx::umma_f16_elect(d, ad + (uint64_t)(2 * ks), bt + (uint64_t)(128 * ks), idesc_t, acc0 | (uint32_t)(ks != 0));
+                  if (t) ptx::umma_f16_elect(d + 128u, ad + (uint64_t)(2 * ks), bd + (uint64_t)(2 * ks), idesc_d, acc0 | (uint32_t)(ks != 0));
                 }
               }
             }
-            ptx::umma_commit_elect(t ? b_tfull1 : b_tfull0);
           }
-#ifdef SM_RES_TRACE
-          { long long n = clock64(); tr_c += n - tr_t; tr_t = n; }
-#endif
-          ptx::mbar_wait(b_xready, p_x, a.err_flag, 24); p_x ^= 1u;
+        };
+        const int klo = s.two ? 2 : s.nkc;            // chunks [0, klo) = columns 0..127; single tile: everything
+        for (int32_t k = 0; k < a.max_iter; ++k) {
+          if (k == a.switch_iter) bf = false;     // 0 < switch_iter < max_iter (host-checked), tol <= 0
+          // ---- product 1
+          if (k > 0) { ptx::mbar_wait(b_x0, p_x0, a.err_flag, 24); p_x0 ^= 1u; ptx::tc_fence_after(); }
+          p1(0, 0, min(klo, s.nkc), true);
+          if (k > 0) { ptx::mbar_wait(b_x1, p_x1, a.err_flag, 24); p_x1 ^= 1u; ptx::tc_fence_after(); }
+          if (s.two) {
+            p1(1, 0, s.nkc, true);
+            ptx::umma_commit_elect(b_tfull1);
+            p1(0, klo, s.nkc, false);
+          }
+          ptx::umma_commit_elect(b_tfull0);
+          // ---- product 2
+          ptx::mbar_wait(b_w1, p_w1, a.err_flag, 23); p_w1 ^= 1u;
           ptx::tc_fence_after();
-#ifdef SM_RES_TRACE
-          { long long n = clock64(); tr_d += n - tr_t; tr_t = n; }
-          if (last && blockIdx.x == 0 && lane == 0) printf("res trace c=%lld m=%d Pd=%d steps=%d issue1=%lld wait1=%lld issue2=%lld wait2=%lld (cycles per step)\n", (long long)c, s.m, s.Pd, k + 1, tr_a / (k + 1), tr_b / (k + 1), tr_c / (k + 1), tr_d / (k + 1));
-#endif
-          if (last) break;
+          if (s.two) { p2(0, klo, s.nkc, true); p2(1, klo, s.nkc, true); }
+          ptx::mbar_wait(b_w0, p_w0, a.err_flag, 23); p_w0 ^= 1u;
+          ptx::tc_fence_after();
+          bool last = k + 1 == a.max_iter;
+          if (a.tol > 0.0 && residual_now(s.m) < a.tol) last = true;
+          p2(0, 0, min(klo, s.nkc), !s.two);
+          ptx::umma_commit_elect(b_tfull0);
+          if (s.two) { p2(1, 0, klo, false); ptx::umma_commit_elect(b_tfull1); }
+          if (last) {
+            // nothing follows this submatrix: consume the two X' barriers so that the parities stay in step
+            ptx::mbar_wait(b_x0, p_x0, a.err_flag, 24); p_x0 ^= 1u;
+            ptx::mbar_wait(b_x1, p_x1, a.err_flag, 24); p_x1 ^= 1u;
+            ptx::tc_fence_after();
+            break;
+          }
         }
       }
     }
@@ -236,7 +250,7 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_umma_resident(RArgs a) {
     const int w = warp - 2;
     const int q = warp & 3;                       // TMEM lane quadrant this warp may access
     const int sub = w >> 2;                       // which column blocks of the quadrant's rows it takes
-    uint32_t p_xload = 0, p_t[2] = {0, 0}, p_w = 0, p_x = 0;
+    uint32_t p_xload = 0, p_t[2] = {0, 0}, p_w0 = 0, p_x0 = 0, p_x1 = 0;
     for (;;) {
       ptx::mbar_wait(b_xload, p_xload, a.err_flag, 25); p_xload ^= 1u;
       const int64_t c = *cur_c;
@@ -261,8 +275,8 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_umma_resident(RArgs a) {
             ptx::mbar_wait(t ? b_tfull1 : b_tfull0, p_t[t], a.err_flag, 26); p_t[t] ^= 1u;
             ptx::tc_fence_after();
             const int32_t R0 = 128 * t + 32 * q;
-            if (R0 >= s.Pd) continue;
-            const uint32_t taddr = tmem_base + (t ? 128u : 0u) + ((uint32_t)(q * 32) << 16);
+            if (R0 < s.Pd) {
+            const uint32_t taddr = tmem_base + (t ? 128u : (P2 ? 384u : 0u)) + ((uint32_t)(q * 32) << 16);
             const uint32_t rb = ((uint32_t)R0 & 63u) >> 3;            // first 16-byte chunk of columns R0.. in their line
             for (int bi = sub; bi * 32 <= R0; bi += RES_EPI_WARPS / 4) {
               const int32_t C0 = bi * 32;
@@ -341,34 +355,43 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_umma_resident(RArgs a) {
                 }
               }
             }
+            }   // R0 < Pd
+            // this tile's part of Wh / X' is written and its accumulator drained: tell the MMA issuer.  (The residual
+            // partial of the step goes out with the LAST tile of product 1, T0.)
+            if (!P2 && t == 0) {
+              float rs = res + 2.f * res2;
+              for (int d = 16; d > 0; d >>= 1) rs += __shfl_xor_sync(0xffffffffu, rs, d);
+              if (lane == 0) res_s[w] = rs;
+            }
+            ptx::tc_fence_before();
+            ptx::fence_proxy_async_smem();          // generic-proxy stores -> the MMA's async-proxy reads
+            __syncwarp();
+            if (lane == 0) ptx::mbar_arrive(P2 ? (t ? b_x1 : b_x0) : (t ? b_w1 : b_w0));
           }
+          if (!s.two && lane == 0) ptx::mbar_arrive(P2 ? b_x1 : b_w1);      // single tile: the T1 barriers complete as well
           res += 2.f * res2;
         };
 
         // ---- epilogue 1: Wh -> WS, residual
         float res = 0.f;
         pass(false, bf, res);
-        for (int d = 16; d > 0; d >>= 1) res += __shfl_xor_sync(0xffffffffu, res, d);
-        if (lane == 0) res_s[w] = res;
-        ptx::tc_fence_before();
-        ptx::fence_proxy_async_smem();          // generic-proxy stores -> the MMA's async-proxy reads
-        __syncwarp();
-        if (lane == 0) ptx::mbar_arrive(b_wready);
-        ptx::mbar_wait(b_wready, p_w, a.err_flag, 27); p_w ^= 1u;
         bool last = k + 1 == a.max_iter;
-        if (a.tol > 0.0 || last) r_last = residual_now(s.m);      // fixed counts: only the last residual is reported
+        ptx::mbar_wait(b_w0, p_w0, a.err_flag, 27); p_w0 ^= 1u;        // all 16 partial sums of the step are there
+        if (a.tol > 0.0 || last) r_last = residual_now(s.m);          // fixed counts: only the last residual is reported
         if (a.tol > 0.0 && r_last < a.tol) last = true;
         // ---- epilogue 2: X' -> XS (the update that reaches switch_iter writes fp16)
         const bool bf_next = bf && (k + 1 != a.switch_iter);
         float dummy = 0.f;
         pass(true, bf_next, dummy);
-        ptx::tc_fence_before();
-        ptx::fence_proxy_async_smem();
-        __syncwarp();
-        if (lane == 0) ptx::mbar_arrive(b_xready);
-        ptx::mbar_wait(b_xready, p_x, a.err_flag, 28); p_x ^= 1u;
         bf = bf_next;
         iters_done = k + 1;
+        // the partial sums of this step are consumed by every role before any warp can rewrite its slot: a warp
+        // rewrites it in the next step's epilogue 1, which follows MMAs that the issuer starts only after b_x0 / b_x1,
+        // i.e. after every warp has passed this point
+        if (last || k + 1 == a.max_iter) {
+          ptx::mbar_wait(b_x0, p_x0, a.err_flag, 28); ptx::mbar_wait(b_x1, p_x1, a.err_flag, 28);
+        }
+        p_x0 ^= 1u; p_x1 ^= 1u;
         if (last) break;
       }
       if (w == 0 && lane == 0) {
