@@ -493,9 +493,9 @@ def run_ours(args, cfg, cfg_run):
         flops_per_launch = flops_step * args.steps / max(gemm_launches, 1)
         achieved = flops_per_launch / (avg_ms * 1e-3) / 1e12
         if x_dtype == "f64":
-            te = np.ceil(dims[order] / 128.0)
-            pd = np.ceil(dims[order] / pad) * pad
-            issued_step = float((2 * 2.0 * 128 * 128 * (te * (te + 1) / 2) * np.ceil(dims[order] / 16.0) * 16 * k_eff).sum()) \
+            tl = 64.0 if dims.max() <= 384 else 128.0        # k_dmma_gemm tile edge (sign_simt.cu: by the largest submatrix)
+            te = np.ceil(dims[order] / tl)
+            issued_step = float((2 * 2.0 * tl * tl * (te * (te + 1) / 2) * np.ceil(dims[order] / 16.0) * 16 * k_eff).sum()) \
                 if dims.max() > 96 else flops_step
         else:
             te = np.ceil(dims[order] / 64.0)           # k_ffma_sym: lower-triangle 64 x 64 tiles

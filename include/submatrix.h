@@ -284,6 +284,7 @@ int32_t sm_density_from_sign(const sm_bcsr_t *A, const sm_pattern_t *P, int32_t 
  *   "umma.stages"   [SM_UMMA_STAGES]   0|3|4 16-bit grouped tiles: depth of the operand ring (0 = by size)
  *   "umma.stream"   [SM_UMMA_STREAM]   0|1   16-bit, tol <= 0: one launch walks every product of every step
  *   "f64.simt"      [SM_F64_SIMT]      0|1   fp64: tensor-core m8n8k4 tiles / DFMA register tiles
+ *   "f64.tile"      [SM_F64_TILE]      0|64|128  fp64 tensor-core tile edge (0: 64 when the largest submatrix is <= 384, else 128)
  *   "f32.sym"       [SM_F32_SYM]       1|0   fp32: lower-triangle 64 x 64 FFMA tiles with 8 x 8 register blocks and mirrored
  *                                            stores (exactly symmetric iterates) / all tiles with 4 x 4 blocks
  *   "gather.tma"    [SM_GATHER_TMA]    0|1   sm_gather, 16-bit X: element-wise kernel / source-driven kernel staged through

@@ -131,9 +131,15 @@ k_simt_gemm(const int32_t *__restrict__ cols, const int64_t *__restrict__ col_of
 //   Bs[16][132]  rows k of X (PHASE 1) or Y (PHASE 2), n contiguous (true product, no transposition).
 // Padding rows/columns of X, Y and the alternate buffer hold zeros (gather / memset), so loads are only
 // bounded by the padded dimension.
-constexpr int DT = 128, DK = 16, DLA = 20, DLB = 132;
-constexpr int DMMA_STAGE_DOUBLES = DT * DLA + DK * DLB;
-constexpr int DMMA_SMEM = 2 * DMMA_STAGE_DOUBLES * 8;
+// TILE = 128 (8 warps as 4 x 2, warp tile 32 x 64) for large submatrices, TILE = 64 (warp tile 16 x 32) where 128-row tiles
+// would mostly multiply padding (m ~ 186 pads to 2 x 2 tiles of 128 = 1.9x the work; to 3 x 3 tiles of 64 = 1.07x).
+constexpr int DT = 128, DK = 16, DLA = 20;
+template <int TILE> struct DCfg {
+  static constexpr int LB = TILE + 4;
+  static constexpr int STAGE_DOUBLES = TILE * DLA + DK * LB;
+  static constexpr int SMEM = 2 * STAGE_DOUBLES * 8;
+};
+constexpr int DMMA_SMEM = DCfg<128>::SMEM;
 
 __device__ __forceinline__ void dmma_m8n8k4(double (&d)[2], double a, double b) {
   asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};"
@@ -146,7 +152,7 @@ __device__ __forceinline__ void cp_async16(void *smem, const void *gmem, bool va
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(sa), "l"(gmem), "r"(n) : "memory");
 }
 
-template <int PHASE, bool SYM>
+template <int PHASE, bool SYM, int TILE = 128>
 __global__ void __launch_bounds__(256)
 k_dmma_gemm(const int32_t *__restrict__ cols, const int64_t *__restrict__ col_off,
             const int32_t *__restrict__ dim, const int32_t *__restrict__ dim_pad, int32_t max_tiles_edge,
@@ -159,39 +165,41 @@ k_dmma_gemm(const int32_t *__restrict__ cols, const int64_t *__restrict__ col_of
   if (PHASE == 1 && s.last[c]) return;
   const int32_t i = cols ? cols[c] : c;
   const int32_t m = dim[i], Pd = dim_pad[i];
-  const int32_t te = (m + DT - 1) / DT;
+  constexpr int DLB = DCfg<TILE>::LB, DMMA_STAGE_DOUBLES = DCfg<TILE>::STAGE_DOUBLES;
+  constexpr int NA = TILE / 32, NB = TILE / 16;                 // m8n8 accumulators per warp: NA x NB
+  const int32_t te = (m + TILE - 1) / TILE;
   const int32_t tr = t / max_tiles_edge, tc = t - tr * max_tiles_edge;
   if (tr >= te || tc >= te || (SYM && tc > tr)) return;       // SYM: lower-triangle tiles only
   const double *A = Xsrc + col_off[c];
   const double *B = (PHASE == 1 ? Xsrc : Ybuf) + col_off[c];
   double *O = Out + col_off[c];
-  const int32_t row0 = tr * DT, col0 = tc * DT;
+  const int32_t row0 = tr * TILE, col0 = tc * TILE;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int wr = (warp >> 1) * 32, wc = (warp & 1) * 64;      // warp tile origin inside the CTA tile
+  const int wr = (warp >> 1) * (TILE / 4), wc = (warp & 1) * (TILE / 2);      // warp tile origin inside the CTA tile
   const int g = lane >> 2, q = lane & 3;
 
-  double acc[4][8][2];
+  double acc[NA][NB][2];
 #pragma unroll
-  for (int a = 0; a < 4; ++a)
+  for (int a = 0; a < NA; ++a)
 #pragma unroll
-    for (int b = 0; b < 8; ++b) acc[a][b][0] = acc[a][b][1] = 0.0;
+    for (int b = 0; b < NB; ++b) acc[a][b][0] = acc[a][b][1] = 0.0;
 
   auto load_stage = [&](int st, int32_t k0) {
-    double *As = dsm + st * DMMA_STAGE_DOUBLES, *Bs = As + DT * DLA;
-    // A: 128 rows x 8 chunks of 2 doubles
+    double *As = dsm + st * DMMA_STAGE_DOUBLES, *Bs = As + TILE * DLA;
+    // A: TILE rows x 8 chunks of 2 doubles
 #pragma unroll
-    for (int l = 0; l < 4; ++l) {
+    for (int l = 0; l < TILE / 32; ++l) {
       int e = threadIdx.x + l * 256;
       int r = e >> 3, ch = e & 7;
       int32_t gr = row0 + r, gk = k0 + ch * 2;
       bool ok = gr < Pd && gk < Pd;
       cp_async16(As + r * DLA + ch * 2, ok ? A + (int64_t)gr * Pd + gk : A, ok);
     }
-    // B: 16 k rows x 64 chunks of 2 doubles
+    // B: 16 k rows x TILE / 2 chunks of 2 doubles
 #pragma unroll
-    for (int l = 0; l < 4; ++l) {
+    for (int l = 0; l < TILE / 32; ++l) {
       int e = threadIdx.x + l * 256;
-      int k = e >> 6, ch = e & 63;
+      int k = e / (TILE / 2), ch = e % (TILE / 2);
       int32_t gk = k0 + k, gc = col0 + ch * 2;
       bool ok = gk < Pd && gc < Pd;
       cp_async16(Bs + k * DLB + ch * 2, ok ? B + (int64_t)gk * Pd + gc : B, ok);
@@ -209,18 +217,18 @@ k_dmma_gemm(const int32_t *__restrict__ cols, const int64_t *__restrict__ col_of
       asm volatile("cp.async.wait_group 0;" ::: "memory");
     }
     __syncthreads();
-    const double *As = dsm + (kc & 1) * DMMA_STAGE_DOUBLES, *Bs = As + DT * DLA;
+    const double *As = dsm + (kc & 1) * DMMA_STAGE_DOUBLES, *Bs = As + TILE * DLA;
 #pragma unroll
     for (int k4 = 0; k4 < DK; k4 += 4) {
-      double af[4], bf[8];
+      double af[NA], bf[NB];
 #pragma unroll
-      for (int a = 0; a < 4; ++a) af[a] = As[(wr + a * 8 + g) * DLA + k4 + q];
+      for (int a = 0; a < NA; ++a) af[a] = As[(wr + a * 8 + g) * DLA + k4 + q];
 #pragma unroll
-      for (int b = 0; b < 8; ++b) bf[b] = Bs[(k4 + q) * DLB + wc + b * 8 + g];
+      for (int b = 0; b < NB; ++b) bf[b] = Bs[(k4 + q) * DLB + wc + b * 8 + g];
 #pragma unroll
-      for (int a = 0; a < 4; ++a)
+      for (int a = 0; a < NA; ++a)
 #pragma unroll
-        for (int b = 0; b < 8; ++b) dmma_m8n8k4(acc[a][b], af[a], bf[b]);
+        for (int b = 0; b < NB; ++b) dmma_m8n8k4(acc[a][b], af[a], bf[b]);
     }
     __syncthreads();
   }
@@ -231,10 +239,10 @@ k_dmma_gemm(const int32_t *__restrict__ cols, const int64_t *__restrict__ col_of
   // count twice in the residual.
   double res = 0.0;
 #pragma unroll
-  for (int a = 0; a < 4; ++a) {
+  for (int a = 0; a < NA; ++a) {
     const int32_t gr = row0 + wr + a * 8 + g;
 #pragma unroll
-    for (int b = 0; b < 8; ++b) {
+    for (int b = 0; b < NB; ++b) {
 #pragma unroll
       for (int e = 0; e < 2; ++e) {
         const int32_t gc = col0 + wc + b * 8 + 2 * q + e;
@@ -419,7 +427,9 @@ static int32_t sign_simt_t(const sm_pattern_t *P, const int32_t *cols, int32_t n
   const bool dmma = sizeof(T) == 8 && opt(OPT_F64_SIMT) == 0 && P->max_dim > 96;
   // fp32, symmetric iterates: lower-triangle 64 x 64 tiles with 8 x 8 register blocks (option "f32.sym", default on)
   const bool fsym = sizeof(T) == 4 && !nonsym && opt(OPT_F32_SYM) != 0 && (P->pad_to & 3) == 0;
-  const int32_t TS = dmma ? DT : ST;
+  // fp64 tiles: 64 x 64 where 128-row tiles would mostly multiply padding (option "f64.tile": 0 = by size, 64, 128)
+  const int32_t dt = !dmma ? ST : (!nonsym && (opt(OPT_F64_TILE) == 64 || (opt(OPT_F64_TILE) == 0 && P->max_dim <= 384))) ? 64 : DT;
+  const int32_t TS = dt;
   const int32_t edge = (P->max_dim + TS - 1) / TS;
   const int64_t grid64 = (int64_t)n_cols * edge * edge;
   if (grid64 > 0x7fffffffLL) return SM_ERR_UNSUPPORTED;
@@ -440,6 +450,8 @@ static int32_t sign_simt_t(const sm_pattern_t *P, const int32_t *cols, int32_t n
     SM_CUDA(cudaFuncSetAttribute(k_dmma_gemm<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, DMMA_SMEM));
     SM_CUDA(cudaFuncSetAttribute(k_dmma_gemm<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, DMMA_SMEM));
     SM_CUDA(cudaFuncSetAttribute(k_dmma_gemm<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, DMMA_SMEM));
+    SM_CUDA(cudaFuncSetAttribute(k_dmma_gemm<1, true, 64>, cudaFuncAttributeMaxDynamicSharedMemorySize, DCfg<64>::SMEM));
+    SM_CUDA(cudaFuncSetAttribute(k_dmma_gemm<2, true, 64>, cudaFuncAttributeMaxDynamicSharedMemorySize, DCfg<64>::SMEM));
     // padding of Y and of the alternate X buffer must read as zeros (the kernel stores true elements only)
     SM_CUDA(cudaMemsetAsync(w.Y, 0, packed_elems * sizeof(T), st));
     SM_CUDA(cudaMemsetAsync(w.X2, 0, packed_elems * sizeof(T), st));
@@ -455,6 +467,9 @@ static int32_t sign_simt_t(const sm_pattern_t *P, const int32_t *cols, int32_t n
     if (dmma && nonsym)
       k_dmma_gemm<1, false><<<grid, 256, DMMA_SMEM, st>>>(cols, col_off, P->dim, P->dim_pad, edge, (const double *)src,
                                                           (const double *)Y, (double *)Y, s);
+    else if (dmma && dt == 64)
+      k_dmma_gemm<1, true, 64><<<grid, 256, DCfg<64>::SMEM, st>>>(cols, col_off, P->dim, P->dim_pad, edge, (const double *)src,
+                                                                 (const double *)Y, (double *)Y, s);
     else if (dmma)
       k_dmma_gemm<1, true><<<grid, 256, DMMA_SMEM, st>>>(cols, col_off, P->dim, P->dim_pad, edge, (const double *)src,
                                                          (const double *)Y, (double *)Y, s);
@@ -471,6 +486,9 @@ static int32_t sign_simt_t(const sm_pattern_t *P, const int32_t *cols, int32_t n
     if (dmma && nonsym)
       k_dmma_gemm<2, false><<<grid, 256, DMMA_SMEM, st>>>(cols, col_off, P->dim, P->dim_pad, edge, (const double *)src,
                                                           (const double *)Y, (double *)dst, s);
+    else if (dmma && dt == 64)
+      k_dmma_gemm<2, true, 64><<<grid, 256, DCfg<64>::SMEM, st>>>(cols, col_off, P->dim, P->dim_pad, edge, (const double *)src,
+                                                                 (const double *)Y, (double *)dst, s);
     else if (dmma)
       k_dmma_gemm<2, true><<<grid, 256, DMMA_SMEM, st>>>(cols, col_off, P->dim, P->dim_pad, edge, (const double *)src,
                                                          (const double *)Y, (double *)dst, s);
