@@ -327,7 +327,7 @@ template <bool BF16, int PHASE, int NCTA, bool SYM, bool MC = false, int NST = 0
 __global__ void __launch_bounds__(UMMA_THREADS, 1)
 k_umma_gemm(UArgs a, const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapB) {
   static_assert(!DYN || NCTA == 1, "dynamic tile scheduling: one CTA per tile");
-  static_assert(EPI == 0 || (SYM && NCTA == 1 && PHASE != 0), "staged epilogue: single CTAs, SYM tiles, one launch per product");
+  static_assert(EPI == 0 || (SYM && NCTA == 1), "staged epilogue: single CTAs, SYM tiles");
   constexpr bool STG = EPI == 1;
   static_assert(PHASE != 0 || (DYN && SYM), "stream mode needs the dynamic deal and symmetric tiles");
   constexpr bool STREAM = PHASE == 0;
@@ -693,6 +693,7 @@ k_umma_gemm(UArgs a, const __grid_constant__ CUtensorMap mapA, const __grid_cons
     const bool leader = warp == 2 + 8 * team && lane == 0;
     auto team_bar = [&]() { asm volatile("bar.sync %0, %1;" ::"r"(1 + team), "r"(256) : "memory"); };
     const int g = lane >> 2, q2 = lane & 3, rl = lane & 7, ml = lane >> 3;
+    int32_t *pend = nullptr;                       // stream: completion counter of the tile whose stores are in flight
     uint32_t it = 0;
     TileDesc nxt = load_desc(a, max((int64_t)0, min(unit, total - 1)));
     int64_t t = unit;
@@ -717,9 +718,16 @@ k_umma_gemm(UArgs a, const __grid_constant__ CUtensorMap mapA, const __grid_cons
       UTile u = make_tile<PHASE>(a, cur);
       if (!u.valid) continue;
       const uint32_t as = it % NACC, aphase = (it / NACC) & 1u;
-      constexpr bool p1 = PHASE == 1;
-      uint16_t *Og = (uint16_t *)a.Out + u.base;
+      const bool p1 = STREAM ? (cur.pad0 & 1) == 0 : PHASE == 1;
+      // stream: product ph of step ph / 2 writes Wh (even ph) or the X buffer that step does not read (odd ph)
+      uint16_t *Og = (uint16_t *)(!STREAM ? a.Out : p1 ? a.Ybuf : (((cur.pad0 >> 1) & 1) ? (void *)a.Xsrc : a.Out)) + u.base;
       if (SM_DBG(a, 1)) Og = nullptr;
+      if (STREAM && leader) {
+        // completion of the PREVIOUS tile's bulk stores is signalled one tile late, so that the wait for the stores to
+        // land overlaps this tile's MMAs instead of stalling the team (the dependants are whole products away)
+        if (pend) { ptx::bulk_wait0(); __threadfence(); atomicAdd(pend, EPI_WARPS / 2); pend = nullptr; }
+        if (cur.pad0 + 1 < a.n_ph) pend = a.done + (int64_t)cur.pad1 * a.n_ph + cur.pad0;
+      }
       const int32_t R0 = u.row0 + q * 32;                     // this warp's 32 rows of the tile
       const int32_t a_rows = min(UM, u.Pd - u.row0);
       const int32_t n_below = max(0, min(u.nt, u.row0 - u.n0)) >> 6;   // whole chunks left of the diagonal square
@@ -831,7 +839,10 @@ k_umma_gemm(UArgs a, const __grid_constant__ CUtensorMap mapA, const __grid_cons
       }
       ++it;
     }
-    if (leader) ptx::bulk_wait0();
+    if (leader) {
+      ptx::bulk_wait0();
+      if (STREAM && pend) { __threadfence(); atomicAdd(pend, EPI_WARPS / 2); }
+    }
   } else {
     // ===================== epilogue (warps 2..17) =====================
     // EPI_WARPS / 4 warps per TMEM lane quadrant; a warp owns 32 rows and every (EPI_WARPS/4)-th
@@ -1089,8 +1100,8 @@ static int32_t umma_dbg() {
 static int32_t umma_sym_mode(int32_t nonsym, bool fused, int32_t ncta, double tol, int32_t max_iter) {
   if (fused) return 1;
   if (nonsym || opt(OPT_UMMA_SYM) == 0) return 0;
-  const bool stream = opt(OPT_UMMA_STREAM) == 1 && !(tol > 0.0) && max_iter > 0;
-  return (opt(OPT_UMMA_EPI) != 0 && ncta == 1 && !stream) ? 2 : 1;
+  (void)tol; (void)max_iter;
+  return (opt(OPT_UMMA_EPI) != 0 && ncta == 1) ? 2 : 1;
 }
 // all listed columns with Pd <= this go through k_umma_resident (0: none)
 static int32_t umma_resident_pd(int32_t sym) { return (sym && opt(OPT_UMMA_RESIDENT) != 0) ? RES_MAX_PD : 0; }
@@ -1345,7 +1356,8 @@ int32_t sign_umma(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, co
     SM_CUDA(cudaMemsetAsync(w.done, 0, sizeof(int32_t) * n_done, st));
     UArgs a{cols, col_off, P->dim, P->dim_pad, w.tile_ptr, w.tiles, n_cols, 0, X, w.Y, w.X2, s, w.err, 0, w.counters,
             2 * max_iter, w.done, umma_dbg(), 0, 0, 0};
-    int32_t rc = launch_umma_t<0, 1, true, false, 0, false, true>(bf16, a, maps[0], n_sm, st);
+    int32_t rc = sym == 2 ? launch_umma_t<0, 1, true, false, 0, false, true, 1>(bf16, a, maps[0], n_sm, st)
+                          : launch_umma_t<0, 1, true, false, 0, false, true>(bf16, a, maps[0], n_sm, st);
     if (rc != SM_OK) return rc;
     k_fused_post<<<(n_cols + 7) / 8, 256, 0, st>>>(n_cols, cols, P->dim, P->dim_pad, res_pd, w.partial, w.parts_per_col, w.n_parts,
                                                    max_iter, iters, residual);

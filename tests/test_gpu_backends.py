@@ -146,6 +146,7 @@ SYM_VARIANTS = [
     {"SM_UMMA_RESIDENT": "0", "SM_UMMA_EPI": "1"},
     {"SM_UMMA_RESIDENT": "0", "SM_UMMA_EPI": "1", "SM_UMMA_DYN": "0"},
     {"SM_UMMA_RESIDENT": "0", "SM_UMMA_EPI": "1", "SM_UMMA_LT": "1"},
+    {"SM_UMMA_RESIDENT": "0", "SM_UMMA_EPI": "1", "SM_UMMA_STREAM": "1"},
 ]
 SYM_VARIANTS_MEASURE = [
     {"SM_UMMA_FUSED": "0", "SM_UMMA_NCTA": "2", "SM_UMMA_MC": "1"},
