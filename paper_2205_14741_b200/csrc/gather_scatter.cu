@@ -254,7 +254,7 @@ __global__ void __launch_bounds__(256) k_gather(GatherArgs g, const TA *__restri
 // instructions per output element, issue-bound at 0.29 of the HBM peak) the work per output
 // element is ~1/4.  Arithmetic and rounding are those of k_gather (fp32, one rounding): the images are bit-identical.
 constexpr int GS_ROWS = 64, GS_TILE_CHUNKS = 4, GS_TILE_BYTES = GS_TILE_CHUNKS * GS_ROWS * 128;
-constexpr int GS_MAX_PAIRS = 512, GS_UNROLL = 6;
+constexpr int GS_MAX_PAIRS = 512;
 
 template <typename TA, typename TX>
 __global__ void __launch_bounds__(256) k_gather_staged(GatherArgs g, const TA *__restrict__ vals, TX *__restrict__ X) {
@@ -268,7 +268,8 @@ __global__ void __launch_bounds__(256) k_gather_staged(GatherArgs g, const TA *_
   const uint32_t base = (raw + 1023u) & ~1023u;
   uint8_t *const tile0 = gs_smem + (base - raw);
   int64_t *const pair_src = reinterpret_cast<int64_t *>(tile0 + 2 * GS_TILE_BYTES);          // [GS_MAX_PAIRS]
-  int32_t *const off = reinterpret_cast<int32_t *>(tile0 + 2 * GS_TILE_BYTES + GS_MAX_PAIRS * 8);
+  uint16_t *const rowblk = reinterpret_cast<uint16_t *>(tile0 + 2 * GS_TILE_BYTES + GS_MAX_PAIRS * 8);    // [GS_ROWS]
+  int32_t *const off = reinterpret_cast<int32_t *>(tile0 + 2 * GS_TILE_BYTES + GS_MAX_PAIRS * 8 + GS_ROWS * 2);
   const int32_t lo = g.rp[i], cnt = g.rp[i + 1] - lo;
   for (int32_t a = threadIdx.x; a < cnt; a += blockDim.x) off[a] = g.row_off[lo + a];
   if (threadIdx.x == 0) off[cnt] = m;
@@ -284,6 +285,10 @@ __global__ void __launch_bounds__(256) k_gather_staged(GatherArgs g, const TA *_
     while (h - l > 1) { const int32_t mid = (l + h) >> 1; if (off[mid] < r1) l = mid; else h = mid; }
     a_hi = l + 1;
   }
+  // neighbour block of every true row of the band
+  for (int32_t a = a_lo + threadIdx.x; a < a_hi; a += blockDim.x)
+    for (int32_t r = max(off[a], r0); r < min(off[a + 1], r1); ++r) rowblk[r - r0] = (uint16_t)a;
+  __syncthreads();
   const int32_t *gm = g.gmap + g.gmap_ptr[i];
   const float inv_sf = (float)(1.0 / g.scale[c_list]), muf = (float)g.mu;
   char *Xs = (char *)(X + g.col_off[c_list]);
@@ -303,48 +308,40 @@ __global__ void __launch_bounds__(256) k_gather_staged(GatherArgs g, const TA *_
       while (cb_lo + 1 < cnt && off[cb_lo + 1] <= c_beg) ++cb_lo;
       int32_t cb_hi = cb_lo;
       while (cb_hi < cnt && off[cb_hi] < c_end) ++cb_hi;
-      const int32_t n_c = cb_hi - cb_lo, n_pairs = (a_hi - a_lo) * n_c;
-      // resolve the pairs of the tile in parallel (gather-map entry -> value offset: two dependent loads per pair, taken
-      // by one thread each instead of in front of every warp's copy loop)
-      for (int32_t q0 = 0; q0 < n_pairs; q0 += GS_MAX_PAIRS) {
-        const int32_t nq = min(GS_MAX_PAIRS, n_pairs - q0);
+      const int32_t n_c = cb_hi - cb_lo, n_a = a_hi - a_lo, nrows = r1 - r0;
+      // column blocks in chunks whose (row block, column block) pairs fit the table; the pairs are resolved in parallel
+      // first (gather-map entry -> value offset: two dependent loads per pair), then every thread takes items
+      // (row of the band, column block): it walks the row of the stored block (consecutive source addresses; the
+      // lanes of a warp are consecutive rows of the same block, i.e. one contiguous piece of memory) and writes the
+      // elements to their swizzled places in the tile
+      const int32_t cbc = max(1, GS_MAX_PAIRS / n_a);
+      for (int32_t c0 = 0; c0 < n_c; c0 += cbc) {
+        const int32_t nc_here = min(cbc, n_c - c0);
         __syncthreads();
-        for (int32_t q = threadIdx.x; q < nq; q += blockDim.x) {
-          const int32_t a = a_lo + (q0 + q) / n_c, cb = cb_lo + (q0 + q) % n_c;
+        for (int32_t q = threadIdx.x; q < n_a * nc_here; q += blockDim.x) {
+          const int32_t a = a_lo + q / nc_here, cb = cb_lo + c0 + q % nc_here;
           const int32_t p = __ldg(gm + (int64_t)a * cnt + cb);
           pair_src[q] = p >= 0 ? __ldg(g.vp + p) : -1;
         }
         __syncthreads();
-        for (int32_t q = warp; q < nq; q += 8) {
-          const int64_t so = pair_src[q];
+        for (int32_t it = threadIdx.x; it < nrows * nc_here; it += blockDim.x) {
+          const int32_t cbi = it / nrows, rl = it - cbi * nrows;
+          const int32_t r = r0 + rl, a = rowblk[rl], cb = cb_lo + c0 + cbi;
+          const int64_t so = pair_src[(a - a_lo) * nc_here + cbi];
           if (so < 0) continue;                                            // absent pair: stays zero
-          const int32_t a = a_lo + (q0 + q) / n_c, cb = cb_lo + (q0 + q) % n_c;
-          const int32_t ra0 = off[a], ba = off[a + 1] - ra0, rc0 = off[cb], bc = off[cb + 1] - rc0;
-          const TA *src = vals + so;
-          // rows of the block inside the band, all columns of the block (those outside the tile are skipped per element)
-          const int32_t ra_lo = max(0, r0 - ra0), ra_hi = min(ba, r1 - ra0);
-          const float inv_bc = 1.0f / (float)bc;
-          const int32_t e_hi = ra_hi * bc;
-          for (int32_t e0 = ra_lo * bc + lane; e0 < e_hi; e0 += 32 * GS_UNROLL) {
-            TA xv[GS_UNROLL];
-#pragma unroll
-            for (int u = 0; u < GS_UNROLL; ++u) {                         // all loads of the batch first: memory-level parallelism
-              const int32_t e = e0 + 32 * u;
-              xv[u] = e < e_hi ? __ldg(src + e) : (TA)0;
-            }
-#pragma unroll
-            for (int u = 0; u < GS_UNROLL; ++u) {
-              const int32_t e = e0 + 32 * u;
-              const int32_t ra = (int32_t)(((float)e + 0.5f) * inv_bc), rc = e - ra * bc;
-              const int32_t r = ra0 + ra, c = rc0 + rc;
-              if (e >= e_hi || c < c_beg || c >= c_end) continue;
-              float x = (float)xv[u];
-              if (r == c) x -= muf;
-              const TX v = from_float<TX>(x * inv_sf);
-              const uint32_t o = (uint32_t)((c - c_beg) >> 6) * (GS_ROWS * 128u) + (uint32_t)(r - r0) * 128u +
-                                 (((((uint32_t)c & 63u) >> 3) ^ ((uint32_t)r & 7u)) << 4) + ((uint32_t)c & 7u) * 2u;
-              *reinterpret_cast<TX *>(tile + o) = v;
-            }
+          const int32_t rc0 = off[cb], bc = off[cb + 1] - rc0;
+          const TA *src = vals + so + (int64_t)(r - off[a]) * bc;
+          const int32_t rc_lo = max(0, c_beg - rc0), rc_hi = min(bc, c_end - rc0);
+          uint8_t *const trow = tile + (uint32_t)rl * 128u;
+          const uint32_t r7 = (uint32_t)r & 7u;
+#pragma unroll 4
+          for (int32_t rc = rc_lo; rc < rc_hi; ++rc) {
+            const int32_t c = rc0 + rc;
+            float x = (float)__ldg(src + rc);
+            if (r == c) x -= muf;
+            const uint32_t o = (uint32_t)((c - c_beg) >> 6) * (GS_ROWS * 128u) + (((((uint32_t)c & 63u) >> 3) ^ r7) << 4) +
+                               ((uint32_t)c & 7u) * 2u;
+            *reinterpret_cast<TX *>(trow + o) = from_float<TX>(x * inv_sf);
           }
         }
       }
@@ -573,7 +570,7 @@ static int32_t launch_gather(const GatherArgs &g, const void *vals, void *X, int
   dim3 grid(n_cols, (max_pd + GATHER_ROWS - 1) / GATHER_ROWS);
   if constexpr (IMG) {
     if (opt(OPT_GATHER_TMA) != 0) {
-      const int smem_s = 2 * GS_TILE_BYTES + 1024 + GS_MAX_PAIRS * 8 + (max_nbr + 1) * 4 + 16;
+      const int smem_s = 2 * GS_TILE_BYTES + 1024 + GS_MAX_PAIRS * 8 + GS_ROWS * 2 + (max_nbr + 1) * 4 + 16;
       SM_CUDA(cudaFuncSetAttribute(k_gather_staged<TA, TX>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_s));
       k_gather_staged<TA, TX><<<grid, 256, smem_s, st>>>(g, (const TA *)vals, (TX *)X);
       SM_LAUNCHED();
