@@ -727,3 +727,51 @@ def test_global_scale_is_a_valid_deterministic_bound(sm):
     d_or, _ = orc.density_columns(wl0, n_threads=THREADS)
     _, _, plan = run_density(sm, wl0, "f64", 100, 1e-8, "global")
     assert np.abs(plan.D.cpu().numpy() - d_or).max() <= 1e-10
+
+
+# ------------------------------------------------------------------- tile-boundary sweep
+
+SWEEP_M = [1, 2, 15, 16, 17, 31, 33, 63, 64, 65, 96, 127, 128, 129, 191, 192, 193, 255, 256, 257, 319, 321, 383, 385, 447, 449,
+           511, 513, 577, 640, 703, 767, 769, 1000, 1023, 1025, 1281, 1537]
+_sweep_ref = {}
+
+
+def _sweep_reference(k):
+    """NS-k reference iterates of the sweep workload: the Jacobi oracle for m <= 257, its LAPACK variant (pinned to the Jacobi
+    path in test_oracle_pins.py) above, where cyclic Jacobi takes 10 s .. minutes per submatrix."""
+    if k not in _sweep_ref:
+        ms = np.array(SWEEP_M, dtype=np.int32)
+        wl = make_workload(len(ms), ms, np.maximum(1, ms // 3), 0.0, seed=91)
+        small = [i for i, m in enumerate(SWEEP_M) if m <= 257]
+        large = [i for i, m in enumerate(SWEEP_M) if m > 257]
+        d_s, _ = orc.density_columns(wl, cols=small, mode="nsk", k_fixed=k, n_threads=THREADS)
+        d_l, _ = orc.density_columns_lapack(wl, cols=large, mode="nsk", k_fixed=k)
+        _sweep_ref[k] = (wl, d_s + d_l)
+    return _sweep_ref[k]
+
+
+@pytest.mark.parametrize("x_dtype,pad,tol_abs", [("bf16", 64, 1.5e-2), ("f16", 64, 2e-3), ("f64", 16, 1e-12), ("f32", 16, 1e-5)])
+def test_submatrix_dimension_sweep_across_tile_boundaries(sm, x_dtype, pad, tol_abs):
+    """One block-diagonal workload whose diagonal blocks have the dimensions of SWEEP_M (cutoff 0: T_i = H_ii), so one call
+    runs a submatrix of every size around the tile / chunk / panel boundaries of all kernels (resident kernel: 64, 128, 192,
+    256; grouped tiles: 128-row panels, 256-column tiles, 64-column chunks, 32-column epilogue blocks, 16-element k
+    steps; DMMA / FFMA tiles of 64 and 128; scatter strips) through gather, k = 4 Newton-Schulz steps, scatter and density.
+    With cutoff 0 the only block of column i is the whole of D_i = (I - X_i) / 2, so every element of every iterate is
+    compared with the oracle's NS-4 polynomial; the symmetric kernels must also give exactly symmetric blocks."""
+    k = 4
+    wl, d_ref = _sweep_reference(k)
+    A = sm.Bcsr(wl)
+    P = sm.sm_build_pattern(A, pad)
+    assert np.array_equal(sm.pattern_to_host(P).dim, np.array(SWEEP_M))
+    plan = sm.DensityPlan(A, P, x_dtype)
+    sm.sm_density(A, P, plan, 0.0, "gershgorin", k, 0.0)
+    torch.cuda.synchronize()
+    assert (plan.iters == k).all()
+    d = plan.D.cpu().numpy().astype(np.float64)
+    vp = np.asarray(wl.val_ptr, dtype=np.int64)
+    for i, m in enumerate(SWEEP_M):
+        blk = d[vp[i]:vp[i + 1]].reshape(m, m)
+        ref = d_ref[vp[i]:vp[i + 1]].reshape(m, m)
+        err = np.abs(blk - ref).max()
+        assert err <= tol_abs, (m, err)
+        assert np.array_equal(blk, blk.T), (m, "iterate must be exactly symmetric")
