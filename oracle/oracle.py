@@ -128,14 +128,15 @@ def sign(T: np.ndarray) -> np.ndarray:
     return S
 
 
-def ns_polynomial(T: np.ndarray, scale: float, k: int) -> np.ndarray:
-    """Exact-arithmetic result of k Newton-Schulz steps from T/scale (reading A13)."""
+def ns_polynomial(T: np.ndarray, scale: float, k: int, order: int = 2) -> np.ndarray:
+    """Exact-arithmetic result of k Newton-Schulz steps from T/scale (reading A13).  order 3 (f3, reading A22):
+    k steps of x <- x (15 - 10 x^2 + 3 x^4) / 8 instead of x <- x (3 - x^2) / 2."""
     w, V, _ = jacobi_eigh(T)
     m = T.shape[0]
     S = np.zeros((m, m))
     Vt = np.ascontiguousarray(V.T)
-    lib().orc_nsk_from_eig(C.c_int32(m), _p(Vt, C.c_double), _p(w, C.c_double), C.c_double(scale),
-                           C.c_int32(k), _p(S, C.c_double))
+    fn = {2: lib().orc_nsk_from_eig, 3: lib().orc_ns3k_from_eig}[order]
+    fn(C.c_int32(m), _p(Vt, C.c_double), _p(w, C.c_double), C.c_double(scale), C.c_int32(k), _p(S, C.c_double))
     return S
 
 
@@ -144,7 +145,8 @@ def density_columns(w, mu: float = 0.0, cols=None, mode: str = "exact", k_fixed:
     """Raw D = 1/2 (I - sign(T_i - mu I)) blocks of the listed block columns (all if None).
 
     Returns (d_vals in H's block-CSR layout with only the listed columns' blocks
-    written, stats).  mode "nsk": the NS-k polynomial at scale (Gershgorin if None).
+    written, stats).  mode "nsk": the NS-k polynomial at scale (Gershgorin if None); "ns3k": k_fixed steps of the
+    third-order iteration (f3, reading A22).
     """
     vp = np.ascontiguousarray(w.val_ptr, dtype=np.int64)
     vals = np.ascontiguousarray(w.vals, dtype=np.float64)
@@ -156,7 +158,7 @@ def density_columns(w, mu: float = 0.0, cols=None, mode: str = "exact", k_fixed:
     sc = None if scale is None else np.ascontiguousarray(scale, dtype=np.float64)
     rc = lib().orc_density_columns(
         *_csr(w), _p(vp, C.c_int64), _p(vals, C.c_double), C.c_double(mu), C.c_int32(nc),
-        _p(cols_a, C.c_int32), C.c_int32(0 if mode == "exact" else 1), C.c_int32(k_fixed),
+        _p(cols_a, C.c_int32), C.c_int32({"exact": 0, "nsk": 1, "ns3k": 2}[mode]), C.c_int32(k_fixed),
         _p(sc, C.c_double), _p(d, C.c_double), _p(st.min_abs_eig, C.c_double),
         _p(st.scale, C.c_double), _p(st.sweeps, C.c_int32), _p(st.n_neg, C.c_int32),
         C.c_int32(n_threads))
@@ -247,7 +249,7 @@ def density_columns_lapack(w, mu: float = 0.0, cols=None, mode: str = "exact", k
         else:
             x = lam / (gs if scale is None else float(scale[ci]))
             for _ in range(k_fixed):
-                x = 0.5 * x * (3.0 - x * x)
+                x = x * (15.0 - 10.0 * x * x + 3.0 * x ** 4) / 8.0 if mode == "ns3k" else 0.5 * x * (3.0 - x * x)
             f = x
         S = (V * f) @ V.T
         nb = np.asarray(w.col_idx[w.row_ptr[i]:w.row_ptr[i + 1]])

@@ -316,6 +316,27 @@ void orc_nsk_from_eig(int32_t m, const double *Vt, const double *w, double scale
     free(f);
 }
 
+/* Third-order iteration, k steps ("various iterative methods", reading A22 in
+ * DESIGN.md): V diag(g3^k(w/scale)) V^T with g3(x) = x (15 - 10 x^2 + 3 x^4) / 8, the next member after
+ * g(x) = x (3 - x^2) / 2 of the family x (1 - w)^-1/2, w = 1 - x^2, truncated after w^2:
+ * x (1 + w/2 + 3 w^2 / 8).  Fixed points 0, +-1, +-sqrt(7/3); g3' = g3'' = 0 at +-1 (cubic convergence);
+ * converges to sgn(x) for 0 < |x| < sqrt(7/3). */
+void orc_ns3k_from_eig(int32_t m, const double *Vt, const double *w, double scale, int32_t k,
+                       double *S)
+{
+    double *f = (double *)malloc((size_t)(m > 0 ? m : 1) * sizeof(double));
+    for (int32_t e = 0; e < m; ++e) {
+        double x = w[e] / scale;
+        for (int32_t it = 0; it < k; ++it) {
+            double x2 = x * x;
+            x = x * (15.0 - 10.0 * x2 + 3.0 * x2 * x2) / 8.0;
+        }
+        f[e] = x;
+    }
+    spectral_sum(m, Vt, f, S);
+    free(f);
+}
+
 /* --------------------------- steps 1-3 + Eq. 14 for a list of block columns */
 
 typedef struct {
@@ -326,7 +347,7 @@ typedef struct {
     double mu;
     int32_t n_cols;
     const int32_t *cols;
-    int32_t mode;          /* 0: exact sign; 1: NS-k polynomial with Gershgorin scale */
+    int32_t mode;          /* 0: exact sign; 1: NS-k polynomial with Gershgorin scale; 2: third-order, k steps */
     int32_t k_fixed;
     const double *scale_in; /* mode 1: optional per-column scale (NULL -> Gershgorin) */
     double *d_vals;        /* out: D = 1/2 (I - S) blocks of the listed columns, A's layout */
@@ -356,6 +377,7 @@ static void density_one(orc_job_t *J, int32_t ci)
     double mn = INFINITY; int32_t nneg = 0;
     for (int32_t k = 0; k < m; ++k) { if (fabs(w[k]) < mn) mn = fabs(w[k]); if (w[k] < 0.0) ++nneg; }
     if (J->mode == 0) orc_sign_from_eig(m, Vt, w, S);
+    else if (J->mode == 2) orc_ns3k_from_eig(m, Vt, w, J->scale_in ? J->scale_in[ci] : gs, J->k_fixed, S);
     else orc_nsk_from_eig(m, Vt, w, J->scale_in ? J->scale_in[ci] : gs, J->k_fixed, S);
     /* step 3: rows = all of N(i), columns = local position of block i.
      * By structural symmetry block (N(i)[a'], i) is found in row N(i)[a']. */

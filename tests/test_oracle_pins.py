@@ -127,6 +127,61 @@ def test_ns_polynomial_scalar_recursion_and_limit():
     T = _rand_sym(16, 34)
     assert np.abs(orc.ns_polynomial(T, orc.gershgorin(T), 60) - orc.sign(T)).max() < 1e-10
 
+# ------------------------------------------------------------ third-order iteration (f3, reading A22)
+
+@pytest.mark.parametrize("k", [0, 1, 4, 9])
+def test_ns3_polynomial_equals_matrix_iteration(k):
+    # spectral form == k explicit steps X <- X (I + W/2 + 3 W^2 / 8), W = I - X^2 (the series of (I - W)^-1/2 cut after W^2)
+    T = _rand_sym(24, 35)
+    s = orc.gershgorin(T)
+    X = T / s
+    eye = np.eye(24)
+    for _ in range(k):
+        W = eye - X @ X
+        X = X @ (eye + 0.5 * W + 0.375 * W @ W)
+    assert np.abs(orc.ns_polynomial(T, s, k, order=3) - X).max() < 1e-12
+
+
+def test_ns3_scalar_map_fixed_points_order_and_basin():
+    g3 = lambda x: float(orc.ns_polynomial(np.array([[x]]), 1.0, 1, order=3)[0, 0])
+    # fixed points 0, +-1 and the repelling pair +-sqrt(7/3) (3 x^4 - 10 x^2 + 7 = 0)
+    for x in (0.0, 1.0, -1.0, np.sqrt(7.0 / 3.0), -np.sqrt(7.0 / 3.0)):
+        assert abs(g3(x) - x) < 1e-14
+    # odd; g3 = x (15 - 10 x^2 + 3 x^4) / 8 at a rational point: g3(1/2) = (1/2)(15 - 5/2 + 3/16)/8 = 203/256
+    assert g3(0.5) == 203.0 / 256.0 and g3(-0.5) == -203.0 / 256.0
+    # cubic contact at 1: g3(1 - e) = 1 - (5/2) e^3 + O(e^4)  (first and second derivative vanish at 1, the third is 15)
+    for e in (1e-2, 1e-3):
+        assert abs((1.0 - g3(1.0 - e)) / e ** 3 - 2.5) < 4.0 * e
+    # basin: converges to sgn(x) inside sqrt(7/3) = 1.5275, leaves it outside (order 2: sqrt(3))
+    conv = lambda x, k: float(orc.ns_polynomial(np.array([[x]]), 1.0, k, order=3)[0, 0])
+    assert abs(conv(1.52, 12) - 1.0) < 1e-12 and abs(conv(-1.52, 12) + 1.0) < 1e-12
+    assert abs(conv(1.535, 6)) > 10.0           # escapes (overflows to inf/nan a few steps later)
+    # small x grow by 15/8 per step instead of 3/2: x0 = 1e-3 is converged after 15 order-3 steps, order 2 needs ~22
+    x2 = float(orc.ns_polynomial(np.array([[1e-3]]), 1.0, 15)[0, 0])
+    assert abs(conv(1e-3, 1) / 1e-3 - 1.875) < 1e-5
+    assert abs(conv(1e-3, 15) - 1.0) < 1e-12 and abs(x2 - 1.0) > 0.3
+
+
+def test_ns3_converges_to_sign_and_density_modes_agree():
+    T = _rand_sym(16, 36)
+    assert np.abs(orc.ns_polynomial(T, orc.gershgorin(T), 40, order=3) - orc.sign(T)).max() < 1e-10
+    w = make_workload(6, 4, 2, 7.0, seed=5)
+    d_j, _ = orc.density_columns(w, mode="ns3k", k_fixed=5)
+    d_l, _ = orc.density_columns_lapack(w, mode="ns3k", k_fixed=5)
+    assert np.abs(d_j - d_l).max() < 1e-12
+    # column 0 by hand: D blocks = owned columns of (I - p(T_0)) / 2
+    T0 = orc.gather(w, 0)
+    S0 = orc.ns_polynomial(T0, orc.gershgorin(T0), 5, order=3)
+    nb = w.col_idx[w.row_ptr[0]:w.row_ptr[1]]
+    own = int(np.where(nb == 0)[0][0])
+    p = int(w.row_ptr[0]) + own
+    b = int(w.blk_size[0])
+    blk = d_j[w.val_ptr[p]:w.val_ptr[p + 1]].reshape(b, b)
+    assert np.abs(blk - 0.5 * (np.eye(b) - S0[own * b:(own + 1) * b, own * b:(own + 1) * b])).max() < 1e-13
+    d2, _ = orc.density_columns(w, mode="nsk", k_fixed=5)
+    assert np.abs(d2 - d_j).max() > 1e-6          # and it is a different polynomial than order 2
+
+
 
 def test_gershgorin_bounds_spectral_radius():
     T = _rand_sym(50, 40)
