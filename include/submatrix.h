@@ -170,8 +170,14 @@ int32_t sm_sign_ns(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols,
  *     bf16 operands, update switch_iter-1 rounds its result to fp16 and the remaining updates run on fp16 operands
  *     (same kind::f16 MMA, 11 instead of 8 significand bits; |x| <= ~1 after scaling, so the range is safe).
  *     X_packed then holds SM_F16 images on return.
+ *   flags & SM_SIGN_ORDER3: the third-order member of the same family instead of Newton-Schulz ("various
+ *     iterative methods"; reading A22): X <- X (15 I - 10 X^2 + 3 X^4) / 8, three products per
+ *     step, cubic convergence, basin |x| < sqrt(7/3).  Same workspace, same stopping rule (the residual of step k is
+ *     still ||X_k^2 - I||_F / sqrt(m)); symmetric matrices only (with SM_SIGN_NONSYMMETRIC: SM_ERR_UNSUPPORTED); all
+ *     four x_dtype (16-bit: Q = 3/4 (I - X^2), Z = 2/3 (Q + Q Q), X' = X + X Z on the grouped tcgen05 kernels).
  * ws >= sm_sign_ws_bytes_ex(..., flags). */
 #define SM_SIGN_NONSYMMETRIC 1
+#define SM_SIGN_ORDER3 2
 int64_t sm_sign_ws_bytes_ex(const sm_pattern_t *P, int32_t n_cols, int64_t packed_elems, int32_t x_dtype,
                             int32_t flags);
 int32_t sm_sign_ns_ex(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols,
@@ -203,6 +209,10 @@ int32_t sm_symmetrise(const sm_bcsr_t *A, const sm_pattern_t *P, int32_t r_dtype
  * packed elements per chunk (>= max_dim_pad^2; P->packed_elems for a single chunk).  Asynchronous. */
 int64_t sm_density_ws_bytes(const sm_bcsr_t *A, const sm_pattern_t *P, int32_t x_dtype,
                             int64_t max_chunk_elems);
+/* The same for sm_density_ex(..., sign_flags, ...) (sm_density_ws_bytes = sign_flags 0): the third-order iteration
+ * keeps two scratch images even where Newton-Schulz runs entirely on chip. */
+int64_t sm_density_ws_bytes_ex(const sm_bcsr_t *A, const sm_pattern_t *P, int32_t x_dtype,
+                               int64_t max_chunk_elems, int32_t sign_flags);
 int32_t sm_density(const sm_bcsr_t *A, const void *A_vals, int32_t a_dtype, double mu,
                    int32_t x_dtype, int32_t scale_mode, int32_t max_iter, double tol,
                    int32_t symmetrise, const sm_pattern_t *P, const int32_t *h_dim_pad /*host [N]*/,
@@ -211,10 +221,11 @@ int32_t sm_density(const sm_bcsr_t *A, const void *A_vals, int32_t a_dtype, doub
                    void *stream);
 /* sm_density with a precision schedule (SURVEY 8(f) f3; PAPER.md:104 "FP16 operations with FP32 accumulation", :15):
  * switch_iter >= 0 (x_dtype SM_BF16, tol <= 0, 0 < switch_iter < max_iter) runs the first switch_iter updates on bf16
- * operands and the rest on fp16 operands (see sm_sign_ns_ex); switch_iter < 0 is sm_density. */
+ * operands and the rest on fp16 operands (see sm_sign_ns_ex); switch_iter < 0 is sm_density.  sign_flags: 0 or
+ * SM_SIGN_ORDER3 (third-order iteration in a3, see sm_sign_ns_ex); anything else is SM_ERR_ARG. */
 int32_t sm_density_ex(const sm_bcsr_t *A, const void *A_vals, int32_t a_dtype, double mu,
                       int32_t x_dtype, int32_t scale_mode, int32_t max_iter, double tol, int32_t switch_iter,
-                      int32_t symmetrise, const sm_pattern_t *P, const int32_t *h_dim_pad /*host [N]*/,
+                      int32_t sign_flags, int32_t symmetrise, const sm_pattern_t *P, const int32_t *h_dim_pad /*host [N]*/,
                       int64_t max_chunk_elems, void *ws, int64_t ws_bytes, int32_t d_dtype,
                       void *D_vals, double *trace, int32_t *iters, double *residual, double *scale,
                       void *stream);

@@ -34,8 +34,9 @@ EXPORTS = ["sm_last_cuda_error", "sm_pattern_sizes", "sm_build_pattern", "sm_pla
            "sm_scatter", "sm_symmetrise", "sm_density_ws_bytes", "sm_density", "sm_density_from_sign",
            "sm_mu_search", "sm_launch_count", "sm_profile_enable", "sm_profile_read", "sm_sign_ws_bytes_ex",
            "sm_sign_ns_ex", "sm_set_option", "sm_get_option", "sm_build_info", "sm_last_device_error",
-           "sm_inv_sqrt_ws_bytes", "sm_inv_sqrt", "sm_density_nonorth_ws_bytes", "sm_density_nonorth", "sm_density_ex"]
-SM_SIGN_NONSYMMETRIC = 1
+           "sm_inv_sqrt_ws_bytes", "sm_inv_sqrt", "sm_density_nonorth_ws_bytes", "sm_density_nonorth", "sm_density_ex",
+           "sm_density_ws_bytes_ex"]
+SM_SIGN_NONSYMMETRIC, SM_SIGN_ORDER3 = 1, 2      # sm_sign_ns_ex flags
 
 
 class SmError(RuntimeError):
@@ -72,6 +73,7 @@ _lib.sm_sign_ws_bytes_ex.restype = C.c_int64
 _lib.sm_inv_sqrt_ws_bytes.restype = C.c_int64
 _lib.sm_density_nonorth_ws_bytes.restype = C.c_int64
 _lib.sm_density_ws_bytes.restype = C.c_int64
+_lib.sm_density_ws_bytes_ex.restype = C.c_int64
 
 
 def _ptr(t):
@@ -250,7 +252,7 @@ def sm_sign_ws_bytes(P: Pattern, n_cols, n_elems, x_dtype, flags=0) -> int:
 
 def sm_sign_ns(P: Pattern, cols, col_off, n_cols, n_elems, x_dtype, X, max_iter, tol, ws=None,
                iters=None, residual=None, flags=0, switch_iter=-1):
-    """flags / switch_iter non-default: sm_sign_ns_ex (non-symmetric matrices, bf16 -> fp16 schedule)."""
+    """flags / switch_iter non-default: sm_sign_ns_ex (non-symmetric matrices, third-order iteration, bf16 -> fp16 schedule)."""
     x_dt = DTYPES[x_dtype] if isinstance(x_dtype, str) else x_dtype
     if ws is None:
         ws = torch.empty(sm_sign_ws_bytes(P, n_cols, n_elems, x_dt, flags), dtype=torch.uint8, device=P.device)
@@ -306,12 +308,14 @@ def sm_density_from_sign(A: Bcsr, P: Pattern, RD, d_dtype="f64"):
 class DensityPlan:
     """Buffers for repeated sm_density calls on one geometry (allocated once)."""
 
-    def __init__(self, A: Bcsr, P: Pattern, x_dtype, max_chunk_elems=None, d_dtype="f64"):
+    def __init__(self, A: Bcsr, P: Pattern, x_dtype, max_chunk_elems=None, d_dtype="f64", order=2):
         self.x_dt = DTYPES[x_dtype] if isinstance(x_dtype, str) else x_dtype
         self.d_dt = DTYPES[d_dtype] if isinstance(d_dtype, str) else d_dtype
         self.max_chunk_elems = int(max_chunk_elems or P.packed_elems)
-        wsb = int(_lib.sm_density_ws_bytes(C.byref(A.c), C.byref(P.c), C.c_int32(self.x_dt),
-                                           C.c_int64(self.max_chunk_elems)))
+        self.order = order          # workspace sized for sm_density(..., order=this)
+        wsb = int(_lib.sm_density_ws_bytes_ex(C.byref(A.c), C.byref(P.c), C.c_int32(self.x_dt),
+                                              C.c_int64(self.max_chunk_elems),
+                                              C.c_int32(SM_SIGN_ORDER3 if order == 3 else 0)))
         if wsb < 0:
             raise SmError("sm_density_ws_bytes", wsb)
         dev = A.device
@@ -325,15 +329,21 @@ class DensityPlan:
 
 
 def sm_density(A: Bcsr, P: Pattern, plan: DensityPlan, mu=0.0, scale_mode="gershgorin", max_iter=100,
-               tol=0.0, symmetrise=False, A_vals=None, switch_iter=-1):
+               tol=0.0, symmetrise=False, A_vals=None, switch_iter=-1, order=2):
     """Whole path; returns the plan (D, trace, iters, residual, scale live in it; the per-column
-    arrays are indexed by position in P.order).  switch_iter >= 0: bf16 -> fp16 schedule (sm_density_ex)."""
+    arrays are indexed by position in P.order).  switch_iter >= 0: bf16 -> fp16 schedule; order = 3: third-order
+    iteration in a3 (both through sm_density_ex)."""
     sc = SCALES[scale_mode] if isinstance(scale_mode, str) else scale_mode
     vals = A.vals if A_vals is None else A_vals
-    if switch_iter >= 0:
+    if order not in (2, 3):
+        raise ValueError("order must be 2 or 3")
+    if order == 3 and plan.order != 3:
+        raise ValueError("the plan's workspace was sized for order 2: DensityPlan(..., order=3)")
+    if switch_iter >= 0 or order == 3:
         _check("sm_density_ex", _lib.sm_density_ex(
             C.byref(A.c), _ptr(vals), C.c_int32(A.val_dtype), C.c_double(mu), C.c_int32(plan.x_dt), C.c_int32(sc),
-            C.c_int32(max_iter), C.c_double(tol), C.c_int32(switch_iter), C.c_int32(1 if symmetrise else 0), C.byref(P.c),
+            C.c_int32(max_iter), C.c_double(tol), C.c_int32(switch_iter), C.c_int32(SM_SIGN_ORDER3 if order == 3 else 0),
+            C.c_int32(1 if symmetrise else 0), C.byref(P.c),
             plan.h_dim_pad.ctypes.data_as(C.c_void_p), C.c_int64(plan.max_chunk_elems), _ptr(plan.ws),
             C.c_int64(plan.ws.numel()), C.c_int32(plan.d_dt), _ptr(plan.D), _ptr(plan.trace), _ptr(plan.iters),
             _ptr(plan.residual), _ptr(plan.scale), _stream()))

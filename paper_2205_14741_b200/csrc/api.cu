@@ -129,7 +129,9 @@ extern "C" int32_t sm_last_device_error(void) {
 extern "C" int64_t sm_sign_ws_bytes_ex(const sm_pattern_t *P, int32_t n_cols, int64_t packed_elems,
                                        int32_t x_dtype, int32_t flags) {
   if (!P || n_cols <= 0 || packed_elems <= 0) return SM_ERR_ARG;
-  if (is_16bit(x_dtype)) return sign_umma_ws_bytes(P, n_cols, packed_elems, x_dtype, flags & SM_SIGN_NONSYMMETRIC);
+  if (flags & ~(SM_SIGN_NONSYMMETRIC | SM_SIGN_ORDER3)) return SM_ERR_ARG;
+  if (is_16bit(x_dtype))
+    return sign_umma_ws_bytes(P, n_cols, packed_elems, x_dtype, flags & SM_SIGN_NONSYMMETRIC, (flags & SM_SIGN_ORDER3) ? 3 : 2);
   if (x_dtype == SM_F32 || x_dtype == SM_F64) return sign_simt_ws_bytes(P, n_cols, packed_elems, x_dtype);
   return SM_ERR_UNSUPPORTED;
 }
@@ -145,16 +147,17 @@ extern "C" int32_t sm_sign_ns_ex(const sm_pattern_t *P, const int32_t *cols, int
   if (!P || !col_off || !X_packed || !ws || !iters || !residual) return SM_ERR_ARG;
   if (!cols) n_cols = P->n_blk;
   if (n_cols <= 0 || max_iter < 0 || packed_elems <= 0) return SM_ERR_ARG;
-  if (flags & ~SM_SIGN_NONSYMMETRIC) return SM_ERR_ARG;
+  if (flags & ~(SM_SIGN_NONSYMMETRIC | SM_SIGN_ORDER3)) return SM_ERR_ARG;
   cudaStream_t st = (cudaStream_t)stream;
-  const int32_t nonsym = flags & SM_SIGN_NONSYMMETRIC;
+  const int32_t nonsym = flags & SM_SIGN_NONSYMMETRIC, order = (flags & SM_SIGN_ORDER3) ? 3 : 2;
+  if (order == 3 && nonsym) return SM_ERR_UNSUPPORTED;
   if (is_16bit(x_dtype))
     return sign_umma(P, cols, n_cols, col_off, packed_elems, x_dtype, X_packed, ws, ws_bytes, max_iter, tol,
-                     iters, residual, nonsym, switch_iter, st);
+                     iters, residual, nonsym, switch_iter, order, st);
   if (switch_iter >= 0) return SM_ERR_ARG;
   if (x_dtype == SM_F32 || x_dtype == SM_F64)
     return sign_simt(P, cols, n_cols, col_off, packed_elems, x_dtype, X_packed, ws, ws_bytes, max_iter, tol,
-                     iters, residual, nonsym, st);
+                     iters, residual, nonsym, order, st);
   return SM_ERR_UNSUPPORTED;
 }
 extern "C" int32_t sm_sign_ns(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols,
@@ -186,25 +189,30 @@ namespace {
 struct DensityWs { int64_t *col_off; void *X; void *gws; int64_t gws_bytes; void *sws; int64_t sws_bytes; int64_t used; };
 
 DensityWs density_layout(void *ws, int64_t ws_bytes, const sm_bcsr_t *A, const sm_pattern_t *P, int32_t x_dtype,
-                         int64_t max_chunk_elems) {
+                         int64_t max_chunk_elems, int32_t sign_flags) {
   WsCursor cur(ws, ws_bytes);
   DensityWs w;
   w.col_off = cur.take<int64_t>(P->n_blk + 1);
   w.X = cur.take<char>(max_chunk_elems * dtype_bytes(x_dtype));
   w.gws_bytes = sm_gather_ws_bytes(A, P, P->n_blk);
   w.gws = cur.take<char>(w.gws_bytes);
-  w.sws_bytes = sm_sign_ws_bytes(P, P->n_blk, max_chunk_elems, x_dtype);
+  w.sws_bytes = sm_sign_ws_bytes_ex(P, P->n_blk, max_chunk_elems, x_dtype, sign_flags);
   w.sws = cur.take<char>(w.sws_bytes > 0 ? w.sws_bytes : 1);
   w.used = cur.used + 256;
   return w;
 }
 }  // namespace
 
-extern "C" int64_t sm_density_ws_bytes(const sm_bcsr_t *A, const sm_pattern_t *P, int32_t x_dtype,
-                                       int64_t max_chunk_elems) {
+extern "C" int64_t sm_density_ws_bytes_ex(const sm_bcsr_t *A, const sm_pattern_t *P, int32_t x_dtype,
+                                          int64_t max_chunk_elems, int32_t sign_flags) {
   if (!A || !P || dtype_bytes(x_dtype) == 0) return SM_ERR_ARG;
   if (max_chunk_elems < (int64_t)P->max_dim_pad * P->max_dim_pad) return SM_ERR_ARG;
-  return density_layout(nullptr, 0, A, P, x_dtype, max_chunk_elems).used;
+  if (sign_flags & ~SM_SIGN_ORDER3) return SM_ERR_ARG;
+  return density_layout(nullptr, 0, A, P, x_dtype, max_chunk_elems, sign_flags).used;
+}
+extern "C" int64_t sm_density_ws_bytes(const sm_bcsr_t *A, const sm_pattern_t *P, int32_t x_dtype,
+                                       int64_t max_chunk_elems) {
+  return sm_density_ws_bytes_ex(A, P, x_dtype, max_chunk_elems, 0);
 }
 
 extern "C" int32_t sm_density(const sm_bcsr_t *A, const void *A_vals, int32_t a_dtype, double mu,
@@ -213,13 +221,13 @@ extern "C" int32_t sm_density(const sm_bcsr_t *A, const void *A_vals, int32_t a_
                               int64_t max_chunk_elems, void *ws, int64_t ws_bytes, int32_t d_dtype,
                               void *D_vals, double *trace, int32_t *iters, double *residual, double *scale,
                               void *stream) {
-  return sm_density_ex(A, A_vals, a_dtype, mu, x_dtype, scale_mode, max_iter, tol, -1, symmetrise, P, h_dim_pad,
+  return sm_density_ex(A, A_vals, a_dtype, mu, x_dtype, scale_mode, max_iter, tol, -1, 0, symmetrise, P, h_dim_pad,
                        max_chunk_elems, ws, ws_bytes, d_dtype, D_vals, trace, iters, residual, scale, stream);
 }
 
 extern "C" int32_t sm_density_ex(const sm_bcsr_t *A, const void *A_vals, int32_t a_dtype, double mu,
                                  int32_t x_dtype, int32_t scale_mode, int32_t max_iter, double tol, int32_t switch_iter,
-                                 int32_t symmetrise, const sm_pattern_t *P, const int32_t *h_dim_pad,
+                                 int32_t sign_flags, int32_t symmetrise, const sm_pattern_t *P, const int32_t *h_dim_pad,
                                  int64_t max_chunk_elems, void *ws, int64_t ws_bytes, int32_t d_dtype,
                                  void *D_vals, double *trace, int32_t *iters, double *residual, double *scale,
                                  void *stream) {
@@ -227,7 +235,8 @@ extern "C" int32_t sm_density_ex(const sm_bcsr_t *A, const void *A_vals, int32_t
   if (dtype_bytes(x_dtype) == 0) return SM_ERR_UNSUPPORTED;
   if (d_dtype != SM_F64 && d_dtype != SM_F32) return SM_ERR_UNSUPPORTED;
   if (max_chunk_elems < (int64_t)P->max_dim_pad * P->max_dim_pad) return SM_ERR_ARG;
-  DensityWs w = density_layout(ws, ws_bytes, A, P, x_dtype, max_chunk_elems);
+  if (sign_flags & ~SM_SIGN_ORDER3) return SM_ERR_ARG;       // the density path is symmetric
+  DensityWs w = density_layout(ws, ws_bytes, A, P, x_dtype, max_chunk_elems, sign_flags);
   if (w.sws_bytes < 0) return (int32_t)w.sws_bytes;
   if (w.used > ws_bytes) return SM_ERR_SPACE;
   const int32_t n = P->n_blk;
@@ -252,7 +261,7 @@ extern "C" int32_t sm_density_ex(const sm_bcsr_t *A, const void *A_vals, int32_t
     rc = sm_gather(A, A_vals, a_dtype, P, cols, nc, w.col_off, mu, scale_mode, x_dtype, w.X, scale + lo, w.gws,
                    w.gws_bytes, stream);
     if (rc != SM_OK) return rc;
-    rc = sm_sign_ns_ex(P, cols, nc, w.col_off, elems, x_dtype, w.X, w.sws, w.sws_bytes, max_iter, tol, 0, switch_iter,
+    rc = sm_sign_ns_ex(P, cols, nc, w.col_off, elems, x_dtype, w.X, w.sws, w.sws_bytes, max_iter, tol, sign_flags, switch_iter,
                        iters + lo, residual + lo, stream);
     if (rc != SM_OK) return rc;
     // after a bf16 -> fp16 schedule the images hold fp16

@@ -118,15 +118,16 @@ int32_t power_scale(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, 
 // switch_iter >= 0: bf16 -> fp16 precision schedule (16-bit only)
 int32_t sign_simt(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, const int64_t *col_off,
                   int64_t packed_elems, int32_t x_dtype, void *X, void *ws, int64_t ws_bytes,
-                  int32_t max_iter, double tol, int32_t *iters, double *residual, int32_t nonsym, cudaStream_t st);
+                  int32_t max_iter, double tol, int32_t *iters, double *residual, int32_t nonsym, int32_t order, cudaStream_t st);
 int32_t sign_umma(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, const int64_t *col_off,
                   int64_t packed_elems, int32_t x_dtype, void *X, void *ws, int64_t ws_bytes,
-                  int32_t max_iter, double tol, int32_t *iters, double *residual, int32_t nonsym, int32_t switch_iter,
+                  int32_t max_iter, double tol, int32_t *iters, double *residual, int32_t nonsym, int32_t switch_iter, int32_t order,
                   cudaStream_t st);
 int64_t sign_simt_ws_bytes(const sm_pattern_t *P, int32_t n_cols, int64_t packed_elems, int32_t x_dtype);
 int32_t dense_product(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, const int64_t *col_off, int32_t x_dtype,
                       const void *A, const void *B, void *O, int32_t *active, int32_t *last_zero, cudaStream_t st);   // sign_simt.cu
-int64_t sign_umma_ws_bytes(const sm_pattern_t *P, int32_t n_cols, int64_t packed_elems, int32_t x_dtype, int32_t nonsym);
+int64_t sign_umma_ws_bytes(const sm_pattern_t *P, int32_t n_cols, int64_t packed_elems, int32_t x_dtype, int32_t nonsym,
+                           int32_t order);
 int32_t *device_err_word();        // pinned, device-mapped host word the kernels write a protocol-failure code to (api.cu)
 
 // ---- variant selection (api.cu): sm_set_option / environment at first use.  Ids are indices into the table there.

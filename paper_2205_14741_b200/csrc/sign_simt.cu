@@ -9,7 +9,8 @@ constexpr int ST = 64;    // output tile edge
 constexpr int SK = 16;    // k step
 constexpr int SPAD = 4;
 
-// PHASE 1: Y = X X, partial ||Y - I||_F^2.   PHASE 2: X' = 1.5 X - 0.5 X Y.   PHASE 3: O = X Y (plain product, f2).
+// PHASE 1: Y = X X, partial ||Y - I||_F^2.   PHASE 2: X' = 1.5 X - 0.5 X Y.   PHASE 3: O = X Y (plain product, f2; the
+// third product X' = X Z of the order-3 iteration).   PHASE 4 (order 3, reading A22; Xsrc = Y): Z = (15 I - 10 Y + 3 Y Y) / 8.
 template <typename T, int PHASE>
 __global__ void __launch_bounds__(256)
 k_simt_gemm(const int32_t *__restrict__ cols, const int64_t *__restrict__ col_off,
@@ -25,7 +26,7 @@ k_simt_gemm(const int32_t *__restrict__ cols, const int64_t *__restrict__ col_of
   const int32_t tr = t / max_tiles_edge, tc = t - tr * max_tiles_edge;
   if (tr >= te || tc >= te) return;
   const T *A = Xsrc + col_off[c];
-  const T *B = (PHASE == 1 ? Xsrc : Ybuf) + col_off[c];
+  const T *B = ((PHASE == 1 || PHASE == 4) ? Xsrc : Ybuf) + col_off[c];
   T *O = Out + col_off[c];
 
   __shared__ T As[SK][ST + SPAD];
@@ -99,6 +100,8 @@ k_simt_gemm(const int32_t *__restrict__ cols, const int64_t *__restrict__ col_of
       if (gr < m && gc < m) {
         if (PHASE == 3) {
           O[(int64_t)gr * Pd + gc] = acc[q][p];
+        } else if (PHASE == 4) {
+          O[(int64_t)gr * Pd + gc] = (T)0.375 * acc[q][p] - (T)1.25 * A[(int64_t)gr * Pd + gc] + (gr == gc ? (T)1.875 : (T)0);
         } else if (PHASE == 1) {
           O[(int64_t)gr * Pd + gc] = acc[q][p];
           double d = (double)acc[q][p] - (gr == gc ? 1.0 : 0.0);
@@ -171,7 +174,7 @@ k_dmma_gemm(const int32_t *__restrict__ cols, const int64_t *__restrict__ col_of
   const int32_t tr = t / max_tiles_edge, tc = t - tr * max_tiles_edge;
   if (tr >= te || tc >= te || (SYM && tc > tr)) return;       // SYM: lower-triangle tiles only
   const double *A = Xsrc + col_off[c];
-  const double *B = (PHASE == 1 ? Xsrc : Ybuf) + col_off[c];
+  const double *B = ((PHASE == 1 || PHASE == 4) ? Xsrc : Ybuf) + col_off[c];
   double *O = Out + col_off[c];
   const int32_t row0 = tr * TILE, col0 = tc * TILE;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -253,6 +256,8 @@ k_dmma_gemm(const int32_t *__restrict__ cols, const int64_t *__restrict__ col_of
             res += ((!SYM || gr == gc) ? 1.0 : 2.0) * d * d;
           } else if (PHASE == 2) {
             val = 1.5 * A[(int64_t)gr * Pd + gc] - 0.5 * val;
+          } else if (PHASE == 4) {
+            val = 0.375 * val - 1.25 * A[(int64_t)gr * Pd + gc] + (gr == gc ? 1.875 : 0.0);
           }
           O[(int64_t)gr * Pd + gc] = val;
           if (SYM && gc < gr) O[(int64_t)gc * Pd + gr] = val;
@@ -299,7 +304,7 @@ k_ffma_sym(const int32_t *__restrict__ cols, const int64_t *__restrict__ col_off
   const int32_t tr = t / max_tiles_edge, tc = t - tr * max_tiles_edge;
   if (tr >= te || tc > tr) return;                              // lower-triangle tiles only
   const float *A = Xsrc + col_off[c];
-  const float *B = (PHASE == 1 ? Xsrc : Ybuf) + col_off[c];
+  const float *B = ((PHASE == 1 || PHASE == 4) ? Xsrc : Ybuf) + col_off[c];
   float *O = Out + col_off[c];
   const int32_t row0 = tr * FT, col0 = tc * FT;
   __shared__ __align__(16) float As[2][FK][FT];
@@ -364,8 +369,10 @@ k_ffma_sym(const int32_t *__restrict__ cols, const int64_t *__restrict__ col_off
         if (PHASE == 1) {
           const double d = (double)val - (gr == gc ? 1.0 : 0.0);
           res += (gr == gc ? 1.0 : 2.0) * d * d;
-        } else {
+        } else if (PHASE == 2) {
           val = 1.5f * A[(int64_t)gr * Pd + gc] - 0.5f * val;
+        } else if (PHASE == 4) {
+          val = 0.375f * val - 1.25f * A[(int64_t)gr * Pd + gc] + (gr == gc ? 1.875f : 0.f);
         }
         O[(int64_t)gr * Pd + gc] = val;
         if (gc < gr) O[(int64_t)gc * Pd + gr] = val;
@@ -415,11 +422,56 @@ int64_t sign_simt_ws_bytes(const sm_pattern_t *P, int32_t n_cols, int64_t packed
   return simt_layout(nullptr, 0, P, n_cols, packed_elems, dtype_bytes(x_dtype)).used;
 }
 
+// Which product kernel a call uses (one choice per call, every phase).
+enum SimtMode { M_GENERIC = 0, M_DMMA_FULL, M_DMMA_SYM64, M_DMMA_SYM128, M_FFMA_SYM };
+
+template <int PHASE>
+static int32_t dmma_attrs() {
+  // per device attribute: set on every call (a process may use several devices)
+  SM_CUDA(cudaFuncSetAttribute(k_dmma_gemm<PHASE, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, DMMA_SMEM));
+  SM_CUDA(cudaFuncSetAttribute(k_dmma_gemm<PHASE, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, DMMA_SMEM));
+  SM_CUDA(cudaFuncSetAttribute(k_dmma_gemm<PHASE, true, 64>, cudaFuncAttributeMaxDynamicSharedMemorySize, DCfg<64>::SMEM));
+  return SM_OK;
+}
+
+template <typename T, int PHASE>
+static int32_t launch_simt(int mode, int32_t grid, int32_t edge, const sm_pattern_t *P, const int32_t *cols,
+                           const int64_t *col_off, const T *A, const T *B, T *O, SignState s, cudaStream_t st) {
+  int slot = -1;
+  { int32_t rc = prof_begin(st, &slot); if (rc != SM_OK) return rc; }
+  bool done = false;
+  if constexpr (sizeof(T) == 8) {
+    if (mode == M_DMMA_FULL) {
+      k_dmma_gemm<PHASE, false><<<grid, 256, DMMA_SMEM, st>>>(cols, col_off, P->dim, P->dim_pad, edge, A, B, O, s);
+      done = true;
+    } else if (mode == M_DMMA_SYM64) {
+      k_dmma_gemm<PHASE, true, 64><<<grid, 256, DCfg<64>::SMEM, st>>>(cols, col_off, P->dim, P->dim_pad, edge, A, B, O, s);
+      done = true;
+    } else if (mode == M_DMMA_SYM128) {
+      k_dmma_gemm<PHASE, true><<<grid, 256, DMMA_SMEM, st>>>(cols, col_off, P->dim, P->dim_pad, edge, A, B, O, s);
+      done = true;
+    }
+  } else {
+    if (mode == M_FFMA_SYM) {
+      k_ffma_sym<PHASE><<<grid, 64, 0, st>>>(cols, col_off, P->dim, P->dim_pad, edge, A, B, O, s);
+      done = true;
+    }
+  }
+  if (!done) k_simt_gemm<T, PHASE><<<grid, 256, 0, st>>>(cols, col_off, P->dim, P->dim_pad, edge, A, B, O, s);
+  SM_LAUNCHED();
+  return prof_end(st, slot);
+}
+
+// order 2: Newton-Schulz, two products per step (Y = X X; X' = 1.5 X - 0.5 X Y), X alternates between X and ws.X2.
+// order 3 (f3, reading A22; symmetric iterates only): three products per step on the same three buffers --
+//   Y = X X -> the buffer X' will be written to;  Z = (15 I - 10 Y + 3 Y Y) / 8 -> ws.X2;  X' = X Z over the dead Y;
+// X alternates between X and ws.Y.
 template <typename T>
 static int32_t sign_simt_t(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, const int64_t *col_off,
                            int64_t packed_elems, T *X, void *ws, int64_t ws_bytes, int32_t max_iter,
-                           double tol, int32_t *iters, double *residual, int32_t nonsym, cudaStream_t st) {
+                           double tol, int32_t *iters, double *residual, int32_t nonsym, int32_t order, cudaStream_t st) {
   if ((P->pad_to & 3) != 0) return SM_ERR_ARG;   // 16-byte alignment of every submatrix
+  if (order == 3 && nonsym) return SM_ERR_UNSUPPORTED;
   SimtWs w = simt_layout(ws, ws_bytes, P, n_cols, packed_elems, (int32_t)sizeof(T));
   if (w.used > ws_bytes) return SM_ERR_SPACE;
   SignState s{w.active, w.last, w.n_still, w.partial, w.parts_per_col};
@@ -429,6 +481,7 @@ static int32_t sign_simt_t(const sm_pattern_t *P, const int32_t *cols, int32_t n
   const bool fsym = sizeof(T) == 4 && !nonsym && opt(OPT_F32_SYM) != 0 && (P->pad_to & 3) == 0;
   // fp64 tiles: 64 x 64 where 128-row tiles would mostly multiply padding (option "f64.tile": 0 = by size, 64, 128)
   const int32_t dt = !dmma ? ST : (!nonsym && (opt(OPT_F64_TILE) == 64 || (opt(OPT_F64_TILE) == 0 && P->max_dim <= 384))) ? 64 : DT;
+  const int mode = dmma ? (nonsym ? M_DMMA_FULL : dt == 64 ? M_DMMA_SYM64 : M_DMMA_SYM128) : fsym ? M_FFMA_SYM : M_GENERIC;
   const int32_t TS = dt;
   const int32_t edge = (P->max_dim + TS - 1) / TS;
   const int64_t grid64 = (int64_t)n_cols * edge * edge;
@@ -438,66 +491,37 @@ static int32_t sign_simt_t(const sm_pattern_t *P, const int32_t *cols, int32_t n
   SM_LAUNCHED();
   k_tile_nparts<<<nb, 256, 0, st>>>(n_cols, TS, cols, P->dim, w.n_parts);
   SM_LAUNCHED();
-  if (fsym) {
-    // padding of Y / the alternate X buffer must read as zeros; slots of the skipped upper tiles too
-    SM_CUDA(cudaMemsetAsync(w.Y, 0, packed_elems * sizeof(T), st));
-    SM_CUDA(cudaMemsetAsync(w.X2, 0, packed_elems * sizeof(T), st));
-    SM_CUDA(cudaMemsetAsync(w.partial, 0, (size_t)n_cols * w.parts_per_col * sizeof(double), st));
-  }
   if (dmma) {
-    // per device attribute: set on every call (a process may use several devices)
-    SM_CUDA(cudaFuncSetAttribute(k_dmma_gemm<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, DMMA_SMEM));
-    SM_CUDA(cudaFuncSetAttribute(k_dmma_gemm<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, DMMA_SMEM));
-    SM_CUDA(cudaFuncSetAttribute(k_dmma_gemm<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, DMMA_SMEM));
-    SM_CUDA(cudaFuncSetAttribute(k_dmma_gemm<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, DMMA_SMEM));
-    SM_CUDA(cudaFuncSetAttribute(k_dmma_gemm<1, true, 64>, cudaFuncAttributeMaxDynamicSharedMemorySize, DCfg<64>::SMEM));
-    SM_CUDA(cudaFuncSetAttribute(k_dmma_gemm<2, true, 64>, cudaFuncAttributeMaxDynamicSharedMemorySize, DCfg<64>::SMEM));
-    // padding of Y and of the alternate X buffer must read as zeros (the kernel stores true elements only)
+    int32_t rc = dmma_attrs<1>();
+    if (rc == SM_OK) rc = dmma_attrs<2>();
+    if (rc == SM_OK && order == 3) rc = dmma_attrs<3>();
+    if (rc == SM_OK && order == 3) rc = dmma_attrs<4>();
+    if (rc != SM_OK) return rc;
+  }
+  {
+    // padding of the two scratch buffers must read as zeros (the kernels store true elements only; whole padded
+    // images are copied back), and so must the partial-sum slots of the skipped upper-triangle tiles, never written
     SM_CUDA(cudaMemsetAsync(w.Y, 0, packed_elems * sizeof(T), st));
     SM_CUDA(cudaMemsetAsync(w.X2, 0, packed_elems * sizeof(T), st));
-    // partial-sum slots of the skipped upper-triangle tiles are never written: they must read as zero
     SM_CUDA(cudaMemsetAsync(w.partial, 0, (size_t)n_cols * w.parts_per_col * sizeof(double), st));
   }
-  T *buf[2] = {X, (T *)w.X2};
-  T *Y = (T *)w.Y;
+  T *buf[2] = {X, order == 3 ? (T *)w.Y : (T *)w.X2};
   for (int32_t k = 0; k < max_iter; ++k) {
     T *src = buf[k & 1], *dst = buf[(k + 1) & 1];
-    int slot = -1;
-    { int32_t rc = prof_begin(st, &slot); if (rc != SM_OK) return rc; }
-    if (dmma && nonsym)
-      k_dmma_gemm<1, false><<<grid, 256, DMMA_SMEM, st>>>(cols, col_off, P->dim, P->dim_pad, edge, (const double *)src,
-                                                          (const double *)Y, (double *)Y, s);
-    else if (dmma && dt == 64)
-      k_dmma_gemm<1, true, 64><<<grid, 256, DCfg<64>::SMEM, st>>>(cols, col_off, P->dim, P->dim_pad, edge, (const double *)src,
-                                                                 (const double *)Y, (double *)Y, s);
-    else if (dmma)
-      k_dmma_gemm<1, true><<<grid, 256, DMMA_SMEM, st>>>(cols, col_off, P->dim, P->dim_pad, edge, (const double *)src,
-                                                         (const double *)Y, (double *)Y, s);
-    else if (fsym)
-      k_ffma_sym<1><<<grid, 64, 0, st>>>(cols, col_off, P->dim, P->dim_pad, edge, (const float *)src, (const float *)Y, (float *)Y, s);
-    else
-      k_simt_gemm<T, 1><<<grid, 256, 0, st>>>(cols, col_off, P->dim, P->dim_pad, edge, src, Y, Y, s);
-    SM_LAUNCHED();
-    { int32_t rc = prof_end(st, slot); if (rc != SM_OK) return rc; }
+    T *Y = order == 3 ? dst : (T *)w.Y;
+    int32_t rc = launch_simt<T, 1>(mode, grid, edge, P, cols, col_off, src, Y, Y, s, st);
+    if (rc != SM_OK) return rc;
     SM_CUDA(cudaMemsetAsync(w.n_still, 0, sizeof(int32_t), st));
     k_sign_post<<<(n_cols + 7) / 8, 256, 0, st>>>(n_cols, cols, P->dim, s, w.n_parts, tol, iters, residual);
     SM_LAUNCHED();
-    { int32_t rc = prof_begin(st, &slot); if (rc != SM_OK) return rc; }
-    if (dmma && nonsym)
-      k_dmma_gemm<2, false><<<grid, 256, DMMA_SMEM, st>>>(cols, col_off, P->dim, P->dim_pad, edge, (const double *)src,
-                                                          (const double *)Y, (double *)dst, s);
-    else if (dmma && dt == 64)
-      k_dmma_gemm<2, true, 64><<<grid, 256, DCfg<64>::SMEM, st>>>(cols, col_off, P->dim, P->dim_pad, edge, (const double *)src,
-                                                                 (const double *)Y, (double *)dst, s);
-    else if (dmma)
-      k_dmma_gemm<2, true><<<grid, 256, DMMA_SMEM, st>>>(cols, col_off, P->dim, P->dim_pad, edge, (const double *)src,
-                                                         (const double *)Y, (double *)dst, s);
-    else if (fsym)
-      k_ffma_sym<2><<<grid, 64, 0, st>>>(cols, col_off, P->dim, P->dim_pad, edge, (const float *)src, (const float *)Y, (float *)dst, s);
-    else
-      k_simt_gemm<T, 2><<<grid, 256, 0, st>>>(cols, col_off, P->dim, P->dim_pad, edge, src, Y, dst, s);
-    SM_LAUNCHED();
-    { int32_t rc = prof_end(st, slot); if (rc != SM_OK) return rc; }
+    if (order == 3) {
+      T *Z = (T *)w.X2;
+      rc = launch_simt<T, 4>(mode, grid, edge, P, cols, col_off, Y, Y, Z, s, st);
+      if (rc == SM_OK) rc = launch_simt<T, 3>(mode, grid, edge, P, cols, col_off, src, Z, dst, s, st);
+    } else {
+      rc = launch_simt<T, 2>(mode, grid, edge, P, cols, col_off, src, Y, dst, s, st);
+    }
+    if (rc != SM_OK) return rc;
     if (tol > 0.0 && k >= 5 && (k & 1)) {
       // convergence mode: read back how many submatrices continue (the only host sync of the path)
       int32_t still = 1;
@@ -507,7 +531,7 @@ static int32_t sign_simt_t(const sm_pattern_t *P, const int32_t *cols, int32_t n
     }
   }
   dim3 cg(n_cols, 8);
-  k_copy_back<<<cg, 256, 0, st>>>(cols, col_off, iters, (int32_t)sizeof(T), P->dim_pad, 0, (const char *)w.X2, (char *)X);
+  k_copy_back<<<cg, 256, 0, st>>>(cols, col_off, iters, (int32_t)sizeof(T), P->dim_pad, 0, (const char *)buf[1], (char *)X);
   SM_LAUNCHED();
   return SM_OK;
 }
@@ -540,13 +564,14 @@ int32_t dense_product(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols
 
 int32_t sign_simt(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, const int64_t *col_off,
                   int64_t packed_elems, int32_t x_dtype, void *X, void *ws, int64_t ws_bytes,
-                  int32_t max_iter, double tol, int32_t *iters, double *residual, int32_t nonsym, cudaStream_t st) {
+                  int32_t max_iter, double tol, int32_t *iters, double *residual, int32_t nonsym, int32_t order,
+                  cudaStream_t st) {
   if (x_dtype == SM_F64)
     return sign_simt_t<double>(P, cols, n_cols, col_off, packed_elems, (double *)X, ws, ws_bytes, max_iter,
-                               tol, iters, residual, nonsym, st);
+                               tol, iters, residual, nonsym, order, st);
   if (x_dtype == SM_F32)
     return sign_simt_t<float>(P, cols, n_cols, col_off, packed_elems, (float *)X, ws, ws_bytes, max_iter,
-                              tol, iters, residual, nonsym, st);
+                              tol, iters, residual, nonsym, order, st);
   return SM_ERR_UNSUPPORTED;
 }
 

@@ -114,6 +114,9 @@ struct UArgs {
   // submatrix writes the full image (lt_out = 0, or s.last in convergence mode): sm_scatter reads whole rows.
   int32_t lt_in, lt_out;
   int32_t out_f16;           // precision schedule (f3): this launch reads bf16 operands and rounds its output to fp16
+  // third-order iteration (f3, reading A22): product 1 stores Q = w_scale (Y - I) (-1/2: Newton-Schulz; -3/4: order 3),
+  // the update-type product scales its accumulator by out_scale (1; 2/3 for Z = 2/3 (Q + Q Q))
+  float w_scale, out_scale;
 };
 
 // Tile geometry.  Only elements (r, c) with c <= r are computed, so tile row tm (rows tm*R ..
@@ -772,7 +775,9 @@ k_umma_gemm(UArgs a, const __grid_constant__ CUtensorMap mapA, const __grid_cons
                   } else {
                     acc = fmaf(f0, f0, acc); acc = fmaf(f1, f1, acc);
                   }
-                  f0 *= -0.5f; f1 *= -0.5f;                 // Wh = -1/2 W is what PHASE 2 multiplies by
+                  f0 *= a.w_scale; f1 *= a.w_scale;         // Wh = -1/2 W is what PHASE 2 multiplies by
+                } else if (a.out_scale != 1.f) {
+                  f0 *= a.out_scale; f1 *= a.out_scale;
                 }
                 o[ti][tj] = (BF16 && !a.out_f16) ? pack2<true>(f0, f1) : pack2<false>(f0, f1);
               }
@@ -937,7 +942,10 @@ k_umma_gemm(UArgs a, const __grid_constant__ CUtensorMap mapA, const __grid_cons
                 for (int e = 0; e < 8; ++e) acc = fmaf(f[e], f[e], acc);
               }
 #pragma unroll
-              for (int e = 0; e < 8; ++e) f[e] *= -0.5f;           // Wh = -1/2 W is what PHASE 2 multiplies by
+              for (int e = 0; e < 8; ++e) f[e] *= a.w_scale;       // Wh = -1/2 W is what PHASE 2 multiplies by
+            } else if (a.out_scale != 1.f) {
+#pragma unroll
+              for (int e = 0; e < 8; ++e) f[e] *= a.out_scale;
             }
 #pragma unroll
             for (int e2 = 0; e2 < 4; ++e2)
@@ -1107,7 +1115,7 @@ static int32_t umma_sym_mode(int32_t nonsym, bool fused, int32_t ncta, double to
 static int32_t umma_resident_pd(int32_t sym) { return (sym && opt(OPT_UMMA_RESIDENT) != 0) ? RES_MAX_PD : 0; }
 
 static UmmaWs umma_layout(void *ws, int64_t ws_bytes, const sm_pattern_t *P, int32_t n_cols,
-                          int64_t packed_elems, int32_t sym) {
+                          int64_t packed_elems, int32_t sym, bool o3) {
   WsCursor cur(ws, ws_bytes);
   UmmaWs w;
   // sized for whichever variant sign_umma picks (the query does not know tol): per-phase launches with
@@ -1117,8 +1125,9 @@ static UmmaWs umma_layout(void *ws, int64_t ws_bytes, const sm_pattern_t *P, int
   const int32_t t_fused = u_tiles(P->max_dim, UM * 2);
   const int32_t max_tiles = t_sel > t_fused ? t_sel : t_fused;
   w.parts_per_col = (t_sel * ncta > t_fused * 2 ? t_sel * ncta : t_fused * 2) * EPI_WARPS;
-  // when every listed column can be resident the grouped path's two image buffers are not needed
-  const bool all_res = umma_resident_pd(sym) >= P->max_dim_pad;
+  // when every listed column can be resident the grouped path's two image buffers are not needed (the third-order
+  // iteration has no resident kernel)
+  const bool all_res = !o3 && umma_resident_pd(sym) >= P->max_dim_pad;
   w.Y = cur.take<char>(all_res ? 0 : packed_elems * 2);
   w.X2 = cur.take<char>(all_res ? 0 : packed_elems * 2);
   w.active = cur.take<int32_t>(n_cols);
@@ -1136,11 +1145,11 @@ static UmmaWs umma_layout(void *ws, int64_t ws_bytes, const sm_pattern_t *P, int
 }
 
 int64_t sign_umma_ws_bytes(const sm_pattern_t *P, int32_t n_cols, int64_t packed_elems, int32_t x_dtype,
-                           int32_t nonsym) {
+                           int32_t nonsym, int32_t order) {
   (void)x_dtype;
   // sized for the larger of the tile tables the call may pick (the query does not know tol / max_iter)
-  const int64_t a = umma_layout(nullptr, 0, P, n_cols, packed_elems, umma_sym_mode(nonsym, false, umma_ncta(), 0.0, 1)).used;
-  const int64_t b = umma_layout(nullptr, 0, P, n_cols, packed_elems, umma_sym_mode(nonsym, false, umma_ncta(), 1.0, 1)).used;
+  const int64_t a = umma_layout(nullptr, 0, P, n_cols, packed_elems, umma_sym_mode(nonsym, false, umma_ncta(), 0.0, 1), order == 3).used;
+  const int64_t b = umma_layout(nullptr, 0, P, n_cols, packed_elems, umma_sym_mode(nonsym, false, umma_ncta(), 1.0, 1), order == 3).used;
   return a > b ? a : b;
 }
 
@@ -1256,17 +1265,20 @@ static int32_t launch_resident(bool bf16, const RArgs &a, int32_t n_sm, cudaStre
 int32_t sign_umma(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, const int64_t *col_off,
                   int64_t packed_elems, int32_t x_dtype, void *X, void *ws, int64_t ws_bytes,
                   int32_t max_iter, double tol, int32_t *iters, double *residual, int32_t nonsym, int32_t switch_iter,
-                  cudaStream_t st) {
+                  int32_t order, cudaStream_t st) {
   if ((P->pad_to % 64) != 0) return SM_ERR_ARG;
   const bool bf16 = x_dtype == SM_BF16;
+  // third-order iteration (f3, reading A22): three grouped products per step (no resident / stream / fused variant)
+  const bool o3 = order == 3;
+  if (o3 && nonsym) return SM_ERR_UNSUPPORTED;
   if (switch_iter >= 0) {
     // mixed schedule (f3): bf16 in, fp16 out; fixed iteration counts, symmetric iterates
     if (!bf16 || nonsym || tol > 0.0 || switch_iter < 1 || switch_iter >= max_iter) return SM_ERR_ARG;
   }
-  const bool fused = !nonsym && switch_iter < 0 && umma_fused(tol);
+  const bool fused = !nonsym && !o3 && switch_iter < 0 && umma_fused(tol);
   const int32_t ncta = fused ? 2 : umma_ncta(), R = UM * ncta;
   const int32_t sym = umma_sym_mode(nonsym, fused, ncta, tol, max_iter);
-  UmmaWs w = umma_layout(ws, ws_bytes, P, n_cols, packed_elems, sym);
+  UmmaWs w = umma_layout(ws, ws_bytes, P, n_cols, packed_elems, sym, order == 3);
   if (w.used > ws_bytes) return SM_ERR_SPACE;
   int dev = 0, n_sm = 0;
   SM_CUDA(cudaGetDevice(&dev));
@@ -1277,7 +1289,7 @@ int32_t sign_umma(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, co
   const int32_t nb = (n_cols + 255) / 256;
 
   // ---- small submatrices: all steps inside one CTA (k_umma_resident)
-  const int32_t res_pd = fused ? 0 : umma_resident_pd(sym);
+  const int32_t res_pd = (fused || o3) ? 0 : umma_resident_pd(sym);
   if (res_pd > 0) {
     SM_CUDA(cudaMemsetAsync(w.counters + UMMA_MAX_COUNTERS, 0, sizeof(unsigned long long), st));
     RArgs r{cols, col_off, P->dim, P->dim_pad, n_cols, max_iter, tol, X, iters, residual,
@@ -1346,16 +1358,17 @@ int32_t sign_umma(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, co
   }
 #endif
   const int32_t nst_opt = opt(OPT_UMMA_STAGES);
-  const bool dyn = opt(OPT_UMMA_DYN) != 0 && mode == 1 && sym && 2 * max_iter <= UMMA_MAX_COUNTERS;
+  const int32_t nper = o3 ? 3 : 2;           // products (launches, tile counters) per step
+  const bool dyn = opt(OPT_UMMA_DYN) != 0 && mode == 1 && sym && nper * max_iter <= UMMA_MAX_COUNTERS;
   // ring depth: with the static deal large submatrices want the shallow ring (see UCfg); the dynamic deal removes
   // the drift that made the deep ring costly (configs[4], 25 steps: 603 ms with 4 stages, 615 ms with 3)
   const int32_t nst = nst_opt ? nst_opt : (mode == 4 ? 6 : ((!dyn && P->max_dim > 1024) ? 3 : 4));
   if (dyn) SM_CUDA(cudaMemsetAsync(w.counters, 0, sizeof(unsigned long long) * UMMA_MAX_COUNTERS, st));
-  if (opt(OPT_UMMA_STREAM) == 1 && dyn && !(tol > 0.0) && max_iter > 0 && switch_iter < 0) {
+  if (opt(OPT_UMMA_STREAM) == 1 && dyn && !o3 && !(tol > 0.0) && max_iter > 0 && switch_iter < 0) {
     const int64_t n_done = (int64_t)(n_cols / STREAM_G + 1) * 2 * max_iter;
     SM_CUDA(cudaMemsetAsync(w.done, 0, sizeof(int32_t) * n_done, st));
     UArgs a{cols, col_off, P->dim, P->dim_pad, w.tile_ptr, w.tiles, n_cols, 0, X, w.Y, w.X2, s, w.err, 0, w.counters,
-            2 * max_iter, w.done, umma_dbg(), 0, 0, 0};
+            2 * max_iter, w.done, umma_dbg(), 0, 0, 0, -0.5f, 1.f};
     int32_t rc = sym == 2 ? launch_umma_t<0, 1, true, false, 0, false, true, 1>(bf16, a, maps[0], n_sm, st)
                           : launch_umma_t<0, 1, true, false, 0, false, true>(bf16, a, maps[0], n_sm, st);
     if (rc != SM_OK) return rc;
@@ -1368,17 +1381,26 @@ int32_t sign_umma(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, co
     return SM_OK;
   }
   const int32_t rev_on = opt(OPT_UMMA_REV) != 0 ? 1 : 0;
-  void *buf[2] = {X, w.X2};
+#ifdef SM_MEASURE
+  if (o3 && mode != 1) return SM_ERR_UNSUPPORTED;
+#endif
+  // Newton-Schulz: X alternates between X and ws.X2, Wh lives in ws.Y.  Order 3: X alternates between X and ws.Y,
+  // Q = 3/4 (I - X X) is written where X' will go (it is dead after the second product), Z = 2/3 (Q + Q Q) lives in
+  // ws.X2, X' = X + X Z.  The second product IS the update product with X := Q, Wh := Q (the identity MMAs add Q).
+  void *buf[2] = {X, o3 ? w.Y : w.X2};
   for (int32_t k = 0; k < max_iter; ++k) {
     void *src = buf[k & 1], *dst = buf[(k + 1) & 1];
-    UArgs a{cols, col_off, P->dim, P->dim_pad, w.tile_ptr, w.tiles, n_cols, tol > 0.0 ? 1 : 0, src, w.Y, w.Y, s, w.err, 0, nullptr, 0, nullptr, umma_dbg(), 0, 0, 0};
+    void *Wb = o3 ? dst : w.Y;
+    UArgs a{cols, col_off, P->dim, P->dim_pad, w.tile_ptr, w.tiles, n_cols, tol > 0.0 ? 1 : 0, src, Wb, Wb, s, w.err, 0, nullptr, 0, nullptr, umma_dbg(), 0, 0, 0,
+            o3 ? -0.75f : -0.5f, 1.f};
     // "128-lower" storage (staged epilogue only): Wh is always written and read that way; X is read that way from the
     // second step on (X0 from sm_gather is a full image, a superset) and written that way except by the last update
     // of a submatrix (fixed counts: the last step; convergence mode: per submatrix, s.last)
-    const int32_t lt = (sym == 2 && opt(OPT_UMMA_LT) != 0) ? 1 : 0;
+    const int32_t lt = (sym == 2 && !o3 && opt(OPT_UMMA_LT) != 0) ? 1 : 0;
     a.lt_in = lt && k > 0; a.lt_out = lt;
-    a.rev = 0;
-    a.counter = dyn ? w.counters + 2 * k : nullptr;
+    int32_t launch = nper * k;                 // launches alternate their walk through the tile table (option umma.rev)
+    a.rev = o3 ? (rev_on & launch) & 1 : 0;
+    a.counter = dyn ? w.counters + launch : nullptr;
     const UMaps m1{maps[k & 1].a, maps[k & 1].b}, m2{maps[k & 1].a, maps[2].b};
     // precision schedule (f3): updates 0 .. switch_iter-1 run on bf16 operands, update switch_iter-1 rounds X' to fp16
     const bool bf16_k = bf16 && (switch_iter < 0 || k < switch_iter);
@@ -1394,11 +1416,22 @@ int32_t sign_umma(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, co
                                                      max_iter, iters, residual);
       SM_LAUNCHED();
     }
+    if (o3) {
+      ++launch;
+      UArgs z = a;
+      z.Xsrc = Wb; z.Ybuf = Wb; z.Out = w.X2; z.out_scale = 2.f / 3.f;
+      z.rev = (rev_on & launch) & 1;
+      z.counter = dyn ? w.counters + launch : nullptr;
+      rc = launch_umma_any<2>(bf16_k, mode, sym, nst, z, m2, n_sm, st);
+      if (rc != SM_OK) return rc;
+      a.Ybuf = w.X2;
+    }
+    ++launch;
     a.Out = dst;
     a.lt_in = lt;              // PHASE 2 reads X (lower from step 1 on; X0 is full, which is a superset) and Wh (lower)
     a.lt_out = lt && k + 1 < max_iter;     // (convergence mode: an earlier last update is mirrored per submatrix, s.last)
-    a.rev = rev_on;            // PHASE 2 starts where PHASE 1 ended, the next PHASE 1 where this launch ends
-    a.counter = dyn ? w.counters + 2 * k + 1 : nullptr;
+    a.rev = o3 ? (rev_on & launch) & 1 : rev_on;   // PHASE 2 starts where PHASE 1 ended, the next PHASE 1 where this launch ends
+    a.counter = dyn ? w.counters + launch : nullptr;
     a.out_f16 = (bf16_k && k + 1 == switch_iter) ? 1 : 0;
     rc = launch_umma_any<2>(bf16_k, mode, sym, nst, a, m2, n_sm, st);
     if (rc != SM_OK) return rc;
@@ -1410,7 +1443,7 @@ int32_t sign_umma(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, co
     }
   }
   dim3 cg(n_cols, 8);
-  k_copy_back<<<cg, 256, 0, st>>>(cols, col_off, iters, 2, P->dim_pad, res_pd, (const char *)w.X2, (char *)X);
+  k_copy_back<<<cg, 256, 0, st>>>(cols, col_off, iters, 2, P->dim_pad, res_pd, (const char *)buf[1], (char *)X);
   SM_LAUNCHED();
   return SM_OK;
 }

@@ -775,3 +775,93 @@ def test_submatrix_dimension_sweep_across_tile_boundaries(sm, x_dtype, pad, tol_
         err = np.abs(blk - ref).max()
         assert err <= tol_abs, (m, err)
         assert np.array_equal(blk, blk.T), (m, "iterate must be exactly symmetric")
+
+
+# ------------------------------------------------------------------- third-order iteration (f3, reading A22)
+
+def _density_o3(sm, wl, x_dtype, max_iter, tol, pad=None, switch_iter=-1, max_chunk_elems=None):
+    A = sm.Bcsr(wl)
+    P = sm.sm_build_pattern(A, pad or (64 if x_dtype in ("bf16", "f16") else 16))
+    plan = sm.DensityPlan(A, P, x_dtype, max_chunk_elems=max_chunk_elems, order=3)
+    sm.sm_density(A, P, plan, 0.0, "gershgorin", max_iter, tol, switch_iter=switch_iter, order=3)
+    torch.cuda.synchronize()
+    return A, P, plan
+
+
+@pytest.mark.parametrize("x_dtype,k,tol_abs", [("f64", 3, 1e-12), ("f64", 4, 1e-12), ("f32", 3, 1e-5), ("f32", 4, 1e-5),
+                                                ("f16", 3, 2e-3), ("f16", 4, 2e-3), ("bf16", 3, 1.5e-2), ("bf16", 4, 1.5e-2)])
+def test_order3_fixed_count_matches_the_ns3k_polynomial(sm, x_dtype, k, tol_abs):
+    """k steps of X <- X (15 I - 10 X^2 + 3 X^4) / 8 (odd and even k: both result buffers) against the oracle's
+    polynomial on the spectrum, all columns of configs[0]; the 2nd-order polynomial of the same k must NOT match."""
+    wl = make_config(0)
+    d3, _ = orc.density_columns(wl, mode="ns3k", k_fixed=k, n_threads=THREADS)
+    d2, _ = orc.density_columns(wl, mode="nsk", k_fixed=k, n_threads=THREADS)
+    _, _, plan = _density_o3(sm, wl, x_dtype, k, 0.0)
+    assert (plan.iters == k).all()
+    D = plan.D.cpu().numpy().astype(np.float64)
+    assert np.abs(D - d3).max() <= tol_abs
+    assert np.abs(D - d2).max() > 0.05
+
+
+@pytest.mark.parametrize("x_dtype,tol_abs", [("bf16", 1.5e-2), ("f16", 2e-3), ("f64", 1e-12), ("f32", 1e-5)])
+def test_order3_dimension_sweep(sm, x_dtype, tol_abs):
+    """The tile-boundary sweep (every kernel's tile / chunk / panel edges) for the three-product step."""
+    k = 3
+    ms = np.array(SWEEP_M, dtype=np.int32)
+    wl = make_workload(len(ms), ms, np.maximum(1, ms // 3), 0.0, seed=91)
+    small = [i for i, m in enumerate(SWEEP_M) if m <= 257]
+    large = [i for i, m in enumerate(SWEEP_M) if m > 257]
+    d_ref = orc.density_columns(wl, cols=small, mode="ns3k", k_fixed=k, n_threads=THREADS)[0] + \
+        orc.density_columns_lapack(wl, cols=large, mode="ns3k", k_fixed=k)[0]
+    _, _, plan = _density_o3(sm, wl, x_dtype, k, 0.0)
+    d = plan.D.cpu().numpy().astype(np.float64)
+    vp = np.asarray(wl.val_ptr, dtype=np.int64)
+    for i, m in enumerate(SWEEP_M):
+        blk = d[vp[i]:vp[i + 1]].reshape(m, m)
+        err = np.abs(blk - d_ref[vp[i]:vp[i + 1]].reshape(m, m)).max()
+        assert err <= tol_abs, (m, err)
+        assert np.array_equal(blk, blk.T), (m, "iterate must be exactly symmetric")
+
+
+def test_order3_convergence_mode_needs_fewer_steps_and_reaches_the_sign(sm):
+    wl = make_config(0)
+    d_or, _ = orc.density_columns(wl, n_threads=THREADS)
+    _, _, p3 = _density_o3(sm, wl, "f64", 100, 1e-8)
+    _, _, p2 = run_density(sm, wl, "f64", 100, 1e-8, "gershgorin")
+    assert np.abs(p3.D.cpu().numpy() - d_or).max() <= 1e-10
+    assert sm.sm_sign_status(p3.residual, 1e-8) == sm.SM_OK
+    i3, i2 = p3.iters.cpu().numpy(), p2.iters.cpu().numpy()
+    assert (i3 < i2).all() and 3 * i3.sum() <= 2 * i2.sum() * 1.1      # products: 3 per step vs 2 per step
+    # chunked (several sm_sign_ns_ex calls, columns stopping at different steps in each) gives the same blocks
+    _, P, pc = _density_o3(sm, wl, "f64", 100, 1e-8, max_chunk_elems=40 * int(P_max_sq(sm, wl)))
+    assert torch.equal(pc.D, p3.D)
+    # 16-bit convergence mode: per-submatrix stopping inside the grouped tcgen05 launches
+    _, _, ph = _density_o3(sm, wl, "f16", 40, 2e-3)
+    assert np.abs(ph.D.cpu().numpy() - d_or).max() <= 2e-3
+    assert (ph.iters.cpu().numpy() < 40).all()
+
+
+def P_max_sq(sm, wl):
+    P = sm.sm_build_pattern(sm.Bcsr(wl), 16)
+    return P.max_dim_pad ** 2
+
+
+def test_order3_with_precision_schedule_and_flag_errors(sm):
+    wl = make_config(0)
+    d_or, _ = orc.density_columns(wl, n_threads=THREADS)
+    _, _, pb = _density_o3(sm, wl, "bf16", 9, 0.0)
+    _, _, ps = _density_o3(sm, wl, "bf16", 9, 0.0, switch_iter=1)
+    eb = np.abs(pb.D.cpu().numpy() - d_or).max()
+    es = np.abs(ps.D.cpu().numpy() - d_or).max()
+    assert es < eb and es <= 4e-3, (eb, es)
+    # non-symmetric matrices are not supported by the third-order path
+    A = sm.Bcsr(wl)
+    P = sm.sm_build_pattern(A, 16)
+    cols, col_off, n = sm.sm_plan_columns(P, P.order)
+    X, _ = sm.sm_gather(A, P, cols, col_off, n, 0.0, "gershgorin", "f64")
+    with pytest.raises(sm.SmError) as e:
+        sm.sm_sign_ns(P, cols, col_off, n, P.packed_elems, "f64", X, 3, 0.0, flags=sm.SM_SIGN_ORDER3 | sm.SM_SIGN_NONSYMMETRIC)
+    assert e.value.status == sm.SM_ERR_UNSUPPORTED
+    with pytest.raises(sm.SmError) as e:
+        sm.sm_sign_ns(P, cols, col_off, n, P.packed_elems, "f64", X, 3, 0.0, flags=4)
+    assert e.value.status == sm.SM_ERR_ARG
