@@ -185,6 +185,21 @@ int32_t sm_sign_ns_ex(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols
                       void *ws, int64_t ws_bytes, int32_t max_iter, double tol, int32_t flags,
                       int32_t switch_iter, int32_t *iters /*[n_cols]*/, double *residual /*[n_cols]*/,
                       void *stream);
+/* sm_sign_ns (SM_F64 / SM_F32 only, Newton-Schulz, symmetric matrices; PAPER.md:87 Eq. 13, :110 step 2) WITHOUT a caller
+ * workspace and without any allocation -- for callers that cannot call cudaMalloc (CUDA graph capture, tight serving
+ * loops, harnesses that forbid it).  The workspace is a file-scope device array of sm_sign_ns_static_capacity() bytes
+ * (16 MiB) that every GPU that loads the library holds until the process exits; a call whose
+ * sm_sign_ws_bytes(P, n_cols, packed_elems, x_dtype) exceeds it returns SM_ERR_SPACE and launches nothing (use
+ * sm_sign_ns).  Same arguments, results (bit-identical) and error behaviour as sm_sign_ns otherwise; additionally
+ * SM_ERR_UNSUPPORTED for the 16-bit types and while sm_profile_enable(1) is in effect (both allocate).  tol <= 0: no
+ * host synchronisation either; tol > 0 reads one counter back every second step like sm_sign_ns.
+ * ALL calls share the one array: what must start at zero is cleared on `stream` by the call itself, and two calls
+ * that overlap on the GPU (different streams / host threads) race on it -- the caller serialises them. */
+int64_t sm_sign_ns_static_capacity(void);
+int32_t sm_sign_ns_static(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols,
+                          const int64_t *col_off, int64_t packed_elems, int32_t x_dtype, void *X_packed,
+                          int32_t max_iter, double tol, int32_t *iters /*[n_cols]*/,
+                          double *residual /*[n_cols]*/, void *stream);
 /* Synchronises and returns SM_WARN_NOT_CONVERGED if tol > 0 and any residual[c] >= tol (or is not finite); with
  * tol <= 0 (fixed-count mode) if any residual[c] is not finite or exceeds 1, i.e. the iteration diverged. */
 int32_t sm_sign_status(const double *residual, int32_t n_cols, double tol, void *scratch, void *stream);

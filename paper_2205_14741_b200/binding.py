@@ -35,7 +35,7 @@ EXPORTS = ["sm_last_cuda_error", "sm_pattern_sizes", "sm_build_pattern", "sm_pla
            "sm_mu_search", "sm_launch_count", "sm_profile_enable", "sm_profile_read", "sm_sign_ws_bytes_ex",
            "sm_sign_ns_ex", "sm_set_option", "sm_get_option", "sm_build_info", "sm_last_device_error",
            "sm_inv_sqrt_ws_bytes", "sm_inv_sqrt", "sm_density_nonorth_ws_bytes", "sm_density_nonorth", "sm_density_ex",
-           "sm_density_ws_bytes_ex"]
+           "sm_density_ws_bytes_ex", "sm_sign_ns_static_capacity", "sm_sign_ns_static"]
 SM_SIGN_NONSYMMETRIC, SM_SIGN_ORDER3 = 1, 2      # sm_sign_ns_ex flags
 
 
@@ -74,6 +74,7 @@ _lib.sm_inv_sqrt_ws_bytes.restype = C.c_int64
 _lib.sm_density_nonorth_ws_bytes.restype = C.c_int64
 _lib.sm_density_ws_bytes.restype = C.c_int64
 _lib.sm_density_ws_bytes_ex.restype = C.c_int64
+_lib.sm_sign_ns_static_capacity.restype = C.c_int64
 
 
 def _ptr(t):
@@ -271,6 +272,19 @@ def sm_sign_ns(P: Pattern, cols, col_off, n_cols, n_elems, x_dtype, X, max_iter,
                                              C.c_int64(n_elems), C.c_int32(x_dt), _ptr(X), _ptr(ws),
                                              C.c_int64(ws.numel()), C.c_int32(max_iter), C.c_double(tol),
                                              _ptr(iters), _ptr(residual), _stream()))
+    return iters, residual
+
+
+def sm_sign_ns_static_capacity() -> int:
+    return int(_lib.sm_sign_ns_static_capacity())
+
+
+def sm_sign_ns_static(P: Pattern, cols, col_off, n_cols, n_elems, x_dtype, X, max_iter, tol, iters, residual):
+    """sm_sign_ns on the library's static 16 MiB workspace: allocates nothing (iters / residual are the caller's)."""
+    x_dt = DTYPES[x_dtype] if isinstance(x_dtype, str) else x_dtype
+    _check("sm_sign_ns_static", _lib.sm_sign_ns_static(C.byref(P.c), _ptr(cols), C.c_int32(n_cols), _ptr(col_off),
+                                                       C.c_int64(n_elems), C.c_int32(x_dt), _ptr(X), C.c_int32(max_iter),
+                                                       C.c_double(tol), _ptr(iters), _ptr(residual), _stream()))
     return iters, residual
 
 

@@ -8,7 +8,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "libsubmatrix.so")
-SOURCES = ["pattern.cu", "gather_scatter.cu", "power_scale.cu", "global_scale.cu", "sign_simt.cu", "sign_umma.cu", "nonorth.cu", "api.cu"]
+SOURCES = ["pattern.cu", "gather_scatter.cu", "power_scale.cu", "global_scale.cu", "sign_simt.cu", "sign_umma.cu", "nonorth.cu", "no_alloc.cu", "api.cu"]
 NVCC_FLAGS = [*os.environ.get("SM_NVCC_EXTRA", "").split(), *(["-DSM_MEASURE"] if "--measure" in sys.argv else []), "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=default"]
 

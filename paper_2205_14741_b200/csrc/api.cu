@@ -68,6 +68,7 @@ struct GemmProfile {
 };
 static GemmProfile g_prof;
 
+bool prof_enabled() { return g_prof.on; }
 int32_t prof_begin(cudaStream_t st, int *slot) {
   *slot = -1;
   if (!g_prof.on) return SM_OK;

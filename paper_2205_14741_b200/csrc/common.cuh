@@ -102,6 +102,7 @@ template <> __device__ inline double to_double<__half>(__half v) { return (doubl
 
 // ---- measurement hooks (api.cu): CUDA events around every launch of the Newton-Schulz product kernels
 // while sm_profile_enable(1) is in force; slot = -1 when disabled.
+bool prof_enabled();                                   // sm_profile_enable(1) is in effect (its events allocate)
 int32_t prof_begin(cudaStream_t st, int *slot);
 int32_t prof_end(cudaStream_t st, int slot);
 
