@@ -206,7 +206,12 @@ def oracle_sample(wl, cfg_run, n_cols_sample, seed, n_threads):
     m = np.array([wl.blk_size[wl.col_idx[wl.row_ptr[i]:wl.row_ptr[i + 1]]].sum() for i in cols], dtype=np.float64)
     k = cfg_run["max_iter"] if cfg_run["tol"] <= 0 else 15   # convergence runs: ~15 updates
     t0 = time.perf_counter()
-    orc.density_columns(wl, cols=cols, n_threads=n_threads)
+    if m.max() > 1000:
+        # configs[4]: cyclic Jacobi needs ~5 min per submatrix at m ~ 1650; the oracle's LAPACK variant (same steps,
+        # numpy.linalg.eigh as the eigensolver; pinned to the Jacobi path in tests/test_oracle_pins.py) keeps the sample bounded
+        orc.density_columns_lapack(wl, cols=cols)
+    else:
+        orc.density_columns(wl, cols=cols, n_threads=n_threads)
     dt = time.perf_counter() - t0
     return dt, 4.0 * float((m ** 3).sum()) * k, cols
 
@@ -215,7 +220,7 @@ def oracle_sample_size(cfg_index, cores):
     # ~10-30 s of CPU work: per-submatrix cost of the Jacobi oracle ~ 2.2e-8 * m^3 s (measured here)
     per = {0: 0.003, 1: 0.25, 2: 4.0, 3: 0.25, 4: 600.0}[cfg_index]      # cfg2: 32 columns took 7 s on 16 cores
     return max(1, min(int(20.0 * cores / per), {0: 32, 1: 1000, 2: 3000, 3: 10000, 4: 2000}[cfg_index])) \
-        if per < 100 else max(1, min(cores, 8))
+        if per < 100 else 32           # configs[4]: LAPACK variant of the oracle, ~1-2 s per submatrix
 
 
 def run_reference(args, cfg, cfg_run):
@@ -233,7 +238,8 @@ def run_reference(args, cfg, cfg_run):
         dt, fl, cols = oracle_sample(wl, cfg_run, n_sample, 9000 + s, cores)
         total_t += dt; total_f += fl; total_cols += len(cols)
     val = total_f / total_t / 1e12
-    sample = f"{n_sample} seeded block columns of {cfg['name']} per step (of {wl.n_blk})"
+    sample = f"{n_sample} seeded block columns of {cfg['name']} per step (of {wl.n_blk})" + \
+        (", LAPACK-eigensolver variant of the oracle" if args.config == 4 else "")
     line = {
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total_t / args.steps,
@@ -522,7 +528,8 @@ def run_ours(args, cfg, cfg_run):
         dt, fl_eq, cols = oracle_sample(make_config(args.config), cfg_run, n_sample, 9000, cores)
         cpu = {"value": fl_eq / dt / 1e12, "unit": UNIT + " (equivalent: 4*sum m^3*k_gpu / t_oracle)",
                "cores": cores, "kind": "oracle", "block_columns_per_s": len(cols) / dt, "seconds": dt,
-               "sample": f"{len(cols)} seeded block columns of {cfg['name']} (of {wl.n_blk}), fp64 Jacobi"}
+               "sample": f"{len(cols)} seeded block columns of {cfg['name']} (of {wl.n_blk}), fp64 " +
+                         ("LAPACK-eigensolver variant of the oracle" if args.config == 4 else "Jacobi")}
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
