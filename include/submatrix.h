@@ -280,8 +280,10 @@ int32_t sm_inv_sqrt(const sm_bcsr_t *S, const void *S_vals, int32_t s_dtype, int
 /* sm_density_nonorth: Eq. 14 with S != I by the submatrix method on the pair (H, S) (one block pattern, two value
  * arrays of type a_dtype): per block column, Z = T_S^-1/2 as in sm_inv_sqrt, S^-1 = Z Z, A = S^-1 T_H - mu I (not
  * symmetric) scaled by its infinity norm, sign(A) by the non-symmetric Newton-Schulz kernels, P_i = 1/2 (I - sign(A)) S^-1,
- * owned columns inserted (optionally symmetrised).  x_dtype = d_dtype = SM_F64 or SM_F32 (the dense products run on
- * the DMMA / FFMA kernels; 16-bit: SM_ERR_UNSUPPORTED).  trace_ps (device fp64 scalar, may be NULL; synchronises once)
+ * owned columns inserted (optionally symmetrised).  x_dtype SM_F64 / SM_F32: d_dtype = x_dtype, a_dtype = x_dtype or
+ * SM_F64 (the dense products run on the DMMA / FFMA kernels).  x_dtype SM_BF16 / SM_F16 (pad_to % 64 == 0): a_dtype and
+ * d_dtype SM_F64 or SM_F32 independently; the products run on the non-symmetric tcgen05 update kernel with its identity
+ * term switched off, every intermediate is a 16-bit image.  Other combinations: SM_ERR_UNSUPPORTED.  trace_ps (device fp64 scalar, may be NULL; synchronises once)
  * receives Tr(P S), the electron count.  iters / residual / scale report the sign(A) iteration.  Asynchronous
  * otherwise. */
 int64_t sm_density_nonorth_ws_bytes(const sm_bcsr_t *A, const sm_pattern_t *P, int32_t x_dtype, int64_t max_chunk_elems2);

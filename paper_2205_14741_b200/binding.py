@@ -404,8 +404,10 @@ def sm_inv_sqrt(S: Bcsr, P: Pattern, x_dtype, max_iter=100, tol=0.0, max_chunk_e
 
 def sm_density_nonorth(A: Bcsr, S_vals, P: Pattern, x_dtype, mu=0.0, max_iter=100, tol=0.0, symmetrise=False,
                        max_chunk_elems2=None):
-    """f2 (Eq. 14 with S != I): returns (P_vals, Tr(P S), iters, residual, scale)."""
+    """f2 (Eq. 14 with S != I): returns (P_vals, Tr(P S), iters, residual, scale); P_vals in the arithmetic type for
+    fp64 / fp32, fp64 for the 16-bit types."""
     x_dt = DTYPES[x_dtype]
+    d_dt = x_dt if x_dt in (SM_F64, SM_F32) else SM_F64
     total2, largest2 = _doubled_elems(P)
     mce = max(int(max_chunk_elems2 or total2), largest2)
     wsb = int(_lib.sm_density_nonorth_ws_bytes(C.byref(A.c), C.byref(P.c), C.c_int32(x_dt), C.c_int64(mce)))
@@ -413,7 +415,7 @@ def sm_density_nonorth(A: Bcsr, S_vals, P: Pattern, x_dtype, mu=0.0, max_iter=10
         raise SmError("sm_density_nonorth_ws_bytes", wsb)
     dev = A.device
     ws = torch.empty(wsb, dtype=torch.uint8, device=dev)
-    Pv = torch.zeros(A.n_vals, dtype=TORCH_DTYPE[x_dt], device=dev)
+    Pv = torch.zeros(A.n_vals, dtype=TORCH_DTYPE[d_dt], device=dev)
     tr = torch.zeros(1, dtype=torch.float64, device=dev)
     iters = torch.zeros(A.n_blk, dtype=torch.int32, device=dev)
     residual = torch.zeros(A.n_blk, dtype=torch.float64, device=dev)
@@ -422,7 +424,7 @@ def sm_density_nonorth(A: Bcsr, S_vals, P: Pattern, x_dtype, mu=0.0, max_iter=10
     _check("sm_density_nonorth", _lib.sm_density_nonorth(
         C.byref(A.c), _ptr(A.vals), _ptr(S_vals), C.c_int32(A.val_dtype), C.c_double(mu), C.c_int32(x_dt),
         C.c_int32(max_iter), C.c_double(tol), C.c_int32(1 if symmetrise else 0), C.byref(P.c),
-        h_dim.ctypes.data_as(C.c_void_p), C.c_int64(mce), _ptr(ws), C.c_int64(ws.numel()), C.c_int32(x_dt), _ptr(Pv),
+        h_dim.ctypes.data_as(C.c_void_p), C.c_int64(mce), _ptr(ws), C.c_int64(ws.numel()), C.c_int32(d_dt), _ptr(Pv),
         _ptr(tr), _ptr(iters), _ptr(residual), _ptr(scale), _stream()))
     return Pv, tr, iters, residual, scale
 

@@ -129,6 +129,8 @@ int32_t dense_product(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols
                       const void *A, const void *B, void *O, int32_t *active, int32_t *last_zero, cudaStream_t st);   // sign_simt.cu
 int64_t sign_umma_ws_bytes(const sm_pattern_t *P, int32_t n_cols, int64_t packed_elems, int32_t x_dtype, int32_t nonsym,
                            int32_t order);
+int32_t umma_product(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, const int64_t *col_off, int64_t packed_elems,
+                     int32_t x_dtype, const void *A, const void *B, void *O, void *ws, int64_t ws_bytes, cudaStream_t st);   // sign_umma.cu
 int32_t *device_err_word();        // pinned, device-mapped host word the kernels write a protocol-failure code to (api.cu)
 
 // ---- variant selection (api.cu): sm_set_option / environment at first use.  Ids are indices into the table there.

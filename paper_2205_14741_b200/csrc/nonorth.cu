@@ -9,7 +9,7 @@
 // +-sqrt(lambda(T_i)) / s_i, inside (0, 1] in modulus), run the SAME Newton-Schulz kernels on it at doubled dimension
 // with the non-symmetric flag (a3, sm_sign_ns_ex), take the lower-left block T_i^-1/2 (and the upper-right T_i^1/2) and
 // insert the owned columns into block-sparse results (a4).  sign(M / s) = sign(M): no rescaling of the blocks.
-// sm_density_nonorth: Eq. 14 per submatrix of the pair (H, S), fp64 / fp32: Z = T_S^-1/2 as above, S^-1 = Z Z,
+// sm_density_nonorth: Eq. 14 per submatrix of the pair (H, S), all four dtypes: Z = T_S^-1/2 as above, S^-1 = Z Z,
 // A = S^-1 T_H - mu I (not symmetric), scaled by its infinity norm (>= spectral radius), sign(A) by the non-symmetric
 // Newton-Schulz kernels, P_i = 1/2 (I - sign(A)) S^-1, owned columns inserted; Tr(P S) = electron count.
 #include <algorithm>
@@ -75,8 +75,8 @@ __global__ void k_block2_extract(const int32_t *__restrict__ cols, const int32_t
   }
 }
 
-// A_c <- (A_c - mu I) / s_c with s_c = max row sum of |A_c - mu I| (>= spectral radius); row-major fp64 / fp32.
-template <typename T>
+// A_c <- (A_c - mu I) / s_c with s_c = max row sum of |A_c - mu I| (>= spectral radius).
+template <typename T, bool IMG>
 __global__ void k_shift_scale(const int32_t *__restrict__ cols, const int32_t *__restrict__ dim,
                               const int32_t *__restrict__ dim_pad, const int64_t *__restrict__ col_off, double mu,
                               T *__restrict__ A, double *__restrict__ scale) {
@@ -87,7 +87,7 @@ __global__ void k_shift_scale(const int32_t *__restrict__ cols, const int32_t *_
   double best = 0.0;
   for (int32_t r = threadIdx.x; r < m; r += blockDim.x) {
     double sum = 0.0;
-    for (int32_t cc = 0; cc < m; ++cc) sum += fabs(to_double<T>(Ac[(int64_t)r * Pd + cc]) - (cc == r ? mu : 0.0));
+    for (int32_t cc = 0; cc < m; ++cc) sum += fabs(to_double<T>(Ac[eoff<T, IMG>(Pd, r, cc)]) - (cc == r ? mu : 0.0));
     best = fmax(best, sum);
   }
   red[threadIdx.x] = best;
@@ -100,13 +100,13 @@ __global__ void k_shift_scale(const int32_t *__restrict__ cols, const int32_t *_
   if (threadIdx.x == 0) scale[c] = s;
   for (int64_t e = threadIdx.x; e < (int64_t)m * m; e += blockDim.x) {
     const int32_t r = (int32_t)(e / m), cc = (int32_t)(e - (int64_t)r * m);
-    const int64_t o = (int64_t)r * Pd + cc;
+    const int64_t o = eoff<T, IMG>(Pd, r, cc);
     Ac[o] = from_double<T>((to_double<T>(Ac[o]) - (cc == r ? mu : 0.0)) / s);
   }
 }
 
 // Q_c <- 1/2 (I - S_c), true part only (padding stays 0)
-template <typename T>
+template <typename T, bool IMG>
 __global__ void k_half_i_minus(const int32_t *__restrict__ cols, const int32_t *__restrict__ dim,
                                const int32_t *__restrict__ dim_pad, const int64_t *__restrict__ col_off,
                                T *__restrict__ S) {
@@ -115,7 +115,7 @@ __global__ void k_half_i_minus(const int32_t *__restrict__ cols, const int32_t *
   T *Sc = S + col_off[c];
   for (int64_t e = (int64_t)blockIdx.y * blockDim.x + threadIdx.x; e < (int64_t)m * m; e += (int64_t)gridDim.y * blockDim.x) {
     const int32_t r = (int32_t)(e / m), cc = (int32_t)(e - (int64_t)r * m);
-    const int64_t o = (int64_t)r * Pd + cc;
+    const int64_t o = eoff<T, IMG>(Pd, r, cc);
     Sc[o] = from_double<T>(0.5 * ((cc == r ? 1.0 : 0.0) - to_double<T>(Sc[o])));
   }
 }
@@ -149,6 +149,9 @@ sm_pattern_t doubled_pattern(const sm_pattern_t *P, int32_t *dim2, int32_t *dim_
   return Q;
 }
 
+// element stride between the m-dimension buffers of nonorth_chunk (bulk copies need 16-byte aligned images)
+inline int64_t buf_stride(int64_t max2) { return (max2 + 4095) & ~(int64_t)4095; }
+
 struct InvWs {
   int64_t *col_off, *col_off2; int32_t *dim2, *dim_pad2, *ones, *zeros; void *X, *X2, *gws, *sws;
   int64_t gws_bytes, sws_bytes, used;
@@ -165,7 +168,8 @@ InvWs inv_layout(void *ws, int64_t ws_bytes, const sm_bcsr_t *S, const sm_patter
   w.ones = cur.take<int32_t>(n);
   w.zeros = cur.take<int32_t>(n);
   const int64_t eb = dtype_bytes(x_dtype);
-  w.X = cur.take<char>(max2 * eb * (1 + n_extra));      // m-dimension buffers (each <= the doubled chunk size)
+  // m-dimension buffers (each <= the doubled chunk size), at a stride that keeps every one of them 8 KB aligned
+  w.X = cur.take<char>(buf_stride(max2) * eb * (1 + n_extra));
   w.X2 = cur.take<char>(max2 * eb);
   w.gws_bytes = sm_gather_ws_bytes(S, P, n);
   w.gws = cur.take<char>(w.gws_bytes);
@@ -284,35 +288,41 @@ extern "C" int32_t sm_inv_sqrt(const sm_bcsr_t *S, const void *S_vals, int32_t s
 extern "C" int64_t sm_density_nonorth_ws_bytes(const sm_bcsr_t *A, const sm_pattern_t *P, int32_t x_dtype,
                                                int64_t max_chunk_elems2) {
   if (!A || !P) return SM_ERR_ARG;
-  if (x_dtype != SM_F64 && x_dtype != SM_F32) return SM_ERR_UNSUPPORTED;
+  if (dtype_bytes(x_dtype) == 0) return SM_ERR_UNSUPPORTED;
   const int64_t p2 = (2 * (int64_t)P->max_dim + P->pad_to - 1) / P->pad_to * P->pad_to;
   if (max_chunk_elems2 < p2 * p2) return SM_ERR_ARG;
   return inv_layout(nullptr, 0, A, P, x_dtype, max_chunk_elems2, 3).used;
 }
 
-template <typename T>
+template <typename T, bool IMG>
 static int32_t nonorth_chunk(const sm_bcsr_t *A, const void *H_vals, const void *S_vals, int32_t a_dtype, double mu,
                              int32_t x_dtype, int32_t max_iter, double tol, const sm_pattern_t *P, const sm_pattern_t *Q,
                              const InvWs &w, const Chunk &ch, int64_t max2, int32_t d_dtype, void *P_vals, int32_t *iters,
                              double *residual, double *scale, cudaStream_t st) {
   const int32_t nc = ch.hi - ch.lo;
   const int32_t *cols = P->order + ch.lo;
-  T *B0 = (T *)w.X, *B1 = B0 + max2, *B2 = B1 + max2, *B3 = B2 + max2;
+  const int64_t bs = buf_stride(max2);
+  T *B0 = (T *)w.X, *B1 = B0 + bs, *B2 = B1 + bs, *B3 = B2 + bs;
   // the product kernels write the true m x m part only and the DMMA kernel reads whole padded tiles: padding must be 0
   SM_CUDA(cudaMemsetAsync(B2, 0, (size_t)ch.elems * sizeof(T), st));
   SM_CUDA(cudaMemsetAsync(B3, 0, (size_t)ch.elems * sizeof(T), st));
+  // fp64 / fp32: the DMMA / FFMA product kernels; 16-bit: the non-symmetric tcgen05 update kernel without its "+ X"
+  auto product = [&](const T *Am, const T *Bm, T *Om) -> int32_t {
+    if (IMG) return umma_product(P, cols, nc, w.col_off, ch.elems, x_dtype, Am, Bm, Om, w.sws, w.sws_bytes, st);
+    return dense_product(P, cols, nc, w.col_off, x_dtype, Am, Bm, Om, w.ones, w.zeros, st);
+  };
   // Z = T_S^-1/2 -> B1 (B0 is the gather / extraction scratch of inv_sqrt_chunk)
-  int32_t rc = inv_sqrt_chunk<T, false>(A, S_vals, a_dtype, x_dtype, max_iter, tol, P, Q, w, ch, B1, iters, residual, scale, st);
+  int32_t rc = inv_sqrt_chunk<T, IMG>(A, S_vals, a_dtype, x_dtype, max_iter, tol, P, Q, w, ch, B1, iters, residual, scale, st);
   if (rc != SM_OK) return rc;
   // S^-1 = Z Z -> B2
-  rc = dense_product(P, cols, nc, w.col_off, x_dtype, B1, B1, B2, w.ones, w.zeros, st);
+  rc = product(B1, B1, B2);
   if (rc != SM_OK) return rc;
   // T_H (unscaled) -> B0; A = S^-1 T_H -> B3; A <- (A - mu I) / ||A - mu I||_inf
   rc = sm_gather(A, H_vals, a_dtype, P, cols, nc, w.col_off, 0.0, SM_SCALE_NONE, x_dtype, B0, scale + ch.lo, w.gws, w.gws_bytes, st);
   if (rc != SM_OK) return rc;
-  rc = dense_product(P, cols, nc, w.col_off, x_dtype, B2, B0, B3, w.ones, w.zeros, st);
+  rc = product(B2, B0, B3);
   if (rc != SM_OK) return rc;
-  k_shift_scale<T><<<nc, 256, 0, st>>>(cols, P->dim, P->dim_pad, w.col_off, mu, B3, scale + ch.lo);
+  k_shift_scale<T, IMG><<<nc, 256, 0, st>>>(cols, P->dim, P->dim_pad, w.col_off, mu, B3, scale + ch.lo);
   SM_LAUNCHED();
   // sign(A), non-symmetric Newton-Schulz at dimension m
   rc = sm_sign_ns_ex(P, cols, nc, w.col_off, ch.elems, x_dtype, B3, w.sws, w.sws_bytes, max_iter, tol, SM_SIGN_NONSYMMETRIC,
@@ -320,9 +330,9 @@ static int32_t nonorth_chunk(const sm_bcsr_t *A, const void *H_vals, const void 
   if (rc != SM_OK) return rc;
   // P_i = 1/2 (I - sign(A)) S^-1 -> B0, owned columns inserted (P_i is symmetric: the owned rows are read)
   dim3 g2(nc, 16);
-  k_half_i_minus<T><<<g2, 256, 0, st>>>(cols, P->dim, P->dim_pad, w.col_off, B3);
+  k_half_i_minus<T, IMG><<<g2, 256, 0, st>>>(cols, P->dim, P->dim_pad, w.col_off, B3);
   SM_LAUNCHED();
-  rc = dense_product(P, cols, nc, w.col_off, x_dtype, B3, B2, B0, w.ones, w.zeros, st);
+  rc = product(B3, B2, B0);
   if (rc != SM_OK) return rc;
   return sm_scatter(A, P, cols, nc, w.col_off, x_dtype, B0, d_dtype, P_vals, 0, st);
 }
@@ -333,9 +343,12 @@ extern "C" int32_t sm_density_nonorth(const sm_bcsr_t *A, const void *H_vals, co
                                       int64_t ws_bytes, int32_t d_dtype, void *P_vals, double *trace_ps, int32_t *iters,
                                       double *residual, double *scale, void *stream) {
   if (!A || !H_vals || !S_vals || !P || !h_dim || !ws || !P_vals || !iters || !residual || !scale) return SM_ERR_ARG;
-  if (x_dtype != SM_F64 && x_dtype != SM_F32) return SM_ERR_UNSUPPORTED;
-  if (d_dtype != x_dtype) return SM_ERR_UNSUPPORTED;          // Tr(P S) is taken on equal-typed value arrays
-  if (a_dtype != x_dtype && a_dtype != SM_F64) return SM_ERR_UNSUPPORTED;
+  if (dtype_bytes(x_dtype) == 0) return SM_ERR_UNSUPPORTED;
+  const bool img = x_dtype == SM_BF16 || x_dtype == SM_F16;
+  if (d_dtype != SM_F64 && d_dtype != SM_F32) return SM_ERR_UNSUPPORTED;
+  if (!img && d_dtype != x_dtype) return SM_ERR_UNSUPPORTED;   // fp64 / fp32: P in the arithmetic type
+  if (a_dtype != SM_F64 && a_dtype != SM_F32) return SM_ERR_UNSUPPORTED;
+  if (!img && a_dtype != x_dtype && a_dtype != SM_F64) return SM_ERR_UNSUPPORTED;
   const int64_t p2 = (2 * (int64_t)P->max_dim + P->pad_to - 1) / P->pad_to * P->pad_to;
   if (max_chunk_elems2 < p2 * p2) return SM_ERR_ARG;
   InvWs w = inv_layout(ws, ws_bytes, A, P, x_dtype, max_chunk_elems2, 3);
@@ -352,9 +365,11 @@ extern "C" int32_t sm_density_nonorth(const sm_bcsr_t *A, const void *H_vals, co
   sm_pattern_t Q = doubled_pattern(P, w.dim2, w.dim_pad2);
   std::vector<int32_t> ord;
   for (const Chunk &ch : plan_chunks(P, h_dim, max_chunk_elems2, ord)) {
-    int32_t rc = x_dtype == SM_F64
-                     ? nonorth_chunk<double>(A, H_vals, S_vals, a_dtype, mu, x_dtype, max_iter, tol, P, &Q, w, ch, max_chunk_elems2, d_dtype, P_vals, iters, residual, scale, st)
-                     : nonorth_chunk<float>(A, H_vals, S_vals, a_dtype, mu, x_dtype, max_iter, tol, P, &Q, w, ch, max_chunk_elems2, d_dtype, P_vals, iters, residual, scale, st);
+    int32_t rc =
+        x_dtype == SM_F64 ? nonorth_chunk<double, false>(A, H_vals, S_vals, a_dtype, mu, x_dtype, max_iter, tol, P, &Q, w, ch, max_chunk_elems2, d_dtype, P_vals, iters, residual, scale, st)
+        : x_dtype == SM_F32 ? nonorth_chunk<float, false>(A, H_vals, S_vals, a_dtype, mu, x_dtype, max_iter, tol, P, &Q, w, ch, max_chunk_elems2, d_dtype, P_vals, iters, residual, scale, st)
+        : x_dtype == SM_BF16 ? nonorth_chunk<__nv_bfloat16, true>(A, H_vals, S_vals, a_dtype, mu, x_dtype, max_iter, tol, P, &Q, w, ch, max_chunk_elems2, d_dtype, P_vals, iters, residual, scale, st)
+                             : nonorth_chunk<__half, true>(A, H_vals, S_vals, a_dtype, mu, x_dtype, max_iter, tol, P, &Q, w, ch, max_chunk_elems2, d_dtype, P_vals, iters, residual, scale, st);
     if (rc != SM_OK) return rc;
   }
   if (symmetrise) {
@@ -366,7 +381,8 @@ extern "C" int32_t sm_density_nonorth(const sm_bcsr_t *A, const void *H_vals, co
     int64_t n_vals = 0;
     SM_CUDA(cudaMemcpyAsync(&n_vals, A->val_ptr + A->nnzb, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
     SM_CUDA(cudaStreamSynchronize(st));
-    if (d_dtype == SM_F64) k_dot<double, double><<<1, 1024, 0, st>>>(n_vals, (const double *)P_vals, (const double *)S_vals, trace_ps);
+    if (d_dtype == SM_F64 && a_dtype == SM_F32) k_dot<double, float><<<1, 1024, 0, st>>>(n_vals, (const double *)P_vals, (const float *)S_vals, trace_ps);
+    else if (d_dtype == SM_F64) k_dot<double, double><<<1, 1024, 0, st>>>(n_vals, (const double *)P_vals, (const double *)S_vals, trace_ps);
     else if (a_dtype == SM_F32) k_dot<float, float><<<1, 1024, 0, st>>>(n_vals, (const float *)P_vals, (const float *)S_vals, trace_ps);
     else k_dot<float, double><<<1, 1024, 0, st>>>(n_vals, (const float *)P_vals, (const double *)S_vals, trace_ps);
     SM_LAUNCHED();

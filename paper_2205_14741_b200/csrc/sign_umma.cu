@@ -117,6 +117,7 @@ struct UArgs {
   // third-order iteration (f3, reading A22): product 1 stores Q = w_scale (Y - I) (-1/2: Newton-Schulz; -3/4: order 3),
   // the update-type product scales its accumulator by out_scale (1; 2/3 for Z = 2/3 (Q + Q Q))
   float w_scale, out_scale;
+  int32_t no_ident;          // update product without its "+ X" (identity MMAs skipped): a plain product O = X Wh (f2, Eq. 14)
 };
 
 // Tile geometry.  Only elements (r, c) with c <= r are computed, so tile row tm (rows tm*R ..
@@ -657,7 +658,7 @@ k_umma_gemm(UArgs a, const __grid_constant__ CUtensorMap mapA, const __grid_cons
             for (int ks = 0; ks < ksteps; ++ks)
               mma(d_tmem, adesc + (uint64_t)(2 * ks), bdesc + bstep * (uint64_t)ks, idesc, (uint32_t)((kc | ks) != 0));
           }
-          if (p2 && !SM_DBG(a, 2)) {
+          if (p2 && !a.no_ident && !SM_DBG(a, 2)) {
             // "+ X": the A chunk in this stage holds X[rows, 64 kc .. 64 kc + 63]; add it to the accumulator
             // columns [lo, hi) of the tile that it covers (B = identity slice, K-major)
             const int32_t lo = max(kc * UK, u.n0), hi = min(kc * UK + UK, u.n0 + u.nt);
@@ -1066,7 +1067,7 @@ static __global__ void k_sign_init_grouped(int32_t n_cols, const int32_t *__rest
   if (c >= n_cols) return;
   const bool mine = dim_pad[cols ? cols[c] : c] > skip_pd;
   active[c] = mine ? 1 : 0; last[c] = 0;
-  if (mine) { iters[c] = 0; residual[c] = 0.0; }
+  if (mine) { if (iters) iters[c] = 0; if (residual) residual[c] = 0.0; }
 }
 
 constexpr int UMMA_MAX_COUNTERS = 256;      // 2 per step; more steps than that fall back to the static deal
@@ -1446,6 +1447,37 @@ int32_t sign_umma(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, co
   k_copy_back<<<cg, 256, 0, st>>>(cols, col_off, iters, 2, P->dim_pad, res_pd, (const char *)buf[1], (char *)X);
   SM_LAUNCHED();
   return SM_OK;
+}
+
+// O_c = A_c B_c for every listed submatrix, 16-bit images, true products on every tile (nothing assumed symmetric):
+// the non-symmetric update kernel (A K-major, B MN-major from its image) with the identity MMAs switched off.
+// ws: a sign workspace of the same call shape (sm_sign_ws_bytes_ex with SM_SIGN_NONSYMMETRIC); only its tile table and
+// flags are used.  Used by sm_density_nonorth (f2, Eq. 14: S^-1 = Z Z, S^-1 T_H, 1/2 (I - sign) S^-1).
+int32_t umma_product(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, const int64_t *col_off,
+                     int64_t packed_elems, int32_t x_dtype, const void *A, const void *B, void *O, void *ws,
+                     int64_t ws_bytes, cudaStream_t st) {
+  if ((P->pad_to % 64) != 0) return SM_ERR_ARG;
+  const int32_t sym = 0, ncta = 1, R = UM;
+  UmmaWs w = umma_layout(ws, ws_bytes, P, n_cols, packed_elems, sym, true);
+  if (w.used > ws_bytes) return SM_ERR_SPACE;
+  int dev = 0, n_sm = 0;
+  SM_CUDA(cudaGetDevice(&dev));
+  SM_CUDA(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
+  w.err = device_err_word();
+  const int32_t nb = (n_cols + 255) / 256;
+  SignState s{w.active, w.last, w.n_still, w.partial, w.parts_per_col};
+  k_sign_init_grouped<<<nb, 256, 0, st>>>(n_cols, cols, P->dim_pad, 0, w.active, w.last, nullptr, nullptr);
+  SM_LAUNCHED();
+  k_umma_tilecounts<<<nb, 256, 0, st>>>(n_cols, R, sym, EPI_WARPS * ncta, 0, cols, P->dim, P->dim_pad, w.tile_ptr, w.n_parts);
+  SM_LAUNCHED();
+  { int32_t rc = exclusive_scan_i64(n_cols, w.tile_ptr, w.tile_ptr, st); if (rc != SM_OK) return rc; }
+  k_umma_build_tiles<<<nb, 256, 0, st>>>(n_cols, R, sym, 0, cols, P->dim, P->dim_pad, col_off, w.tile_ptr, w.tiles);
+  SM_LAUNCHED();
+  SM_CUDA(cudaMemsetAsync(O, 0, packed_elems * 2, st));       // padding of the result reads as zeros
+  UArgs a{cols, col_off, P->dim, P->dim_pad, w.tile_ptr, w.tiles, n_cols, 0, A, B, O, s, w.err, 0, nullptr, 0, nullptr, 0, 0, 0, 0,
+          -0.5f, 1.f, 1};
+  UMaps maps{};
+  return launch_umma_any<2>(x_dtype == SM_BF16, 1, sym, opt(OPT_UMMA_STAGES) ? opt(OPT_UMMA_STAGES) : 4, a, maps, n_sm, st);
 }
 
 }  // namespace sm

@@ -94,3 +94,33 @@ def test_density_nonorth_full_coverage_is_the_generalised_projector(sm):
     torch.cuda.synchronize()
     ev = sl.eigh(wl.dense(), wS.dense(), eigvals_only=True)
     assert abs(tr.item() - (ev < 0).sum()) <= 1e-8            # Tr(P S) = number of generalised eigenvalues below mu
+
+
+# 16-bit Eq. 14 chains five 16-bit-rounded stages (sign of the doubled matrix, Z Z, S^-1 T_H, sign, (I - sign) S^-1 / 2): fp16
+# stays far inside the hot path's relF limit 2e-2; bf16 (8 significand bits) is given twice that limit on the 23-orbital
+# workload (measured 2.5e-2), the price of two chained sign iterations.
+@pytest.mark.parametrize("x_dtype,kind,val_dtype,lim", [("f16", "mid23", "f64", 2e-2), ("bf16", "mid23", "f64", 4e-2),
+                                                         ("f16", "mid6", "f32", 2e-2), ("bf16", "cfg0", "f32", 2e-2),
+                                                         ("f16", "ragged", "f64", 2e-2)])
+def test_density_nonorth_16bit(sm, x_dtype, kind, val_dtype, lim):
+    """Eq. 14 with S != I on the tcgen05 kernels: S^-1/2 by the non-symmetric sign of the doubled matrix, the three dense
+    products by the non-symmetric update kernel without its identity term (umma_product), the sign of S^-1 H - mu I."""
+    wl, wS = pair(kind)
+    mu = 0.05
+    p_or = orc.density_nonorth_columns(wl, wS, mu)
+    A = sm.Bcsr(wl, val_dtype=val_dtype)
+    Sd = sm.Bcsr(wS, val_dtype=val_dtype)
+    P = sm.sm_build_pattern(A, 64)
+    Pv, tr, iters, res, _ = sm.sm_density_nonorth(A, Sd.vals, P, x_dtype, mu=mu, max_iter=30, tol=0.0)
+    torch.cuda.synchronize()
+    Ph = Pv.cpu().numpy()
+    rel = np.linalg.norm(Ph - p_or) / np.linalg.norm(p_or)
+    dtr = abs(tr.item() - float((p_or * wS.vals).sum())) / wl.n
+    print(kind, x_dtype, "relF", rel, "maxabs", np.abs(Ph - p_or).max(), "dTr/n", dtr)
+    assert np.isfinite(Ph).all() and rel <= lim and dtr <= 1.5e-3
+    assert (iters == 30).all()
+    # chunked (buffer stride not a multiple of the image size) = unchunked, bit for bit
+    tot2, big2 = sm._doubled_elems(P)
+    Pc, _, _, _, _ = sm.sm_density_nonorth(A, Sd.vals, P, x_dtype, mu=mu, max_iter=30, tol=0.0, max_chunk_elems2=max(big2, tot2 // 3 + 1))
+    torch.cuda.synchronize()
+    assert torch.equal(Pc, Pv)
