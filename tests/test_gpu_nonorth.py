@@ -17,6 +17,16 @@ def sm():
     return b
 
 
+_ORACLE = {}
+
+
+def oracle_cached(name, kind, fn):
+    """Oracle results are reused by the tests of one workload (the Jacobi sweeps of the 23-orbital pair take 35-70 s)."""
+    if (name, kind) not in _ORACLE:
+        _ORACLE[(name, kind)] = fn()
+    return _ORACLE[(name, kind)]
+
+
 def pair(kind):
     wl = {"cfg0": lambda: make_config(0), "mid6": lambda: make_workload(150, 6, 3, 6.0, seed=71),
           "mid23": lambda: make_workload(24, 23, 4, 5.0, seed=72),
@@ -27,7 +37,7 @@ def pair(kind):
 @pytest.mark.parametrize("kind", ["cfg0", "mid6", "ragged"])
 def test_inv_sqrt_fp64_all_columns(sm, kind):
     wl, wS = pair(kind)
-    z_or, y_or, lam = orc.inv_sqrt_columns(wS)
+    z_or, y_or, lam = oracle_cached("inv_sqrt", kind, lambda: orc.inv_sqrt_columns(wS))
     S = sm.Bcsr(wS)
     P = sm.sm_build_pattern(S, 16)
     Z, Y, iters, res, scale = sm.sm_inv_sqrt(S, P, "f64", max_iter=100, tol=1e-9, want_sqrt=True)
@@ -44,7 +54,7 @@ def test_inv_sqrt_fp64_all_columns(sm, kind):
 
 def test_inv_sqrt_fp32(sm):
     wl, wS = pair("mid6")
-    z_or, _, _ = orc.inv_sqrt_columns(wS)
+    z_or, _, _ = oracle_cached("inv_sqrt", "mid6", lambda: orc.inv_sqrt_columns(wS))
     S = sm.Bcsr(wS)
     P = sm.sm_build_pattern(S, 16)
     Z, _, iters, res, _ = sm.sm_inv_sqrt(S, P, "f32", max_iter=100, tol=1e-5)
@@ -56,7 +66,7 @@ def test_inv_sqrt_fp32(sm):
 def test_inv_sqrt_16bit(sm, x_dtype, kind):
     # doubled images up to 2 * 500 = 1000 rows: non-symmetric tcgen05 path (true products, MN-major B operand)
     wl, wS = pair(kind)
-    z_or, _, _ = orc.inv_sqrt_columns(wS)
+    z_or, _, _ = oracle_cached("inv_sqrt", kind, lambda: orc.inv_sqrt_columns(wS))
     S = sm.Bcsr(wS)
     P = sm.sm_build_pattern(S, 64)
     Z, _, iters, res, _ = sm.sm_inv_sqrt(S, P, x_dtype, max_iter=12, tol=0.0)
@@ -71,7 +81,7 @@ def test_inv_sqrt_16bit(sm, x_dtype, kind):
 def test_density_nonorth_matches_the_oracle(sm, x_dtype, lim, kind):
     wl, wS = pair(kind)
     mu = 0.05
-    p_or = orc.density_nonorth_columns(wl, wS, mu)
+    p_or = oracle_cached("nonorth%g" % mu, kind, lambda: orc.density_nonorth_columns(wl, wS, mu))
     A = sm.Bcsr(wl)
     Sd = sm.Bcsr(wS)
     P = sm.sm_build_pattern(A, 16)
@@ -107,7 +117,7 @@ def test_density_nonorth_16bit(sm, x_dtype, kind, val_dtype, lim):
     products by the non-symmetric update kernel without its identity term (umma_product), the sign of S^-1 H - mu I."""
     wl, wS = pair(kind)
     mu = 0.05
-    p_or = orc.density_nonorth_columns(wl, wS, mu)
+    p_or = oracle_cached("nonorth%g" % mu, kind, lambda: orc.density_nonorth_columns(wl, wS, mu))
     A = sm.Bcsr(wl, val_dtype=val_dtype)
     Sd = sm.Bcsr(wS, val_dtype=val_dtype)
     P = sm.sm_build_pattern(A, 64)

@@ -366,12 +366,19 @@ def test_not_converged_warning_and_odd_iteration_copy_back(sm):
 
 # ------------------------------------- full-size configs, bench.py's launch configuration, sampled columns
 
+_EXACT_CACHE = {}
+
+
 def sampled_errors(wl, P, plan, cols, max_iter, lapack=True, label=""):
     """(relF total vs exact sign, relF truncation, relF rounding vs NS-k, max-abs, |dTr|/rows) on the
     owned columns of the sample (raw D), plus the per-column min / median / max of the three relF figures.
     Truncation / rounding split: DESIGN.md reading A13.  Sample sizes: SURVEY 8(c) "Oracle cost / policy"."""
     dens = orc.density_columns_lapack if lapack else (lambda *a, **k: orc.density_columns(*a, n_threads=THREADS, **k))
-    d_or, st = dens(wl, cols=cols)
+    # the exact-sign reference of a (workload, sample) is shared by the tests that differ only in dtype / scale mode
+    key = (wl.n_blk, wl.nnzb, float(np.asarray(wl.vals[:64]).sum()), tuple(int(c) for c in cols), lapack)
+    if key not in _EXACT_CACHE:
+        _EXACT_CACHE[key] = dens(wl, cols=cols)
+    d_or, st = _EXACT_CACHE[key]
     order = P.order.cpu().numpy()
     pos = {int(c): k for k, c in enumerate(order)}
     sc = plan.scale.cpu().numpy()[[pos[int(c)] for c in cols]]
