@@ -221,7 +221,11 @@ int32_t sm_symmetrise(const sm_bcsr_t *A, const sm_pattern_t *P, int32_t r_dtype
  * chunks that fit ws_bytes; h_dim_pad is a HOST copy of P->dim_pad (needed to plan chunks).
  * d_dtype SM_F64 or SM_F32; trace is a device fp64 scalar; iters/residual/scale are [N] device
  * arrays.  ws >= sm_density_ws_bytes(P, x_dtype, max_chunk_elems) where max_chunk_elems bounds the
- * packed elements per chunk (>= max_dim_pad^2; P->packed_elems for a single chunk).  Asynchronous. */
+ * packed elements per chunk (>= max_dim_pad^2; P->packed_elems for a single chunk).  Asynchronous.
+ * With tol <= 0 the call enqueues kernels and memsets only (no host synchronisation; after the first call of a
+ * process nothing is allocated), so it can be captured into a CUDA graph and replayed on the same buffers
+ * (tests/test_gpu_parity.py::test_fixed_count_density_is_graph_capturable); tol > 0 reads one counter back every
+ * second step and cannot be captured. */
 int64_t sm_density_ws_bytes(const sm_bcsr_t *A, const sm_pattern_t *P, int32_t x_dtype,
                             int64_t max_chunk_elems);
 /* The same for sm_density_ex(..., sign_flags, ...) (sm_density_ws_bytes = sign_flags 0): the third-order iteration

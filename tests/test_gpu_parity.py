@@ -872,3 +872,36 @@ def test_order3_with_precision_schedule_and_flag_errors(sm):
     with pytest.raises(sm.SmError) as e:
         sm.sm_sign_ns(P, cols, col_off, n, P.packed_elems, "f64", X, 3, 0.0, flags=4)
     assert e.value.status == sm.SM_ERR_ARG
+
+
+# ------------------------------------------------------------------- CUDA graph capture of the fixed-count path
+
+@pytest.mark.parametrize("x_dtype,val_dtype,scale_mode", [("f64", "f64", "gershgorin"), ("bf16", "f32", "global"), ("f16", "f32", "global")])
+def test_fixed_count_density_is_graph_capturable(sm, x_dtype, val_dtype, scale_mode):
+    """With tol <= 0 sm_density enqueues only kernels and memsets on the caller's stream (no host synchronisation, no
+    allocation after the first call), so the whole path a1..a5 of a step can be captured once into a CUDA graph and
+    replayed: the replay reproduces the eager call bit for bit, also after the inputs changed in place."""
+    wl = make_config(0)
+    A = sm.Bcsr(wl, val_dtype=val_dtype)
+    P = sm.sm_build_pattern(A, 64 if x_dtype in ("bf16", "f16") else 16)
+    plan = sm.DensityPlan(A, P, x_dtype)
+    call = lambda: sm.sm_density(A, P, plan, 0.0, scale_mode, 12, 0.0, symmetrise=True)
+    call()                                       # warm-up: lazy one-time set-up happens outside the capture
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        with torch.cuda.graph(g, stream=s):
+            call()
+    for scale_h in (1.0, 0.97):                  # second round: H changed in place, same pattern
+        A.vals.mul_(scale_h)
+        call()
+        torch.cuda.synchronize()
+        D_eager, tr_eager, res_eager = plan.D.clone(), plan.trace.clone(), plan.residual.clone()
+        plan.D.zero_(); plan.trace.zero_(); plan.residual.zero_()
+        g.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(plan.D, D_eager) and torch.equal(plan.trace, tr_eager) and torch.equal(plan.residual, res_eager)
+    # sign(0.97 H) = sign(H): the replayed result is still the density of the workload (12 fixed steps: loose bound)
+    d_or, _ = orc.density_columns(wl, n_threads=THREADS)
+    assert np.isfinite(plan.D.cpu().numpy()).all() and abs(plan.trace.item() - orc.trace(wl, d_or)) <= 1e-2 * wl.n
