@@ -88,7 +88,8 @@ def issued_flops_per_step(dims, pad, k_eff, resident_pd=256):
     """Tensor-core FLOPs the 16-bit kernels ISSUE for one Newton-Schulz step of every submatrix (both products), with
     padding, the lower-triangle tile selection and the identity MMAs of the update product -- what goes against the
     hardware peak ("state both, never mix").  Mirrors the tile geometry of sign_umma.cu (128-row tiles,
-    columns up to the next multiple of 32 cut into equal tiles of <= 256) and of k_umma_resident (Pd <= 256)."""
+    columns up to the next multiple of 32 cut into equal tiles of <= 256, short last panel folded into columns) and of
+    k_umma_resident (Pd <= 256)."""
     total = 0.0
     for m, k in zip(dims.astype(np.int64), k_eff):
         m = int(m)
@@ -101,8 +102,13 @@ def issued_flops_per_step(dims, pad, k_eff, resident_pd=256):
             f *= 2                                      # both products issue the same shapes
         else:
             n32 = -(-m // 32) * 32
-            for tm in range(-(-m // 128)):
+            Tm = -(-m // 128)
+            fn = n32 - (Tm - 1) * 128               # folded geometry (sign_umma.cu, w_fold): a last panel of <= 64 rows
+            fn = fn if (Tm >= 2 and fn <= 64) else 0     # becomes fn extra columns of the other panels + its own square
+            for tm in range(Tm):
                 nc = min(n32, 128 * (tm + 1))
+                if fn:
+                    nc = 128 * (tm + 1) + fn if tm + 1 < Tm else fn
                 tn_cnt = -(-nc // 256)
                 nb = -(-(-(-nc // 32)) // tn_cnt) * 32
                 for tn in range(tn_cnt):

@@ -311,6 +311,8 @@ int32_t sm_density_from_sign(const sm_bcsr_t *A, const sm_pattern_t *P, int32_t 
  *                                            shared-memory staging, bulk stores; 3-stage operand ring)
  *   "umma.lt"       [SM_UMMA_LT]       0|1   with umma.epi = 1: iterates stored "128-lower" (nothing above the 128 x 128
  *                                            diagonal squares), the rest read through MN-major descriptors
+ *   "umma.fold"     [SM_UMMA_FOLD]     1|0   16-bit grouped symmetric tiles: a last 128-row panel of <= 64 rows is computed as extra
+ *                                            columns of the other panels and mirrored into place / as a row panel of its own
  *   "umma.dyn"      [SM_UMMA_DYN]      1|0   16-bit grouped tiles handed out by a global counter / dealt round robin
  *   "umma.rev"      [SM_UMMA_REV]      1|0   16-bit: the update product walks the tile table backwards / forwards
  *   "umma.stages"   [SM_UMMA_STAGES]   0|3|4 16-bit grouped tiles: depth of the operand ring (0 = by size)

@@ -79,6 +79,7 @@ template <int NCTA, bool MC = false, int NST = 0, int EPI = 0> struct UCfg {
 
 struct UTile {
   int32_t c, m, Pd, row0, n0, nt, kmax, lt, valid;
+  int32_t fb, fs;   // folded geometry: tile column (virtual index) v >= fb is column v + fs of the matrix (fb = INT_MAX: none)
   int64_t base;   // element offset of the submatrix in the packed buffer
 };
 
@@ -118,6 +119,7 @@ struct UArgs {
   // the update-type product scales its accumulator by out_scale (1; 2/3 for Z = 2/3 (Q + Q Q))
   float w_scale, out_scale;
   int32_t no_ident;          // update product without its "+ X" (identity MMAs skipped): a plain product O = X Wh (f2, Eq. 14)
+  int32_t fold;              // the tile table was built with the folded geometry (w_* functions)
 };
 
 // Tile geometry.  Only elements (r, c) with c <= r are computed, so tile row tm (rows tm*R ..
@@ -139,6 +141,34 @@ __host__ __device__ inline int32_t u_row_nb(int32_t m, int32_t R, int32_t tm) {
 __host__ __device__ inline int32_t u_tiles(int32_t m, int32_t R) {
   int32_t t = 0;
   for (int32_t tm = 0; tm < u_Tm(m, R); ++tm) t += u_row_tiles(m, R, tm);
+  return t;
+}
+
+// "Folded" geometry of the 128-row symmetric tiles (option "umma.fold", single-CTA tiles only).  When the last 128-row
+// panel holds at most 64 rows (m rounded up to 32), running it as a row panel costs an M = 128 MMA over ALL columns
+// for <= 64 useful rows -- at m = 414 (configs[2]'s median) 35 % of a product's MMA work and 30 % of its B-operand
+// loads for 7 % of its rows.  Instead the other panels take those rows as fn extra COLUMNS behind their own (virtual
+// column v of panel tm: v < (tm + 1) 128 is column v, else column F0 + v - (tm + 1) 128, F0 = first row of the last
+// panel), their mirrored stores fill the last rows, and the last panel keeps only its fn x fn diagonal square.
+// MMA work at m = 414: 1184 -> 896 column panels (-24 %), operand rows loaded 1824 -> 1600 (-12 %).
+__host__ __device__ inline int32_t w_fold(int32_t m) {
+  const int32_t Tm = u_Tm(m, UM);
+  if (Tm < 2) return 0;
+  const int32_t fn = ((m + 31) & ~31) - (Tm - 1) * UM;
+  return fn <= 64 ? fn : 0;
+}
+__host__ __device__ inline int32_t w_ncols(int32_t m, int32_t tm, int32_t fn) {
+  if (!fn) return u_ncols(m, UM, tm);
+  return tm + 1 < u_Tm(m, UM) ? (tm + 1) * UM + fn : fn;
+}
+__host__ __device__ inline int32_t w_row_tiles(int32_t m, int32_t tm, int32_t fn) { return (w_ncols(m, tm, fn) + UN - 1) / UN; }
+__host__ __device__ inline int32_t w_row_nb(int32_t m, int32_t tm, int32_t fn) {
+  const int32_t nc = w_ncols(m, tm, fn), Tn = (nc + UN - 1) / UN;
+  return (((nc + 31) / 32 + Tn - 1) / Tn) * 32;
+}
+__host__ __device__ inline int32_t w_tiles(int32_t m, int32_t fn) {
+  int32_t t = 0;
+  for (int32_t tm = 0; tm < u_Tm(m, UM); ++tm) t += w_row_tiles(m, tm, fn);
   return t;
 }
 
@@ -183,6 +213,11 @@ __device__ __forceinline__ UTile make_tile(const UArgs &a, const TileDesc &d) {
   u.c = d.c; u.m = d.m; u.Pd = d.Pd; u.base = d.base;
   u.row0 = d.row0; u.n0 = d.n0; u.nt = d.nt; u.lt = d.lt;
   u.kmax = u_n16(d.m);
+  u.fb = 0x7fffffff; u.fs = 0;
+  if (a.fold) {
+    const int32_t fn = w_fold(d.m), F0 = (u_Tm(d.m, UM) - 1) * UM;
+    if (fn && d.row0 < F0) { u.fb = d.row0 + UM; u.fs = F0 - u.fb; }
+  }
   int32_t act = 1;
   if (a.check_flags) {
     act = a.s.active[d.c];
@@ -192,7 +227,7 @@ __device__ __forceinline__ UTile make_tile(const UArgs &a, const TileDesc &d) {
   return u;
 }
 
-static __global__ void k_umma_build_tiles(int32_t n_cols, int32_t R, int32_t sym, int32_t skip_pd, const int32_t *__restrict__ cols,
+static __global__ void k_umma_build_tiles(int32_t n_cols, int32_t R, int32_t sym, int32_t fold, int32_t skip_pd, const int32_t *__restrict__ cols,
                                           const int32_t *__restrict__ dim, const int32_t *__restrict__ dim_pad,
                                           const int64_t *__restrict__ col_off,
                                           const int64_t *__restrict__ tile_ptr, TileDesc *__restrict__ tiles) {
@@ -210,6 +245,16 @@ static __global__ void k_umma_build_tiles(int32_t n_cols, int32_t R, int32_t sym
       const int32_t cnt = v_row_tiles(m, tm), nc = v_ncols(m, tm);
       for (int32_t tn = 0; tn < cnt; ++tn, ++lt, ++t) {
         d.row0 = tm * UM; d.n0 = tn * UN; d.nt = min(UN, nc - d.n0); d.lt = lt;
+        tiles[t] = d;
+      }
+    }
+  } else if (sym && fold && R == UM) {
+    const int32_t fn = w_fold(m), Tm = u_Tm(m, UM);
+    for (int32_t tm = 0; tm < Tm; ++tm) {
+      const int32_t cnt = w_row_tiles(m, tm, fn), nb = w_row_nb(m, tm, fn), nc = w_ncols(m, tm, fn);
+      const int32_t v0 = (fn && tm + 1 == Tm) ? tm * UM : 0;       // the last panel's square starts at its own first column
+      for (int32_t tn = 0; tn < cnt; ++tn, ++lt, ++t) {
+        d.row0 = tm * UM; d.n0 = v0 + tn * nb; d.nt = min(nb, v0 + nc - d.n0); d.lt = lt;
         tiles[t] = d;
       }
     }
@@ -535,7 +580,12 @@ k_umma_gemm(UArgs a, const __grid_constant__ CUtensorMap mapA, const __grid_cons
             // this CTA's half of the B rows, delivered into both CTAs at its place in the whole tile
             ptx::tma_bulk_g2s_mc(sb + h * b_bytes, Bg + chunk + (int64_t)brow0 * 128, b_bytes, full_bar(stage), (uint16_t)3);
           } else if (SYM) {
-            ptx::tma_bulk_g2s(sb, Bg + chunk + (int64_t)brow0 * 128, b_bytes, full_bar(stage));
+            // rows [brow0, brow0 + b_cnt) of the tile's (virtual) columns: those from u.fb on are the folded rows
+            const int32_t n1 = max(0, min(b_cnt, u.fb - brow0));
+            if (n1) ptx::tma_bulk_g2s(sb, Bg + chunk + (int64_t)brow0 * 128, (uint32_t)n1 * 128u, full_bar(stage));
+            if (n1 < b_cnt)
+              ptx::tma_bulk_g2s(sb + (uint32_t)n1 * 128u, Bg + chunk + (int64_t)(max(brow0, u.fb) + u.fs) * 128,
+                                (uint32_t)(b_cnt - n1) * 128u, full_bar(stage));
           } else {
             for (int32_t j = 0; j < n_atoms; ++j)    // rows k of chunk-column (atom0 + j): 64 x 128 B
               ptx::tma_bulk_g2s(sb + (uint32_t)j * 8192u,
@@ -661,13 +711,22 @@ k_umma_gemm(UArgs a, const __grid_constant__ CUtensorMap mapA, const __grid_cons
           if (p2 && !a.no_ident && !SM_DBG(a, 2)) {
             // "+ X": the A chunk in this stage holds X[rows, 64 kc .. 64 kc + 63]; add it to the accumulator
             // columns [lo, hi) of the tile that it covers (B = identity slice, K-major)
-            const int32_t lo = max(kc * UK, u.n0), hi = min(kc * UK + UK, u.n0 + u.nt);
-            if (lo < hi) {
-              const uint32_t idesc2 = ptx::make_idesc_f16(BF16, PAIR ? 2 * UM : UM, (uint32_t)(hi - lo), false);
-              const uint64_t idd = ptx::make_sw128_kmajor_desc(ident + ident_row(PAIR, lo - kc * UK, hi - lo) * 128u);
+            // (tile columns are virtual: [u.n0, min(u.n0 + u.nt, u.fb)) are columns of the same index, the rest -- the
+            // folded rows of the last panel -- are columns v + u.fs)
+            const int32_t vend = u.n0 + u.nt;
 #pragma unroll
-              for (int ks = 0; ks < UK / 16; ++ks)
-                mma(d_tmem + (uint32_t)(lo - u.n0), adesc + (uint64_t)(2 * ks), idd + (uint64_t)(2 * ks), idesc2, 1u);
+            for (int part = 0; part < 2; ++part) {
+              const int32_t g0 = part ? max(u.n0, u.fb) + u.fs : u.n0, g1 = part ? vend + u.fs : min(vend, u.fb);
+              if (part && vend <= u.fb) break;
+              const int32_t lo = max(kc * UK, g0), hi = min(kc * UK + UK, g1);
+              if (lo < hi) {
+                const uint32_t idesc2 = ptx::make_idesc_f16(BF16, PAIR ? 2 * UM : UM, (uint32_t)(hi - lo), false);
+                const uint64_t idd = ptx::make_sw128_kmajor_desc(ident + ident_row(PAIR, lo - kc * UK, hi - lo) * 128u);
+                const uint32_t acol = (uint32_t)(lo - (part ? u.fs : 0) - u.n0);
+#pragma unroll
+                for (int ks = 0; ks < UK / 16; ++ks)
+                  mma(d_tmem + acol, adesc + (uint64_t)(2 * ks), idd + (uint64_t)(2 * ks), idesc2, 1u);
+              }
             }
           }
           // frees the smem slot (in both CTAs of a pair) when these MMAs finish
@@ -902,8 +961,13 @@ k_umma_gemm(UArgs a, const __grid_constant__ CUtensorMap mapA, const __grid_cons
       if (R0 < u.Pd && !SM_DBG(a, 8)) {
         const uint32_t r7 = (uint32_t)lane & 7u;                 // r & 7 (R0 is a multiple of 32)
         for (int bi = sub; bi < nblk; bi += NSUB) {
-          const int32_t C0 = u.n0 + bi * 32;
-          if (SYM ? (C0 > R0) : (C0 >= u.Pd)) break;             // above the diagonal / past the padded dimension
+          const int32_t vc = u.n0 + bi * 32;                     // virtual column; from u.fb on: a folded row of the last panel
+          const bool fcol = vc >= u.fb;
+          const int32_t C0 = fcol ? vc + u.fs : vc;
+          if (SYM ? (!fcol && C0 > R0) : (C0 >= u.Pd)) {         // above the diagonal / past the padded dimension
+            if (SYM && u.fb != 0x7fffffff) continue;             // folded columns may still follow
+            break;
+          }
           uint32_t v[32];
           ptx::tmem_ld16(taddr + (uint32_t)(bi * 32), *reinterpret_cast<uint32_t(*)[16]>(&v[0]));
           ptx::tmem_ld16(taddr + (uint32_t)(bi * 32 + 16), *reinterpret_cast<uint32_t(*)[16]>(&v[16]));
@@ -1047,14 +1111,18 @@ static __global__ void k_fused_post(int32_t n_cols, const int32_t *__restrict__ 
   }
 }
 
-static __global__ void k_umma_tilecounts(int32_t n_cols, int32_t R, int32_t sym, int32_t parts_per_tile, int32_t skip_pd,
+static __global__ void k_umma_tilecounts(int32_t n_cols, int32_t R, int32_t sym, int32_t fold, int32_t parts_per_tile, int32_t skip_pd,
                                          const int32_t *__restrict__ cols, const int32_t *__restrict__ dim,
                                          const int32_t *__restrict__ dim_pad, int64_t *__restrict__ tiles,
                                          int32_t *__restrict__ n_parts) {
   int32_t c = blockIdx.x * blockDim.x + threadIdx.x;
   if (c >= n_cols) return;
   int32_t i = cols ? cols[c] : c;
-  int32_t nt = dim_pad[i] <= skip_pd ? 0 : (sym == 2 ? v_tiles(dim[i]) : sym ? u_tiles(dim[i], R) : f_tiles(dim_pad[i], R));
+  int32_t nt = dim_pad[i] <= skip_pd ? 0
+               : sym == 2            ? v_tiles(dim[i])
+               : (sym && fold && R == UM) ? w_tiles(dim[i], w_fold(dim[i]))
+               : sym                 ? u_tiles(dim[i], R)
+                                     : f_tiles(dim_pad[i], R);
   tiles[c] = nt;
   n_parts[c] = nt * parts_per_tile;
 }
@@ -1122,7 +1190,8 @@ static UmmaWs umma_layout(void *ws, int64_t ws_bytes, const sm_pattern_t *P, int
   // sized for whichever variant sign_umma picks (the query does not know tol): per-phase launches with
   // the selected NCTA / SYM, or the fused kernel (CTA pairs, SYM)
   const int32_t ncta = umma_ncta();
-  const int32_t t_sel = sym == 2 ? v_tiles(P->max_dim) : sym ? u_tiles(P->max_dim, UM * ncta) : f_tiles(P->max_dim_pad, UM * ncta);
+  // (the folded geometry can need one tile more than the unfolded one at a smaller dimension: + 1)
+  const int32_t t_sel = sym == 2 ? v_tiles(P->max_dim) : sym ? u_tiles(P->max_dim, UM * ncta) + 1 : f_tiles(P->max_dim_pad, UM * ncta);
   const int32_t t_fused = u_tiles(P->max_dim, UM * 2);
   const int32_t max_tiles = t_sel > t_fused ? t_sel : t_fused;
   w.parts_per_col = (t_sel * ncta > t_fused * 2 ? t_sel * ncta : t_fused * 2) * EPI_WARPS;
@@ -1304,11 +1373,13 @@ int32_t sign_umma(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, co
   SignState s{w.active, w.last, w.n_still, w.partial, w.parts_per_col};
   k_sign_init_grouped<<<nb, 256, 0, st>>>(n_cols, cols, P->dim_pad, res_pd, w.active, w.last, iters, residual);
   SM_LAUNCHED();
-  k_umma_tilecounts<<<nb, 256, 0, st>>>(n_cols, R, sym, EPI_WARPS * ncta, res_pd, cols, P->dim, P->dim_pad, w.tile_ptr,
+  // folded geometry of the symmetric single-CTA tiles (option "umma.fold"; see w_fold)
+  const int32_t fold = (sym == 1 && ncta == 1 && opt(OPT_UMMA_FOLD) != 0) ? 1 : 0;
+  k_umma_tilecounts<<<nb, 256, 0, st>>>(n_cols, R, sym, fold, EPI_WARPS * ncta, res_pd, cols, P->dim, P->dim_pad, w.tile_ptr,
                                         w.n_parts);
   SM_LAUNCHED();
   { int32_t rc = exclusive_scan_i64(n_cols, w.tile_ptr, w.tile_ptr, st); if (rc != SM_OK) return rc; }
-  k_umma_build_tiles<<<nb, 256, 0, st>>>(n_cols, R, sym, res_pd, cols, P->dim, P->dim_pad, col_off, w.tile_ptr, w.tiles);
+  k_umma_build_tiles<<<nb, 256, 0, st>>>(n_cols, R, sym, fold, res_pd, cols, P->dim, P->dim_pad, col_off, w.tile_ptr, w.tiles);
   SM_LAUNCHED();
   // Y and the alternate X buffer start as zeros so that padding never holds NaN/Inf bit patterns.
   SM_CUDA(cudaMemsetAsync(w.Y, 0, packed_elems * 2, st));
@@ -1370,6 +1441,7 @@ int32_t sign_umma(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, co
     SM_CUDA(cudaMemsetAsync(w.done, 0, sizeof(int32_t) * n_done, st));
     UArgs a{cols, col_off, P->dim, P->dim_pad, w.tile_ptr, w.tiles, n_cols, 0, X, w.Y, w.X2, s, w.err, 0, w.counters,
             2 * max_iter, w.done, umma_dbg(), 0, 0, 0, -0.5f, 1.f};
+    a.fold = fold;
     int32_t rc = sym == 2 ? launch_umma_t<0, 1, true, false, 0, false, true, 1>(bf16, a, maps[0], n_sm, st)
                           : launch_umma_t<0, 1, true, false, 0, false, true>(bf16, a, maps[0], n_sm, st);
     if (rc != SM_OK) return rc;
@@ -1399,6 +1471,7 @@ int32_t sign_umma(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, co
     // of a submatrix (fixed counts: the last step; convergence mode: per submatrix, s.last)
     const int32_t lt = (sym == 2 && !o3 && opt(OPT_UMMA_LT) != 0) ? 1 : 0;
     a.lt_in = lt && k > 0; a.lt_out = lt;
+    a.fold = fold;
     int32_t launch = nper * k;                 // launches alternate their walk through the tile table (option umma.rev)
     a.rev = o3 ? (rev_on & launch) & 1 : 0;
     a.counter = dyn ? w.counters + launch : nullptr;
@@ -1468,10 +1541,10 @@ int32_t umma_product(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols,
   SignState s{w.active, w.last, w.n_still, w.partial, w.parts_per_col};
   k_sign_init_grouped<<<nb, 256, 0, st>>>(n_cols, cols, P->dim_pad, 0, w.active, w.last, nullptr, nullptr);
   SM_LAUNCHED();
-  k_umma_tilecounts<<<nb, 256, 0, st>>>(n_cols, R, sym, EPI_WARPS * ncta, 0, cols, P->dim, P->dim_pad, w.tile_ptr, w.n_parts);
+  k_umma_tilecounts<<<nb, 256, 0, st>>>(n_cols, R, sym, 0, EPI_WARPS * ncta, 0, cols, P->dim, P->dim_pad, w.tile_ptr, w.n_parts);
   SM_LAUNCHED();
   { int32_t rc = exclusive_scan_i64(n_cols, w.tile_ptr, w.tile_ptr, st); if (rc != SM_OK) return rc; }
-  k_umma_build_tiles<<<nb, 256, 0, st>>>(n_cols, R, sym, 0, cols, P->dim, P->dim_pad, col_off, w.tile_ptr, w.tiles);
+  k_umma_build_tiles<<<nb, 256, 0, st>>>(n_cols, R, sym, 0, 0, cols, P->dim, P->dim_pad, col_off, w.tile_ptr, w.tiles);
   SM_LAUNCHED();
   SM_CUDA(cudaMemsetAsync(O, 0, packed_elems * 2, st));       // padding of the result reads as zeros
   UArgs a{cols, col_off, P->dim, P->dim_pad, w.tile_ptr, w.tiles, n_cols, 0, A, B, O, s, w.err, 0, nullptr, 0, nullptr, 0, 0, 0, 0,

@@ -12,6 +12,7 @@ environment forces (each in its own process: the selection is read once per proc
   SM_UMMA_FUSED=1|0  one launch runs every step of a submatrix (k_umma_fused) / one launch per product
   SM_UMMA_RESIDENT=1|0  submatrices with Pd <= 256 iterate inside one SM (k_umma_resident) / grouped tiles for all
   SM_UMMA_LT=0|1     grouped tiles: iterates stored lower-triangular, the upper part read through MN-major descriptors
+  SM_UMMA_FOLD=1|0   single-CTA symmetric tiles: a short last row panel is computed as extra columns of the other panels / as a panel
   SM_F64_SIMT=0|1    DMMA tensor tiles (default) / DFMA register tiles
 The two-CTA and fused variants exist only in a -DSM_MEASURE build of the library (build.py --measure); their cases
 are skipped on the default build.
@@ -81,6 +82,10 @@ CASES = [
     # env, x_dtype, pad, (n_mol, b, n_occ, cutoff), steps, tolerance (max-abs vs the NS-k polynomial), exact symmetry, build
     ({"SM_UMMA_NCTA": "1", "SM_UMMA_SYM": "1"}, "bf16", 64, (90, 23, 4, 5.0), 3, 2.5e-2, True, None),
     ({"SM_UMMA_DYN": "0"}, "f16", 64, (90, 23, 4, 5.0), 3, 3e-3, True, None),
+    ({"SM_UMMA_FOLD": "0"}, "f16", 64, (90, 23, 4, 5.0), 3, 3e-3, True, None),
+    ({"SM_UMMA_FOLD": "0", "SM_UMMA_RESIDENT": "0"}, "bf16", 64, (300, 6, 3, 6.0), 3, 2.5e-2, True, None),
+    ({"SM_UMMA_FOLD": "1", "SM_UMMA_RESIDENT": "0"}, "f16", 64, (300, 6, 3, 6.0), 5, 3e-3, True, None),
+    ({"SM_UMMA_FOLD": "1", "SM_UMMA_STREAM": "1", "SM_UMMA_RESIDENT": "0"}, "f16", 64, (300, 6, 3, 6.0), 4, 3e-3, True, None),
     ({"SM_UMMA_STREAM": "1"}, "f16", 64, (90, 23, 4, 5.0), 4, 3e-3, True, None),
     ({"SM_UMMA_SYM": "0"}, "f16", 64, (90, 23, 4, 5.0), 3, 3e-3, False, None),
     ({"SM_UMMA_SYM": "0"}, "bf16", 64, (300, 6, 3, 6.0), 3, 2.5e-2, False, None),
@@ -179,6 +184,9 @@ def test_symmetric_tile_variants_are_bit_identical():
     seen = {}
     for env in SYM_VARIANTS + (SYM_VARIANTS_MEASURE if _measure_build() else []):
         e = dict(os.environ)
+        # the folded geometry (default) takes the last rows of a submatrix from the TRANSPOSED tile elements: equal in
+        # exact arithmetic, not to the bit (X Wh is symmetric only because X and Wh commute); it has its own tests
+        e["SM_UMMA_FOLD"] = "0"
         e.update(env)
         p = subprocess.run([sys.executable, "-c", HASH_SNIPPET.format(root=ROOT)], env=e, capture_output=True,
                            text=True, timeout=600, cwd=ROOT)
