@@ -237,6 +237,8 @@ def run_reference(args, cfg, cfg_run):
     wl = make_config(args.config)
     cores = os.cpu_count() or 1
     n_sample = oracle_sample_size(args.config, cores)
+    if args.steps > 10:                  # keep the whole run within a few minutes: ~10 default samples of CPU work in total
+        n_sample = max(cores, n_sample * 10 // args.steps)
     for w in range(args.warmup):
         oracle_sample(wl, cfg_run, max(1, n_sample // 8), 7000 + w, cores)
     total_t, total_f, total_cols = 0.0, 0.0, 0
