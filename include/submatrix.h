@@ -321,6 +321,8 @@ int32_t sm_density_from_sign(const sm_bcsr_t *A, const sm_pattern_t *P, int32_t 
  *   "f64.tile"      [SM_F64_TILE]      0|64|128  fp64 tensor-core tile edge (0: 64 when the largest submatrix is <= 384, else 128)
  *   "f32.sym"       [SM_F32_SYM]       1|0   fp32: lower-triangle 64 x 64 FFMA tiles with 8 x 8 register blocks and mirrored
  *                                            stores (exactly symmetric iterates) / all tiles with 4 x 4 blocks
+ *   "gather.lean"   [SM_GATHER_LEAN]   1|0   sm_gather, 16-bit X, blocks >= 4 wide: per-CTA tables of the runs' blocks / blocks resolved
+ *                                            per run (bit-identical)
  *   "gather.tma"    [SM_GATHER_TMA]    0|1   sm_gather, 16-bit X: element-wise kernel / source-driven kernel staged through
  *                                            shared memory with bulk TMA stores (bit-identical; measured slower)
  * A library built with -DSM_MEASURE (build.py --measure; sm_build_info() & 1) additionally has the measured-slower

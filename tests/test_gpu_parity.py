@@ -690,6 +690,46 @@ def test_staged_gather_is_bit_identical(sm):
         sm.set_option("gather.tma", 0)
 
 
+def test_table_driven_gather_is_bit_identical_and_exact(sm):
+    # the table-driven walk of k_gather (default for 16-bit images when every block of N(i) is >= 4 wide; option
+    # "gather.lean") against the walk that resolves the blocks per run: same fp32 arithmetic, one rounding -> identical
+    # images; two-block (widths >= 8) and three-block (widths 4..7) variants, mixed widths, narrow blocks (falls back),
+    # fp64 and fp32 H, mu on the diagonal, listed subsets; and against the oracle's gather within one 16-bit rounding
+    cases = [make_config(0), make_workload(90, 23, 4, 5.0, seed=33),
+             make_workload(60, np.array([8, 9, 23, 17, 12] * 12), np.array([3, 4, 4, 5, 2] * 12), 6.0, seed=13),
+             make_workload(60, np.array([4, 5, 23, 7, 6] * 12), np.array([2, 2, 4, 3, 3] * 12), 6.0, seed=15),
+             make_workload(80, np.array([4, 4, 9, 4, 16, 5, 4, 8] * 10), np.array([2, 2, 4, 2, 3, 2, 1, 3] * 10), 7.0, seed=16),
+             ragged_workload(), make_config(1)]
+    try:
+        for wi, wl in enumerate(cases):
+            for val_dtype in ("f64", "f32"):
+                A = sm.Bcsr(wl, val_dtype=val_dtype)
+                P = sm.sm_build_pattern(A, 64)
+                Ph = sm.pattern_to_host(P)
+                lists = [P.order] + ([np.array([5, 0, 17, 3], np.int32)] if wl.n_blk > 17 else [])
+                for cols_in in lists:
+                    cols, col_off, n = sm.sm_plan_columns(P, cols_in)
+                    for x_dtype, eps, mode, mu in (("bf16", 2.0 ** -8, "gershgorin", 0.0), ("f16", 2.0 ** -11, "none", 0.13)):
+                        imgs = []
+                        for o in (0, 1):
+                            sm.set_option("gather.lean", o)
+                            X, sc = sm.sm_gather(A, P, cols, col_off, n, mu, mode, x_dtype)
+                            torch.cuda.synchronize()
+                            imgs.append(X.view(torch.int16).clone())
+                        assert torch.equal(imgs[0], imgs[1]), (wi, val_dtype, x_dtype)
+                        if wi in (2, 3) and cols_in is P.order and val_dtype == "f64" and mode == "gershgorin":
+                            order, off = P.order.cpu().numpy(), col_off.cpu().numpy()
+                            for pos in (0, n // 2, n - 1):
+                                i = int(order[pos])
+                                T = orc.gather(wl, i, mu)
+                                mm = T.shape[0]
+                                x = unpack(X, Ph, i, x_dtype, col_off=off, pos=pos)
+                                assert np.abs(x[:mm, :mm] - T / orc.gershgorin(T)).max() <= eps * 1.01
+                                assert not x[mm:].any() and not x[:, mm:].any()
+    finally:
+        sm.set_option("gather.lean", 1)
+
+
 def test_fixed_count_divergence_is_reported(sm):
     # a spectral scale below rho / sqrt(3) makes Newton-Schulz diverge; in fixed-count mode (tol <= 0) sm_sign_status
     # reports it (non-finite or > 1 residual) instead of answering SM_OK (SM_SCALE_GLOBAL is an estimate)
