@@ -50,7 +50,7 @@ k_global_spmv(const int32_t *__restrict__ blk, const int32_t *__restrict__ rp, c
               const int64_t *__restrict__ vp, const TA *__restrict__ vals, double mu,
               const int64_t *__restrict__ voff, const double *__restrict__ v, const double *__restrict__ scal,
               double *__restrict__ y, double *__restrict__ part) {
-  extern __shared__ double sm_y[];               // [SPMV_WARPS][bi], bi <= GLOBAL_MAX_BLK
+  extern __shared__ double sm_y[];               // [SPMV_WARPS][slots][rps] <= [SPMV_WARPS][GLOBAL_MAX_BLK]
   const int32_t i = blockIdx.x, bi = blk[i];
   if (bi > GLOBAL_MAX_BLK) {                     // unsupported block size: poison the estimate, the caller keeps Gershgorin
     if (threadIdx.x == 0) part[i] = -1.0;
@@ -58,19 +58,26 @@ k_global_spmv(const int32_t *__restrict__ blk, const int32_t *__restrict__ rp, c
   }
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   const double inv = scal[0];
-  double *mine = sm_y + (size_t)wid * bi;
-  for (int32_t r = lane; r < bi; r += 32) mine[r] = 0.0;
+  // Small blocks (round 2): with a lane per row a 6 x 6 block keeps 6 of 32 lanes busy (configs[3]: 75 us per step for 45 MB).
+  // A warp is cut into `slots` groups of rps = 2^k >= bi lanes; each group takes its own stored block, so a warp walks `slots`
+  // blocks at once (6-wide blocks: 4 groups of 8 lanes, 24 of 32 lanes busy).  Every (warp, slot) keeps its own partial rows;
+  // they are added in a fixed order at the end: deterministic.  bi > 16: one slot, the walk of round 1.
+  int32_t rps = 32;
+  while (rps >= 2 * bi && rps > 1) rps >>= 1;
+  const int32_t slots = 32 / rps, slot = lane / rps, row = lane - slot * rps;
+  double *mine = sm_y + ((size_t)wid * slots + slot) * (bi > 32 ? bi : rps);
+  for (int32_t r = row; r < bi; r += rps) mine[r] = 0.0;
   __syncwarp();
-  for (int32_t p = rp[i] + wid; p < rp[i + 1]; p += SPMV_WARPS) {
+  for (int32_t p = rp[i] + wid * slots + slot; p < rp[i + 1]; p += SPMV_WARPS * slots) {
     const int32_t j = ci[p], bj = blk[j];
     const TA *blkp = vals + vp[p];
     const double *vj = v + voff[j];
-    for (int32_t r = lane; r < bi; r += 32) {            // a lane owns a row: no shuffles, fixed summation order
-      const TA *row = blkp + (int64_t)r * bj;
+    for (int32_t r = row; r < bi; r += rps) {              // a lane owns a row: no shuffles, fixed summation order
+      const TA *rowp = blkp + (int64_t)r * bj;
       double s = 0.0;
 #pragma unroll 8
       for (int32_t c = 0; c < bj; ++c) {
-        double a = to_double<TA>(__ldg(row + c));
+        double a = to_double<TA>(__ldg(rowp + c));
         if (j == i && c == r) a -= mu;
         s = fma(a, vj[c] * inv, s);
       }
@@ -79,9 +86,10 @@ k_global_spmv(const int32_t *__restrict__ blk, const int32_t *__restrict__ rp, c
   }
   __syncthreads();
   double sq = 0.0;
+  const int32_t stride = bi > 32 ? bi : rps, nparts = SPMV_WARPS * slots;
   for (int32_t r = threadIdx.x; r < bi; r += blockDim.x) {
     double t = 0.0;
-    for (int w = 0; w < SPMV_WARPS; ++w) t += sm_y[(size_t)w * bi + r];
+    for (int w = 0; w < nparts; ++w) t += sm_y[(size_t)w * stride + r];
     y[voff[i] + r] = t;
     sq += t * t;
   }
