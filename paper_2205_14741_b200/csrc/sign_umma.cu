@@ -1127,6 +1127,40 @@ static __global__ void k_umma_tilecounts(int32_t n_cols, int32_t R, int32_t sym,
   n_parts[c] = nt * parts_per_tile;
 }
 
+// What the symmetric single-CTA tiles never write of the two scratch images of a grouped submatrix, zeroed once per call
+// instead of clearing both buffers whole (2 x 1.26 GB at configs[2]: 0.5 ms per call; at configs[3] 2 x 0.73 GB for the
+// 229 submatrices that are not resident).  The epilogues write every element (r < Pd, c < n32), n32 = m rounded up to 32
+// (lower blocks directly, upper ones mirrored) -- except, with the folded geometry, the rows >= n32 left of the last
+// panel's square.  Rows [n32, Pd) are read as A-operand rows and columns [n32, Pd) travel with copy-back: both must be 0.
+// One CTA per listed column; in the image a row range of a 64-column chunk is contiguous.
+static __global__ void __launch_bounds__(256)
+k_zero_padding(int32_t n_cols, const int32_t *__restrict__ cols, const int32_t *__restrict__ dim,
+               const int32_t *__restrict__ dim_pad, const int64_t *__restrict__ col_off, int32_t skip_pd,
+               uint16_t *__restrict__ B0, uint16_t *__restrict__ B1) {
+  const int32_t c = blockIdx.x, i = cols ? cols[c] : c;
+  const int32_t m = dim[i], Pd = dim_pad[i], n32 = (m + 31) & ~31;
+  if (Pd <= skip_pd || n32 >= Pd) return;
+  const uint4 z = make_uint4(0u, 0u, 0u, 0u);
+  const int32_t pr = Pd - n32;                                   // padding rows = padding columns
+#pragma unroll
+  for (int b = 0; b < 2; ++b) {
+    uint16_t *img = (b ? B1 : B0) + col_off[c];
+    // rows [n32, Pd) of every chunk: pr x 128 B contiguous
+    const int32_t per = pr * 8;                                  // 16-byte units per chunk
+    for (int32_t e = threadIdx.x; e < (Pd >> 6) * per; e += blockDim.x) {
+      const int32_t ch = e / per, u = e - ch * per;
+      reinterpret_cast<uint4 *>(img + (int64_t)ch * Pd * 64 + (int64_t)n32 * 64)[u] = z;
+    }
+    // columns [n32, Pd) of rows [0, n32): 16-byte units (n32 & 63) / 8 .. 7 of the last chunk, at their swizzled places
+    const int32_t u0 = (n32 & 63) >> 3, nu = 8 - u0;
+    uint16_t *last = img + (int64_t)((Pd >> 6) - 1) * Pd * 64;
+    for (int32_t e = threadIdx.x; e < n32 * nu; e += blockDim.x) {
+      const int32_t r = e / nu, u = u0 + (e - r * nu);
+      reinterpret_cast<uint4 *>(last + (int64_t)r * 64)[u ^ (r & 7)] = z;
+    }
+  }
+}
+
 // iters / residual of the columns the resident kernel does not take start at zero; its own are written by it
 static __global__ void k_sign_init_grouped(int32_t n_cols, const int32_t *__restrict__ cols,
                                            const int32_t *__restrict__ dim_pad, int32_t skip_pd, int32_t *active,
@@ -1381,9 +1415,16 @@ int32_t sign_umma(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, co
   { int32_t rc = exclusive_scan_i64(n_cols, w.tile_ptr, w.tile_ptr, st); if (rc != SM_OK) return rc; }
   k_umma_build_tiles<<<nb, 256, 0, st>>>(n_cols, R, sym, fold, res_pd, cols, P->dim, P->dim_pad, col_off, w.tile_ptr, w.tiles);
   SM_LAUNCHED();
-  // Y and the alternate X buffer start as zeros so that padding never holds NaN/Inf bit patterns.
-  SM_CUDA(cudaMemsetAsync(w.Y, 0, packed_elems * 2, st));
-  SM_CUDA(cudaMemsetAsync(w.X2, 0, packed_elems * 2, st));
+  // Y and the alternate X buffer: what the kernels read or copy back without ever writing it must be zero (and never a
+  // NaN/Inf bit pattern).  The symmetric single-CTA tiles leave only padding rows / columns unwritten (k_zero_padding);
+  // the other variants get both buffers cleared whole.
+  if (sym == 1 && ncta == 1) {
+    k_zero_padding<<<n_cols, 256, 0, st>>>(n_cols, cols, P->dim, P->dim_pad, col_off, res_pd, (uint16_t *)w.Y, (uint16_t *)w.X2);
+    SM_LAUNCHED();
+  } else {
+    SM_CUDA(cudaMemsetAsync(w.Y, 0, packed_elems * 2, st));
+    SM_CUDA(cudaMemsetAsync(w.X2, 0, packed_elems * 2, st));
+  }
 #ifdef SM_MEASURE
   if (fused) {
     // fixed iteration count: one launch runs every step of every submatrix (k_umma_fused)

@@ -945,3 +945,36 @@ def test_fixed_count_density_is_graph_capturable(sm, x_dtype, val_dtype, scale_m
     # sign(0.97 H) = sign(H): the replayed result is still the density of the workload (12 fixed steps: loose bound)
     d_or, _ = orc.density_columns(wl, n_threads=THREADS)
     assert np.isfinite(plan.D.cpu().numpy()).all() and abs(plan.trace.item() - orc.trace(wl, d_or)) <= 1e-2 * wl.n
+
+
+@pytest.mark.parametrize("x_dtype", ["bf16", "f16"])
+def test_workspace_contents_do_not_matter(sm, x_dtype):
+    """The scratch images of the grouped kernels are not cleared whole: only what the tiles never write but read or copy
+    back (padding rows and columns) is zeroed per call.  A workspace full of NaN bit patterns (0xFF bytes) must give the
+    bits of a zeroed one: every size of the tile-boundary sweep, odd and even step counts (result copied back from the
+    scratch image or not), Newton-Schulz and the third-order iteration, convergence mode."""
+    ms = np.array(SWEEP_M, dtype=np.int32)
+    wl = make_workload(len(ms), ms, np.maximum(1, ms // 3), 0.0, seed=91)
+    A = sm.Bcsr(wl, val_dtype="f32")
+    P = sm.sm_build_pattern(A, 64)
+    Ph = sm.pattern_to_host(P)
+    cols, col_off, n = sm.sm_plan_columns(P, P.order)
+    X0, _ = sm.sm_gather(A, P, cols, col_off, n, 0.0, "gershgorin", x_dtype)
+    nbytes = max(sm.sm_sign_ws_bytes(P, n, P.packed_elems, x_dtype, f) for f in (0, sm.SM_SIGN_ORDER3))
+    for k, tol, flags in ((3, 0.0, 0), (4, 0.0, 0), (3, 0.0, sm.SM_SIGN_ORDER3), (2, 0.0, sm.SM_SIGN_ORDER3), (9, 0.05, 0)):
+        out = []
+        for fill in (0, 255):
+            ws = torch.full((nbytes,), fill, dtype=torch.uint8, device="cuda")
+            X = X0.clone()
+            it, res = sm.sm_sign_ns(P, cols, col_off, n, P.packed_elems, x_dtype, X, k, tol, ws=ws, flags=flags)
+            torch.cuda.synchronize()
+            out.append((X.view(torch.int16).clone(), it.clone(), res.clone()))
+        assert torch.equal(out[0][0], out[1][0]) and torch.equal(out[0][1], out[1][1]) and torch.equal(out[0][2], out[1][2]), (k, tol, flags)
+        assert bool(torch.isfinite(out[1][0].view(torch.bfloat16 if x_dtype == "bf16" else torch.float16).float()).all())
+        # padding of every image is zero
+        off = col_off.cpu().numpy()
+        order = P.order.cpu().numpy()
+        for pos in range(0, n, 5):
+            i = int(order[pos]); m = int(Ph.dim[i])
+            x = unpack(out[1][0].view(torch.bfloat16 if x_dtype == "bf16" else torch.float16), Ph, i, x_dtype, col_off=off, pos=pos)
+            assert not x[m:].any() and not x[:, m:].any(), (k, flags, m)
