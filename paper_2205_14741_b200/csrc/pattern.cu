@@ -130,14 +130,31 @@ __global__ void k_tmap(const int32_t *__restrict__ rp, const int32_t *__restrict
 // order: rank of i under the key (dim_pad descending, id ascending), by counting.  One CTA per
 // group of block columns; O(N^2 / threads) integer compares, once per geometry.
 __global__ void k_order(int32_t n, const int32_t *__restrict__ dim_pad, int32_t *__restrict__ order) {
-  int32_t i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n) return;
-  int32_t key = dim_pad[i], rank = 0;
-  for (int32_t j = 0; j < n; ++j) {
-    int32_t kj = __ldg(dim_pad + j);
-    rank += (kj > key) || (kj == key && j < i);
+  // eight lanes share one i: lane s counts the keys of every eighth vector of four (n threads alone left most of the
+  // GPU idle: 169 us at n = 10 000), the partial ranks are added by shuffles
+  const int32_t i = (blockIdx.x * blockDim.x + threadIdx.x) >> 3, s = threadIdx.x & 7;
+  const bool live = i < n;
+  const int32_t key = live ? dim_pad[i] : 0;
+  int32_t rank = 0;
+  // keys four at a time (cudaMalloc'd arrays are 16-byte aligned); j < i decides ties
+  const int32_t n4 = ((reinterpret_cast<uintptr_t>(dim_pad) & 15) == 0) ? (n & ~3) : 0;
+  if (live) {
+    for (int32_t j = 4 * s; j < n4; j += 32) {
+      const int4 k4 = __ldg(reinterpret_cast<const int4 *>(dim_pad + j));
+      rank += (k4.x > key) || (k4.x == key && j < i);
+      rank += (k4.y > key) || (k4.y == key && j + 1 < i);
+      rank += (k4.z > key) || (k4.z == key && j + 2 < i);
+      rank += (k4.w > key) || (k4.w == key && j + 3 < i);
+    }
+    for (int32_t j = n4 + s; j < n; j += 8) {
+      const int32_t kj = __ldg(dim_pad + j);
+      rank += (kj > key) || (kj == key && j < i);
+    }
   }
-  order[rank] = i;
+  rank += __shfl_xor_sync(0xffffffffu, rank, 1);
+  rank += __shfl_xor_sync(0xffffffffu, rank, 2);
+  rank += __shfl_xor_sync(0xffffffffu, rank, 4);
+  if (live && s == 0) order[rank] = i;
 }
 
 __global__ void k_plan_columns(const int32_t *__restrict__ cols, int32_t n_cols,
@@ -211,7 +228,7 @@ extern "C" int32_t sm_build_pattern(const sm_bcsr_t *A, int32_t pad_to, sm_patte
   SM_LAUNCHED();
   k_tmap<<<n, 64, 0, st>>>(A->row_ptr, A->col_idx, P->tmap);
   SM_LAUNCHED();
-  k_order<<<(n + 127) / 128, 128, 0, st>>>(n, P->dim_pad, P->order);
+  k_order<<<(n + 15) / 16, 128, 0, st>>>(n, P->dim_pad, P->order);      // 8 lanes per block column
   SM_LAUNCHED();
   return SM_OK;
 }
