@@ -23,7 +23,7 @@ static const OptDef kOpt[OPT_COUNT] = {
     {"umma.lt", "SM_UMMA_LT", 0},             {"f64.simt", "SM_F64_SIMT", 0},     {"gather.tma", "SM_GATHER_TMA", 0},
     {"umma.epi", "SM_UMMA_EPI", 0},           {"f32.sym", "SM_F32_SYM", 1},
     {"f64.tile", "SM_F64_TILE", 0},           {"umma.fold", "SM_UMMA_FOLD", 1},
-    {"gather.lean", "SM_GATHER_LEAN", 1},
+    {"gather.lean", "SM_GATHER_LEAN", 1},     {"umma.sharea", "SM_UMMA_SHAREA", 1},
     {"umma.ncta", "SM_UMMA_NCTA", 1},         {"umma.mc", "SM_UMMA_MC", 1},       {"umma.tmap", "SM_UMMA_TMAP", 0},
     {"umma.fused", "SM_UMMA_FUSED", 0},       {"umma.slots", "SM_UMMA_SLOTS", 2}, {"umma.dbg", "SM_UMMA_DBG", 0}};
 #ifdef SM_MEASURE

@@ -136,7 +136,7 @@ int32_t *device_err_word();        // pinned, device-mapped host word the kernel
 // ---- variant selection (api.cu): sm_set_option / environment at first use.  Ids are indices into the table there.
 enum OptId {
   OPT_UMMA_SYM = 0, OPT_UMMA_DYN, OPT_UMMA_REV, OPT_UMMA_STAGES, OPT_UMMA_STREAM, OPT_UMMA_RESIDENT, OPT_UMMA_LT,
-  OPT_F64_SIMT, OPT_GATHER_TMA, OPT_UMMA_EPI, OPT_F32_SYM, OPT_F64_TILE, OPT_UMMA_FOLD, OPT_GATHER_LEAN,
+  OPT_F64_SIMT, OPT_GATHER_TMA, OPT_UMMA_EPI, OPT_F32_SYM, OPT_F64_TILE, OPT_UMMA_FOLD, OPT_GATHER_LEAN, OPT_UMMA_SHAREA,
   OPT_FIRST_MEASURE,                 // the ones below exist only in a -DSM_MEASURE build
   OPT_UMMA_NCTA = OPT_FIRST_MEASURE, OPT_UMMA_MC, OPT_UMMA_TMAP, OPT_UMMA_FUSED, OPT_UMMA_SLOTS, OPT_UMMA_DBG,
   OPT_COUNT

@@ -120,7 +120,19 @@ struct UArgs {
   float w_scale, out_scale;
   int32_t no_ident;          // update product without its "+ X" (identity MMAs skipped): a plain product O = X Wh (f2, Eq. 14)
   int32_t fold;              // the tile table was built with the folded geometry (w_* functions)
+  // product 1 (Y = X X^T) only, single-CTA symmetric tiles (option "umma.sharea"): when the tile's A rows are among the B
+  // rows it stages (the tile holds its panel's diagonal square), no A copy is issued and the A descriptor points into
+  // the B stage -- at m = 414 a quarter of the product's L2 -> SM bytes
+  int32_t share_a;
 };
+
+// Row offset of a tile's A rows inside its B stage when product 1 can read A from there (share_a), else -1.
+__device__ __forceinline__ int32_t share_a_off(const UArgs &a, const UTile &u, bool p2) {
+  if (!a.share_a || p2) return -1;
+  const int32_t a_rows = min(UM, u.Pd - u.row0);
+  const int32_t n1 = min(u.nt, u.fb - u.n0);          // B rows [n0, n0 + n1) are matrix rows of the same index
+  return (u.row0 >= u.n0 && u.row0 + a_rows <= u.n0 + n1) ? u.row0 - u.n0 : -1;
+}
 
 // Tile geometry.  Only elements (r, c) with c <= r are computed, so tile row tm (rows tm*R ..
 // tm*R + R - 1, R = 128 * NCTA) needs the columns [0, min(n16, tm*R + R)); they are split into the
@@ -227,7 +239,16 @@ __device__ __forceinline__ UTile make_tile(const UArgs &a, const TileDesc &d) {
   return u;
 }
 
-static __global__ void k_umma_build_tiles(int32_t n_cols, int32_t R, int32_t sym, int32_t fold, int32_t skip_pd, const int32_t *__restrict__ cols,
+// Column split of a row panel whose tiles start at multiples of nb: with `dl` the tiles before the last one are narrowed
+// (whole 32-column blocks) until the last tile starts at or before the panel's first row, so that it holds the whole
+// diagonal square and product 1 can take its A rows from the B stage (share_a_off); the tile count does not change.
+__host__ __device__ inline int32_t dl_nb(int32_t nb, int32_t cnt, int32_t row0, int32_t nc, int32_t dl) {
+  if (!dl || cnt < 2) return nb;
+  const int32_t nb2 = min(nb, (row0 / (cnt - 1)) & ~31);
+  return (nb2 >= 32 && nc - (cnt - 1) * nb2 <= UN) ? nb2 : nb;
+}
+
+static __global__ void k_umma_build_tiles(int32_t n_cols, int32_t R, int32_t sym, int32_t fold, int32_t dl, int32_t skip_pd, const int32_t *__restrict__ cols,
                                           const int32_t *__restrict__ dim, const int32_t *__restrict__ dim_pad,
                                           const int64_t *__restrict__ col_off,
                                           const int64_t *__restrict__ tile_ptr, TileDesc *__restrict__ tiles) {
@@ -251,18 +272,18 @@ static __global__ void k_umma_build_tiles(int32_t n_cols, int32_t R, int32_t sym
   } else if (sym && fold && R == UM) {
     const int32_t fn = w_fold(m), Tm = u_Tm(m, UM);
     for (int32_t tm = 0; tm < Tm; ++tm) {
-      const int32_t cnt = w_row_tiles(m, tm, fn), nb = w_row_nb(m, tm, fn), nc = w_ncols(m, tm, fn);
+      const int32_t cnt = w_row_tiles(m, tm, fn), nc = w_ncols(m, tm, fn), nb = dl_nb(w_row_nb(m, tm, fn), cnt, tm * UM, nc, dl);
       const int32_t v0 = (fn && tm + 1 == Tm) ? tm * UM : 0;       // the last panel's square starts at its own first column
       for (int32_t tn = 0; tn < cnt; ++tn, ++lt, ++t) {
-        d.row0 = tm * UM; d.n0 = v0 + tn * nb; d.nt = min(nb, v0 + nc - d.n0); d.lt = lt;
+        d.row0 = tm * UM; d.n0 = v0 + tn * nb; d.nt = tn + 1 < cnt ? nb : v0 + nc - d.n0; d.lt = lt;      // the last tile takes the rest
         tiles[t] = d;
       }
     }
   } else if (sym) {
     for (int32_t tm = 0; tm < u_Tm(m, R); ++tm) {
-      int32_t cnt = u_row_tiles(m, R, tm), nb = u_row_nb(m, R, tm), nc = u_ncols(m, R, tm);
+      int32_t cnt = u_row_tiles(m, R, tm), nc = u_ncols(m, R, tm), nb = dl_nb(u_row_nb(m, R, tm), cnt, tm * R, nc, R == UM ? dl : 0);
       for (int32_t tn = 0; tn < cnt; ++tn, ++lt, ++t) {
-        d.row0 = tm * R; d.n0 = tn * nb; d.nt = min(nb, nc - d.n0); d.lt = lt;
+        d.row0 = tm * R; d.n0 = tn * nb; d.nt = tn + 1 < cnt ? nb : nc - d.n0; d.lt = lt;
         tiles[t] = d;
       }
     }
@@ -509,6 +530,7 @@ k_umma_gemm(UArgs a, const __grid_constant__ CUtensorMap mapA, const __grid_cons
         const uint32_t a_bytes = a_rows * 128u;
         const uint32_t b_bytes = SYM ? (uint32_t)b_cnt * 128u : (uint32_t)n_atoms * 8192u;
         const int nkc = (u.kmax + UK - 1) / UK;
+        const bool a_shared = SYM && NCTA == 1 && share_a_off(a, u, p2) >= 0;
         if (TM) {
           // boxes: 128 rows (A: one copy; rows past the padded dimension are harmless) and 64 rows (B: b_cnt rounded
           // up to whole boxes -- few, large copies: ten 2 KB boxes per stage kept the producer thread busy longer
@@ -573,9 +595,10 @@ k_umma_gemm(UArgs a, const __grid_constant__ CUtensorMap mapA, const __grid_cons
             if (++stage == USTAGES) { stage = 0; phase ^= 1u; }
             continue;
           }
-          ptx::mbar_expect_tx(full_bar(stage), a_bytes + (MC ? 2u * b_bytes : b_bytes));
+          const uint32_t a_tx = a_shared ? 0u : a_bytes;     // product 1: the A rows are among the B rows of this stage
+          ptx::mbar_expect_tx(full_bar(stage), a_tx + (MC ? 2u * b_bytes : b_bytes));
           const int64_t chunk = (int64_t)kc * u.Pd * 128;     // byte offset of k chunk kc
-          if (a_bytes) ptx::tma_bulk_g2s(sa, Ag + chunk + (int64_t)arow0 * 128, a_bytes, full_bar(stage));
+          if (a_tx) ptx::tma_bulk_g2s(sa, Ag + chunk + (int64_t)arow0 * 128, a_tx, full_bar(stage));
           if (MC) {
             // this CTA's half of the B rows, delivered into both CTAs at its place in the whole tile
             ptx::tma_bulk_g2s_mc(sb + h * b_bytes, Bg + chunk + (int64_t)brow0 * 128, b_bytes, full_bar(stage), (uint16_t)3);
@@ -665,12 +688,13 @@ k_umma_gemm(UArgs a, const __grid_constant__ CUtensorMap mapA, const __grid_cons
         const uint32_t idesc = ptx::make_idesc_f16(BF16, PAIR ? 2 * UM : UM, (uint32_t)u.nt, !SYM);
         const int nkc = (u.kmax + UK - 1) / UK;
         const bool p2 = STREAM ? (cur.pad0 & 1) != 0 : PHASE == 2;
+        const int32_t a_off = (SYM && NCTA == 1 && !(STG && a.lt_in)) ? __shfl_sync(0xffffffffu, share_a_off(a, u, p2), 0) : -1;
         for (int kc = 0; kc < nkc; ++kc) {
           ptx::mbar_wait(full_bar(stage), phase, a.err_flag, 3);
           if (PAIR && !TM) ptx::mbar_wait(pfull_bar(stage), phase, a.err_flag, 6);
           ptx::tc_fence_after();
           const uint32_t sa = tiles + stage * STAGE_BYTES, sb = sa + A_BYTES;
-          const uint64_t adesc = ptx::make_sw128_kmajor_desc(sa);
+          const uint64_t adesc = ptx::make_sw128_kmajor_desc(a_off >= 0 ? sb + (uint32_t)a_off * 128u : sa);
           const uint64_t bdesc = SYM ? ptx::make_sw128_kmajor_desc(sb) : ptx::make_sw128_mnmajor_desc(sb, 8192u, 1024u);
           const uint64_t bstep = SYM ? 2u : 128u;   // 16 k: 32 B inside a K-major atom / 16 rows of 128 B
           const int ksteps = SM_DBG(a, 2) ? 0 : min(UK / 16, (u.kmax - kc * UK) / 16);
@@ -1413,7 +1437,9 @@ int32_t sign_umma(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, co
                                         w.n_parts);
   SM_LAUNCHED();
   { int32_t rc = exclusive_scan_i64(n_cols, w.tile_ptr, w.tile_ptr, st); if (rc != SM_OK) return rc; }
-  k_umma_build_tiles<<<nb, 256, 0, st>>>(n_cols, R, sym, fold, res_pd, cols, P->dim, P->dim_pad, col_off, w.tile_ptr, w.tiles);
+  // product 1 reads its A rows from the B stage where a tile holds its diagonal square (option "umma.sharea"; see share_a_off)
+  const int32_t share_a = (sym == 1 && ncta == 1 && opt(OPT_UMMA_SHAREA) != 0) ? 1 : 0;
+  k_umma_build_tiles<<<nb, 256, 0, st>>>(n_cols, R, sym, fold, share_a, res_pd, cols, P->dim, P->dim_pad, col_off, w.tile_ptr, w.tiles);
   SM_LAUNCHED();
   // Y and the alternate X buffer: what the kernels read or copy back without ever writing it must be zero (and never a
   // NaN/Inf bit pattern).  The symmetric single-CTA tiles leave only padding rows / columns unwritten (k_zero_padding);
@@ -1482,7 +1508,7 @@ int32_t sign_umma(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, co
     SM_CUDA(cudaMemsetAsync(w.done, 0, sizeof(int32_t) * n_done, st));
     UArgs a{cols, col_off, P->dim, P->dim_pad, w.tile_ptr, w.tiles, n_cols, 0, X, w.Y, w.X2, s, w.err, 0, w.counters,
             2 * max_iter, w.done, umma_dbg(), 0, 0, 0, -0.5f, 1.f};
-    a.fold = fold;
+    a.fold = fold; a.share_a = share_a;
     int32_t rc = sym == 2 ? launch_umma_t<0, 1, true, false, 0, false, true, 1>(bf16, a, maps[0], n_sm, st)
                           : launch_umma_t<0, 1, true, false, 0, false, true>(bf16, a, maps[0], n_sm, st);
     if (rc != SM_OK) return rc;
@@ -1512,7 +1538,7 @@ int32_t sign_umma(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols, co
     // of a submatrix (fixed counts: the last step; convergence mode: per submatrix, s.last)
     const int32_t lt = (sym == 2 && !o3 && opt(OPT_UMMA_LT) != 0) ? 1 : 0;
     a.lt_in = lt && k > 0; a.lt_out = lt;
-    a.fold = fold;
+    a.fold = fold; a.share_a = share_a;
     int32_t launch = nper * k;                 // launches alternate their walk through the tile table (option umma.rev)
     a.rev = o3 ? (rev_on & launch) & 1 : 0;
     a.counter = dyn ? w.counters + launch : nullptr;
@@ -1585,7 +1611,7 @@ int32_t umma_product(const sm_pattern_t *P, const int32_t *cols, int32_t n_cols,
   k_umma_tilecounts<<<nb, 256, 0, st>>>(n_cols, R, sym, 0, EPI_WARPS * ncta, 0, cols, P->dim, P->dim_pad, w.tile_ptr, w.n_parts);
   SM_LAUNCHED();
   { int32_t rc = exclusive_scan_i64(n_cols, w.tile_ptr, w.tile_ptr, st); if (rc != SM_OK) return rc; }
-  k_umma_build_tiles<<<nb, 256, 0, st>>>(n_cols, R, sym, 0, 0, cols, P->dim, P->dim_pad, col_off, w.tile_ptr, w.tiles);
+  k_umma_build_tiles<<<nb, 256, 0, st>>>(n_cols, R, sym, 0, 0, 0, cols, P->dim, P->dim_pad, col_off, w.tile_ptr, w.tiles);
   SM_LAUNCHED();
   SM_CUDA(cudaMemsetAsync(O, 0, packed_elems * 2, st));       // padding of the result reads as zeros
   UArgs a{cols, col_off, P->dim, P->dim_pad, w.tile_ptr, w.tiles, n_cols, 0, A, B, O, s, w.err, 0, nullptr, 0, nullptr, 0, 0, 0, 0,

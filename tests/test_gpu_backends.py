@@ -13,6 +13,7 @@ environment forces (each in its own process: the selection is read once per proc
   SM_UMMA_RESIDENT=1|0  submatrices with Pd <= 256 iterate inside one SM (k_umma_resident) / grouped tiles for all
   SM_UMMA_LT=0|1     grouped tiles: iterates stored lower-triangular, the upper part read through MN-major descriptors
   SM_UMMA_FOLD=1|0   single-CTA symmetric tiles: a short last row panel is computed as extra columns of the other panels / as a panel
+  SM_UMMA_SHAREA=1|0 product 1: a tile that holds its panel's diagonal square reads its A rows from the B stage / loads them
   SM_F64_SIMT=0|1    DMMA tensor tiles (default) / DFMA register tiles
 The two-CTA and fused variants exist only in a -DSM_MEASURE build of the library (build.py --measure); their cases
 are skipped on the default build.
@@ -83,6 +84,8 @@ CASES = [
     ({"SM_UMMA_NCTA": "1", "SM_UMMA_SYM": "1"}, "bf16", 64, (90, 23, 4, 5.0), 3, 2.5e-2, True, None),
     ({"SM_UMMA_DYN": "0"}, "f16", 64, (90, 23, 4, 5.0), 3, 3e-3, True, None),
     ({"SM_UMMA_FOLD": "0"}, "f16", 64, (90, 23, 4, 5.0), 3, 3e-3, True, None),
+    ({"SM_UMMA_SHAREA": "0"}, "f16", 64, (90, 23, 4, 5.0), 3, 3e-3, True, None),
+    ({"SM_UMMA_SHAREA": "0", "SM_UMMA_RESIDENT": "0"}, "bf16", 64, (300, 6, 3, 6.0), 3, 2.5e-2, True, None),
     ({"SM_UMMA_FOLD": "0", "SM_UMMA_RESIDENT": "0"}, "bf16", 64, (300, 6, 3, 6.0), 3, 2.5e-2, True, None),
     ({"SM_UMMA_FOLD": "1", "SM_UMMA_RESIDENT": "0"}, "f16", 64, (300, 6, 3, 6.0), 5, 3e-3, True, None),
     ({"SM_UMMA_FOLD": "1", "SM_UMMA_STREAM": "1", "SM_UMMA_RESIDENT": "0"}, "f16", 64, (300, 6, 3, 6.0), 4, 3e-3, True, None),
@@ -156,6 +159,7 @@ HASH_SNIPPET = textwrap.dedent("""
 
 SYM_VARIANTS = [
     {"SM_UMMA_RESIDENT": "0"},
+    {"SM_UMMA_RESIDENT": "0", "SM_UMMA_SHAREA": "0"},
     {"SM_UMMA_RESIDENT": "0", "SM_UMMA_REV": "0"},
     {"SM_UMMA_RESIDENT": "0", "SM_UMMA_STAGES": "3"},
     {"SM_UMMA_RESIDENT": "0", "SM_UMMA_DYN": "0"},
@@ -200,3 +204,20 @@ def test_symmetric_tile_variants_are_bit_identical():
     ref = next(iter(seen.values()))
     for v in seen.values():
         assert abs(v[1] - ref[1]) <= 1e-6 * abs(ref[1]) and abs(v[2] - ref[2]) <= 1e-6 * abs(ref[2]), seen
+
+
+def test_share_a_is_bit_identical_with_the_folded_geometry():
+    """umma.sharea only changes where product 1 reads its A rows from (the B stage instead of a copy of their own) and
+    which of a panel's tiles is the narrow one: every output element is the same k-ordered sum, so the iterates of the
+    default (folded) geometry agree to the bit with and without it, per-phase launches and stream mode."""
+    for base in ({"SM_UMMA_RESIDENT": "0"}, {"SM_UMMA_RESIDENT": "0", "SM_UMMA_STREAM": "1"}):
+        hashes = []
+        for v in ("0", "1"):
+            e = dict(os.environ)
+            e.update(base)
+            e["SM_UMMA_SHAREA"] = v
+            p = subprocess.run([sys.executable, "-c", HASH_SNIPPET.format(root=ROOT)], env=e, capture_output=True,
+                               text=True, timeout=600, cwd=ROOT)
+            assert p.returncode == 0, p.stdout[-2000:] + p.stderr[-4000:]
+            hashes.append([ln for ln in p.stdout.splitlines() if ln.startswith("HASH")][0].split()[1])
+        assert hashes[0] == hashes[1], (base, hashes)
