@@ -313,6 +313,8 @@ int32_t sm_density_from_sign(const sm_bcsr_t *A, const sm_pattern_t *P, int32_t 
  *                                            diagonal squares), the rest read through MN-major descriptors
  *   "umma.fold"     [SM_UMMA_FOLD]     1|0   16-bit grouped symmetric tiles: a last 128-row panel of <= 64 rows is computed as extra
  *                                            columns of the other panels and mirrored into place / as a row panel of its own
+ *   "umma.sharea"   [SM_UMMA_SHAREA]   1|0   16-bit grouped symmetric tiles, product X X^T: a tile that holds its panel's diagonal
+ *                                            square reads its A rows from the B rows it stages / loads them separately (bit-identical)
  *   "umma.dyn"      [SM_UMMA_DYN]      1|0   16-bit grouped tiles handed out by a global counter / dealt round robin
  *   "umma.rev"      [SM_UMMA_REV]      1|0   16-bit: the update product walks the tile table backwards / forwards
  *   "umma.stages"   [SM_UMMA_STAGES]   0|3|4 16-bit grouped tiles: depth of the operand ring (0 = by size)
