@@ -461,10 +461,13 @@ k_umma_gemm(UArgs a, const __grid_constant__ CUtensorMap mapA, const __grid_cons
 
   if (warp == 0) {
     // ===================== TMA producer (every CTA: its A rows and its share of the B rows) ==========
-    if (lane == 0) {
+    // CONV: the whole warp walks the tiles converged and one elected lane issues each copy (tma_bulk_g2s_elect); lane 0
+    // alone pops / publishes the tile (fetch) and broadcasts it.  The other variants keep the single producer thread.
+    constexpr bool CONV = NCTA == 1 && SYM && !MC && !TM && EPI == 0;
+    if (CONV || lane == 0) {
       int stage = 0; uint32_t phase = 0;
       TileDesc nxt = load_desc(a, max((int64_t)0, min(unit, total - 1)));
-      int64_t t = DYN ? (int64_t)atomicAdd(a.counter, 1ULL) : unit;
+      int64_t t = DYN ? (lane == 0 ? (int64_t)atomicAdd(a.counter, 1ULL) : 0) : unit;
       uint32_t qs = 0, qp = 0;
       int32_t sg_c0 = 0;                                                     // STREAM: current super-group
       int64_t sg_lo = 0, sg_hi = STREAM ? a.tile_ptr[min(STREAM_SG, a.n_cols)] : 0;
@@ -514,6 +517,55 @@ k_umma_gemm(UArgs a, const __grid_constant__ CUtensorMap mapA, const __grid_cons
         return true;
       };
       TileDesc cur;
+      if (CONV) {
+        constexpr uint32_t FULL = 0xffffffffu;
+        for (;;) {
+          int32_t ok = 0;
+          if (lane == 0) ok = fetch(cur) ? 1 : 0;
+          __syncwarp();
+          if (!__shfl_sync(FULL, ok, 0)) break;
+          {
+            uint32_t blo = (uint32_t)(uint64_t)cur.base, bhi = (uint32_t)((uint64_t)cur.base >> 32);
+            blo = __shfl_sync(FULL, blo, 0); bhi = __shfl_sync(FULL, bhi, 0);
+            cur.base = (int64_t)(((uint64_t)bhi << 32) | blo);
+            cur.c = __shfl_sync(FULL, cur.c, 0); cur.m = __shfl_sync(FULL, cur.m, 0);
+            cur.Pd = __shfl_sync(FULL, cur.Pd, 0); cur.row0 = __shfl_sync(FULL, cur.row0, 0);
+            cur.n0 = __shfl_sync(FULL, cur.n0, 0); cur.nt = __shfl_sync(FULL, cur.nt, 0);
+            cur.lt = __shfl_sync(FULL, cur.lt, 0); cur.pad0 = __shfl_sync(FULL, cur.pad0, 0);
+          }
+          UTile u = make_tile<PHASE>(a, cur);
+          u.valid = __shfl_sync(FULL, u.valid, 0);
+          if (!u.valid) continue;
+          const bool p2 = STREAM ? (cur.pad0 & 1) != 0 : PHASE == 2;
+          const void *Xcur = (STREAM && ((cur.pad0 >> 1) & 1)) ? a.Out : a.Xsrc;     // stream: X ping-pongs per step
+          const uint32_t a_rows = (uint32_t)max(0, min(UM, u.Pd - u.row0));
+          // product 1: the A rows are among the B rows of the stage (share_a_off): no copy of their own
+          const uint32_t a_tx = share_a_off(a, u, p2) >= 0 ? 0u : a_rows * 128u;
+          // B rows [n0, n0 + nt) of the tile's (virtual) columns: those from u.fb on are the folded rows
+          const int32_t n1 = max(0, min(u.nt, u.fb - u.n0));
+          const uint32_t b1_tx = (uint32_t)n1 * 128u, b2_tx = (uint32_t)(u.nt - n1) * 128u;
+          const char *pA = (const char *)Xcur + u.base * ESZ + (int64_t)u.row0 * 128;
+          const char *Bg = (const char *)(p2 ? a.Ybuf : Xcur) + u.base * ESZ;
+          const char *pB1 = Bg + (int64_t)u.n0 * 128, *pB2 = Bg + (int64_t)(max(u.n0, u.fb) + u.fs) * 128;
+          const int64_t cs = (int64_t)u.Pd * 128;                                  // bytes between k chunks
+          const int nkc = (u.kmax + UK - 1) / UK;
+          for (int kc = 0; kc < nkc; ++kc) {
+            ptx::mbar_wait(empty_bar(stage), phase ^ 1u, a.err_flag, 1);
+            const uint32_t sa = tiles + stage * STAGE_BYTES, sb = sa + A_BYTES, fb_ = full_bar(stage);
+            if (SM_DBG(a, 4)) {
+              if (lane == 0) ptx::mbar_arrive(fb_);
+              __syncwarp();
+            } else {
+              ptx::mbar_expect_tx_elect(fb_, a_tx + b1_tx + b2_tx);
+              if (a_tx) ptx::tma_bulk_g2s_elect(sa, pA, a_tx, fb_);
+              if (b1_tx) ptx::tma_bulk_g2s_elect(sb, pB1, b1_tx, fb_);
+              if (b2_tx) ptx::tma_bulk_g2s_elect(sb + b1_tx, pB2, b2_tx, fb_);
+              pA += cs; pB1 += cs; pB2 += cs;
+            }
+            if (++stage == USTAGES) { stage = 0; phase ^= 1u; }
+          }
+        }
+      } else
       while (fetch(cur)) {
         UTile u = make_tile<PHASE>(a, cur);
         if (!u.valid) continue;

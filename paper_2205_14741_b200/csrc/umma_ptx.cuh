@@ -73,6 +73,31 @@ __device__ __forceinline__ void tma_bulk_g2s(uint32_t dst_smem, const void *src_
       : "memory");
 }
 
+// Warp-convergent forms (see umma_f16_elect): EVERY lane of the converged warp executes them with the same operands and
+// one elected lane issues.  Under `if (lane == 0)` ptxas wraps each bulk copy in an ELECT / R2UR.BROADCAST / BRA.U.ANY
+// loop; the producer thread then needed ~1000 cycles per k chunk (ncu source page, round 2: 93 % of its samples outside
+// the barrier wait) while the chunk's MMAs take ~400.
+__device__ __forceinline__ void tma_bulk_g2s_elect(uint32_t dst_smem, const void *src_gmem, uint32_t bytes, uint32_t bar) {
+  asm volatile(
+      "{\n"
+      ".reg .pred q;\n"
+      "elect.sync _|q, 0xffffffff;\n"
+      "@q cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n"
+      "}\n" ::"r"(dst_smem),
+      "l"(src_gmem), "r"(bytes), "r"(bar)
+      : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx_elect(uint32_t bar, uint32_t bytes) {
+  asm volatile(
+      "{\n"
+      ".reg .pred q;\n"
+      "elect.sync _|q, 0xffffffff;\n"
+      "@q mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n"
+      "}\n" ::"r"(bar),
+      "r"(bytes)
+      : "memory");
+}
+
 // ---- bulk TMA: shared -> global (bulk async-group completion), L2 prefetch ---------------------------
 __device__ __forceinline__ void tma_bulk_s2g(void *dst_gmem, uint32_t src_smem, uint32_t bytes) {
   asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst_gmem), "r"(src_smem), "r"(bytes)
