@@ -352,11 +352,26 @@ __device__ __forceinline__ uint32_t ident_row(bool pair, int32_t s, int32_t N) {
 // C0 .. C0 + 31 as 16 packed pairs: element (r, C0 + j) goes to row C0 + j, column r of the swizzled image.
 __device__ __forceinline__ void mirror_store(uint16_t *Og, int32_t Pd, int32_t R0, int32_t C0, int lane,
                                              const uint32_t (&o)[16]) {
+#ifdef SM_MIRROR_U16
   uint16_t *Mb = Og + (int64_t)(R0 >> 6) * Pd * 64 + (int64_t)C0 * 64 + (lane & 7);
   const uint32_t ch = (((uint32_t)R0 & 63u) >> 3) + ((uint32_t)lane >> 3);   // chunk of column r before the swizzle
 #pragma unroll
   for (int j = 0; j < 32; ++j)
     Mb[j * 64 + ((ch ^ (uint32_t)(j & 7)) << 3)] = (uint16_t)(o[j >> 1] >> ((j & 1) * 16));
+#else
+  // Lane pairs (r, r ^ 1) exchange halves first, so that a lane holds the two ADJACENT columns r & ~1, (r & ~1) + 1 of one
+  // mirrored row -- the even lane of row C0 + 2e, the odd lane of row C0 + 2e + 1 -- and stores 4 bytes: 16 store
+  // instructions per block instead of 32 (each instruction still fills two whole sectors per row, now of two rows).
+  const uint32_t odd = (uint32_t)lane & 1u;
+  uint16_t *Mb = Og + (int64_t)(R0 >> 6) * Pd * 64 + (int64_t)(C0 + (int32_t)odd) * 64 + (lane & 6);
+  const uint32_t chx = ((((uint32_t)R0 & 63u) >> 3) + ((uint32_t)lane >> 3)) ^ odd;   // chunk of column r, swizzle bit 0 of the row folded in
+#pragma unroll
+  for (int e = 0; e < 16; ++e) {
+    const uint32_t x = __shfl_xor_sync(0xffffffffu, o[e], 1);
+    const uint32_t w = odd ? __byte_perm(x, o[e], 0x7632) : __byte_perm(o[e], x, 0x5410);
+    *reinterpret_cast<uint32_t *>(Mb + (2 * e) * 64 + ((chx ^ (uint32_t)((2 * e) & 7)) << 3)) = w;
+  }
+#endif
 }
 
 // SYM = true : K-major B (X X^T form), lower-triangle tiles, mirrored stores (exactly symmetric iterates).
