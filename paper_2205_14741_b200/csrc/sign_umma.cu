@@ -791,6 +791,9 @@ k_umma_gemm(UArgs a, const __grid_constant__ CUtensorMap mapA, const __grid_cons
             } else {
               for (int ks = 0; ks < ksteps; ++ks) issue(ks);
             }
+          } else if (SYM && !PAIR && ksteps == UK / 16) {
+            ptx::umma_f16_elect_k4(d_tmem, ptx::sw128_kmajor_lo(a_off >= 0 ? sb + (uint32_t)a_off * 128u : sa), ptx::sw128_kmajor_lo(sb),
+                                   idesc, (uint32_t)(kc != 0));
           } else if (ksteps == UK / 16) {
 #pragma unroll
             for (int ks = 0; ks < UK / 16; ++ks)
@@ -814,9 +817,14 @@ k_umma_gemm(UArgs a, const __grid_constant__ CUtensorMap mapA, const __grid_cons
                 const uint32_t idesc2 = ptx::make_idesc_f16(BF16, PAIR ? 2 * UM : UM, (uint32_t)(hi - lo), false);
                 const uint64_t idd = ptx::make_sw128_kmajor_desc(ident + ident_row(PAIR, lo - kc * UK, hi - lo) * 128u);
                 const uint32_t acol = (uint32_t)(lo - (part ? u.fs : 0) - u.n0);
+                if (!PAIR) {
+                  ptx::umma_f16_elect_k4(d_tmem + acol, ptx::sw128_kmajor_lo(sa),
+                                         ptx::sw128_kmajor_lo(ident + ident_row(PAIR, lo - kc * UK, hi - lo) * 128u), idesc2, 1u);
+                } else {
 #pragma unroll
-                for (int ks = 0; ks < UK / 16; ++ks)
-                  mma(d_tmem + acol, adesc + (uint64_t)(2 * ks), idd + (uint64_t)(2 * ks), idesc2, 1u);
+                  for (int ks = 0; ks < UK / 16; ++ks)
+                    mma(d_tmem + acol, adesc + (uint64_t)(2 * ks), idd + (uint64_t)(2 * ks), idesc2, 1u);
+                }
               }
             }
           }

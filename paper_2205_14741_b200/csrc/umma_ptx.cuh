@@ -156,6 +156,44 @@ __device__ __forceinline__ void umma_f16_elect(uint32_t tmem_d, uint64_t adesc, 
       "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
       : "memory");
 }
+// The four K = 16 steps of one 64-wide k chunk, both operands K-major SW128 (descriptor high word 0x40004040: SBO 1024 B,
+// version 1, swizzle 128 B; low word = (address >> 4) | LBO field, see make_sw128_kmajor_desc), issued by ONE elected lane
+// from ONE asm block: one ELECT and 32-bit descriptor arithmetic instead of four elect / 64-bit add sequences.  The MMA
+// warp's instruction stream is on the critical path (round 2: ~15 more instructions per chunk cost 10 % at configs[4]).
+__device__ __forceinline__ uint32_t sw128_kmajor_lo(uint32_t smem_addr) { return ((smem_addr & 0x3FFFFu) >> 4) | 0x10000u; }
+__device__ __forceinline__ void umma_f16_elect_k4(uint32_t tmem_d, uint32_t a_lo, uint32_t b_lo, uint32_t idesc,
+                                                  uint32_t accumulate0) {
+  asm volatile(
+      "{\n"
+      ".reg .pred q, p, t;\n"
+      ".reg .b32 hi, al, bl;\n"
+      ".reg .b64 da, db;\n"
+      "elect.sync _|q, 0xffffffff;\n"
+      "setp.ne.b32 p, %4, 0;\n"
+      "setp.eq.b32 t, 0, 0;\n"
+      "mov.b32 hi, 0x40004040;\n"
+      "mov.b64 da, {%1, hi};\n"
+      "mov.b64 db, {%2, hi};\n"
+      "@q tcgen05.mma.cta_group::1.kind::f16 [%0], da, db, %3, p;\n"
+      "add.u32 al, %1, 2;\n"
+      "add.u32 bl, %2, 2;\n"
+      "mov.b64 da, {al, hi};\n"
+      "mov.b64 db, {bl, hi};\n"
+      "@q tcgen05.mma.cta_group::1.kind::f16 [%0], da, db, %3, t;\n"
+      "add.u32 al, %1, 4;\n"
+      "add.u32 bl, %2, 4;\n"
+      "mov.b64 da, {al, hi};\n"
+      "mov.b64 db, {bl, hi};\n"
+      "@q tcgen05.mma.cta_group::1.kind::f16 [%0], da, db, %3, t;\n"
+      "add.u32 al, %1, 6;\n"
+      "add.u32 bl, %2, 6;\n"
+      "mov.b64 da, {al, hi};\n"
+      "mov.b64 db, {bl, hi};\n"
+      "@q tcgen05.mma.cta_group::1.kind::f16 [%0], da, db, %3, t;\n"
+      "}\n" ::"r"(tmem_d),
+      "r"(a_lo), "r"(b_lo), "r"(idesc), "r"(accumulate0)
+      : "memory");
+}
 __device__ __forceinline__ void umma_commit_elect(uint32_t bar) {
   asm volatile(
       "{\n"
