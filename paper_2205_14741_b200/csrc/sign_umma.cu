@@ -14,11 +14,13 @@
 // amplifies any antisymmetric perturbation by ~2x per step (measured: NaN after ~18 bf16 steps),
 // while exactly symmetric iterates make X X^T == X^2 and keep the iteration on Eq. 13's fixed point.
 //
-// Kernel: persistent, one CTA per SM, 320 threads = 1 TMA producer warp, 1 MMA issuer warp (also
-// owns TMEM), 8 epilogue warps.  Tile = 128 x (<=256) fp32 accumulator in TMEM, double buffered
-// (2 x 256 columns) so the epilogue of tile t overlaps the main loop of tile t+1; 4-stage smem ring.
-//   PHASE 1: W = X X^T - I, epilogue writes W and the fused ||W||_F^2 partial sums (warp shuffles).
-//   PHASE 2: X' = X - 0.5 X W^T (= 1.5 X - 0.5 X Y), epilogue reads the X tile and writes X'.
+// Kernel: persistent, one CTA per SM, 576 threads = 1 TMA producer warp (warp-convergent: one elected lane issues the
+// bulk copies), 1 MMA issuer warp (also owns TMEM; elected-lane issue), 16 epilogue warps (4 per TMEM lane quadrant).
+// Tile = 128 x (<=256) fp32 accumulator in TMEM, double buffered (2 x 256 columns) so the epilogue of tile t overlaps
+// the main loop of tile t+1; 4-stage smem ring of 48 KB stages; tiles handed out by a global counter.
+//   PHASE 1: Y = X X^T; the epilogue stores Wh = -1/2 (Y - I) and the fused ||Y - I||_F^2 partial sums (warp shuffles).
+//            A tile that holds its panel's diagonal square reads its A rows from the B rows it stages (share_a_off).
+//   PHASE 2: X' = X + X Wh as ONE accumulation (identity MMAs add X); the epilogue only converts and stores.
 #include <cuda.h>   // CUtensorMap (type only; the encoder is fetched through cudaGetDriverEntryPoint)
 #include <cstdio>
 #include <cstdlib>
