@@ -165,8 +165,8 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_umma_resident(RArgs a) {
             const int ksteps = min(4, (s.kmax - kc * 64) / 16);
             const uint32_t acc0 = (uint32_t)(!first || kc != k_lo);
             if (ksteps == 4) {
-#pragma unroll
-              for (int ks = 0; ks < 4; ++ks) ptx::umma_f16_elect(d, ad + (uint64_t)(2 * ks), bd + (uint64_t)(2 * ks), idesc, acc0 | (uint32_t)(ks != 0));
+              ptx::umma_f16_elect_k4(d, ptx::sw128_kmajor_lo(xs + (uint32_t)kc * Pd * 128u + (t ? 128u * 128u : 0u)),
+                                     ptx::sw128_kmajor_lo(xs + (uint32_t)kc * Pd * 128u), idesc, acc0);
             } else {
               for (int ks = 0; ks < ksteps; ++ks) ptx::umma_f16_elect(d, ad + (uint64_t)(2 * ks), bd + (uint64_t)(2 * ks), idesc, acc0 | (uint32_t)(ks != 0));
             }
@@ -184,8 +184,8 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_umma_resident(RArgs a) {
               const uint32_t idesc = ptx::make_idesc_f16(bf, 128, N, false);
               const uint64_t bd = ptx::make_sw128_kmajor_desc(ws + res_woff((uint32_t)kc, Pd));
               if (ksteps == 4) {
-#pragma unroll
-                for (int ks = 0; ks < 4; ++ks) ptx::umma_f16_elect(d, ad + (uint64_t)(2 * ks), bd + (uint64_t)(2 * ks), idesc, acc0 | (uint32_t)(ks != 0));
+                ptx::umma_f16_elect_k4(d, ptx::sw128_kmajor_lo(xs + (uint32_t)kc * Pd * 128u + (t ? 128u * 128u : 0u)),
+                                       ptx::sw128_kmajor_lo(ws + res_woff((uint32_t)kc, Pd)), idesc, acc0);
               } else {
                 for (int ks = 0; ks < ksteps; ++ks) ptx::umma_f16_elect(d, ad + (uint64_t)(2 * ks), bd + (uint64_t)(2 * ks), idesc, acc0 | (uint32_t)(ks != 0));
               }
@@ -197,11 +197,9 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_umma_resident(RArgs a) {
               const uint32_t idesc_d = ptx::make_idesc_f16(bf, 128, t ? Pd - 128u : 16u, false);
               const uint64_t bd = ptx::make_sw128_kmajor_desc(ws + res_woff((uint32_t)kc, Pd));
               if (ksteps == 4) {
-#pragma unroll
-                for (int ks = 0; ks < 4; ++ks) {
-                  ptx::umma_f16_elect(d, ad + (uint64_t)(2 * ks), bt + (uint64_t)(128 * ks), idesc_t, acc0 | (uint32_t)(ks != 0));
-                  if (t) ptx::umma_f16_elect(d + 128u, ad + (uint64_t)(2 * ks), bd + (uint64_t)(2 * ks), idesc_d, acc0 | (uint32_t)(ks != 0));
-                }
+                const uint32_t a_lo = ptx::sw128_kmajor_lo(xs + (uint32_t)kc * Pd * 128u + (t ? 128u * 128u : 0u));
+                ptx::umma_f16_elect_k4_bmn(d, a_lo, ptx::sw128_mnmajor_lo(ws + (uint32_t)kc * 64u * 128u, Pd * 128u), idesc_t, acc0);
+                if (t) ptx::umma_f16_elect_k4(d + 128u, a_lo, ptx::sw128_kmajor_lo(ws + res_woff((uint32_t)kc, Pd)), idesc_d, acc0);
               } else {
                 for (int ks = 0; ks < ksteps; ++ks) {
                   ptx::umma_f16_elect(d, ad + (uint64_t)(2 * ks), bt + (uint64_t)(128 * ks), idesc_t, acc0 | (uint32_t)(ks != 0));

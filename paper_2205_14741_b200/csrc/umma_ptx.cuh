@@ -64,7 +64,19 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity, int32_t
   }
 }
 
-// ---- bulk TMA: contiguous global -> shared, completion on an mbarrier ------------------------
+// Spinning form (plain try_wait in a loop, no suspend-time hint) for waits on a SERIAL critical path: in k_umma_resident every
+// hand-over MMA -> epilogue -> MMA is exposed, so the wake-up out of a hinted wait adds to every step.
+__device__ __forceinline__ void mbar_wait_spin(uint32_t bar, uint32_t parity, int32_t *err_flag, int32_t code) {
+  for (uint32_t i = 0; !mbar_try_wait(bar, parity); ++i) {
+    if (i > 200000000u) {
+      if (err_flag) atomicExch(err_flag, code);
+      __threadfence_system();
+      __trap();
+    }
+  }
+}
+
+
 __device__ __forceinline__ void tma_bulk_g2s(uint32_t dst_smem, const void *src_gmem, uint32_t bytes,
                                              uint32_t bar) {
   asm volatile(
@@ -187,6 +199,43 @@ __device__ __forceinline__ void umma_f16_elect_k4(uint32_t tmem_d, uint32_t a_lo
       "@q tcgen05.mma.cta_group::1.kind::f16 [%0], da, db, %3, t;\n"
       "add.u32 al, %1, 6;\n"
       "add.u32 bl, %2, 6;\n"
+      "mov.b64 da, {al, hi};\n"
+      "mov.b64 db, {bl, hi};\n"
+      "@q tcgen05.mma.cta_group::1.kind::f16 [%0], da, db, %3, t;\n"
+      "}\n" ::"r"(tmem_d),
+      "r"(a_lo), "r"(b_lo), "r"(idesc), "r"(accumulate0)
+      : "memory");
+}
+// Same with an MN-major B operand (descriptor low word carries the LBO field; 16 k = 16 rows of 128 B = +128 per step).
+__device__ __forceinline__ uint32_t sw128_mnmajor_lo(uint32_t smem_addr, uint32_t lbo_bytes) {
+  return ((smem_addr & 0x3FFFFu) >> 4) | (((lbo_bytes >> 4) & 0x3FFFu) << 16);
+}
+__device__ __forceinline__ void umma_f16_elect_k4_bmn(uint32_t tmem_d, uint32_t a_lo, uint32_t b_lo, uint32_t idesc,
+                                                      uint32_t accumulate0) {
+  asm volatile(
+      "{\n"
+      ".reg .pred q, p, t;\n"
+      ".reg .b32 hi, al, bl;\n"
+      ".reg .b64 da, db;\n"
+      "elect.sync _|q, 0xffffffff;\n"
+      "setp.ne.b32 p, %4, 0;\n"
+      "setp.eq.b32 t, 0, 0;\n"
+      "mov.b32 hi, 0x40004040;\n"
+      "mov.b64 da, {%1, hi};\n"
+      "mov.b64 db, {%2, hi};\n"
+      "@q tcgen05.mma.cta_group::1.kind::f16 [%0], da, db, %3, p;\n"
+      "add.u32 al, %1, 2;\n"
+      "add.u32 bl, %2, 128;\n"
+      "mov.b64 da, {al, hi};\n"
+      "mov.b64 db, {bl, hi};\n"
+      "@q tcgen05.mma.cta_group::1.kind::f16 [%0], da, db, %3, t;\n"
+      "add.u32 al, %1, 4;\n"
+      "add.u32 bl, %2, 256;\n"
+      "mov.b64 da, {al, hi};\n"
+      "mov.b64 db, {bl, hi};\n"
+      "@q tcgen05.mma.cta_group::1.kind::f16 [%0], da, db, %3, t;\n"
+      "add.u32 al, %1, 6;\n"
+      "add.u32 bl, %2, 384;\n"
       "mov.b64 da, {al, hi};\n"
       "mov.b64 db, {bl, hi};\n"
       "@q tcgen05.mma.cta_group::1.kind::f16 [%0], da, db, %3, t;\n"
