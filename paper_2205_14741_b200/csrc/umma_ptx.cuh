@@ -64,19 +64,7 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity, int32_t
   }
 }
 
-// Spinning form (plain try_wait in a loop, no suspend-time hint) for waits on a SERIAL critical path: in k_umma_resident every
-// hand-over MMA -> epilogue -> MMA is exposed, so the wake-up out of a hinted wait adds to every step.
-__device__ __forceinline__ void mbar_wait_spin(uint32_t bar, uint32_t parity, int32_t *err_flag, int32_t code) {
-  for (uint32_t i = 0; !mbar_try_wait(bar, parity); ++i) {
-    if (i > 200000000u) {
-      if (err_flag) atomicExch(err_flag, code);
-      __threadfence_system();
-      __trap();
-    }
-  }
-}
-
-
+// ---- bulk TMA: contiguous global -> shared, completion on an mbarrier ------------------------
 __device__ __forceinline__ void tma_bulk_g2s(uint32_t dst_smem, const void *src_gmem, uint32_t bytes,
                                              uint32_t bar) {
   asm volatile(
