@@ -265,7 +265,8 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_umma_resident(RArgs a) {
         // store four stmatrix.x4.trans (one 8-column strip each, transposed in flight) -- instead of 32 two-byte
         // stores with their address arithmetic (ncu, first version of this kernel: 530 instructions per block, the
         // epilogue issue-bound on the sub-partition of the lowest rows).
-        auto pass = [&](const bool P2, const bool bf_out, float &res) {
+        // RES: accumulate the residual partial sums (product 1; fixed counts need them only in the last step)
+        auto pass = [&](const bool P2, const bool bf_out, const bool RES, float &res) {
           float res2 = 0.f;
           const int g = lane >> 2, q2 = lane & 3, rl = lane & 7, ml = lane >> 3;
           for (int tt = 0; tt < (s.two ? 2 : 1); ++tt) {
@@ -305,11 +306,11 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_umma_resident(RArgs a) {
                       // row / column inside the block; tiles above the diagonal are not used (overwritten by mirrors)
                       const int rr = 8 * ti + g, c0 = 8 * tj + 2 * q2;
                       if (R0 + rr < s.m) { if (c0 == rr) f0 -= 1.f; if (c0 + 1 == rr) f1 -= 1.f; }   // W = Y - I
-                      if (tj <= ti) {
+                      if (RES && tj <= ti) {
                         if (c0 <= rr) acc = fmaf(c0 == rr ? f0 : 2.f * f0, f0, acc);
                         if (c0 + 1 <= rr) acc = fmaf(c0 + 1 == rr ? f1 : 2.f * f1, f1, acc);
                       }
-                    } else {
+                    } else if (RES) {
                       acc = fmaf(f0, f0, acc); acc = fmaf(f1, f1, acc);
                     }
                     f0 *= -0.5f; f1 *= -0.5f;
@@ -356,7 +357,7 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_umma_resident(RArgs a) {
             }   // R0 < Pd
             // this tile's part of Wh / X' is written and its accumulator drained: tell the MMA issuer.  (The residual
             // partial of the step goes out with the LAST tile of product 1, T0.)
-            if (!P2 && t == 0) {
+            if (!P2 && t == 0 && RES) {
               float rs = res + 2.f * res2;
               for (int d = 16; d > 0; d >>= 1) rs += __shfl_xor_sync(0xffffffffu, rs, d);
               if (lane == 0) res_s[w] = rs;
@@ -372,15 +373,15 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_umma_resident(RArgs a) {
 
         // ---- epilogue 1: Wh -> WS, residual
         float res = 0.f;
-        pass(false, bf, res);
         bool last = k + 1 == a.max_iter;
+        pass(false, bf, a.tol > 0.0 || last, res);
         ptx::mbar_wait(b_w0, p_w0, a.err_flag, 27); p_w0 ^= 1u;        // all 16 partial sums of the step are there
         if (a.tol > 0.0 || last) r_last = residual_now(s.m);          // fixed counts: only the last residual is reported
         if (a.tol > 0.0 && r_last < a.tol) last = true;
         // ---- epilogue 2: X' -> XS (the update that reaches switch_iter writes fp16)
         const bool bf_next = bf && (k + 1 != a.switch_iter);
         float dummy = 0.f;
-        pass(true, bf_next, dummy);
+        pass(true, bf_next, false, dummy);
         bf = bf_next;
         iters_done = k + 1;
         // the partial sums of this step are consumed by every role before any warp can rewrite its slot: a warp
